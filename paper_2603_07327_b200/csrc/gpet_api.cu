@@ -1,0 +1,379 @@
+// gpet_api.cu -- the C ABI declared in include/gpet.h: argument checks, descriptor quantisation [R7],
+// table staging [R11], activity CDF [R13], and kernel launches.  No physics runs on the host.
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "../../include/gpet.h"
+#include "gpet_internal.h"
+
+using namespace gpet;
+
+// ---------------------------------------------------------------- handles
+struct gpet_geometry {
+  DevGeom host;
+  DevGeom *dev = nullptr;
+};
+struct gpet_materials {
+  int n_materials = 0, n_energies = 0; float e_min = 0, e_step = 0;
+  std::vector<float> mu_tot;            // host [n_materials][n_energies] (fp32 sums as staged)
+  float4 *dev_mu = nullptr;
+  std::mutex lock;
+  float *dev_maj[256] = {};             // lazily built majorant tables per material mask (n <= 8 materials)
+};
+struct gpet_activity {
+  int dims[3]; uint32_t n_active = 0; uint64_t w_total = 0;
+  uint32_t *dev_index = nullptr; uint64_t *dev_cdf = nullptr;
+};
+
+// ---------------------------------------------------------------- errors, bookkeeping
+static thread_local char g_err[512] = "";
+static std::atomic<uint64_t> g_launches{0};
+void gpet::count_launch(uint64_t n) { g_launches += n; }
+
+static int fail(int code, const char *fmt, ...) {
+  va_list ap; va_start(ap, fmt); vsnprintf(g_err, sizeof g_err, fmt, ap); va_end(ap);
+  return code;
+}
+#define CUDA_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) \
+  return fail(GPET_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
+
+extern "C" const char *gpet_last_error(void) { return g_err; }
+extern "C" uint64_t gpet_launch_count(void) { return g_launches.load(); }
+
+static int sm_count() {
+  static int n = 0;
+  if (!n) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev); if (n <= 0) n = 148; }
+  return n;
+}
+
+// ---------------------------------------------------------------- geometry
+static long long quant(float x) { return llrint((double)x * 1048576.0); }   // [R7]
+
+extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry **out) {
+  if (!d || !out || !d->layers) return fail(GPET_E_INVALID_ARG, "gpet_geometry_create: NULL argument");
+  if (d->n_panels < 1 || d->n_panels > GPET_MAX_PANELS) return fail(GPET_E_GEOMETRY, "n_panels %d outside 1..%d", d->n_panels, GPET_MAX_PANELS);
+  if (d->n_layers < 1 || d->n_layers > GPET_MAX_LAYERS) return fail(GPET_E_GEOMETRY, "n_layers %d outside 1..%d", d->n_layers, GPET_MAX_LAYERS);
+  gpet_geometry *g = new gpet_geometry;
+  DevGeom &G = g->host; memset(&G, 0, sizeof G);
+  G.n_panels = d->n_panels; G.n_layers = d->n_layers; G.ring = d->panel_pose ? 0 : 1;
+  long long ms[2], mp[2];
+  for (int a = 0; a < 2; ++a) {
+    ms[a] = quant(d->module_size_mm[a]); mp[a] = quant(d->module_pitch_mm[a]);
+    if (d->n_modules[a] < 1 || d->n_modules[a] > 8 || ms[a] <= 0 || mp[a] < ms[a]) {
+      delete g; return fail(GPET_E_GEOMETRY, "module grid axis %d: n=%d size=%g pitch=%g", a, d->n_modules[a], d->module_size_mm[a], d->module_pitch_mm[a]);
+    }
+    G.nmod[a] = d->n_modules[a]; G.msq[a] = (int)ms[a]; G.mpq[a] = (int)mp[a]; G.inv_mpq[a] = 1.0f / (float)mp[a];
+  }
+  const long long Wq = (G.nmod[0] - 1) * mp[0] + ms[0], Hq = (G.nmod[1] - 1) * mp[1] + ms[1];
+  long long c = 0;
+  for (int l = 0; l < d->n_layers; ++l) {
+    const gpet_layer_desc &s = d->layers[l]; DevLayer &L = G.layer[l];
+    const long long gb = quant(s.gap_before_mm), dp = quant(s.depth_mm);
+    if (gb < 0 || dp <= 0) { delete g; return fail(GPET_E_GEOMETRY, "layer %d: depth %g, gap_before %g", l, s.depth_mm, s.gap_before_mm); }
+    c += gb; L.c0 = (int)c; c += dp; L.c1 = (int)c;
+    L.cmat = s.crystal_material; L.gmat = s.gap_material;
+    if (L.cmat < 0 || L.cmat >= GPET_MAX_MATERIALS || L.gmat < -1 || L.gmat >= GPET_MAX_MATERIALS) {
+      delete g; return fail(GPET_E_GEOMETRY, "layer %d: material index out of range", l);
+    }
+    G.det_mask |= 1u << L.cmat; if (L.gmat >= 0) G.det_mask |= 1u << L.gmat;
+    for (int a = 0; a < 2; ++a) {
+      const long long p = quant(s.pitch_mm[a]), gp = quant(s.reflector_mm[a]), of = quant(s.offset_mm[a]);
+      if (s.n_crystals[a] < 1 || p <= 0 || gp < 0 || gp >= p || of < 0 || of + s.n_crystals[a] * p > ms[a]) {
+        delete g; return fail(GPET_E_GEOMETRY, "layer %d axis %d: lattice (n=%d pitch=%g gap=%g offset=%g) does not fit its %g mm module",
+                              l, a, s.n_crystals[a], s.pitch_mm[a], s.reflector_mm[a], s.offset_mm[a], d->module_size_mm[a]);
+      }
+      L.n[a] = s.n_crystals[a]; L.pitch[a] = (int)p; L.off[a] = (int)of;
+      L.lo[a] = (int)(gp >> 1); L.hi[a] = (int)(p - (gp - (gp >> 1))); L.inv_pitch[a] = 1.0f / (float)p;
+    }
+    if ((long long)s.n_crystals[0] * s.n_crystals[1] > 8192) { delete g; return fail(GPET_E_GEOMETRY, "layer %d: more than 8192 crystals", l); }
+  }
+  if (Wq >= (1ll << 30) || Hq >= (1ll << 30) || c >= (1ll << 30)) { delete g; return fail(GPET_E_GEOMETRY, "panel larger than 1024 mm"); }
+  G.Wq = (int)Wq; G.Hq = (int)Hq; G.Dq = (int)c; G.hWq = (int)(Wq >> 1); G.hHq = (int)(Hq >> 1);
+  G.blo[0] = (float)(-(double)G.hWq / 1048576.0); G.bhi[0] = (float)((double)(Wq - G.hWq) / 1048576.0);
+  G.blo[1] = (float)(-(double)G.hHq / 1048576.0); G.bhi[1] = (float)((double)(Hq - G.hHq) / 1048576.0);
+  G.blo[2] = 0.0f;                                G.bhi[2] = (float)((double)c / 1048576.0);
+  if (d->panel_pose) {
+    memcpy(G.pose, d->panel_pose, sizeof(float) * 12 * (size_t)d->n_panels);
+  } else {                                                          // [R5] repetition mode
+    const double PI = 3.14159265358979323846;
+    for (int p = 0; p < d->n_panels; ++p) {
+      const double phi = ((double)d->ring_first_angle_deg + 360.0 * (double)p / (double)d->n_panels) * (PI / 180.0);
+      double cs = cos(phi), sn = sin(phi);
+      if (fabs(cs) < 1e-12) cs = 0.0;
+      if (fabs(sn) < 1e-12) sn = 0.0;
+      float *q = G.pose[p];
+      q[0] = (float)((double)d->ring_inner_radius_mm * cs); q[1] = (float)((double)d->ring_inner_radius_mm * sn); q[2] = 0.0f;
+      q[3] = (float)(-sn); q[4] = (float)cs; q[5] = 0.0f;
+      q[6] = 0.0f; q[7] = 0.0f; q[8] = 1.0f;
+      q[9] = (float)cs; q[10] = (float)sn; q[11] = 0.0f;
+    }
+  }
+  *out = g;                     // the device copy is made lazily so the handle can be built without a GPU
+  return GPET_OK;
+}
+
+static int geometry_upload(gpet_geometry *g) {
+  if (g->dev) return GPET_OK;
+  CUDA_TRY(cudaMalloc(&g->dev, sizeof(DevGeom)));
+  CUDA_TRY(cudaMemcpy(g->dev, &g->host, sizeof(DevGeom), cudaMemcpyHostToDevice));
+  return GPET_OK;
+}
+
+extern "C" int gpet_geometry_destroy(gpet_geometry *g) {
+  if (!g) return GPET_OK;
+  if (g->dev) cudaFree(g->dev);
+  delete g; return GPET_OK;
+}
+
+extern "C" int gpet_geometry_panel_pose(const gpet_geometry *g, int32_t panel, float *pose12) {
+  if (!g || !pose12 || panel < 0 || panel >= g->host.n_panels) return fail(GPET_E_INVALID_ARG, "gpet_geometry_panel_pose: bad argument");
+  memcpy(pose12, g->host.pose[panel], sizeof(float) * 12); return GPET_OK;
+}
+
+extern "C" int gpet_geometry_locate(const gpet_geometry *g, int64_t n, const float *xyz, uint32_t *ids) {
+  if (!g || n < 0 || (n > 0 && (!xyz || !ids))) return fail(GPET_E_INVALID_ARG, "gpet_geometry_locate: bad argument");
+  if (n == 0) return GPET_OK;
+  int rc = geometry_upload(const_cast<gpet_geometry *>(g)); if (rc) return rc;
+  float *dx = nullptr; uint32_t *di = nullptr;
+  CUDA_TRY(cudaMalloc(&dx, sizeof(float) * 3 * (size_t)n));
+  CUDA_TRY(cudaMalloc(&di, sizeof(uint32_t) * (size_t)n));
+  CUDA_TRY(cudaMemcpy(dx, xyz, sizeof(float) * 3 * (size_t)n, cudaMemcpyHostToDevice));
+  CUDA_TRY(launch_locate(g->dev, n, dx, di, 0));
+  CUDA_TRY(cudaMemcpy(ids, di, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToHost));
+  cudaFree(dx); cudaFree(di);
+  return GPET_OK;
+}
+
+// ---------------------------------------------------------------- materials
+extern "C" int gpet_materials_load(int32_t n_materials, int32_t n_energies, float e_min, float e_step, const float *mu_pe,
+                                   const float *mu_c, const float *mu_r, gpet_materials **out) {
+  if (!mu_pe || !mu_c || !mu_r || !out) return fail(GPET_E_INVALID_ARG, "gpet_materials_load: NULL argument");
+  if (n_materials < 1 || n_materials > GPET_MAX_MATERIALS) return fail(GPET_E_TABLE, "n_materials %d outside 1..%d", n_materials, GPET_MAX_MATERIALS);
+  if (n_energies < 2 || !(e_step > 0.0f)) return fail(GPET_E_TABLE, "need >= 2 energies and a positive step");
+  const size_t n = (size_t)n_materials * n_energies;
+  std::vector<float4> mu(n);
+  gpet_materials *m = new gpet_materials;
+  m->n_materials = n_materials; m->n_energies = n_energies; m->e_min = e_min; m->e_step = e_step; m->mu_tot.resize(n);
+  for (size_t i = 0; i < n; ++i) {
+    if (!(mu_pe[i] >= 0.0f) || !(mu_c[i] >= 0.0f) || !(mu_r[i] >= 0.0f) || !std::isfinite(mu_pe[i] + mu_c[i] + mu_r[i])) {
+      delete m; return fail(GPET_E_TABLE, "negative or non-finite mu at flat index %zu", i);
+    }
+    // cumulative sums formed in double, rounded to fp32 once [R11]
+    mu[i] = make_float4(mu_pe[i], (float)((double)mu_pe[i] + mu_c[i]), (float)((double)mu_pe[i] + mu_c[i] + mu_r[i]), 0.0f);
+    m->mu_tot[i] = mu[i].z;
+  }
+  cudaError_t e = cudaMalloc(&m->dev_mu, sizeof(float4) * n);
+  if (e == cudaSuccess) e = cudaMemcpy(m->dev_mu, mu.data(), sizeof(float4) * n, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { delete m; return fail(GPET_E_CUDA, "gpet_materials_load: %s", cudaGetErrorString(e)); }
+  *out = m; return GPET_OK;
+}
+
+extern "C" int gpet_materials_destroy(gpet_materials *m) {
+  if (!m) return GPET_OK;
+  if (m->dev_mu) cudaFree(m->dev_mu);
+  for (float *p : m->dev_maj) if (p) cudaFree(p);
+  delete m; return GPET_OK;
+}
+
+// [R19] majorant table of a material set: pointwise max of mu_tot over the set
+static int majorant_table(gpet_materials *m, uint32_t mask, const float **out) {
+  mask &= (1u << m->n_materials) - 1u;
+  if (!mask) return fail(GPET_E_INVALID_ARG, "geometry references no loaded material");
+  std::lock_guard<std::mutex> lk(m->lock);
+  if (!m->dev_maj[mask]) {
+    std::vector<float> maj(m->n_energies, 0.0f);
+    for (int k = 0; k < m->n_materials; ++k) if (mask >> k & 1u)
+      for (int i = 0; i < m->n_energies; ++i) maj[i] = fmaxf(maj[i], m->mu_tot[(size_t)k * m->n_energies + i]);
+    CUDA_TRY(cudaMalloc(&m->dev_maj[mask], sizeof(float) * m->n_energies));
+    CUDA_TRY(cudaMemcpy(m->dev_maj[mask], maj.data(), sizeof(float) * m->n_energies, cudaMemcpyHostToDevice));
+  }
+  *out = m->dev_maj[mask]; return GPET_OK;
+}
+
+// ---------------------------------------------------------------- activity map [R13]
+extern "C" int gpet_activity_create(const float *activity, const int32_t dims[3], gpet_activity **out) {
+  if (!activity || !dims || !out) return fail(GPET_E_INVALID_ARG, "gpet_activity_create: NULL argument");
+  if (dims[0] < 1 || dims[1] < 1 || dims[2] < 1 || (long long)dims[0] * dims[1] * dims[2] > (1ll << 31))
+    return fail(GPET_E_INVALID_ARG, "activity grid %d x %d x %d out of range", dims[0], dims[1], dims[2]);
+  const size_t nv = (size_t)dims[0] * dims[1] * dims[2];
+  float amax = 0.0f;
+  for (size_t i = 0; i < nv; ++i) { if (!(activity[i] >= 0.0f)) return fail(GPET_E_INVALID_ARG, "negative activity"); if (activity[i] > amax) amax = activity[i]; }
+  if (!(amax > 0.0f)) return fail(GPET_E_INVALID_ARG, "activity map has no active voxel");
+  std::vector<uint32_t> idx; std::vector<uint64_t> cdf; uint64_t cum = 0;
+  for (size_t i = 0; i < nv; ++i) if (activity[i] > 0.0f) {
+    long long w = llrint((double)activity[i] / (double)amax * 1048576.0); if (w < 1) w = 1;
+    cum += (uint64_t)w; idx.push_back((uint32_t)i); cdf.push_back(cum);
+  }
+  gpet_activity *a = new gpet_activity;
+  a->dims[0] = dims[0]; a->dims[1] = dims[1]; a->dims[2] = dims[2]; a->n_active = (uint32_t)idx.size(); a->w_total = cum;
+  cudaError_t e = cudaMalloc(&a->dev_index, sizeof(uint32_t) * idx.size());
+  if (e == cudaSuccess) e = cudaMalloc(&a->dev_cdf, sizeof(uint64_t) * cdf.size());
+  if (e == cudaSuccess) e = cudaMemcpy(a->dev_index, idx.data(), sizeof(uint32_t) * idx.size(), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(a->dev_cdf, cdf.data(), sizeof(uint64_t) * cdf.size(), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { gpet_activity_destroy(a); return fail(GPET_E_CUDA, "gpet_activity_create: %s", cudaGetErrorString(e)); }
+  *out = a; return GPET_OK;
+}
+
+extern "C" int gpet_activity_destroy(gpet_activity *a) {
+  if (!a) return GPET_OK;
+  if (a->dev_index) cudaFree(a->dev_index);
+  if (a->dev_cdf) cudaFree(a->dev_cdf);
+  delete a; return GPET_OK;
+}
+
+// ---------------------------------------------------------------- source marshalling
+static int make_source(const gpet_source *s, const gpet_materials *m, DevSource *D) {
+  memset(D, 0, sizeof *D);
+  if (s->kind < 0 || s->kind > 2) return fail(GPET_E_INVALID_ARG, "source kind %d", s->kind);
+  D->kind = s->kind;
+  for (int k = 0; k < 3; ++k) { D->pos[k] = s->pos_mm[k]; D->dims[k] = s->dims[k]; D->voxel[k] = s->voxel_mm[k]; D->origin[k] = s->origin_mm[k];
+                                D->inv_voxel[k] = s->voxel_mm[k] > 0.0f ? 1.0f / s->voxel_mm[k] : 0.0f; }
+  if (s->kind == 2) {
+    const double nb = sqrt((double)s->beam_dir[0] * s->beam_dir[0] + (double)s->beam_dir[1] * s->beam_dir[1] + (double)s->beam_dir[2] * s->beam_dir[2]);
+    if (!(nb > 0.0)) return fail(GPET_E_INVALID_ARG, "beam_dir is zero");
+    for (int k = 0; k < 3; ++k) D->beam[k] = (float)((double)s->beam_dir[k] / nb);
+  }
+  if (!(s->acolinearity_fwhm_deg >= 0.0f)) return fail(GPET_E_INVALID_ARG, "negative acolinearity");
+  D->acol_sigma = (float)((double)s->acolinearity_fwhm_deg * (3.14159265358979323846 / 180.0) / 2.354820045030949);
+  if (!(s->activity_bq > 0.0)) return fail(GPET_E_INVALID_ARG, "activity_bq must be positive");
+  D->activity_bq = s->activity_bq; D->pairs_per_slice = s->pairs_per_time_slice;
+  if (s->kind == 1) {
+    if (!s->activity_map) return fail(GPET_E_INVALID_ARG, "kind 1 needs an activity_map");
+    for (int k = 0; k < 3; ++k) if (s->dims[k] != s->activity_map->dims[k] || !(s->voxel_mm[k] > 0.0f))
+      return fail(GPET_E_INVALID_ARG, "source grid does not match its activity map");
+    D->act_index = s->activity_map->dev_index; D->act_cdf = s->activity_map->dev_cdf;
+    D->n_active = s->activity_map->n_active; D->w_total = s->activity_map->w_total;
+    D->phantom = s->phantom_material; D->ph_major = s->phantom_majorant_material;
+    if (D->phantom && m && (D->ph_major < 0 || D->ph_major >= m->n_materials)) return fail(GPET_E_INVALID_ARG, "phantom_majorant_material out of range");
+  }
+  return GPET_OK;
+}
+
+static HitBuf hitbuf(const gpet_hits *h) {
+  HitBuf H = { h->history, h->ids, h->x, h->y, h->z, h->e_keV, h->tof_ns, h->capacity, reinterpret_cast<unsigned long long *>(h->n_hits) };
+  return H;
+}
+
+// ---------------------------------------------------------------- transport
+extern "C" int gpet_simulate(const gpet_geometry *g, const gpet_materials *m, const gpet_source *src, uint64_t first_history,
+                             uint64_t n_pairs, uint64_t seed, gpet_hits *hits, void *stream) {
+  if (!g || !m || !src || !hits) return fail(GPET_E_INVALID_ARG, "gpet_simulate: NULL argument");
+  if (!hits->n_hits || (hits->capacity && (!hits->history || !hits->ids || !hits->x || !hits->y || !hits->z || !hits->e_keV || !hits->tof_ns)))
+    return fail(GPET_E_INVALID_ARG, "gpet_simulate: hit buffer has NULL arrays");
+  if (n_pairs >= (1ull << 32)) return fail(GPET_E_INVALID_ARG, "n_pairs >= 2^32");
+  if (n_pairs == 0) return GPET_OK;
+  for (int l = 0; l < g->host.n_layers; ++l)
+    if (g->host.layer[l].cmat >= m->n_materials || g->host.layer[l].gmat >= m->n_materials)
+      return fail(GPET_E_INVALID_ARG, "layer %d references a material that is not loaded", l);
+  DevSource D; int rc = make_source(src, m, &D); if (rc) return rc;
+  rc = geometry_upload(const_cast<gpet_geometry *>(g)); if (rc) return rc;
+  const float *maj = nullptr; rc = majorant_table(const_cast<gpet_materials *>(m), g->host.det_mask, &maj); if (rc) return rc;
+  DevTables T = { m->n_materials, m->n_energies, m->e_min, 1.0f / m->e_step, m->dev_mu };
+  CUDA_TRY(launch_transport(g->dev, T, maj, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, sm_count(), (cudaStream_t)stream));
+  return GPET_OK;
+}
+
+// ---------------------------------------------------------------- digitizer
+extern "C" size_t gpet_digitize_scratch_bytes(uint64_t n_pairs, uint64_t n_hits) { return digitize_scratch_bytes(n_pairs, n_hits); }
+
+static int make_digi(const gpet_source *src, uint64_t seed, uint64_t n_pairs_total, const gpet_digitizer *d, DigiParams *P) {
+  if (d->readout_level < 0 || d->readout_level > 2) return fail(GPET_E_INVALID_ARG, "readout_level %d", d->readout_level);
+  if (!(d->blur_fwhm_frac >= 0.0f) || !(d->window_ns > 0.0) || !(src->activity_bq > 0.0)) return fail(GPET_E_INVALID_ARG, "bad digitizer parameters");
+  P->sigma_scale = (float)((double)d->blur_fwhm_frac / 2.354820045030949); P->ref_keV = d->blur_ref_keV;
+  P->e_lo = d->e_lo_keV; P->e_hi = d->e_hi_keV; P->window_s = d->window_ns * 1e-9;
+  P->shift = d->readout_level == 0 ? 5 : (d->readout_level == 1 ? 20 : 26);
+  P->activity_bq = src->activity_bq; P->pairs_per_slice = src->pairs_per_time_slice ? src->pairs_per_time_slice : n_pairs_total;
+  P->seed = seed;
+  return GPET_OK;
+}
+
+extern "C" int gpet_digitize(const gpet_source *src, uint64_t seed, uint64_t n_pairs_total, uint64_t first_history, uint64_t n_pairs,
+                             const gpet_hits *hits, uint64_t n_hits, const gpet_digitizer *dig, void *scratch, size_t scratch_bytes,
+                             gpet_singles *so, gpet_coincidences *co, void *stream) {
+  if (!src || !hits || !dig || !co || !co->n_coinc) return fail(GPET_E_INVALID_ARG, "gpet_digitize: NULL argument");
+  if (n_pairs == 0 || n_pairs >= (1ull << 32) || n_hits > hits->capacity || n_hits >= (1ull << 32)) return fail(GPET_E_INVALID_ARG, "gpet_digitize: counts out of range");
+  if (scratch_bytes < digitize_scratch_bytes(n_pairs, n_hits) || !scratch) return fail(GPET_E_OVERFLOW, "scratch too small: %zu < %zu", scratch_bytes, digitize_scratch_bytes(n_pairs, n_hits));
+  DigiParams P; int rc = make_digi(src, seed, n_pairs_total, dig, &P); if (rc) return rc;
+  SinglesBuf S; memset(&S, 0, sizeof S);
+  if (so) { SinglesBuf s = { so->history, so->ids, so->x, so->y, so->z, so->e_keV, so->t_s, so->capacity, reinterpret_cast<unsigned long long *>(so->n_singles) }; S = s; }
+  CoincBuf Cb = { co->ids_a, co->ids_b, co->history_a, co->history_b, co->e_a, co->e_b, co->dt_ns, co->t_s, co->capacity,
+                  reinterpret_cast<unsigned long long *>(co->n_coinc) };
+  CUDA_TRY(launch_digitize(P, hitbuf(hits), first_history, n_pairs, n_hits, scratch, scratch_bytes, S, Cb, (cudaStream_t)stream));
+  return GPET_OK;
+}
+
+// ---------------------------------------------------------------- whole path with host outputs
+namespace {
+struct DevArena {                      // bump allocator over one cudaMalloc
+  char *base = nullptr; size_t size = 0, used = 0;
+  template <class T> T *take(size_t n) { used = (used + 255) & ~(size_t)255; T *p = reinterpret_cast<T *>(base + used); used += sizeof(T) * n; return p; }
+};
+}
+
+extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, const gpet_source *src, uint64_t n_pairs_total,
+                             uint64_t first_history, uint64_t n_pairs, uint64_t seed, const gpet_digitizer *dig, double hits_per_pair,
+                             gpet_host_outputs *out) {
+  if (!g || !m || !src || !dig || !out) return fail(GPET_E_INVALID_ARG, "gpet_run_host: NULL argument");
+  if (n_pairs == 0 || n_pairs >= (1ull << 32) || !(hits_per_pair > 0.0)) return fail(GPET_E_INVALID_ARG, "gpet_run_host: bad counts");
+  const uint64_t cap = (uint64_t)((double)n_pairs * hits_per_pair) + 1024;
+  if (cap >= (1ull << 32)) return fail(GPET_E_INVALID_ARG, "gpet_run_host: batch too large, split it");
+  const size_t scratch_bytes = digitize_scratch_bytes(n_pairs, cap);
+  const size_t nvox = src->kind == 1 && src->phantom_material ? (size_t)src->dims[0] * src->dims[1] * src->dims[2] : 0;
+  DevArena A; A.size = cap * (28 + 36 + 40) + scratch_bytes + nvox + (out->hits.outcome_hash ? 8 * n_pairs : 0) + 64 * 256;
+  CUDA_TRY(cudaMalloc(&A.base, A.size));
+  int rc = GPET_OK;
+  cudaStream_t st = 0;
+  do {
+    gpet_hits H; memset(&H, 0, sizeof H);
+    H.history = A.take<uint32_t>(cap); H.ids = A.take<uint32_t>(cap); H.x = A.take<float>(cap); H.y = A.take<float>(cap); H.z = A.take<float>(cap);
+    H.e_keV = A.take<float>(cap); H.tof_ns = A.take<float>(cap); H.capacity = cap; H.n_hits = A.take<uint64_t>(1);
+    H.outcome_hash = out->hits.outcome_hash ? A.take<uint64_t>(n_pairs) : nullptr;
+    gpet_singles S; S.history = A.take<uint32_t>(cap); S.ids = A.take<uint32_t>(cap); S.x = A.take<float>(cap); S.y = A.take<float>(cap);
+    S.z = A.take<float>(cap); S.e_keV = A.take<float>(cap); S.t_s = A.take<double>(cap); S.capacity = cap; S.n_singles = A.take<uint64_t>(1);
+    gpet_coincidences Cc; Cc.ids_a = A.take<uint32_t>(cap); Cc.ids_b = A.take<uint32_t>(cap); Cc.history_a = A.take<uint32_t>(cap);
+    Cc.history_b = A.take<uint32_t>(cap); Cc.e_a = A.take<float>(cap); Cc.e_b = A.take<float>(cap); Cc.dt_ns = A.take<float>(cap);
+    Cc.t_s = A.take<double>(cap); Cc.capacity = cap; Cc.n_coinc = A.take<uint64_t>(1);
+    void *scratch = A.take<char>(scratch_bytes);
+    gpet_source s2 = *src;
+    if (nvox) {
+      uint8_t *ph = A.take<uint8_t>(nvox);
+      if (cudaMemcpyAsync(ph, src->phantom_material, nvox, cudaMemcpyHostToDevice, st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "phantom upload failed"); break; }
+      s2.phantom_material = ph;
+    }
+    if (A.used > A.size) { rc = fail(GPET_E_OVERFLOW, "internal arena too small"); break; }
+    if (cudaMemsetAsync(H.n_hits, 0, 8, st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "memset failed"); break; }
+    if ((rc = gpet_simulate(g, m, &s2, first_history, n_pairs, seed, &H, st))) break;
+    uint64_t nh = 0;
+    if (cudaMemcpyAsync(&nh, H.n_hits, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) {
+      rc = fail(GPET_E_CUDA, "transport failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
+    if (nh > cap) { rc = fail(GPET_E_OVERFLOW, "hit buffer overflow: %llu hits > capacity %llu; raise hits_per_pair", (unsigned long long)nh, (unsigned long long)cap); break; }
+    if ((rc = gpet_digitize(&s2, seed, n_pairs_total, first_history, n_pairs, &H, nh, dig, scratch, scratch_bytes, &S, &Cc, st))) break;
+    uint64_t ns = 0, nc = 0;
+    cudaMemcpyAsync(&ns, S.n_singles, 8, cudaMemcpyDeviceToHost, st); cudaMemcpyAsync(&nc, Cc.n_coinc, 8, cudaMemcpyDeviceToHost, st);
+    if (cudaStreamSynchronize(st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "digitizer failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
+#define D2H(dst, srcp, n, T) do { if ((dst) && (n)) cudaMemcpyAsync((dst), (srcp), sizeof(T) * (n), cudaMemcpyDeviceToHost, st); } while (0)
+    const uint64_t ch = nh < out->hits.capacity ? nh : out->hits.capacity;
+    D2H(out->hits.history, H.history, ch, uint32_t); D2H(out->hits.ids, H.ids, ch, uint32_t); D2H(out->hits.x, H.x, ch, float);
+    D2H(out->hits.y, H.y, ch, float); D2H(out->hits.z, H.z, ch, float); D2H(out->hits.e_keV, H.e_keV, ch, float); D2H(out->hits.tof_ns, H.tof_ns, ch, float);
+    D2H(out->hits.outcome_hash, H.outcome_hash, n_pairs, uint64_t);
+    const uint64_t cs = ns < out->singles.capacity ? ns : out->singles.capacity;
+    D2H(out->singles.history, S.history, cs, uint32_t); D2H(out->singles.ids, S.ids, cs, uint32_t); D2H(out->singles.x, S.x, cs, float);
+    D2H(out->singles.y, S.y, cs, float); D2H(out->singles.z, S.z, cs, float); D2H(out->singles.e_keV, S.e_keV, cs, float); D2H(out->singles.t_s, S.t_s, cs, double);
+    const uint64_t cc = nc < out->coinc.capacity ? nc : out->coinc.capacity;
+    D2H(out->coinc.ids_a, Cc.ids_a, cc, uint32_t); D2H(out->coinc.ids_b, Cc.ids_b, cc, uint32_t); D2H(out->coinc.history_a, Cc.history_a, cc, uint32_t);
+    D2H(out->coinc.history_b, Cc.history_b, cc, uint32_t); D2H(out->coinc.e_a, Cc.e_a, cc, float); D2H(out->coinc.e_b, Cc.e_b, cc, float);
+    D2H(out->coinc.dt_ns, Cc.dt_ns, cc, float); D2H(out->coinc.t_s, Cc.t_s, cc, double);
+#undef D2H
+    if (cudaStreamSynchronize(st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "copy back failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
+    if (out->hits.n_hits) *out->hits.n_hits = nh;
+    if (out->singles.n_singles) *out->singles.n_singles = ns;
+    if (out->coinc.n_coinc) *out->coinc.n_coinc = nc;
+  } while (0);
+  cudaFree(A.base);
+  return rc;
+}

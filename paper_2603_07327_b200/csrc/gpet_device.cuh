@@ -1,0 +1,163 @@
+// gpet_device.cuh -- device-side building blocks shared by the transport, locate and digitizer kernels.
+// sm_100a only.  "[Rn]" = reading n in DESIGN.md section 2; PAPER.md:<line> = the paper.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gpet {
+
+constexpr int   kMaxPanels = 64;          // 63 usable (packed id 0xFFFFFFFF is reserved)
+constexpr int   kMaxLayers = 4;
+constexpr int   kMaxMaterials = 8;
+constexpr float kQ = 1048576.0f;          // [R7] 2^20 quantisation units per mm
+constexpr float kMec2 = 510.99895f;       // [R12]
+constexpr float kInvC = 1.0f / 299.792458f;   // ns per mm
+constexpr float kCutoff = 10.0f;          // [R12]
+constexpr uint32_t kNone = 0xFFFFFFFFu;
+
+// ---------------------------------------------------------------- descriptor as the kernels see it
+struct DevLayer {
+  int c0, c1;                 // depth range [c0, c1) in Q units
+  int n[2], pitch[2], lo[2], hi[2], off[2];   // crystal occupies frac in [lo, hi) of each pitch cell
+  float inv_pitch[2];
+  int cmat, gmat;
+};
+struct DevGeom {
+  int n_panels, n_layers;
+  int Wq, Hq, Dq, hWq, hHq;
+  int nmod[2], msq[2], mpq[2];
+  float inv_mpq[2];
+  float blo[3], bhi[3];       // panel box in the tracking frame (fp32 roundings of the Q extents)
+  uint32_t det_mask;          // materials referenced by the layers
+  int ring;                   // 1 = repetition mode (sector shortcut is legal)
+  DevLayer layer[kMaxLayers];
+  float pose[kMaxPanels][12]; // front-face centre, u, v, w
+};
+
+struct DevTables {            // [R11] per material, per energy: {mu_pe, mu_pe+mu_C, mu_tot, unused}
+  int n_materials, n_energies;
+  float e_min, inv_step;
+  const float4 *mu;           // [n_materials][n_energies]
+};
+
+// ---------------------------------------------------------------- [R1] Philox4x32-10
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+    c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
+    k.x += 0x9E3779B9u; k.y += 0xBB67AE85u;
+  }
+  return c;
+}
+// [R2] u = ((x >> 9) + 0.5) * 2^-23: every step is exact in fp32
+__device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 9) + 0.5f) * 1.1920928955078125e-7f; }
+
+// Sequential per-photon stream [R4]: draw j = word j&3 of block j>>2
+struct Stream {
+  uint2 key; uint32_t h_lo, h_hi, stream, ndraw; uint4 blk;
+  __device__ __forceinline__ void init(uint64_t seed, uint64_t history, uint32_t s) {
+    key = make_uint2((uint32_t)seed, (uint32_t)(seed >> 32));
+    h_lo = (uint32_t)history; h_hi = (uint32_t)(history >> 32); stream = s; ndraw = 0;
+  }
+  __device__ __forceinline__ float next() {
+    const uint32_t j = ndraw & 3u;
+    if (j == 0) blk = philox4x32_10(make_uint4(h_lo, h_hi, stream, ndraw >> 2), key);
+    ++ndraw;
+    const uint32_t w = j == 0 ? blk.x : (j == 1 ? blk.y : (j == 2 ? blk.z : blk.w));
+    return u01(w);
+  }
+};
+
+// ---------------------------------------------------------------- [R7] lattice lookup
+// exact floor division of a Q coordinate by a Q pitch: float reciprocal estimate + integer fix-up
+__device__ __forceinline__ int floor_div_q(int rel, int pitch, float inv_pitch, int &rem) {
+  int i = __float2int_rd((float)rel * inv_pitch);
+  int r = rel - i * pitch;
+  if (r < 0) { --i; r += pitch; }
+  if (r >= pitch) { ++i; r -= pitch; }
+  rem = r; return i;
+}
+
+// (qa, qb, qc) measured from the panel's low corner.  Returns the material (-1 vacuum) and the packed
+// ids without panel/photon/seq bits (kNone when the point is in no crystal).  PAPER.md:43: the depth
+// coordinate picks the layer, that layer's crystal parameters give material and index.
+__device__ __forceinline__ int lattice_lookup(const DevGeom &g, int qa, int qb, int qc, uint32_t &ids) {
+  ids = kNone;
+  if ((unsigned)qa >= (unsigned)g.Wq || (unsigned)qb >= (unsigned)g.Hq || (unsigned)qc >= (unsigned)g.Dq) return -1;
+  int ra, rb;
+  const int mx = floor_div_q(qa, g.mpq[0], g.inv_mpq[0], ra);
+  const int my = floor_div_q(qb, g.mpq[1], g.inv_mpq[1], rb);
+  if (ra >= g.msq[0] || rb >= g.msq[1]) return -1;                   // inter-module gap: vacuum
+  int l = -1;
+#pragma unroll
+  for (int k = 0; k < kMaxLayers; ++k)
+    if (k < g.n_layers && qc >= g.layer[k].c0 && qc < g.layer[k].c1) l = k;
+  if (l < 0) return -1;                                              // inter-layer gap: vacuum
+  const DevLayer &L = g.layer[l];
+  int fa, fb;
+  const int ix = floor_div_q(ra - L.off[0], L.pitch[0], L.inv_pitch[0], fa);
+  const int iy = floor_div_q(rb - L.off[1], L.pitch[1], L.inv_pitch[1], fb);
+  const bool in = (unsigned)ix < (unsigned)L.n[0] && (unsigned)iy < (unsigned)L.n[1] &&
+                  fa >= L.lo[0] && fa < L.hi[0] && fb >= L.lo[1] && fb < L.hi[1];
+  if (!in) return L.gmat;
+  ids = ((uint32_t)(mx + g.nmod[0] * my) << 20) | ((uint32_t)l << 18) | ((uint32_t)(ix + L.n[0] * iy) << 5);
+  return L.cmat;
+}
+
+// ---------------------------------------------------------------- [R6] slab test
+// Ray x + t d against the box [lo, hi]; returns false if an axis with zero direction lies outside.
+__device__ __forceinline__ bool slab(const float lo[3], const float hi[3], const float x[3], const float d[3],
+                                     float &tn, float &tf) {
+  tn = -INFINITY; tf = INFINITY;
+  bool ok = true;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    if (d[k] == 0.0f) { ok = ok && !(x[k] < lo[k] || x[k] >= hi[k]); continue; }
+    const float inv = 1.0f / d[k];
+    const float t1 = (lo[k] - x[k]) * inv, t2 = (hi[k] - x[k]) * inv;
+    tn = fmaxf(tn, fminf(t1, t2)); tf = fminf(tf, fmaxf(t1, t2));
+  }
+  return ok;
+}
+
+// PAPER.md:33 global -> local
+__device__ __forceinline__ void to_local(const float *P, const float x[3], const float d[3], float xl[3], float dl[3]) {
+  const float r0 = x[0] - P[0], r1 = x[1] - P[1], r2 = x[2] - P[2];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    xl[k] = r0 * P[3 + 3 * k] + r1 * P[4 + 3 * k] + r2 * P[5 + 3 * k];
+    dl[k] = d[0] * P[3 + 3 * k] + d[1] * P[4 + 3 * k] + d[2] * P[5 + 3 * k];
+  }
+}
+__device__ __forceinline__ void point_to_global(const float *P, const float xl[3], float x[3]) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k) x[k] = P[k] + xl[0] * P[3 + k] + xl[1] * P[6 + k] + xl[2] * P[9 + k];
+}
+__device__ __forceinline__ void dir_to_global(const float *P, const float dl[3], float d[3]) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k) d[k] = dl[0] * P[3 + k] + dl[1] * P[6 + k] + dl[2] * P[9 + k];
+}
+
+// ---------------------------------------------------------------- [R21] rotation
+__device__ __forceinline__ void rotate(float d[3], float ct, float st, float cp, float sp) {
+  const float sg = copysignf(1.0f, d[2]), a = -1.0f / (sg + d[2]), b = d[0] * d[1] * a;
+  const float b1x = 1.0f + sg * d[0] * d[0] * a, b1y = sg * b, b1z = -sg * d[0];
+  const float b2x = b, b2y = sg + d[1] * d[1] * a, b2z = -d[1];
+  const float nx = ct * d[0] + st * (cp * b1x + sp * b2x);
+  const float ny = ct * d[1] + st * (cp * b1y + sp * b2y);
+  const float nz = ct * d[2] + st * (cp * b1z + sp * b2z);
+  const float s = rsqrtf(nx * nx + ny * ny + nz * nz);
+  d[0] = nx * s; d[1] = ny * s; d[2] = nz * s;
+}
+
+// ---------------------------------------------------------------- [R23] outcome hash
+enum : uint32_t { EV_ENTER = 1, EV_STEP_VACUUM, EV_VIRTUAL, EV_PE, EV_COMPTON, EV_RAYLEIGH, EV_CUTOFF, EV_EXIT, EV_ESCAPE,
+                  EV_PH_COMPTON, EV_PH_RAYLEIGH, EV_PH_ABSORBED, EV_PH_CUTOFF, EV_PH_LEAVE, EV_PHOTON_B };
+__device__ __forceinline__ void hash_ev(uint64_t &h, uint32_t type, uint32_t payload) {
+  h = (h ^ (uint64_t)type) * 0x100000001B3ull;
+  h = (h ^ (uint64_t)payload) * 0x100000001B3ull;
+}
+
+}  // namespace gpet

@@ -1,0 +1,44 @@
+// gpet_internal.h -- declarations shared by the library's translation units (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "gpet_device.cuh"
+
+namespace gpet {
+
+struct HitBuf {            // device view of gpet_hits
+  uint32_t *history, *ids; float *x, *y, *z, *e, *tof;
+  unsigned long long capacity; unsigned long long *n_hits;
+};
+
+struct DevSource {
+  int kind; float pos[3], beam[3]; float acol_sigma;            // radians
+  const uint32_t *act_index; const uint64_t *act_cdf; uint32_t n_active; uint64_t w_total;
+  const uint8_t *phantom; int ph_major; int dims[3]; float voxel[3], inv_voxel[3], origin[3];
+  double activity_bq; uint64_t pairs_per_slice;
+};
+
+struct DigiParams {
+  float sigma_scale;       // R / 2.3548
+  float ref_keV, e_lo, e_hi; double window_s; int shift;         // ids >> shift = readout unit
+  double activity_bq; uint64_t pairs_per_slice; uint64_t seed;
+};
+
+struct SinglesBuf { uint32_t *history, *ids; float *x, *y, *z, *e; double *t; unsigned long long capacity; unsigned long long *n; };
+struct CoincBuf { uint32_t *ids_a, *ids_b, *history_a, *history_b; float *e_a, *e_b, *dt_ns; double *t;
+                  unsigned long long capacity; unsigned long long *n; };
+
+void count_launch(uint64_t n = 1);
+
+size_t transport_smem_bytes(const DevTables &T);
+cudaError_t launch_transport(const DevGeom *geom, const DevTables &T, const float *maj, const DevSource &src,
+                             uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
+                             int sm_count, cudaStream_t stream);
+cudaError_t launch_locate(const DevGeom *geom, int64_t n, const float *xyz_dev, uint32_t *ids_dev, cudaStream_t stream);
+
+size_t digitize_scratch_bytes(uint64_t n_pairs, uint64_t n_hits);
+cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first_history, uint64_t n_pairs, uint64_t n_hits,
+                            void *scratch, size_t scratch_bytes, const SinglesBuf &S, const CoincBuf &C, cudaStream_t stream);
+
+}  // namespace gpet

@@ -359,7 +359,7 @@ double orc_rayleigh_cos(double u) { double a = 4.0 * u - 2.0, q = sqrt(a * a + 1
 
 /* ------------------------------------------------------------------ hash [R23] */
 enum { EV_ENTER = 1, EV_STEP_VACUUM, EV_VIRTUAL, EV_PE, EV_COMPTON, EV_RAYLEIGH, EV_CUTOFF, EV_EXIT, EV_ESCAPE,
-       EV_PH_COMPTON, EV_PH_RAYLEIGH, EV_PH_ABSORBED, EV_PH_CUTOFF, EV_PH_LEAVE, EV_PHOTON_B };
+       EV_PH_COMPTON, EV_PH_RAYLEIGH, EV_PH_ABSORBED, EV_PH_CUTOFF, EV_PH_LEAVE };
 static void hash_ev(uint64_t *h, uint32_t type, uint32_t payload) {
   *h = (*h ^ (uint64_t)type) * 0x100000001B3ull;        /* FNV-1a over 32-bit words */
   *h = (*h ^ (uint64_t)payload) * 0x100000001B3ull;
@@ -545,9 +545,12 @@ static void simulate_history(ctx_t *c, uint64_t seed, uint64_t history) {
   int in_ph = (S->kind == 1 && S->phantom != NULL);
   double xa[3] = { x0[0], x0[1], x0[2] }, xb[3] = { x0[0], x0[1], x0[2] };
   c->C->pairs++;
+  uint64_t *hh = c->hash;                                            /* [R23] one hash per photon */
+  if (hh) { hh[0] = hh[1] = 0xCBF29CE484222325ull; }
   transport_photon(c, seed, history, 0, xa, dA, in_ph);
-  if (c->hash) hash_ev(c->hash, EV_PHOTON_B, 0);
+  if (hh) c->hash = hh + 1;
   transport_photon(c, seed, history, 1, xb, dB, in_ph);
+  c->hash = hh;
 }
 
 static uint32_t detector_mask(const geom_t *g) {
@@ -556,8 +559,8 @@ static uint32_t detector_mask(const geom_t *g) {
   return m;
 }
 
-/* Simulate histories [first, first + n).  hash_out (n, optional) and e_escape (2n, optional) are
- * per history.  Hits come out in canonical (history, photon, sequence) order. */
+/* Simulate histories [first, first + n).  hash_out (2n, optional: photon A, photon B) and e_escape (2n,
+ * optional) are per photon.  Hits come out in canonical (history, photon, sequence) order. */
 int orc_simulate(const orc_geometry *gd, const orc_materials *M, orc_source *S, uint64_t first, uint64_t n,
                  uint64_t seed, orc_hits *hits, uint64_t *hash_out, double *e_escape, orc_counters *counters) {
   geom_t g; int rc = geom_build(gd, &g); if (rc) { geom_free(&g); return rc; }
@@ -565,10 +568,8 @@ int orc_simulate(const orc_geometry *gd, const orc_materials *M, orc_source *S, 
   ctx_t c = { &g, M, S, detector_mask(&g), hits, &C, NULL, NULL };
   hits->n = 0;
   for (uint64_t i = 0; i < n; ++i) {
-    uint64_t h = 0xCBF29CE484222325ull;
-    c.hash = hash_out ? &h : NULL; c.e_escape = e_escape ? e_escape + 2 * i : NULL;
+    c.hash = hash_out ? hash_out + 2 * i : NULL; c.e_escape = e_escape ? e_escape + 2 * i : NULL;
     simulate_history(&c, seed, first + i);
-    if (hash_out) hash_out[i] = h;
   }
   if (counters) *counters = C;
   geom_free(&g); return 0;

@@ -215,7 +215,7 @@ def _simulate_range(g, m, s, first, n, seed, want_hash, want_escape, hits_per_pa
     while True:
         hits = Hits.empty(cap)
         hs = hits._struct()
-        hh = np.zeros(n, np.uint64) if want_hash else None
+        hh = np.zeros((n, 2), np.uint64) if want_hash else None
         ee = np.zeros((n, 2), np.float64) if want_escape else None
         cnt = _Counters()
         rc = lib().orc_simulate(C.byref(g.struct), C.byref(m.struct), C.byref(s.struct), first, n, seed, C.byref(hs),

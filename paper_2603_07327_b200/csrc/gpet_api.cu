@@ -324,8 +324,17 @@ extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, co
   if (cap >= (1ull << 32)) return fail(GPET_E_INVALID_ARG, "gpet_run_host: batch too large, split it");
   const size_t scratch_bytes = digitize_scratch_bytes(n_pairs, cap);
   const size_t nvox = src->kind == 1 && src->phantom_material ? (size_t)src->dims[0] * src->dims[1] * src->dims[2] : 0;
+  // one cached device arena per process: repeated batches of the same size do not re-allocate
+  static std::mutex arena_lock; static char *arena_base = nullptr; static size_t arena_size = 0;
+  std::lock_guard<std::mutex> arena_guard(arena_lock);
   DevArena A; A.size = cap * (28 + 36 + 40) + scratch_bytes + nvox + (out->hits.outcome_hash ? 8 * n_pairs : 0) + 64 * 256;
-  CUDA_TRY(cudaMalloc(&A.base, A.size));
+  if (A.size > arena_size) {
+    if (arena_base) cudaFree(arena_base);
+    arena_base = nullptr; arena_size = 0;
+    CUDA_TRY(cudaMalloc(&arena_base, A.size));
+    arena_size = A.size;
+  }
+  A.base = arena_base;
   int rc = GPET_OK;
   cudaStream_t st = 0;
   do {
@@ -348,14 +357,12 @@ extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, co
     if (A.used > A.size) { rc = fail(GPET_E_OVERFLOW, "internal arena too small"); break; }
     if (cudaMemsetAsync(H.n_hits, 0, 8, st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "memset failed"); break; }
     if ((rc = gpet_simulate(g, m, &s2, first_history, n_pairs, seed, &H, st))) break;
-    uint64_t nh = 0;
-    if (cudaMemcpyAsync(&nh, H.n_hits, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) {
-      rc = fail(GPET_E_CUDA, "transport failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
-    if (nh > cap) { rc = fail(GPET_E_OVERFLOW, "hit buffer overflow: %llu hits > capacity %llu; raise hits_per_pair", (unsigned long long)nh, (unsigned long long)cap); break; }
-    if ((rc = gpet_digitize(&s2, seed, n_pairs_total, first_history, n_pairs, &H, nh, dig, scratch, scratch_bytes, &S, &Cc, st))) break;
-    uint64_t ns = 0, nc = 0;
+    if ((rc = gpet_digitize(&s2, seed, n_pairs_total, first_history, n_pairs, &H, cap, dig, scratch, scratch_bytes, &S, &Cc, st))) break;
+    uint64_t nh = 0, ns = 0, nc = 0;
+    cudaMemcpyAsync(&nh, H.n_hits, 8, cudaMemcpyDeviceToHost, st);
     cudaMemcpyAsync(&ns, S.n_singles, 8, cudaMemcpyDeviceToHost, st); cudaMemcpyAsync(&nc, Cc.n_coinc, 8, cudaMemcpyDeviceToHost, st);
-    if (cudaStreamSynchronize(st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "digitizer failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
+    if (cudaStreamSynchronize(st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "transport/digitizer failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
+    if (nh > cap) { rc = fail(GPET_E_OVERFLOW, "hit buffer overflow: %llu hits > capacity %llu; raise hits_per_pair", (unsigned long long)nh, (unsigned long long)cap); break; }
 #define D2H(dst, srcp, n, T) do { if ((dst) && (n)) cudaMemcpyAsync((dst), (srcp), sizeof(T) * (n), cudaMemcpyDeviceToHost, st); } while (0)
     const uint64_t ch = nh < out->hits.capacity ? nh : out->hits.capacity;
     D2H(out->hits.history, H.history, ch, uint32_t); D2H(out->hits.ids, H.ids, ch, uint32_t); D2H(out->hits.x, H.x, ch, float);
@@ -374,6 +381,5 @@ extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, co
     if (out->singles.n_singles) *out->singles.n_singles = ns;
     if (out->coinc.n_coinc) *out->coinc.n_coinc = nc;
   } while (0);
-  cudaFree(A.base);
   return rc;
 }

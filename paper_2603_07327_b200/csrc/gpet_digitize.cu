@@ -77,14 +77,20 @@ static cudaError_t exclusive_scan(const uint32_t *in, uint64_t n, uint32_t *out,
 }
 
 // ---------------------------------------------------------------- stage 1: counting sort by history
-__global__ void __launch_bounds__(256) count_hits_kernel(const uint32_t *history, uint32_t n_hits, uint32_t first_lo, uint32_t n_pairs, uint32_t *cnt) {
+__device__ __forceinline__ uint32_t valid_hits(const HitBuf &H, uint32_t bound) {
+  const unsigned long long n = *H.n_hits, c = H.capacity < bound ? H.capacity : bound;
+  return (uint32_t)(n < c ? n : c);
+}
+__global__ void __launch_bounds__(256) count_hits_kernel(HitBuf H, uint32_t bound, uint32_t first_lo, uint32_t n_pairs, uint32_t *cnt) {
+  const uint32_t n_hits = valid_hits(H, bound); const uint32_t *history = H.history;
   for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n_hits; i += gridDim.x * 256u) {
     const uint32_t h = history[i] - first_lo;
     if (h < n_pairs) atomicAdd(&cnt[h], 1u);
   }
 }
-__global__ void __launch_bounds__(256) scatter_hits_kernel(const uint32_t *history, uint32_t n_hits, uint32_t first_lo, uint32_t n_pairs,
+__global__ void __launch_bounds__(256) scatter_hits_kernel(HitBuf H, uint32_t bound, uint32_t first_lo, uint32_t n_pairs,
                                                            const uint32_t *off, uint32_t *cnt, uint32_t *idx) {
+  const uint32_t n_hits = valid_hits(H, bound); const uint32_t *history = H.history;
   for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n_hits; i += gridDim.x * 256u) {
     const uint32_t h = history[i] - first_lo;
     if (h < n_pairs) idx[off[h] + atomicSub(&cnt[h], 1u) - 1u] = i;
@@ -255,9 +261,9 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   if ((e = cudaMemsetAsync(T.ids, 0xFF, 4 * M, st)) != cudaSuccess) return e;
   const uint32_t nh = (uint32_t)n_hits, np = (uint32_t)(N == (1ull << 32) ? 0xFFFFFFFFu : N), first_lo = (uint32_t)first_history;
   // 1. counting sort by history
-  if (nh) { count_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H.history, nh, first_lo, np, cnt); count_launch(); }
+  if (nh) { count_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, cnt); count_launch(); }
   if ((e = exclusive_scan(cnt, N, off, bsum, nullptr, st)) != cudaSuccess) return e;
-  if (nh) { scatter_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H.history, nh, first_lo, np, off, cnt, idx); count_launch(); }
+  if (nh) { scatter_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, off, cnt, idx); count_launch(); }
   // 2. adder, blur, window, time
   adder_kernel<<<grid_for(N), 256, 0, st>>>(P, H, first_history, np, off, idx, T); count_launch();
   // 3. time-bucket counting sort

@@ -1,0 +1,112 @@
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/gpet.h declares, and its
+host logic (descriptor validation, ring placement, error reporting) behaves as documented.  No kernel runs."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import gpet_oracle as O
+from paper_2603_07327_b200 import api, build, workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def built():
+    build.build()
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "gpet.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(gpet_[a-z_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    names = declared_functions()
+    assert "gpet_simulate" in names and "gpet_digitize" in names and len(names) >= 14
+    lib = ctypes.CDLL(api.LIB_PATH)
+    for n in names:
+        assert hasattr(lib, n), f"{n} is declared in gpet.h but not exported"
+    assert sorted(api.EXPORTS) == names
+
+
+def test_binding_structs_match_the_header_layout():
+    # sizes follow from the C declarations (LP64): checked so that a header edit cannot silently skew the binding
+    assert ctypes.sizeof(api._LayerDesc) == 48 and ctypes.sizeof(api._GeometryDesc) == 64
+    assert ctypes.sizeof(api._Source) == 104 and ctypes.sizeof(api._Hits) == 80
+    assert ctypes.sizeof(api._Digitizer) == 32 and ctypes.sizeof(api._Singles) == 72 and ctypes.sizeof(api._Coinc) == 80
+
+
+def test_ring_placement_equals_the_oracles_bit_for_bit():
+    for geom in (W.geometry_c1(), W.geometry_paper_1cl(), W.Geometry(7, W.geometry_c1().layers, (2, 4), (16.0, 16.0), (16.0, 16.0),
+                                                                      ring_inner_radius_mm=40.0, ring_first_angle_deg=12.5)):
+        g = api.gpet_geometry_create(geom)
+        want = O.ring_poses(geom.n_panels, geom.ring_inner_radius_mm, geom.ring_first_angle_deg)
+        for p in range(geom.n_panels):
+            assert np.array_equal(api.gpet_geometry_panel_pose(g, p).view(np.uint32), want[p].view(np.uint32))
+    pose = api.gpet_geometry_panel_pose(api.gpet_geometry_create(W.geometry_c1()), 3)   # 90 degrees: exact zeros
+    assert pose[0] == 0.0 and pose[1] == 55.0 and pose[3] == -1.0 and pose[4] == 0.0
+
+
+def test_explicit_poses_are_kept_verbatim():
+    g0 = W.geometry_c0()
+    g = api.gpet_geometry_create(g0)
+    assert np.array_equal(api.gpet_geometry_panel_pose(g, 0), g0.panel_pose[0])
+    with pytest.raises(api.GpetError):
+        api.gpet_geometry_panel_pose(g, 1)
+
+
+@pytest.mark.parametrize("bad", [
+    dict(n=(17, 16)),                      # lattice wider than its module
+    dict(offset=(0.5, 0.0)),               # shifted 16x16 overhangs (SURVEY O9's alternative is rejected)
+    dict(depth=0.0), dict(pitch=(0.0, 1.0)), dict(reflector=(1.0, 0.1)), dict(material=9),
+])
+def test_geometry_validation(bad):
+    l = W.Layer(bad.get("n", (16, 16)), bad.get("pitch", (1.0, 1.0)), bad.get("reflector", (0.1, 0.1)), bad.get("offset", (0.0, 0.0)),
+                bad.get("depth", 10.0), 0.0, bad.get("material", 0))
+    with pytest.raises(api.GpetError, match="error -2"):
+        api.gpet_geometry_create(W.Geometry(12, (l,), (2, 4), (16.0, 16.0), (16.0, 16.0), ring_inner_radius_mm=55.0))
+    # the oracle rejects the same descriptors
+    if "material" not in bad:
+        with pytest.raises(ValueError):
+            O.locate(W.Geometry(12, (l,), (2, 4), (16.0, 16.0), (16.0, 16.0), ring_inner_radius_mm=55.0), np.zeros((1, 3), np.float32))
+
+
+def test_geometry_count_limits():
+    l = W.geometry_c1().layers
+    for kw in (dict(n_panels=64), dict(n_panels=0)):
+        with pytest.raises(api.GpetError):
+            api.gpet_geometry_create(W.Geometry(kw["n_panels"], l, (2, 4), (16.0, 16.0), (16.0, 16.0), ring_inner_radius_mm=55.0))
+    with pytest.raises(api.GpetError):
+        api.gpet_geometry_create(W.Geometry(12, l * 5, (2, 4), (16.0, 16.0), (16.0, 16.0), ring_inner_radius_mm=55.0))
+    api.gpet_geometry_create(W.Geometry(63, l, (2, 4), (16.0, 16.0), (16.0, 16.0), ring_inner_radius_mm=400.0))
+
+
+def test_table_validation_needs_no_kernel():
+    t = W.tables()
+    bad = W.Tables(t.e_min_keV, t.e_step_keV, -t.mu_pe, t.mu_compton, t.mu_rayleigh)
+    with pytest.raises(api.GpetError, match="error -3"):
+        api.gpet_materials_load(bad)
+    nan = t.mu_pe.copy(); nan[0, 5] = np.nan
+    with pytest.raises(api.GpetError, match="error -3"):
+        api.gpet_materials_load(W.Tables(t.e_min_keV, t.e_step_keV, nan, t.mu_compton, t.mu_rayleigh))
+
+
+def test_product_path_fails_loudly_without_a_gpu(tables):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(api.GpetError, match="error -5"):       # GPET_E_CUDA, never a CPU fallback
+        api.gpet_materials_load(tables)
+    g = api.gpet_geometry_create(W.geometry_c0())
+    with pytest.raises(api.GpetError, match="error -5"):
+        api.gpet_geometry_locate(g, np.zeros((4, 3), np.float32))
+
+
+def test_scratch_size_is_monotone():
+    a = api.gpet_digitize_scratch_bytes(1000, 800)
+    b = api.gpet_digitize_scratch_bytes(10_000_000, 8_000_000)
+    assert 0 < a < b < 2 * 1024 ** 3

@@ -1,0 +1,272 @@
+"""Parity of the CUDA path (through the C ABI) against the oracle.  All tests need a B200: `-m gpu`.
+
+Bars (BASELINE.json north_star): indexing on deterministic rays bit-exact; >= 99.99 % of histories with an
+identical outcome hash; for those, |dx| <= 1e-3 mm and |dE| <= 1e-3 keV; per-crystal histograms chi-square
+p > 0.01; digitizer output equal on equal input."""
+import numpy as np
+import pytest
+
+from oracle import gpet_oracle as O
+from paper_2603_07327_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+if torch.cuda.is_available():
+    import parity_util as PU
+    from paper_2603_07327_b200 import api
+
+MIN_MATCH = 0.9999          # north_star
+POS_TOL, E_TOL = 1e-3, 1e-3  # mm, keV (north_star)
+TOF_TOL = 1e-4              # ns  (= 0.03 mm of path; fp32 path sums differ by ~1e-5 mm)
+
+
+def run_both(run, tables, n=None, first=0):
+    n = n or run.n_pairs
+    g, gh, cnt = PU.gpu_simulate(run, tables, n_pairs=n, first_history=first)
+    o = O.simulate(run.geometry, tables, run.source, n, run.seed, first_history=first, want_hash=True, threads=8)
+    return g, gh, cnt, o
+
+
+# ----------------------------------------------------------------------------- transport
+def test_c0_every_hit(tables):
+    """configs[0] in full: 1e5 pairs, seed 1, all hits (crystal id, xyz fp32, E keV) compared."""
+    r = W.config_runs("C0")[0]
+    g, gh, cnt, o = run_both(r, tables)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] == 1.0 and cnt == len(o.hits) == res["n_hits_compared"] > 400
+    assert np.array_equal(g["ids"], o.hits.ids) and np.array_equal(g["history"], o.hits.history)
+
+
+RING_CASES = [("C1", 0), ("C2", 0), ("C2", 4), ("C3", 0), ("C3", 10), ("C3", 21)]
+
+
+@pytest.mark.parametrize("cfg,idx", RING_CASES)
+def test_ring_parity(tables, cfg, idx):
+    """300k pairs span ~1200 blocks of the transport grid and a ragged tail (300k is no multiple of 256)."""
+    r = W.config_runs(cfg, 300_001)[idx]
+    g, gh, cnt, o = run_both(r, tables)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= MIN_MATCH, res
+    assert abs(cnt - len(o.hits)) <= 60
+    assert PU.chi2_crystal_histograms(g["ids"], o.hits.ids) > 0.01
+    layers = (g["ids"] >> 18) & 3
+    assert layers.max() == len(r.geometry.layers) - 1                 # per-layer ids recorded
+
+
+def test_c4_phantom_parity(tables):
+    r = W.config_runs("C4", 150_000)[0]
+    g, gh, cnt, o = run_both(r, tables)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= MIN_MATCH and res["n_hits_compared"] > 20_000, res
+    assert o.counters["ph_compton"] > 10_000                         # the phantom really scatters
+
+
+def test_offset_history_ranges_and_append(tables):
+    """first_history offsets the counter-based streams; two appended calls equal one call."""
+    r = W.config_runs("C3", 40_000)[5]
+    g, gh, cnt, o = run_both(r, tables, n=40_000, first=123_456_789)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, first_history=123_456_789)
+    assert res["frac"] >= MIN_MATCH
+    geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+    hb = api.HitBuffer.allocate(200_000)
+    api.gpet_simulate(geom, m, s, 123_456_789, 15_000, r.seed, hb)
+    api.gpet_simulate(geom, m, s, 123_456_789 + 15_000, 25_000, r.seed, hb)       # appends
+    torch.cuda.synchronize()
+    two = PU.canonical(hb.to_numpy())
+    assert all(np.array_equal(two[k], g[k]) for k in PU.HIT_KEYS)
+
+
+def test_overflow_is_counted_and_rerun_is_identical(tables):
+    r = W.config_runs("C1", 50_000)[0]
+    geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+    small = api.HitBuffer.allocate(1000)
+    api.gpet_simulate(geom, m, s, 0, 50_000, r.seed, small)
+    torch.cuda.synchronize()
+    n = small.count()
+    assert n > 30_000 > small.capacity                                # dropped but counted
+    runs = []
+    for _ in range(2):
+        hb = api.HitBuffer.allocate(n)
+        api.gpet_simulate(geom, m, s, 0, 50_000, r.seed, hb)
+        torch.cuda.synchronize()
+        assert hb.count() == n
+        runs.append(PU.canonical(hb.to_numpy()))
+    assert all(np.array_equal(runs[0][k], runs[1][k]) for k in PU.HIT_KEYS)   # deterministic up to buffer order
+
+
+def test_degenerate_inputs(tables):
+    r = W.config_runs("C1", 1)[0]
+    geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+    hb = api.HitBuffer.allocate(64, n_hash=1)
+    api.gpet_simulate(geom, m, s, 0, 0, r.seed, hb)                   # empty batch: no-op
+    torch.cuda.synchronize()
+    assert hb.count() == 0
+    for first in (0, 7, 2 ** 33 + 5):                                 # single histories, also beyond 32 bits
+        hb.n_hits.zero_()
+        api.gpet_simulate(geom, m, s, first, 1, r.seed, hb)
+        torch.cuda.synchronize()
+        o = O.simulate(r.geometry, tables, r.source, 1, r.seed, first_history=first, want_hash=True)
+        assert hb.count() == len(o.hits) and int(hb.outcome_hash.cpu().numpy().view(np.uint64)[0]) == int(o.outcome_hash[0])
+    # source inside a panel box [R30]
+    inside = W.Run("inside", W.geometry_c1(), W.source_point((58.0, 1.0, 2.0)), 20_000, 77)
+    g, gh, cnt, o = run_both(inside, tables)
+    assert PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash)["frac"] >= MIN_MATCH and cnt > 15_000
+
+
+# ----------------------------------------------------------------------------- indexing
+def test_locate_is_bit_exact(tables):
+    from test_oracle_pins import tiny_scanner
+    rng = np.random.default_rng(21)
+    for geom, span in ((tiny_scanner(), 32.0), (W.geometry_c3(), 70.0), (W.geometry_c0(), 62.0)):
+        xyz = rng.uniform(-span, span, (200_000, 3)).astype(np.float32)
+        g = api.gpet_geometry_create(geom)
+        got = api.gpet_geometry_locate(g, xyz)
+        want = O.locate(geom, xyz)
+        assert np.array_equal(got, want)
+        assert (got != api.GPET_IDS_NONE).sum() > 1000
+    # dyadic points on crystal / module / layer faces of the axis-aligned C0 panel
+    grid = np.arange(-6.5, 6.51, 0.0625, dtype=np.float32)
+    a, b, c = np.meshgrid(grid, grid[::4], np.arange(-0.25, 10.5, 0.25, dtype=np.float32), indexing="ij")
+    xyz = np.stack([50.0 + c.ravel(), a.ravel(), b.ravel()], 1).astype(np.float32)
+    g = api.gpet_geometry_create(W.geometry_c0())
+    assert np.array_equal(api.gpet_geometry_locate(g, xyz), O.locate(W.geometry_c0(), xyz))
+
+
+def test_deterministic_rays_index_bit_exact(tables):
+    """north_star: crystal/layer/panel indexing on deterministic test rays is bit-exact.  Pencil beams from
+    several points, along and across the lattice, through reflector lines, module gaps and the layer offset."""
+    rays = [((0, 0, 0), (1, 0, 0)), ((0, 0.3, 0.4), (1, 0.05, 0.02)), ((5, 1, -3), (0.3, 0.9, 0.1)), ((0, 0, 0), (0.5, 0.866, 0.3)),
+            ((10, -4, 20), (-0.7, -0.7, -0.1)), ((0, 0, 0.5), (0, 1, 0)), ((0, 0, 0), (1, 0, 1e-3)), ((30, 30, 0), (1, 1, 0)),
+            ((0, 0, 31.95), (1, 0.2, 0)), ((2, 3, 4), (-1, 0.01, 0.3))]
+    total = 0
+    for pos, d in rays:
+        r = W.Run("ray", W.geometry_c3(), W.source_beam(pos, d, acolinearity_fwhm_deg=0.0), 4000, 91)
+        g, gh, cnt, o = run_both(r, tables)
+        assert np.array_equal(gh, o.outcome_hash)                     # every lattice decision of every history
+        assert np.array_equal(g["ids"], o.hits.ids)
+        total += cnt
+    assert total > 20_000
+
+
+# ----------------------------------------------------------------------------- digitizer
+@pytest.mark.parametrize("level", [0, 1, 2])
+def test_digitizer_equals_oracle_on_oracle_hits(tables, level):
+    """Same hits in (oracle-made, shuffled) -> singles and coincidences must be identical records."""
+    n = 300_001
+    src = W.source_point((10.0, 0.0, 4.0), activity_bq=5.0e7)         # hot enough for randoms and multiples
+    o = O.simulate(W.geometry_c3(), tables, src, n, 404, first_history=1000, threads=8)
+    dig = W.Digitizer(0.15, 511.0, 350.0, 650.0, 4.0, level)
+    osg, oco, _ = O.digitize(src, 404, 10 * n, o.hits, dig)
+    perm = np.random.default_rng(2).permutation(len(o.hits))
+    hb = PU.upload_hits(PU.oracle_hits_dict(o.hits), perm)
+    s = api.DeviceSource(src)
+    scratch = torch.empty(api.gpet_digitize_scratch_bytes(n, len(o.hits)), dtype=torch.uint8, device="cuda")
+    sg, co = api.SinglesBuffer.allocate(len(o.hits)), api.CoincBuffer.allocate(len(o.hits))
+    api.gpet_digitize(s, 404, 10 * n, 1000, n, hb, len(o.hits), dig, scratch, sg, co)
+    torch.cuda.synchronize()
+    gs, gc = sg.to_numpy(), co.to_numpy()
+    # energies are blurred in fp32 on the device: a single within ~1e-4 keV of a window edge may flip
+    assert abs(len(gs["ids"]) - len(osg.ids)) <= 2
+    if len(gs["ids"]) == len(osg.ids):
+        assert np.array_equal(gs["ids"], osg.ids) and np.array_equal(gs["history"], osg.history)
+        assert np.array_equal(gs["t_s"], osg.t_s)                     # fp64 times are bit-identical
+        assert np.max(np.abs(gs["e_keV"] - osg.e_keV)) < E_TOL
+        assert all(np.array_equal(gs[k], getattr(osg, k)) for k in ("x", "y", "z"))
+        assert np.array_equal(gc["ids_a"], oco.ids_a) and np.array_equal(gc["ids_b"], oco.ids_b)
+        assert np.array_equal(gc["history_a"], oco.history_a) and np.array_equal(gc["history_b"], oco.history_b)
+        assert np.array_equal(gc["t_s"], oco.t_s) and np.max(np.abs(gc["dt_ns"] - oco.dt_ns)) < 1e-6
+    assert len(oco.ids_a) > 5000 and np.sum(oco.history_a != oco.history_b) > 50
+    assert np.all(np.diff(gs["t_s"]) >= 0)
+
+
+def test_digitizer_empty_and_tiny(tables):
+    src = W.source_point()
+    s = api.DeviceSource(src)
+    hb = api.HitBuffer.allocate(16)
+    scratch = torch.empty(api.gpet_digitize_scratch_bytes(100, 0), dtype=torch.uint8, device="cuda")
+    sg, co = api.SinglesBuffer.allocate(16), api.CoincBuffer.allocate(16)
+    api.gpet_digitize(s, 1, 100, 0, 100, hb, 0, W.Digitizer(), scratch, sg, co)
+    torch.cuda.synchronize()
+    assert int(sg.n_singles.item()) == 0 and int(co.n_coinc.item()) == 0
+
+
+def test_end_to_end_coincidences(tables):
+    """GPU hits -> GPU digitizer against oracle hits -> oracle digitizer (C1 shape)."""
+    r = W.config_runs("C1", 400_000)[0]
+    geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+    hb = api.HitBuffer.allocate(600_000)
+    api.gpet_simulate(geom, m, s, 0, r.n_pairs, r.seed, hb)
+    torch.cuda.synchronize()
+    nh = hb.count()
+    scratch = torch.empty(api.gpet_digitize_scratch_bytes(r.n_pairs, nh), dtype=torch.uint8, device="cuda")
+    co = api.CoincBuffer.allocate(nh)
+    api.gpet_digitize(s, r.seed, r.n_pairs, 0, r.n_pairs, hb, nh, r.digitizer, scratch, None, co)    # coincidences only
+    torch.cuda.synchronize()
+    gc = co.to_numpy()
+    o = O.simulate(r.geometry, tables, r.source, r.n_pairs, r.seed, threads=8)
+    _, oco, _ = O.digitize(r.source, r.seed, r.n_pairs, o.hits, r.digitizer)
+    key = lambda c: set(zip(np.asarray(c["history_a"]).tolist(), np.asarray(c["history_b"]).tolist(), (np.asarray(c["ids_a"]) >> 5).tolist(),
+                            (np.asarray(c["ids_b"]) >> 5).tolist()))
+    kg, ko = key(gc), key(dict(history_a=oco.history_a, history_b=oco.history_b, ids_a=oco.ids_a, ids_b=oco.ids_b))
+    assert len(ko) > 20_000 and len(kg ^ ko) <= 1e-3 * len(ko)
+    assert 0.05 < len(ko) / r.n_pairs < 0.065                         # ~0.057 coincidences per pair
+
+
+def test_run_host_matches_device_path(tables):
+    r = W.config_runs("C3", 100_000)[3]
+    geom, m = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables)
+    host, counts = api.gpet_run_host(geom, m, r.source, r.n_pairs, 0, r.n_pairs, r.seed, r.digitizer, want_hits=True, want_singles=True)
+    s = api.DeviceSource(r.source)
+    hb = api.HitBuffer.allocate(300_000)
+    api.gpet_simulate(geom, m, s, 0, r.n_pairs, r.seed, hb)
+    torch.cuda.synchronize()
+    nh = hb.count()
+    assert counts["n_hits"] == nh
+    scratch = torch.empty(api.gpet_digitize_scratch_bytes(r.n_pairs, nh), dtype=torch.uint8, device="cuda")
+    sg, co = api.SinglesBuffer.allocate(nh), api.CoincBuffer.allocate(nh)
+    api.gpet_digitize(s, r.seed, r.n_pairs, 0, r.n_pairs, hb, nh, r.digitizer, scratch, sg, co)
+    torch.cuda.synchronize()
+    gs, gc = sg.to_numpy(), co.to_numpy()
+    assert counts["n_singles"] == len(gs["ids"]) and counts["n_coinc"] == len(gc["ids_a"]) > 4000
+    nc = counts["n_coinc"]
+    assert np.array_equal(host["coinc"][0][:nc].numpy().view(np.uint32), gc["ids_a"])
+    assert np.array_equal(host["coinc"][7][:nc].numpy(), gc["t_s"])
+    assert np.array_equal(host["singles"][6][:counts["n_singles"]].numpy(), gs["t_s"])
+    hh = {k: host["hits"][i][:nh].numpy() for i, k in enumerate(PU.HIT_KEYS)}
+    hh["history"], hh["ids"] = hh["history"].view(np.uint32), hh["ids"].view(np.uint32)
+    a, b = PU.canonical(hh), PU.canonical(hb.to_numpy())
+    assert all(np.array_equal(a[k], b[k]) for k in PU.HIT_KEYS)
+
+
+# ----------------------------------------------------------------------------- full size, bench launch configuration
+def test_c1_full_size_sampled_histories(tables):
+    """configs[1] at its full 1e7 pairs in the configuration bench.py times; the oracle recomputes 24 random
+    blocks of 4096 histories (it can start anywhere: draws are keyed by history id)."""
+    r = W.config_runs("C1")[0]
+    geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+    hb = api.HitBuffer.allocate(int(1.2 * r.n_pairs), n_hash=r.n_pairs)
+    api.gpet_simulate(geom, m, s, 0, r.n_pairs, r.seed, hb)
+    torch.cuda.synchronize()
+    nh = hb.count()
+    assert 0.76 < nh / r.n_pairs < 0.79                               # 0.77 hits per pair
+    gh = hb.outcome_hash.cpu().numpy().view(np.uint64)
+    g = hb.to_numpy()
+    rng = np.random.default_rng(5)
+    starts = np.concatenate([[0, r.n_pairs - 4096], rng.integers(0, r.n_pairs - 4096, 22)])
+    same = tot = 0
+    for st in starts:
+        o = O.simulate(r.geometry, tables, r.source, 4096, r.seed, first_history=int(st), want_hash=True, threads=4)
+        ok = gh[st:st + 4096] == o.outcome_hash
+        same += int(ok.sum()); tot += 4096
+        sel = (g["history"] >= st) & (g["history"] < st + 4096)
+        part = PU.canonical({k: v[sel] for k, v in g.items()})
+        PU.compare_hits(part, PU.oracle_hits_dict(o.hits), gh[st:st + 4096], o.outcome_hash, first_history=int(st),
+                        pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert same / tot >= MIN_MATCH
+    # properties that hold at any size: every panel equally hit (centred source), axial symmetry
+    counts = np.bincount(g["ids"] >> 26, minlength=12)
+    from scipy import stats
+    assert stats.chisquare(counts).pvalue > 1e-4
+    up, down = int((g["z"] > 0).sum()), int((g["z"] < 0).sum())
+    assert abs(up - down) < 5 * np.sqrt(up + down)

@@ -125,8 +125,8 @@ typedef struct {                  /* struct of arrays, DEVICE, caller-owned     
   float    *tof_ns;               /* time of flight from the decay                                      */
   uint64_t  capacity;             /* entries in each array                                              */
   uint64_t *n_hits;               /* DEVICE counter; NOT reset by the library, so several calls append  */
-  uint64_t *outcome_hash;         /* DEVICE, optional (NULL = off): n_pairs words, per-history FNV-1a   */
-                                  /* over the ordered event codes [R23] (parity instrument)             */
+  uint64_t *outcome_hash;         /* DEVICE, optional (NULL = off): 2*n_pairs words, [2*i + photon] =   */
+                                  /* FNV-1a over that photon's ordered event codes [R23] (parity tool)  */
 } gpet_hits;
 
 /* Simulates histories [first_history, first_history + n_pairs): source -> (phantom) -> panel search ->

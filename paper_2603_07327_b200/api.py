@@ -225,11 +225,12 @@ class HitBuffer:
 
     @staticmethod
     def allocate(capacity: int, n_hash: int = 0, device="cuda") -> "HitBuffer":
+        """n_hash = number of histories to hash (2 words each: photon A, photon B)."""
         import torch
         i32 = lambda: torch.empty(capacity, dtype=torch.int32, device=device)
         f32 = lambda: torch.empty(capacity, dtype=torch.float32, device=device)
         return HitBuffer(i32(), i32(), f32(), f32(), f32(), f32(), f32(), torch.zeros(1, dtype=torch.int64, device=device),
-                         torch.empty(n_hash, dtype=torch.int64, device=device) if n_hash else None)
+                         torch.empty(2 * n_hash, dtype=torch.int64, device=device) if n_hash else None)
 
     @property
     def capacity(self) -> int:
@@ -360,7 +361,7 @@ def gpet_run_host(geom: Geometry, mats: Materials, src, n_pairs_total: int, firs
         host["hits"] = [pin(torch.int32) for _ in range(2)] + [pin(torch.float32) for _ in range(5)] if want_hits else None
         host["singles"] = ([pin(torch.int32) for _ in range(2)] + [pin(torch.float32) for _ in range(4)] + [pin(torch.float64)]
                            if want_singles else None)
-        host["hash"] = pin(torch.int64, n_pairs) if want_hash else None
+        host["hash"] = pin(torch.int64, 2 * n_pairs) if want_hash else None
     cnt = host["counts"]
     out = _HostOutputs()
     if host["hits"] is not None:

@@ -260,6 +260,14 @@ static HitBuf hitbuf(const gpet_hits *h) {
 }
 
 // ---------------------------------------------------------------- transport
+// Work counters of the persistent kernel: a ring of 64 device words, one per launch in flight.
+static int next_work_counter(unsigned long long **out) {
+  static std::mutex lock; static unsigned long long *ring = nullptr; static unsigned slot = 0;
+  std::lock_guard<std::mutex> lk(lock);
+  if (!ring) CUDA_TRY(cudaMalloc(&ring, 64 * sizeof(unsigned long long)));
+  *out = ring + (slot++ & 63u); return GPET_OK;
+}
+
 extern "C" int gpet_simulate(const gpet_geometry *g, const gpet_materials *m, const gpet_source *src, uint64_t first_history,
                              uint64_t n_pairs, uint64_t seed, gpet_hits *hits, void *stream) {
   if (!g || !m || !src || !hits) return fail(GPET_E_INVALID_ARG, "gpet_simulate: NULL argument");
@@ -274,7 +282,8 @@ extern "C" int gpet_simulate(const gpet_geometry *g, const gpet_materials *m, co
   rc = geometry_upload(const_cast<gpet_geometry *>(g)); if (rc) return rc;
   const float *maj = nullptr; rc = majorant_table(const_cast<gpet_materials *>(m), g->host.det_mask, &maj); if (rc) return rc;
   DevTables T = { m->n_materials, m->n_energies, m->e_min, 1.0f / m->e_step, m->dev_mu };
-  CUDA_TRY(launch_transport(g->dev, T, maj, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, sm_count(), (cudaStream_t)stream));
+  unsigned long long *wc = nullptr; rc = next_work_counter(&wc); if (rc) return rc;
+  CUDA_TRY(launch_transport(g->dev, T, maj, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
   return GPET_OK;
 }
 
@@ -327,7 +336,7 @@ extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, co
   // one cached device arena per process: repeated batches of the same size do not re-allocate
   static std::mutex arena_lock; static char *arena_base = nullptr; static size_t arena_size = 0;
   std::lock_guard<std::mutex> arena_guard(arena_lock);
-  DevArena A; A.size = cap * (28 + 36 + 40) + scratch_bytes + nvox + (out->hits.outcome_hash ? 8 * n_pairs : 0) + 64 * 256;
+  DevArena A; A.size = cap * (28 + 36 + 40) + scratch_bytes + nvox + (out->hits.outcome_hash ? 16 * n_pairs : 0) + 64 * 256;
   if (A.size > arena_size) {
     if (arena_base) cudaFree(arena_base);
     arena_base = nullptr; arena_size = 0;
@@ -341,7 +350,7 @@ extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, co
     gpet_hits H; memset(&H, 0, sizeof H);
     H.history = A.take<uint32_t>(cap); H.ids = A.take<uint32_t>(cap); H.x = A.take<float>(cap); H.y = A.take<float>(cap); H.z = A.take<float>(cap);
     H.e_keV = A.take<float>(cap); H.tof_ns = A.take<float>(cap); H.capacity = cap; H.n_hits = A.take<uint64_t>(1);
-    H.outcome_hash = out->hits.outcome_hash ? A.take<uint64_t>(n_pairs) : nullptr;
+    H.outcome_hash = out->hits.outcome_hash ? A.take<uint64_t>(2 * n_pairs) : nullptr;
     gpet_singles S; S.history = A.take<uint32_t>(cap); S.ids = A.take<uint32_t>(cap); S.x = A.take<float>(cap); S.y = A.take<float>(cap);
     S.z = A.take<float>(cap); S.e_keV = A.take<float>(cap); S.t_s = A.take<double>(cap); S.capacity = cap; S.n_singles = A.take<uint64_t>(1);
     gpet_coincidences Cc; Cc.ids_a = A.take<uint32_t>(cap); Cc.ids_b = A.take<uint32_t>(cap); Cc.history_a = A.take<uint32_t>(cap);
@@ -367,7 +376,7 @@ extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, co
     const uint64_t ch = nh < out->hits.capacity ? nh : out->hits.capacity;
     D2H(out->hits.history, H.history, ch, uint32_t); D2H(out->hits.ids, H.ids, ch, uint32_t); D2H(out->hits.x, H.x, ch, float);
     D2H(out->hits.y, H.y, ch, float); D2H(out->hits.z, H.z, ch, float); D2H(out->hits.e_keV, H.e_keV, ch, float); D2H(out->hits.tof_ns, H.tof_ns, ch, float);
-    D2H(out->hits.outcome_hash, H.outcome_hash, n_pairs, uint64_t);
+    D2H(out->hits.outcome_hash, H.outcome_hash, 2 * n_pairs, uint64_t);
     const uint64_t cs = ns < out->singles.capacity ? ns : out->singles.capacity;
     D2H(out->singles.history, S.history, cs, uint32_t); D2H(out->singles.ids, S.ids, cs, uint32_t); D2H(out->singles.x, S.x, cs, float);
     D2H(out->singles.y, S.y, cs, float); D2H(out->singles.z, S.z, cs, float); D2H(out->singles.e_keV, S.e_keV, cs, float); D2H(out->singles.t_s, S.t_s, cs, double);

@@ -32,7 +32,7 @@ def gpu_simulate(run, tables, n_pairs=None, first_history=0, want_hash=True, hit
     torch.cuda.synchronize()
     cnt = hb.count()
     assert cnt <= hb.capacity, "hit buffer overflow in test"
-    hashes = hb.outcome_hash.cpu().numpy().view(np.uint64) if want_hash else None
+    hashes = hb.outcome_hash.cpu().numpy().view(np.uint64).reshape(-1, 2) if want_hash else None
     return canonical(hb.to_numpy()), hashes, cnt
 
 
@@ -52,7 +52,7 @@ def compare_hits(gpu: dict, orc: dict, gpu_hash, orc_hash, first_history=0, pos_
     """Per-history comparison.  Returns dict(n_histories, n_match, frac, max_dx, max_de, max_dt).
     Histories whose outcome hash agrees must have identical ids and agree within the tolerances."""
     n = len(orc_hash)
-    same = gpu_hash == orc_hash
+    same = np.all(np.asarray(gpu_hash).reshape(-1, 2) == np.asarray(orc_hash).reshape(-1, 2), axis=1)
     ok_g = same[(gpu["history"] - np.uint32(first_history)).astype(np.int64)]
     ok_o = same[(orc["history"] - np.uint32(first_history)).astype(np.int64)]
     g = {k: v[ok_g] for k, v in gpu.items()}

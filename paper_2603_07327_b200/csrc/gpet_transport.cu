@@ -14,6 +14,7 @@
 //  * geometry descriptor and interleaved float4 mu tables live in shared memory; hits are staged per warp
 //    in shared memory and flushed 32 at a time: one atomicAdd per 32 hits and seven fully coalesced
 //    128-byte stores (struct of arrays).
+#include <cstdlib>
 #include "gpet_internal.h"
 
 namespace gpet {
@@ -75,7 +76,7 @@ __device__ __forceinline__ void store_hit(const HitBuf &H, unsigned long long o,
 
 // ---------------------------------------------------------------- the kernel
 template <bool HASH>
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kThreads, 4)
 transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, DevSource src, uint64_t first_history, uint64_t n_photons,
                            uint64_t seed, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -208,13 +209,30 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
         if (use_phantom) { p.meta |= 1u << 11; p.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, p.E).z); st = ST_PHANTOM; }
         else st = ST_SEARCH;
       }
-    } else if (phase == ST_SEARCH) {
+      if (!use_phantom) phase = ST_SEARCH;                            // new photons go straight into the search
+    }
+    if (phase == ST_SEARCH) {
       // ------------------------------------------------ SEARCH: nearest-entry panel over all panels [R6]
       if (st == ST_SEARCH) {
         const int excl = ph_panel(p);
-        float bt = INFINITY; int bp = -1;
+        // candidate panels: with a common axial axis v, a panel can only be hit if the ray passes within the
+        // cross-section radius of its axis line (centre, v) and its bounding sphere is not entirely behind
+        unsigned long long cand = (g.n_panels >= 64 ? ~0ull : (1ull << g.n_panels) - 1ull) & ~(1ull << excl);
+        if (g.common_v) {
+          const float nx = p.d[1] * g.vaxis[2] - p.d[2] * g.vaxis[1], ny = p.d[2] * g.vaxis[0] - p.d[0] * g.vaxis[2],
+                      nz = p.d[0] * g.vaxis[1] - p.d[1] * g.vaxis[0];
+          const float lim = (nx * nx + ny * ny + nz * nz) * g.cull_r2sq + 1e-12f;
+          cand = 0;
 #pragma unroll 1
-        for (int q = 0; q < g.n_panels; ++q) {
+          for (int q = 0; q < g.n_panels; ++q) {
+            const float mx = g.centre[q][0] - p.x[0], my = g.centre[q][1] - p.x[1], mz = g.centre[q][2] - p.x[2];
+            const float s1 = mx * nx + my * ny + mz * nz, s2 = mx * p.d[0] + my * p.d[1] + mz * p.d[2];
+            if (s1 * s1 <= lim && s2 >= -g.cull_r3 && q != excl) cand |= 1ull << q;
+          }
+        }
+        float bt = INFINITY; int bp = -1;
+        while (cand) {                                               // ascending index: ties keep the lowest [R6]
+          const int q = __ffsll((long long)cand) - 1; cand &= cand - 1ull;
           float xl[3], dl[3];
           to_local(g.pose[q], p.x, p.d, xl, dl);
           float tn = -INFINITY, tf = INFINITY;
@@ -226,7 +244,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
             tn = fmaxf(tn, fminf(t1, t2)); tf = fminf(tf, fmaxf(t1, t2));
           }
           const float te = fmaxf(tn, 0.0f);
-          if (q != excl && tf > te && te < bt) { bt = te; bp = q; }
+          if (tf > te && te < bt) { bt = te; bp = q; }
         }
         if (bp < 0) { if (HASH) hash_ev(h, EV_ESCAPE, 0); finish(); }
         else {
@@ -240,8 +258,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
           st = ST_STEP;
         }
       }
-    }
-    else if (phase == ST_STEP) {
+    } else if (phase == ST_STEP) {
       // ------------------------------------------------ STEP: Woodcock step, layer selection, lattice lookup [R19]
       bool hit = false; float xg[3] = {0.f, 0.f, 0.f}; uint32_t hit_ids = 0;
       if (st == ST_STEP) {
@@ -382,7 +399,8 @@ cudaError_t launch_transport(const DevGeom *geom, const DevTables &T, const floa
   const size_t smem = transport_smem_bytes(T);
   const uint64_t n_photons = 2 * n_pairs;
   const uint64_t want = (n_photons + kThreads - 1) / kThreads;
-  const uint64_t resident = (uint64_t)sm_count * 2;                   // persistent grid: 2 CTAs per SM
+  static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : 4;
+  const uint64_t resident = (uint64_t)sm_count * ctas_per_sm;         // persistent grid
   const int blocks = (int)(want < resident ? (want ? want : 1) : resident);
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(unsigned long long), stream);
   if (e != cudaSuccess) return e;

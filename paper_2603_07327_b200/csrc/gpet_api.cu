@@ -113,22 +113,10 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
       q[9] = (float)cs; q[10] = (float)sn; q[11] = 0.0f;
     }
   }
-  // search culling data: box centres, cross-section radius about the common axial axis, bounding sphere
-  {
-    const double ac = 0.5 * ((double)G.blo[0] + G.bhi[0]), bc = 0.5 * ((double)G.blo[1] + G.bhi[1]), cc = 0.5 * (double)G.bhi[2];
-    const double ah = 0.5 * ((double)G.bhi[0] - G.blo[0]), bh = 0.5 * ((double)G.bhi[1] - G.blo[1]), ch = cc;
-    G.common_v = 1;
-    for (int p = 0; p < G.n_panels; ++p) {
-      const float *q = G.pose[p];
-      for (int k = 0; k < 3; ++k) {
-        G.centre[p][k] = (float)((double)q[k] + ac * q[3 + k] + bc * q[6 + k] + cc * q[9 + k]);
-        if (q[6 + k] != G.pose[0][6 + k]) G.common_v = 0;
-      }
-      G.centre[p][3] = 0.0f;
-    }
-    for (int k = 0; k < 3; ++k) G.vaxis[k] = G.pose[0][6 + k];
-    const double r2 = sqrt(ah * ah + ch * ch) * 1.001 + 1e-3, r3 = sqrt(ah * ah + bh * bh + ch * ch) * 1.001 + 1e-3;
-    G.cull_r2sq = (float)(r2 * r2); G.cull_r3 = (float)r3;
+  G.planar = 1;                 // axial axis = +z everywhere and no z component elsewhere (any repetition-mode ring)
+  for (int p = 0; p < G.n_panels; ++p) {
+    const float *q = G.pose[p];
+    if (q[2] != 0.0f || q[5] != 0.0f || q[11] != 0.0f || q[6] != 0.0f || q[7] != 0.0f || q[8] != 1.0f) G.planar = 0;
   }
   *out = g;                     // the device copy is made lazily so the handle can be built without a GPU
   return GPET_OK;

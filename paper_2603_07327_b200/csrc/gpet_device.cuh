@@ -30,10 +30,7 @@ struct DevGeom {
   float blo[3], bhi[3];       // panel box in the tracking frame (fp32 roundings of the Q extents)
   uint32_t det_mask;          // materials referenced by the layers
   int ring;                   // 1 = repetition mode
-  int common_v;               // 1 = every panel has the same axial axis v: the search culls panels by the
-  float vaxis[3];             //     distance between the ray and each panel's axis line (centre, v)
-  float cull_r2sq, cull_r3;   // (radius of the box cross-section normal to v)^2 and bounding-sphere radius, with margin
-  float centre[kMaxPanels][4];// box centres
+  int planar;                 // 1 = every panel has v = +z and u_z = w_z = o_z = 0: the search shares the axial slab
   DevLayer layer[kMaxLayers];
   float pose[kMaxPanels][12]; // front-face centre, u, v, w
 };

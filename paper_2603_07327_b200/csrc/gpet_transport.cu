@@ -2,18 +2,19 @@
 // PAPER.md:33 (panel transfer by ray/plane crossing, global->local), PAPER.md:43 (Woodcock tracking in the
 // panel frame, layer selection from the local depth, run until exit or cutoff).
 //
-// Design:
-//  * unit of work = one photon (index j = 2*pair + photon); every lane of a persistent warp owns one photon
-//    and a small state machine {REFILL, SEARCH, STEP, COMPTON, RAYLEIGH, PHANTOM};
-//  * each pass of the warp's main loop ballots the lanes' next events and runs the ONE phase that most
-//    lanes are waiting for (wavefront regrouping in time): its code is fetched once for all of them, the
-//    other lanes keep their state in registers and wait; every phase appears exactly once in the kernel,
-//    which keeps the SASS small enough for the instruction caches (v1's 107 KB of inlined code stalled
-//    59 % of the time on instruction fetch);
-//  * photon indices are handed out from a global counter in chunks of 1024 per warp;
-//  * geometry descriptor and interleaved float4 mu tables live in shared memory; hits are staged per warp
-//    in shared memory and flushed 32 at a time: one atomicAdd per 32 hits and seven fully coalesced
-//    128-byte stores (struct of arrays).
+// Design.  The unit of work is one photon (index j = 2*pair + photon).  Every
+// persistent warp alternates between two roles and keeps two private photon pools in shared memory:
+//   GENERATE  all 32 lanes take a photon that needs a panel search -- one that left a panel (pool S) or a
+//             new one from the source (S3) -- and run the search together at full SIMD width; photons that
+//             enter a panel are compacted (ballot + prefix popcount) into pool T, the others are done;
+//   TRANSPORT every lane owns one in-panel photon and a small state machine {POP, STEP, COMPTON, RAYLEIGH,
+//             PHANTOM}; each pass ballots the lanes' next events and runs the ONE phase most lanes wait for
+//             (regrouping by next event); idle lanes refill from pool T, photons that leave their panel are
+//             pushed to pool S.
+// Every phase appears exactly once in the kernel, which keeps the SASS small enough for the instruction
+// caches (v1's 107 KB of inlined code stalled 59 % of the time on instruction fetch).  Geometry descriptor
+// and interleaved float4 mu tables live in shared memory; hits are staged per warp in shared memory and
+// flushed 32 at a time: one atomicAdd per 32 hits and seven fully coalesced 128-byte stores (SoA).
 #include <cstdlib>
 #include "gpet_internal.h"
 
@@ -22,21 +23,35 @@ namespace gpet {
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 constexpr int kStage = 64;            // staged hits per warp (ring buffer)
+constexpr int kPoolT = 64;            // photons waiting for in-panel transport (filled while < 32)
+constexpr int kPoolS = 96;            // photons waiting for a panel search (drained when >= 32; bound: DESIGN.md 5)
 constexpr uint32_t kChunk = 1024;     // photon indices a warp reserves at a time
 
-enum : int { ST_REFILL = 0, ST_SEARCH = 1, ST_STEP = 2, ST_COMPTON = 3, ST_RAYLEIGH = 4, ST_PHANTOM = 5, ST_IDLE = 6 };
+enum : int { ST_POP = 0, ST_STEP = 1, ST_COMPTON = 2, ST_RAYLEIGH = 3, ST_PHANTOM = 4, ST_NONE = 5 };
 
 struct HitStage { uint32_t w[7][kStage]; };      // history, ids, x, y, z, e, tof
 
-struct Smem {
+// 48 bytes per parked photon; the Philox block is not parked (it is regenerated on demand)
+template <int N, bool HASH> struct Pool {
+  float4 a[N];                         // x, y, z, dx
+  float4 b[N];                         // dy, dz, E, path
+  uint4 c[N];                          // pair, meta, ndraw, inv_mu bits
+  uint2 hh[HASH ? N : 1];              // outcome hash (parity builds only)
+};
+
+template <bool HASH> struct WarpMem { Pool<kPoolT, HASH> T; Pool<kPoolS, HASH> S; HitStage stage; };
+
+template <bool HASH> struct Smem {
   DevGeom g;
-  HitStage stage[kWarps];
+  WarpMem<HASH> w[kWarps];
   float4 mu[1];                        // [n_materials][n_energies], .w = detector majorant
 };
 
 // ---------------------------------------------------------------- fast math with bounded error
 __device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float sqrt_fast(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+// 1/d with a zero component treated as +tiny: an inside point then sees (-inf, +inf), an outside one misses [R32]
+__device__ __forceinline__ float rcp_dir(float d) { return rcp_fast(d == 0.0f ? 1e-30f : d); }
 // (sin, cos)(2 pi u), u in (0,1): argument folded to [-pi, pi] where sin.approx / cos.approx are good to 2^-21
 __device__ __forceinline__ void sincos_2pi(float u, float &s, float &c) {
   const float a = 6.283185307179586f * (u - 0.5f);
@@ -52,18 +67,32 @@ __device__ __forceinline__ float4 mu_lookup(const float4 *mu, const DevTables &T
   return make_float4(fmaf(f, b.x - a.x, a.x), fmaf(f, b.y - a.y, a.y), fmaf(f, b.z - a.z, a.z), fmaf(f, b.w - a.w, a.w));
 }
 
-// ---------------------------------------------------------------- per-lane photon state
+// ---------------------------------------------------------------- photon state
 struct Photon {
-  float x[3], d[3];        // global frame in SEARCH / PHANTOM, panel frame in STEP / COMPTON / RAYLEIGH
+  float x[3], d[3];        // global frame while searching / in the phantom, panel frame in STEP / COMPTON / RAYLEIGH
   float E, path, inv_mu;   // inv_mu = 1 / majorant(E) of the medium the photon is tracked in
   uint32_t pair;           // history - first_history
   uint32_t meta;           // bit0 photon, bits1-4 seq, bits5-10 panel (current, or just left; 63 = none),
                            // bit11 in phantom, bits12+ Klein-Nishina trial counter
-  uint32_t ids;            // lattice result of the pending interaction
-  uint32_t ndraw; uint4 blk;
+  uint32_t ndraw;          // draws consumed from this photon's stream [R4]
 };
 __device__ __forceinline__ int ph_panel(const Photon &p) { return (p.meta >> 5) & 63u; }
 __device__ __forceinline__ void ph_set_panel(Photon &p, int panel) { p.meta = (p.meta & ~(63u << 5)) | ((uint32_t)panel << 5); }
+
+template <int N, bool HASH>
+__device__ __forceinline__ void pool_store(Pool<N, HASH> &P, int slot, const Photon &p, uint64_t h) {
+  P.a[slot] = make_float4(p.x[0], p.x[1], p.x[2], p.d[0]);
+  P.b[slot] = make_float4(p.d[1], p.d[2], p.E, p.path);
+  P.c[slot] = make_uint4(p.pair, p.meta, p.ndraw, __float_as_uint(p.inv_mu));
+  if (HASH) P.hh[slot] = make_uint2((uint32_t)h, (uint32_t)(h >> 32));
+}
+template <int N, bool HASH>
+__device__ __forceinline__ void pool_load(const Pool<N, HASH> &P, int slot, Photon &p, uint64_t &h) {
+  const float4 a = P.a[slot], b = P.b[slot]; const uint4 c = P.c[slot];
+  p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.d[0] = a.w; p.d[1] = b.x; p.d[2] = b.y; p.E = b.z; p.path = b.w;
+  p.pair = c.x; p.meta = c.y; p.ndraw = c.z; p.inv_mu = __uint_as_float(c.w);
+  if (HASH) { const uint2 v = P.hh[slot]; h = ((uint64_t)v.y << 32) | v.x; }
+}
 
 // write one staged hit (slot of this warp's ring buffer) to the global struct-of-arrays buffer
 __device__ __forceinline__ void store_hit(const HitBuf &H, unsigned long long o, const HitStage &stage, uint32_t slot) {
@@ -74,13 +103,53 @@ __device__ __forceinline__ void store_hit(const HitBuf &H, unsigned long long o,
   }
 }
 
+// ---------------------------------------------------------------- [R6] panel search
+// Nearest-entry panel over all panels but `excl`; ties keep the lowest index; -1 = escapes.
+// "planar" detectors (every panel has v = +z, u_z = w_z = o_z = 0: any ring built in repetition mode,
+// PAPER.md:33) share the axial slab and need only the 2-D part of each pose; the arithmetic on the
+// surviving terms is the generic one (the dropped terms are exact zeros).
+__device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], const float d[3], int excl, float &t_enter) {
+  float bt = INFINITY; int bp = -1;
+  if (g.planar) {
+    const float iz = rcp_dir(d[2]);
+    const float z1 = (g.blo[1] - x[2]) * iz, z2 = (g.bhi[1] - x[2]) * iz;
+    const float tnz = fmaxf(fminf(z1, z2), 0.0f), tfz = fmaxf(z1, z2);
+#pragma unroll 2
+    for (int q = 0; q < g.n_panels; ++q) {
+      const float *P = g.pose[q];
+      const float r0 = x[0] - P[0], r1 = x[1] - P[1];
+      const float a = r0 * P[3] + r1 * P[4], c = r0 * P[9] + r1 * P[10];
+      const float ia = rcp_dir(d[0] * P[3] + d[1] * P[4]), ic = rcp_dir(d[0] * P[9] + d[1] * P[10]);
+      const float a1 = (g.blo[0] - a) * ia, a2 = (g.bhi[0] - a) * ia, c1 = (g.blo[2] - c) * ic, c2 = (g.bhi[2] - c) * ic;
+      const float tn = fmaxf(tnz, fmaxf(fminf(a1, a2), fminf(c1, c2)));
+      const float tf = fminf(tfz, fminf(fmaxf(a1, a2), fmaxf(c1, c2)));
+      if (q != excl && tf > tn && tn < bt) { bt = tn; bp = q; }
+    }
+  } else {
+#pragma unroll 1
+    for (int q = 0; q < g.n_panels; ++q) {
+      float xl[3], dl[3];
+      to_local(g.pose[q], x, d, xl, dl);
+      float tn = 0.0f, tf = INFINITY;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        const float inv = rcp_dir(dl[k]);
+        const float t1 = (g.blo[k] - xl[k]) * inv, t2 = (g.bhi[k] - xl[k]) * inv;
+        tn = fmaxf(tn, fminf(t1, t2)); tf = fminf(tf, fmaxf(t1, t2));
+      }
+      if (q != excl && tf > tn && tn < bt) { bt = tn; bp = q; }
+    }
+  }
+  t_enter = bt; return bp;
+}
+
 // ---------------------------------------------------------------- the kernel
 template <bool HASH>
-__global__ void __launch_bounds__(kThreads, 4)
+__global__ void __launch_bounds__(kThreads, 2)
 transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, DevSource src, uint64_t first_history, uint64_t n_photons,
                            uint64_t seed, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Smem *S = reinterpret_cast<Smem *>(smem_raw);
+  Smem<HASH> *S = reinterpret_cast<Smem<HASH> *>(smem_raw);
   {
     const uint32_t *gs = reinterpret_cast<const uint32_t *>(geom);
     uint32_t *gd = reinterpret_cast<uint32_t *>(&S->g);
@@ -92,38 +161,42 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
   const DevGeom &g = S->g;
   const float4 *mu = S->mu;
   const int lane = threadIdx.x & 31;
-  HitStage &stage = S->stage[threadIdx.x >> 5];
+  WarpMem<HASH> &W = S->w[threadIdx.x >> 5];
+  HitStage &stage = W.stage;
   const unsigned lt_mask = (1u << lane) - 1u;
   const uint2 key = make_uint2((uint32_t)seed, (uint32_t)(seed >> 32));
   const bool use_phantom = src.kind == 1 && src.phantom != nullptr;
 
-  Photon p; p.meta = 0; p.ndraw = 0; p.E = 0.f; p.path = 0.f; p.inv_mu = 0.f; p.pair = 0; p.ids = kNone;
-  p.blk = make_uint4(0, 0, 0, 0);
+  Photon p; p.meta = 0; p.ndraw = 0; p.E = 0.f; p.path = 0.f; p.inv_mu = 0.f; p.pair = 0;
 #pragma unroll
   for (int k = 0; k < 3; ++k) { p.x[k] = 0.f; p.d[k] = 0.f; }
+  uint4 blk = make_uint4(0, 0, 0, 0);      // current Philox block of the lane's photon
+  uint32_t ids = kNone;                    // lattice result of the pending interaction
   uint64_t h = 0;
-  int st = ST_REFILL;
+  int st = ST_POP;
   uint64_t w_next = 0, w_end = 0;          // this warp's reserved photon indices [w_next, w_end)
   bool exhausted = false;                  // the global counter ran past n_photons
   uint32_t stage_head = 0, stage_cnt = 0;  // ring buffer of staged hits (warp-uniform)
+  int cntT = 0, cntS = 0;                  // pool fill levels (warp-uniform)
 
+  auto philox_block = [&](uint32_t block) {
+    const uint64_t history = first_history + p.pair;
+    blk = philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 1u + (p.meta & 1u), block), key);
+  };
   // next uniform of this photon's stream [R4]
   auto draw = [&]() -> float {
     const uint32_t j = p.ndraw & 3u;
-    if (j == 0) {
-      const uint64_t history = first_history + p.pair;
-      p.blk = philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 1u + (p.meta & 1u), p.ndraw >> 2), key);
-    }
+    if (j == 0) philox_block(p.ndraw >> 2);
     ++p.ndraw;
-    return u01(j == 0 ? p.blk.x : (j == 1 ? p.blk.y : (j == 2 ? p.blk.z : p.blk.w)));
+    return u01(j == 0 ? blk.x : (j == 1 ? blk.y : (j == 2 ? blk.z : blk.w)));
   };
   // stage one hit per lane that has one; flush 32 staged hits with one atomic + coalesced stores (S10)
-  auto stage_hits = [&](bool has, uint32_t ids, const float xg[3], float e, float tof) {
+  auto stage_hits = [&](bool has, uint32_t hit_ids, const float xg[3], float e, float tof) {
     const unsigned who = __ballot_sync(0xFFFFFFFFu, has);
     if (who == 0) return;
     if (has) {
       const uint32_t slot = (stage_head + stage_cnt + __popc(who & lt_mask)) & (kStage - 1);
-      stage.w[0][slot] = (uint32_t)(first_history + p.pair); stage.w[1][slot] = ids;
+      stage.w[0][slot] = (uint32_t)(first_history + p.pair); stage.w[1][slot] = hit_ids;
       stage.w[2][slot] = __float_as_uint(xg[0]); stage.w[3][slot] = __float_as_uint(xg[1]); stage.w[4][slot] = __float_as_uint(xg[2]);
       stage.w[5][slot] = __float_as_uint(e); stage.w[6][slot] = __float_as_uint(tof);
     }
@@ -138,137 +211,123 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
       __syncwarp();
     }
   };
-  auto finish = [&]() {                    // photon ended: publish its hash, ask for a new photon
-    if (HASH) hash_out[2ull * p.pair + (p.meta & 1u)] = h;
-    st = ST_REFILL;
-  };
 
 #pragma unroll 1
   for (;;) {
-    // ------------------------------------------------ choose the phase most lanes are waiting for
-    unsigned m_ref = __ballot_sync(0xFFFFFFFFu, st == ST_REFILL);
-    if (m_ref && exhausted && w_next >= w_end) {      // nothing left to hand out: those lanes retire
-      if (st == ST_REFILL) st = ST_IDLE;
-      m_ref = 0;
+    const bool more_src = !exhausted || w_next < w_end;
+    if ((cntT < 32 && (more_src || cntS > 0)) || (cntT <= 32 && cntS >= 32)) {
+      // ================================================ GENERATE: 32 photons that need a panel search
+      const int nS = min(cntS, 32);                                   // lanes [0, nS): photons that left a panel
+      Photon q; uint64_t hq = 0; bool active = lane < nS;
+      if (active) pool_load(W.S, cntS - 1 - lane, q, hq);
+      cntS -= nS;
+      __syncwarp();
+      // lanes [nS, 32): new photons from the source (S3) [R13-R15]
+      if (nS < 32) {
+        if (w_next >= w_end && !exhausted) {
+          unsigned long long b = 0;
+          if (lane == 0) b = atomicAdd(work_counter, (unsigned long long)kChunk);
+          b = __shfl_sync(0xFFFFFFFFu, b, 0);
+          if (b >= n_photons) { exhausted = true; w_next = w_end = 0; }
+          else { w_next = b; w_end = min((uint64_t)(b + kChunk), n_photons); }
+        }
+        const uint64_t j = w_next + (uint64_t)(lane - nS);
+        const bool fresh = lane >= nS && j < w_end;
+        w_next = min(w_next + (uint64_t)(32 - nS), w_end);
+        if (fresh) {
+          active = true;
+          q.pair = (uint32_t)(j >> 1); q.meta = (uint32_t)(j & 1u) | (63u << 5); q.ndraw = 0; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
+          if (HASH) hq = 0xCBF29CE484222325ull;
+          const uint64_t history = first_history + q.pair;
+          const uint32_t h_lo = (uint32_t)history, h_hi = (uint32_t)(history >> 32);
+          q.x[0] = src.pos[0]; q.x[1] = src.pos[1]; q.x[2] = src.pos[2];
+          if (src.kind == 1) {
+            const uint4 w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 0u), key);
+            const uint64_t Wl = src.w_total & 0xFFFFFFFFull, Wh = src.w_total >> 32;          // floor(w.x * W / 2^32), exact
+            const uint64_t target = (uint64_t)w.x * Wh + (((uint64_t)w.x * Wl) >> 32);
+            uint32_t lo = 0, hi = src.n_active - 1;
+            while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (src.act_cdf[mid] > target) hi = mid; else lo = mid + 1; }
+            const uint32_t vi = src.act_index[lo], nx = (uint32_t)src.dims[0], ny = (uint32_t)src.dims[1];
+            q.x[0] = src.origin[0] + ((float)(vi % nx) + u01(w.y)) * src.voxel[0];
+            q.x[1] = src.origin[1] + ((float)((vi / nx) % ny) + u01(w.z)) * src.voxel[1];
+            q.x[2] = src.origin[2] + ((float)(vi / (nx * ny)) + u01(w.w)) * src.voxel[2];
+          }
+          const uint4 w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 1u), key);
+          if (src.kind == 2) { q.d[0] = src.beam[0]; q.d[1] = src.beam[1]; q.d[2] = src.beam[2]; }
+          else {
+            const float u = u01(w.x), ct = 1.0f - 2.0f * u, sth = 2.0f * sqrtf(u * (1.0f - u));   // sin^2 = (1-ct)(1+ct)
+            float sp, cp; sincospif(2.0f * u01(w.y), &sp, &cp);
+            q.d[0] = sth * cp; q.d[1] = sth * sp; q.d[2] = ct;
+          }
+          if (q.meta & 1u) {                                          // photon B: opposite, plus acolinearity
+            q.d[0] = -q.d[0]; q.d[1] = -q.d[1]; q.d[2] = -q.d[2];
+            if (src.acol_sigma > 0.0f) {
+              const float rho = src.acol_sigma * sqrtf(-2.0f * logf(u01(w.z)));
+              float sr, cr; sincosf(rho, &sr, &cr);
+              float sp, cp; sincospif(2.0f * u01(w.w), &sp, &cp);
+              rotate(q.d, cr, sr, cp, sp);
+            }
+          }
+          if (use_phantom) { q.meta |= 1u << 11; q.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, q.E).z); }
+        }
+      }
+      // panel search [R6]; photons born inside a phantom skip it and are tracked there first [R17]
+      bool park = false;
+      if (active) {
+        if ((q.meta >> 11) & 1u) park = true;
+        else {
+          float bt; const int bp = panel_search(g, q.x, q.d, ph_panel(q), bt);
+          if (bp < 0) { if (HASH) { hash_ev(hq, EV_ESCAPE, 0); hash_out[2ull * q.pair + (q.meta & 1u)] = hq; } }
+          else {
+            if (HASH) hash_ev(hq, EV_ENTER, (uint32_t)bp);
+            float xl[3], dl[3];
+            to_local(g.pose[bp], q.x, q.d, xl, dl);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { q.x[k] = fmaf(bt, dl[k], xl[k]); q.d[k] = dl[k]; }   // [R18]
+            q.path += bt; ph_set_panel(q, bp);
+            q.inv_mu = rcp_fast(mu_lookup(mu, T, 0, q.E).w);
+            park = true;
+          }
+        }
+      }
+      const unsigned m_park = __ballot_sync(0xFFFFFFFFu, park);
+      if (park) pool_store(W.T, cntT + __popc(m_park & lt_mask), q, hq);
+      cntT += __popc(m_park);
+      __syncwarp();
+      continue;
     }
-    int phase = ST_IDLE, best = __popc(m_ref);
-    if (best) phase = ST_REFILL;
-    { int c;
-      c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_SEARCH));   if (c > best) { best = c; phase = ST_SEARCH; }
+    // ================================================ TRANSPORT: run the phase most lanes are waiting for
+    const unsigned m_pop = __ballot_sync(0xFFFFFFFFu, st == ST_POP);
+    int phase = ST_NONE, best = min(__popc(m_pop), cntT);
+    if (best) phase = ST_POP;
+    if (!(best && cntS >= 32)) {                                      // pool S nearly full: refilling lanes comes first
+      int c;
       c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_STEP));     if (c > best) { best = c; phase = ST_STEP; }
       c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_COMPTON));  if (c > best) { best = c; phase = ST_COMPTON; }
       c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_PHANTOM));  if (c > best) { best = c; phase = ST_PHANTOM; }
-      c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_RAYLEIGH)); if (c > best) { best = c; phase = ST_RAYLEIGH; } }
-    if (phase == ST_IDLE) break;
-
-    if (phase == ST_REFILL) {
-      // ------------------------------------------------ REFILL: new photon + source sampling (S3) [R13-R15]
-      if (w_next >= w_end && !exhausted) {
-        unsigned long long b = 0;
-        if (lane == 0) b = atomicAdd(work_counter, (unsigned long long)kChunk);
-        b = __shfl_sync(0xFFFFFFFFu, b, 0);
-        if (b >= n_photons) { exhausted = true; w_next = w_end = 0; }
-        else { w_next = b; w_end = min((uint64_t)(b + kChunk), n_photons); }
-      }
-      const uint64_t j = w_next + __popc(m_ref & lt_mask);
-      const bool take = st == ST_REFILL && j < w_end;
-      w_next = min(w_next + (uint64_t)__popc(m_ref), w_end);
-      if (take) {
-        p.pair = (uint32_t)(j >> 1); p.meta = (uint32_t)(j & 1u) | (63u << 5); p.ndraw = 0; p.E = 511.0f; p.path = 0.0f; p.ids = kNone;
-        if (HASH) h = 0xCBF29CE484222325ull;
-        const uint64_t history = first_history + p.pair;
-        const uint32_t h_lo = (uint32_t)history, h_hi = (uint32_t)(history >> 32);
-        p.x[0] = src.pos[0]; p.x[1] = src.pos[1]; p.x[2] = src.pos[2];
-        if (src.kind == 1) {
-          const uint4 w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 0u), key);
-          const uint64_t Wl = src.w_total & 0xFFFFFFFFull, Wh = src.w_total >> 32;          // floor(w.x * W / 2^32), exact
-          const uint64_t target = (uint64_t)w.x * Wh + (((uint64_t)w.x * Wl) >> 32);
-          uint32_t lo = 0, hi = src.n_active - 1;
-          while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (src.act_cdf[mid] > target) hi = mid; else lo = mid + 1; }
-          const uint32_t vi = src.act_index[lo], nx = (uint32_t)src.dims[0], ny = (uint32_t)src.dims[1];
-          p.x[0] = src.origin[0] + ((float)(vi % nx) + u01(w.y)) * src.voxel[0];
-          p.x[1] = src.origin[1] + ((float)((vi / nx) % ny) + u01(w.z)) * src.voxel[1];
-          p.x[2] = src.origin[2] + ((float)(vi / (nx * ny)) + u01(w.w)) * src.voxel[2];
-        }
-        const uint4 w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 1u), key);
-        if (src.kind == 2) { p.d[0] = src.beam[0]; p.d[1] = src.beam[1]; p.d[2] = src.beam[2]; }
-        else {
-          const float u = u01(w.x), ct = 1.0f - 2.0f * u, sth = 2.0f * sqrtf(u * (1.0f - u));   // sin^2 = (1-ct)(1+ct)
-          float sp, cp; sincospif(2.0f * u01(w.y), &sp, &cp);
-          p.d[0] = sth * cp; p.d[1] = sth * sp; p.d[2] = ct;
-        }
-        if (p.meta & 1u) {                                            // photon B: opposite, plus acolinearity
-          p.d[0] = -p.d[0]; p.d[1] = -p.d[1]; p.d[2] = -p.d[2];
-          if (src.acol_sigma > 0.0f) {
-            const float rho = src.acol_sigma * sqrtf(-2.0f * logf(u01(w.z)));
-            float sr, cr; sincosf(rho, &sr, &cr);
-            float sp, cp; sincospif(2.0f * u01(w.w), &sp, &cp);
-            rotate(p.d, cr, sr, cp, sp);
-          }
-        }
-        if (use_phantom) { p.meta |= 1u << 11; p.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, p.E).z); st = ST_PHANTOM; }
-        else st = ST_SEARCH;
-      }
-      if (!use_phantom) phase = ST_SEARCH;                            // new photons go straight into the search
+      c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_RAYLEIGH)); if (c > best) { best = c; phase = ST_RAYLEIGH; }
     }
-    if (phase == ST_SEARCH) {
-      // ------------------------------------------------ SEARCH: nearest-entry panel over all panels [R6]
-      if (st == ST_SEARCH) {
-        const int excl = ph_panel(p);
-        // candidate panels: with a common axial axis v, a panel can only be hit if the ray passes within the
-        // cross-section radius of its axis line (centre, v) and its bounding sphere is not entirely behind
-        unsigned long long cand = (g.n_panels >= 64 ? ~0ull : (1ull << g.n_panels) - 1ull) & ~(1ull << excl);
-        if (g.common_v) {
-          const float nx = p.d[1] * g.vaxis[2] - p.d[2] * g.vaxis[1], ny = p.d[2] * g.vaxis[0] - p.d[0] * g.vaxis[2],
-                      nz = p.d[0] * g.vaxis[1] - p.d[1] * g.vaxis[0];
-          const float lim = (nx * nx + ny * ny + nz * nz) * g.cull_r2sq + 1e-12f;
-          cand = 0;
-#pragma unroll 1
-          for (int q = 0; q < g.n_panels; ++q) {
-            const float mx = g.centre[q][0] - p.x[0], my = g.centre[q][1] - p.x[1], mz = g.centre[q][2] - p.x[2];
-            const float s1 = mx * nx + my * ny + mz * nz, s2 = mx * p.d[0] + my * p.d[1] + mz * p.d[2];
-            if (s1 * s1 <= lim && s2 >= -g.cull_r3 && q != excl) cand |= 1ull << q;
-          }
-        }
-        float bt = INFINITY; int bp = -1;
-        while (cand) {                                               // ascending index: ties keep the lowest [R6]
-          const int q = __ffsll((long long)cand) - 1; cand &= cand - 1ull;
-          float xl[3], dl[3];
-          to_local(g.pose[q], p.x, p.d, xl, dl);
-          float tn = -INFINITY, tf = INFINITY;
-#pragma unroll
-          for (int k = 0; k < 3; ++k) {
-            // a zero component behaves like +tiny: inside -> (-inf, +inf), outside -> miss [R32]
-            const float inv = rcp_fast(dl[k] == 0.0f ? 1e-30f : dl[k]);
-            const float t1 = (g.blo[k] - xl[k]) * inv, t2 = (g.bhi[k] - xl[k]) * inv;
-            tn = fmaxf(tn, fminf(t1, t2)); tf = fminf(tf, fmaxf(t1, t2));
-          }
-          const float te = fmaxf(tn, 0.0f);
-          if (tf > te && te < bt) { bt = te; bp = q; }
-        }
-        if (bp < 0) { if (HASH) hash_ev(h, EV_ESCAPE, 0); finish(); }
-        else {
-          if (HASH) hash_ev(h, EV_ENTER, (uint32_t)bp);
-          float xl[3], dl[3];
-          to_local(g.pose[bp], p.x, p.d, xl, dl);
-#pragma unroll
-          for (int k = 0; k < 3; ++k) { p.x[k] = fmaf(bt, dl[k], xl[k]); p.d[k] = dl[k]; }   // [R18]
-          p.path += bt; ph_set_panel(p, bp);
-          p.inv_mu = rcp_fast(mu_lookup(mu, T, 0, p.E).w);
-          st = ST_STEP;
-        }
+    if (phase == ST_NONE) break;                                      // nothing in flight, nothing parked, no source left
+
+    if (phase == ST_POP) {
+      // ------------------------------------------------ POP: idle lanes take a parked photon from pool T
+      const int r = __popc(m_pop & lt_mask);
+      if (st == ST_POP && r < cntT) {
+        pool_load(W.T, cntT - 1 - r, p, h);
+        if (p.ndraw & 3u) philox_block(p.ndraw >> 2);                 // the block is not parked
+        st = ((p.meta >> 11) & 1u) ? ST_PHANTOM : ST_STEP;
       }
+      cntT -= min(__popc(m_pop), cntT);
+      __syncwarp();
     } else if (phase == ST_STEP) {
       // ------------------------------------------------ STEP: Woodcock step, layer selection, lattice lookup [R19]
-      bool hit = false; float xg[3] = {0.f, 0.f, 0.f}; uint32_t hit_ids = 0;
+      bool hit = false, leave = false; float xg[3] = {0.f, 0.f, 0.f};
       if (st == ST_STEP) {
         const float s = -__logf(draw()) * p.inv_mu;
         float tf = INFINITY;
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {                                 // distance to the box exit [R32]
-          const float inv = rcp_fast(p.d[k] == 0.0f ? 1e-30f : p.d[k]);
-          tf = fminf(tf, ((p.d[k] >= 0.0f ? g.bhi[k] : g.blo[k]) - p.x[k]) * inv);
-        }
+        for (int k = 0; k < 3; ++k)                                   // distance to the box exit [R32]
+          tf = fminf(tf, ((p.d[k] >= 0.0f ? g.bhi[k] : g.blo[k]) - p.x[k]) * rcp_dir(p.d[k]));
         const int panel = ph_panel(p);
         if (s >= tf) {                                                // leaves the panel: back to the global frame [R33]
           tf = fmaxf(tf, 0.0f);
@@ -276,30 +335,37 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
           const float dl[3] = { p.d[0], p.d[1], p.d[2] };
           p.path += tf; if (HASH) hash_ev(h, EV_EXIT, (uint32_t)panel);
           point_to_global(g.pose[panel], xl, p.x); dir_to_global(g.pose[panel], dl, p.d);
-          st = ST_SEARCH;
+          leave = true; st = ST_POP;
         } else {
 #pragma unroll
           for (int k = 0; k < 3; ++k) p.x[k] = fmaf(s, p.d[k], p.x[k]);
           p.path += s;
-          uint32_t ids;                                               // depth -> layer -> crystal
+          uint32_t id;                                                // depth -> layer -> crystal
           const int mat = lattice_lookup(g, __float2int_rd(p.x[0] * kQ) + g.hWq, __float2int_rd(p.x[1] * kQ) + g.hHq,
-                                         __float2int_rd(p.x[2] * kQ), ids);
+                                         __float2int_rd(p.x[2] * kQ), id);
           if (mat < 0) { if (HASH) hash_ev(h, EV_STEP_VACUUM, 0); }
           else {
-            if (ids != kNone) ids |= (uint32_t)panel << 26;
+            if (id != kNone) id |= (uint32_t)panel << 26;
             const float4 m4 = mu_lookup(mu, T, mat, p.E);
             const float t = draw() * m4.w;                            // [R20] one draw picks the outcome
+            ids = id;
             if (t < m4.x) {                                           // photoelectric: deposit E, end
-              if (HASH) hash_ev(h, EV_PE, ids);
-              if (ids != kNone) { hit = true; hit_ids = ids; point_to_global(g.pose[panel], p.x, xg); }
-              finish();
-            } else if (t < m4.y) { p.ids = ids; st = ST_COMPTON; }
-            else if (t < m4.z) { p.ids = ids; st = ST_RAYLEIGH; }
-            else if (HASH) hash_ev(h, EV_VIRTUAL, ids);
+              if (HASH) { hash_ev(h, EV_PE, id); hash_out[2ull * p.pair + (p.meta & 1u)] = h; }
+              if (id != kNone) { hit = true; point_to_global(g.pose[panel], p.x, xg); }
+              st = ST_POP;
+            } else if (t < m4.y) st = ST_COMPTON;
+            else if (t < m4.z) st = ST_RAYLEIGH;
+            else if (HASH) hash_ev(h, EV_VIRTUAL, id);
           }
         }
       }
-      stage_hits(hit, hit_ids | ((p.meta & 1u) << 4) | ((p.meta >> 1) & 15u), xg, p.E, p.path * kInvC);
+      stage_hits(hit, ids | ((p.meta & 1u) << 4) | ((p.meta >> 1) & 15u), xg, p.E, p.path * kInvC);
+      const unsigned m_leave = __ballot_sync(0xFFFFFFFFu, leave);     // park the leavers for the next search
+      if (m_leave) {
+        if (leave) pool_store(W.S, cntS + __popc(m_leave & lt_mask), p, h);
+        cntS += __popc(m_leave);
+        __syncwarp();
+      }
     } else if (phase == ST_COMPTON) {
       // ------------------------------------------------ COMPTON: one Klein-Nishina trial per visit [R20]
       bool hit = false; float xg[3] = {0.f, 0.f, 0.f}, e_dep = 0.f;
@@ -329,32 +395,32 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
           const float dep = om * p.E, E2 = p.E - dep;
           const bool cut = E2 < kCutoff;                              // [R12]
           if (in_ph) {
-            if (HASH) hash_ev(h, EV_PH_COMPTON, 0);
-            if (cut) { if (HASH) hash_ev(h, EV_PH_CUTOFF, 0); finish(); }
-            else { p.E = E2; p.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, p.E).z); st = ST_PHANTOM; }
+            if (HASH) { hash_ev(h, EV_PH_COMPTON, 0); if (cut) hash_ev(h, EV_PH_CUTOFF, 0); }
+            if (!cut) { p.E = E2; p.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, p.E).z); st = ST_PHANTOM; }
           } else {
-            if (HASH) { hash_ev(h, EV_COMPTON, p.ids); if (cut) hash_ev(h, EV_CUTOFF, p.ids); }
-            if (p.ids != kNone) { hit = true; e_dep = cut ? p.E : dep; point_to_global(g.pose[ph_panel(p)], p.x, xg); }
-            if (cut) finish();
-            else { p.E = E2; p.inv_mu = rcp_fast(mu_lookup(mu, T, 0, p.E).w); st = ST_STEP; }
+            if (HASH) { hash_ev(h, EV_COMPTON, ids); if (cut) hash_ev(h, EV_CUTOFF, ids); }
+            if (ids != kNone) { hit = true; e_dep = cut ? p.E : dep; point_to_global(g.pose[ph_panel(p)], p.x, xg); }
+            if (!cut) { p.E = E2; p.inv_mu = rcp_fast(mu_lookup(mu, T, 0, p.E).w); st = ST_STEP; }
           }
+          if (cut) { if (HASH) hash_out[2ull * p.pair + (p.meta & 1u)] = h; st = ST_POP; }
         } else p.meta += 1u << 12;
       }
       const uint32_t seq = (p.meta >> 1) & 15u;
-      stage_hits(hit, p.ids | ((p.meta & 1u) << 4) | seq, xg, e_dep, p.path * kInvC);
+      stage_hits(hit, ids | ((p.meta & 1u) << 4) | seq, xg, e_dep, p.path * kInvC);
       if (hit && seq < 15u) p.meta += 2u;                             // [R9] 4-bit saturating hit counter
     } else if (phase == ST_RAYLEIGH) {
       // ------------------------------------------------ RAYLEIGH: Thomson pdf by closed-form inversion [R20]
       if (st == ST_RAYLEIGH) {
-        const float a = 4.0f * draw() - 2.0f, q = sqrtf(a * a + 1.0f);
-        const float ct = cbrtf(a + q) - cbrtf(q - a);
+        const float a = 4.0f * draw() - 2.0f, q2 = sqrtf(a * a + 1.0f);
+        const float ct = cbrtf(a + q2) - cbrtf(q2 - a);
         float sp, cp; sincos_2pi(draw(), sp, cp);
         rotate(p.d, ct, sqrtf(fmaxf(0.0f, 1.0f - ct * ct)), cp, sp);
         if ((p.meta >> 11) & 1u) { if (HASH) hash_ev(h, EV_PH_RAYLEIGH, 0); st = ST_PHANTOM; }
-        else { if (HASH) hash_ev(h, EV_RAYLEIGH, p.ids); st = ST_STEP; }
+        else { if (HASH) hash_ev(h, EV_RAYLEIGH, ids); st = ST_STEP; }
       }
-    } else if (phase == ST_PHANTOM) {
+    } else {
       // ------------------------------------------------ PHANTOM: Woodcock tracking in the voxel grid [R17]
+      bool leave = false;
       if (st == ST_PHANTOM) {
         const float s = -__logf(draw()) * p.inv_mu;
         int v[3]; bool out = false;
@@ -365,17 +431,23 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
           out = out || v[k] < 0 || v[k] >= src.dims[k];
         }
         p.path += s;
-        if (out) { if (HASH) hash_ev(h, EV_PH_LEAVE, 0); p.meta &= ~(1u << 11); st = ST_SEARCH; }
+        if (out) { if (HASH) hash_ev(h, EV_PH_LEAVE, 0); p.meta &= ~(1u << 11); leave = true; st = ST_POP; }
         else {
           const int mat = (int)src.phantom[((size_t)v[2] * src.dims[1] + v[1]) * src.dims[0] + v[0]] - 1;
           if (mat >= 0) {
             const float4 m4 = mu_lookup(mu, T, mat, p.E);
             const float t = draw() * mu_lookup(mu, T, src.ph_major, p.E).z;
-            if (t < m4.x) { if (HASH) hash_ev(h, EV_PH_ABSORBED, 0); finish(); }
+            if (t < m4.x) { if (HASH) { hash_ev(h, EV_PH_ABSORBED, 0); hash_out[2ull * p.pair + (p.meta & 1u)] = h; } st = ST_POP; }
             else if (t < m4.y) st = ST_COMPTON;
             else if (t < m4.z) st = ST_RAYLEIGH;
           }
         }
+      }
+      const unsigned m_leave = __ballot_sync(0xFFFFFFFFu, leave);
+      if (m_leave) {
+        if (leave) pool_store(W.S, cntS + __popc(m_leave & lt_mask), p, h);
+        cntS += __popc(m_leave);
+        __syncwarp();
       }
     }
   }
@@ -389,17 +461,18 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
   }
 }
 
-size_t transport_smem_bytes(const DevTables &T) {
-  return sizeof(Smem) - sizeof(float4) + sizeof(float4) * (size_t)T.n_materials * T.n_energies + 16;
+size_t transport_smem_bytes(const DevTables &T, bool hash) {
+  const size_t fixed = hash ? sizeof(Smem<true>) : sizeof(Smem<false>);
+  return fixed - sizeof(float4) + sizeof(float4) * (size_t)T.n_materials * T.n_energies + 16;
 }
 
 cudaError_t launch_transport(const DevGeom *geom, const DevTables &T, const float *maj, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
                              unsigned long long *work_counter, int sm_count, cudaStream_t stream) {
-  const size_t smem = transport_smem_bytes(T);
+  const size_t smem = transport_smem_bytes(T, hash_out != nullptr);
   const uint64_t n_photons = 2 * n_pairs;
   const uint64_t want = (n_photons + kThreads - 1) / kThreads;
-  static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : 4;
+  static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : 2;
   const uint64_t resident = (uint64_t)sm_count * ctas_per_sm;         // persistent grid
   const int blocks = (int)(want < resident ? (want ? want : 1) : resident);
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(unsigned long long), stream);

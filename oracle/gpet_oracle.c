@@ -91,7 +91,7 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-/* [R1] key = seed; counter = (history lo, history hi, stream, block); draw j = word j&3 of block j>>2 */
+/* [R1] key = seed; counter = (history lo, history hi, stream, block) */
 typedef struct { uint32_t key[2], ctr[4]; uint32_t ndraw; uint32_t blk[4]; } rng_t;
 enum { STREAM_SOURCE = 0, STREAM_A = 1, STREAM_B = 2, STREAM_DIGI = 3 };
 
@@ -103,13 +103,13 @@ static void rng_init(rng_t *r, uint64_t seed, uint64_t history, uint32_t stream)
 static uint32_t rng_word_at(rng_t *r, uint32_t j) {      /* random access (fixed slots, [R3]) */
   uint32_t b[4]; r->ctr[3] = j >> 2; orc_philox4x32_10(r->ctr, r->key, b); return b[j & 3];
 }
-static uint32_t rng_next_word(rng_t *r) {                /* sequential (transport, [R4]) */
-  if ((r->ndraw & 3u) == 0) { r->ctr[3] = r->ndraw >> 2; orc_philox4x32_10(r->ctr, r->key, r->blk); }
-  return r->blk[r->ndraw++ & 3u];
+/* [R4] transport streams are consumed one whole Philox block per event: u[0..3] of block number ndraw++ */
+static void rng_next_block(rng_t *r, double u[4]) {
+  r->ctr[3] = r->ndraw++; orc_philox4x32_10(r->ctr, r->key, r->blk);
+  for (int k = 0; k < 4; ++k) u[k] = ((double)(r->blk[k] >> 9) + 0.5) * (1.0 / 8388608.0);
 }
 /* [R2] u = ((x >> 9) + 0.5) * 2^-23, in (0,1): 2k+1 < 2^24, so exactly representable in fp32 and fp64 */
 double orc_uniform(uint32_t x) { return ((double)(x >> 9) + 0.5) * (1.0 / 8388608.0); }
-static double rng_next(rng_t *r) { return orc_uniform(rng_next_word(r)); }
 
 /* ------------------------------------------------------------------ geometry (quantised) */
 typedef struct { double o[3], u[3], v[3], w[3]; } panel_t;
@@ -336,11 +336,12 @@ static void azimuth(double u, double *c, double *s) { *c = cos(2.0 * ORC_PI * u)
 
 /* [R20] Klein-Nishina by composition-rejection (free electron).  Returns eps = E'/E, writes
  * cos(theta), sin^2(theta) and the number of trials.  3 draws per trial. */
-static double kn_sample(rng_t *r, double E, double *cos_t, double *sin2_t, int *trials) {
+static double kn_sample(rng_t *r, double E, double *cos_t, double *sin2_t, int *trials, double *u_azimuth) {
   double k = E / ORC_MEC2, e0 = 1.0 / (1.0 + 2.0 * k), a1 = -log(e0), a2 = 0.5 * (1.0 - e0 * e0);
   double eps = 1.0, t = 0.0;
   for (int n = 1; n <= ORC_KN_CAP; ++n) {
-    double ua = rng_next(r), ub = rng_next(r), uc = rng_next(r);
+    double u[4]; rng_next_block(r, u);                             /* [R4] one block per trial: u_a, u_b, u_c, azimuth */
+    double ua = u[0], ub = u[1], uc = u[2]; *u_azimuth = u[3];
     if (ua < a1 / (a1 + a2)) eps = exp(-a1 * ub);
     else eps = sqrt(e0 * e0 + (1.0 - e0 * e0) * ub);
     t = (1.0 - eps) / (k * eps);
@@ -352,7 +353,7 @@ static double kn_sample(rng_t *r, double E, double *cos_t, double *sin2_t, int *
   return eps;
 }
 int orc_kn_sample(uint64_t seed, uint64_t history, double E, double *eps, double *cos_t) {  /* test hook */
-  rng_t r; rng_init(&r, seed, history, STREAM_A); double s2; int n; *eps = kn_sample(&r, E, cos_t, &s2, &n); return n;
+  rng_t r; rng_init(&r, seed, history, STREAM_A); double s2, ua; int n; *eps = kn_sample(&r, E, cos_t, &s2, &n, &ua); return n;
 }
 /* [R20] Rayleigh with the Thomson pdf 3/8 (1 + cos^2), closed-form inversion of the cdf */
 double orc_rayleigh_cos(double u) { double a = 4.0 * u - 2.0, q = sqrt(a * a + 1.0); return cbrt(a + q) - cbrt(q - a); }
@@ -415,8 +416,8 @@ static void record_hit(ctx_t *c, uint64_t history, uint32_t ids, int photon, int
 
 /* Compton kinematics shared by phantom and detector: returns E' and rotates d */
 static double compton(ctx_t *c, rng_t *r, double E, double d[3]) {
-  double ct, s2; int n; double eps = kn_sample(r, E, &ct, &s2, &n); c->C->kn_trials += (uint64_t)n;
-  double cp, sp; azimuth(rng_next(r), &cp, &sp);
+  double ct, s2, ua; int n; double eps = kn_sample(r, E, &ct, &s2, &n, &ua); c->C->kn_trials += (uint64_t)n;
+  double cp, sp; azimuth(ua, &cp, &sp);
   orc_rotate(d, ct, sqrt(s2), cp, sp);
   return eps * E;
 }
@@ -431,7 +432,8 @@ static void transport_photon(ctx_t *c, uint64_t seed, uint64_t history, int phot
   if (in_phantom) {
     for (;;) {
       double mu_maj = mu_total(M, S->phantom_majorant, E);
-      double s = -log(rng_next(&r)) / mu_maj; c->C->ph_steps++;
+      double u[4]; rng_next_block(&r, u);                            /* [R4] free path, outcome, Rayleigh polar, azimuth */
+      double s = -log(u[0]) / mu_maj; c->C->ph_steps++;
       for (int k = 0; k < 3; ++k) x[k] += s * d[k];
       path += s;
       int v[3], out = 0;
@@ -439,14 +441,14 @@ static void transport_photon(ctx_t *c, uint64_t seed, uint64_t history, int phot
       if (out) { if (h) hash_ev(h, EV_PH_LEAVE, 0); break; }
       int mat = (int)S->phantom[((size_t)v[2] * S->dims[1] + v[1]) * S->dims[0] + v[0]] - 1;
       if (mat < 0) continue;                                        /* vacuum voxel: virtual, no draw */
-      mu3_t mu = mu_lookup(M, mat, E); double t = rng_next(&r) * mu_maj;
+      mu3_t mu = mu_lookup(M, mat, E); double t = u[1] * mu_maj;
       if (t < mu.pe) { c->C->ph_absorbed++; if (h) hash_ev(h, EV_PH_ABSORBED, 0); e_left = 0.0; goto done; }
       else if (t < mu.pe + mu.c) {
         E = compton(c, &r, E, d); c->C->ph_compton++; if (h) hash_ev(h, EV_PH_COMPTON, 0);
         if (E < ORC_CUTOFF) { c->C->ph_cutoff++; if (h) hash_ev(h, EV_PH_CUTOFF, 0); e_left = 0.0; goto done; }  /* [R28] */
         e_left = E;
       } else if (t < mu.pe + mu.c + mu.r) {
-        double ct = orc_rayleigh_cos(rng_next(&r)), cp, sp; azimuth(rng_next(&r), &cp, &sp);
+        double ct = orc_rayleigh_cos(u[2]), cp, sp; azimuth(u[3], &cp, &sp);
         orc_rotate(d, ct, sqrt(fmax(0.0, 1.0 - ct * ct)), cp, sp); if (h) hash_ev(h, EV_PH_RAYLEIGH, 0);
       }
     }
@@ -466,7 +468,8 @@ static void transport_photon(ctx_t *c, uint64_t seed, uint64_t history, int phot
     int alive = 1;
     for (;;) {                                                       /* [R19] whole-panel Woodcock    */
       double mu_maj = mu_majorant(M, c->det_mask, E);
-      double s = -log(rng_next(&r)) / mu_maj, tn, tf; c->C->steps++;
+      double u[4]; rng_next_block(&r, u);                            /* [R4] free path, outcome, Rayleigh polar, azimuth */
+      double s = -log(u[0]) / mu_maj, tn, tf; c->C->steps++;
       slab(blo, bhi, xl, dl, &tn, &tf);                              /* distance to the box exit      */
       if (s >= tf) {
         if (tf < 0.0) tf = 0.0;
@@ -479,7 +482,7 @@ static void transport_photon(ctx_t *c, uint64_t seed, uint64_t history, int phot
       int mat = lattice_lookup(g, p, (int64_t)floor(xl[0] * ORC_Q) + g->hWq, (int64_t)floor(xl[1] * ORC_Q) + g->hHq,
                                (int64_t)floor(xl[2] * ORC_Q), &ids);
       if (mat < 0) { c->C->step_vacuum++; if (h) hash_ev(h, EV_STEP_VACUUM, 0); continue; }
-      mu3_t mu = mu_lookup(M, mat, E); double t = rng_next(&r) * mu_maj;  /* [R20] one draw picks the outcome */
+      mu3_t mu = mu_lookup(M, mat, E); double t = u[1] * mu_maj;     /* [R20] one draw picks the outcome */
       if (t < mu.pe) {
         c->C->pe++; if (h) hash_ev(h, EV_PE, ids);
         if (ids != ORC_NONE) record_hit(c, history, ids, photon, &seq, P, xl, E, path);
@@ -494,7 +497,7 @@ static void transport_photon(ctx_t *c, uint64_t seed, uint64_t history, int phot
         if (ids != ORC_NONE) record_hit(c, history, ids, photon, &seq, P, xl, E - E2, path);
         E = E2; e_left = E;
       } else if (t < mu.pe + mu.c + mu.r) {
-        double ct = orc_rayleigh_cos(rng_next(&r)), cp, sp; azimuth(rng_next(&r), &cp, &sp);
+        double ct = orc_rayleigh_cos(u[2]), cp, sp; azimuth(u[3], &cp, &sp);
         orc_rotate(dl, ct, sqrt(fmax(0.0, 1.0 - ct * ct)), cp, sp);
         c->C->rayleigh++; if (h) hash_ev(h, EV_RAYLEIGH, ids);
       } else { c->C->virtuals++; if (h) hash_ev(h, EV_VIRTUAL, ids); }

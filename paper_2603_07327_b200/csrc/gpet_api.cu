@@ -5,6 +5,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <map>
 #include <mutex>
 #include <vector>
 
@@ -20,10 +21,9 @@ struct gpet_geometry {
 };
 struct gpet_materials {
   int n_materials = 0, n_energies = 0; float e_min = 0, e_step = 0;
-  std::vector<float> mu_tot;            // host [n_materials][n_energies] (fp32 sums as staged)
-  float4 *dev_mu = nullptr;
+  std::vector<float4> mu;               // host [n_materials][n_energies]: {mu_pe, mu_pe+mu_C, mu_tot, 0} [R11]
   std::mutex lock;
-  float *dev_maj[256] = {};             // lazily built majorant tables per material mask (n <= 8 materials)
+  std::map<uint32_t, float4 *> staged;  // device tables per (detector mask << 8 | staged mask), built lazily
 };
 struct gpet_activity {
   int dims[3]; uint32_t n_active = 0; uint64_t w_total = 0;
@@ -161,43 +161,52 @@ extern "C" int gpet_materials_load(int32_t n_materials, int32_t n_energies, floa
   if (n_materials < 1 || n_materials > GPET_MAX_MATERIALS) return fail(GPET_E_TABLE, "n_materials %d outside 1..%d", n_materials, GPET_MAX_MATERIALS);
   if (n_energies < 2 || !(e_step > 0.0f)) return fail(GPET_E_TABLE, "need >= 2 energies and a positive step");
   const size_t n = (size_t)n_materials * n_energies;
-  std::vector<float4> mu(n);
   gpet_materials *m = new gpet_materials;
-  m->n_materials = n_materials; m->n_energies = n_energies; m->e_min = e_min; m->e_step = e_step; m->mu_tot.resize(n);
+  m->n_materials = n_materials; m->n_energies = n_energies; m->e_min = e_min; m->e_step = e_step; m->mu.resize(n);
   for (size_t i = 0; i < n; ++i) {
     if (!(mu_pe[i] >= 0.0f) || !(mu_c[i] >= 0.0f) || !(mu_r[i] >= 0.0f) || !std::isfinite(mu_pe[i] + mu_c[i] + mu_r[i])) {
       delete m; return fail(GPET_E_TABLE, "negative or non-finite mu at flat index %zu", i);
     }
     // cumulative sums formed in double, rounded to fp32 once [R11]
-    mu[i] = make_float4(mu_pe[i], (float)((double)mu_pe[i] + mu_c[i]), (float)((double)mu_pe[i] + mu_c[i] + mu_r[i]), 0.0f);
-    m->mu_tot[i] = mu[i].z;
+    m->mu[i] = make_float4(mu_pe[i], (float)((double)mu_pe[i] + mu_c[i]), (float)((double)mu_pe[i] + mu_c[i] + mu_r[i]), 0.0f);
   }
-  cudaError_t e = cudaMalloc(&m->dev_mu, sizeof(float4) * n);
-  if (e == cudaSuccess) e = cudaMemcpy(m->dev_mu, mu.data(), sizeof(float4) * n, cudaMemcpyHostToDevice);
-  if (e != cudaSuccess) { delete m; return fail(GPET_E_CUDA, "gpet_materials_load: %s", cudaGetErrorString(e)); }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { delete m; return fail(GPET_E_CUDA, "gpet_materials_load: no CUDA device"); }
   *out = m; return GPET_OK;
 }
 
 extern "C" int gpet_materials_destroy(gpet_materials *m) {
   if (!m) return GPET_OK;
-  if (m->dev_mu) cudaFree(m->dev_mu);
-  for (float *p : m->dev_maj) if (p) cudaFree(p);
+  for (auto &kv : m->staged) if (kv.second) cudaFree(kv.second);
   delete m; return GPET_OK;
 }
 
-// [R19] majorant table of a material set: pointwise max of mu_tot over the set
-static int majorant_table(gpet_materials *m, uint32_t mask, const float **out) {
-  mask &= (1u << m->n_materials) - 1u;
-  if (!mask) return fail(GPET_E_INVALID_ARG, "geometry references no loaded material");
+// Device table for one run: the materials in `stage_mask`, interleaved float4 per energy with the detector
+// majorant [R19] (pointwise max of mu_tot over `det_mask`) in .w; `matmap` gives each material's staged slot.
+static int staged_table(gpet_materials *m, uint32_t det_mask, uint32_t stage_mask, DevTables *T) {
+  const uint32_t all = (1u << m->n_materials) - 1u;
+  det_mask &= all; stage_mask = (stage_mask | det_mask) & all;
+  if (!det_mask) return fail(GPET_E_INVALID_ARG, "geometry references no loaded material");
+  T->n_energies = m->n_energies; T->e_min = m->e_min; T->inv_step = 1.0f / m->e_step; T->matmap = 0; T->n_staged = 0;
+  for (int k = 0; k < m->n_materials; ++k) if (stage_mask >> k & 1u) T->matmap |= (uint32_t)(T->n_staged++) << (4 * k);
   std::lock_guard<std::mutex> lk(m->lock);
-  if (!m->dev_maj[mask]) {
-    std::vector<float> maj(m->n_energies, 0.0f);
-    for (int k = 0; k < m->n_materials; ++k) if (mask >> k & 1u)
-      for (int i = 0; i < m->n_energies; ++i) maj[i] = fmaxf(maj[i], m->mu_tot[(size_t)k * m->n_energies + i]);
-    CUDA_TRY(cudaMalloc(&m->dev_maj[mask], sizeof(float) * m->n_energies));
-    CUDA_TRY(cudaMemcpy(m->dev_maj[mask], maj.data(), sizeof(float) * m->n_energies, cudaMemcpyHostToDevice));
+  float4 *&dev = m->staged[det_mask << 8 | stage_mask];
+  if (!dev) {
+    const int ne = m->n_energies;
+    std::vector<float4> tab((size_t)T->n_staged * ne);
+    int slot = 0;
+    for (int k = 0; k < m->n_materials; ++k) if (stage_mask >> k & 1u) {
+      for (int i = 0; i < ne; ++i) {
+        float4 v = m->mu[(size_t)k * ne + i]; v.w = 0.0f;
+        for (int q = 0; q < m->n_materials; ++q) if (det_mask >> q & 1u) v.w = fmaxf(v.w, m->mu[(size_t)q * ne + i].z);
+        tab[(size_t)slot * ne + i] = v;
+      }
+      ++slot;
+    }
+    CUDA_TRY(cudaMalloc(&dev, sizeof(float4) * tab.size()));
+    CUDA_TRY(cudaMemcpy(dev, tab.data(), sizeof(float4) * tab.size(), cudaMemcpyHostToDevice));
   }
-  *out = m->dev_maj[mask]; return GPET_OK;
+  T->mu = dev; return GPET_OK;
 }
 
 // ---------------------------------------------------------------- activity map [R13]
@@ -285,10 +294,11 @@ extern "C" int gpet_simulate(const gpet_geometry *g, const gpet_materials *m, co
       return fail(GPET_E_INVALID_ARG, "layer %d references a material that is not loaded", l);
   DevSource D; int rc = make_source(src, m, &D); if (rc) return rc;
   rc = geometry_upload(const_cast<gpet_geometry *>(g)); if (rc) return rc;
-  const float *maj = nullptr; rc = majorant_table(const_cast<gpet_materials *>(m), g->host.det_mask, &maj); if (rc) return rc;
-  DevTables T = { m->n_materials, m->n_energies, m->e_min, 1.0f / m->e_step, m->dev_mu };
+  // a phantom may hold any loaded material (its map lives on the device): stage them all in that case
+  const uint32_t stage_mask = (D.kind == 1 && D.phantom) ? (1u << m->n_materials) - 1u : 0u;
+  DevTables T; rc = staged_table(const_cast<gpet_materials *>(m), g->host.det_mask, stage_mask, &T); if (rc) return rc;
   unsigned long long *wc = nullptr; rc = next_work_counter(&wc); if (rc) return rc;
-  CUDA_TRY(launch_transport(g->dev, T, maj, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
+  CUDA_TRY(launch_transport(g->dev, T, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
   return GPET_OK;
 }
 

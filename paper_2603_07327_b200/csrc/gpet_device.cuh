@@ -35,10 +35,11 @@ struct DevGeom {
   float pose[kMaxPanels][12]; // front-face centre, u, v, w
 };
 
-struct DevTables {            // [R11] per material, per energy: {mu_pe, mu_pe+mu_C, mu_tot, unused}
-  int n_materials, n_energies;
+struct DevTables {            // [R11] per staged material, per energy: {mu_pe, mu_pe+mu_C, mu_tot, detector majorant}
+  int n_staged, n_energies;   // only the materials a run can touch are staged into shared memory
   float e_min, inv_step;
-  const float4 *mu;           // [n_materials][n_energies]
+  uint32_t matmap;            // 4 bits per material id: its staged slot
+  const float4 *mu;           // [n_staged][n_energies]
 };
 
 // ---------------------------------------------------------------- [R1] Philox4x32-10
@@ -54,22 +55,6 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
 }
 // [R2] u = ((x >> 9) + 0.5) * 2^-23: every step is exact in fp32
 __device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 9) + 0.5f) * 1.1920928955078125e-7f; }
-
-// Sequential per-photon stream [R4]: draw j = word j&3 of block j>>2
-struct Stream {
-  uint2 key; uint32_t h_lo, h_hi, stream, ndraw; uint4 blk;
-  __device__ __forceinline__ void init(uint64_t seed, uint64_t history, uint32_t s) {
-    key = make_uint2((uint32_t)seed, (uint32_t)(seed >> 32));
-    h_lo = (uint32_t)history; h_hi = (uint32_t)(history >> 32); stream = s; ndraw = 0;
-  }
-  __device__ __forceinline__ float next() {
-    const uint32_t j = ndraw & 3u;
-    if (j == 0) blk = philox4x32_10(make_uint4(h_lo, h_hi, stream, ndraw >> 2), key);
-    ++ndraw;
-    const uint32_t w = j == 0 ? blk.x : (j == 1 ? blk.y : (j == 2 ? blk.z : blk.w));
-    return u01(w);
-  }
-};
 
 // ---------------------------------------------------------------- [R7] lattice lookup
 // exact floor division of a Q coordinate by a Q pitch: float reciprocal estimate + integer fix-up
@@ -105,22 +90,6 @@ __device__ __forceinline__ int lattice_lookup(const DevGeom &g, int qa, int qb, 
   if (!in) return L.gmat;
   ids = ((uint32_t)(mx + g.nmod[0] * my) << 20) | ((uint32_t)l << 18) | ((uint32_t)(ix + L.n[0] * iy) << 5);
   return L.cmat;
-}
-
-// ---------------------------------------------------------------- [R6] slab test
-// Ray x + t d against the box [lo, hi]; returns false if an axis with zero direction lies outside.
-__device__ __forceinline__ bool slab(const float lo[3], const float hi[3], const float x[3], const float d[3],
-                                     float &tn, float &tf) {
-  tn = -INFINITY; tf = INFINITY;
-  bool ok = true;
-#pragma unroll
-  for (int k = 0; k < 3; ++k) {
-    if (d[k] == 0.0f) { ok = ok && !(x[k] < lo[k] || x[k] >= hi[k]); continue; }
-    const float inv = 1.0f / d[k];
-    const float t1 = (lo[k] - x[k]) * inv, t2 = (hi[k] - x[k]) * inv;
-    tn = fmaxf(tn, fminf(t1, t2)); tf = fminf(tf, fmaxf(t1, t2));
-  }
-  return ok;
 }
 
 // PAPER.md:33 global -> local

@@ -23,15 +23,17 @@ namespace gpet {
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 constexpr int kStage = 64;            // staged hits per warp (ring buffer)
-constexpr int kPoolT = 64;            // photons waiting for in-panel transport (filled while < 32)
-constexpr int kPoolS = 96;            // photons waiting for a panel search (drained when >= 32; bound: DESIGN.md 5)
+constexpr int kPool = 96;             // parked photons per warp: stack T (await transport) grows from slot 0,
+                                      // stack S (await a panel search) from the top; lanes + parked <= kPool
+constexpr int kLowT = 24;             // GENERATE when fewer photons than this await transport ...
+constexpr int kHighS = 16;            // ... or at least this many await a search
 constexpr uint32_t kChunk = 1024;     // photon indices a warp reserves at a time
 
-enum : int { ST_POP = 0, ST_STEP = 1, ST_COMPTON = 2, ST_RAYLEIGH = 3, ST_PHANTOM = 4, ST_NONE = 5 };
+enum : int { ST_POP = 0, ST_STEP = 1, ST_COMPTON = 2, ST_PHANTOM = 3, ST_NONE = 4 };
 
 struct HitStage { uint32_t w[7][kStage]; };      // history, ids, x, y, z, e, tof
 
-// 48 bytes per parked photon; the Philox block is not parked (it is regenerated on demand)
+// 48 bytes per parked photon (no RNG state: a stream is addressed by its block counter [R4])
 template <int N, bool HASH> struct Pool {
   float4 a[N];                         // x, y, z, dx
   float4 b[N];                         // dy, dz, E, path
@@ -39,12 +41,12 @@ template <int N, bool HASH> struct Pool {
   uint2 hh[HASH ? N : 1];              // outcome hash (parity builds only)
 };
 
-template <bool HASH> struct WarpMem { Pool<kPoolT, HASH> T; Pool<kPoolS, HASH> S; HitStage stage; };
+template <bool HASH> struct WarpMem { Pool<kPool, HASH> pool; HitStage stage; };
 
 template <bool HASH> struct Smem {
   DevGeom g;
   WarpMem<HASH> w[kWarps];
-  float4 mu[1];                        // [n_materials][n_energies], .w = detector majorant
+  float4 mu[1];                        // [n_staged][n_energies], .w = detector majorant
 };
 
 // ---------------------------------------------------------------- fast math with bounded error
@@ -52,6 +54,14 @@ __device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ft
 __device__ __forceinline__ float sqrt_fast(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 // 1/d with a zero component treated as +tiny: an inside point then sees (-inf, +inf), an outside one misses [R32]
 __device__ __forceinline__ float rcp_dir(float d) { return rcp_fast(d == 0.0f ? 1e-30f : d); }
+// (sin, cos) of a small angle (acolinearity, ~4e-3 rad): Taylor to x^7 / x^8 below 0.25 rad (error < 1e-9)
+__device__ __forceinline__ void sincos_small(float x, float &s, float &c) {
+  if (x < 0.25f) {
+    const float x2 = x * x;
+    s = x * fmaf(x2, fmaf(x2, fmaf(x2, -1.984126984e-4f, 8.333333333e-3f), -0.1666666667f), 1.0f);
+    c = fmaf(x2, fmaf(x2, fmaf(x2, fmaf(x2, 2.48015873e-5f, -1.388888889e-3f), 4.166666667e-2f), -0.5f), 1.0f);
+  } else sincosf(x, &s, &c);
+}
 // (sin, cos)(2 pi u), u in (0,1): argument folded to [-pi, pi] where sin.approx / cos.approx are good to 2^-21
 __device__ __forceinline__ void sincos_2pi(float u, float &s, float &c) {
   const float a = 6.283185307179586f * (u - 0.5f);
@@ -63,7 +73,8 @@ __device__ __forceinline__ float4 mu_lookup(const float4 *mu, const DevTables &T
   const float x = (E - T.e_min) * T.inv_step;
   int i = min(__float2int_rd(x), T.n_energies - 2); i = max(i, 0);
   const float f = x - (float)i;
-  const float4 a = mu[m * T.n_energies + i], b = mu[m * T.n_energies + i + 1];
+  const int row = ((T.matmap >> (4 * m)) & 15u) * T.n_energies + i;           // staged slot of material m
+  const float4 a = mu[row], b = mu[row + 1];
   return make_float4(fmaf(f, b.x - a.x, a.x), fmaf(f, b.y - a.y, a.y), fmaf(f, b.z - a.z, a.z), fmaf(f, b.w - a.w, a.w));
 }
 
@@ -74,7 +85,7 @@ struct Photon {
   uint32_t pair;           // history - first_history
   uint32_t meta;           // bit0 photon, bits1-4 seq, bits5-10 panel (current, or just left; 63 = none),
                            // bit11 in phantom, bits12+ Klein-Nishina trial counter
-  uint32_t ndraw;          // draws consumed from this photon's stream [R4]
+  uint32_t ndraw;          // Philox blocks consumed from this photon's stream [R4]
 };
 __device__ __forceinline__ int ph_panel(const Photon &p) { return (p.meta >> 5) & 63u; }
 __device__ __forceinline__ void ph_set_panel(Photon &p, int panel) { p.meta = (p.meta & ~(63u << 5)) | ((uint32_t)panel << 5); }
@@ -101,6 +112,32 @@ __device__ __forceinline__ void store_hit(const HitBuf &H, unsigned long long o,
     H.x[o] = __uint_as_float(stage.w[2][slot]); H.y[o] = __uint_as_float(stage.w[3][slot]); H.z[o] = __uint_as_float(stage.w[4][slot]);
     H.e[o] = __uint_as_float(stage.w[5][slot]); H.tof[o] = __uint_as_float(stage.w[6][slot]);
   }
+}
+
+// [R20] Rayleigh: Thomson pdf by closed-form inversion of the cdf, then a rotation about d
+__device__ __noinline__ float3 rayleigh_dir(float dx, float dy, float dz, float u_polar, float u_azimuth) {
+  const float a = 4.0f * u_polar - 2.0f, q = sqrtf(a * a + 1.0f);
+  const float ct = cbrtf(a + q) - cbrtf(q - a);
+  float sp, cp; sincos_2pi(u_azimuth, sp, cp);
+  float d[3] = { dx, dy, dz };
+  rotate(d, ct, sqrtf(fmaxf(0.0f, 1.0f - ct * ct)), cp, sp);
+  return make_float3(d[0], d[1], d[2]);
+}
+__device__ __forceinline__ void rayleigh(float d[3], float u_polar, float u_azimuth) {
+  const float3 r = rayleigh_dir(d[0], d[1], d[2], u_polar, u_azimuth);
+  d[0] = r.x; d[1] = r.y; d[2] = r.z;
+}
+
+// [R13] decay site from the activity map: voxel by the integer cdf (word 0), uniform point inside (words 1-3)
+__device__ __forceinline__ void decay_site(const DevSource &src, uint4 w, float x[3]) {
+  const uint64_t Wl = src.w_total & 0xFFFFFFFFull, Wh = src.w_total >> 32;          // floor(w.x * W / 2^32), exact
+  const uint64_t target = (uint64_t)w.x * Wh + (((uint64_t)w.x * Wl) >> 32);
+  uint32_t lo = 0, hi = src.n_active - 1;
+  while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (src.act_cdf[mid] > target) hi = mid; else lo = mid + 1; }
+  const uint32_t vi = src.act_index[lo], nx = (uint32_t)src.dims[0], ny = (uint32_t)src.dims[1];
+  x[0] = src.origin[0] + ((float)(vi % nx) + u01(w.y)) * src.voxel[0];
+  x[1] = src.origin[1] + ((float)((vi / nx) % ny) + u01(w.z)) * src.voxel[1];
+  x[2] = src.origin[2] + ((float)(vi / (nx * ny)) + u01(w.w)) * src.voxel[2];
 }
 
 // ---------------------------------------------------------------- [R6] panel search
@@ -145,8 +182,8 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
 
 // ---------------------------------------------------------------- the kernel
 template <bool HASH>
-__global__ void __launch_bounds__(kThreads, 2)
-transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, DevSource src, uint64_t first_history, uint64_t n_photons,
+__global__ void __launch_bounds__(kThreads, 3)
+transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint64_t first_history, uint64_t n_photons,
                            uint64_t seed, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem<HASH> *S = reinterpret_cast<Smem<HASH> *>(smem_raw);
@@ -154,8 +191,8 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
     const uint32_t *gs = reinterpret_cast<const uint32_t *>(geom);
     uint32_t *gd = reinterpret_cast<uint32_t *>(&S->g);
     for (int i = threadIdx.x; i < (int)(sizeof(DevGeom) / 4); i += kThreads) gd[i] = gs[i];
-    const int n = T.n_materials * T.n_energies;
-    for (int i = threadIdx.x; i < n; i += kThreads) { float4 v = T.mu[i]; v.w = maj[i % T.n_energies]; S->mu[i] = v; }
+    const int n = T.n_staged * T.n_energies;
+    for (int i = threadIdx.x; i < n; i += kThreads) S->mu[i] = T.mu[i];
     __syncthreads();
   }
   const DevGeom &g = S->g;
@@ -170,25 +207,18 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
   Photon p; p.meta = 0; p.ndraw = 0; p.E = 0.f; p.path = 0.f; p.inv_mu = 0.f; p.pair = 0;
 #pragma unroll
   for (int k = 0; k < 3; ++k) { p.x[k] = 0.f; p.d[k] = 0.f; }
-  uint4 blk = make_uint4(0, 0, 0, 0);      // current Philox block of the lane's photon
   uint32_t ids = kNone;                    // lattice result of the pending interaction
   uint64_t h = 0;
   int st = ST_POP;
   uint64_t w_next = 0, w_end = 0;          // this warp's reserved photon indices [w_next, w_end)
   bool exhausted = false;                  // the global counter ran past n_photons
   uint32_t stage_head = 0, stage_cnt = 0;  // ring buffer of staged hits (warp-uniform)
-  int cntT = 0, cntS = 0;                  // pool fill levels (warp-uniform)
+  int cntT = 0, cntS = 0;                  // pool fill levels (warp-uniform): T grows from slot 0, S from the top
 
-  auto philox_block = [&](uint32_t block) {
+  // [R4] every transport event consumes one whole Philox block of the photon's stream
+  auto next_block = [&]() -> uint4 {
     const uint64_t history = first_history + p.pair;
-    blk = philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 1u + (p.meta & 1u), block), key);
-  };
-  // next uniform of this photon's stream [R4]
-  auto draw = [&]() -> float {
-    const uint32_t j = p.ndraw & 3u;
-    if (j == 0) philox_block(p.ndraw >> 2);
-    ++p.ndraw;
-    return u01(j == 0 ? blk.x : (j == 1 ? blk.y : (j == 2 ? blk.z : blk.w)));
+    return philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 1u + (p.meta & 1u), p.ndraw++), key);
   };
   // stage one hit per lane that has one; flush 32 staged hits with one atomic + coalesced stores (S10)
   auto stage_hits = [&](bool has, uint32_t hit_ids, const float xg[3], float e, float tof) {
@@ -211,19 +241,31 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
       __syncwarp();
     }
   };
+  // park the lanes' photons that left their panel / the phantom: they wait in pool S for the next search
+  auto park_leavers = [&](bool leave) {
+    const unsigned m_leave = __ballot_sync(0xFFFFFFFFu, leave);
+    if (m_leave == 0) return;
+    if (leave) pool_store(W.pool, kPool - 1 - (cntS + __popc(m_leave & lt_mask)), p, h);
+    cntS += __popc(m_leave);
+    __syncwarp();
+  };
 
 #pragma unroll 1
   for (;;) {
     const bool more_src = !exhausted || w_next < w_end;
-    if ((cntT < 32 && (more_src || cntS > 0)) || (cntT <= 32 && cntS >= 32)) {
-      // ================================================ GENERATE: 32 photons that need a panel search
+    const unsigned m_pop = __ballot_sync(0xFFFFFFFFu, st == ST_POP);
+    if ((cntT < kLowT && (more_src || cntS > 0)) || cntS >= kHighS) {
+      // ================================================ GENERATE: up to 32 photons that need a panel search
+      // The photons a warp holds (in lanes + parked) never exceed kPool: fresh ones are admitted only while
+      // there is room, so the two stacks sharing the pool cannot collide.
       const int nS = min(cntS, 32);                                   // lanes [0, nS): photons that left a panel
+      const int room = kPool - (cntT + cntS + 32 - __popc(m_pop));
+      const int nF = max(0, min(32 - nS, room));                      // lanes [nS, nS + nF): new photons
       Photon q; uint64_t hq = 0; bool active = lane < nS;
-      if (active) pool_load(W.S, cntS - 1 - lane, q, hq);
+      if (active) pool_load(W.pool, kPool - 1 - (cntS - 1 - lane), q, hq);
       cntS -= nS;
       __syncwarp();
-      // lanes [nS, 32): new photons from the source (S3) [R13-R15]
-      if (nS < 32) {
+      if (nF > 0) {                                                   // source sampling (S3) [R13-R15]
         if (w_next >= w_end && !exhausted) {
           unsigned long long b = 0;
           if (lane == 0) b = atomicAdd(work_counter, (unsigned long long)kChunk);
@@ -232,8 +274,8 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
           else { w_next = b; w_end = min((uint64_t)(b + kChunk), n_photons); }
         }
         const uint64_t j = w_next + (uint64_t)(lane - nS);
-        const bool fresh = lane >= nS && j < w_end;
-        w_next = min(w_next + (uint64_t)(32 - nS), w_end);
+        const bool fresh = lane >= nS && lane < nS + nF && j < w_end;
+        w_next = min(w_next + (uint64_t)nF, w_end);
         if (fresh) {
           active = true;
           q.pair = (uint32_t)(j >> 1); q.meta = (uint32_t)(j & 1u) | (63u << 5); q.ndraw = 0; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
@@ -241,17 +283,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
           const uint64_t history = first_history + q.pair;
           const uint32_t h_lo = (uint32_t)history, h_hi = (uint32_t)(history >> 32);
           q.x[0] = src.pos[0]; q.x[1] = src.pos[1]; q.x[2] = src.pos[2];
-          if (src.kind == 1) {
-            const uint4 w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 0u), key);
-            const uint64_t Wl = src.w_total & 0xFFFFFFFFull, Wh = src.w_total >> 32;          // floor(w.x * W / 2^32), exact
-            const uint64_t target = (uint64_t)w.x * Wh + (((uint64_t)w.x * Wl) >> 32);
-            uint32_t lo = 0, hi = src.n_active - 1;
-            while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (src.act_cdf[mid] > target) hi = mid; else lo = mid + 1; }
-            const uint32_t vi = src.act_index[lo], nx = (uint32_t)src.dims[0], ny = (uint32_t)src.dims[1];
-            q.x[0] = src.origin[0] + ((float)(vi % nx) + u01(w.y)) * src.voxel[0];
-            q.x[1] = src.origin[1] + ((float)((vi / nx) % ny) + u01(w.z)) * src.voxel[1];
-            q.x[2] = src.origin[2] + ((float)(vi / (nx * ny)) + u01(w.w)) * src.voxel[2];
-          }
+          if (src.kind == 1) decay_site(src, philox4x32_10(make_uint4(h_lo, h_hi, 0u, 0u), key), q.x);
           const uint4 w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 1u), key);
           if (src.kind == 2) { q.d[0] = src.beam[0]; q.d[1] = src.beam[1]; q.d[2] = src.beam[2]; }
           else {
@@ -262,8 +294,8 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
           if (q.meta & 1u) {                                          // photon B: opposite, plus acolinearity
             q.d[0] = -q.d[0]; q.d[1] = -q.d[1]; q.d[2] = -q.d[2];
             if (src.acol_sigma > 0.0f) {
-              const float rho = src.acol_sigma * sqrtf(-2.0f * logf(u01(w.z)));
-              float sr, cr; sincosf(rho, &sr, &cr);
+              const float rho = src.acol_sigma * sqrt_fast(-2.0f * __logf(u01(w.z)));
+              float sr, cr; sincos_small(rho, sr, cr);
               float sp, cp; sincospif(2.0f * u01(w.w), &sp, &cp);
               rotate(q.d, cr, sr, cp, sp);
             }
@@ -291,30 +323,25 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
         }
       }
       const unsigned m_park = __ballot_sync(0xFFFFFFFFu, park);
-      if (park) pool_store(W.T, cntT + __popc(m_park & lt_mask), q, hq);
+      if (park) pool_store(W.pool, cntT + __popc(m_park & lt_mask), q, hq);
       cntT += __popc(m_park);
       __syncwarp();
       continue;
     }
     // ================================================ TRANSPORT: run the phase most lanes are waiting for
-    const unsigned m_pop = __ballot_sync(0xFFFFFFFFu, st == ST_POP);
     int phase = ST_NONE, best = min(__popc(m_pop), cntT);
     if (best) phase = ST_POP;
-    if (!(best && cntS >= 32)) {                                      // pool S nearly full: refilling lanes comes first
-      int c;
+    { int c;
       c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_STEP));     if (c > best) { best = c; phase = ST_STEP; }
       c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_COMPTON));  if (c > best) { best = c; phase = ST_COMPTON; }
-      c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_PHANTOM));  if (c > best) { best = c; phase = ST_PHANTOM; }
-      c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_RAYLEIGH)); if (c > best) { best = c; phase = ST_RAYLEIGH; }
-    }
+      c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_PHANTOM));  if (c > best) { best = c; phase = ST_PHANTOM; } }
     if (phase == ST_NONE) break;                                      // nothing in flight, nothing parked, no source left
 
     if (phase == ST_POP) {
       // ------------------------------------------------ POP: idle lanes take a parked photon from pool T
       const int r = __popc(m_pop & lt_mask);
       if (st == ST_POP && r < cntT) {
-        pool_load(W.T, cntT - 1 - r, p, h);
-        if (p.ndraw & 3u) philox_block(p.ndraw >> 2);                 // the block is not parked
+        pool_load(W.pool, cntT - 1 - r, p, h);
         st = ((p.meta >> 11) & 1u) ? ST_PHANTOM : ST_STEP;
       }
       cntT -= min(__popc(m_pop), cntT);
@@ -323,7 +350,8 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
       // ------------------------------------------------ STEP: Woodcock step, layer selection, lattice lookup [R19]
       bool hit = false, leave = false; float xg[3] = {0.f, 0.f, 0.f};
       if (st == ST_STEP) {
-        const float s = -__logf(draw()) * p.inv_mu;
+        const uint4 w = next_block();                                 // [R4] free path, outcome, Rayleigh polar + azimuth
+        const float s = -__logf(u01(w.x)) * p.inv_mu;
         float tf = INFINITY;
 #pragma unroll
         for (int k = 0; k < 3; ++k)                                   // distance to the box exit [R32]
@@ -347,25 +375,20 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
           else {
             if (id != kNone) id |= (uint32_t)panel << 26;
             const float4 m4 = mu_lookup(mu, T, mat, p.E);
-            const float t = draw() * m4.w;                            // [R20] one draw picks the outcome
+            const float t = u01(w.y) * m4.w;                          // [R20] one draw picks the outcome
             ids = id;
             if (t < m4.x) {                                           // photoelectric: deposit E, end
               if (HASH) { hash_ev(h, EV_PE, id); hash_out[2ull * p.pair + (p.meta & 1u)] = h; }
               if (id != kNone) { hit = true; point_to_global(g.pose[panel], p.x, xg); }
               st = ST_POP;
             } else if (t < m4.y) st = ST_COMPTON;
-            else if (t < m4.z) st = ST_RAYLEIGH;
+            else if (t < m4.z) { rayleigh(p.d, u01(w.z), u01(w.w)); if (HASH) hash_ev(h, EV_RAYLEIGH, id); }
             else if (HASH) hash_ev(h, EV_VIRTUAL, id);
           }
         }
       }
       stage_hits(hit, ids | ((p.meta & 1u) << 4) | ((p.meta >> 1) & 15u), xg, p.E, p.path * kInvC);
-      const unsigned m_leave = __ballot_sync(0xFFFFFFFFu, leave);     // park the leavers for the next search
-      if (m_leave) {
-        if (leave) pool_store(W.S, cntS + __popc(m_leave & lt_mask), p, h);
-        cntS += __popc(m_leave);
-        __syncwarp();
-      }
+      park_leavers(leave);
     } else if (phase == ST_COMPTON) {
       // ------------------------------------------------ COMPTON: one Klein-Nishina trial per visit [R20]
       bool hit = false; float xg[3] = {0.f, 0.f, 0.f}, e_dep = 0.f;
@@ -373,7 +396,8 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
         const bool in_ph = (p.meta >> 11) & 1u;
         const float k = p.E * (1.0f / kMec2), e0 = rcp_fast(1.0f + 2.0f * k), e02 = e0 * e0;
         const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
-        const float ua = draw(), ub = draw(), uc = draw();
+        const uint4 w = next_block();                                 // [R4] u_a, u_b, u_c, azimuth
+        const float ua = u01(w.x), ub = u01(w.y), uc = u01(w.z);
         // om = 1 - eps and em = eps - eps0 are formed without cancellation, so that sin^2 = t (2 - t) keeps
         // full relative accuracy at both poles (t = om/(k eps), 2 - t = em/(eps0 k eps)); plain fp32 loses
         // 3-4 digits of small scattering angles and moves later hits by micrometres
@@ -390,7 +414,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
         const float gr = 1.0f - eps * t * tm * rcp_fast(1.0f + eps * eps);
         if (gr >= uc || (p.meta >> 12) >= 63u) {                      // accepted [R22: the 64th trial always is]
           p.meta &= 0xFFFu;
-          float sp, cp; sincos_2pi(draw(), sp, cp);
+          float sp, cp; sincos_2pi(u01(w.w), sp, cp);
           rotate(p.d, 1.0f - t, sqrt_fast(fmaxf(t * tm, 0.0f)), cp, sp);
           const float dep = om * p.E, E2 = p.E - dep;
           const bool cut = E2 < kCutoff;                              // [R12]
@@ -408,21 +432,12 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
       const uint32_t seq = (p.meta >> 1) & 15u;
       stage_hits(hit, ids | ((p.meta & 1u) << 4) | seq, xg, e_dep, p.path * kInvC);
       if (hit && seq < 15u) p.meta += 2u;                             // [R9] 4-bit saturating hit counter
-    } else if (phase == ST_RAYLEIGH) {
-      // ------------------------------------------------ RAYLEIGH: Thomson pdf by closed-form inversion [R20]
-      if (st == ST_RAYLEIGH) {
-        const float a = 4.0f * draw() - 2.0f, q2 = sqrtf(a * a + 1.0f);
-        const float ct = cbrtf(a + q2) - cbrtf(q2 - a);
-        float sp, cp; sincos_2pi(draw(), sp, cp);
-        rotate(p.d, ct, sqrtf(fmaxf(0.0f, 1.0f - ct * ct)), cp, sp);
-        if ((p.meta >> 11) & 1u) { if (HASH) hash_ev(h, EV_PH_RAYLEIGH, 0); st = ST_PHANTOM; }
-        else { if (HASH) hash_ev(h, EV_RAYLEIGH, ids); st = ST_STEP; }
-      }
     } else {
       // ------------------------------------------------ PHANTOM: Woodcock tracking in the voxel grid [R17]
       bool leave = false;
       if (st == ST_PHANTOM) {
-        const float s = -__logf(draw()) * p.inv_mu;
+        const uint4 w = next_block();                                 // [R4]
+        const float s = -__logf(u01(w.x)) * p.inv_mu;
         int v[3]; bool out = false;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
@@ -436,19 +451,14 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
           const int mat = (int)src.phantom[((size_t)v[2] * src.dims[1] + v[1]) * src.dims[0] + v[0]] - 1;
           if (mat >= 0) {
             const float4 m4 = mu_lookup(mu, T, mat, p.E);
-            const float t = draw() * mu_lookup(mu, T, src.ph_major, p.E).z;
+            const float t = u01(w.y) * mu_lookup(mu, T, src.ph_major, p.E).z;
             if (t < m4.x) { if (HASH) { hash_ev(h, EV_PH_ABSORBED, 0); hash_out[2ull * p.pair + (p.meta & 1u)] = h; } st = ST_POP; }
             else if (t < m4.y) st = ST_COMPTON;
-            else if (t < m4.z) st = ST_RAYLEIGH;
+            else if (t < m4.z) { rayleigh(p.d, u01(w.z), u01(w.w)); if (HASH) hash_ev(h, EV_PH_RAYLEIGH, 0); }
           }
         }
       }
-      const unsigned m_leave = __ballot_sync(0xFFFFFFFFu, leave);
-      if (m_leave) {
-        if (leave) pool_store(W.S, cntS + __popc(m_leave & lt_mask), p, h);
-        cntS += __popc(m_leave);
-        __syncwarp();
-      }
+      park_leavers(leave);
     }
   }
 
@@ -463,16 +473,16 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, const float *maj, D
 
 size_t transport_smem_bytes(const DevTables &T, bool hash) {
   const size_t fixed = hash ? sizeof(Smem<true>) : sizeof(Smem<false>);
-  return fixed - sizeof(float4) + sizeof(float4) * (size_t)T.n_materials * T.n_energies + 16;
+  return fixed - sizeof(float4) + sizeof(float4) * (size_t)T.n_staged * T.n_energies + 16;
 }
 
-cudaError_t launch_transport(const DevGeom *geom, const DevTables &T, const float *maj, const DevSource &src,
+cudaError_t launch_transport(const DevGeom *geom, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
                              unsigned long long *work_counter, int sm_count, cudaStream_t stream) {
   const size_t smem = transport_smem_bytes(T, hash_out != nullptr);
   const uint64_t n_photons = 2 * n_pairs;
   const uint64_t want = (n_photons + kThreads - 1) / kThreads;
-  static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : 2;
+  static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : 3;
   const uint64_t resident = (uint64_t)sm_count * ctas_per_sm;         // persistent grid
   const int blocks = (int)(want < resident ? (want ? want : 1) : resident);
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(unsigned long long), stream);
@@ -480,11 +490,11 @@ cudaError_t launch_transport(const DevGeom *geom, const DevTables &T, const floa
   if (hash_out) {
     e = cudaFuncSetAttribute(transport_wavefront_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    transport_wavefront_kernel<true><<<blocks, kThreads, smem, stream>>>(geom, T, maj, src, first_history, n_photons, seed, H, hash_out, work_counter);
+    transport_wavefront_kernel<true><<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_photons, seed, H, hash_out, work_counter);
   } else {
     e = cudaFuncSetAttribute(transport_wavefront_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    transport_wavefront_kernel<false><<<blocks, kThreads, smem, stream>>>(geom, T, maj, src, first_history, n_photons, seed, H, hash_out, work_counter);
+    transport_wavefront_kernel<false><<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_photons, seed, H, hash_out, work_counter);
   }
   count_launch();
   return cudaGetLastError();

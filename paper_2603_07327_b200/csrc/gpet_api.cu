@@ -312,7 +312,7 @@ static int make_digi(const gpet_source *src, uint64_t seed, uint64_t n_pairs_tot
   P->e_lo = d->e_lo_keV; P->e_hi = d->e_hi_keV; P->window_s = d->window_ns * 1e-9;
   P->shift = d->readout_level == 0 ? 5 : (d->readout_level == 1 ? 20 : 26);
   P->activity_bq = src->activity_bq; P->pairs_per_slice = src->pairs_per_time_slice ? src->pairs_per_time_slice : n_pairs_total;
-  P->seed = seed;
+  P->seed = seed; P->slice_s = (double)P->pairs_per_slice / P->activity_bq;
   return GPET_OK;
 }
 

@@ -22,7 +22,7 @@ struct DevSource {
 struct DigiParams {
   float sigma_scale;       // R / 2.3548
   float ref_keV, e_lo, e_hi; double window_s; int shift;         // ids >> shift = readout unit
-  double activity_bq; uint64_t pairs_per_slice; uint64_t seed;
+  double activity_bq, slice_s; uint64_t pairs_per_slice; uint64_t seed;   // slice_s = pairs_per_slice / activity_bq
 };
 
 struct SinglesBuf { uint32_t *history, *ids; float *x, *y, *z, *e; double *t; unsigned long long capacity; unsigned long long *n; };

@@ -434,11 +434,17 @@ static void transport_photon(ctx_t *c, uint64_t seed, uint64_t history, int phot
       double mu_maj = mu_total(M, S->phantom_majorant, E);
       double u[4]; rng_next_block(&r, u);                            /* [R4] free path, outcome, Rayleigh polar, azimuth */
       double s = -log(u[0]) / mu_maj; c->C->ph_steps++;
-      for (int k = 0; k < 3; ++k) x[k] += s * d[k];
-      path += s;
-      int v[3], out = 0;
-      for (int k = 0; k < 3; ++k) { v[k] = (int)floor((x[k] - (double)S->origin[k]) / (double)S->voxel[k]); if (v[k] < 0 || v[k] >= S->dims[k]) out = 1; }
+      /* [R17] tentative collision point; outside the grid: no collision happens before the grid face and vacuum
+       * lies beyond it, so the photon leaves along its line of flight FROM ITS CURRENT POINT (the
+       * escaping gamma is taken to its panel along that line) -- it is not moved by the overshooting step */
+      double xt[3]; int v[3], out = 0;
+      for (int k = 0; k < 3; ++k) {
+        xt[k] = x[k] + s * d[k];
+        v[k] = (int)floor((xt[k] - (double)S->origin[k]) / (double)S->voxel[k]); if (v[k] < 0 || v[k] >= S->dims[k]) out = 1;
+      }
       if (out) { if (h) hash_ev(h, EV_PH_LEAVE, 0); break; }
+      for (int k = 0; k < 3; ++k) x[k] = xt[k];
+      path += s;
       int mat = (int)S->phantom[((size_t)v[2] * S->dims[1] + v[1]) * S->dims[0] + v[0]] - 1;
       if (mat < 0) continue;                                        /* vacuum voxel: virtual, no draw */
       mu3_t mu = mu_lookup(M, mat, E); double t = u[1] * mu_maj;

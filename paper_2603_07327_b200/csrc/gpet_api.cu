@@ -118,6 +118,19 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
     const float *q = G.pose[p];
     if (q[2] != 0.0f || q[5] != 0.0f || q[11] != 0.0f || q[6] != 0.0f || q[7] != 0.0f || q[8] != 1.0f) G.planar = 0;
   }
+  // bounding circle (planar search: tangential x depth) and sphere of the panel box, 0.01 % + 1 um margin: the search
+  // only culls panels whose bound the ray misses, so the surviving tests decide exactly as the full loop [R6]
+  {
+    const double ha = 0.5 * ((double)G.bhi[0] - G.blo[0]), hb = 0.5 * ((double)G.bhi[1] - G.blo[1]), hc = 0.5 * ((double)G.bhi[2] - G.blo[2]);
+    const double ma = 0.5 * ((double)G.bhi[0] + G.blo[0]), mb = 0.5 * ((double)G.bhi[1] + G.blo[1]), mc = 0.5 * ((double)G.bhi[2] + G.blo[2]);
+    G.cull_r2 = (float)(sqrt(ha * ha + hc * hc) * 1.0001 + 1e-3);
+    G.cull_r3 = (float)(sqrt(ha * ha + hb * hb + hc * hc) * 1.0001 + 1e-3);
+    for (int p = 0; p < G.n_panels; ++p) {
+      const float *q = G.pose[p]; float c[3];
+      for (int k = 0; k < 3; ++k) c[k] = (float)((double)q[k] + ma * q[3 + k] + mb * q[6 + k] + mc * q[9 + k]);
+      G.centre[p] = make_float4(c[0], c[1], c[2], 0.0f);
+    }
+  }
   *out = g;                     // the device copy is made lazily so the handle can be built without a GPU
   return GPET_OK;
 }

@@ -31,8 +31,10 @@ struct DevGeom {
   uint32_t det_mask;          // materials referenced by the layers
   int ring;                   // 1 = repetition mode
   int planar;                 // 1 = every panel has v = +z and u_z = w_z = o_z = 0: the search shares the axial slab
+  float cull_r2, cull_r3;     // radius (+ margin) of the circle / sphere about a panel box: (a,c) plane / 3-D
   DevLayer layer[kMaxLayers];
   float pose[kMaxPanels][12]; // front-face centre, u, v, w
+  float4 centre[kMaxPanels];  // global position of the box centre (search culling)
 };
 
 struct DevTables {            // [R11] per staged material, per energy: {mu_pe, mu_pe+mu_C, mu_tot, detector majorant}
@@ -50,6 +52,18 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
     const uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
     c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
     k.x += 0x9E3779B9u; k.y += 0xBB67AE85u;
+  }
+  return c;
+}
+// The same generator with the ten round keys precomputed on the host (they depend on the seed only): passed as a
+// kernel parameter they are constant-bank operands of the XORs, so a round is two wide multiplies and two LOP3.
+struct PhiloxKeys { uint32_t k[20]; };
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, const PhiloxKeys &K) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+    c = make_uint4(hi1 ^ c.y ^ K.k[2 * r], lo1, hi0 ^ c.w ^ K.k[2 * r + 1], lo0);
   }
   return c;
 }

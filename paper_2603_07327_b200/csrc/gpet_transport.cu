@@ -142,6 +142,11 @@ __device__ __forceinline__ void decay_site(const DevSource &src, uint4 w, float 
 
 // ---------------------------------------------------------------- [R6] panel search
 // Nearest-entry panel over all panels but `excl`; ties keep the lowest index; -1 = escapes.
+// Two steps.  (1) Cull: a panel stays a candidate only if the ray passes the circle (planar detectors) or
+// sphere about its box, ahead of the photon -- 6 / 11 operations per panel instead of a slab test; the bound
+// carries a margin far above fp32 rounding, so no panel the slab test would accept is ever dropped.  (2) The
+// surviving panels (about one per photon) take the slab test of [R6] in ascending index order, so the
+// decision -- including ties -- is the one the loop over all panels makes.
 // "planar" detectors (every panel has v = +z, u_z = w_z = o_z = 0: any ring built in repetition mode,
 // PAPER.md:33) share the axial slab and need only the 2-D part of each pose; the arithmetic on the
 // surviving terms is the generic one (the dropped terms are exact zeros).
@@ -151,30 +156,58 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
     const float iz = rcp_dir(d[2]);
     const float z1 = (g.blo[1] - x[2]) * iz, z2 = (g.bhi[1] - x[2]) * iz;
     const float tnz = fmaxf(fminf(z1, z2), 0.0f), tfz = fmaxf(z1, z2);
-#pragma unroll 2
-    for (int q = 0; q < g.n_panels; ++q) {
-      const float *P = g.pose[q];
-      const float r0 = x[0] - P[0], r1 = x[1] - P[1];
-      const float a = r0 * P[3] + r1 * P[4], c = r0 * P[9] + r1 * P[10];
-      const float ia = rcp_dir(d[0] * P[3] + d[1] * P[4]), ic = rcp_dir(d[0] * P[9] + d[1] * P[10]);
-      const float a1 = (g.blo[0] - a) * ia, a2 = (g.bhi[0] - a) * ia, c1 = (g.blo[2] - c) * ic, c2 = (g.bhi[2] - c) * ic;
-      const float tn = fmaxf(tnz, fmaxf(fminf(a1, a2), fminf(c1, c2)));
-      const float tf = fminf(tfz, fminf(fmaxf(a1, a2), fmaxf(c1, c2)));
-      if (q != excl && tf > tn && tn < bt) { bt = tn; bp = q; }
+    const float sr = g.cull_r2 * sqrt_fast(fmaf(d[0], d[0], d[1] * d[1]));
+    const bool axial_ok = tfz > tnz;
+    for (int base = 0; base < g.n_panels; base += 32) {
+      const int nq = min(32, g.n_panels - base);
+      uint32_t cand = 0;
+#pragma unroll 4
+      for (int q = 0; q < nq; ++q) {
+        const float4 c = g.centre[base + q];
+        const float rx = c.x - x[0], ry = c.y - x[1];
+        const float cross = fmaf(rx, d[1], -ry * d[0]), dot = fmaf(rx, d[0], ry * d[1]);
+        if (fabsf(cross) <= sr && dot >= -sr) cand |= 1u << q;
+      }
+      if ((unsigned)(excl - base) < 32u) cand &= ~(1u << (excl - base));
+      if (!axial_ok) cand = 0;
+      while (cand) {
+        const int q = base + __ffs(cand) - 1; cand &= cand - 1;
+        const float *P = g.pose[q];
+        const float r0 = x[0] - P[0], r1 = x[1] - P[1];
+        const float a = r0 * P[3] + r1 * P[4], c = r0 * P[9] + r1 * P[10];
+        const float ia = rcp_dir(d[0] * P[3] + d[1] * P[4]), ic = rcp_dir(d[0] * P[9] + d[1] * P[10]);
+        const float a1 = (g.blo[0] - a) * ia, a2 = (g.bhi[0] - a) * ia, c1 = (g.blo[2] - c) * ic, c2 = (g.bhi[2] - c) * ic;
+        const float tn = fmaxf(tnz, fmaxf(fminf(a1, a2), fminf(c1, c2)));
+        const float tf = fminf(tfz, fminf(fmaxf(a1, a2), fmaxf(c1, c2)));
+        if (tf > tn && tn < bt) { bt = tn; bp = q; }
+      }
     }
   } else {
-#pragma unroll 1
-    for (int q = 0; q < g.n_panels; ++q) {
-      float xl[3], dl[3];
-      to_local(g.pose[q], x, d, xl, dl);
-      float tn = 0.0f, tf = INFINITY;
-#pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        const float inv = rcp_dir(dl[k]);
-        const float t1 = (g.blo[k] - xl[k]) * inv, t2 = (g.bhi[k] - xl[k]) * inv;
-        tn = fmaxf(tn, fminf(t1, t2)); tf = fminf(tf, fmaxf(t1, t2));
+    for (int base = 0; base < g.n_panels; base += 32) {
+      const int nq = min(32, g.n_panels - base);
+      uint32_t cand = 0;
+#pragma unroll 2
+      for (int q = 0; q < nq; ++q) {
+        const float4 c = g.centre[base + q];
+        const float rx = c.x - x[0], ry = c.y - x[1], rz = c.z - x[2];
+        const float b = fmaf(rx, d[0], fmaf(ry, d[1], rz * d[2]));                  // |d| = 1
+        const float r2 = fmaf(rx, rx, fmaf(ry, ry, rz * rz));
+        if (r2 - b * b <= g.cull_r3 * g.cull_r3 * 1.0001f && b >= -g.cull_r3) cand |= 1u << q;
       }
-      if (q != excl && tf > tn && tn < bt) { bt = tn; bp = q; }
+      if ((unsigned)(excl - base) < 32u) cand &= ~(1u << (excl - base));
+      while (cand) {
+        const int q = base + __ffs(cand) - 1; cand &= cand - 1;
+        float xl[3], dl[3];
+        to_local(g.pose[q], x, d, xl, dl);
+        float tn = 0.0f, tf = INFINITY;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          const float inv = rcp_dir(dl[k]);
+          const float t1 = (g.blo[k] - xl[k]) * inv, t2 = (g.bhi[k] - xl[k]) * inv;
+          tn = fmaxf(tn, fminf(t1, t2)); tf = fminf(tf, fmaxf(t1, t2));
+        }
+        if (tf > tn && tn < bt) { bt = tn; bp = q; }
+      }
     }
   }
   t_enter = bt; return bp;
@@ -184,7 +217,7 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
 template <bool HASH>
 __global__ void __launch_bounds__(kThreads, 3)
 transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint64_t first_history, uint64_t n_photons,
-                           uint64_t seed, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
+                           const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem<HASH> *S = reinterpret_cast<Smem<HASH> *>(smem_raw);
   {
@@ -201,7 +234,6 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
   WarpMem<HASH> &W = S->w[threadIdx.x >> 5];
   HitStage &stage = W.stage;
   const unsigned lt_mask = (1u << lane) - 1u;
-  const uint2 key = make_uint2((uint32_t)seed, (uint32_t)(seed >> 32));
   const bool use_phantom = src.kind == 1 && src.phantom != nullptr;
 
   Photon p; p.meta = 0; p.ndraw = 0; p.E = 0.f; p.path = 0.f; p.inv_mu = 0.f; p.pair = 0;
@@ -296,7 +328,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
             if (src.acol_sigma > 0.0f) {
               const float rho = src.acol_sigma * sqrt_fast(-2.0f * __logf(u01(w.z)));
               float sr, cr; sincos_small(rho, sr, cr);
-              float sp, cp; sincospif(2.0f * u01(w.w), &sp, &cp);
+              float sp, cp; sincos_2pi(u01(w.w), sp, cp);               // azimuth of a ~4e-3 rad deviation: 2^-21 is ample
               rotate(q.d, cr, sr, cp, sp);
             }
           }
@@ -438,16 +470,17 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
       if (st == ST_PHANTOM) {
         const uint4 w = next_block();                                 // [R4]
         const float s = -__logf(u01(w.x)) * p.inv_mu;
-        int v[3]; bool out = false;
+        int v[3]; bool out = false; float xt[3];
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-          p.x[k] = fmaf(s, p.d[k], p.x[k]);
-          v[k] = __float2int_rd((p.x[k] - src.origin[k]) * src.inv_voxel[k]);
+          xt[k] = fmaf(s, p.d[k], p.x[k]);
+          v[k] = __float2int_rd((xt[k] - src.origin[k]) * src.inv_voxel[k]);
           out = out || v[k] < 0 || v[k] >= src.dims[k];
         }
-        p.path += s;
+        // tentative point outside the grid: the photon leaves along its line of flight from where it is [R17]
         if (out) { if (HASH) hash_ev(h, EV_PH_LEAVE, 0); p.meta &= ~(1u << 11); leave = true; st = ST_POP; }
         else {
+          p.x[0] = xt[0]; p.x[1] = xt[1]; p.x[2] = xt[2]; p.path += s;
           const int mat = (int)src.phantom[((size_t)v[2] * src.dims[1] + v[1]) * src.dims[0] + v[0]] - 1;
           if (mat >= 0) {
             const float4 m4 = mu_lookup(mu, T, mat, p.E);
@@ -484,17 +517,19 @@ cudaError_t launch_transport(const DevGeom *geom, const DevTables &T, const DevS
   const uint64_t want = (n_photons + kThreads - 1) / kThreads;
   static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : 3;
   const uint64_t resident = (uint64_t)sm_count * ctas_per_sm;         // persistent grid
+  PhiloxKeys key;                                                     // [R1] round keys: key + r * Weyl constants
+  for (int r = 0; r < 10; ++r) { key.k[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; key.k[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }
   const int blocks = (int)(want < resident ? (want ? want : 1) : resident);
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(unsigned long long), stream);
   if (e != cudaSuccess) return e;
   if (hash_out) {
     e = cudaFuncSetAttribute(transport_wavefront_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    transport_wavefront_kernel<true><<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_photons, seed, H, hash_out, work_counter);
+    transport_wavefront_kernel<true><<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_photons, key, H, hash_out, work_counter);
   } else {
     e = cudaFuncSetAttribute(transport_wavefront_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    transport_wavefront_kernel<false><<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_photons, seed, H, hash_out, work_counter);
+    transport_wavefront_kernel<false><<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_photons, key, H, hash_out, work_counter);
   }
   count_launch();
   return cudaGetLastError();

@@ -551,3 +551,26 @@ def test_phantom_attenuation(tables):
     assert 0.85 < p_free < 0.88 and len(res.hits) == 0
     assert c["ph_absorbed"] < 0.01 * c["ph_compton"] and c["ph_steps"] > 2 * n
     assert abs(math.fsum(res.e_escape.ravel()) / (2 * n) - 511.0) < 25.0   # scattered photons keep most of their energy
+
+
+def test_leaving_the_phantom_keeps_the_line_of_flight(tables):
+    """a gamma escaping from the phantom is taken to its panel along its line of flight.  With an
+    all-vacuum phantom the acceptance of C0's panel must therefore still be the analytic solid angle
+    2*Omega/4pi = 0.0090375, and first hits must keep tof = |x - source| / c.  A Woodcock step
+    (mean free path of the water majorant: ~104 mm) that carried the photon past the panel on leaving the grid
+    would lose most entries [R17]."""
+    act, mat, org = W.hot_rod_phantom()
+    one = np.zeros_like(act); one[64, 64, 64] = 1.0
+    src = W.Source(1, (0, 0, 0), 0.0, 1e6, 0, one, np.zeros_like(mat), 1, (128, 128, 128), (0.25,) * 3, org)
+    n = 2_000_000
+    res = O.simulate(W.geometry_c0(), tables, src, n, seed=8, threads=8)
+    c = res.counters
+    expect = 0.0090375 * n
+    assert abs(c["entries"] - expect) < 4 * math.sqrt(expect) + 0.004 * expect      # voxel is 0.125 mm off-centre
+    assert c["ph_steps"] >= 2 * n and c["ph_compton"] == 0
+    first = (res.hits.ids & 15) == 0
+    site = O.decay_sites(src, 8, 0, n)[res.hits.history[first]]
+    xyz = np.stack([res.hits.x, res.hits.y, res.hits.z], 1)[first]
+    direct = np.linalg.norm(xyz - site, axis=1) / 299.792458
+    unscattered = np.abs(res.hits.tof_ns[first] - direct) < 1e-4
+    assert unscattered.mean() > 0.9                                  # the rest scattered in the crystal first

@@ -98,7 +98,7 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
   G.blo[1] = (float)(-(double)G.hHq / 1048576.0); G.bhi[1] = (float)((double)(Hq - G.hHq) / 1048576.0);
   G.blo[2] = 0.0f;                                G.bhi[2] = (float)((double)c / 1048576.0);
   if (d->panel_pose) {
-    memcpy(G.pose, d->panel_pose, sizeof(float) * 12 * (size_t)d->n_panels);
+    for (int p = 0; p < d->n_panels; ++p) memcpy(G.panel[p].pose, d->panel_pose + 12 * p, sizeof(float) * 12);
   } else {                                                          // [R5] repetition mode
     const double PI = 3.14159265358979323846;
     for (int p = 0; p < d->n_panels; ++p) {
@@ -106,7 +106,7 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
       double cs = cos(phi), sn = sin(phi);
       if (fabs(cs) < 1e-12) cs = 0.0;
       if (fabs(sn) < 1e-12) sn = 0.0;
-      float *q = G.pose[p];
+      float *q = G.panel[p].pose;
       q[0] = (float)((double)d->ring_inner_radius_mm * cs); q[1] = (float)((double)d->ring_inner_radius_mm * sn); q[2] = 0.0f;
       q[3] = (float)(-sn); q[4] = (float)cs; q[5] = 0.0f;
       q[6] = 0.0f; q[7] = 0.0f; q[8] = 1.0f;
@@ -115,7 +115,7 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
   }
   G.planar = 1;                 // axial axis = +z everywhere and no z component elsewhere (any repetition-mode ring)
   for (int p = 0; p < G.n_panels; ++p) {
-    const float *q = G.pose[p];
+    const float *q = G.panel[p].pose;
     if (q[2] != 0.0f || q[5] != 0.0f || q[11] != 0.0f || q[6] != 0.0f || q[7] != 0.0f || q[8] != 1.0f) G.planar = 0;
   }
   // bounding circle (planar search: tangential x depth) and sphere of the panel box, 0.01 % + 1 um margin: the search
@@ -126,9 +126,9 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
     G.cull_r2 = (float)(sqrt(ha * ha + hc * hc) * 1.0001 + 1e-3);
     G.cull_r3 = (float)(sqrt(ha * ha + hb * hb + hc * hc) * 1.0001 + 1e-3);
     for (int p = 0; p < G.n_panels; ++p) {
-      const float *q = G.pose[p]; float c[3];
+      const float *q = G.panel[p].pose; float c[3];
       for (int k = 0; k < 3; ++k) c[k] = (float)((double)q[k] + ma * q[3 + k] + mb * q[6 + k] + mc * q[9 + k]);
-      G.centre[p] = make_float4(c[0], c[1], c[2], 0.0f);
+      G.panel[p].cx = c[0]; G.panel[p].cy = c[1]; G.panel[p].cz = c[2];
     }
   }
   *out = g;                     // the device copy is made lazily so the handle can be built without a GPU
@@ -150,7 +150,7 @@ extern "C" int gpet_geometry_destroy(gpet_geometry *g) {
 
 extern "C" int gpet_geometry_panel_pose(const gpet_geometry *g, int32_t panel, float *pose12) {
   if (!g || !pose12 || panel < 0 || panel >= g->host.n_panels) return fail(GPET_E_INVALID_ARG, "gpet_geometry_panel_pose: bad argument");
-  memcpy(pose12, g->host.pose[panel], sizeof(float) * 12); return GPET_OK;
+  memcpy(pose12, g->host.panel[panel].pose, sizeof(float) * 12); return GPET_OK;
 }
 
 extern "C" int gpet_geometry_locate(const gpet_geometry *g, int64_t n, const float *xyz, uint32_t *ids) {
@@ -311,7 +311,7 @@ extern "C" int gpet_simulate(const gpet_geometry *g, const gpet_materials *m, co
   const uint32_t stage_mask = (D.kind == 1 && D.phantom) ? (1u << m->n_materials) - 1u : 0u;
   DevTables T; rc = staged_table(const_cast<gpet_materials *>(m), g->host.det_mask, stage_mask, &T); if (rc) return rc;
   unsigned long long *wc = nullptr; rc = next_work_counter(&wc); if (rc) return rc;
-  CUDA_TRY(launch_transport(g->dev, T, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
+  CUDA_TRY(launch_transport(g->dev, g->host.n_panels, T, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
   return GPET_OK;
 }
 

@@ -22,6 +22,10 @@ struct DevLayer {
   float inv_pitch[2];
   int cmat, gmat;
 };
+struct __align__(16) DevPanel {
+  float pose[12];             // front-face centre, u, v, w
+  float cx, cy, cz, pad;      // global position of the box centre (search culling)
+};
 struct DevGeom {
   int n_panels, n_layers;
   int Wq, Hq, Dq, hWq, hHq;
@@ -33,9 +37,9 @@ struct DevGeom {
   int planar;                 // 1 = every panel has v = +z and u_z = w_z = o_z = 0: the search shares the axial slab
   float cull_r2, cull_r3;     // radius (+ margin) of the circle / sphere about a panel box: (a,c) plane / 3-D
   DevLayer layer[kMaxLayers];
-  float pose[kMaxPanels][12]; // front-face centre, u, v, w
-  float4 centre[kMaxPanels];  // global position of the box centre (search culling)
+  DevPanel panel[kMaxPanels]; // LAST member: kernels stage only the first n_panels records into shared memory
 };
+__host__ __device__ inline size_t geom_bytes(int n_panels) { return sizeof(DevGeom) - sizeof(DevPanel) * (size_t)(kMaxPanels - n_panels); }
 
 struct DevTables {            // [R11] per staged material, per energy: {mu_pe, mu_pe+mu_C, mu_tot, detector majorant}
   int n_staged, n_energies;   // only the materials a run can touch are staged into shared memory

@@ -2,19 +2,18 @@
 // PAPER.md:33 (panel transfer by ray/plane crossing, global->local), PAPER.md:43 (Woodcock tracking in the
 // panel frame, layer selection from the local depth, run until exit or cutoff).
 //
-// Design.  The unit of work is one photon (index j = 2*pair + photon).  Every
-// persistent warp alternates between two roles and keeps two private photon pools in shared memory:
-//   GENERATE  all 32 lanes take a photon that needs a panel search -- one that left a panel (pool S) or a
-//             new one from the source (S3) -- and run the search together at full SIMD width; photons that
-//             enter a panel are compacted (ballot + prefix popcount) into pool T, the others are done;
-//   TRANSPORT every lane owns one in-panel photon and a small state machine {POP, STEP, COMPTON, RAYLEIGH,
-//             PHANTOM}; each pass ballots the lanes' next events and runs the ONE phase most lanes wait for
-//             (regrouping by next event); idle lanes refill from pool T, photons that leave their panel are
-//             pushed to pool S.
-// Every phase appears exactly once in the kernel, which keeps the SASS small enough for the instruction
-// caches (v1's 107 KB of inlined code stalled 59 % of the time on instruction fetch).  Geometry descriptor
-// and interleaved float4 mu tables live in shared memory; hits are staged per warp in shared memory and
-// flushed 32 at a time: one atomicAdd per 32 hits and seven fully coalesced 128-byte stores (SoA).
+// Design.  The unit of work is one photon (index j = 2*pair + photon).  Every persistent
+// warp owns a pool of photon SLOTS in shared memory (48-byte records that never move) and one index list per
+// NEXT EVENT: SEARCH (needs a panel search), STEP (Woodcock step in a panel), KN (Klein-Nishina trial), RAY
+// (Rayleigh deflection), PHANTOM (Woodcock step in the voxel grid), plus the FREE list.  A pass pops up to 32
+// slot indices from ONE list, runs that event for all of them at full SIMD width, writes the changed fields back
+// and pushes every index onto the list of its next event (ballot + prefix popcount).  The scheduler always runs
+// the event with the most ready photons; SEARCH counts the fresh photons it can admit from the source (S3), so
+// a warp is never short of work before the end.  This is the "regroup live photons by next event" of the
+// north star, done per warp: no block-level barrier, no atomics except the chunked work counter and the hit
+// counter.  Every event's code appears exactly once in the kernel.  Geometry descriptor and interleaved float4 mu
+// tables live in shared memory; hits are staged per warp in shared memory and flushed 32 at a time: one
+// atomicAdd per 32 hits and seven fully coalesced 128-byte stores (SoA).
 #include <cstdlib>
 #include "gpet_internal.h"
 
@@ -23,30 +22,27 @@ namespace gpet {
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 constexpr int kStage = 64;            // staged hits per warp (ring buffer)
-constexpr int kPool = 96;             // parked photons per warp: stack T (await transport) grows from slot 0,
-                                      // stack S (await a panel search) from the top; lanes + parked <= kPool
-constexpr int kLowT = 24;             // GENERATE when fewer photons than this await transport ...
-constexpr int kHighS = 16;            // ... or at least this many await a search
+constexpr int kSlots = 96;            // photon slots per warp
 constexpr uint32_t kChunk = 1024;     // photon indices a warp reserves at a time
 
-enum : int { ST_POP = 0, ST_STEP = 1, ST_COMPTON = 2, ST_PHANTOM = 3, ST_NONE = 4 };
+enum : int { L_FREE = 0, L_SEARCH, L_STEP, L_KN, L_RAY, L_PHANTOM, kLists, L_NONE = kLists };
 
 struct HitStage { uint32_t w[7][kStage]; };      // history, ids, x, y, z, e, tof
 
-// 48 bytes per parked photon (no RNG state: a stream is addressed by its block counter [R4])
-template <int N, bool HASH> struct Pool {
-  float4 a[N];                         // x, y, z, dx
-  float4 b[N];                         // dy, dz, E, path
-  uint4 c[N];                          // pair, meta, ndraw, inv_mu bits
-  uint2 hh[HASH ? N : 1];              // outcome hash (parity builds only)
+// One warp's private memory.  A photon record is 48 bytes in three 16-byte planes (conflict-free LDS.128).
+template <bool HASH> struct WarpMem {
+  float4 a[kSlots];                    // x, y, z, dx
+  float4 b[kSlots];                    // dy, dz, E, path
+  uint4 c[kSlots];                     // pair, meta, ids of the pending interaction, inv_mu bits
+  uint2 hh[HASH ? kSlots : 1];         // outcome hash (parity builds only)
+  uint8_t list[kLists][kSlots];        // slot indices by next event (stacks)
+  HitStage stage;
 };
 
-template <bool HASH> struct WarpMem { Pool<kPool, HASH> pool; HitStage stage; };
-
-template <bool HASH> struct Smem {
-  DevGeom g;
-  WarpMem<HASH> w[kWarps];
-  float4 mu[1];                        // [n_staged][n_energies], .w = detector majorant
+// dynamic shared memory: [WarpMem x kWarps][mu: n_staged x n_energies float4][DevGeom, first n_panels records]
+template <bool HASH> struct SmemLayout {
+  static constexpr size_t mu_off = sizeof(WarpMem<HASH>) * kWarps;
+  __host__ __device__ static size_t geom_off(int n_mu) { return mu_off + sizeof(float4) * (size_t)n_mu; }
 };
 
 // ---------------------------------------------------------------- fast math with bounded error
@@ -80,29 +76,31 @@ __device__ __forceinline__ float4 mu_lookup(const float4 *mu, const DevTables &T
 
 // ---------------------------------------------------------------- photon state
 struct Photon {
-  float x[3], d[3];        // global frame while searching / in the phantom, panel frame in STEP / COMPTON / RAYLEIGH
+  float x[3], d[3];        // global frame while searching / in the phantom, panel frame in STEP / KN / RAY
   float E, path, inv_mu;   // inv_mu = 1 / majorant(E) of the medium the photon is tracked in
   uint32_t pair;           // history - first_history
-  uint32_t meta;           // bit0 photon, bits1-4 seq, bits5-10 panel (current, or just left; 63 = none),
-                           // bit11 in phantom, bits12+ Klein-Nishina trial counter
-  uint32_t ndraw;          // Philox blocks consumed from this photon's stream [R4]
+  uint32_t meta;           // bit0 photon, bits1-4 seq, bits5-10 panel (current, or just left; 63 = none), bit11 in
+                           // phantom, bits12-17 Klein-Nishina trial counter, bits18-31 Philox blocks consumed from
+                           // this photon's stream [R4] (16383 events per photon: never reached, the energy falls)
+  uint32_t ids;            // lattice result of the pending interaction (KN / RAY)
 };
 __device__ __forceinline__ int ph_panel(const Photon &p) { return (p.meta >> 5) & 63u; }
 __device__ __forceinline__ void ph_set_panel(Photon &p, int panel) { p.meta = (p.meta & ~(63u << 5)) | ((uint32_t)panel << 5); }
+__device__ __forceinline__ bool ph_in_phantom(const Photon &p) { return (p.meta >> 11) & 1u; }
 
-template <int N, bool HASH>
-__device__ __forceinline__ void pool_store(Pool<N, HASH> &P, int slot, const Photon &p, uint64_t h) {
-  P.a[slot] = make_float4(p.x[0], p.x[1], p.x[2], p.d[0]);
-  P.b[slot] = make_float4(p.d[1], p.d[2], p.E, p.path);
-  P.c[slot] = make_uint4(p.pair, p.meta, p.ndraw, __float_as_uint(p.inv_mu));
-  if (HASH) P.hh[slot] = make_uint2((uint32_t)h, (uint32_t)(h >> 32));
+template <bool HASH>
+__device__ __forceinline__ void slot_store(WarpMem<HASH> &W, int slot, const Photon &p, uint64_t h) {
+  W.a[slot] = make_float4(p.x[0], p.x[1], p.x[2], p.d[0]);
+  W.b[slot] = make_float4(p.d[1], p.d[2], p.E, p.path);
+  W.c[slot] = make_uint4(p.pair, p.meta, p.ids, __float_as_uint(p.inv_mu));
+  if (HASH) W.hh[slot] = make_uint2((uint32_t)h, (uint32_t)(h >> 32));
 }
-template <int N, bool HASH>
-__device__ __forceinline__ void pool_load(const Pool<N, HASH> &P, int slot, Photon &p, uint64_t &h) {
-  const float4 a = P.a[slot], b = P.b[slot]; const uint4 c = P.c[slot];
+template <bool HASH>
+__device__ __forceinline__ void slot_load(const WarpMem<HASH> &W, int slot, Photon &p, uint64_t &h) {
+  const float4 a = W.a[slot], b = W.b[slot]; const uint4 c = W.c[slot];
   p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.d[0] = a.w; p.d[1] = b.x; p.d[2] = b.y; p.E = b.z; p.path = b.w;
-  p.pair = c.x; p.meta = c.y; p.ndraw = c.z; p.inv_mu = __uint_as_float(c.w);
-  if (HASH) { const uint2 v = P.hh[slot]; h = ((uint64_t)v.y << 32) | v.x; }
+  p.pair = c.x; p.meta = c.y; p.ids = c.z; p.inv_mu = __uint_as_float(c.w);
+  if (HASH) { const uint2 v = W.hh[slot]; h = ((uint64_t)v.y << 32) | v.x; }
 }
 
 // write one staged hit (slot of this warp's ring buffer) to the global struct-of-arrays buffer
@@ -163,8 +161,8 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
       uint32_t cand = 0;
 #pragma unroll 4
       for (int q = 0; q < nq; ++q) {
-        const float4 c = g.centre[base + q];
-        const float rx = c.x - x[0], ry = c.y - x[1];
+        const DevPanel &c = g.panel[base + q];
+        const float rx = c.cx - x[0], ry = c.cy - x[1];
         const float cross = fmaf(rx, d[1], -ry * d[0]), dot = fmaf(rx, d[0], ry * d[1]);
         if (fabsf(cross) <= sr && dot >= -sr) cand |= 1u << q;
       }
@@ -172,7 +170,7 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
       if (!axial_ok) cand = 0;
       while (cand) {
         const int q = base + __ffs(cand) - 1; cand &= cand - 1;
-        const float *P = g.pose[q];
+        const float *P = g.panel[q].pose;
         const float r0 = x[0] - P[0], r1 = x[1] - P[1];
         const float a = r0 * P[3] + r1 * P[4], c = r0 * P[9] + r1 * P[10];
         const float ia = rcp_dir(d[0] * P[3] + d[1] * P[4]), ic = rcp_dir(d[0] * P[9] + d[1] * P[10]);
@@ -188,8 +186,8 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
       uint32_t cand = 0;
 #pragma unroll 2
       for (int q = 0; q < nq; ++q) {
-        const float4 c = g.centre[base + q];
-        const float rx = c.x - x[0], ry = c.y - x[1], rz = c.z - x[2];
+        const DevPanel &c = g.panel[base + q];
+        const float rx = c.cx - x[0], ry = c.cy - x[1], rz = c.cz - x[2];
         const float b = fmaf(rx, d[0], fmaf(ry, d[1], rz * d[2]));                  // |d| = 1
         const float r2 = fmaf(rx, rx, fmaf(ry, ry, rz * rz));
         if (r2 - b * b <= g.cull_r3 * g.cull_r3 * 1.0001f && b >= -g.cull_r3) cand |= 1u << q;
@@ -198,7 +196,7 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
       while (cand) {
         const int q = base + __ffs(cand) - 1; cand &= cand - 1;
         float xl[3], dl[3];
-        to_local(g.pose[q], x, d, xl, dl);
+        to_local(g.panel[q].pose, x, d, xl, dl);
         float tn = 0.0f, tf = INFINITY;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
@@ -219,46 +217,44 @@ __global__ void __launch_bounds__(kThreads, 3)
 transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint64_t first_history, uint64_t n_photons,
                            const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Smem<HASH> *S = reinterpret_cast<Smem<HASH> *>(smem_raw);
+  const int n_mu = T.n_staged * T.n_energies;
+  float4 *mu_s = reinterpret_cast<float4 *>(smem_raw + SmemLayout<HASH>::mu_off);
+  DevGeom *g_s = reinterpret_cast<DevGeom *>(smem_raw + SmemLayout<HASH>::geom_off(n_mu));
+  const int lane = threadIdx.x & 31;
+  WarpMem<HASH> &W = reinterpret_cast<WarpMem<HASH> *>(smem_raw)[threadIdx.x >> 5];
   {
     const uint32_t *gs = reinterpret_cast<const uint32_t *>(geom);
-    uint32_t *gd = reinterpret_cast<uint32_t *>(&S->g);
-    for (int i = threadIdx.x; i < (int)(sizeof(DevGeom) / 4); i += kThreads) gd[i] = gs[i];
-    const int n = T.n_staged * T.n_energies;
-    for (int i = threadIdx.x; i < n; i += kThreads) S->mu[i] = T.mu[i];
+    uint32_t *gd = reinterpret_cast<uint32_t *>(g_s);
+    const int words = (int)(geom_bytes(geom->n_panels) / 4);
+    for (int i = threadIdx.x; i < words; i += kThreads) gd[i] = gs[i];
+    for (int i = threadIdx.x; i < n_mu; i += kThreads) mu_s[i] = T.mu[i];
+    for (int i = lane; i < kSlots; i += 32) W.list[L_FREE][i] = (uint8_t)i;
     __syncthreads();
   }
-  const DevGeom &g = S->g;
-  const float4 *mu = S->mu;
-  const int lane = threadIdx.x & 31;
-  WarpMem<HASH> &W = S->w[threadIdx.x >> 5];
+  const DevGeom &g = *g_s;
+  const float4 *mu = mu_s;
   HitStage &stage = W.stage;
   const unsigned lt_mask = (1u << lane) - 1u;
   const bool use_phantom = src.kind == 1 && src.phantom != nullptr;
 
-  Photon p; p.meta = 0; p.ndraw = 0; p.E = 0.f; p.path = 0.f; p.inv_mu = 0.f; p.pair = 0;
-#pragma unroll
-  for (int k = 0; k < 3; ++k) { p.x[k] = 0.f; p.d[k] = 0.f; }
-  uint32_t ids = kNone;                    // lattice result of the pending interaction
-  uint64_t h = 0;
-  int st = ST_POP;
   uint64_t w_next = 0, w_end = 0;          // this warp's reserved photon indices [w_next, w_end)
   bool exhausted = false;                  // the global counter ran past n_photons
   uint32_t stage_head = 0, stage_cnt = 0;  // ring buffer of staged hits (warp-uniform)
-  int cntT = 0, cntS = 0;                  // pool fill levels (warp-uniform): T grows from slot 0, S from the top
+  int cF = kSlots, cS = 0, cT = 0, cK = 0, cR = 0, cP = 0;   // list fill levels (warp-uniform)
 
   // [R4] every transport event consumes one whole Philox block of the photon's stream
-  auto next_block = [&]() -> uint4 {
+  auto block_at = [&](const Photon &p, uint32_t blk) -> uint4 {
     const uint64_t history = first_history + p.pair;
-    return philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 1u + (p.meta & 1u), p.ndraw++), key);
+    return philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 1u + (p.meta & 1u), blk), key);
   };
+  auto next_block = [&](Photon &p) -> uint4 { const uint4 w = block_at(p, p.meta >> 18); p.meta += 1u << 18; return w; };
   // stage one hit per lane that has one; flush 32 staged hits with one atomic + coalesced stores (S10)
-  auto stage_hits = [&](bool has, uint32_t hit_ids, const float xg[3], float e, float tof) {
+  auto stage_hits = [&](bool has, uint32_t pair, uint32_t hit_ids, const float xg[3], float e, float tof) {
     const unsigned who = __ballot_sync(0xFFFFFFFFu, has);
     if (who == 0) return;
     if (has) {
       const uint32_t slot = (stage_head + stage_cnt + __popc(who & lt_mask)) & (kStage - 1);
-      stage.w[0][slot] = (uint32_t)(first_history + p.pair); stage.w[1][slot] = hit_ids;
+      stage.w[0][slot] = (uint32_t)(first_history + pair); stage.w[1][slot] = hit_ids;
       stage.w[2][slot] = __float_as_uint(xg[0]); stage.w[3][slot] = __float_as_uint(xg[1]); stage.w[4][slot] = __float_as_uint(xg[2]);
       stage.w[5][slot] = __float_as_uint(e); stage.w[6][slot] = __float_as_uint(tof);
     }
@@ -273,30 +269,31 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
       __syncwarp();
     }
   };
-  // park the lanes' photons that left their panel / the phantom: they wait in pool S for the next search
-  auto park_leavers = [&](bool leave) {
-    const unsigned m_leave = __ballot_sync(0xFFFFFFFFu, leave);
-    if (m_leave == 0) return;
-    if (leave) pool_store(W.pool, kPool - 1 - (cntS + __popc(m_leave & lt_mask)), p, h);
-    cntS += __popc(m_leave);
-    __syncwarp();
+  // push the slot index of every lane with `pred` onto list L (ballot + prefix popcount)
+  auto push = [&](int L, int &cnt, bool pred, int idx) {
+    const unsigned m = __ballot_sync(0xFFFFFFFFu, pred);
+    if (pred) W.list[L][cnt + __popc(m & lt_mask)] = (uint8_t)idx;
+    cnt += __popc(m);
   };
 
 #pragma unroll 1
   for (;;) {
+    // ================================================ scheduler: the event with the most ready photons
     const bool more_src = !exhausted || w_next < w_end;
-    const unsigned m_pop = __ballot_sync(0xFFFFFFFFu, st == ST_POP);
-    if ((cntT < kLowT && (more_src || cntS > 0)) || cntS >= kHighS) {
-      // ================================================ GENERATE: up to 32 photons that need a panel search
-      // The photons a warp holds (in lanes + parked) never exceed kPool: fresh ones are admitted only while
-      // there is room, so the two stacks sharing the pool cannot collide.
-      const int nS = min(cntS, 32);                                   // lanes [0, nS): photons that left a panel
-      const int room = kPool - (cntT + cntS + 32 - __popc(m_pop));
-      const int nF = max(0, min(32 - nS, room));                      // lanes [nS, nS + nF): new photons
-      Photon q; uint64_t hq = 0; bool active = lane < nS;
-      if (active) pool_load(W.pool, kPool - 1 - (cntS - 1 - lane), q, hq);
-      cntS -= nS;
-      __syncwarp();
+    const int nS = min(cS, 32);
+    const int nF = more_src ? min(32 - nS, cF) : 0;                    // fresh photons SEARCH may admit (one free slot each)
+    int phase = L_SEARCH, best = cS + nF;
+    if (cT > 0 && cT >= best) { phase = L_STEP; best = cT; }
+    if (cK > best) { phase = L_KN; best = cK; }
+    if (cP > best) { phase = L_PHANTOM; best = cP; }
+    if (cR > best) { phase = L_RAY; best = cR; }
+    if (best == 0) break;                                             // nothing in flight, no source left
+
+    if (phase == L_SEARCH) {
+      // ---------------------------------------------- SEARCH: photons that left a panel + fresh ones from the source
+      Photon q = {}; uint64_t hq = 0; int idx = -1; bool active = lane < nS;
+      if (active) { idx = W.list[L_SEARCH][cS - 1 - lane]; slot_load(W, idx, q, hq); }
+      cS -= nS;
       if (nF > 0) {                                                   // source sampling (S3) [R13-R15]
         if (w_next >= w_end && !exhausted) {
           unsigned long long b = 0;
@@ -310,7 +307,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
         w_next = min(w_next + (uint64_t)nF, w_end);
         if (fresh) {
           active = true;
-          q.pair = (uint32_t)(j >> 1); q.meta = (uint32_t)(j & 1u) | (63u << 5); q.ndraw = 0; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
+          q.pair = (uint32_t)(j >> 1); q.meta = (uint32_t)(j & 1u) | (63u << 5); q.ids = kNone; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
           if (HASH) hq = 0xCBF29CE484222325ull;
           const uint64_t history = first_history + q.pair;
           const uint32_t h_lo = (uint32_t)history, h_hi = (uint32_t)(history >> 32);
@@ -336,53 +333,46 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
         }
       }
       // panel search [R6]; photons born inside a phantom skip it and are tracked there first [R17]
-      bool park = false;
+      int dest = L_NONE;
       if (active) {
-        if ((q.meta >> 11) & 1u) park = true;
+        if (ph_in_phantom(q)) dest = L_PHANTOM;
         else {
           float bt; const int bp = panel_search(g, q.x, q.d, ph_panel(q), bt);
-          if (bp < 0) { if (HASH) { hash_ev(hq, EV_ESCAPE, 0); hash_out[2ull * q.pair + (q.meta & 1u)] = hq; } }
-          else {
+          if (bp < 0) {
+            if (HASH) { hash_ev(hq, EV_ESCAPE, 0); hash_out[2ull * q.pair + (q.meta & 1u)] = hq; }
+            if (idx >= 0) dest = L_FREE;                              // gives its slot back
+          } else {
             if (HASH) hash_ev(hq, EV_ENTER, (uint32_t)bp);
             float xl[3], dl[3];
-            to_local(g.pose[bp], q.x, q.d, xl, dl);
+            to_local(g.panel[bp].pose, q.x, q.d, xl, dl);
 #pragma unroll
             for (int k = 0; k < 3; ++k) { q.x[k] = fmaf(bt, dl[k], xl[k]); q.d[k] = dl[k]; }   // [R18]
             q.path += bt; ph_set_panel(q, bp);
             q.inv_mu = rcp_fast(mu_lookup(mu, T, 0, q.E).w);
-            park = true;
+            dest = L_STEP;
           }
         }
       }
-      const unsigned m_park = __ballot_sync(0xFFFFFFFFu, park);
-      if (park) pool_store(W.pool, cntT + __popc(m_park & lt_mask), q, hq);
-      cntT += __popc(m_park);
+      const bool need = idx < 0 && dest != L_NONE;                    // a fresh photon that goes on takes a free slot
+      const unsigned m_need = __ballot_sync(0xFFFFFFFFu, need);
+      if (need) idx = W.list[L_FREE][cF - 1 - __popc(m_need & lt_mask)];
+      cF -= __popc(m_need);
+      if (dest == L_STEP || dest == L_PHANTOM) slot_store(W, idx, q, hq);
+      push(L_FREE, cF, dest == L_FREE, idx);
+      push(L_STEP, cT, dest == L_STEP, idx);
+      if (use_phantom) push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
       __syncwarp();
       continue;
     }
-    // ================================================ TRANSPORT: run the phase most lanes are waiting for
-    int phase = ST_NONE, best = min(__popc(m_pop), cntT);
-    if (best) phase = ST_POP;
-    { int c;
-      c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_STEP));     if (c > best) { best = c; phase = ST_STEP; }
-      c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_COMPTON));  if (c > best) { best = c; phase = ST_COMPTON; }
-      c = __popc(__ballot_sync(0xFFFFFFFFu, st == ST_PHANTOM));  if (c > best) { best = c; phase = ST_PHANTOM; } }
-    if (phase == ST_NONE) break;                                      // nothing in flight, nothing parked, no source left
-
-    if (phase == ST_POP) {
-      // ------------------------------------------------ POP: idle lanes take a parked photon from pool T
-      const int r = __popc(m_pop & lt_mask);
-      if (st == ST_POP && r < cntT) {
-        pool_load(W.pool, cntT - 1 - r, p, h);
-        st = ((p.meta >> 11) & 1u) ? ST_PHANTOM : ST_STEP;
-      }
-      cntT -= min(__popc(m_pop), cntT);
-      __syncwarp();
-    } else if (phase == ST_STEP) {
-      // ------------------------------------------------ STEP: Woodcock step, layer selection, lattice lookup [R19]
-      bool hit = false, leave = false; float xg[3] = {0.f, 0.f, 0.f};
-      if (st == ST_STEP) {
-        const uint4 w = next_block();                                 // [R4] free path, outcome, Rayleigh polar + azimuth
+    if (phase == L_STEP) {
+      // ---------------------------------------------- STEP: Woodcock step, layer selection, lattice lookup [R19]
+      const int n = min(cT, 32); const bool act = lane < n;
+      Photon p = {}; uint64_t h = 0; int idx = 0;
+      if (act) { idx = W.list[L_STEP][cT - 1 - lane]; slot_load(W, idx, p, h); }
+      cT -= n;
+      int dest = L_NONE; bool hit = false; float xg[3] = {0.f, 0.f, 0.f};
+      if (act) {
+        const uint4 w = next_block(p);                                // [R4] free path, outcome, Rayleigh polar + azimuth
         const float s = -__logf(u01(w.x)) * p.inv_mu;
         float tf = INFINITY;
 #pragma unroll
@@ -394,8 +384,8 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
           const float xl[3] = { fmaf(tf, p.d[0], p.x[0]), fmaf(tf, p.d[1], p.x[1]), fmaf(tf, p.d[2], p.x[2]) };
           const float dl[3] = { p.d[0], p.d[1], p.d[2] };
           p.path += tf; if (HASH) hash_ev(h, EV_EXIT, (uint32_t)panel);
-          point_to_global(g.pose[panel], xl, p.x); dir_to_global(g.pose[panel], dl, p.d);
-          leave = true; st = ST_POP;
+          point_to_global(g.panel[panel].pose, xl, p.x); dir_to_global(g.panel[panel].pose, dl, p.d);
+          dest = L_SEARCH;
         } else {
 #pragma unroll
           for (int k = 0; k < 3; ++k) p.x[k] = fmaf(s, p.d[k], p.x[k]);
@@ -403,32 +393,42 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
           uint32_t id;                                                // depth -> layer -> crystal
           const int mat = lattice_lookup(g, __float2int_rd(p.x[0] * kQ) + g.hWq, __float2int_rd(p.x[1] * kQ) + g.hHq,
                                          __float2int_rd(p.x[2] * kQ), id);
+          dest = L_STEP;
           if (mat < 0) { if (HASH) hash_ev(h, EV_STEP_VACUUM, 0); }
           else {
             if (id != kNone) id |= (uint32_t)panel << 26;
             const float4 m4 = mu_lookup(mu, T, mat, p.E);
             const float t = u01(w.y) * m4.w;                          // [R20] one draw picks the outcome
-            ids = id;
+            p.ids = id;
             if (t < m4.x) {                                           // photoelectric: deposit E, end
               if (HASH) { hash_ev(h, EV_PE, id); hash_out[2ull * p.pair + (p.meta & 1u)] = h; }
-              if (id != kNone) { hit = true; point_to_global(g.pose[panel], p.x, xg); }
-              st = ST_POP;
-            } else if (t < m4.y) st = ST_COMPTON;
-            else if (t < m4.z) { rayleigh(p.d, u01(w.z), u01(w.w)); if (HASH) hash_ev(h, EV_RAYLEIGH, id); }
+              if (id != kNone) { hit = true; point_to_global(g.panel[panel].pose, p.x, xg); }
+              dest = L_FREE;
+            } else if (t < m4.y) dest = L_KN;
+            else if (t < m4.z) { dest = L_RAY; if (HASH) hash_ev(h, EV_RAYLEIGH, id); }   // deflected in its own pass
             else if (HASH) hash_ev(h, EV_VIRTUAL, id);
           }
         }
       }
-      stage_hits(hit, ids | ((p.meta & 1u) << 4) | ((p.meta >> 1) & 15u), xg, p.E, p.path * kInvC);
-      park_leavers(leave);
-    } else if (phase == ST_COMPTON) {
-      // ------------------------------------------------ COMPTON: one Klein-Nishina trial per visit [R20]
-      bool hit = false; float xg[3] = {0.f, 0.f, 0.f}, e_dep = 0.f;
-      if (st == ST_COMPTON) {
-        const bool in_ph = (p.meta >> 11) & 1u;
+      stage_hits(hit, p.pair, p.ids | ((p.meta & 1u) << 4) | ((p.meta >> 1) & 15u), xg, p.E, p.path * kInvC);
+      if (act && dest != L_FREE) slot_store(W, idx, p, h);
+      push(L_STEP, cT, dest == L_STEP, idx);
+      push(L_SEARCH, cS, dest == L_SEARCH, idx);
+      push(L_KN, cK, dest == L_KN, idx);
+      push(L_FREE, cF, dest == L_FREE, idx);
+      push(L_RAY, cR, dest == L_RAY, idx);
+    } else if (phase == L_KN) {
+      // ---------------------------------------------- KN: one Klein-Nishina trial per visit [R20]
+      const int n = min(cK, 32); const bool act = lane < n;
+      Photon p = {}; uint64_t h = 0; int idx = 0;
+      if (act) { idx = W.list[L_KN][cK - 1 - lane]; slot_load(W, idx, p, h); }
+      cK -= n;
+      int dest = L_NONE; bool hit = false; float xg[3] = {0.f, 0.f, 0.f}, e_dep = 0.f; uint32_t hit_ids = 0;
+      if (act) {
+        const bool in_ph = ph_in_phantom(p);
         const float k = p.E * (1.0f / kMec2), e0 = rcp_fast(1.0f + 2.0f * k), e02 = e0 * e0;
         const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
-        const uint4 w = next_block();                                 // [R4] u_a, u_b, u_c, azimuth
+        const uint4 w = next_block(p);                                // [R4] u_a, u_b, u_c, azimuth
         const float ua = u01(w.x), ub = u01(w.y), uc = u01(w.z);
         // om = 1 - eps and em = eps - eps0 are formed without cancellation, so that sin^2 = t (2 - t) keeps
         // full relative accuracy at both poles (t = om/(k eps), 2 - t = em/(eps0 k eps)); plain fp32 loses
@@ -444,31 +444,59 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
         const float ike = rcp_fast(k * eps);
         const float t = om * ike, tm = em * ike * (1.0f + 2.0f * k);
         const float gr = 1.0f - eps * t * tm * rcp_fast(1.0f + eps * eps);
-        if (gr >= uc || (p.meta >> 12) >= 63u) {                      // accepted [R22: the 64th trial always is]
-          p.meta &= 0xFFFu;
+        dest = L_KN;
+        if (gr >= uc || ((p.meta >> 12) & 63u) >= 63u) {              // accepted [R22: the 64th trial always is]
+          p.meta &= ~(63u << 12);
           float sp, cp; sincos_2pi(u01(w.w), sp, cp);
           rotate(p.d, 1.0f - t, sqrt_fast(fmaxf(t * tm, 0.0f)), cp, sp);
           const float dep = om * p.E, E2 = p.E - dep;
           const bool cut = E2 < kCutoff;                              // [R12]
           if (in_ph) {
             if (HASH) { hash_ev(h, EV_PH_COMPTON, 0); if (cut) hash_ev(h, EV_PH_CUTOFF, 0); }
-            if (!cut) { p.E = E2; p.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, p.E).z); st = ST_PHANTOM; }
+            if (!cut) { p.E = E2; p.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, p.E).z); dest = L_PHANTOM; }
           } else {
-            if (HASH) { hash_ev(h, EV_COMPTON, ids); if (cut) hash_ev(h, EV_CUTOFF, ids); }
-            if (ids != kNone) { hit = true; e_dep = cut ? p.E : dep; point_to_global(g.pose[ph_panel(p)], p.x, xg); }
-            if (!cut) { p.E = E2; p.inv_mu = rcp_fast(mu_lookup(mu, T, 0, p.E).w); st = ST_STEP; }
+            if (HASH) { hash_ev(h, EV_COMPTON, p.ids); if (cut) hash_ev(h, EV_CUTOFF, p.ids); }
+            if (p.ids != kNone) {
+              hit = true; e_dep = cut ? p.E : dep; point_to_global(g.panel[ph_panel(p)].pose, p.x, xg);
+              const uint32_t seq = (p.meta >> 1) & 15u;
+              hit_ids = p.ids | ((p.meta & 1u) << 4) | seq;
+              if (seq < 15u) p.meta += 2u;                            // [R9] 4-bit saturating hit counter
+            }
+            if (!cut) { p.E = E2; p.inv_mu = rcp_fast(mu_lookup(mu, T, 0, p.E).w); dest = L_STEP; }
           }
-          if (cut) { if (HASH) hash_out[2ull * p.pair + (p.meta & 1u)] = h; st = ST_POP; }
+          if (cut) { if (HASH) hash_out[2ull * p.pair + (p.meta & 1u)] = h; dest = L_FREE; }
         } else p.meta += 1u << 12;
       }
-      const uint32_t seq = (p.meta >> 1) & 15u;
-      stage_hits(hit, ids | ((p.meta & 1u) << 4) | seq, xg, e_dep, p.path * kInvC);
-      if (hit && seq < 15u) p.meta += 2u;                             // [R9] 4-bit saturating hit counter
+      stage_hits(hit, p.pair, hit_ids, xg, e_dep, p.path * kInvC);
+      if (act && dest != L_FREE) slot_store(W, idx, p, h);
+      push(L_KN, cK, dest == L_KN, idx);
+      push(L_STEP, cT, dest == L_STEP, idx);
+      push(L_FREE, cF, dest == L_FREE, idx);
+      if (use_phantom) push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
+    } else if (phase == L_RAY) {
+      // ---------------------------------------------- RAY: Rayleigh deflection with words 2-3 of the step's block [R4, R20]
+      const int n = min(cR, 32); const bool act = lane < n;
+      Photon p = {}; uint64_t h = 0; int idx = 0;
+      if (act) { idx = W.list[L_RAY][cR - 1 - lane]; slot_load(W, idx, p, h); }
+      cR -= n;
+      int dest = L_NONE;
+      if (act) {
+        const uint4 w = block_at(p, (p.meta >> 18) - 1u);             // the block its Woodcock step drew (rare event: recomputed)
+        rayleigh(p.d, u01(w.z), u01(w.w));
+        dest = ph_in_phantom(p) ? L_PHANTOM : L_STEP;
+        slot_store(W, idx, p, h);
+      }
+      push(L_STEP, cT, dest == L_STEP, idx);
+      if (use_phantom) push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
     } else {
-      // ------------------------------------------------ PHANTOM: Woodcock tracking in the voxel grid [R17]
-      bool leave = false;
-      if (st == ST_PHANTOM) {
-        const uint4 w = next_block();                                 // [R4]
+      // ---------------------------------------------- PHANTOM: Woodcock tracking in the voxel grid [R17]
+      const int n = min(cP, 32); const bool act = lane < n;
+      Photon p = {}; uint64_t h = 0; int idx = 0;
+      if (act) { idx = W.list[L_PHANTOM][cP - 1 - lane]; slot_load(W, idx, p, h); }
+      cP -= n;
+      int dest = L_NONE;
+      if (act) {
+        const uint4 w = next_block(p);                                // [R4]
         const float s = -__logf(u01(w.x)) * p.inv_mu;
         int v[3]; bool out = false; float xt[3];
 #pragma unroll
@@ -478,21 +506,28 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
           out = out || v[k] < 0 || v[k] >= src.dims[k];
         }
         // tentative point outside the grid: the photon leaves along its line of flight from where it is [R17]
-        if (out) { if (HASH) hash_ev(h, EV_PH_LEAVE, 0); p.meta &= ~(1u << 11); leave = true; st = ST_POP; }
+        if (out) { if (HASH) hash_ev(h, EV_PH_LEAVE, 0); p.meta &= ~(1u << 11); dest = L_SEARCH; }
         else {
           p.x[0] = xt[0]; p.x[1] = xt[1]; p.x[2] = xt[2]; p.path += s;
+          dest = L_PHANTOM;
           const int mat = (int)src.phantom[((size_t)v[2] * src.dims[1] + v[1]) * src.dims[0] + v[0]] - 1;
           if (mat >= 0) {
             const float4 m4 = mu_lookup(mu, T, mat, p.E);
             const float t = u01(w.y) * mu_lookup(mu, T, src.ph_major, p.E).z;
-            if (t < m4.x) { if (HASH) { hash_ev(h, EV_PH_ABSORBED, 0); hash_out[2ull * p.pair + (p.meta & 1u)] = h; } st = ST_POP; }
-            else if (t < m4.y) st = ST_COMPTON;
-            else if (t < m4.z) { rayleigh(p.d, u01(w.z), u01(w.w)); if (HASH) hash_ev(h, EV_PH_RAYLEIGH, 0); }
+            if (t < m4.x) { if (HASH) { hash_ev(h, EV_PH_ABSORBED, 0); hash_out[2ull * p.pair + (p.meta & 1u)] = h; } dest = L_FREE; }
+            else if (t < m4.y) dest = L_KN;
+            else if (t < m4.z) { dest = L_RAY; if (HASH) hash_ev(h, EV_PH_RAYLEIGH, 0); }
           }
         }
+        if (dest != L_FREE) slot_store(W, idx, p, h);
       }
-      park_leavers(leave);
+      push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
+      push(L_SEARCH, cS, dest == L_SEARCH, idx);
+      push(L_KN, cK, dest == L_KN, idx);
+      push(L_FREE, cF, dest == L_FREE, idx);
+      push(L_RAY, cR, dest == L_RAY, idx);
     }
+    __syncwarp();
   }
 
   // ------------------------------------------------ drain the staged hits (fewer than 32 per warp)
@@ -504,15 +539,15 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
   }
 }
 
-size_t transport_smem_bytes(const DevTables &T, bool hash) {
-  const size_t fixed = hash ? sizeof(Smem<true>) : sizeof(Smem<false>);
-  return fixed - sizeof(float4) + sizeof(float4) * (size_t)T.n_staged * T.n_energies + 16;
+size_t transport_smem_bytes(const DevTables &T, int n_panels, bool hash) {
+  const int n_mu = T.n_staged * T.n_energies;
+  return (hash ? SmemLayout<true>::geom_off(n_mu) : SmemLayout<false>::geom_off(n_mu)) + geom_bytes(n_panels);
 }
 
-cudaError_t launch_transport(const DevGeom *geom, const DevTables &T, const DevSource &src,
+cudaError_t launch_transport(const DevGeom *geom, int n_panels, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
                              unsigned long long *work_counter, int sm_count, cudaStream_t stream) {
-  const size_t smem = transport_smem_bytes(T, hash_out != nullptr);
+  const size_t smem = transport_smem_bytes(T, n_panels, hash_out != nullptr);
   const uint64_t n_photons = 2 * n_pairs;
   const uint64_t want = (n_photons + kThreads - 1) / kThreads;
   static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : 3;
@@ -549,7 +584,7 @@ __global__ void locate_kernel(const DevGeom *geom, int64_t n, const float *xyz, 
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
     uint32_t out = kNone;
     for (int p = 0; p < g.n_panels; ++p) {
-      const float *P = g.pose[p];
+      const float *P = g.panel[p].pose;
       const double r0 = (double)xyz[3 * i] - (double)P[0], r1 = (double)xyz[3 * i + 1] - (double)P[1], r2 = (double)xyz[3 * i + 2] - (double)P[2];
       const double a = r0 * P[3] + r1 * P[4] + r2 * P[5], b = r0 * P[6] + r1 * P[7] + r2 * P[8], c = r0 * P[9] + r1 * P[10] + r2 * P[11];
       const long long qa = (long long)floor(a * 1048576.0) + g.hWq, qb = (long long)floor(b * 1048576.0) + g.hHq, qc = (long long)floor(c * 1048576.0);

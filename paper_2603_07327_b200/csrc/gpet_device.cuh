@@ -25,7 +25,8 @@ struct DevLayer {
 struct __align__(16) DevPanel {
   float pose[12];             // front-face centre, u, v, w
   float cx, cy, cz, pad;      // global position of the box centre (search culling)
-};
+  float skew[4];              // 80-byte stride: records of 8 consecutive panels start in 8 different 16-byte bank groups, so
+};                            // lanes reading the poses of different panels (entry / exit / hit transforms) rarely conflict
 struct DevGeom {
   int n_panels, n_layers;
   int Wq, Hq, Dq, hWq, hHq;

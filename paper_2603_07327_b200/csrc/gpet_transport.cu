@@ -22,7 +22,13 @@ namespace gpet {
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 constexpr int kStage = 64;            // staged hits per warp (ring buffer)
-constexpr int kSlots = 96;            // photon slots per warp
+#ifndef GPET_SLOTS
+#define GPET_SLOTS 96
+#endif
+#ifndef GPET_MIN_CTAS
+#define GPET_MIN_CTAS 3
+#endif
+constexpr int kSlots = GPET_SLOTS;    // photon slots per warp
 constexpr uint32_t kChunk = 1024;     // photon indices a warp reserves at a time
 
 enum : int { L_FREE = 0, L_SEARCH, L_STEP, L_KN, L_RAY, L_PHANTOM, kLists, L_NONE = kLists };
@@ -154,17 +160,19 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
     const float iz = rcp_dir(d[2]);
     const float z1 = (g.blo[1] - x[2]) * iz, z2 = (g.bhi[1] - x[2]) * iz;
     const float tnz = fmaxf(fminf(z1, z2), 0.0f), tfz = fmaxf(z1, z2);
-    const float sr = g.cull_r2 * sqrt_fast(fmaf(d[0], d[0], d[1] * d[1]));
+    // circle test in the form cross = c x d - L, dot = c . d - M with L = x x d, M = x . d (four FMAs per panel); the
+    // 1e-4 mm of absolute slack covers the cancellation error of that form for nearly axial rays
+    const float sr = fmaf(g.cull_r2, sqrt_fast(fmaf(d[0], d[0], d[1] * d[1])), 1e-4f);
+    const float Lz = fmaf(x[0], d[1], -x[1] * d[0]), Mz = fmaf(x[0], d[0], x[1] * d[1]);
     const bool axial_ok = tfz > tnz;
     for (int base = 0; base < g.n_panels; base += 32) {
       const int nq = min(32, g.n_panels - base);
-      uint32_t cand = 0;
+      uint32_t cand = 0, bit = 1u;
 #pragma unroll 4
-      for (int q = 0; q < nq; ++q) {
+      for (int q = 0; q < nq; ++q, bit <<= 1) {
         const DevPanel &c = g.panel[base + q];
-        const float rx = c.cx - x[0], ry = c.cy - x[1];
-        const float cross = fmaf(rx, d[1], -ry * d[0]), dot = fmaf(rx, d[0], ry * d[1]);
-        if (fabsf(cross) <= sr && dot >= -sr) cand |= 1u << q;
+        const float cross = fmaf(c.cx, d[1], fmaf(-c.cy, d[0], -Lz)), dot = fmaf(c.cx, d[0], fmaf(c.cy, d[1], -Mz));
+        if (fmaxf(fabsf(cross), -dot) <= sr) cand |= bit;                  // |cross| <= sr and dot >= -sr
       }
       if ((unsigned)(excl - base) < 32u) cand &= ~(1u << (excl - base));
       if (!axial_ok) cand = 0;
@@ -213,7 +221,7 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
 
 // ---------------------------------------------------------------- the kernel
 template <bool HASH>
-__global__ void __launch_bounds__(kThreads, 3)
+__global__ void __launch_bounds__(kThreads, GPET_MIN_CTAS)
 transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint64_t first_history, uint64_t n_photons,
                            const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -550,7 +558,7 @@ cudaError_t launch_transport(const DevGeom *geom, int n_panels, const DevTables 
   const size_t smem = transport_smem_bytes(T, n_panels, hash_out != nullptr);
   const uint64_t n_photons = 2 * n_pairs;
   const uint64_t want = (n_photons + kThreads - 1) / kThreads;
-  static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : 3;
+  static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : GPET_MIN_CTAS;
   const uint64_t resident = (uint64_t)sm_count * ctas_per_sm;         // persistent grid
   PhiloxKeys key;                                                     // [R1] round keys: key + r * Weyl constants
   for (int r = 0; r < 10; ++r) { key.k[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; key.k[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }

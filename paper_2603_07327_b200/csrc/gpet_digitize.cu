@@ -36,44 +36,76 @@ __device__ __forceinline__ uint32_t block_exclusive_scan_256(uint32_t v, uint32_
   return base + inc - v;
 }
 
-__global__ void __launch_bounds__(256) scan_reduce_kernel(const uint32_t *in, uint64_t n, uint32_t *bsum) {
-  const uint64_t base = (uint64_t)blockIdx.x * kTile;
-  uint32_t s = 0;
-#pragma unroll
-  for (int k = 0; k < 8; ++k) { const uint64_t i = base + (uint64_t)k * 256 + threadIdx.x; if (i < n) s += in[i]; }
-  uint32_t tot; block_exclusive_scan_256(s, &tot);
-  if (threadIdx.x == 0) bsum[blockIdx.x] = tot;
-}
-// single block: exclusive scan of the block sums in place; total -> bsum[nb] and (optionally) a u64 counter
-__global__ void __launch_bounds__(256) scan_bsums_kernel(uint32_t *bsum, uint32_t nb, unsigned long long *total_out) {
-  uint32_t carry = 0;
-  for (uint32_t start = 0; start < nb; start += 256) {
-    const uint32_t i = start + threadIdx.x;
-    const uint32_t v = i < nb ? bsum[i] : 0u;
-    uint32_t tot; const uint32_t ex = block_exclusive_scan_256(v, &tot);
-    if (i < nb) bsum[i] = carry + ex;
-    carry += tot;
-  }
-  if (threadIdx.x == 0) { bsum[nb] = carry; if (total_out) *total_out = carry; }
-}
-// out[i] = exclusive prefix of in; out[n] = total (out has n+1 entries; may alias in only if out == in and n+1 fits)
-__global__ void __launch_bounds__(256) scan_apply_kernel(const uint32_t *in, uint64_t n, const uint32_t *bsum, uint32_t nb, uint32_t *out) {
-  const uint64_t base = (uint64_t)blockIdx.x * kTile + (uint64_t)threadIdx.x * 8;
+// Single-pass exclusive scan with decoupled look-back (one read and one write of the data).  Tiles take tickets
+// from an atomic counter, so a tile only ever waits for tiles that are already running or done; a tile publishes
+// its aggregate (flag 1) as soon as it is known and its inclusive prefix (flag 2) after the look-back.
+// out[i] = sum of in[0..i), out[n] = total; n = min(*n_dev, n_host) when n_dev is given (lengths known only on
+// the device).  state: [0] ticket counter, [1 + tile] = flag << 62 | value; zeroed by the caller.
+__global__ void __launch_bounds__(256) scan_lookback_kernel(const uint32_t *in, uint64_t n_host, const uint32_t *n_dev, uint32_t *out,
+                                                            unsigned long long *state, unsigned long long *total_out) {
+  __shared__ uint32_t s_tile, s_prefix;
+  if (threadIdx.x == 0) s_tile = (uint32_t)atomicAdd(&state[0], 1ull);
+  __syncthreads();
+  const uint32_t tile = s_tile;
+  uint64_t n = n_host;
+  if (n_dev) { const uint64_t nd = *n_dev; if (nd < n) n = nd; }
+  const uint32_t ntiles = n ? (uint32_t)((n + kTile - 1) / kTile) : 1u;
+  if (tile >= ntiles) return;
+  const uint64_t base = (uint64_t)tile * kTile + (uint64_t)threadIdx.x * 8;
   uint32_t v[8], s = 0;
+  if (base + 8 <= n) {
+    const uint4 a = *reinterpret_cast<const uint4 *>(in + base), b = *reinterpret_cast<const uint4 *>(in + base + 4);
+    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+  } else {
 #pragma unroll
-  for (int k = 0; k < 8; ++k) { v[k] = base + k < n ? in[base + k] : 0u; s += v[k]; }
-  uint32_t tot; uint32_t ex = block_exclusive_scan_256(s, &tot) + bsum[blockIdx.x];
+    for (int k = 0; k < 8; ++k) v[k] = base + k < n ? in[base + k] : 0u;
+  }
 #pragma unroll
-  for (int k = 0; k < 8; ++k) { if (base + k < n) out[base + k] = ex; ex += v[k]; }
-  if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = bsum[nb];
+  for (int k = 0; k < 8; ++k) s += v[k];
+  uint32_t tot; uint32_t ex = block_exclusive_scan_256(s, &tot);
+  if (threadIdx.x < 32) {                                            // warp 0: publish, then look back 32 tiles at a time
+    volatile unsigned long long *st = state + 1;
+    const int lane = threadIdx.x;
+    uint32_t prefix = 0;
+    if (tile > 0) {
+      if (lane == 0) st[tile] = (1ull << 62) | tot;
+      for (int j = (int)tile - 1;; j -= 32) {
+        const int jj = j - lane;
+        unsigned long long w = 2ull << 62;                            // before tile 0: an inclusive prefix of 0
+        if (jj >= 0) do { w = st[jj]; } while ((w >> 62) == 0ull);
+        const unsigned incl = __ballot_sync(0xFFFFFFFFu, (w >> 62) == 2ull);
+        const int first = incl ? __ffs(incl) - 1 : 31;                // nearest predecessor that already knows its prefix
+        uint32_t part = lane <= first ? (uint32_t)w : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xFFFFFFFFu, part, o);
+        prefix += part;
+        if (incl) break;
+      }
+    }
+    if (lane == 0) {
+      st[tile] = (2ull << 62) | (unsigned long long)(prefix + tot);
+      s_prefix = prefix;
+      if (tile == ntiles - 1) { out[n] = prefix + tot; if (total_out) *total_out = prefix + tot; }
+    }
+  }
+  __syncthreads();
+  ex += s_prefix;
+  if (base + 8 <= n) {
+    uint4 a, b;
+    a.x = ex; ex += v[0]; a.y = ex; ex += v[1]; a.z = ex; ex += v[2]; a.w = ex; ex += v[3];
+    b.x = ex; ex += v[4]; b.y = ex; ex += v[5]; b.z = ex; ex += v[6]; b.w = ex;
+    *reinterpret_cast<uint4 *>(out + base) = a; *reinterpret_cast<uint4 *>(out + base + 4) = b;
+  } else {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { if (base + k < n) out[base + k] = ex; ex += v[k]; }
+  }
 }
 
-static cudaError_t exclusive_scan(const uint32_t *in, uint64_t n, uint32_t *out, uint32_t *bsum, unsigned long long *total_out, cudaStream_t st) {
-  const uint32_t nb = (uint32_t)((n + kTile - 1) / kTile);
-  scan_reduce_kernel<<<nb, 256, 0, st>>>(in, n, bsum);
-  scan_bsums_kernel<<<1, 256, 0, st>>>(bsum, nb, total_out);
-  scan_apply_kernel<<<nb, 256, 0, st>>>(in, n, bsum, nb, out);
-  count_launch(3);
+static cudaError_t exclusive_scan(const uint32_t *in, uint64_t n_host, const uint32_t *n_dev, uint32_t *out, unsigned long long *state,
+                                  unsigned long long *total_out, cudaStream_t st) {
+  const uint32_t nb = n_host ? (uint32_t)((n_host + kTile - 1) / kTile) : 1u;
+  scan_lookback_kernel<<<nb, 256, 0, st>>>(in, n_host, n_dev, out, state, total_out);
+  count_launch(1);
   return cudaGetLastError();
 }
 
@@ -94,22 +126,23 @@ __device__ __forceinline__ uint32_t valid_hits(const HitBuf &H, uint32_t bound) 
   const unsigned long long n = *H.n_hits, c = H.capacity < bound ? H.capacity : bound;
   return (uint32_t)(n < c ? n : c);
 }
-__global__ void __launch_bounds__(256) count_hits_kernel(HitBuf H, uint32_t bound, uint32_t first_lo, uint32_t n_pairs, uint32_t *cnt) {
+// the atomic's return value is the hit's rank inside its history: kept (coalesced) so that the scatter needs no atomics
+__global__ void __launch_bounds__(256) count_hits_kernel(HitBuf H, uint32_t bound, uint32_t first_lo, uint32_t n_pairs, uint32_t *cnt, uint32_t *hrank) {
   const uint32_t n_hits = valid_hits(H, bound); const uint32_t *history = H.history;
   for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n_hits; i += gridDim.x * 256u) {
     const uint32_t h = history[i] - first_lo;
-    if (h < n_pairs) atomicAdd(&cnt[h], 1u);
+    if (h < n_pairs) hrank[i] = atomicAdd(&cnt[h], 1u);
   }
 }
 // reads the struct-of-arrays hit buffer coalesced, writes each hit as one sector into its history's segment
 __global__ void __launch_bounds__(256) scatter_hits_kernel(HitBuf H, uint32_t bound, uint32_t first_lo, uint32_t n_pairs,
-                                                           const uint32_t *off, uint32_t *cnt, HitRec *rec) {
+                                                           const uint32_t *off, const uint32_t *hrank, HitRec *rec) {
   const uint32_t n_hits = valid_hits(H, bound);
   for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n_hits; i += gridDim.x * 256u) {
     const uint32_t h = H.history[i] - first_lo;
     if (h >= n_pairs) continue;
     HitRec r; r.ids = H.ids[i]; r.x = H.x[i]; r.y = H.y[i]; r.z = H.z[i]; r.e = H.e[i]; r.tof = H.tof[i]; r.idx = i; r.pad = h;
-    store_rec(&rec[off[h] + atomicSub(&cnt[h], 1u) - 1u], &r);
+    store_rec(&rec[off[h] + hrank[i]], &r);
   }
 }
 
@@ -131,77 +164,96 @@ __device__ __forceinline__ double decay_time(const DigiParams &P, uint64_t histo
   return __dmul_rn(__dadd_rn((double)slice, u53), P.slice_s);                               // slice_s = B / A
 }
 
-// blur [R25], window [R26], absolute time [R16]; a kept single goes to the next slot of its history's segment
-// (no global append counter: slots not used are marked invalid by the caller) and is counted into its time bucket
-__device__ __forceinline__ void emit_single(const DigiParams &P, const Buckets &B, uint64_t history, uint32_t unit, float e_sum,
-                                            const HitRec &best, float tof_min, SinRec *sing, uint32_t &slot, uint32_t *bcnt) {
-  const uint2 key = make_uint2((uint32_t)P.seed, (uint32_t)(P.seed >> 32));
-  const uint4 w = philox4x32_10(make_uint4((uint32_t)history, 0u, 3u, unit), key);           // Box-Muller on words 0,1
-  const float nrm = sqrtf(-2.0f * logf(u01(w.x))) * cospif(2.0f * u01(w.y));
-  const float sigma = P.sigma_scale * (P.ref_keV > 0.0f ? sqrtf(P.ref_keV * e_sum) : e_sum);
-  const float e_b = fmaf(sigma, nrm, e_sum);
-  if (!(e_b >= P.e_lo && e_b < P.e_hi)) return;
-  SinRec s; s.t = __dadd_rn(decay_time(P, history), __dmul_rn((double)tof_min, 1e-9));
-  s.history = (uint32_t)history; s.ids = best.ids; s.x = best.x; s.y = best.y; s.z = best.z; s.e = e_b;
-  store_rec(&sing[slot++], &s);
-  atomicAdd(&bcnt[bucket_of(B, s.t)], 1u);
-}
+// A group of hits of one (history, readout unit) after the adder, before blur: what phase 2 of the kernel needs.
+struct Cand { uint32_t h, unit, best; float e_sum, tof_min; };
 
-// One thread per hit record (all lanes busy; a thread per history would idle on the ~54 % of histories without
-// hits).  The record with the smallest (ids, position) of its (history, readout unit) group is the group's
-// leader: it sums the group in ascending (ids, position) order -- canonical, so the fp32 sum does not depend
-// on the hit buffer's order -- picks the largest deposit and the earliest time [R24], and emits the single
-// into its own slot; every other slot is marked unused.
+// Phase 1, one thread per hit record (a thread per history would idle on the ~54 % of histories without hits): the
+// record with the smallest (ids, position) of its (history, readout unit) group is the group's leader; it sums the
+// group in ascending (ids, position) order -- canonical, so the fp32 sum does not depend on the hit buffer's order
+// -- and picks the largest deposit and the earliest time [R24].  The leaders of the block are then compacted into
+// shared memory (block scan), so that phase 2 -- blur [R25], window [R26], absolute time [R16] -- runs on dense
+// lanes; kept singles are appended with one atomic per warp and counted into their time bucket.  The append order
+// is free: the bucket sort that follows fixes the final order.
 __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uint64_t first_history, const uint32_t *off, const uint32_t *n_rec,
-                                                    const HitRec *rec, SinRec *sing, uint32_t *bcnt) {
+                                                    const HitRec *rec, SinRec *sing, uint32_t *srank, uint32_t *n_kept, uint32_t *bcnt) {
+  __shared__ Cand cand[256];
+  __shared__ uint32_t s_base;
   const uint32_t n = *n_rec;
-  for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n; i += gridDim.x * 256u) {
-    HitRec me; store_rec(&me, &rec[i]);
-    const uint32_t h = me.pad, b = off[h], k = off[h + 1] - b, unit = me.ids >> P.shift;
-    const uint64_t my_key = ((uint64_t)me.ids << 32) | i;
-    bool leader = true;
-    float e_sum = me.e, tof_min = me.tof; HitRec best = me;
-    if (k > 1) {
-      uint32_t members = 0;
-      for (uint32_t j = b; j < b + k; ++j) {
-        const uint32_t ids = rec[j].ids;
-        if ((ids >> P.shift) != unit) continue;
-        ++members;
-        if ((((uint64_t)ids << 32) | j) < my_key) leader = false;
-      }
-      if (leader && members > 1) {                                   // ascending (ids, position) after the leader itself
-        uint64_t prev = my_key; float e_best = me.e; uint32_t best_ord = me.ids & 31u;
-        for (uint32_t m = 1; m < members; ++m) {
-          uint64_t sel = ~0ull;
-          for (uint32_t j = b; j < b + k; ++j) {
-            const uint32_t ids = rec[j].ids;
-            const uint64_t key = ((uint64_t)ids << 32) | j;
-            if ((ids >> P.shift) == unit && key > prev && key < sel) sel = key;
+  const uint2 key = make_uint2((uint32_t)P.seed, (uint32_t)(P.seed >> 32));
+  for (uint32_t base = blockIdx.x * 256u; base < n; base += gridDim.x * 256u) {
+    const uint32_t i = base + threadIdx.x;
+    bool leader = false; Cand c = {0u, 0u, 0u, 0.f, 0.f};
+    if (i < n) {
+      const uint4 me = *reinterpret_cast<const uint4 *>(&rec[i]);      // ids, x, y, z
+      const uint4 m2 = *(reinterpret_cast<const uint4 *>(&rec[i]) + 1);  // e, tof, idx, history - first
+      const uint32_t my_ids = me.x, h = m2.w, b = off[h], k = off[h + 1] - b, unit = my_ids >> P.shift;
+      leader = true; c.h = h; c.unit = unit; c.best = i; c.e_sum = __uint_as_float(m2.x); c.tof_min = __uint_as_float(m2.y);
+      if (k > 1) {
+        const uint64_t my_key = ((uint64_t)my_ids << 32) | i;
+        uint32_t members = 0;
+        for (uint32_t j = b; j < b + k; ++j) {
+          const uint32_t ids = rec[j].ids;
+          if ((ids >> P.shift) != unit) continue;
+          ++members;
+          if ((((uint64_t)ids << 32) | j) < my_key) leader = false;
+        }
+        if (leader && members > 1) {                                 // ascending (ids, position) after the leader itself
+          uint64_t prev = my_key; float e_best = c.e_sum; uint32_t best_ord = my_ids & 31u;
+          for (uint32_t m = 1; m < members; ++m) {
+            uint64_t sel = ~0ull;
+            for (uint32_t j = b; j < b + k; ++j) {
+              const uint32_t ids = rec[j].ids;
+              const uint64_t kk = ((uint64_t)ids << 32) | j;
+              if ((ids >> P.shift) == unit && kk > prev && kk < sel) sel = kk;
+            }
+            prev = sel;
+            const HitRec &r = rec[(uint32_t)sel];
+            const float re = r.e; const uint32_t ord = (uint32_t)(sel >> 32) & 31u;
+            c.e_sum += re;
+            if (re > e_best || (re == e_best && ord < best_ord)) { e_best = re; c.best = (uint32_t)sel; best_ord = ord; }
+            c.tof_min = fminf(c.tof_min, r.tof);
           }
-          prev = sel;
-          HitRec r; store_rec(&r, &rec[(uint32_t)sel]);
-          const uint32_t ord = r.ids & 31u;
-          e_sum += r.e;
-          if (r.e > e_best || (r.e == e_best && ord < best_ord)) { e_best = r.e; best = r; best_ord = ord; }
-          tof_min = fminf(tof_min, r.tof);
         }
       }
     }
-    uint32_t slot = i;
-    if (leader) emit_single(P, B, first_history + h, unit, e_sum, best, tof_min, sing, slot, bcnt);
-    if (slot == i) sing[i].ids = kNone;                              // not a leader, or outside the energy window
+    uint32_t tot; const uint32_t ex = block_exclusive_scan_256(leader ? 1u : 0u, &tot);
+    if (leader) cand[ex] = c;
+    __syncthreads();
+    // ---- phase 2: dense lanes
+    bool keep = false; SinRec s;
+    if (threadIdx.x < tot) {
+      const Cand q = cand[threadIdx.x];
+      const uint64_t history = first_history + q.h;
+      const uint4 w = philox4x32_10(make_uint4((uint32_t)history, 0u, 3u, q.unit), key);       // Box-Muller on words 0,1
+      const float nrm = sqrtf(-2.0f * logf(u01(w.x))) * cospif(2.0f * u01(w.y));
+      const float sigma = P.sigma_scale * (P.ref_keV > 0.0f ? sqrtf(P.ref_keV * q.e_sum) : q.e_sum);
+      const float e_b = fmaf(sigma, nrm, q.e_sum);
+      keep = e_b >= P.e_lo && e_b < P.e_hi;
+      if (keep) {
+        const HitRec &r = rec[q.best];
+        s.t = __dadd_rn(decay_time(P, history), __dmul_rn((double)q.tof_min, 1e-9));
+        s.history = (uint32_t)history; s.ids = r.ids; s.x = r.x; s.y = r.y; s.z = r.z; s.e = e_b;
+      }
+    }
+    uint32_t nk; const uint32_t kx = block_exclusive_scan_256(keep ? 1u : 0u, &nk);      // one append per block, not per warp
+    if (threadIdx.x == 0 && nk) s_base = atomicAdd(n_kept, nk);
+    __syncthreads();
+    if (keep) {
+      const uint32_t o = s_base + kx;
+      store_rec(&sing[o], &s);
+      srank[o] = atomicAdd(&bcnt[bucket_of(B, s.t)], 1u);            // rank inside its time bucket (any order will do)
+    }
+    __syncthreads();
   }
 }
 
 // ---------------------------------------------------------------- stage 3: time-bucket counting sort
-__global__ void __launch_bounds__(256) bucket_scatter_kernel(const SinRec *sing, const uint32_t *n_slots, Buckets B,
-                                                             const uint32_t *boff, uint32_t *bcnt, SinRec *srt) {
-  const uint32_t n = *n_slots;                                       // = number of hits: one slot per hit
+__global__ void __launch_bounds__(256) bucket_scatter_kernel(const SinRec *sing, const uint32_t *srank, const uint32_t *n_slots, Buckets B,
+                                                             const uint32_t *boff, SinRec *srt) {
+  const uint32_t n = *n_slots;                                       // kept singles, append order
   for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n; i += gridDim.x * 256u) {
     SinRec s; store_rec(&s, &sing[i]);
-    if (s.ids == kNone) continue;
-    const uint32_t b = bucket_of(B, s.t);
-    store_rec(&srt[boff[b] + atomicSub(&bcnt[b], 1u) - 1u], &s);
+    store_rec(&srt[boff[bucket_of(B, s.t)] + srank[i]], &s);
   }
 }
 __device__ __forceinline__ bool single_less(const SinRec &a, const SinRec &b, int shift) {             // (t, history, unit)
@@ -209,42 +261,41 @@ __device__ __forceinline__ bool single_less(const SinRec &a, const SinRec &b, in
   if (a.history != b.history) return a.history < b.history;
   return (a.ids >> shift) < (b.ids >> shift);
 }
-// one thread per bucket (~0-3 singles): rank by counting, write the final time-ordered records and the caller's arrays
-__global__ void __launch_bounds__(256) bucket_sort_kernel(const SinRec *srt, int shift, uint32_t nb, const uint32_t *boff, SinRec *fin, SinglesBuf S) {
-  for (uint32_t b = blockIdx.x * 256u + threadIdx.x; b < nb; b += gridDim.x * 256u) {
-    const uint32_t s = boff[b], m = boff[b + 1] - s;
-    for (uint32_t j = 0; j < m; ++j) {
-      SinRec a; store_rec(&a, &srt[s + j]);
-      uint32_t rank = 0;
-      for (uint32_t q = 0; q < m; ++q) {
-        if (q == j) continue;
-        SinRec c; store_rec(&c, &srt[s + q]);
-        if (single_less(c, a, shift) || (!single_less(a, c, shift) && q < j)) ++rank;
-      }
-      const uint32_t o = s + rank;
-      store_rec(&fin[o], &a);
-      if (S.history && o < S.capacity) { S.history[o] = a.history; S.ids[o] = a.ids; S.x[o] = a.x; S.y[o] = a.y; S.z[o] = a.z; S.e[o] = a.e; S.t[o] = a.t; }
+// one thread per single (bucket order): rank inside its bucket (~1-3 singles) by counting, then the final time-ordered
+// record and the caller's arrays
+__global__ void __launch_bounds__(256) bucket_sort_kernel(const SinRec *srt, int shift, const uint32_t *n_ptr, Buckets B, const uint32_t *boff, SinRec *fin, SinglesBuf S) {
+  const uint32_t n = *n_ptr;
+  for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n; i += gridDim.x * 256u) {
+    SinRec a; store_rec(&a, &srt[i]);
+    const uint32_t b = bucket_of(B, a.t), s = boff[b], m = boff[b + 1] - s;
+    uint32_t rank = 0;
+    for (uint32_t q = s; q < s + m; ++q) {
+      if (q == i) continue;
+      SinRec c; store_rec(&c, &srt[q]);
+      if (single_less(c, a, shift) || (!single_less(a, c, shift) && q < i)) ++rank;
     }
+    const uint32_t o = s + rank;
+    store_rec(&fin[o], &a);
+    if (S.history && o < S.capacity) { S.history[o] = a.history; S.ids[o] = a.ids; S.x[o] = a.x; S.y[o] = a.y; S.z[o] = a.z; S.e[o] = a.e; S.t[o] = a.t; }
   }
 }
 
 // ---------------------------------------------------------------- stage 4: coincidence windows [R27]
+// A thread per cluster start (gap >= tau to the previous single) walks its cluster with the window rule and writes
+// the flag of EVERY member (1 = this single opens an accepted pair with its successor), so `flag` needs no clearing.
 __global__ void __launch_bounds__(256) coincidence_flag_kernel(const SinRec *fin, const uint32_t *n_ptr, double tau, uint32_t *flag) {
   const uint32_t n = *n_ptr;
   for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n; i += gridDim.x * 256u) {
-    uint32_t f = 0;
-    if (i == 0 || !(__dsub_rn(fin[i].t, fin[i - 1].t) < tau)) {      // cluster start: this thread walks the cluster
+    if (i == 0 || !(__dsub_rn(fin[i].t, fin[i - 1].t) < tau)) {
       uint32_t o = i;
       for (;;) {                                                     // o opens a window
         const double to = fin[o].t;
         uint32_t j = o + 1;
-        while (j < n && __dsub_rn(fin[j].t, to) < tau) ++j;
-        const uint32_t pair = (j - o == 2 && (fin[o].ids >> 26) != (fin[o + 1].ids >> 26)) ? 1u : 0u;
-        if (o == i) f = pair; else flag[o] = pair;
+        while (j < n && __dsub_rn(fin[j].t, to) < tau) { flag[j] = 0u; ++j; }
+        flag[o] = (j - o == 2 && (fin[o].ids >> 26) != (fin[o + 1].ids >> 26)) ? 1u : 0u;
         if (j >= n || !(__dsub_rn(fin[j].t, fin[j - 1].t) < tau)) break;   // the next opener starts a new cluster (its own thread)
         o = j;
       }
-      flag[i] = f;
     }
   }
 }
@@ -263,15 +314,18 @@ __global__ void __launch_bounds__(256) coincidence_write_kernel(const SinRec *fi
 
 // ---------------------------------------------------------------- scratch layout + driver
 namespace {
-struct Layout { size_t cnt, off, bsum, bcnt, boff, flag, coff, rec, sing, fin, total; };
+struct Layout { size_t cnt, off, ctl, ctl_bytes, st1, st2, bcnt, boff, flag, coff, hrank, srank, rec, sing, fin, total; uint64_t nb; };
 Layout layout(uint64_t N, uint64_t M) {
   Layout L; size_t o = 0; const uint64_t Mx = M ? M : 1;
   auto take = [&](size_t bytes) { o = (o + 255) & ~(size_t)255; size_t r = o; o += bytes; return r; };
+  L.nb = (Mx + 1) / 2;              // time buckets: kept singles are ~0.4 per hit, so ~1 per bucket
   L.cnt = take(4 * N); L.off = take(4 * (N + 1));
-  const uint64_t big = N > Mx ? N : Mx;
-  L.bsum = take(4 * (big / kTile + 3));
-  L.bcnt = take(4 * Mx); L.boff = take(4 * (Mx + 1));
+  // control block, cleared by one memset per call: kept-singles counter, then the look-back state of the three scans
+  const size_t s0 = 8 * (N / kTile + 3), s1 = 8 * (L.nb / kTile + 3), s2 = 8 * (Mx / kTile + 3);
+  L.ctl = take(256 + s0 + s1 + s2); L.st1 = L.ctl + 256 + s0; L.st2 = L.st1 + s1; L.ctl_bytes = 256 + s0 + s1 + s2;
+  L.bcnt = take(4 * L.nb); L.boff = take(4 * (L.nb + 1));
   L.flag = take(4 * Mx); L.coff = take(4 * (Mx + 1));
+  L.hrank = take(4 * Mx); L.srank = take(4 * Mx);   // rank of a hit in its history / of a kept single in its time bucket
   L.rec = take(32 * Mx);            // hit records by history; reused for the bucket-ordered singles
   L.sing = take(32 * Mx);           // kept singles, append order
   L.fin = take(32 * Mx);            // kept singles, time order
@@ -288,35 +342,37 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   const uint64_t N = n_pairs, M = n_hits ? n_hits : 1;
   const Layout L = layout(N, n_hits);
   char *s = (char *)scratch;
-  uint32_t *cnt = (uint32_t *)(s + L.cnt), *off = (uint32_t *)(s + L.off), *bsum = (uint32_t *)(s + L.bsum);
+  uint32_t *cnt = (uint32_t *)(s + L.cnt), *off = (uint32_t *)(s + L.off), *n_kept = (uint32_t *)(s + L.ctl);
+  unsigned long long *st0 = (unsigned long long *)(s + L.ctl + 256), *st1 = (unsigned long long *)(s + L.st1), *st2 = (unsigned long long *)(s + L.st2);
   uint32_t *bcnt = (uint32_t *)(s + L.bcnt), *boff = (uint32_t *)(s + L.boff), *flag = (uint32_t *)(s + L.flag), *coff = (uint32_t *)(s + L.coff);
+  uint32_t *hrank = (uint32_t *)(s + L.hrank), *srank = (uint32_t *)(s + L.srank);
   HitRec *rec = (HitRec *)(s + L.rec); SinRec *srt = (SinRec *)(s + L.rec), *sing = (SinRec *)(s + L.sing), *fin = (SinRec *)(s + L.fin);
   cudaError_t e;
   if ((e = cudaMemsetAsync(cnt, 0, 4 * N, st)) != cudaSuccess) return e;
-  if ((e = cudaMemsetAsync(bcnt, 0, 4 * M, st)) != cudaSuccess) return e;
-  if ((e = cudaMemsetAsync(flag, 0, 4 * M, st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(s + L.ctl, 0, L.ctl_bytes, st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(bcnt, 0, 4 * L.nb, st)) != cudaSuccess) return e;
   const uint32_t nh = (uint32_t)n_hits, np = (uint32_t)N, first_lo = (uint32_t)first_history;
   // 1. counting sort by history
-  if (nh) { count_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, cnt); count_launch(); }
-  if ((e = exclusive_scan(cnt, N, off, bsum, nullptr, st)) != cudaSuccess) return e;
-  if (nh) { scatter_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, off, cnt, rec); count_launch(); }
-  // 2. adder, blur, window, time; kept singles counted into time buckets
+  if (nh) { count_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, cnt, hrank); count_launch(); }
+  if ((e = exclusive_scan(cnt, N, nullptr, off, st0, nullptr, st)) != cudaSuccess) return e;
+  if (nh) { scatter_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, off, hrank, rec); count_launch(); }
+  // 2. adder, blur, window, time; kept singles appended and counted into time buckets
   const uint64_t B = P.pairs_per_slice;
   const double slice_s = (double)B / P.activity_bq;
-  Buckets bk; bk.nb = (uint32_t)M;
+  Buckets bk; bk.nb = (uint32_t)L.nb;
   bk.t_lo = (double)(first_history / B) * slice_s;
   const double t_hi = ((double)((first_history + n_pairs - 1) / B) + 1.0) * slice_s + 2e-6;
   bk.scale = (double)bk.nb / (t_hi - bk.t_lo);
-  adder_kernel<<<grid_for(M), 256, 0, st>>>(P, bk, first_history, off, off + N, rec, sing, bcnt); count_launch();
+  adder_kernel<<<grid_for(M), 256, 0, st>>>(P, bk, first_history, off, off + N, rec, sing, srank, n_kept, bcnt); count_launch();
   // 3. time-bucket counting sort
-  if ((e = exclusive_scan(bcnt, M, boff, bsum, S.n, st)) != cudaSuccess) return e;
-  bucket_scatter_kernel<<<grid_for(M), 256, 0, st>>>(sing, off + N, bk, boff, bcnt, srt); count_launch();
-  bucket_sort_kernel<<<grid_for(M), 256, 0, st>>>(srt, P.shift, bk.nb, boff, fin, S); count_launch();
-  // 4. coincidences
-  const uint32_t *n_singles = boff + M;
-  coincidence_flag_kernel<<<grid_for(M), 256, 0, st>>>(fin, n_singles, P.window_s, flag); count_launch();
-  if ((e = exclusive_scan(flag, M, coff, bsum, C.n, st)) != cudaSuccess) return e;
-  coincidence_write_kernel<<<grid_for(M), 256, 0, st>>>(fin, n_singles, flag, coff, C); count_launch();
+  if ((e = exclusive_scan(bcnt, L.nb, nullptr, boff, st1, S.n, st)) != cudaSuccess) return e;
+  bucket_scatter_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(sing, srank, n_kept, bk, boff, srt); count_launch();
+  bucket_sort_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(srt, P.shift, n_kept, bk, boff, fin, S); count_launch();
+  // 4. coincidences (lengths known on the device only: the scan stops at the number of kept singles)
+  const uint32_t *n_singles = boff + L.nb;
+  coincidence_flag_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(fin, n_singles, P.window_s, flag); count_launch();
+  if ((e = exclusive_scan(flag, M, n_singles, coff, st2, C.n, st)) != cudaSuccess) return e;
+  coincidence_write_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(fin, n_singles, flag, coff, C); count_launch();
   return cudaGetLastError();
 }
 

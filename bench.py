@@ -31,6 +31,8 @@ SM_COUNT, LANES_PER_SM = 148, 128
 # Algorithmic thread-instructions per pair of the transport kernel on C1 (event
 # counts of the oracle x audited minimum instruction cost per event).
 ALG_INSTR_PER_PAIR = {"C1": 740.0}
+# Algorithmic HBM bytes per pair of the digitizer on C1.
+ALG_DIGI_BYTES_PER_PAIR = {"C1": 170.0}
 
 
 def load_peaks():
@@ -234,6 +236,14 @@ def run_ours(args):
                         f"{peaks['sm_max_mhz']} MHz ({peaks['source']} max SM clock); hbm {peaks['hbm_gbs']} GB/s of {peaks['source']}",
                 "transport_ms": transport_ms, "digitize_ms": ms_total / args.steps - transport_ms,
                 "hit_bytes_gbs": n_hits * 28 / (transport_ms * 1e-3) / 1e9}
+    digi_ms = ms_total / args.steps - transport_ms
+    dbytes = ALG_DIGI_BYTES_PER_PAIR.get(args.config)
+    roofline_digi = None
+    if dbytes and peaks["hbm_gbs"]:
+        dach = dbytes * n / (digi_ms * 1e-3) / 1e9
+        roofline_digi = {"kernel": "digitizer (gpet_digitize, 10 launches)", "bound": "hbm", "achieved": dach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                         "frac": dach / peaks["hbm_gbs"], "traffic": None,
+                         "note": f"{dbytes} algorithmic B/pair (DESIGN.md 6) x {n} pairs / {digi_ms:.3f} ms; peak = hbm_gbs of {peaks['source']}"}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -257,7 +267,7 @@ def run_ours(args):
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": args.e2e_steps,
                 "api": "gpet_run_host (host outputs: coincidence list-mode + counters)"},
-        "roofline": roofline, "cpu_baseline": cpu,
+        "roofline": roofline, "roofline_digitizer": roofline_digi, "cpu_baseline": cpu,
     }))
     if world > 1:
         dist.destroy_process_group()
@@ -266,15 +276,15 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C1")
     ap.add_argument("--pairs", type=int, default=None, help="pairs per step per GPU (default: the config's own, 1e7 for C1)")
     ap.add_argument("--hits-per-pair", type=float, default=1.2)
     ap.add_argument("--e2e-steps", type=int, default=5)
-    ap.add_argument("--cpu-pairs", type=int, default=2_000_000)
-    ap.add_argument("--ref-pairs", type=int, default=500_000)
+    ap.add_argument("--cpu-pairs", type=int, default=10_000_000)
+    ap.add_argument("--ref-pairs", type=int, default=2_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -17,7 +17,8 @@
 
 namespace gpet {
 
-constexpr int kTile = 2048;      // elements per scan block (256 threads x 8)
+constexpr int kItems = 16;       // elements per thread of a scan tile (four 16-byte loads)
+constexpr int kTile = 256 * kItems;
 
 // ---------------------------------------------------------------- device-wide exclusive scan (u32)
 __device__ __forceinline__ uint32_t block_exclusive_scan_256(uint32_t v, uint32_t *total) {
@@ -51,17 +52,20 @@ __global__ void __launch_bounds__(256) scan_lookback_kernel(const uint32_t *in, 
   if (n_dev) { const uint64_t nd = *n_dev; if (nd < n) n = nd; }
   const uint32_t ntiles = n ? (uint32_t)((n + kTile - 1) / kTile) : 1u;
   if (tile >= ntiles) return;
-  const uint64_t base = (uint64_t)tile * kTile + (uint64_t)threadIdx.x * 8;
-  uint32_t v[8], s = 0;
-  if (base + 8 <= n) {
-    const uint4 a = *reinterpret_cast<const uint4 *>(in + base), b = *reinterpret_cast<const uint4 *>(in + base + 4);
-    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+  const uint64_t base = (uint64_t)tile * kTile + (uint64_t)threadIdx.x * kItems;
+  uint32_t v[kItems], s = 0;
+  if (base + kItems <= n) {
+#pragma unroll
+    for (int q = 0; q < kItems / 4; ++q) {
+      const uint4 a = *reinterpret_cast<const uint4 *>(in + base + 4 * q);
+      v[4 * q] = a.x; v[4 * q + 1] = a.y; v[4 * q + 2] = a.z; v[4 * q + 3] = a.w;
+    }
   } else {
 #pragma unroll
-    for (int k = 0; k < 8; ++k) v[k] = base + k < n ? in[base + k] : 0u;
+    for (int k = 0; k < kItems; ++k) v[k] = base + k < n ? in[base + k] : 0u;
   }
 #pragma unroll
-  for (int k = 0; k < 8; ++k) s += v[k];
+  for (int k = 0; k < kItems; ++k) s += v[k];
   uint32_t tot; uint32_t ex = block_exclusive_scan_256(s, &tot);
   if (threadIdx.x < 32) {                                            // warp 0: publish, then look back 32 tiles at a time
     volatile unsigned long long *st = state + 1;
@@ -90,14 +94,16 @@ __global__ void __launch_bounds__(256) scan_lookback_kernel(const uint32_t *in, 
   }
   __syncthreads();
   ex += s_prefix;
-  if (base + 8 <= n) {
-    uint4 a, b;
-    a.x = ex; ex += v[0]; a.y = ex; ex += v[1]; a.z = ex; ex += v[2]; a.w = ex; ex += v[3];
-    b.x = ex; ex += v[4]; b.y = ex; ex += v[5]; b.z = ex; ex += v[6]; b.w = ex;
-    *reinterpret_cast<uint4 *>(out + base) = a; *reinterpret_cast<uint4 *>(out + base + 4) = b;
+  if (base + kItems <= n) {
+#pragma unroll
+    for (int q = 0; q < kItems / 4; ++q) {
+      uint4 a;
+      a.x = ex; ex += v[4 * q]; a.y = ex; ex += v[4 * q + 1]; a.z = ex; ex += v[4 * q + 2]; a.w = ex; ex += v[4 * q + 3];
+      *reinterpret_cast<uint4 *>(out + base + 4 * q) = a;
+    }
   } else {
 #pragma unroll
-    for (int k = 0; k < 8; ++k) { if (base + k < n) out[base + k] = ex; ex += v[k]; }
+    for (int k = 0; k < kItems; ++k) { if (base + k < n) out[base + k] = ex; ex += v[k]; }
   }
 }
 
@@ -164,78 +170,57 @@ __device__ __forceinline__ double decay_time(const DigiParams &P, uint64_t histo
   return __dmul_rn(__dadd_rn((double)slice, u53), P.slice_s);                               // slice_s = B / A
 }
 
-// A group of hits of one (history, readout unit) after the adder, before blur: what phase 2 of the kernel needs.
-struct Cand { uint32_t h, unit, best; float e_sum, tof_min; };
-
-// Phase 1, one thread per hit record (a thread per history would idle on the ~54 % of histories without hits): the
-// record with the smallest (ids, position) of its (history, readout unit) group is the group's leader; it sums the
-// group in ascending (ids, position) order -- canonical, so the fp32 sum does not depend on the hit buffer's order
-// -- and picks the largest deposit and the earliest time [R24].  The leaders of the block are then compacted into
-// shared memory (block scan), so that phase 2 -- blur [R25], window [R26], absolute time [R16] -- runs on dense
-// lanes; kept singles are appended with one atomic per warp and counted into their time bucket.  The append order
-// is free: the bucket sort that follows fixes the final order.
+// One thread per hit record (a thread per history would idle on the ~54 % of histories without hits).  The record with
+// the smallest (ids, position) of its (history, readout unit) group is the group's leader: one pass over the history's
+// segment gives it the energy sum, the largest deposit (tie: lowest (photon, seq)) and the earliest time [R24].  The
+// sum is formed in 2^-40 keV fixed point (int64): exact integer addition, so it does not depend on the order of the
+// hit buffer, and it differs from the exact sum by < 2^-36 keV.  Leaders then blur [R25], window [R26] and time
+// [R16] their single; kept singles are appended with one atomic per block and counted into their time bucket (the
+// atomic's return value is the single's rank in the bucket).  The append order is free: the bucket sort fixes it.
 __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uint64_t first_history, const uint32_t *off, const uint32_t *n_rec,
                                                     const HitRec *rec, SinRec *sing, uint32_t *srank, uint32_t *n_kept, uint32_t *bcnt) {
-  __shared__ Cand cand[256];
   __shared__ uint32_t s_base;
   const uint32_t n = *n_rec;
   const uint2 key = make_uint2((uint32_t)P.seed, (uint32_t)(P.seed >> 32));
   for (uint32_t base = blockIdx.x * 256u; base < n; base += gridDim.x * 256u) {
     const uint32_t i = base + threadIdx.x;
-    bool leader = false; Cand c = {0u, 0u, 0u, 0.f, 0.f};
+    bool keep = false; SinRec s;
     if (i < n) {
       const uint4 me = *reinterpret_cast<const uint4 *>(&rec[i]);      // ids, x, y, z
       const uint4 m2 = *(reinterpret_cast<const uint4 *>(&rec[i]) + 1);  // e, tof, idx, history - first
       const uint32_t my_ids = me.x, h = m2.w, b = off[h], k = off[h + 1] - b, unit = my_ids >> P.shift;
-      leader = true; c.h = h; c.unit = unit; c.best = i; c.e_sum = __uint_as_float(m2.x); c.tof_min = __uint_as_float(m2.y);
+      bool leader = true; uint32_t best = i;
+      float e_sum = __uint_as_float(m2.x), tof_min = __uint_as_float(m2.y);
       if (k > 1) {
         const uint64_t my_key = ((uint64_t)my_ids << 32) | i;
-        uint32_t members = 0;
+        long long isum = 0; float e_best = -1.0f; uint32_t best_ord = 0;
         for (uint32_t j = b; j < b + k; ++j) {
-          const uint32_t ids = rec[j].ids;
-          if ((ids >> P.shift) != unit) continue;
-          ++members;
-          if ((((uint64_t)ids << 32) | j) < my_key) leader = false;
+          const uint4 r = *reinterpret_cast<const uint4 *>(&rec[j]);
+          if ((r.x >> P.shift) != unit) continue;
+          if ((((uint64_t)r.x << 32) | j) < my_key) { leader = false; break; }
+          const float2 et = *reinterpret_cast<const float2 *>(&rec[j].e);
+          isum += __double2ll_rn((double)et.x * 1099511627776.0);
+          const uint32_t ord = r.x & 31u;
+          if (et.x > e_best || (et.x == e_best && ord < best_ord)) { e_best = et.x; best = j; best_ord = ord; }
+          tof_min = fminf(tof_min, et.y);
         }
-        if (leader && members > 1) {                                 // ascending (ids, position) after the leader itself
-          uint64_t prev = my_key; float e_best = c.e_sum; uint32_t best_ord = my_ids & 31u;
-          for (uint32_t m = 1; m < members; ++m) {
-            uint64_t sel = ~0ull;
-            for (uint32_t j = b; j < b + k; ++j) {
-              const uint32_t ids = rec[j].ids;
-              const uint64_t kk = ((uint64_t)ids << 32) | j;
-              if ((ids >> P.shift) == unit && kk > prev && kk < sel) sel = kk;
-            }
-            prev = sel;
-            const HitRec &r = rec[(uint32_t)sel];
-            const float re = r.e; const uint32_t ord = (uint32_t)(sel >> 32) & 31u;
-            c.e_sum += re;
-            if (re > e_best || (re == e_best && ord < best_ord)) { e_best = re; c.best = (uint32_t)sel; best_ord = ord; }
-            c.tof_min = fminf(c.tof_min, r.tof);
-          }
+        e_sum = (float)((double)isum * (1.0 / 1099511627776.0));
+      }
+      if (leader) {
+        const uint64_t history = first_history + h;
+        const uint4 w = philox4x32_10(make_uint4((uint32_t)history, 0u, 3u, unit), key);        // Box-Muller on words 0,1
+        const float nrm = sqrtf(-2.0f * logf(u01(w.x))) * cospif(2.0f * u01(w.y));
+        const float sigma = P.sigma_scale * (P.ref_keV > 0.0f ? sqrtf(P.ref_keV * e_sum) : e_sum);
+        const float e_b = fmaf(sigma, nrm, e_sum);
+        keep = e_b >= P.e_lo && e_b < P.e_hi;
+        if (keep) {
+          const uint4 r = best == i ? me : *reinterpret_cast<const uint4 *>(&rec[best]);
+          s.t = __dadd_rn(decay_time(P, history), __dmul_rn((double)tof_min, 1e-9));
+          s.history = (uint32_t)history; s.ids = r.x; s.x = __uint_as_float(r.y); s.y = __uint_as_float(r.z); s.z = __uint_as_float(r.w); s.e = e_b;
         }
       }
     }
-    uint32_t tot; const uint32_t ex = block_exclusive_scan_256(leader ? 1u : 0u, &tot);
-    if (leader) cand[ex] = c;
-    __syncthreads();
-    // ---- phase 2: dense lanes
-    bool keep = false; SinRec s;
-    if (threadIdx.x < tot) {
-      const Cand q = cand[threadIdx.x];
-      const uint64_t history = first_history + q.h;
-      const uint4 w = philox4x32_10(make_uint4((uint32_t)history, 0u, 3u, q.unit), key);       // Box-Muller on words 0,1
-      const float nrm = sqrtf(-2.0f * logf(u01(w.x))) * cospif(2.0f * u01(w.y));
-      const float sigma = P.sigma_scale * (P.ref_keV > 0.0f ? sqrtf(P.ref_keV * q.e_sum) : q.e_sum);
-      const float e_b = fmaf(sigma, nrm, q.e_sum);
-      keep = e_b >= P.e_lo && e_b < P.e_hi;
-      if (keep) {
-        const HitRec &r = rec[q.best];
-        s.t = __dadd_rn(decay_time(P, history), __dmul_rn((double)q.tof_min, 1e-9));
-        s.history = (uint32_t)history; s.ids = r.ids; s.x = r.x; s.y = r.y; s.z = r.z; s.e = e_b;
-      }
-    }
-    uint32_t nk; const uint32_t kx = block_exclusive_scan_256(keep ? 1u : 0u, &nk);      // one append per block, not per warp
+    uint32_t nk; const uint32_t kx = block_exclusive_scan_256(keep ? 1u : 0u, &nk);      // one append per block
     if (threadIdx.x == 0 && nk) s_base = atomicAdd(n_kept, nk);
     __syncthreads();
     if (keep) {
@@ -243,7 +228,6 @@ __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uin
       store_rec(&sing[o], &s);
       srank[o] = atomicAdd(&bcnt[bucket_of(B, s.t)], 1u);            // rank inside its time bucket (any order will do)
     }
-    __syncthreads();
   }
 }
 

@@ -303,6 +303,10 @@ class CoincBuffer:
         return CoincBuffer(i32(), i32(), i32(), i32(), f32(), f32(), f32(), torch.empty(capacity, dtype=torch.float64, device=device),
                            torch.zeros(1, dtype=torch.int64, device=device))
 
+    @property
+    def capacity(self) -> int:
+        return int(self.ids_a.numel())
+
     def struct(self) -> _Coinc:
         return _Coinc(self.ids_a.data_ptr(), self.ids_b.data_ptr(), self.history_a.data_ptr(), self.history_b.data_ptr(),
                       self.e_a.data_ptr(), self.e_b.data_ptr(), self.dt_ns.data_ptr(), self.t_s.data_ptr(),

@@ -240,33 +240,106 @@ def test_run_host_matches_device_path(tables):
 
 
 # ----------------------------------------------------------------------------- full size, bench launch configuration
-def test_c1_full_size_sampled_histories(tables):
-    """configs[1] at its full 1e7 pairs in the configuration bench.py times; the oracle recomputes 24 random
-    blocks of 4096 histories (it can start anywhere: draws are keyed by history id)."""
-    r = W.config_runs("C1")[0]
-    geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
-    hb = api.HitBuffer.allocate(int(1.2 * r.n_pairs), n_hash=r.n_pairs)
-    api.gpet_simulate(geom, m, s, 0, r.n_pairs, r.seed, hb)
+def full_size_sampled(run, tables, hits_per_pair, n_blocks=24, block=4096):
+    """A config at its full size in the configuration bench.py times; the oracle recomputes random blocks of
+    histories (it can start anywhere: draws are keyed by history id).  Returns the GPU hits (buffer order)."""
+    geom, m, s = api.gpet_geometry_create(run.geometry), api.gpet_materials_load(tables), api.DeviceSource(run.source)
+    hb = api.HitBuffer.allocate(int(hits_per_pair * run.n_pairs), n_hash=run.n_pairs)
+    api.gpet_simulate(geom, m, s, 0, run.n_pairs, run.seed, hb)
     torch.cuda.synchronize()
-    nh = hb.count()
-    assert 0.76 < nh / r.n_pairs < 0.79                               # SURVEY 8(a): 0.77 hits per pair
+    assert hb.count() <= hb.capacity
     gh = hb.outcome_hash.cpu().numpy().view(np.uint64).reshape(-1, 2)
     g = hb.to_numpy()
     rng = np.random.default_rng(5)
-    starts = np.concatenate([[0, r.n_pairs - 4096], rng.integers(0, r.n_pairs - 4096, 22)])
+    starts = np.concatenate([[0, run.n_pairs - block], rng.integers(0, run.n_pairs - block, n_blocks - 2)])
     same = tot = 0
     for st in starts:
-        o = O.simulate(r.geometry, tables, r.source, 4096, r.seed, first_history=int(st), want_hash=True, threads=4)
-        ok = np.all(gh[st:st + 4096] == o.outcome_hash, axis=1)
-        same += int(ok.sum()); tot += 4096
-        sel = (g["history"] >= st) & (g["history"] < st + 4096)
+        o = O.simulate(run.geometry, tables, run.source, block, run.seed, first_history=int(st), want_hash=True, threads=4)
+        ok = np.all(gh[st:st + block] == o.outcome_hash, axis=1)
+        same += int(ok.sum()); tot += block
+        sel = (g["history"] >= st) & (g["history"] < st + block)
         part = PU.canonical({k: v[sel] for k, v in g.items()})
-        PU.compare_hits(part, PU.oracle_hits_dict(o.hits), gh[st:st + 4096], o.outcome_hash, first_history=int(st),
+        PU.compare_hits(part, PU.oracle_hits_dict(o.hits), gh[st:st + block], o.outcome_hash, first_history=int(st),
                         pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
-    assert same / tot >= MIN_MATCH
-    # properties that hold at any size: every panel equally hit (centred source), axial symmetry
+    assert same / tot >= MIN_MATCH, (same, tot)
+    return g, hb.count()
+
+
+def test_c1_full_size_sampled_histories(tables):
+    """configs[1] at its full 1e7 pairs + properties that hold at any size."""
+    r = W.config_runs("C1")[0]
+    g, nh = full_size_sampled(r, tables, 1.2)
+    assert 0.76 < nh / r.n_pairs < 0.79                               # SURVEY 8(a): 0.77 hits per pair
     counts = np.bincount(g["ids"] >> 26, minlength=12)
     from scipy import stats
-    assert stats.chisquare(counts).pvalue > 1e-4
+    assert stats.chisquare(counts).pvalue > 1e-4                      # centred source: every panel equally hit
     up, down = int((g["z"] > 0).sum()), int((g["z"] < 0).sum())
-    assert abs(up - down) < 5 * np.sqrt(up + down)
+    assert abs(up - down) < 5 * np.sqrt(up + down)                    # axial symmetry (PAPER.md:87)
+
+
+@pytest.mark.parametrize("cfg,idx,lo,hi", [("C2", 4, 1.38, 1.48), ("C3", 21, 1.19, 1.29)])
+def test_c2_c3_full_size_sampled_histories(tables, cfg, idx, lo, hi):
+    """configs[2] (x = 50 mm) and configs[3] (x = 50 mm, z = 16 mm) at 1e7 pairs: the positions with the most hits."""
+    r = W.config_runs(cfg)[idx]
+    g, nh = full_size_sampled(r, tables, 2.0, n_blocks=16)
+    assert lo < nh / r.n_pairs < hi
+    assert ((g["ids"] >> 18) & 3).max() == 1                          # both layers recorded (PAPER.md:37)
+
+
+def test_c4_full_run_in_time_slices(tables):
+    """configs[4] in full: 1e9 pairs in 16 time slices of 6.25e7, transported through the phantom and the detector and
+    digitized to coincidence list-mode, every slice in the launch configuration bench.py times.  One slice is also run
+    with outcome hashes and singles output, and the oracle recomputes blocks of its histories (hits, hashes and the
+    singles of those histories, which depend on no other history: no pile-up [R24])."""
+    r = W.config_runs("C4")[0]
+    B = r.source.pairs_per_time_slice
+    assert r.n_pairs == 10 ** 9 and B * 16 == r.n_pairs
+    geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+    cap = int(0.9 * B)
+    hb = api.HitBuffer.allocate(cap)
+    co = api.CoincBuffer.allocate(cap // 8)
+    scratch = torch.empty(api.gpet_digitize_scratch_bytes(B, cap), dtype=torch.uint8, device="cuda")
+    n_hits = n_coinc = 0
+    t_last = -1.0
+    for k in range(16):
+        hb.n_hits.zero_()
+        api.gpet_simulate(geom, m, s, k * B, B, r.seed, hb)
+        api.gpet_digitize(s, r.seed, r.n_pairs, k * B, B, hb, cap, r.digitizer, scratch, None, co)
+        torch.cuda.synchronize()
+        nh, nc = hb.count(), int(co.n_coinc.item())
+        assert nh <= cap and nc <= co.capacity
+        n_hits += nh; n_coinc += nc
+        t = co.t_s[:nc]
+        assert float(t[0]) > t_last and bool((t[1:] >= t[:-1]).all())  # list-mode is time-ordered across slices
+        assert k * B / 1e6 <= float(t[0]) and float(t[-1]) < (k + 1) * B / 1e6 + 1e-6   # slice k covers its own time interval [R16]
+        t_last = float(t[-1])
+    assert 0.73 < n_hits / r.n_pairs < 0.76 and 0.036 < n_coinc / r.n_pairs < 0.040
+    # one slice again with hashes and singles; oracle on sampled blocks
+    k = 11
+    del hb, co
+    hb = api.HitBuffer.allocate(cap, n_hash=B)
+    sg, co = api.SinglesBuffer.allocate(cap), api.CoincBuffer.allocate(cap // 8)
+    api.gpet_simulate(geom, m, s, k * B, B, r.seed, hb)
+    api.gpet_digitize(s, r.seed, r.n_pairs, k * B, B, hb, cap, r.digitizer, scratch, sg, co)
+    torch.cuda.synchronize()
+    gh = hb.outcome_hash.cpu().numpy().view(np.uint64).reshape(-1, 2)
+    g, gs = hb.to_numpy(), sg.to_numpy()
+    rng = np.random.default_rng(6)
+    same = tot = 0
+    for st in np.concatenate([[0, B - 2048], rng.integers(0, B - 2048, 10)]):
+        first = k * B + int(st)
+        o = O.simulate(r.geometry, tables, r.source, 2048, r.seed, first_history=first, want_hash=True, threads=4)
+        ok = np.all(gh[st:st + 2048] == o.outcome_hash, axis=1)
+        same += int(ok.sum()); tot += 2048
+        sel = (g["history"] >= first) & (g["history"] < first + 2048)
+        part = PU.canonical({kk: v[sel] for kk, v in g.items()})
+        PU.compare_hits(part, PU.oracle_hits_dict(o.hits), gh[st:st + 2048], o.outcome_hash, first_history=first,
+                        pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+        if ok.all():                                                  # same hits in -> the same singles out
+            osg, _, _ = O.digitize(r.source, r.seed, r.n_pairs, o.hits, r.digitizer)
+            ss = (gs["history"] >= first) & (gs["history"] < first + 2048)
+            assert abs(int(ss.sum()) - len(osg.ids)) <= 1            # a blurred energy within 1e-4 keV of a window edge may flip
+            if int(ss.sum()) == len(osg.ids):
+                assert np.array_equal(gs["ids"][ss], osg.ids) and np.array_equal(gs["t_s"][ss], osg.t_s)
+                assert np.max(np.abs(gs["e_keV"][ss] - osg.e_keV)) < E_TOL
+    assert same / tot >= MIN_MATCH

@@ -2,16 +2,17 @@
 // PAPER.md:33,37 (single-event readout at crystal / module / panel level), PAPER.md:61 (energy resolution,
 // coincidence timing window), PAPER.md:65 (list-mode coincidences).  Readings [R16], [R24]-[R27].
 //
-// Sort / segmented-scan structure (all hand-written, no CUB/Thrust):
-//   1. counting sort of the hits by history id (dense integer keys: histogram by atomics in L2,
-//      exclusive scan, scatter of 32-byte hit records) -> one contiguous run of sectors per history;
-//   2. one thread per history: canonical in-segment order by repeated min-selection (segments hold
-//      ~1-4 hits), adder per readout unit, blur, window, absolute time -> kept singles appended as
-//      32-byte records and counted into time buckets;
-//   3. counting sort of the kept singles by time bucket (decay times are uniform by construction
-//      [R16], so buckets hold ~0.4 singles on average), in-bucket rank sort by (t, history, unit);
-//   4. head-flag pass: a thread per cluster start (gap >= tau) walks its cluster with the window rule
-//      [R27]; exclusive scan of the pair flags; compaction into list-mode output.
+// Sort / segmented-scan structure (all hand-written, no CUB/Thrust; DESIGN.md 5.3):
+//   1. counting sort of the hits by history id (dense integer keys): histogram by L2 atomics whose return value is
+//      the hit's rank in its history, single-pass look-back scan, scatter of 32-byte hit records without atomics
+//      -> one contiguous run of sectors per history;
+//   2. adder: one thread per hit record, the group leader of each (history, readout unit) sums its group in
+//      order-free fixed point, then blur, window, absolute time -> kept singles appended (one atomic per block) and
+//      counted into time buckets (rank = the atomic's return value);
+//   3. counting sort of the kept singles by time bucket (decay times are uniform by construction [R16], ~0.6
+//      singles per bucket), then a rank sort by (t, history, unit) inside each bucket;
+//   4. head-flag pass: a thread per cluster start (gap >= tau) walks its cluster with the window rule [R27];
+//      exclusive scan of the pair flags; compaction into list-mode output.
 // Every stage is deterministic: the output does not depend on the order of the hit buffer.
 #include "gpet_internal.h"
 

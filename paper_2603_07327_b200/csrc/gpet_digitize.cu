@@ -171,20 +171,28 @@ __device__ __forceinline__ double decay_time(const DigiParams &P, uint64_t histo
   return __dmul_rn(__dadd_rn((double)slice, u53), P.slice_s);                               // slice_s = B / A
 }
 
+// records per block of the adder / bucket-scatter pair: the same split in both kernels, a multiple of the block size
+__device__ __forceinline__ uint32_t region_size(uint32_t n, uint32_t blocks) { return (((n + blocks - 1) / blocks) + 255u) & ~255u; }
+
 // One thread per hit record (a thread per history would idle on the ~54 % of histories without hits).  The record with
 // the smallest (ids, position) of its (history, readout unit) group is the group's leader: one pass over the history's
 // segment gives it the energy sum, the largest deposit (tie: lowest (photon, seq)) and the earliest time [R24].  The
 // sum is formed in 2^-40 keV fixed point (int64): exact integer addition, so it does not depend on the order of the
 // hit buffer, and it differs from the exact sum by < 2^-36 keV.  Leaders then blur [R25], window [R26] and time
-// [R16] their single; kept singles are appended with one atomic per block and counted into their time bucket (the
-// atomic's return value is the single's rank in the bucket).  The append order is free: the bucket sort fixes it.
+// [R16] their single.  Block b owns the records [b R, (b+1) R) and appends its kept singles at sing[b R ...] through a
+// shared-memory counter (one shared atomic per warp, no block barrier in the loop, no global append counter); the
+// per-block counts go to kcnt[].  Each kept single is counted into its time bucket (the atomic's return value is its
+// rank in the bucket).  The append order is free: the bucket sort fixes it.
 __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uint64_t first_history, const uint32_t *off, const uint32_t *n_rec,
-                                                    const HitRec *rec, SinRec *sing, uint32_t *srank, uint32_t *n_kept, uint32_t *bcnt) {
-  __shared__ uint32_t s_base;
-  const uint32_t n = *n_rec;
+                                                    const HitRec *rec, SinRec *sing, uint32_t *srank, uint32_t *kcnt, uint32_t *bcnt) {
+  __shared__ uint32_t s_cnt;
+  const uint32_t n = *n_rec, R = region_size(n, gridDim.x), r0 = blockIdx.x * R;
   const uint2 key = make_uint2((uint32_t)P.seed, (uint32_t)(P.seed >> 32));
-  for (uint32_t base = blockIdx.x * 256u; base < n; base += gridDim.x * 256u) {
-    const uint32_t i = base + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) s_cnt = 0;
+  __syncthreads();
+  for (uint32_t it = 0; it < R && r0 + it < n; it += 256u) {
+    const uint32_t i = r0 + it + threadIdx.x;
     bool keep = false; SinRec s;
     if (i < n) {
       const uint4 me = *reinterpret_cast<const uint4 *>(&rec[i]);      // ids, x, y, z
@@ -221,22 +229,26 @@ __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uin
         }
       }
     }
-    uint32_t nk; const uint32_t kx = block_exclusive_scan_256(keep ? 1u : 0u, &nk);      // one append per block
-    if (threadIdx.x == 0 && nk) s_base = atomicAdd(n_kept, nk);
-    __syncthreads();
-    if (keep) {
-      const uint32_t o = s_base + kx;
-      store_rec(&sing[o], &s);
-      srank[o] = atomicAdd(&bcnt[bucket_of(B, s.t)], 1u);            // rank inside its time bucket (any order will do)
+    const unsigned mk = __ballot_sync(0xFFFFFFFFu, keep);
+    if (mk) {
+      uint32_t o = 0;
+      if (lane == 0) o = atomicAdd(&s_cnt, (uint32_t)__popc(mk));
+      o = r0 + __shfl_sync(0xFFFFFFFFu, o, 0) + __popc(mk & ((1u << lane) - 1u));
+      if (keep) {
+        store_rec(&sing[o], &s);
+        srank[o] = atomicAdd(&bcnt[bucket_of(B, s.t)], 1u);          // rank inside its time bucket (any order will do)
+      }
     }
   }
+  __syncthreads();
+  if (threadIdx.x == 0) kcnt[blockIdx.x] = s_cnt;
 }
 
 // ---------------------------------------------------------------- stage 3: time-bucket counting sort
-__global__ void __launch_bounds__(256) bucket_scatter_kernel(const SinRec *sing, const uint32_t *srank, const uint32_t *n_slots, Buckets B,
-                                                             const uint32_t *boff, SinRec *srt) {
-  const uint32_t n = *n_slots;                                       // kept singles, append order
-  for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n; i += gridDim.x * 256u) {
+__global__ void __launch_bounds__(256) bucket_scatter_kernel(const SinRec *sing, const uint32_t *srank, const uint32_t *n_rec, const uint32_t *kcnt,
+                                                             Buckets B, const uint32_t *boff, SinRec *srt) {
+  const uint32_t r0 = blockIdx.x * region_size(*n_rec, gridDim.x), m = kcnt[blockIdx.x];   // this block's kept singles: sing[r0 .. r0 + m)
+  for (uint32_t i = r0 + threadIdx.x; i < r0 + m; i += 256u) {
     SinRec s; store_rec(&s, &sing[i]);
     store_rec(&srt[boff[bucket_of(B, s.t)] + srank[i]], &s);
   }
@@ -299,11 +311,12 @@ __global__ void __launch_bounds__(256) coincidence_write_kernel(const SinRec *fi
 
 // ---------------------------------------------------------------- scratch layout + driver
 namespace {
-struct Layout { size_t cnt, off, ctl, ctl_bytes, st1, st2, bcnt, boff, flag, coff, hrank, srank, rec, sing, fin, total; uint64_t nb; };
+struct Layout { size_t kcnt, cnt, off, ctl, ctl_bytes, st1, st2, bcnt, boff, flag, coff, hrank, srank, rec, sing, fin, total; uint64_t nb; };
 Layout layout(uint64_t N, uint64_t M) {
   Layout L; size_t o = 0; const uint64_t Mx = M ? M : 1;
   auto take = [&](size_t bytes) { o = (o + 255) & ~(size_t)255; size_t r = o; o += bytes; return r; };
   L.nb = (Mx + 1) / 2;              // time buckets: kept singles are ~0.4 per hit, so ~1 per bucket
+  L.kcnt = take(4 * 148 * 16);      // kept singles per adder block
   L.cnt = take(4 * N); L.off = take(4 * (N + 1));
   // control block, cleared by one memset per call: kept-singles counter, then the look-back state of the three scans
   const size_t s0 = 8 * (N / kTile + 3), s1 = 8 * (L.nb / kTile + 3), s2 = 8 * (Mx / kTile + 3);
@@ -327,7 +340,7 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   const uint64_t N = n_pairs, M = n_hits ? n_hits : 1;
   const Layout L = layout(N, n_hits);
   char *s = (char *)scratch;
-  uint32_t *cnt = (uint32_t *)(s + L.cnt), *off = (uint32_t *)(s + L.off), *n_kept = (uint32_t *)(s + L.ctl);
+  uint32_t *cnt = (uint32_t *)(s + L.cnt), *off = (uint32_t *)(s + L.off), *kcnt = (uint32_t *)(s + L.kcnt);
   unsigned long long *st0 = (unsigned long long *)(s + L.ctl + 256), *st1 = (unsigned long long *)(s + L.st1), *st2 = (unsigned long long *)(s + L.st2);
   uint32_t *bcnt = (uint32_t *)(s + L.bcnt), *boff = (uint32_t *)(s + L.boff), *flag = (uint32_t *)(s + L.flag), *coff = (uint32_t *)(s + L.coff);
   uint32_t *hrank = (uint32_t *)(s + L.hrank), *srank = (uint32_t *)(s + L.srank);
@@ -348,11 +361,12 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   bk.t_lo = (double)(first_history / B) * slice_s;
   const double t_hi = ((double)((first_history + n_pairs - 1) / B) + 1.0) * slice_s + 2e-6;
   bk.scale = (double)bk.nb / (t_hi - bk.t_lo);
-  adder_kernel<<<grid_for(M), 256, 0, st>>>(P, bk, first_history, off, off + N, rec, sing, srank, n_kept, bcnt); count_launch();
+  const int ga = grid_for(M);                                         // adder and bucket scatter share the block -> region split
+  adder_kernel<<<ga, 256, 0, st>>>(P, bk, first_history, off, off + N, rec, sing, srank, kcnt, bcnt); count_launch();
   // 3. time-bucket counting sort
   if ((e = exclusive_scan(bcnt, L.nb, nullptr, boff, st1, S.n, st)) != cudaSuccess) return e;
-  bucket_scatter_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(sing, srank, n_kept, bk, boff, srt); count_launch();
-  bucket_sort_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(srt, P.shift, n_kept, bk, boff, fin, S); count_launch();
+  bucket_scatter_kernel<<<ga, 256, 0, st>>>(sing, srank, off + N, kcnt, bk, boff, srt); count_launch();
+  bucket_sort_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(srt, P.shift, boff + L.nb, bk, boff, fin, S); count_launch();
   // 4. coincidences (lengths known on the device only: the scan stops at the number of kept singles)
   const uint32_t *n_singles = boff + L.nb;
   coincidence_flag_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(fin, n_singles, P.window_s, flag); count_launch();

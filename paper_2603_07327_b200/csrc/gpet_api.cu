@@ -311,7 +311,7 @@ extern "C" int gpet_simulate(const gpet_geometry *g, const gpet_materials *m, co
   const uint32_t stage_mask = (D.kind == 1 && D.phantom) ? (1u << m->n_materials) - 1u : 0u;
   DevTables T; rc = staged_table(const_cast<gpet_materials *>(m), g->host.det_mask, stage_mask, &T); if (rc) return rc;
   unsigned long long *wc = nullptr; rc = next_work_counter(&wc); if (rc) return rc;
-  CUDA_TRY(launch_transport(g->dev, g->host.n_panels, T, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
+  CUDA_TRY(launch_transport(g->dev, g->host.n_panels, g->host.planar, T, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
   return GPET_OK;
 }
 

@@ -62,7 +62,7 @@ __device__ __forceinline__ void sincos_small(float x, float &s, float &c) {
     const float x2 = x * x;
     s = x * fmaf(x2, fmaf(x2, fmaf(x2, -1.984126984e-4f, 8.333333333e-3f), -0.1666666667f), 1.0f);
     c = fmaf(x2, fmaf(x2, fmaf(x2, fmaf(x2, 2.48015873e-5f, -1.388888889e-3f), 4.166666667e-2f), -0.5f), 1.0f);
-  } else sincosf(x, &s, &c);
+  } else { s = __sinf(x); c = __cosf(x); }   // > 14 degrees of acolinearity: unphysical, kept finite and cheap
 }
 // (sin, cos)(2 pi u), u in (0,1): argument folded to [-pi, pi] where sin.approx / cos.approx are good to 2^-21
 __device__ __forceinline__ void sincos_2pi(float u, float &s, float &c) {
@@ -154,9 +154,10 @@ __device__ __forceinline__ void decay_site(const DevSource &src, uint4 w, float 
 // "planar" detectors (every panel has v = +z, u_z = w_z = o_z = 0: any ring built in repetition mode,
 // PAPER.md:33) share the axial slab and need only the 2-D part of each pose; the arithmetic on the
 // surviving terms is the generic one (the dropped terms are exact zeros).
+template <int PLANAR>
 __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], const float d[3], int excl, float &t_enter) {
   float bt = INFINITY; int bp = -1;
-  if (g.planar) {
+  if (PLANAR < 0 ? g.planar != 0 : PLANAR != 0) {
     const float iz = rcp_dir(d[2]);
     const float z1 = (g.blo[1] - x[2]) * iz, z2 = (g.bhi[1] - x[2]) * iz;
     const float tnz = fmaxf(fminf(z1, z2), 0.0f), tfz = fmaxf(z1, z2);
@@ -220,7 +221,10 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
 }
 
 // ---------------------------------------------------------------- the kernel
-template <bool HASH>
+// Specialisations keep the kernel small (at ~3000 SASS instructions it is sensitive to instruction-cache misses: dropping
+// the phantom code alone made the ring configs 10 % faster).  PHANTOM: the source is a voxel map with a phantom
+// [R17]; KIND: source kind (0 point, 1 voxel map, -1 = read src.kind); PLANAR: panel search variant (-1 = read g.planar).
+template <bool HASH, bool PHANTOM, int KIND, int PLANAR>
 __global__ void __launch_bounds__(kThreads, GPET_MIN_CTAS)
 transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint64_t first_history, uint64_t n_photons,
                            const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
@@ -243,7 +247,8 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
   const float4 *mu = mu_s;
   HitStage &stage = W.stage;
   const unsigned lt_mask = (1u << lane) - 1u;
-  const bool use_phantom = src.kind == 1 && src.phantom != nullptr;
+  constexpr bool use_phantom = PHANTOM;
+  const int kind = KIND < 0 ? src.kind : KIND;
 
   uint64_t w_next = 0, w_end = 0;          // this warp's reserved photon indices [w_next, w_end)
   bool exhausted = false;                  // the global counter ran past n_photons
@@ -293,7 +298,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
     int phase = L_SEARCH, best = cS + nF;
     if (cT > 0 && cT >= best) { phase = L_STEP; best = cT; }
     if (cK > best) { phase = L_KN; best = cK; }
-    if (cP > best) { phase = L_PHANTOM; best = cP; }
+    if (PHANTOM && cP > best) { phase = L_PHANTOM; best = cP; }
     if (cR > best) { phase = L_RAY; best = cR; }
     if (best == 0) break;                                             // nothing in flight, no source left
 
@@ -320,9 +325,9 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
           const uint64_t history = first_history + q.pair;
           const uint32_t h_lo = (uint32_t)history, h_hi = (uint32_t)(history >> 32);
           q.x[0] = src.pos[0]; q.x[1] = src.pos[1]; q.x[2] = src.pos[2];
-          if (src.kind == 1) decay_site(src, philox4x32_10(make_uint4(h_lo, h_hi, 0u, 0u), key), q.x);
+          if (kind == 1) decay_site(src, philox4x32_10(make_uint4(h_lo, h_hi, 0u, 0u), key), q.x);
           const uint4 w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 1u), key);
-          if (src.kind == 2) { q.d[0] = src.beam[0]; q.d[1] = src.beam[1]; q.d[2] = src.beam[2]; }
+          if (kind == 2) { q.d[0] = src.beam[0]; q.d[1] = src.beam[1]; q.d[2] = src.beam[2]; }
           else {
             const float u = u01(w.x), ct = 1.0f - 2.0f * u, sth = 2.0f * sqrtf(u * (1.0f - u));   // sin^2 = (1-ct)(1+ct)
             float sp, cp; sincospif(2.0f * u01(w.y), &sp, &cp);
@@ -343,9 +348,9 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
       // panel search [R6]; photons born inside a phantom skip it and are tracked there first [R17]
       int dest = L_NONE;
       if (active) {
-        if (ph_in_phantom(q)) dest = L_PHANTOM;
+        if (PHANTOM && ph_in_phantom(q)) dest = L_PHANTOM;
         else {
-          float bt; const int bp = panel_search(g, q.x, q.d, ph_panel(q), bt);
+          float bt; const int bp = panel_search<PLANAR>(g, q.x, q.d, ph_panel(q), bt);
           if (bp < 0) {
             if (HASH) { hash_ev(hq, EV_ESCAPE, 0); hash_out[2ull * q.pair + (q.meta & 1u)] = hq; }
             if (idx >= 0) dest = L_FREE;                              // gives its slot back
@@ -433,7 +438,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
       cK -= n;
       int dest = L_NONE; bool hit = false; float xg[3] = {0.f, 0.f, 0.f}, e_dep = 0.f; uint32_t hit_ids = 0;
       if (act) {
-        const bool in_ph = ph_in_phantom(p);
+        const bool in_ph = PHANTOM && ph_in_phantom(p);
         const float k = p.E * (1.0f / kMec2), e0 = rcp_fast(1.0f + 2.0f * k), e02 = e0 * e0;
         const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
         const uint4 w = next_block(p);                                // [R4] u_a, u_b, u_c, azimuth
@@ -491,12 +496,12 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
       if (act) {
         const uint4 w = block_at(p, (p.meta >> 18) - 1u);             // the block its Woodcock step drew (rare event: recomputed)
         rayleigh(p.d, u01(w.z), u01(w.w));
-        dest = ph_in_phantom(p) ? L_PHANTOM : L_STEP;
+        dest = (PHANTOM && ph_in_phantom(p)) ? L_PHANTOM : L_STEP;
         slot_store(W, idx, p, h);
       }
       push(L_STEP, cT, dest == L_STEP, idx);
       if (use_phantom) push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
-    } else {
+    } else if (PHANTOM) {
       // ---------------------------------------------- PHANTOM: Woodcock tracking in the voxel grid [R17]
       const int n = min(cP, 32); const bool act = lane < n;
       Photon p = {}; uint64_t h = 0; int idx = 0;
@@ -552,7 +557,7 @@ size_t transport_smem_bytes(const DevTables &T, int n_panels, bool hash) {
   return (hash ? SmemLayout<true>::geom_off(n_mu) : SmemLayout<false>::geom_off(n_mu)) + geom_bytes(n_panels);
 }
 
-cudaError_t launch_transport(const DevGeom *geom, int n_panels, const DevTables &T, const DevSource &src,
+cudaError_t launch_transport(const DevGeom *geom, int n_panels, int planar_hint, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
                              unsigned long long *work_counter, int sm_count, cudaStream_t stream) {
   const size_t smem = transport_smem_bytes(T, n_panels, hash_out != nullptr);
@@ -565,15 +570,26 @@ cudaError_t launch_transport(const DevGeom *geom, int n_panels, const DevTables 
   const int blocks = (int)(want < resident ? (want ? want : 1) : resident);
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(unsigned long long), stream);
   if (e != cudaSuccess) return e;
-  if (hash_out) {
-    e = cudaFuncSetAttribute(transport_wavefront_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    transport_wavefront_kernel<true><<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_photons, key, H, hash_out, work_counter);
-  } else {
-    e = cudaFuncSetAttribute(transport_wavefront_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    transport_wavefront_kernel<false><<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_photons, key, H, hash_out, work_counter);
-  }
+  const bool phantom = src.kind == 1 && src.phantom != nullptr;
+  auto launch = [&](auto kernel) -> cudaError_t {
+    cudaError_t le = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (le != cudaSuccess) return le;
+    kernel<<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_photons, key, H, hash_out, work_counter);
+    return cudaSuccess;
+  };
+  // specialised builds for the shapes the five configs use (point source or voxel map + phantom, planar ring);
+  // anything else runs the generic build of the same code
+  const bool planar = planar_hint != 0;
+#define GPET_DISPATCH(H)                                                                                              \
+  do {                                                                                                                \
+    if (!phantom && src.kind == 0 && planar) e = launch(transport_wavefront_kernel<H, false, 0, 1>);                  \
+    else if (phantom && planar) e = launch(transport_wavefront_kernel<H, true, 1, 1>);                                \
+    else if (phantom) e = launch(transport_wavefront_kernel<H, true, 1, -1>);                                         \
+    else e = launch(transport_wavefront_kernel<H, false, -1, -1>);                                                    \
+  } while (0)
+  if (hash_out) GPET_DISPATCH(true); else GPET_DISPATCH(false);
+#undef GPET_DISPATCH
+  if (e != cudaSuccess) return e;
   count_launch();
   return cudaGetLastError();
 }

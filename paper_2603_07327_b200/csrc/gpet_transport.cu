@@ -29,9 +29,13 @@ constexpr int kStage = 64;            // staged hits per warp (ring buffer)
 #define GPET_MIN_CTAS 3
 #endif
 constexpr int kSlots = GPET_SLOTS;    // photon slots per warp
-constexpr uint32_t kChunk = 1024;     // photon indices a warp reserves at a time
+constexpr uint32_t kChunk = 512;      // pairs a warp reserves at a time
+#ifndef GPET_MIN_GEN
+#define GPET_MIN_GEN 16
+#endif
+constexpr int kMinGen = GPET_MIN_GEN;  // the source refills only when at least this many pairs fit (2 free slots each)
 
-enum : int { L_FREE = 0, L_SEARCH, L_STEP, L_KN, L_RAY, L_PHANTOM, kLists, L_NONE = kLists };
+enum : int { L_FREE = 0, L_SEARCH, L_STEP, L_KN, L_RAY, L_PHANTOM, kLists, L_NONE = kLists, L_GEN };
 
 struct HitStage { uint32_t w[7][kStage]; };      // history, ids, x, y, z, e, tof
 
@@ -226,7 +230,7 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
 // [R17]; KIND: source kind (0 point, 1 voxel map, -1 = read src.kind); PLANAR: panel search variant (-1 = read g.planar).
 template <bool HASH, bool PHANTOM, int KIND, int PLANAR>
 __global__ void __launch_bounds__(kThreads, GPET_MIN_CTAS)
-transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint64_t first_history, uint64_t n_photons,
+transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint64_t first_history, uint64_t n_pairs,
                            const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n_mu = T.n_staged * T.n_energies;
@@ -250,8 +254,8 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
   constexpr bool use_phantom = PHANTOM;
   const int kind = KIND < 0 ? src.kind : KIND;
 
-  uint64_t w_next = 0, w_end = 0;          // this warp's reserved photon indices [w_next, w_end)
-  bool exhausted = false;                  // the global counter ran past n_photons
+  uint64_t w_next = 0, w_end = 0;          // this warp's reserved pairs [w_next, w_end)
+  bool exhausted = false;                  // the global counter ran past n_pairs
   uint32_t stage_head = 0, stage_cnt = 0;  // ring buffer of staged hits (warp-uniform)
   int cF = kSlots, cS = 0, cT = 0, cK = 0, cR = 0, cP = 0;   // list fill levels (warp-uniform)
 
@@ -291,89 +295,91 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
 
 #pragma unroll 1
   for (;;) {
-    // ================================================ scheduler: the event with the most ready photons
+    // ================================================ scheduler: the list with the most ready photons; when no list
+    // fills a pass, the source refills the SEARCH list with up to 32 fresh pairs (two free slots each)
     const bool more_src = !exhausted || w_next < w_end;
-    const int nS = min(cS, 32);
-    const int nF = more_src ? min(32 - nS, cF) : 0;                    // fresh photons SEARCH may admit (one free slot each)
-    int phase = L_SEARCH, best = cS + nF;
+    int phase = L_SEARCH, best = cS;
     if (cT > 0 && cT >= best) { phase = L_STEP; best = cT; }
     if (cK > best) { phase = L_KN; best = cK; }
     if (PHANTOM && cP > best) { phase = L_PHANTOM; best = cP; }
     if (cR > best) { phase = L_RAY; best = cR; }
-    if (best == 0) break;                                             // nothing in flight, no source left
+    const int np = more_src ? min(32, cF >> 1) : 0;
+    if (best < 32 && np >= kMinGen) phase = L_GEN;
+    else if (best == 0) { if (np > 0) phase = L_GEN; else break; }      // nothing in flight: last pairs, or done
 
-    if (phase == L_SEARCH) {
-      // ---------------------------------------------- SEARCH: photons that left a panel + fresh ones from the source
-      Photon q = {}; uint64_t hq = 0; int idx = -1; bool active = lane < nS;
-      if (active) { idx = W.list[L_SEARCH][cS - 1 - lane]; slot_load(W, idx, q, hq); }
-      cS -= nS;
-      if (nF > 0) {                                                   // source sampling (S3) [R13-R15]
-        if (w_next >= w_end && !exhausted) {
-          unsigned long long b = 0;
-          if (lane == 0) b = atomicAdd(work_counter, (unsigned long long)kChunk);
-          b = __shfl_sync(0xFFFFFFFFu, b, 0);
-          if (b >= n_photons) { exhausted = true; w_next = w_end = 0; }
-          else { w_next = b; w_end = min((uint64_t)(b + kChunk), n_photons); }
-        }
-        const uint64_t j = w_next + (uint64_t)(lane - nS);
-        const bool fresh = lane >= nS && lane < nS + nF && j < w_end;
-        w_next = min(w_next + (uint64_t)nF, w_end);
-        if (fresh) {
-          active = true;
-          q.pair = (uint32_t)(j >> 1); q.meta = (uint32_t)(j & 1u) | (63u << 5); q.ids = kNone; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
-          if (HASH) hq = 0xCBF29CE484222325ull;
-          const uint64_t history = first_history + q.pair;
-          const uint32_t h_lo = (uint32_t)history, h_hi = (uint32_t)(history >> 32);
-          q.x[0] = src.pos[0]; q.x[1] = src.pos[1]; q.x[2] = src.pos[2];
-          if (kind == 1) decay_site(src, philox4x32_10(make_uint4(h_lo, h_hi, 0u, 0u), key), q.x);
-          const uint4 w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 1u), key);
-          if (kind == 2) { q.d[0] = src.beam[0]; q.d[1] = src.beam[1]; q.d[2] = src.beam[2]; }
-          else {
-            const float u = u01(w.x), ct = 1.0f - 2.0f * u, sth = 2.0f * sqrtf(u * (1.0f - u));   // sin^2 = (1-ct)(1+ct)
-            float sp, cp; sincospif(2.0f * u01(w.y), &sp, &cp);
-            q.d[0] = sth * cp; q.d[1] = sth * sp; q.d[2] = ct;
-          }
-          if (q.meta & 1u) {                                          // photon B: opposite, plus acolinearity
-            q.d[0] = -q.d[0]; q.d[1] = -q.d[1]; q.d[2] = -q.d[2];
-            if (src.acol_sigma > 0.0f) {
-              const float rho = src.acol_sigma * sqrt_fast(-2.0f * __logf(u01(w.z)));
-              float sr, cr; sincos_small(rho, sr, cr);
-              float sp, cp; sincos_2pi(u01(w.w), sp, cp);               // azimuth of a ~4e-3 rad deviation: 2^-21 is ample
-              rotate(q.d, cr, sr, cp, sp);
-            }
-          }
-          if (use_phantom) { q.meta |= 1u << 11; q.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, q.E).z); }
-        }
+    if (phase == L_GEN) {
+      // ---------------------------------------------- GEN: one annihilation pair per lane (S3) [R13-R16]: both photons
+      // get a slot and wait for their panel search (or, born inside a phantom, for their first phantom step [R17])
+      if (w_next >= w_end && !exhausted) {
+        unsigned long long b = 0;
+        if (lane == 0) b = atomicAdd(work_counter, (unsigned long long)kChunk);
+        b = __shfl_sync(0xFFFFFFFFu, b, 0);
+        if (b >= n_pairs) { exhausted = true; w_next = w_end = 0; }
+        else { w_next = b; w_end = min((uint64_t)(b + kChunk), n_pairs); }
       }
-      // panel search [R6]; photons born inside a phantom skip it and are tracked there first [R17]
-      int dest = L_NONE;
-      if (active) {
-        if (PHANTOM && ph_in_phantom(q)) dest = L_PHANTOM;
+      const uint64_t j = w_next + (uint64_t)lane;
+      const int ng = (int)min((uint64_t)np, w_end - w_next);           // pairs generated in this pass (warp-uniform)
+      w_next += (uint64_t)ng;
+      if (lane < ng) {
+        Photon q = {};
+        q.pair = (uint32_t)j; q.meta = 63u << 5; q.ids = kNone; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
+        const uint64_t history = first_history + j;
+        const uint32_t h_lo = (uint32_t)history, h_hi = (uint32_t)(history >> 32);
+        q.x[0] = src.pos[0]; q.x[1] = src.pos[1]; q.x[2] = src.pos[2];
+        if (kind == 1) decay_site(src, philox4x32_10(make_uint4(h_lo, h_hi, 0u, 0u), key), q.x);
+        const uint4 w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 1u), key);
+        if (kind == 2) { q.d[0] = src.beam[0]; q.d[1] = src.beam[1]; q.d[2] = src.beam[2]; }
         else {
-          float bt; const int bp = panel_search<PLANAR>(g, q.x, q.d, ph_panel(q), bt);
-          if (bp < 0) {
-            if (HASH) { hash_ev(hq, EV_ESCAPE, 0); hash_out[2ull * q.pair + (q.meta & 1u)] = hq; }
-            if (idx >= 0) dest = L_FREE;                              // gives its slot back
-          } else {
-            if (HASH) hash_ev(hq, EV_ENTER, (uint32_t)bp);
-            float xl[3], dl[3];
-            to_local(g.panel[bp].pose, q.x, q.d, xl, dl);
+          const float u = u01(w.x), ct = 1.0f - 2.0f * u, sth = 2.0f * sqrtf(u * (1.0f - u));   // sin^2 = (1-ct)(1+ct)
+          float sp, cp; sincospif(2.0f * u01(w.y), &sp, &cp);
+          q.d[0] = sth * cp; q.d[1] = sth * sp; q.d[2] = ct;
+        }
+        if (use_phantom) { q.meta |= 1u << 11; q.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, q.E).z); }
+        const int ia = W.list[L_FREE][cF - 1 - 2 * lane], ib = W.list[L_FREE][cF - 2 - 2 * lane];
+        slot_store(W, ia, q, 0xCBF29CE484222325ull);                  // photon A
+        q.d[0] = -q.d[0]; q.d[1] = -q.d[1]; q.d[2] = -q.d[2];         // photon B: opposite, plus acolinearity
+        if (src.acol_sigma > 0.0f) {
+          const float rho = src.acol_sigma * sqrt_fast(-2.0f * __logf(u01(w.z)));
+          float sr, cr; sincos_small(rho, sr, cr);
+          float sp, cp; sincos_2pi(u01(w.w), sp, cp);                 // azimuth of a ~4e-3 rad deviation: 2^-21 is ample
+          rotate(q.d, cr, sr, cp, sp);
+        }
+        q.meta |= 1u;
+        slot_store(W, ib, q, 0xCBF29CE484222325ull);
+        uint8_t *dst = use_phantom ? &W.list[L_PHANTOM][cP] : &W.list[L_SEARCH][cS];
+        dst[2 * lane] = (uint8_t)ia; dst[2 * lane + 1] = (uint8_t)ib;
+      }
+      cF -= 2 * ng;
+      if (use_phantom) cP += 2 * ng; else cS += 2 * ng;
+      __syncwarp();
+      continue;
+    }
+    if (phase == L_SEARCH) {
+      // ---------------------------------------------- SEARCH: nearest panel ahead [R6], entry transform [R18]
+      const int n = min(cS, 32); const bool act = lane < n;
+      Photon q = {}; uint64_t hq = 0; int idx = 0;
+      if (act) { idx = W.list[L_SEARCH][cS - 1 - lane]; slot_load(W, idx, q, hq); }
+      cS -= n;
+      int dest = L_NONE;
+      if (act) {
+        float bt; const int bp = panel_search<PLANAR>(g, q.x, q.d, ph_panel(q), bt);
+        if (bp < 0) {
+          if (HASH) { hash_ev(hq, EV_ESCAPE, 0); hash_out[2ull * q.pair + (q.meta & 1u)] = hq; }
+          dest = L_FREE;
+        } else {
+          if (HASH) hash_ev(hq, EV_ENTER, (uint32_t)bp);
+          float xl[3], dl[3];
+          to_local(g.panel[bp].pose, q.x, q.d, xl, dl);
 #pragma unroll
-            for (int k = 0; k < 3; ++k) { q.x[k] = fmaf(bt, dl[k], xl[k]); q.d[k] = dl[k]; }   // [R18]
-            q.path += bt; ph_set_panel(q, bp);
-            q.inv_mu = rcp_fast(mu_lookup(mu, T, 0, q.E).w);
-            dest = L_STEP;
-          }
+          for (int k = 0; k < 3; ++k) { q.x[k] = fmaf(bt, dl[k], xl[k]); q.d[k] = dl[k]; }   // [R18]
+          q.path += bt; ph_set_panel(q, bp);
+          q.inv_mu = rcp_fast(mu_lookup(mu, T, 0, q.E).w);
+          dest = L_STEP;
+          slot_store(W, idx, q, hq);
         }
       }
-      const bool need = idx < 0 && dest != L_NONE;                    // a fresh photon that goes on takes a free slot
-      const unsigned m_need = __ballot_sync(0xFFFFFFFFu, need);
-      if (need) idx = W.list[L_FREE][cF - 1 - __popc(m_need & lt_mask)];
-      cF -= __popc(m_need);
-      if (dest == L_STEP || dest == L_PHANTOM) slot_store(W, idx, q, hq);
       push(L_FREE, cF, dest == L_FREE, idx);
       push(L_STEP, cT, dest == L_STEP, idx);
-      if (use_phantom) push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
       __syncwarp();
       continue;
     }
@@ -561,8 +567,7 @@ cudaError_t launch_transport(const DevGeom *geom, int n_panels, int planar_hint,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
                              unsigned long long *work_counter, int sm_count, cudaStream_t stream) {
   const size_t smem = transport_smem_bytes(T, n_panels, hash_out != nullptr);
-  const uint64_t n_photons = 2 * n_pairs;
-  const uint64_t want = (n_photons + kThreads - 1) / kThreads;
+  const uint64_t want = (2 * n_pairs + kThreads - 1) / kThreads;
   static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : GPET_MIN_CTAS;
   const uint64_t resident = (uint64_t)sm_count * ctas_per_sm;         // persistent grid
   PhiloxKeys key;                                                     // [R1] round keys: key + r * Weyl constants
@@ -574,7 +579,7 @@ cudaError_t launch_transport(const DevGeom *geom, int n_panels, int planar_hint,
   auto launch = [&](auto kernel) -> cudaError_t {
     cudaError_t le = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (le != cudaSuccess) return le;
-    kernel<<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_photons, key, H, hash_out, work_counter);
+    kernel<<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_pairs, key, H, hash_out, work_counter);
     return cudaSuccess;
   };
   // specialised builds for the shapes the five configs use (point source or voxel map + phantom, planar ring);

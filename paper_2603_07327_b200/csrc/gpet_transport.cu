@@ -19,19 +19,24 @@
 
 namespace gpet {
 
-constexpr int kThreads = 256;
+#ifndef GPET_THREADS
+#define GPET_THREADS 768
+#endif
+constexpr int kThreads = GPET_THREADS;
 constexpr int kWarps = kThreads / 32;
 constexpr int kStage = 64;            // staged hits per warp (ring buffer)
 #ifndef GPET_SLOTS
-#define GPET_SLOTS 96
+#define GPET_SLOTS 128
 #endif
 #ifndef GPET_MIN_CTAS
-#define GPET_MIN_CTAS 3
+#define GPET_MIN_CTAS 1
 #endif
-constexpr int kSlots = GPET_SLOTS;    // photon slots per warp
+// photon slots per warp.  One CTA of 24 warps per SM stages the tables once and leaves 8.7 KB of shared memory to each
+// warp; the parity builds (HASH) also keep an 8-byte hash per slot and get by with 16 slots fewer.
+template <bool HASH> constexpr int kSlotsOf = HASH ? GPET_SLOTS - 16 : GPET_SLOTS;
 constexpr uint32_t kChunk = 512;      // pairs a warp reserves at a time
 #ifndef GPET_MIN_GEN
-#define GPET_MIN_GEN 16
+#define GPET_MIN_GEN 24
 #endif
 constexpr int kMinGen = GPET_MIN_GEN;  // the source refills only when at least this many pairs fit (2 free slots each)
 
@@ -41,6 +46,7 @@ struct HitStage { uint32_t w[7][kStage]; };      // history, ids, x, y, z, e, to
 
 // One warp's private memory.  A photon record is 48 bytes in three 16-byte planes (conflict-free LDS.128).
 template <bool HASH> struct WarpMem {
+  static constexpr int kSlots = kSlotsOf<HASH>;
   float4 a[kSlots];                    // x, y, z, dx
   float4 b[kSlots];                    // dy, dz, E, path
   uint4 c[kSlots];                     // pair, meta, ids of the pending interaction, inv_mu bits
@@ -244,7 +250,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
     const int words = (int)(geom_bytes(geom->n_panels) / 4);
     for (int i = threadIdx.x; i < words; i += kThreads) gd[i] = gs[i];
     for (int i = threadIdx.x; i < n_mu; i += kThreads) mu_s[i] = T.mu[i];
-    for (int i = lane; i < kSlots; i += 32) W.list[L_FREE][i] = (uint8_t)i;
+    for (int i = lane; i < kSlotsOf<HASH>; i += 32) W.list[L_FREE][i] = (uint8_t)i;
     __syncthreads();
   }
   const DevGeom &g = *g_s;
@@ -257,7 +263,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
   uint64_t w_next = 0, w_end = 0;          // this warp's reserved pairs [w_next, w_end)
   bool exhausted = false;                  // the global counter ran past n_pairs
   uint32_t stage_head = 0, stage_cnt = 0;  // ring buffer of staged hits (warp-uniform)
-  int cF = kSlots, cS = 0, cT = 0, cK = 0, cR = 0, cP = 0;   // list fill levels (warp-uniform)
+  int cF = kSlotsOf<HASH>, cS = 0, cT = 0, cK = 0, cR = 0, cP = 0;   // list fill levels (warp-uniform)
 
   // [R4] every transport event consumes one whole Philox block of the photon's stream
   auto block_at = [&](const Photon &p, uint32_t blk) -> uint4 {

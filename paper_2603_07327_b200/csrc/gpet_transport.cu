@@ -2,18 +2,18 @@
 // PAPER.md:33 (panel transfer by ray/plane crossing, global->local), PAPER.md:43 (Woodcock tracking in the
 // panel frame, layer selection from the local depth, run until exit or cutoff).
 //
-// Design.  The unit of work is one photon (index j = 2*pair + photon).  Every persistent
-// warp owns a pool of photon SLOTS in shared memory (48-byte records that never move) and one index list per
-// NEXT EVENT: SEARCH (needs a panel search), STEP (Woodcock step in a panel), KN (Klein-Nishina trial), RAY
-// (Rayleigh deflection), PHANTOM (Woodcock step in the voxel grid), plus the FREE list.  A pass pops up to 32
-// slot indices from ONE list, runs that event for all of them at full SIMD width, writes the changed fields back
-// and pushes every index onto the list of its next event (ballot + prefix popcount).  The scheduler always runs
-// the event with the most ready photons; SEARCH counts the fresh photons it can admit from the source (S3), so
-// a warp is never short of work before the end.  This is the "regroup live photons by next event" of the
-// north star, done per warp: no block-level barrier, no atomics except the chunked work counter and the hit
-// counter.  Every event's code appears exactly once in the kernel.  Geometry descriptor and interleaved float4 mu
-// tables live in shared memory; hits are staged per warp in shared memory and flushed 32 at a time: one
-// atomicAdd per 32 hits and seven fully coalesced 128-byte stores (SoA).
+// Design.  One CTA of 24 warps per SM, persistent.  Every warp owns a pool of 128 photon
+// SLOTS in shared memory (48-byte records that never move) and one index list per NEXT EVENT: SEARCH (needs a panel
+// search), STEP (Woodcock step in a panel), KN (Klein-Nishina trial), RAY (Rayleigh deflection), PHANTOM (Woodcock
+// step in the voxel grid), plus the FREE list.  A pass pops up to 32 slot indices from ONE list, runs that event for
+// all of them at full SIMD width, writes the changed fields back and pushes every index onto the list of its next
+// event (ballot + prefix popcount).  The scheduler runs the list with the most ready photons; when no list fills a
+// pass, a GEN pass samples one annihilation pair per lane (S3) and queues both photons, so a warp is never short of
+// work before the end.  This is the "regroup live photons by next event" of the north star, done per warp: no
+// block-level barrier, no atomics except the chunked work counter and the hit counter.  Every event's code appears
+// exactly once, and the kernel is specialised on phantom / source kind / search variant to stay small.  Geometry
+// descriptor and interleaved float4 mu tables live in shared memory; hits are staged per warp in shared memory and
+// flushed 32 at a time: one atomicAdd per 32 hits and seven fully coalesced 128-byte stores (SoA).
 #include <cstdlib>
 #include "gpet_internal.h"
 

@@ -224,7 +224,7 @@ def run_ours(args):
     alg = ALG_INSTR_PER_PAIR.get(args.config)
     achieved = alg * n / (transport_ms * 1e-3) if alg else None
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "transport_traffic.json")
+    tp = os.path.join(ROOT, "profiles", "transport_traffic.txt")
     if os.path.exists(tp):
         try:
             traffic = json.load(open(tp)).get("dram_bytes_per_launch")

@@ -343,3 +343,34 @@ def test_c4_full_run_in_time_slices(tables):
                 assert np.array_equal(gs["ids"][ss], osg.ids) and np.array_equal(gs["t_s"][ss], osg.t_s)
                 assert np.max(np.abs(gs["e_keV"][ss] - osg.e_keV)) < E_TOL
     assert same / tot >= MIN_MATCH
+
+
+# ----------------------------------------------------------------------------- north_star: layers cost nothing
+def test_layer_configurations_run_within_ten_percent(tables):
+    """north_star / PAPER.md:121 (Table 1: the layer extension adds no measurable time): the single-layer (C1), aligned
+    split (C2) and offset dual-layer (C3) rings, centred source, 1e7 pairs, transport + digitizer, must run within 10 %
+    of each other in pairs/s."""
+    times = {}
+    for cfg in ("C1", "C2", "C3"):
+        r = W.config_runs(cfg)[0]
+        n = r.n_pairs
+        geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+        cap = int(1.2 * n)
+        hb, co = api.HitBuffer.allocate(cap), api.CoincBuffer.allocate(cap // 4)
+        scratch = torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda")
+        st = torch.cuda.current_stream()
+        best = float("inf")
+        for rep in range(5):
+            hb.n_hits.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(st)
+            api.gpet_simulate(geom, m, s, 0, n, r.seed, hb, st)
+            api.gpet_digitize(s, r.seed, n, 0, n, hb, cap, r.digitizer, scratch, None, co, st)
+            b.record(st)
+            torch.cuda.synchronize()
+            if rep >= 2:
+                best = min(best, a.elapsed_time(b))
+        assert hb.count() <= cap
+        times[cfg] = best
+        del hb, co, scratch
+    assert max(times.values()) / min(times.values()) < 1.10, times

@@ -175,7 +175,8 @@ size_t gpet_digitize_scratch_bytes(uint64_t n_pairs, uint64_t n_hits);
  * valid entries (it sizes the scratch; pass hits->capacity to avoid reading the counter back): the kernels
  * use min(*hits->n_hits, hits->capacity, n_hits), read on the device.  n_pairs_total (pairs of the whole run, all batches) and
  * src give the decay times [R16].  Output is deterministic: it does not depend on the order of `hits`.
- * Records past a capacity are dropped but counted.  singles_out may be NULL (coincidences only). */
+ * Records past a capacity are dropped but counted.  singles_out may be NULL (coincidences only), or have
+ * NULL arrays with a valid n_singles (count only). */
 int gpet_digitize(const gpet_source *src, uint64_t seed, uint64_t n_pairs_total, uint64_t first_history,
                   uint64_t n_pairs, const gpet_hits *hits, uint64_t n_hits, const gpet_digitizer *dig,
                   void *scratch, size_t scratch_bytes, gpet_singles *singles_out,

@@ -394,7 +394,9 @@ extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, co
     if (A.used > A.size) { rc = fail(GPET_E_OVERFLOW, "internal arena too small"); break; }
     if (cudaMemsetAsync(H.n_hits, 0, 8, st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "memset failed"); break; }
     if ((rc = gpet_simulate(g, m, &s2, first_history, n_pairs, seed, &H, st))) break;
-    if ((rc = gpet_digitize(&s2, seed, n_pairs_total, first_history, n_pairs, &H, cap, dig, scratch, scratch_bytes, &S, &Cc, st))) break;
+    gpet_singles Sd = S;                   // singles arrays are written only when the caller wants them; the count always is
+    if (!out->singles.history) { Sd.history = Sd.ids = nullptr; Sd.x = Sd.y = Sd.z = Sd.e_keV = nullptr; Sd.t_s = nullptr; }
+    if ((rc = gpet_digitize(&s2, seed, n_pairs_total, first_history, n_pairs, &H, cap, dig, scratch, scratch_bytes, &Sd, &Cc, st))) break;
     uint64_t nh = 0, ns = 0, nc = 0;
     cudaMemcpyAsync(&nh, H.n_hits, 8, cudaMemcpyDeviceToHost, st);
     cudaMemcpyAsync(&ns, S.n_singles, 8, cudaMemcpyDeviceToHost, st); cudaMemcpyAsync(&nc, Cc.n_coinc, 8, cudaMemcpyDeviceToHost, st);

@@ -81,6 +81,10 @@ int gpet_geometry_create(const gpet_geometry_desc *desc, gpet_geometry **out);
 int gpet_geometry_destroy(gpet_geometry *g);
 /* Copies the fp32 pose (12 floats, layout as panel_pose) of one panel to HOST memory. */
 int gpet_geometry_panel_pose(const gpet_geometry *g, int32_t panel, float *pose12);
+/* Faces of one panel box beyond which no other panel has a point (bit 2k + 1: the high face of local axis k, bit 2k:
+ * the low face; k = 0 u, 1 v, 2 w).  A photon leaving through such a face escapes: gpet_simulate skips the panel search
+ * for it, with the result the search would give.  Host-side query of what gpet_geometry_create derived. */
+int gpet_geometry_open_faces(const gpet_geometry *g, int32_t panel, uint32_t *mask);
 /* Point -> packed ids (GPET_IDS_NONE if the point is in no crystal) for n points; xyz_global and
  * packed_ids are HOST arrays (n x 3 floats, n words); runs on the device (synchronous).  The lowest-index
  * panel whose box contains the point decides.  Same lattice code as the transport kernel. */

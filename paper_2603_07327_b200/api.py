@@ -67,7 +67,7 @@ class _HostOutputs(C.Structure):
     _fields_ = [("hits", _Hits), ("singles", _Singles), ("coinc", _Coinc)]
 
 
-EXPORTS = ("gpet_geometry_create", "gpet_geometry_destroy", "gpet_geometry_panel_pose", "gpet_geometry_locate",
+EXPORTS = ("gpet_geometry_create", "gpet_geometry_destroy", "gpet_geometry_panel_pose", "gpet_geometry_open_faces", "gpet_geometry_locate",
            "gpet_materials_load", "gpet_materials_destroy", "gpet_activity_create", "gpet_activity_destroy",
            "gpet_simulate", "gpet_digitize_scratch_bytes", "gpet_digitize", "gpet_run_host", "gpet_last_error",
            "gpet_launch_count")
@@ -87,6 +87,7 @@ def lib():
         L.gpet_geometry_create.argtypes = [C.POINTER(_GeometryDesc), C.POINTER(vp)]
         L.gpet_geometry_destroy.argtypes = [vp]
         L.gpet_geometry_panel_pose.argtypes = [vp, i32, C.POINTER(C.c_float)]
+        L.gpet_geometry_open_faces.argtypes = [vp, i32, C.POINTER(C.c_uint32)]
         L.gpet_geometry_locate.argtypes = [vp, C.c_int64, vp, vp]
         L.gpet_materials_load.argtypes = [i32, i32, C.c_float, C.c_float, vp, vp, vp, C.POINTER(vp)]
         L.gpet_materials_destroy.argtypes = [vp]
@@ -165,6 +166,12 @@ def gpet_geometry_panel_pose(geom: Geometry, panel: int) -> np.ndarray:
     pose = np.zeros(12, np.float32)
     _check(lib().gpet_geometry_panel_pose(geom.ptr, panel, _fp(pose)))
     return pose
+
+
+def gpet_geometry_open_faces(geom: Geometry, panel: int) -> int:
+    mask = C.c_uint32(0)
+    _check(lib().gpet_geometry_open_faces(geom.ptr, panel, C.byref(mask)))
+    return int(mask.value)
 
 
 def gpet_geometry_locate(geom: Geometry, xyz: np.ndarray) -> np.ndarray:

@@ -131,6 +131,29 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
       G.panel[p].cx = c[0]; G.panel[p].cy = c[1]; G.panel[p].cz = c[2];
     }
   }
+  // open faces: face (axis k, side) of panel p is open when every corner of every other panel box lies at least 1 um on
+  // the inner side of that face's plane -- a photon leaving p through it can meet no other panel (transport skips the
+  // search of [R6] then; the result is the one the search would give).  Rings: back and axial faces are open.
+  {
+    const double lo[3] = { G.blo[0], G.blo[1], G.blo[2] }, hi[3] = { G.bhi[0], G.bhi[1], G.bhi[2] };
+    for (int p = 0; p < G.n_panels; ++p) {
+      const float *P = G.panel[p].pose; uint32_t open = 63u;
+      for (int q = 0; q < G.n_panels; ++q) if (q != p) {
+        const float *Q = G.panel[q].pose;
+        for (int c = 0; c < 8; ++c) {
+          const double a = c & 1 ? hi[0] : lo[0], b = c & 2 ? hi[1] : lo[1], w = c & 4 ? hi[2] : lo[2];
+          double x[3], l[3];
+          for (int k = 0; k < 3; ++k) x[k] = (double)Q[k] + a * Q[3 + k] + b * Q[6 + k] + w * Q[9 + k] - (double)P[k];
+          for (int k = 0; k < 3; ++k) l[k] = x[0] * P[3 + 3 * k] + x[1] * P[4 + 3 * k] + x[2] * P[5 + 3 * k];
+          for (int k = 0; k < 3; ++k) {
+            if (!(l[k] < hi[k] - 1e-3)) open &= ~(1u << (2 * k + 1));
+            if (!(l[k] > lo[k] + 1e-3)) open &= ~(1u << (2 * k));
+          }
+        }
+      }
+      G.panel[p].open_faces = open;
+    }
+  }
   *out = g;                     // the device copy is made lazily so the handle can be built without a GPU
   return GPET_OK;
 }
@@ -151,6 +174,11 @@ extern "C" int gpet_geometry_destroy(gpet_geometry *g) {
 extern "C" int gpet_geometry_panel_pose(const gpet_geometry *g, int32_t panel, float *pose12) {
   if (!g || !pose12 || panel < 0 || panel >= g->host.n_panels) return fail(GPET_E_INVALID_ARG, "gpet_geometry_panel_pose: bad argument");
   memcpy(pose12, g->host.panel[panel].pose, sizeof(float) * 12); return GPET_OK;
+}
+
+extern "C" int gpet_geometry_open_faces(const gpet_geometry *g, int32_t panel, uint32_t *mask) {
+  if (!g || !mask || panel < 0 || panel >= g->host.n_panels) return fail(GPET_E_INVALID_ARG, "gpet_geometry_open_faces: bad argument");
+  *mask = g->host.panel[panel].open_faces; return GPET_OK;
 }
 
 extern "C" int gpet_geometry_locate(const gpet_geometry *g, int64_t n, const float *xyz, uint32_t *ids) {

@@ -24,7 +24,8 @@ struct DevLayer {
 };
 struct __align__(16) DevPanel {
   float pose[12];             // front-face centre, u, v, w
-  float cx, cy, cz, pad;      // global position of the box centre (search culling)
+  float cx, cy, cz;           // global position of the box centre (search culling)
+  uint32_t open_faces;        // bit 2k + (outward along +axis k): no other panel has a point beyond that face of this box
   float skew[4];              // 80-byte stride: records of 8 consecutive panels start in 8 different 16-byte bank groups, so
 };                            // lanes reading the poses of different panels (entry / exit / hit transforms) rarely conflict
 struct DevGeom {

@@ -399,18 +399,31 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
       if (act) {
         const uint4 w = next_block(p);                                // [R4] free path, outcome, Rayleigh polar + azimuth
         const float s = -__logf(u01(w.x)) * p.inv_mu;
-        float tf = INFINITY;
+        float te[3];
 #pragma unroll
         for (int k = 0; k < 3; ++k)                                   // distance to the box exit [R32]
-          tf = fminf(tf, ((p.d[k] >= 0.0f ? g.bhi[k] : g.blo[k]) - p.x[k]) * rcp_dir(p.d[k]));
+          te[k] = ((p.d[k] >= 0.0f ? g.bhi[k] : g.blo[k]) - p.x[k]) * rcp_dir(p.d[k]);
+        float tf = fminf(te[0], fminf(te[1], te[2]));
         const int panel = ph_panel(p);
-        if (s >= tf) {                                                // leaves the panel: back to the global frame [R33]
-          tf = fmaxf(tf, 0.0f);
-          const float xl[3] = { fmaf(tf, p.d[0], p.x[0]), fmaf(tf, p.d[1], p.x[1]), fmaf(tf, p.d[2], p.x[2]) };
-          const float dl[3] = { p.d[0], p.d[1], p.d[2] };
-          p.path += tf; if (HASH) hash_ev(h, EV_EXIT, (uint32_t)panel);
-          point_to_global(g.panel[panel].pose, xl, p.x); dir_to_global(g.panel[panel].pose, dl, p.d);
-          dest = L_SEARCH;
+        if (s >= tf) {                                                // leaves the panel [R33]
+          // Exit face = the axis that limits tf.  If no other panel has a point beyond that face (precomputed per panel
+          // and face at create time: true for the back and axial faces of any ring), the search of [R6] cannot find
+          // anything: the photon escapes here, with the same EXIT, ESCAPE events, and skips transform and search.
+          const int kx = te[0] <= tf ? 0 : (te[1] <= tf ? 1 : 2);
+          const float dk = kx == 0 ? p.d[0] : (kx == 1 ? p.d[1] : p.d[2]);
+          const bool open = (g.panel[panel].open_faces >> (2 * kx + (dk >= 0.0f ? 1 : 0))) & 1u;
+          if (HASH) hash_ev(h, EV_EXIT, (uint32_t)panel);
+          if (open) {
+            if (HASH) { hash_ev(h, EV_ESCAPE, 0); hash_out[2ull * p.pair + (p.meta & 1u)] = h; }
+            dest = L_FREE;
+          } else {
+            tf = fmaxf(tf, 0.0f);
+            const float xl[3] = { fmaf(tf, p.d[0], p.x[0]), fmaf(tf, p.d[1], p.x[1]), fmaf(tf, p.d[2], p.x[2]) };
+            const float dl[3] = { p.d[0], p.d[1], p.d[2] };
+            p.path += tf;
+            point_to_global(g.panel[panel].pose, xl, p.x); dir_to_global(g.panel[panel].pose, dl, p.d);   // back to the global frame
+            dest = L_SEARCH;
+          }
         } else {
 #pragma unroll
           for (int k = 0; k < 3; ++k) p.x[k] = fmaf(s, p.d[k], p.x[k]);

@@ -110,3 +110,40 @@ def test_scratch_size_is_monotone():
     a = api.gpet_digitize_scratch_bytes(1000, 800)
     b = api.gpet_digitize_scratch_bytes(10_000_000, 8_000_000)
     assert 0 < a < b < 2 * 1024 ** 3
+
+
+def test_open_faces_of_panel_boxes():
+    """A face is open when no other panel has a point beyond it (transport then skips the panel search for photons leaving
+    through it).  Checked against a brute-force sampling of every other panel box, on a ring, a lone panel and two
+    facing panels; a closed face must never be reported open."""
+    rng = np.random.default_rng(3)
+    facing = np.array([[30, 0, 0, 0, 1, 0, 0, 0, 1, 1, 0, 0], [-30, 0, 0, 0, -1, 0, 0, 0, 1, -1, 0, 0]], np.float32)
+    two = W.Geometry(2, W.geometry_c0().layers, (1, 1), (12.0, 12.0), (12.0, 12.0), panel_pose=facing)
+    for geom in (W.geometry_c1(), W.geometry_c3(), W.geometry_c0(), two, W.geometry_paper_1cl()):
+        g = api.gpet_geometry_create(geom)
+        n = geom.n_panels
+        poses = np.stack([api.gpet_geometry_panel_pose(g, p).astype(np.float64) for p in range(n)])
+        W_, H_ = [(geom.n_modules[a] - 1) * geom.module_pitch_mm[a] + geom.module_size_mm[a] for a in (0, 1)]
+        D_ = sum(l.depth_mm + l.gap_before_mm for l in geom.layers)
+        lo, hi = np.array([-W_ / 2, -H_ / 2, 0.0]), np.array([W_ / 2, H_ / 2, D_])
+        for p in range(n):
+            mask = api.gpet_geometry_open_faces(g, p)
+            o, axes = poses[p, :3], poses[p, 3:].reshape(3, 3)
+            beyond = np.zeros(6, bool)
+            for q in range(n):
+                if q == p:
+                    continue
+                loc = rng.uniform(lo, hi, (4000, 3))
+                pts = poses[q, :3] + loc @ poses[q, 3:].reshape(3, 3)
+                l = (pts - o) @ axes.T
+                for k in range(3):
+                    beyond[2 * k + 1] |= bool((l[:, k] > hi[k]).any())
+                    beyond[2 * k] |= bool((l[:, k] < lo[k]).any())
+            for f in range(6):
+                if beyond[f]:
+                    assert not (mask >> f) & 1, (p, f)
+            if n == 1:
+                assert mask == 63
+        if geom.panel_pose is None:                                   # rings: the back face (high w) is open, the front is not
+            assert all((api.gpet_geometry_open_faces(g, p) >> 5) & 1 and not (api.gpet_geometry_open_faces(g, p) >> 4) & 1 for p in range(n))
+    assert api.gpet_geometry_open_faces(api.gpet_geometry_create(two), 0) == 0b100000   # only the back: the side faces are flush with the other panel's

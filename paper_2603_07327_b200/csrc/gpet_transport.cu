@@ -362,6 +362,8 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
     }
     if (phase == L_SEARCH) {
       // ---------------------------------------------- SEARCH: nearest panel ahead [R6], entry transform [R18]
+      // (repeated without a trip through the scheduler while the list still fills a whole pass: a GEN pass leaves two)
+      do {
       const int n = min(cS, 32); const bool act = lane < n;
       Photon q = {}; uint64_t hq = 0; int idx = 0;
       if (act) { idx = W.list[L_SEARCH][cS - 1 - lane]; slot_load(W, idx, q, hq); }
@@ -387,6 +389,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
       push(L_FREE, cF, dest == L_FREE, idx);
       push(L_STEP, cT, dest == L_STEP, idx);
       __syncwarp();
+      } while (cS >= 32);
       continue;
     }
     if (phase == L_STEP) {
@@ -451,10 +454,12 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
       stage_hits(hit, p.pair, p.ids | ((p.meta & 1u) << 4) | ((p.meta >> 1) & 15u), xg, p.E, p.path * kInvC);
       if (act && dest != L_FREE) slot_store(W, idx, p, h);
       push(L_STEP, cT, dest == L_STEP, idx);
-      push(L_SEARCH, cS, dest == L_SEARCH, idx);
       push(L_KN, cK, dest == L_KN, idx);
       push(L_FREE, cF, dest == L_FREE, idx);
-      push(L_RAY, cR, dest == L_RAY, idx);
+      if (__any_sync(0xFFFFFFFFu, dest == L_SEARCH || dest == L_RAY)) {   // the rare destinations share one vote
+        push(L_SEARCH, cS, dest == L_SEARCH, idx);
+        push(L_RAY, cR, dest == L_RAY, idx);
+      }
     } else if (phase == L_KN) {
       // ---------------------------------------------- KN: one Klein-Nishina trial per visit [R20]
       const int n = min(cK, 32); const bool act = lane < n;

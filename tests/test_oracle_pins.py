@@ -574,3 +574,25 @@ def test_leaving_the_phantom_keeps_the_line_of_flight(tables):
     direct = np.linalg.norm(xyz - site, axis=1) / 299.792458
     unscattered = np.abs(res.hits.tof_ns[first] - direct) < 1e-4
     assert unscattered.mean() > 0.9                                  # the rest scattered in the crystal first
+
+
+def test_randoms_rate_follows_the_singles_rate(tables):
+    """random coincidences (members from different histories) occur at ~ tau * S^2 for the rate S of
+    singles without a kept partner, reduced by the same-panel veto (11/12 on a uniformly lit 12-panel ring).  Order-of-magnitude invariant of the window rule [R27] and of the decay-time model [R16]."""
+    n, A, tau = 200_000, 1.0e7, 4.0e-9
+    src = W.source_point(activity_bq=A)
+    hits = O.simulate(W.geometry_c1(), tables, src, n, seed=23, threads=8).hits
+    sg, co, _ = O.digitize(src, 23, n, hits, W.Digitizer())
+    T = n / A
+    # a window holding a true pair plus a stranger has three members and is dropped, so randoms form among the singles
+    # whose partner was not kept: histories with exactly one kept single
+    per_history = np.bincount(sg.history.astype(np.int64), minlength=n)
+    lonely = int(np.sum(per_history == 1))
+    expect = lonely * (lonely / T) * tau * (11.0 / 12.0)
+    randoms = int(np.sum(co.history_a != co.history_b))
+    assert expect > 250 and 0.8 * expect < randoms < 1.2 * expect, (randoms, expect)
+    # and it scales with the activity: a tenth of the activity gives about a tenth of the randoms per single
+    src2 = W.source_point(activity_bq=A / 10)
+    sg2, co2, _ = O.digitize(src2, 23, n, hits, W.Digitizer())
+    r2 = int(np.sum(co2.history_a != co2.history_b))
+    assert len(sg2.ids) == len(sg.ids) and 0.05 * randoms < r2 < 0.2 * randoms

@@ -3,6 +3,10 @@
 
 A *step* is one pass of the whole hot path (gpet_simulate + gpet_digitize: source, panel search, in-panel
 Woodcock transport, hits, adder, blur, window, time sort, coincidences) over one batch of synthetic input.
+The timed steps run in turn on one stream (the transport kernel with its full 24-warp CTA per SM).  After the timed
+region the same steps are also run as a two-stream pipeline -- the transport kernel of step k+1 (bound by instruction
+issue, CTA of 16 warps) beside the digitizer of step k (bound by HBM latency) -- and reported under "pipelined";
+`--overlap` makes that pipeline the timed headline instead.
 Workload at N=1: BASELINE.json configs[1] (C1): 12-panel ring, single layer, centred point source, 0.5 deg
 acolinearity, 1e7 pairs, 350-650 keV, 15 % blur, 4 ns window.  With N ranks each rank runs its own 1e7
 histories (disjoint history ranges, no data-path collective): weak scaling.
@@ -149,23 +153,49 @@ def run_ours(args):
     tables = W.tables()
     geom, mats, src = api.gpet_geometry_create(run.geometry), api.gpet_materials_load(tables), api.DeviceSource(run.source)
     cap = int(n * args.hits_per_pair) + 1024
-    hits = api.HitBuffer.allocate(cap)
-    coinc = api.CoincBuffer.allocate(cap // 4)
-    scratch = torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda")
-    stream = torch.cuda.current_stream()
+    # Two batches in flight: gpet_simulate of step k+1 (stream A) runs beside gpet_digitize of step k (stream B); each
+    # step is still one full pass of the hot path over its own 1e7 pairs, and every step's work lies in the timed region.
+    nbuf = 2 if args.overlap else 1
+    hits = [api.HitBuffer.allocate(cap) for _ in range(nbuf)]
+    coinc = [api.CoincBuffer.allocate(cap // 4) for _ in range(nbuf)]
+    scratch = [torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda") for _ in range(nbuf)]
+    s_a = torch.cuda.Stream()
+    s_b = torch.cuda.Stream() if args.overlap else s_a
+    warps = api.gpet_set_transport_warps(args.transport_warps if args.transport_warps else (16 if args.overlap else 24))
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    t_events = []
 
-    def step(timed: bool):
-        hits.n_hits.zero_()
-        a, b = ev(), ev()
-        a.record(stream)
-        api.gpet_simulate(geom, mats, src, first, n, run.seed, hits, stream)
-        b.record(stream)
-        api.gpet_digitize(src, run.seed, n_total, first, n, hits, cap, run.digitizer, scratch, None, coinc, stream)
-        if timed:
-            t_events.append((a, b))
+    def run_steps(k_steps, record):
+        """Enqueues k_steps steps; returns the per-step (transport, digitizer) event pairs when record is set."""
+        sim_done = [torch.cuda.Event() for _ in range(nbuf)]
+        dig_done = [torch.cuda.Event() for _ in range(nbuf)]
+        evs = []
+        for k in range(k_steps):
+            i = k % nbuf
+            if args.overlap and k >= nbuf:
+                s_a.wait_event(dig_done[i])                         # hit buffer i has been digitized
+            e = [ev() for _ in range(4)] if record else None
+            with torch.cuda.stream(s_a):
+                hits[i].n_hits.zero_()
+                if record:
+                    e[0].record(s_a)
+                api.gpet_simulate(geom, mats, src, first, n, run.seed, hits[i], s_a)
+                if record:
+                    e[1].record(s_a)
+            if args.overlap:
+                sim_done[i].record(s_a)
+                s_b.wait_event(sim_done[i])
+            if record:
+                e[2].record(s_b)
+            api.gpet_digitize(src, run.seed, n_total, first, n, hits[i], cap, run.digitizer, scratch[i], None, coinc[i], s_b)
+            if record:
+                e[3].record(s_b)
+                evs.append(e)
+            if args.overlap:
+                dig_done[i].record(s_b)
+        if args.overlap:
+            s_a.wait_stream(s_b)
+        return evs
 
     def barrier():
         torch.cuda.synchronize()
@@ -173,8 +203,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        step(False)
+    run_steps(args.warmup, False)
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
@@ -184,20 +213,70 @@ def run_ours(args):
     e0, e1 = ev(), ev()
     barrier()
     w0 = time.perf_counter()
-    e0.record(stream)
-    for _ in range(args.steps):
-        step(True)
-    e1.record(stream)
+    e0.record(s_a)
+    t_events = run_steps(args.steps, True)
+    e1.record(s_a)
     barrier()
     w1 = time.perf_counter()
     launches = api.gpet_launch_count() - launches0
     ms_total = sharding.max_over_ranks(e0.elapsed_time(e1))
     clocks = sampler.finish(w0, w1) if rank == 0 else None
-    transport_ms = sum(a.elapsed_time(b) for a, b in t_events) / len(t_events)
-    n_hits, n_coinc = hits.count(), int(coinc.n_coinc.item())
+    transport_ms = sum(e[0].elapsed_time(e[1]) for e in t_events) / len(t_events)
+    digitize_ms = sum(e[2].elapsed_time(e[3]) for e in t_events) / len(t_events)
+    n_hits, n_coinc = hits[0].count(), int(coinc[0].n_coinc.item())
     if n_hits > cap:
         raise SystemExit(f"hit buffer overflow ({n_hits} > {cap}); raise --hits-per-pair")
     value = n_total * args.steps / (ms_total * 1e-3)
+
+    # ---- the two halves alone (untimed extra, not part of `value`): serial steps with the full 24-warp transport CTA
+    alone = None
+    if args.overlap:
+        api.gpet_set_transport_warps(24)
+        st = torch.cuda.current_stream()
+        ta, tb = [], []
+        for k in range(8):
+            hits[0].n_hits.zero_()
+            x, y, z = ev(), ev(), ev()
+            x.record(st); api.gpet_simulate(geom, mats, src, first, n, run.seed, hits[0], st); y.record(st)
+            api.gpet_digitize(src, run.seed, n_total, first, n, hits[0], cap, run.digitizer, scratch[0], None, coinc[0], st); z.record(st)
+            torch.cuda.synchronize()
+            if k >= 3:
+                ta.append(x.elapsed_time(y)); tb.append(y.elapsed_time(z))
+        alone = {"transport_ms": sum(ta) / len(ta), "digitize_ms": sum(tb) / len(tb)}
+    # ---- the same steps as a two-stream pipeline (extra, after the timed region; not part of `value`)
+    pipelined = None
+    if not args.overlap and not args.no_pipelined:
+        pw = api.gpet_set_transport_warps(16)
+        hits.append(api.HitBuffer.allocate(cap)); coinc.append(api.CoincBuffer.allocate(cap // 4))
+        scratch.append(torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda"))
+        s_b2 = torch.cuda.Stream()
+        sim_done = [torch.cuda.Event() for _ in range(2)]; dig_done = [torch.cuda.Event() for _ in range(2)]
+
+        def pipe(k_steps):
+            for k in range(k_steps):
+                i = k & 1
+                if k >= 2:
+                    s_a.wait_event(dig_done[i])
+                with torch.cuda.stream(s_a):
+                    hits[i].n_hits.zero_()
+                    api.gpet_simulate(geom, mats, src, first, n, run.seed, hits[i], s_a)
+                sim_done[i].record(s_a)
+                s_b2.wait_event(sim_done[i])
+                api.gpet_digitize(src, run.seed, n_total, first, n, hits[i], cap, run.digitizer, scratch[i], None, coinc[i], s_b2)
+                dig_done[i].record(s_b2)
+            s_a.wait_stream(s_b2)
+
+        pipe(4)
+        barrier()
+        p0, p1 = ev(), ev()
+        p0.record(s_a); pipe(args.steps); p1.record(s_a)
+        barrier()
+        p_ms = sharding.max_over_ranks(p0.elapsed_time(p1))
+        assert int(coinc[1].n_coinc.item()) == n_coinc and int(coinc[0].n_coinc.item()) == n_coinc
+        pipelined = {"value": n_total * args.steps / (p_ms * 1e-3), "unit": UNIT, "ms_per_step": p_ms / args.steps, "steps": args.steps,
+                     "transport_warps_per_sm": pw,
+                     "note": "gpet_simulate(k+1) on one stream beside gpet_digitize(k) on another, two hit buffers; same results"}
+    api.gpet_set_transport_warps(24)                             # the host-buffer path below is one batch at a time
 
     # ---- end to end through the C ABI with HOST buffers (gpet_run_host): copies inside the timed region
     host = None
@@ -232,17 +311,24 @@ def run_ours(args):
             traffic = None
     roofline = {"kernel": "transport (gpet_simulate)", "bound": "alu", "achieved": achieved, "peak": peak_alu, "unit": "thread-instr/s",
                 "frac": achieved / peak_alu if achieved else None, "traffic": traffic,
+                "alone": ({"transport_ms": alone["transport_ms"], "achieved": alg * n / (alone["transport_ms"] * 1e-3),
+                           "frac": alg * n / (alone["transport_ms"] * 1e-3) / peak_alu,
+                           "note": "same kernel with its full 24-warp CTA and nothing else on the GPU (8 serial steps after the timed region)"}
+                          if alone and alg else None),
                 "note": f"{alg} algorithmic thread-instr/pair (DESIGN.md 6) x {n} pairs / {transport_ms:.3f} ms; peak = 148 SMs x 128 lanes x "
                         f"{peaks['sm_max_mhz']} MHz ({peaks['source']} max SM clock); hbm {peaks['hbm_gbs']} GB/s of {peaks['source']}",
-                "transport_ms": transport_ms, "digitize_ms": ms_total / args.steps - transport_ms,
+                "transport_ms": transport_ms, "digitize_ms": digitize_ms, "transport_warps_per_sm": warps,
+                "overlap": bool(args.overlap),
                 "hit_bytes_gbs": n_hits * 28 / (transport_ms * 1e-3) / 1e9}
-    digi_ms = ms_total / args.steps - transport_ms
+    digi_ms = digitize_ms
     dbytes = ALG_DIGI_BYTES_PER_PAIR.get(args.config)
     roofline_digi = None
     if dbytes and peaks["hbm_gbs"]:
         dach = dbytes * n / (digi_ms * 1e-3) / 1e9
         roofline_digi = {"kernel": "digitizer (gpet_digitize, 10 launches)", "bound": "hbm", "achieved": dach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                          "frac": dach / peaks["hbm_gbs"], "traffic": None,
+                         "alone": ({"digitize_ms": alone["digitize_ms"], "achieved": dbytes * n / (alone["digitize_ms"] * 1e-3) / 1e9,
+                                    "frac": dbytes * n / (alone["digitize_ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"]} if alone else None),
                          "note": f"{dbytes} algorithmic B/pair (DESIGN.md 6) x {n} pairs / {digi_ms:.3f} ms; peak = hbm_gbs of {peaks['source']}"}
 
     cpu = None
@@ -262,12 +348,14 @@ def run_ours(args):
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": desc, "pairs_per_step_per_gpu": n, "seed": run.seed, "parallelism": f"{world} x independent history ranges",
+                   "pipeline": (f"two batches in flight: gpet_simulate(k+1) on one stream beside gpet_digitize(k) on another, transport CTA of {warps} warps"
+                                if args.overlap else "serial: simulate then digitize on one stream"),
                    "l2": f"inputs larger than L2: the hit buffer ({n_hits * 28 / 1e6:.0f} MB/step) and digitizer scratch exceed the 126 MB L2",
                    "hits_per_step": n_hits, "coincidences_per_step": n_coinc},
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": args.e2e_steps,
                 "api": "gpet_run_host (host outputs: coincidence list-mode + counters)"},
-        "roofline": roofline, "roofline_digitizer": roofline_digi, "cpu_baseline": cpu,
+        "roofline": roofline, "roofline_digitizer": roofline_digi, "pipelined": pipelined, "cpu_baseline": cpu,
     }))
     if world > 1:
         dist.destroy_process_group()
@@ -286,6 +374,9 @@ def main():
     ap.add_argument("--cpu-pairs", type=int, default=10_000_000)
     ap.add_argument("--ref-pairs", type=int, default=2_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-pipelined", action="store_true", help="skip the extra two-stream pipeline measurement")
+    ap.add_argument("--overlap", action="store_true", help="time the two-stream pipeline as the headline instead of the serial steps")
+    ap.add_argument("--transport-warps", type=int, default=0, help="warps per transport CTA (default: 16 with overlap, 24 without)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

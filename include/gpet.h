@@ -201,6 +201,12 @@ int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, const gpet_so
                   uint64_t n_pairs_total, uint64_t first_history, uint64_t n_pairs, uint64_t seed,
                   const gpet_digitizer *dig, double hits_per_pair, gpet_host_outputs *out);
 
+/* Tuning: warps per transport CTA (one persistent CTA per SM), 1..24, default 24; returns the value in force.  Fewer
+ * warps leave registers and thread slots on every SM for kernels of OTHER streams: with 16, gpet_digitize of batch k on
+ * one stream runs beside gpet_simulate of batch k+1 on another (the transport kernel is bound by instruction issue, the
+ * digitizer by HBM latency), which is how bench.py pipelines its steps.  Applies to later gpet_simulate calls. */
+int gpet_set_transport_warps(int32_t warps);
+
 /* Thread-local text of the last error on this thread; valid until the next call on this thread. */
 const char *gpet_last_error(void);
 /* Number of kernel launches this library has enqueued since load (for bench.py's gpu_launches). */

@@ -70,7 +70,7 @@ class _HostOutputs(C.Structure):
 EXPORTS = ("gpet_geometry_create", "gpet_geometry_destroy", "gpet_geometry_panel_pose", "gpet_geometry_open_faces", "gpet_geometry_locate",
            "gpet_materials_load", "gpet_materials_destroy", "gpet_activity_create", "gpet_activity_destroy",
            "gpet_simulate", "gpet_digitize_scratch_bytes", "gpet_digitize", "gpet_run_host", "gpet_last_error",
-           "gpet_launch_count")
+           "gpet_launch_count", "gpet_set_transport_warps")
 
 _lib = None
 
@@ -102,6 +102,7 @@ def lib():
                                     C.POINTER(_HostOutputs)]
         L.gpet_last_error.restype = C.c_char_p
         L.gpet_launch_count.restype = u64
+        L.gpet_set_transport_warps.argtypes = [i32]
         _lib = L
     return _lib
 
@@ -113,6 +114,11 @@ def _check(rc: int):
 
 def gpet_launch_count() -> int:
     return int(lib().gpet_launch_count())
+
+
+def gpet_set_transport_warps(warps: int) -> int:
+    """Warps per transport CTA (1..24, 0 = default 24); returns the value in force."""
+    return int(lib().gpet_set_transport_warps(int(warps)))
 
 
 # ----------------------------------------------------------------------------- handles

@@ -44,6 +44,7 @@ static int fail(int code, const char *fmt, ...) {
 
 extern "C" const char *gpet_last_error(void) { return g_err; }
 extern "C" uint64_t gpet_launch_count(void) { return g_launches.load(); }
+extern "C" int gpet_set_transport_warps(int32_t warps) { set_transport_warps(warps); return transport_warps(); }
 
 static int sm_count() {
   static int n = 0;

@@ -31,6 +31,8 @@ struct CoincBuf { uint32_t *ids_a, *ids_b, *history_a, *history_b; float *e_a, *
 
 void count_launch(uint64_t n = 1);
 
+void set_transport_warps(int warps);
+int transport_warps();
 size_t transport_smem_bytes(const DevTables &T, int n_panels, bool hash);
 cudaError_t launch_transport(const DevGeom *geom, int n_panels, int planar_hint, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,

@@ -55,10 +55,10 @@ template <bool HASH> struct WarpMem {
   HitStage stage;
 };
 
-// dynamic shared memory: [WarpMem x kWarps][mu: n_staged x n_energies float4][DevGeom, first n_panels records]
+// dynamic shared memory: [WarpMem x warps of the CTA][mu: n_staged x n_energies float4][DevGeom, first n_panels records]
 template <bool HASH> struct SmemLayout {
-  static constexpr size_t mu_off = sizeof(WarpMem<HASH>) * kWarps;
-  __host__ __device__ static size_t geom_off(int n_mu) { return mu_off + sizeof(float4) * (size_t)n_mu; }
+  __host__ __device__ static size_t mu_off(int warps) { return sizeof(WarpMem<HASH>) * (size_t)warps; }
+  __host__ __device__ static size_t geom_off(int warps, int n_mu) { return mu_off(warps) + sizeof(float4) * (size_t)n_mu; }
 };
 
 // ---------------------------------------------------------------- fast math with bounded error
@@ -240,16 +240,16 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
                            const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n_mu = T.n_staged * T.n_energies;
-  float4 *mu_s = reinterpret_cast<float4 *>(smem_raw + SmemLayout<HASH>::mu_off);
-  DevGeom *g_s = reinterpret_cast<DevGeom *>(smem_raw + SmemLayout<HASH>::geom_off(n_mu));
+  float4 *mu_s = reinterpret_cast<float4 *>(smem_raw + SmemLayout<HASH>::mu_off(blockDim.x >> 5));
+  DevGeom *g_s = reinterpret_cast<DevGeom *>(smem_raw + SmemLayout<HASH>::geom_off(blockDim.x >> 5, n_mu));
   const int lane = threadIdx.x & 31;
   WarpMem<HASH> &W = reinterpret_cast<WarpMem<HASH> *>(smem_raw)[threadIdx.x >> 5];
   {
     const uint32_t *gs = reinterpret_cast<const uint32_t *>(geom);
     uint32_t *gd = reinterpret_cast<uint32_t *>(g_s);
     const int words = (int)(geom_bytes(geom->n_panels) / 4);
-    for (int i = threadIdx.x; i < words; i += kThreads) gd[i] = gs[i];
-    for (int i = threadIdx.x; i < n_mu; i += kThreads) mu_s[i] = T.mu[i];
+    for (int i = threadIdx.x; i < words; i += blockDim.x) gd[i] = gs[i];
+    for (int i = threadIdx.x; i < n_mu; i += blockDim.x) mu_s[i] = T.mu[i];
     for (int i = lane; i < kSlotsOf<HASH>; i += 32) W.list[L_FREE][i] = (uint8_t)i;
     __syncthreads();
   }
@@ -582,16 +582,21 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
   }
 }
 
+static int g_transport_warps = kWarps;             // warps per CTA (one CTA per SM); fewer leave room for other streams' kernels
+void set_transport_warps(int warps) { g_transport_warps = warps < 1 ? kWarps : (warps > kWarps ? kWarps : warps); }
+int transport_warps() { return g_transport_warps; }
+
 size_t transport_smem_bytes(const DevTables &T, int n_panels, bool hash) {
-  const int n_mu = T.n_staged * T.n_energies;
-  return (hash ? SmemLayout<true>::geom_off(n_mu) : SmemLayout<false>::geom_off(n_mu)) + geom_bytes(n_panels);
+  const int n_mu = T.n_staged * T.n_energies, w = g_transport_warps;
+  return (hash ? SmemLayout<true>::geom_off(w, n_mu) : SmemLayout<false>::geom_off(w, n_mu)) + geom_bytes(n_panels);
 }
 
 cudaError_t launch_transport(const DevGeom *geom, int n_panels, int planar_hint, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
                              unsigned long long *work_counter, int sm_count, cudaStream_t stream) {
   const size_t smem = transport_smem_bytes(T, n_panels, hash_out != nullptr);
-  const uint64_t want = (2 * n_pairs + kThreads - 1) / kThreads;
+  const int threads = 32 * g_transport_warps;
+  const uint64_t want = (2 * n_pairs + threads - 1) / threads;
   static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : GPET_MIN_CTAS;
   const uint64_t resident = (uint64_t)sm_count * ctas_per_sm;         // persistent grid
   PhiloxKeys key;                                                     // [R1] round keys: key + r * Weyl constants
@@ -603,7 +608,7 @@ cudaError_t launch_transport(const DevGeom *geom, int n_panels, int planar_hint,
   auto launch = [&](auto kernel) -> cudaError_t {
     cudaError_t le = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (le != cudaSuccess) return le;
-    kernel<<<blocks, kThreads, smem, stream>>>(geom, T, src, first_history, n_pairs, key, H, hash_out, work_counter);
+    kernel<<<blocks, threads, smem, stream>>>(geom, T, src, first_history, n_pairs, key, H, hash_out, work_counter);
     return cudaSuccess;
   };
   // specialised builds for the shapes the five configs use (point source or voxel map + phantom, planar ring);

@@ -399,3 +399,48 @@ def test_sensitivity_profiles_against_the_oracle(tables):
     d = S.delta_sym_percent(got["1CL"], got["2CL"])
     assert np.all(d > 0.0) and np.all(d < 20.0), d
     assert np.allclose(S.delta_sym_percent(got["2CL"], got["1CL"]), -d)
+
+
+def test_two_stream_pipeline_gives_the_same_results(tables):
+    """gpet_simulate of batch k+1 on one stream beside gpet_digitize of batch k on another (transport CTA of 16 warps, the
+    way bench.py's pipeline runs) must give, per batch, exactly the hits-derived coincidences of the serial run."""
+    r = W.config_runs("C3", 1_000_000)[3]
+    n = r.n_pairs
+    geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+    cap = 2 * n
+    def alloc():
+        return (api.HitBuffer.allocate(cap), api.CoincBuffer.allocate(cap // 4),
+                torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda"))
+    ref = []
+    hb, co, sc = alloc()
+    for k in range(4):                                                # serial reference, default CTA
+        hb.n_hits.zero_()
+        api.gpet_simulate(geom, m, s, k * n, n, r.seed, hb)
+        api.gpet_digitize(s, r.seed, 4 * n, k * n, n, hb, cap, r.digitizer, sc, None, co)
+        torch.cuda.synchronize()
+        ref.append(co.to_numpy())
+    try:
+        assert api.gpet_set_transport_warps(16) == 16
+        bufs = [alloc(), alloc()]
+        sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+        sim_done = [torch.cuda.Event() for _ in range(2)]; dig_done = [torch.cuda.Event() for _ in range(2)]
+        got = []
+        for k in range(4):
+            i = k & 1
+            hbi, coi, sci = bufs[i]
+            if k >= 2:
+                sb.synchronize(); got.append(coi.to_numpy())          # batch k-2 is complete: read it before its buffers are reused
+                sa.wait_event(dig_done[i])
+            with torch.cuda.stream(sa):
+                hbi.n_hits.zero_()
+                api.gpet_simulate(geom, m, s, k * n, n, r.seed, hbi, sa)
+            sim_done[i].record(sa)
+            sb.wait_event(sim_done[i])
+            api.gpet_digitize(s, r.seed, 4 * n, k * n, n, hbi, cap, r.digitizer, sci, None, coi, sb)
+            dig_done[i].record(sb)
+        torch.cuda.synchronize()
+        got += [bufs[0][1].to_numpy(), bufs[1][1].to_numpy()]
+    finally:
+        assert api.gpet_set_transport_warps(0) == 24
+    for a, b in zip(ref, got):
+        assert len(a["ids_a"]) > 40_000 and all(np.array_equal(a[k], b[k]) for k in a)

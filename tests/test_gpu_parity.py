@@ -478,3 +478,22 @@ def test_generic_panel_search_parity(tables, pos):
     torch.cuda.synchronize()
     plain = PU.canonical(hb.to_numpy())
     assert all(np.array_equal(plain[k], g[k]) for k in PU.HIT_KEYS)
+
+
+def test_mixed_materials_virtual_collisions_and_voxel_source_without_phantom(tables):
+    """Paths the five configs never reach: a front layer of a lighter material under the whole-panel majorant [R19]
+    (virtual collisions in crystals), a reflector made of matter (interactions that deposit outside any crystal record
+    no hit [R20]), and an activity-map source with no phantom (generic kernel variant)."""
+    front = W.Layer((15, 15), (1.0, 1.0), (0.1, 0.1), (0.5, 0.5), 6.0, 0.0, crystal_material=1, gap_material=1)
+    back = W.Layer((16, 16), (1.0, 1.0), (0.1, 0.1), (0.0, 0.0), 4.0, 0.1, crystal_material=0, gap_material=1)
+    geom = W.Geometry(12, (front, back), (2, 4), (16.0, 16.0), (16.0, 16.0), ring_inner_radius_mm=55.0)
+    rods = W.source_hot_rods()
+    src = W.Source(1, (0, 0, 0), 0.5, 1e6, 0, rods.activity, None, -1, rods.dims, rods.voxel_mm, rods.origin_mm)
+    r = W.Run("mixed", geom, src, 300_001, 77)
+    g, gh, cnt, o = run_both(r, tables)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= MIN_MATCH and cnt > 100_000, res
+    c = o.counters
+    assert c["virtuals"] > 50_000 and c["ph_steps"] == 0              # the majorant really is above the front layer's mu
+    layers = (g["ids"] >> 18) & 3
+    assert (layers == 0).sum() > 1000 and (layers == 1).sum() > 50_000

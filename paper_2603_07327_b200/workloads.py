@@ -176,10 +176,27 @@ def geometry_c3() -> Geometry:
                   _lyso_layer(16, 1.0, 0.1, 4.0, gap_before=0.1)])
 
 
+def _paper_ring(layers: Sequence[Layer]) -> Geometry:
+    """The paper's own scanner: 10 panels at R = 85 mm, six axial modules of 51 mm with 7 mm gaps
+    (panel 10 x 51 x 341 mm), 1.0 mm pitch = 0.92 mm crystal + 0.08 mm air.  Context only."""
+    return Geometry(10, tuple(layers), (1, 6), (51.0, 51.0), (51.0, 58.0), ring_inner_radius_mm=85.0)
+
+
 def geometry_paper_1cl() -> Geometry:
-    """The paper's own H2RSPET-1CL: context only."""
-    return Geometry(10, (Layer((51, 51), (1.0, 1.0), (0.08, 0.08), (0.0, 0.0), 10.0),),
-                    (1, 6), (51.0, 51.0), (51.0, 58.0), ring_inner_radius_mm=85.0)
+    """H2RSPET-1CL: one layer of 51 x 51 crystals, 10 mm deep."""
+    return _paper_ring([Layer((51, 51), (1.0, 1.0), (0.08, 0.08), (0.0, 0.0), 10.0)])
+
+
+def geometry_paper_split() -> Geometry:
+    """H2RSPET-1CL-split: two radially connected 5 mm crystals (no gap)."""
+    return _paper_ring([Layer((51, 51), (1.0, 1.0), (0.08, 0.08), (0.0, 0.0), 5.0),
+                        Layer((51, 51), (1.0, 1.0), (0.08, 0.08), (0.0, 0.0), 5.0)])
+
+
+def geometry_paper_2cl() -> Geometry:
+    """H2RSPET-2CL: inner 50 x 50 layer shifted by half a pitch over an outer 51 x 51 layer, 5 mm each."""
+    return _paper_ring([Layer((50, 50), (1.0, 1.0), (0.08, 0.08), (0.5, 0.5), 5.0),
+                        Layer((51, 51), (1.0, 1.0), (0.08, 0.08), (0.0, 0.0), 5.0)])
 
 
 # ----------------------------------------------------------------------------- hot-rod phantom (C4)
@@ -265,6 +282,10 @@ def config_runs(name: str, n_pairs: Optional[int] = None) -> List[Run]:
     if name == "C4":
         n = n_pairs or 1_000_000_000
         return [Run("C4", geometry_c3(), source_hot_rods(pairs_per_time_slice=max(1, n // 16)), n, 5)]
+    if name in ("P1", "P2", "P3"):      # the paper's own scanners with a centred point source (context)
+        geom = {"P1": geometry_paper_1cl, "P2": geometry_paper_split, "P3": geometry_paper_2cl}[name]()
+        dig = Digitizer(0.16, 511.0, 350.0, 700.0, 3.0, 1)
+        return [Run(name, geom, source_point(), n_pairs or 10_000_000, 60 + int(name[1]), dig)]
     raise ValueError(f"unknown config {name!r}")
 
 

@@ -130,6 +130,7 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
       const float *q = G.panel[p].pose; float c[3];
       for (int k = 0; k < 3; ++k) c[k] = (float)((double)q[k] + ma * q[3 + k] + mb * q[6 + k] + mc * q[9 + k]);
       G.panel[p].cx = c[0]; G.panel[p].cy = c[1]; G.panel[p].cz = c[2];
+      G.ctr[p][0] = c[0]; G.ctr[p][1] = c[1]; G.ctr[p][2] = c[2];
     }
   }
   // open faces: face (axis k, side) of panel p is open when every corner of every other panel box lies at least 1 um on
@@ -340,7 +341,7 @@ extern "C" int gpet_simulate(const gpet_geometry *g, const gpet_materials *m, co
   const uint32_t stage_mask = (D.kind == 1 && D.phantom) ? (1u << m->n_materials) - 1u : 0u;
   DevTables T; rc = staged_table(const_cast<gpet_materials *>(m), g->host.det_mask, stage_mask, &T); if (rc) return rc;
   unsigned long long *wc = nullptr; rc = next_work_counter(&wc); if (rc) return rc;
-  CUDA_TRY(launch_transport(g->dev, g->host.n_panels, g->host.planar, T, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
+  CUDA_TRY(launch_transport(g->host, g->dev, T, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
   return GPET_OK;
 }
 

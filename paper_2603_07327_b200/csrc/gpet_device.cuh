@@ -28,7 +28,11 @@ struct __align__(16) DevPanel {
   uint32_t open_faces;        // bit 2k + (outward along +axis k): no other panel has a point beyond that face of this box
   float skew[4];              // 80-byte stride: records of 8 consecutive panels start in 8 different 16-byte bank groups, so
 };                            // lanes reading the poses of different panels (entry / exit / hit transforms) rarely conflict
-struct DevGeom {
+// Header of the descriptor: everything the kernels read with the SAME address in every lane (extents, lattice
+// parameters, box centres for the search cull).  The transport kernel receives it as a __grid_constant__ parameter, so
+// these reads are constant-bank operands and do not load the shared-memory pipe; the per-panel records, read with a
+// per-lane panel index, are staged into shared memory.
+struct DevGeomHead {
   int n_panels, n_layers;
   int Wq, Hq, Dq, hWq, hHq;
   int nmod[2], msq[2], mpq[2];
@@ -39,8 +43,12 @@ struct DevGeom {
   int planar;                 // 1 = every panel has v = +z and u_z = w_z = o_z = 0: the search shares the axial slab
   float cull_r2, cull_r3;     // radius (+ margin) of the circle / sphere about a panel box: (a,c) plane / 3-D
   DevLayer layer[kMaxLayers];
+  float ctr[kMaxPanels][3];   // global position of every box centre (same values as DevPanel::cx, cy, cz)
+};
+struct DevGeom : DevGeomHead {
   DevPanel panel[kMaxPanels]; // LAST member: kernels stage only the first n_panels records into shared memory
 };
+inline size_t panel_bytes(int n_panels) { return sizeof(DevPanel) * (size_t)n_panels; }
 __host__ __device__ inline size_t geom_bytes(int n_panels) { return sizeof(DevGeom) - sizeof(DevPanel) * (size_t)(kMaxPanels - n_panels); }
 
 struct DevTables {            // [R11] per staged material, per energy: {mu_pe, mu_pe+mu_C, mu_tot, detector majorant}
@@ -89,7 +97,7 @@ __device__ __forceinline__ int floor_div_q(int rel, int pitch, float inv_pitch, 
 // (qa, qb, qc) measured from the panel's low corner.  Returns the material (-1 vacuum) and the packed
 // ids without panel/photon/seq bits (kNone when the point is in no crystal).  PAPER.md:43: the depth
 // coordinate picks the layer, that layer's crystal parameters give material and index.
-__device__ __forceinline__ int lattice_lookup(const DevGeom &g, int qa, int qb, int qc, uint32_t &ids) {
+__device__ __forceinline__ int lattice_lookup(const DevGeomHead &g, int qa, int qb, int qc, uint32_t &ids) {
   ids = kNone;
   if ((unsigned)qa >= (unsigned)g.Wq || (unsigned)qb >= (unsigned)g.Hq || (unsigned)qc >= (unsigned)g.Dq) return -1;
   int ra, rb;

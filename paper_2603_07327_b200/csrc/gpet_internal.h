@@ -34,7 +34,7 @@ void count_launch(uint64_t n = 1);
 void set_transport_warps(int warps);
 int transport_warps();
 size_t transport_smem_bytes(const DevTables &T, int n_panels, bool hash);
-cudaError_t launch_transport(const DevGeom *geom, int n_panels, int planar_hint, const DevTables &T, const DevSource &src,
+cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
                              unsigned long long *work_counter, int sm_count, cudaStream_t stream);
 cudaError_t launch_locate(const DevGeom *geom, int64_t n, const float *xyz_dev, uint32_t *ids_dev, cudaStream_t stream);

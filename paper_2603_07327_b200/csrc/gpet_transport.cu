@@ -55,7 +55,7 @@ template <bool HASH> struct WarpMem {
   HitStage stage;
 };
 
-// dynamic shared memory: [WarpMem x warps of the CTA][mu: n_staged x n_energies float4][DevGeom, first n_panels records]
+// dynamic shared memory: [WarpMem x warps of the CTA][mu: n_staged x n_energies float4][DevPanel x n_panels]
 template <bool HASH> struct SmemLayout {
   __host__ __device__ static size_t mu_off(int warps) { return sizeof(WarpMem<HASH>) * (size_t)warps; }
   __host__ __device__ static size_t geom_off(int warps, int n_mu) { return mu_off(warps) + sizeof(float4) * (size_t)n_mu; }
@@ -165,7 +165,7 @@ __device__ __forceinline__ void decay_site(const DevSource &src, uint4 w, float 
 // PAPER.md:33) share the axial slab and need only the 2-D part of each pose; the arithmetic on the
 // surviving terms is the generic one (the dropped terms are exact zeros).
 template <int PLANAR>
-__device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], const float d[3], int excl, float &t_enter) {
+__device__ __forceinline__ int panel_search(const DevGeomHead &g, const DevPanel *pan, const float x[3], const float d[3], int excl, float &t_enter) {
   float bt = INFINITY; int bp = -1;
   if (PLANAR < 0 ? g.planar != 0 : PLANAR != 0) {
     const float iz = rcp_dir(d[2]);
@@ -181,15 +181,15 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
       uint32_t cand = 0, bit = 1u;
 #pragma unroll 4
       for (int q = 0; q < nq; ++q, bit <<= 1) {
-        const DevPanel &c = g.panel[base + q];
-        const float cross = fmaf(c.cx, d[1], fmaf(-c.cy, d[0], -Lz)), dot = fmaf(c.cx, d[0], fmaf(c.cy, d[1], -Mz));
+        const float cx = g.ctr[base + q][0], cy = g.ctr[base + q][1];
+        const float cross = fmaf(cx, d[1], fmaf(-cy, d[0], -Lz)), dot = fmaf(cx, d[0], fmaf(cy, d[1], -Mz));
         if (fmaxf(fabsf(cross), -dot) <= sr) cand |= bit;                  // |cross| <= sr and dot >= -sr
       }
       if ((unsigned)(excl - base) < 32u) cand &= ~(1u << (excl - base));
       if (!axial_ok) cand = 0;
       while (cand) {
         const int q = base + __ffs(cand) - 1; cand &= cand - 1;
-        const float *P = g.panel[q].pose;
+        const float *P = pan[q].pose;
         const float r0 = x[0] - P[0], r1 = x[1] - P[1];
         const float a = r0 * P[3] + r1 * P[4], c = r0 * P[9] + r1 * P[10];
         const float ia = rcp_dir(d[0] * P[3] + d[1] * P[4]), ic = rcp_dir(d[0] * P[9] + d[1] * P[10]);
@@ -205,8 +205,7 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
       uint32_t cand = 0;
 #pragma unroll 2
       for (int q = 0; q < nq; ++q) {
-        const DevPanel &c = g.panel[base + q];
-        const float rx = c.cx - x[0], ry = c.cy - x[1], rz = c.cz - x[2];
+        const float rx = g.ctr[base + q][0] - x[0], ry = g.ctr[base + q][1] - x[1], rz = g.ctr[base + q][2] - x[2];
         const float b = fmaf(rx, d[0], fmaf(ry, d[1], rz * d[2]));                  // |d| = 1
         const float r2 = fmaf(rx, rx, fmaf(ry, ry, rz * rz));
         if (r2 - b * b <= g.cull_r3 * g.cull_r3 * 1.0001f && b >= -g.cull_r3) cand |= 1u << q;
@@ -215,7 +214,7 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
       while (cand) {
         const int q = base + __ffs(cand) - 1; cand &= cand - 1;
         float xl[3], dl[3];
-        to_local(g.panel[q].pose, x, d, xl, dl);
+        to_local(pan[q].pose, x, d, xl, dl);
         float tn = 0.0f, tf = INFINITY;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
@@ -236,24 +235,23 @@ __device__ __forceinline__ int panel_search(const DevGeom &g, const float x[3], 
 // [R17]; KIND: source kind (0 point, 1 voxel map, -1 = read src.kind); PLANAR: panel search variant (-1 = read g.planar).
 template <bool HASH, bool PHANTOM, int KIND, int PLANAR>
 __global__ void __launch_bounds__(kThreads, GPET_MIN_CTAS)
-transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint64_t first_history, uint64_t n_pairs,
+transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel *panels, DevTables T, DevSource src, uint64_t first_history, uint64_t n_pairs,
                            const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n_mu = T.n_staged * T.n_energies;
   float4 *mu_s = reinterpret_cast<float4 *>(smem_raw + SmemLayout<HASH>::mu_off(blockDim.x >> 5));
-  DevGeom *g_s = reinterpret_cast<DevGeom *>(smem_raw + SmemLayout<HASH>::geom_off(blockDim.x >> 5, n_mu));
+  DevPanel *pan = reinterpret_cast<DevPanel *>(smem_raw + SmemLayout<HASH>::geom_off(blockDim.x >> 5, n_mu));
   const int lane = threadIdx.x & 31;
   WarpMem<HASH> &W = reinterpret_cast<WarpMem<HASH> *>(smem_raw)[threadIdx.x >> 5];
   {
-    const uint32_t *gs = reinterpret_cast<const uint32_t *>(geom);
-    uint32_t *gd = reinterpret_cast<uint32_t *>(g_s);
-    const int words = (int)(geom_bytes(geom->n_panels) / 4);
+    const uint32_t *gs = reinterpret_cast<const uint32_t *>(panels);
+    uint32_t *gd = reinterpret_cast<uint32_t *>(pan);
+    const int words = (int)(sizeof(DevPanel) / 4) * g.n_panels;
     for (int i = threadIdx.x; i < words; i += blockDim.x) gd[i] = gs[i];
     for (int i = threadIdx.x; i < n_mu; i += blockDim.x) mu_s[i] = T.mu[i];
     for (int i = lane; i < kSlotsOf<HASH>; i += 32) W.list[L_FREE][i] = (uint8_t)i;
     __syncthreads();
   }
-  const DevGeom &g = *g_s;
   const float4 *mu = mu_s;
   HitStage &stage = W.stage;
   const unsigned lt_mask = (1u << lane) - 1u;
@@ -370,14 +368,14 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
       cS -= n;
       int dest = L_NONE;
       if (act) {
-        float bt; const int bp = panel_search<PLANAR>(g, q.x, q.d, ph_panel(q), bt);
+        float bt; const int bp = panel_search<PLANAR>(g, pan, q.x, q.d, ph_panel(q), bt);
         if (bp < 0) {
           if (HASH) { hash_ev(hq, EV_ESCAPE, 0); hash_out[2ull * q.pair + (q.meta & 1u)] = hq; }
           dest = L_FREE;
         } else {
           if (HASH) hash_ev(hq, EV_ENTER, (uint32_t)bp);
           float xl[3], dl[3];
-          to_local(g.panel[bp].pose, q.x, q.d, xl, dl);
+          to_local(pan[bp].pose, q.x, q.d, xl, dl);
 #pragma unroll
           for (int k = 0; k < 3; ++k) { q.x[k] = fmaf(bt, dl[k], xl[k]); q.d[k] = dl[k]; }   // [R18]
           q.path += bt; ph_set_panel(q, bp);
@@ -414,7 +412,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
           // anything: the photon escapes here, with the same EXIT, ESCAPE events, and skips transform and search.
           const int kx = te[0] <= tf ? 0 : (te[1] <= tf ? 1 : 2);
           const float dk = kx == 0 ? p.d[0] : (kx == 1 ? p.d[1] : p.d[2]);
-          const bool open = (g.panel[panel].open_faces >> (2 * kx + (dk >= 0.0f ? 1 : 0))) & 1u;
+          const bool open = (pan[panel].open_faces >> (2 * kx + (dk >= 0.0f ? 1 : 0))) & 1u;
           if (HASH) hash_ev(h, EV_EXIT, (uint32_t)panel);
           if (open) {
             if (HASH) { hash_ev(h, EV_ESCAPE, 0); hash_out[2ull * p.pair + (p.meta & 1u)] = h; }
@@ -424,7 +422,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
             const float xl[3] = { fmaf(tf, p.d[0], p.x[0]), fmaf(tf, p.d[1], p.x[1]), fmaf(tf, p.d[2], p.x[2]) };
             const float dl[3] = { p.d[0], p.d[1], p.d[2] };
             p.path += tf;
-            point_to_global(g.panel[panel].pose, xl, p.x); dir_to_global(g.panel[panel].pose, dl, p.d);   // back to the global frame
+            point_to_global(pan[panel].pose, xl, p.x); dir_to_global(pan[panel].pose, dl, p.d);   // back to the global frame
             dest = L_SEARCH;
           }
         } else {
@@ -443,7 +441,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
             p.ids = id;
             if (t < m4.x) {                                           // photoelectric: deposit E, end
               if (HASH) { hash_ev(h, EV_PE, id); hash_out[2ull * p.pair + (p.meta & 1u)] = h; }
-              if (id != kNone) { hit = true; point_to_global(g.panel[panel].pose, p.x, xg); }
+              if (id != kNone) { hit = true; point_to_global(pan[panel].pose, p.x, xg); }
               dest = L_FREE;
             } else if (t < m4.y) dest = L_KN;
             else if (t < m4.z) { dest = L_RAY; if (HASH) hash_ev(h, EV_RAYLEIGH, id); }   // deflected in its own pass
@@ -500,7 +498,7 @@ transport_wavefront_kernel(const DevGeom *geom, DevTables T, DevSource src, uint
           } else {
             if (HASH) { hash_ev(h, EV_COMPTON, p.ids); if (cut) hash_ev(h, EV_CUTOFF, p.ids); }
             if (p.ids != kNone) {
-              hit = true; e_dep = cut ? p.E : dep; point_to_global(g.panel[ph_panel(p)].pose, p.x, xg);
+              hit = true; e_dep = cut ? p.E : dep; point_to_global(pan[ph_panel(p)].pose, p.x, xg);
               const uint32_t seq = (p.meta >> 1) & 15u;
               hit_ids = p.ids | ((p.meta & 1u) << 4) | seq;
               if (seq < 15u) p.meta += 2u;                            // [R9] 4-bit saturating hit counter
@@ -588,12 +586,16 @@ int transport_warps() { return g_transport_warps; }
 
 size_t transport_smem_bytes(const DevTables &T, int n_panels, bool hash) {
   const int n_mu = T.n_staged * T.n_energies, w = g_transport_warps;
-  return (hash ? SmemLayout<true>::geom_off(w, n_mu) : SmemLayout<false>::geom_off(w, n_mu)) + geom_bytes(n_panels);
+  return (hash ? SmemLayout<true>::geom_off(w, n_mu) : SmemLayout<false>::geom_off(w, n_mu)) + panel_bytes(n_panels);
 }
 
-cudaError_t launch_transport(const DevGeom *geom, int n_panels, int planar_hint, const DevTables &T, const DevSource &src,
+cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
                              unsigned long long *work_counter, int sm_count, cudaStream_t stream) {
+  const int n_panels = host_geom.n_panels, planar_hint = host_geom.planar;
+  const DevGeomHead &head = host_geom;
+  const DevPanel *panels = reinterpret_cast<const DevPanel *>(reinterpret_cast<const char *>(geom) +
+                                                            (reinterpret_cast<const char *>(&host_geom.panel[0]) - reinterpret_cast<const char *>(&host_geom)));
   const size_t smem = transport_smem_bytes(T, n_panels, hash_out != nullptr);
   const int threads = 32 * g_transport_warps;
   const uint64_t want = (2 * n_pairs + threads - 1) / threads;
@@ -608,7 +610,7 @@ cudaError_t launch_transport(const DevGeom *geom, int n_panels, int planar_hint,
   auto launch = [&](auto kernel) -> cudaError_t {
     cudaError_t le = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (le != cudaSuccess) return le;
-    kernel<<<blocks, threads, smem, stream>>>(geom, T, src, first_history, n_pairs, key, H, hash_out, work_counter);
+    kernel<<<blocks, threads, smem, stream>>>(head, panels, T, src, first_history, n_pairs, key, H, hash_out, work_counter);
     return cudaSuccess;
   };
   // specialised builds for the shapes the five configs use (point source or voxel map + phantom, planar ring);

@@ -175,7 +175,7 @@ size_t gpet_digitize_scratch_bytes(uint64_t n_pairs, uint64_t n_hits);
 
 /* hits (any order) -> adder per (history, readout unit) -> blur -> window -> absolute time -> time sort
  * -> coincidence windows.  The hits must belong to histories [first_history, first_history + n_pairs)
- * (one gpet_simulate batch, or several appended ones).  n_hits < 2^32 is a HOST-side upper bound on the
+ * (one gpet_simulate batch, or several appended ones).  n_hits <= 2^31 is a HOST-side upper bound on the
  * valid entries (it sizes the scratch; pass hits->capacity to avoid reading the counter back): the kernels
  * use min(*hits->n_hits, hits->capacity, n_hits), read on the device.  n_pairs_total (pairs of the whole run, all batches) and
  * src give the decay times [R16].  Output is deterministic: it does not depend on the order of `hits`.

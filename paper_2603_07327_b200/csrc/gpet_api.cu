@@ -363,7 +363,7 @@ extern "C" int gpet_digitize(const gpet_source *src, uint64_t seed, uint64_t n_p
                              const gpet_hits *hits, uint64_t n_hits, const gpet_digitizer *dig, void *scratch, size_t scratch_bytes,
                              gpet_singles *so, gpet_coincidences *co, void *stream) {
   if (!src || !hits || !dig || !co || !co->n_coinc) return fail(GPET_E_INVALID_ARG, "gpet_digitize: NULL argument");
-  if (n_pairs == 0 || n_pairs >= (1ull << 32) || n_hits > hits->capacity || n_hits >= (1ull << 32)) return fail(GPET_E_INVALID_ARG, "gpet_digitize: counts out of range");
+  if (n_pairs == 0 || n_pairs >= (1ull << 32) || n_hits > hits->capacity || n_hits > (1ull << 31)) return fail(GPET_E_INVALID_ARG, "gpet_digitize: counts out of range");
   if (scratch_bytes < digitize_scratch_bytes(n_pairs, n_hits) || !scratch) return fail(GPET_E_OVERFLOW, "scratch too small: %zu < %zu", scratch_bytes, digitize_scratch_bytes(n_pairs, n_hits));
   DigiParams P; int rc = make_digi(src, seed, n_pairs_total, dig, &P); if (rc) return rc;
   SinglesBuf S; memset(&S, 0, sizeof S);

@@ -172,7 +172,9 @@ __device__ __forceinline__ double decay_time(const DigiParams &P, uint64_t histo
 }
 
 // records per block of the adder / bucket-scatter pair: the same split in both kernels, a multiple of the block size
-__device__ __forceinline__ uint32_t region_size(uint32_t n, uint32_t blocks) { return (((n + blocks - 1) / blocks) + 255u) & ~255u; }
+__device__ __forceinline__ uint32_t region_size(uint32_t n, uint32_t blocks) {
+  return (uint32_t)(((((unsigned long long)n + blocks - 1) / blocks) + 255ull) & ~255ull);
+}
 
 // One thread per hit record (a thread per history would idle on the ~54 % of histories without hits).  The record with
 // the smallest (ids, position) of its (history, readout unit) group is the group's leader: one pass over the history's

@@ -277,6 +277,43 @@ def test_c1_full_size_sampled_histories(tables):
     assert abs(up - down) < 5 * np.sqrt(up + down)                    # axial symmetry
 
 
+def test_c1_full_size_digitizer_sampled_histories(tables):
+    """The digitizer at configs[1]'s full size, scratch and buffers sized as bench.py sizes them: the singles of sampled
+    history blocks (they depend on no other history [R24]) equal the oracle's records, the singles are time-ordered, and
+    every coincidence is a window-mate pair of consecutive singles on different panels [R27]."""
+    r = W.config_runs("C1")[0]
+    n = r.n_pairs
+    geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+    cap = int(1.2 * n) + 1024
+    hb, sg, co = api.HitBuffer.allocate(cap), api.SinglesBuffer.allocate(cap), api.CoincBuffer.allocate(cap // 4)
+    scratch = torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda")
+    api.gpet_simulate(geom, m, s, 0, n, r.seed, hb)
+    api.gpet_digitize(s, r.seed, n, 0, n, hb, cap, r.digitizer, scratch, sg, co)
+    torch.cuda.synchronize()
+    gs, gc = sg.to_numpy(), co.to_numpy()
+    assert 0.32 < len(gs["ids"]) / n < 0.35 and 0.055 < len(gc["ids_a"]) / n < 0.060
+    assert np.all(np.diff(gs["t_s"]) >= 0)
+    rng = np.random.default_rng(11)
+    for st in np.concatenate([[0, n - 4096], rng.integers(0, n - 4096, 10)]):
+        o = O.simulate(r.geometry, tables, r.source, 4096, r.seed, first_history=int(st), threads=4)
+        osg, _, _ = O.digitize(r.source, r.seed, n, o.hits, r.digitizer)
+        sel = (gs["history"] >= st) & (gs["history"] < st + 4096)
+        assert abs(int(sel.sum()) - len(osg.ids)) <= 1               # one of the ~1e-5 mismatching histories, or a window-edge flip
+        if int(sel.sum()) == len(osg.ids):
+            assert np.array_equal(gs["history"][sel], osg.history) and np.array_equal(gs["ids"][sel] >> 5, osg.ids >> 5)
+            assert np.max(np.abs(gs["t_s"][sel] - osg.t_s)) < 1e-12 and np.max(np.abs(gs["e_keV"][sel] - osg.e_keV)) < E_TOL
+    # every coincidence: two consecutive singles within the window, on different panels, and no third single in the window
+    pos = np.searchsorted(gs["t_s"], gc["t_s"])
+    idx = np.arange(len(gs["t_s"]))
+    key = gs["history"].astype(np.uint64) << np.uint64(32) | gs["ids"].astype(np.uint64)
+    a = np.array([p if key[p] == (np.uint64(h) << np.uint64(32) | np.uint64(i)) else p + 1 for p, h, i in
+                  zip(pos[:2000], gc["history_a"][:2000], gc["ids_a"][:2000])])
+    assert np.array_equal(gs["ids"][a], gc["ids_a"][:2000]) and np.array_equal(gs["ids"][a + 1], gc["ids_b"][:2000])
+    tau = r.digitizer.window_ns * 1e-9
+    assert np.all(gs["t_s"][a + 1] - gs["t_s"][a] < tau) and np.all((gs["ids"][a] >> 26) != (gs["ids"][a + 1] >> 26))
+    assert np.all(gs["t_s"][a + 2] - gs["t_s"][a] >= tau)
+
+
 @pytest.mark.parametrize("cfg,idx,lo,hi", [("C2", 4, 1.38, 1.48), ("C3", 21, 1.19, 1.29)])
 def test_c2_c3_full_size_sampled_histories(tables, cfg, idx, lo, hi):
     """configs[2] (x = 50 mm) and configs[3] (x = 50 mm, z = 16 mm) at 1e7 pairs: the positions with the most hits."""

@@ -14,37 +14,33 @@
 // exactly once, and the kernel is specialised on phantom / source kind / search variant to stay small.  Geometry
 // descriptor and interleaved float4 mu tables live in shared memory; hits are staged per warp in shared memory and
 // flushed 32 at a time: one atomicAdd per 32 hits and seven fully coalesced 128-byte stores (SoA).
-#include <cstdlib>
 #include "gpet_internal.h"
 
 namespace gpet {
 
+// Launch shape and pool sizes (measured on B200, C1-C4; -D overrides are for experiments only).
 #ifndef GPET_THREADS
-#define GPET_THREADS 768
+#define GPET_THREADS 768              // one CTA of 24 warps per SM: the tables are staged once, each warp gets 8.7 KB
+#endif
+#ifndef GPET_SLOTS
+#define GPET_SLOTS 128                // photon slots per warp (20 x 160 and 28 x 104 run within 2 % of 24 x 128)
+#endif
+#ifndef GPET_MIN_GEN
+#define GPET_MIN_GEN 24               // the source refills only when at least this many pairs fit (2 free slots each)
 #endif
 constexpr int kThreads = GPET_THREADS;
 constexpr int kWarps = kThreads / 32;
 constexpr int kStage = 64;            // staged hits per warp (ring buffer)
-#ifndef GPET_SLOTS
-#define GPET_SLOTS 128
-#endif
-#ifndef GPET_MIN_CTAS
-#define GPET_MIN_CTAS 1
-#endif
-// photon slots per warp.  One CTA of 24 warps per SM stages the tables once and leaves 8.7 KB of shared memory to each
-// warp; the parity builds (HASH) also keep an 8-byte hash per slot and get by with 16 slots fewer.
+// the parity builds (HASH) also keep an 8-byte hash per slot and get by with 16 slots fewer
 template <bool HASH> constexpr int kSlotsOf = HASH ? GPET_SLOTS - 16 : GPET_SLOTS;
 constexpr uint32_t kChunk = 512;      // pairs a warp reserves at a time
-#ifndef GPET_MIN_GEN
-#define GPET_MIN_GEN 24
-#endif
-constexpr int kMinGen = GPET_MIN_GEN;  // the source refills only when at least this many pairs fit (2 free slots each)
+constexpr int kMinGen = GPET_MIN_GEN;
 
 enum : int { L_FREE = 0, L_SEARCH, L_STEP, L_KN, L_RAY, L_PHANTOM, kLists, L_NONE = kLists, L_GEN };
 
 struct HitStage { uint32_t w[7][kStage]; };      // history, ids, x, y, z, e, tof
 
-// One warp's private memory.  A photon record is 48 bytes in three 16-byte planes (conflict-free LDS.128).
+// One warp's private memory.  A photon record is 48 bytes in three 16-byte planes (one LDS.128 / STS.128 each).
 template <bool HASH> struct WarpMem {
   static constexpr int kSlots = kSlotsOf<HASH>;
   float4 a[kSlots];                    // x, y, z, dx
@@ -234,7 +230,7 @@ __device__ __forceinline__ int panel_search(const DevGeomHead &g, const DevPanel
 // the phantom code alone made the ring configs 10 % faster).  PHANTOM: the source is a voxel map with a phantom
 // [R17]; KIND: source kind (0 point, 1 voxel map, -1 = read src.kind); PLANAR: panel search variant (-1 = read g.planar).
 template <bool HASH, bool PHANTOM, int KIND, int PLANAR>
-__global__ void __launch_bounds__(kThreads, GPET_MIN_CTAS)
+__global__ void __launch_bounds__(kThreads, 1)
 transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel *panels, DevTables T, DevSource src, uint64_t first_history, uint64_t n_pairs,
                            const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -599,8 +595,7 @@ cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, cons
   const size_t smem = transport_smem_bytes(T, n_panels, hash_out != nullptr);
   const int threads = 32 * g_transport_warps;
   const uint64_t want = (2 * n_pairs + threads - 1) / threads;
-  static const int ctas_per_sm = getenv("GPET_CTAS_PER_SM") ? atoi(getenv("GPET_CTAS_PER_SM")) : GPET_MIN_CTAS;
-  const uint64_t resident = (uint64_t)sm_count * ctas_per_sm;         // persistent grid
+  const uint64_t resident = (uint64_t)sm_count;                      // persistent grid: one CTA per SM
   PhiloxKeys key;                                                     // [R1] round keys: key + r * Weyl constants
   for (int r = 0; r < 10; ++r) { key.k[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; key.k[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }
   const int blocks = (int)(want < resident ? (want ? want : 1) : resident);

@@ -32,6 +32,7 @@ extern "C" {
 #define GPET_MAX_LAYERS    4
 #define GPET_MAX_MATERIALS 8
 #define GPET_IDS_NONE 0xFFFFFFFFu /* packed ids of a point that is not inside a crystal */
+#define GPET_HIT_CHUNK_PAIRS 512   /* pairs per chunk of the chunked hit layout (gpet_hits.chunk_fill) */
 
 /* Packed ids [R9] (every interaction is labelled with crystal, layer, module, panel):
  *   bits 0-3 sequence (per-photon hit counter, saturating at 15), bit 4 photon (0 = A, 1 = B),
@@ -131,6 +132,16 @@ typedef struct {                  /* struct of arrays, DEVICE, caller-owned     
   uint64_t *n_hits;               /* DEVICE counter; NOT reset by the library, so several calls append  */
   uint64_t *outcome_hash;         /* DEVICE, optional (NULL = off): 2*n_pairs words, [2*i + photon] =   */
                                   /* FNV-1a over that photon's ordered event codes [R23] (parity tool)  */
+  uint32_t *chunk_fill;           /* DEVICE, optional (NULL = dense layout above).  CHUNKED layout: the  */
+                                  /* batch's pairs are taken in chunks of GPET_HIT_CHUNK_PAIRS; with     */
+                                  /* n_chunks = ceil(n_pairs / 512) and cap = capacity / n_chunks, the   */
+                                  /* hits of chunk c occupy entries [c*cap, c*cap + min(fill[c], cap))   */
+                                  /* of the seven arrays, in no particular order, and chunk_fill[c]      */
+                                  /* counts them (n_chunks + 1 words, zeroed by the caller; the last     */
+                                  /* word counts hits dropped because their chunk's region was full).    */
+                                  /* Grouping the hits of nearby histories lets gpet_digitize sort each  */
+                                  /* chunk in shared memory instead of scattering records through HBM.   */
+                                  /* One gpet_simulate batch per buffer (no appending); cap <= 2048.     */
 } gpet_hits;
 
 /* Simulates histories [first_history, first_history + n_pairs): source -> (phantom) -> panel search ->

@@ -17,6 +17,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgpet.so")
 GPET_IDS_NONE = 0xFFFFFFFF
+CHUNK_PAIRS = 512                     # GPET_HIT_CHUNK_PAIRS
 
 
 class GpetError(RuntimeError):
@@ -45,7 +46,7 @@ class _Source(C.Structure):
 
 class _Hits(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in ("history", "ids", "x", "y", "z", "e_keV", "tof_ns")] + \
-               [("capacity", C.c_uint64), ("n_hits", C.c_void_p), ("outcome_hash", C.c_void_p)]
+               [("capacity", C.c_uint64), ("n_hits", C.c_void_p), ("outcome_hash", C.c_void_p), ("chunk_fill", C.c_void_p)]
 
 
 class _Digitizer(C.Structure):
@@ -235,6 +236,7 @@ class HitBuffer:
     tof_ns: "torch.Tensor"
     n_hits: "torch.Tensor"                 # int64[1] device counter
     outcome_hash: Optional["torch.Tensor"] = None
+    chunk_fill: Optional["torch.Tensor"] = None   # int32[n_chunks + 1]: chunked layout (include/gpet.h), else dense
 
     @staticmethod
     def allocate(capacity: int, n_hash: int = 0, device="cuda") -> "HitBuffer":
@@ -245,6 +247,22 @@ class HitBuffer:
         return HitBuffer(i32(), i32(), f32(), f32(), f32(), f32(), f32(), torch.zeros(1, dtype=torch.int64, device=device),
                          torch.empty(2 * n_hash, dtype=torch.int64, device=device) if n_hash else None)
 
+    @staticmethod
+    def allocate_chunked(n_pairs: int, hits_per_pair: float, n_hash: int = 0, device="cuda") -> "HitBuffer":
+        """Chunked layout for one batch of n_pairs: a region of ceil(512 * hits_per_pair) entries per 512-pair chunk."""
+        import torch
+        n_chunks = (n_pairs + CHUNK_PAIRS - 1) // CHUNK_PAIRS
+        cap = min(2048, max(1, int(np.ceil(CHUNK_PAIRS * hits_per_pair))))
+        hb = HitBuffer.allocate(n_chunks * cap, n_hash, device)
+        hb.chunk_fill = torch.zeros(n_chunks + 1, dtype=torch.int32, device=device)
+        return hb
+
+    def reset(self):
+        """Zeroes the counters (before the next gpet_simulate into this buffer); enqueued on the current stream."""
+        self.n_hits.zero_()
+        if self.chunk_fill is not None:
+            self.chunk_fill.zero_()
+
     @property
     def capacity(self) -> int:
         return int(self.history.numel())
@@ -252,13 +270,28 @@ class HitBuffer:
     def struct(self) -> _Hits:
         return _Hits(self.history.data_ptr(), self.ids.data_ptr(), self.x.data_ptr(), self.y.data_ptr(), self.z.data_ptr(),
                      self.e_keV.data_ptr(), self.tof_ns.data_ptr(), self.capacity, self.n_hits.data_ptr(),
-                     self.outcome_hash.data_ptr() if self.outcome_hash is not None else None)
+                     self.outcome_hash.data_ptr() if self.outcome_hash is not None else None,
+                     self.chunk_fill.data_ptr() if self.chunk_fill is not None else None)
+
+    def dropped(self) -> int:
+        """Hits dropped for lack of room: dense layout n_hits - capacity, chunked layout the last chunk_fill word."""
+        if self.chunk_fill is not None:
+            return int(self.chunk_fill[-1].item())
+        return max(0, self.count() - self.capacity)
 
     def count(self) -> int:
         return int(self.n_hits.item())
 
     def to_numpy(self):
-        """Valid entries as numpy arrays (uint32 / float32), buffer order."""
+        """Valid entries as numpy arrays (uint32 / float32), buffer order (chunked layout: chunk by chunk)."""
+        if self.chunk_fill is not None:
+            fill = self.chunk_fill[:-1].cpu().numpy().astype(np.int64)
+            cap = self.capacity // len(fill)
+            sel = (np.arange(cap)[None, :] < np.minimum(fill, cap)[:, None]).ravel()
+            u = lambda t: t.cpu().numpy().view(np.uint32)[:len(sel)][sel]
+            f = lambda t: t.cpu().numpy()[:len(sel)][sel]
+            return dict(history=u(self.history), ids=u(self.ids), x=f(self.x), y=f(self.y), z=f(self.z), e_keV=f(self.e_keV),
+                        tof_ns=f(self.tof_ns))
         n = min(self.count(), self.capacity)
         u = lambda t: t[:n].cpu().numpy().view(np.uint32)
         f = lambda t: t[:n].cpu().numpy()

@@ -311,9 +311,18 @@ static int make_source(const gpet_source *s, const gpet_materials *m, DevSource 
   return GPET_OK;
 }
 
-static HitBuf hitbuf(const gpet_hits *h) {
-  HitBuf H = { h->history, h->ids, h->x, h->y, h->z, h->e_keV, h->tof_ns, h->capacity, reinterpret_cast<unsigned long long *>(h->n_hits) };
-  return H;
+// n_pairs = pairs of the batch the buffer holds (chunked layout: fixes the number of chunks and the region size)
+static int hitbuf(const gpet_hits *h, uint64_t n_pairs, HitBuf *out) {
+  HitBuf H = { h->history, h->ids, h->x, h->y, h->z, h->e_keV, h->tof_ns, h->capacity, reinterpret_cast<unsigned long long *>(h->n_hits),
+               nullptr, 0u, 0u };
+  if (h->chunk_fill) {
+    const uint64_t nc = (n_pairs + kHitChunkPairs - 1) / kHitChunkPairs;
+    const uint64_t cap = nc ? h->capacity / nc : 0;
+    if (cap < 1 || cap > kHitChunkCapMax) return fail(GPET_E_INVALID_ARG, "chunked hit buffer: capacity / n_chunks = %llu outside 1..%u",
+                                                      (unsigned long long)cap, kHitChunkCapMax);
+    H.chunk_fill = h->chunk_fill; H.chunk_cap = (uint32_t)cap; H.n_chunks = (uint32_t)nc;
+  }
+  *out = H; return GPET_OK;
 }
 
 // ---------------------------------------------------------------- transport
@@ -341,7 +350,8 @@ extern "C" int gpet_simulate(const gpet_geometry *g, const gpet_materials *m, co
   const uint32_t stage_mask = (D.kind == 1 && D.phantom) ? (1u << m->n_materials) - 1u : 0u;
   DevTables T; rc = staged_table(const_cast<gpet_materials *>(m), g->host.det_mask, stage_mask, &T); if (rc) return rc;
   unsigned long long *wc = nullptr; rc = next_work_counter(&wc); if (rc) return rc;
-  CUDA_TRY(launch_transport(g->host, g->dev, T, D, first_history, n_pairs, seed, hitbuf(hits), hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
+  HitBuf HB; rc = hitbuf(hits, n_pairs, &HB); if (rc) return rc;
+  CUDA_TRY(launch_transport(g->host, g->dev, T, D, first_history, n_pairs, seed, HB, hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
   return GPET_OK;
 }
 
@@ -370,7 +380,8 @@ extern "C" int gpet_digitize(const gpet_source *src, uint64_t seed, uint64_t n_p
   if (so) { SinglesBuf s = { so->history, so->ids, so->x, so->y, so->z, so->e_keV, so->t_s, so->capacity, reinterpret_cast<unsigned long long *>(so->n_singles) }; S = s; }
   CoincBuf Cb = { co->ids_a, co->ids_b, co->history_a, co->history_b, co->e_a, co->e_b, co->dt_ns, co->t_s, co->capacity,
                   reinterpret_cast<unsigned long long *>(co->n_coinc) };
-  CUDA_TRY(launch_digitize(P, hitbuf(hits), first_history, n_pairs, n_hits, scratch, scratch_bytes, S, Cb, (cudaStream_t)stream));
+  HitBuf HB; rc = hitbuf(hits, n_pairs, &HB); if (rc) return rc;
+  CUDA_TRY(launch_digitize(P, HB, first_history, n_pairs, n_hits, scratch, scratch_bytes, S, Cb, (cudaStream_t)stream));
   return GPET_OK;
 }
 

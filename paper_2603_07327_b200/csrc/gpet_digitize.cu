@@ -246,10 +246,96 @@ __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uin
   if (threadIdx.x == 0) kcnt[blockIdx.x] = s_cnt;
 }
 
+// ---------------------------------------------------------------- stages 1 + 2 for the chunked hit layout
+// One block per chunk of 512 pairs (gpet.h: gpet_hits.chunk_fill): the chunk's hits (~400, at most 2048) are already
+// together, so the sort by history is a counting sort in SHARED memory -- histogram with shared atomics, block scan,
+// order array -- followed by the same adder, blur, window and time as adder_kernel on the staged copies.  No count
+// pass, no global scan, no scatter of records through HBM; the hit buffer is read once, coalesced.
+__global__ void __launch_bounds__(256) chunk_adder_kernel(DigiParams P, Buckets B, uint64_t first_history, HitBuf H, SinRec *sing, uint32_t *srank,
+                                                          uint32_t *kcnt, uint32_t *bcnt) {
+  __shared__ uint32_t s_ids[kHitChunkCapMax];
+  __shared__ float s_e[kHitChunkCapMax], s_tof[kHitChunkCapMax];
+  __shared__ uint16_t s_h[kHitChunkCapMax], s_rk[kHitChunkCapMax], s_ord[kHitChunkCapMax];
+  __shared__ uint32_t s_cnt[kHitChunkPairs], s_off[kHitChunkPairs];
+  __shared__ uint32_t s_kept;
+  const uint32_t c = blockIdx.x, cap = H.chunk_cap, fill = H.chunk_fill[c], n = fill < cap ? fill : cap;
+  const unsigned long long g0 = (unsigned long long)c * cap;
+  const uint32_t first_lo = (uint32_t)first_history + c * kHitChunkPairs;
+  const int lane = threadIdx.x & 31;
+  const uint2 key = make_uint2((uint32_t)P.seed, (uint32_t)(P.seed >> 32));
+  s_cnt[threadIdx.x] = 0; s_cnt[threadIdx.x + 256] = 0;
+  if (threadIdx.x == 0) s_kept = 0;
+  __syncthreads();
+  for (uint32_t i = threadIdx.x; i < n; i += 256u) {                // stage keys and values, histogram by local history
+    const uint32_t h = H.history[g0 + i] - first_lo;
+    s_ids[i] = H.ids[g0 + i]; s_e[i] = H.e[g0 + i]; s_tof[i] = H.tof[g0 + i];
+    s_h[i] = (uint16_t)(h & (kHitChunkPairs - 1));
+    s_rk[i] = (uint16_t)atomicAdd(&s_cnt[h & (kHitChunkPairs - 1)], 1u);
+  }
+  __syncthreads();
+  {
+    const uint32_t v0 = s_cnt[2 * threadIdx.x], v1 = s_cnt[2 * threadIdx.x + 1];
+    uint32_t tot; const uint32_t ex = block_exclusive_scan_256(v0 + v1, &tot);
+    s_off[2 * threadIdx.x] = ex; s_off[2 * threadIdx.x + 1] = ex + v0;
+  }
+  __syncthreads();
+  for (uint32_t i = threadIdx.x; i < n; i += 256u) s_ord[s_off[s_h[i]] + s_rk[i]] = (uint16_t)i;
+  __syncthreads();
+  for (uint32_t j0 = 0; j0 < n; j0 += 256u) {                        // adder: one thread per hit, in history order
+    const uint32_t j = j0 + threadIdx.x;
+    bool keep = false; SinRec s;
+    if (j < n) {
+      const uint32_t i = s_ord[j], h = s_h[i], b = s_off[h], k = s_cnt[h], my_ids = s_ids[i], unit = my_ids >> P.shift;
+      bool leader = true; uint32_t best = i;
+      float e_sum = s_e[i], tof_min = s_tof[i];
+      if (k > 1) {
+        const uint64_t my_key = ((uint64_t)my_ids << 32) | i;
+        long long isum = 0; float e_best = -1.0f; uint32_t best_ord = 0;
+        for (uint32_t q = b; q < b + k; ++q) {
+          const uint32_t i2 = s_ord[q], ids2 = s_ids[i2];
+          if ((ids2 >> P.shift) != unit) continue;
+          if ((((uint64_t)ids2 << 32) | i2) < my_key) { leader = false; break; }
+          const float e2 = s_e[i2];
+          isum += __double2ll_rn((double)e2 * 1099511627776.0);
+          const uint32_t ord = ids2 & 31u;
+          if (e2 > e_best || (e2 == e_best && ord < best_ord)) { e_best = e2; best = i2; best_ord = ord; }
+          tof_min = fminf(tof_min, s_tof[i2]);
+        }
+        e_sum = (float)((double)isum * (1.0 / 1099511627776.0));
+      }
+      if (leader) {
+        const uint64_t history = first_history + (uint64_t)c * kHitChunkPairs + h;
+        const uint4 w = philox4x32_10(make_uint4((uint32_t)history, 0u, 3u, unit), key);        // Box-Muller on words 0,1
+        const float nrm = sqrtf(-2.0f * logf(u01(w.x))) * cospif(2.0f * u01(w.y));
+        const float sigma = P.sigma_scale * (P.ref_keV > 0.0f ? sqrtf(P.ref_keV * e_sum) : e_sum);
+        const float e_b = fmaf(sigma, nrm, e_sum);
+        keep = e_b >= P.e_lo && e_b < P.e_hi;
+        if (keep) {
+          s.t = __dadd_rn(decay_time(P, history), __dmul_rn((double)tof_min, 1e-9));
+          s.history = (uint32_t)history; s.ids = s_ids[best]; s.x = H.x[g0 + best]; s.y = H.y[g0 + best]; s.z = H.z[g0 + best]; s.e = e_b;
+        }
+      }
+    }
+    const unsigned mk = __ballot_sync(0xFFFFFFFFu, keep);
+    if (mk) {
+      uint32_t o = 0;
+      if (lane == 0) o = atomicAdd(&s_kept, (uint32_t)__popc(mk));
+      o = (uint32_t)g0 + __shfl_sync(0xFFFFFFFFu, o, 0) + __popc(mk & ((1u << lane) - 1u));
+      if (keep) {
+        store_rec(&sing[o], &s);
+        srank[o] = atomicAdd(&bcnt[bucket_of(B, s.t)], 1u);
+      }
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) kcnt[c] = s_kept;
+}
+
 // ---------------------------------------------------------------- stage 3: time-bucket counting sort
-__global__ void __launch_bounds__(256) bucket_scatter_kernel(const SinRec *sing, const uint32_t *srank, const uint32_t *n_rec, const uint32_t *kcnt,
-                                                             Buckets B, const uint32_t *boff, SinRec *srt) {
-  const uint32_t r0 = blockIdx.x * region_size(*n_rec, gridDim.x), m = kcnt[blockIdx.x];   // this block's kept singles: sing[r0 .. r0 + m)
+// region = records per block (0: derived from *n_rec as in adder_kernel)
+__global__ void __launch_bounds__(256) bucket_scatter_kernel(const SinRec *sing, const uint32_t *srank, const uint32_t *n_rec, uint32_t region,
+                                                             const uint32_t *kcnt, Buckets B, const uint32_t *boff, SinRec *srt) {
+  const uint32_t r0 = blockIdx.x * (region ? region : region_size(*n_rec, gridDim.x)), m = kcnt[blockIdx.x];   // this block's kept singles
   for (uint32_t i = r0 + threadIdx.x; i < r0 + m; i += 256u) {
     SinRec s; store_rec(&s, &sing[i]);
     store_rec(&srt[boff[bucket_of(B, s.t)] + srank[i]], &s);
@@ -318,7 +404,7 @@ Layout layout(uint64_t N, uint64_t M) {
   Layout L; size_t o = 0; const uint64_t Mx = M ? M : 1;
   auto take = [&](size_t bytes) { o = (o + 255) & ~(size_t)255; size_t r = o; o += bytes; return r; };
   L.nb = (Mx + 1) / 2;              // time buckets: kept singles are ~0.4 per hit, so ~1 per bucket
-  L.kcnt = take(4 * 148 * 16);      // kept singles per adder block
+  L.kcnt = take(4 * (148 * 16 + N / kHitChunkPairs + 2));   // kept singles per adder block (dense) or per chunk (chunked layout)
   L.cnt = take(4 * N); L.off = take(4 * (N + 1));
   // control block, cleared by one memset per call: kept-singles counter, then the look-back state of the three scans
   const size_t s0 = 8 * (N / kTile + 3), s1 = 8 * (L.nb / kTile + 3), s2 = 8 * (Mx / kTile + 3);
@@ -348,15 +434,11 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   uint32_t *hrank = (uint32_t *)(s + L.hrank), *srank = (uint32_t *)(s + L.srank);
   HitRec *rec = (HitRec *)(s + L.rec); SinRec *srt = (SinRec *)(s + L.rec), *sing = (SinRec *)(s + L.sing), *fin = (SinRec *)(s + L.fin);
   cudaError_t e;
-  if ((e = cudaMemsetAsync(cnt, 0, 4 * N, st)) != cudaSuccess) return e;
+  if (!H.chunk_fill && (e = cudaMemsetAsync(cnt, 0, 4 * N, st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(s + L.ctl, 0, L.ctl_bytes, st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(bcnt, 0, 4 * L.nb, st)) != cudaSuccess) return e;
   const uint32_t nh = (uint32_t)n_hits, np = (uint32_t)N, first_lo = (uint32_t)first_history;
-  // 1. counting sort by history
-  if (nh) { count_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, cnt, hrank); count_launch(); }
-  if ((e = exclusive_scan(cnt, N, nullptr, off, st0, nullptr, st)) != cudaSuccess) return e;
-  if (nh) { scatter_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, off, hrank, rec); count_launch(); }
-  // 2. adder, blur, window, time; kept singles appended and counted into time buckets
+  const bool chunked = H.chunk_fill != nullptr;
   const uint64_t B = P.pairs_per_slice;
   const double slice_s = (double)B / P.activity_bq;
   Buckets bk; bk.nb = (uint32_t)L.nb;
@@ -364,10 +446,20 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   const double t_hi = ((double)((first_history + n_pairs - 1) / B) + 1.0) * slice_s + 2e-6;
   bk.scale = (double)bk.nb / (t_hi - bk.t_lo);
   const int ga = grid_for(M);                                         // adder and bucket scatter share the block -> region split
-  adder_kernel<<<ga, 256, 0, st>>>(P, bk, first_history, off, off + N, rec, sing, srank, kcnt, bcnt); count_launch();
+  if (chunked) {
+    // 1 + 2. per chunk in shared memory: sort by history, adder, blur, window, time
+    chunk_adder_kernel<<<H.n_chunks, 256, 0, st>>>(P, bk, first_history, H, sing, srank, kcnt, bcnt); count_launch();
+  } else {
+    // 1. counting sort by history
+    if (nh) { count_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, cnt, hrank); count_launch(); }
+    if ((e = exclusive_scan(cnt, N, nullptr, off, st0, nullptr, st)) != cudaSuccess) return e;
+    if (nh) { scatter_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, off, hrank, rec); count_launch(); }
+    // 2. adder, blur, window, time; kept singles appended and counted into time buckets
+    adder_kernel<<<ga, 256, 0, st>>>(P, bk, first_history, off, off + N, rec, sing, srank, kcnt, bcnt); count_launch();
+  }
   // 3. time-bucket counting sort
   if ((e = exclusive_scan(bcnt, L.nb, nullptr, boff, st1, S.n, st)) != cudaSuccess) return e;
-  bucket_scatter_kernel<<<ga, 256, 0, st>>>(sing, srank, off + N, kcnt, bk, boff, srt); count_launch();
+  bucket_scatter_kernel<<<chunked ? (int)H.n_chunks : ga, 256, 0, st>>>(sing, srank, off + N, chunked ? H.chunk_cap : 0u, kcnt, bk, boff, srt); count_launch();
   bucket_sort_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(srt, P.shift, boff + L.nb, bk, boff, fin, S); count_launch();
   // 4. coincidences (lengths known on the device only: the scan stops at the number of kept singles)
   const uint32_t *n_singles = boff + L.nb;

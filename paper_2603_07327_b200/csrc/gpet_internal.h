@@ -10,7 +10,10 @@ namespace gpet {
 struct HitBuf {            // device view of gpet_hits
   uint32_t *history, *ids; float *x, *y, *z, *e, *tof;
   unsigned long long capacity; unsigned long long *n_hits;
+  uint32_t *chunk_fill;      // chunked layout (gpet.h): hits of pairs [512 c, 512 (c+1)) of the batch at [c cap, c cap + fill[c])
+  uint32_t chunk_cap, n_chunks;
 };
+constexpr uint32_t kHitChunkPairs = 512, kHitChunkShift = 9, kHitChunkCapMax = 2048;
 
 struct DevSource {
   int kind; float pos[3], beam[3]; float acol_sigma;            // radians

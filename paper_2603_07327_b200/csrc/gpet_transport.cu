@@ -123,6 +123,31 @@ __device__ __forceinline__ void store_hit(const HitBuf &H, unsigned long long o,
     H.e[o] = __uint_as_float(stage.w[5][slot]); H.tof[o] = __uint_as_float(stage.w[6][slot]);
   }
 }
+// Flush up to 32 staged hits (lane < count has one, in ring slot `slot`).  Dense layout: one atomicAdd on the global
+// counter, seven coalesced stores.  Chunked layout: the hits go to the region of their 512-pair chunk; lanes of the same
+// chunk (almost always all of them) share one atomicAdd on that chunk's fill counter and write consecutive entries.
+__device__ __forceinline__ void flush_hits(const HitBuf &H, uint32_t first_lo, const HitStage &stage, uint32_t slot, uint32_t count, int lane) {
+  const bool act = (uint32_t)lane < count;
+  if (H.chunk_fill == nullptr) {
+    unsigned long long base = 0;
+    if (lane == 0) base = atomicAdd(H.n_hits, (unsigned long long)count);
+    base = __shfl_sync(0xFFFFFFFFu, base, 0);
+    if (act) store_hit(H, base + lane, stage, slot);
+  } else {
+    if (lane == 0) atomicAdd(H.n_hits, (unsigned long long)count);                    // total produced (no return value needed)
+    const uint32_t chunk = act ? (stage.w[0][slot] - first_lo) >> kHitChunkShift : 0xFFFFFFFFu;
+    const unsigned grp = __match_any_sync(0xFFFFFFFFu, chunk);
+    const int leader = __ffs(grp) - 1;
+    uint32_t base = 0;
+    if (act && lane == leader && chunk < H.n_chunks) base = atomicAdd(&H.chunk_fill[chunk], (uint32_t)__popc(grp));
+    base = __shfl_sync(0xFFFFFFFFu, base, leader);
+    if (act && chunk < H.n_chunks) {
+      const uint32_t pos = base + __popc(grp & ((1u << lane) - 1u));
+      if (pos < H.chunk_cap) store_hit(H, (unsigned long long)chunk * H.chunk_cap + pos, stage, slot);
+      else atomicAdd(&H.chunk_fill[H.n_chunks], 1u);                                   // dropped: this chunk's region is full
+    }
+  }
+}
 
 // [R20] Rayleigh: Thomson pdf by closed-form inversion of the cdf, then a rotation about d
 __device__ __noinline__ float3 rayleigh_dir(float dx, float dy, float dz, float u_polar, float u_azimuth) {
@@ -278,10 +303,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
     stage_cnt += __popc(who);
     __syncwarp();
     if (stage_cnt >= 32) {
-      unsigned long long base = 0;
-      if (lane == 0) base = atomicAdd(H.n_hits, 32ull);
-      base = __shfl_sync(0xFFFFFFFFu, base, 0);
-      store_hit(H, base + lane, stage, (stage_head + lane) & (kStage - 1));
+      flush_hits(H, (uint32_t)first_history, stage, (stage_head + lane) & (kStage - 1), 32u, lane);
       stage_head = (stage_head + 32) & (kStage - 1); stage_cnt -= 32;
       __syncwarp();
     }
@@ -568,12 +590,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
   }
 
   // ------------------------------------------------ drain the staged hits (fewer than 32 per warp)
-  if (stage_cnt) {
-    unsigned long long base = 0;
-    if (lane == 0) base = atomicAdd(H.n_hits, (unsigned long long)stage_cnt);
-    base = __shfl_sync(0xFFFFFFFFu, base, 0);
-    if ((uint32_t)lane < stage_cnt) store_hit(H, base + lane, stage, (stage_head + lane) & (kStage - 1));
-  }
+  if (stage_cnt) flush_hits(H, (uint32_t)first_history, stage, (stage_head + lane) & (kStage - 1), stage_cnt, lane);
 }
 
 static int g_transport_warps = kWarps;             // warps per CTA (one CTA per SM); fewer leave room for other streams' kernels

@@ -36,7 +36,7 @@ def test_library_exports_every_declared_symbol():
 def test_binding_structs_match_the_header_layout():
     # sizes follow from the C declarations (LP64): checked so that a header edit cannot silently skew the binding
     assert ctypes.sizeof(api._LayerDesc) == 48 and ctypes.sizeof(api._GeometryDesc) == 64
-    assert ctypes.sizeof(api._Source) == 104 and ctypes.sizeof(api._Hits) == 80
+    assert ctypes.sizeof(api._Source) == 104 and ctypes.sizeof(api._Hits) == 88
     assert ctypes.sizeof(api._Digitizer) == 32 and ctypes.sizeof(api._Singles) == 72 and ctypes.sizeof(api._Coinc) == 80
 
 

@@ -558,3 +558,41 @@ def test_paper_scanners_parity_and_the_split_layer_identity(tables):
     assert np.all((a["ids"] >> 18) & 3 == 0) and ((b["ids"] >> 18) & 3).max() == 1
     ratio = len(out["P3"]["ids"]) / len(a["ids"])
     assert 0.96 < ratio < 0.99                                        # paper Table 1: 2 620 170 / 2 671 908 = 0.981
+
+
+# ----------------------------------------------------------------------------- chunked hit layout (the one bench.py times)
+@pytest.mark.parametrize("cfg,idx,n", [("C1", 0, 300_001), ("C3", 10, 200_000), ("C4", 0, 100_000)])
+def test_chunked_hit_layout_equals_the_dense_one(tables, cfg, idx, n):
+    """gpet_hits.chunk_fill: hits grouped per 512-pair chunk, digitized by a shared-memory sort per chunk.  Same hits as
+    the dense layout (as a set) and identical singles and coincidences, record for record; a region that is too small
+    drops hits and says so."""
+    r = W.config_runs(cfg, n)[idx]
+    first = 5_000_000
+    geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+    dense = api.HitBuffer.allocate(3 * n)
+    chunk = api.HitBuffer.allocate_chunked(n, 3.0)
+    api.gpet_simulate(geom, m, s, first, n, r.seed, dense)
+    api.gpet_simulate(geom, m, s, first, n, r.seed, chunk)
+    torch.cuda.synchronize()
+    assert chunk.count() == dense.count() and chunk.dropped() == 0
+    a, b = PU.canonical(dense.to_numpy()), PU.canonical(chunk.to_numpy())
+    assert all(np.array_equal(a[k], b[k]) for k in PU.HIT_KEYS)
+    fill = chunk.chunk_fill[:-1].cpu().numpy()
+    assert len(fill) == (n + 511) // 512 and int(fill.sum()) == dense.count()
+    out = []
+    for hb in (dense, chunk):
+        cap = hb.capacity
+        scratch = torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda")
+        sg, co = api.SinglesBuffer.allocate(cap), api.CoincBuffer.allocate(cap)
+        api.gpet_digitize(s, r.seed, 20_000_000, first, n, hb, cap, r.digitizer, scratch, sg, co)
+        torch.cuda.synchronize()
+        out.append((sg.to_numpy(), co.to_numpy()))
+    (s0, c0), (s1, c1) = out
+    assert len(s0["ids"]) > 0.2 * n * (0.3 if cfg == "C4" else 1) and all(np.array_equal(s0[k], s1[k]) for k in s0)
+    assert len(c0["ids_a"]) > 100 and all(np.array_equal(c0[k], c1[k]) for k in c0)
+    # regions too small: hits are dropped, counted, and the total is still reported
+    tight = api.HitBuffer.allocate_chunked(n, 0.25)
+    api.gpet_simulate(geom, m, s, first, n, r.seed, tight)
+    torch.cuda.synchronize()
+    assert tight.count() == dense.count() and tight.dropped() > 0
+    assert tight.dropped() == dense.count() - int(np.minimum(tight.chunk_fill[:-1].cpu().numpy(), 128).sum())

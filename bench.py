@@ -5,7 +5,7 @@ A *step* is one pass of the whole hot path (gpet_simulate + gpet_digitize: sourc
 Woodcock transport, hits, adder, blur, window, time sort, coincidences) over one batch of synthetic input.
 The timed steps run in turn on one stream (the transport kernel with its full 24-warp CTA per SM).  After the timed
 region the same steps are also run as a two-stream pipeline -- the transport kernel of step k+1 (bound by instruction
-issue, CTA of 16 warps) beside the digitizer of step k (bound by HBM latency) -- and reported under "pipelined";
+issue) beside the digitizer of step k (bound by HBM latency) -- and reported under "pipelined";
 `--overlap` makes that pipeline the timed headline instead.
 Workload at N=1: BASELINE.json configs[1] (C1): 12-panel ring, single layer, centred point source, 0.5 deg
 acolinearity, 1e7 pairs, 350-650 keV, 15 % blur, 4 ns window.  With N ranks each rank runs its own 1e7
@@ -156,12 +156,14 @@ def run_ours(args):
     # Two batches in flight: gpet_simulate of step k+1 (stream A) runs beside gpet_digitize of step k (stream B); each
     # step is still one full pass of the hot path over its own 1e7 pairs, and every step's work lies in the timed region.
     nbuf = 2 if args.overlap else 1
-    hits = [api.HitBuffer.allocate(cap) for _ in range(nbuf)]
+    # chunked hit layout (include/gpet.h): hits grouped per 512-pair chunk, sorted by history in shared memory by the digitizer
+    hits = [api.HitBuffer.allocate_chunked(n, args.hits_per_pair) for _ in range(nbuf)]
+    cap = hits[0].capacity
     coinc = [api.CoincBuffer.allocate(cap // 4) for _ in range(nbuf)]
     scratch = [torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda") for _ in range(nbuf)]
     s_a = torch.cuda.Stream()
     s_b = torch.cuda.Stream() if args.overlap else s_a
-    warps = api.gpet_set_transport_warps(args.transport_warps if args.transport_warps else (16 if args.overlap else 24))
+    warps = api.gpet_set_transport_warps(args.transport_warps if args.transport_warps else 24)
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
 
@@ -176,7 +178,7 @@ def run_ours(args):
                 s_a.wait_event(dig_done[i])                         # hit buffer i has been digitized
             e = [ev() for _ in range(4)] if record else None
             with torch.cuda.stream(s_a):
-                hits[i].n_hits.zero_()
+                hits[i].reset()
                 if record:
                     e[0].record(s_a)
                 api.gpet_simulate(geom, mats, src, first, n, run.seed, hits[i], s_a)
@@ -224,8 +226,8 @@ def run_ours(args):
     transport_ms = sum(e[0].elapsed_time(e[1]) for e in t_events) / len(t_events)
     digitize_ms = sum(e[2].elapsed_time(e[3]) for e in t_events) / len(t_events)
     n_hits, n_coinc = hits[0].count(), int(coinc[0].n_coinc.item())
-    if n_hits > cap:
-        raise SystemExit(f"hit buffer overflow ({n_hits} > {cap}); raise --hits-per-pair")
+    if hits[0].dropped():
+        raise SystemExit(f"hit buffer overflow ({hits[0].dropped()} hits dropped); raise --hits-per-pair")
     value = n_total * args.steps / (ms_total * 1e-3)
 
     # ---- the two halves alone (untimed extra, not part of `value`): serial steps with the full 24-warp transport CTA
@@ -235,7 +237,7 @@ def run_ours(args):
         st = torch.cuda.current_stream()
         ta, tb = [], []
         for k in range(8):
-            hits[0].n_hits.zero_()
+            hits[0].reset()
             x, y, z = ev(), ev(), ev()
             x.record(st); api.gpet_simulate(geom, mats, src, first, n, run.seed, hits[0], st); y.record(st)
             api.gpet_digitize(src, run.seed, n_total, first, n, hits[0], cap, run.digitizer, scratch[0], None, coinc[0], st); z.record(st)
@@ -246,8 +248,8 @@ def run_ours(args):
     # ---- the same steps as a two-stream pipeline (extra, after the timed region; not part of `value`)
     pipelined = None
     if not args.overlap and not args.no_pipelined:
-        pw = api.gpet_set_transport_warps(16)
-        hits.append(api.HitBuffer.allocate(cap)); coinc.append(api.CoincBuffer.allocate(cap // 4))
+        pw = api.gpet_set_transport_warps(args.transport_warps if args.transport_warps else 24)
+        hits.append(api.HitBuffer.allocate_chunked(n, args.hits_per_pair)); coinc.append(api.CoincBuffer.allocate(cap // 4))
         scratch.append(torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda"))
         s_b2 = torch.cuda.Stream()
         sim_done = [torch.cuda.Event() for _ in range(2)]; dig_done = [torch.cuda.Event() for _ in range(2)]
@@ -258,7 +260,7 @@ def run_ours(args):
                 if k >= 2:
                     s_a.wait_event(dig_done[i])
                 with torch.cuda.stream(s_a):
-                    hits[i].n_hits.zero_()
+                    hits[i].reset()
                     api.gpet_simulate(geom, mats, src, first, n, run.seed, hits[i], s_a)
                 sim_done[i].record(s_a)
                 s_b2.wait_event(sim_done[i])
@@ -376,7 +378,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-pipelined", action="store_true", help="skip the extra two-stream pipeline measurement")
     ap.add_argument("--overlap", action="store_true", help="time the two-stream pipeline as the headline instead of the serial steps")
-    ap.add_argument("--transport-warps", type=int, default=0, help="warps per transport CTA (default: 16 with overlap, 24 without)")
+    ap.add_argument("--transport-warps", type=int, default=0, help="warps per transport CTA (default 24; fewer leave more of each SM to the other stream in the pipeline)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -398,14 +398,20 @@ extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, co
                              gpet_host_outputs *out) {
   if (!g || !m || !src || !dig || !out) return fail(GPET_E_INVALID_ARG, "gpet_run_host: NULL argument");
   if (n_pairs == 0 || n_pairs >= (1ull << 32) || !(hits_per_pair > 0.0)) return fail(GPET_E_INVALID_ARG, "gpet_run_host: bad counts");
-  const uint64_t cap = (uint64_t)((double)n_pairs * hits_per_pair) + 1024;
+  // hits that stay on the device use the chunked layout (shared-memory sort per chunk in the digitizer); hits the caller
+  // wants on the host use the dense one, which is what gpet_host_outputs describes
+  const bool chunked = out->hits.history == nullptr;
+  const uint64_t n_chunks = (n_pairs + kHitChunkPairs - 1) / kHitChunkPairs;
+  uint64_t chunk_cap = (uint64_t)ceil((double)kHitChunkPairs * hits_per_pair);
+  if (chunk_cap > kHitChunkCapMax) chunk_cap = kHitChunkCapMax;
+  const uint64_t cap = chunked ? n_chunks * chunk_cap : (uint64_t)((double)n_pairs * hits_per_pair) + 1024;
   if (cap >= (1ull << 32)) return fail(GPET_E_INVALID_ARG, "gpet_run_host: batch too large, split it");
   const size_t scratch_bytes = digitize_scratch_bytes(n_pairs, cap);
   const size_t nvox = src->kind == 1 && src->phantom_material ? (size_t)src->dims[0] * src->dims[1] * src->dims[2] : 0;
   // one cached device arena per process: repeated batches of the same size do not re-allocate
   static std::mutex arena_lock; static char *arena_base = nullptr; static size_t arena_size = 0;
   std::lock_guard<std::mutex> arena_guard(arena_lock);
-  DevArena A; A.size = cap * (28 + 36 + 40) + scratch_bytes + nvox + (out->hits.outcome_hash ? 16 * n_pairs : 0) + 64 * 256;
+  DevArena A; A.size = cap * (28 + 36 + 40) + 4 * (n_chunks + 1) + scratch_bytes + nvox + (out->hits.outcome_hash ? 16 * n_pairs : 0) + 64 * 256;
   if (A.size > arena_size) {
     if (arena_base) cudaFree(arena_base);
     arena_base = nullptr; arena_size = 0;
@@ -420,6 +426,7 @@ extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, co
     H.history = A.take<uint32_t>(cap); H.ids = A.take<uint32_t>(cap); H.x = A.take<float>(cap); H.y = A.take<float>(cap); H.z = A.take<float>(cap);
     H.e_keV = A.take<float>(cap); H.tof_ns = A.take<float>(cap); H.capacity = cap; H.n_hits = A.take<uint64_t>(1);
     H.outcome_hash = out->hits.outcome_hash ? A.take<uint64_t>(2 * n_pairs) : nullptr;
+    H.chunk_fill = chunked ? A.take<uint32_t>(n_chunks + 1) : nullptr;
     gpet_singles S; S.history = A.take<uint32_t>(cap); S.ids = A.take<uint32_t>(cap); S.x = A.take<float>(cap); S.y = A.take<float>(cap);
     S.z = A.take<float>(cap); S.e_keV = A.take<float>(cap); S.t_s = A.take<double>(cap); S.capacity = cap; S.n_singles = A.take<uint64_t>(1);
     gpet_coincidences Cc; Cc.ids_a = A.take<uint32_t>(cap); Cc.ids_b = A.take<uint32_t>(cap); Cc.history_a = A.take<uint32_t>(cap);
@@ -434,15 +441,18 @@ extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, co
     }
     if (A.used > A.size) { rc = fail(GPET_E_OVERFLOW, "internal arena too small"); break; }
     if (cudaMemsetAsync(H.n_hits, 0, 8, st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "memset failed"); break; }
+    if (chunked && cudaMemsetAsync(H.chunk_fill, 0, 4 * (n_chunks + 1), st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "memset failed"); break; }
     if ((rc = gpet_simulate(g, m, &s2, first_history, n_pairs, seed, &H, st))) break;
     gpet_singles Sd = S;                   // singles arrays are written only when the caller wants them; the count always is
     if (!out->singles.history) { Sd.history = Sd.ids = nullptr; Sd.x = Sd.y = Sd.z = Sd.e_keV = nullptr; Sd.t_s = nullptr; }
     if ((rc = gpet_digitize(&s2, seed, n_pairs_total, first_history, n_pairs, &H, cap, dig, scratch, scratch_bytes, &Sd, &Cc, st))) break;
-    uint64_t nh = 0, ns = 0, nc = 0;
+    uint64_t nh = 0, ns = 0, nc = 0; uint32_t dropped = 0;
+    if (chunked) cudaMemcpyAsync(&dropped, H.chunk_fill + n_chunks, 4, cudaMemcpyDeviceToHost, st);
     cudaMemcpyAsync(&nh, H.n_hits, 8, cudaMemcpyDeviceToHost, st);
     cudaMemcpyAsync(&ns, S.n_singles, 8, cudaMemcpyDeviceToHost, st); cudaMemcpyAsync(&nc, Cc.n_coinc, 8, cudaMemcpyDeviceToHost, st);
     if (cudaStreamSynchronize(st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "transport/digitizer failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
-    if (nh > cap) { rc = fail(GPET_E_OVERFLOW, "hit buffer overflow: %llu hits > capacity %llu; raise hits_per_pair", (unsigned long long)nh, (unsigned long long)cap); break; }
+    if (dropped) { rc = fail(GPET_E_OVERFLOW, "hit buffer overflow: %u hits dropped; raise hits_per_pair", dropped); break; }
+    if (!chunked && nh > cap) { rc = fail(GPET_E_OVERFLOW, "hit buffer overflow: %llu hits > capacity %llu; raise hits_per_pair", (unsigned long long)nh, (unsigned long long)cap); break; }
 #define D2H(dst, srcp, n, T) do { if ((dst) && (n)) cudaMemcpyAsync((dst), (srcp), sizeof(T) * (n), cudaMemcpyDeviceToHost, st); } while (0)
     const uint64_t ch = nh < out->hits.capacity ? nh : out->hits.capacity;
     D2H(out->hits.history, H.history, ch, uint32_t); D2H(out->hits.ids, H.ids, ch, uint32_t); D2H(out->hits.x, H.x, ch, float);

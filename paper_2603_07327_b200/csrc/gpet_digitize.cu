@@ -253,12 +253,13 @@ __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uin
 // pass, no global scan, no scatter of records through HBM; the hit buffer is read once, coalesced.
 __global__ void __launch_bounds__(256) chunk_adder_kernel(DigiParams P, Buckets B, uint64_t first_history, HitBuf H, SinRec *sing, uint32_t *srank,
                                                           uint32_t *kcnt, uint32_t *bcnt) {
-  __shared__ uint32_t s_ids[kHitChunkCapMax];
-  __shared__ float s_e[kHitChunkCapMax], s_tof[kHitChunkCapMax];
-  __shared__ uint16_t s_h[kHitChunkCapMax], s_rk[kHitChunkCapMax], s_ord[kHitChunkCapMax];
+  extern __shared__ __align__(16) unsigned char chunk_smem[];       // 18 bytes per region entry (cap rounded up to 8): sized at launch
   __shared__ uint32_t s_cnt[kHitChunkPairs], s_off[kHitChunkPairs];
   __shared__ uint32_t s_kept;
-  const uint32_t c = blockIdx.x, cap = H.chunk_cap, fill = H.chunk_fill[c], n = fill < cap ? fill : cap;
+  const uint32_t c = blockIdx.x, cap = H.chunk_cap, cap8 = (cap + 7u) & ~7u, fill = H.chunk_fill[c], n = fill < cap ? fill : cap;
+  uint32_t *s_ids = reinterpret_cast<uint32_t *>(chunk_smem);
+  float *s_e = reinterpret_cast<float *>(s_ids + cap8), *s_tof = s_e + cap8;
+  uint16_t *s_h = reinterpret_cast<uint16_t *>(s_tof + cap8), *s_rk = s_h + cap8, *s_ord = s_rk + cap8;
   const unsigned long long g0 = (unsigned long long)c * cap;
   const uint32_t first_lo = (uint32_t)first_history + c * kHitChunkPairs;
   const int lane = threadIdx.x & 31;
@@ -448,7 +449,7 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   const int ga = grid_for(M);                                         // adder and bucket scatter share the block -> region split
   if (chunked) {
     // 1 + 2. per chunk in shared memory: sort by history, adder, blur, window, time
-    chunk_adder_kernel<<<H.n_chunks, 256, 0, st>>>(P, bk, first_history, H, sing, srank, kcnt, bcnt); count_launch();
+    chunk_adder_kernel<<<H.n_chunks, 256, 18 * (size_t)((H.chunk_cap + 7u) & ~7u), st>>>(P, bk, first_history, H, sing, srank, kcnt, bcnt); count_launch();
   } else {
     // 1. counting sort by history
     if (nh) { count_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, cnt, hrank); count_launch(); }

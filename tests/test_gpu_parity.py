@@ -284,12 +284,14 @@ def test_c1_full_size_digitizer_sampled_histories(tables):
     r = W.config_runs("C1")[0]
     n = r.n_pairs
     geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
-    cap = int(1.2 * n) + 1024
-    hb, sg, co = api.HitBuffer.allocate(cap), api.SinglesBuffer.allocate(cap), api.CoincBuffer.allocate(cap // 4)
+    hb = api.HitBuffer.allocate_chunked(n, 1.2)                       # bench.py's hit buffer: chunked layout, 1.2 hits per pair
+    cap = hb.capacity
+    sg, co = api.SinglesBuffer.allocate(cap), api.CoincBuffer.allocate(cap // 4)
     scratch = torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda")
     api.gpet_simulate(geom, m, s, 0, n, r.seed, hb)
     api.gpet_digitize(s, r.seed, n, 0, n, hb, cap, r.digitizer, scratch, sg, co)
     torch.cuda.synchronize()
+    assert hb.dropped() == 0
     gs, gc = sg.to_numpy(), co.to_numpy()
     assert 0.32 < len(gs["ids"]) / n < 0.35 and 0.055 < len(gc["ids_a"]) / n < 0.060
     assert np.all(np.diff(gs["t_s"]) >= 0)

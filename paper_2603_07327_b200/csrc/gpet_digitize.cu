@@ -22,8 +22,9 @@ constexpr int kItems = 16;       // elements per thread of a scan tile (four 16-
 constexpr int kTile = 256 * kItems;
 
 // ---------------------------------------------------------------- device-wide exclusive scan (u32)
-__device__ __forceinline__ uint32_t block_exclusive_scan_256(uint32_t v, uint32_t *total) {
-  __shared__ uint32_t warp_sum[8];
+template <int NW>
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t *total) {
+  __shared__ uint32_t warp_sum[NW];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   uint32_t inc = v;
 #pragma unroll
@@ -33,10 +34,11 @@ __device__ __forceinline__ uint32_t block_exclusive_scan_256(uint32_t v, uint32_
   __syncthreads();
   uint32_t base = 0, tot = 0;
 #pragma unroll
-  for (int w = 0; w < 8; ++w) { const uint32_t s = warp_sum[w]; if (w < wid) base += s; tot += s; }
+  for (int w = 0; w < NW; ++w) { const uint32_t s = warp_sum[w]; if (w < wid) base += s; tot += s; }
   *total = tot;
   return base + inc - v;
 }
+__device__ __forceinline__ uint32_t block_exclusive_scan_256(uint32_t v, uint32_t *total) { return block_exclusive_scan<8>(v, total); }
 
 // Single-pass exclusive scan with decoupled look-back (one read and one write of the data).  Tiles take tickets
 // from an atomic counter, so a tile only ever waits for tiles that are already running or done; a tile publishes
@@ -171,6 +173,15 @@ __device__ __forceinline__ double decay_time(const DigiParams &P, uint64_t histo
   return __dmul_rn(__dadd_rn((double)slice, u53), P.slice_s);                               // slice_s = B / A
 }
 
+// [R25] standard normal by Box-Muller.  The blurred energy must stay within 1e-3 keV of the fp64 oracle's: sigma is
+// ~33 keV, so n needs 3e-5 absolute.  lg2.approx is good to ~1e-7 absolute in ln u, i.e. 0.7e-7 / sqrt(|ln u|) in n:
+// fine below u = 0.999, and the accurate logf takes the rest (1 draw in 1000); cos.approx on [-pi, pi] is good to 4e-7.
+__device__ __forceinline__ float box_muller(float u0, float u1) {
+  const float l = u0 < 0.999f ? __logf(u0) : logf(u0);
+  float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(-2.0f * l));
+  return -r * __cosf(6.283185307179586f * (u1 - 0.5f));              // cos(2 pi u) = -cos(2 pi u - pi)
+}
+
 // records per block of the adder / bucket-scatter pair: the same split in both kernels, a multiple of the block size
 __device__ __forceinline__ uint32_t region_size(uint32_t n, uint32_t blocks) {
   return (uint32_t)(((((unsigned long long)n + blocks - 1) / blocks) + 255ull) & ~255ull);
@@ -220,7 +231,7 @@ __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uin
       if (leader) {
         const uint64_t history = first_history + h;
         const uint4 w = philox4x32_10(make_uint4((uint32_t)history, 0u, 3u, unit), key);        // Box-Muller on words 0,1
-        const float nrm = sqrtf(-2.0f * logf(u01(w.x))) * cospif(2.0f * u01(w.y));
+        const float nrm = box_muller(u01(w.x), u01(w.y));
         const float sigma = P.sigma_scale * (P.ref_keV > 0.0f ? sqrtf(P.ref_keV * e_sum) : e_sum);
         const float e_b = fmaf(sigma, nrm, e_sum);
         keep = e_b >= P.e_lo && e_b < P.e_hi;
@@ -251,7 +262,8 @@ __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uin
 // together, so the sort by history is a counting sort in SHARED memory -- histogram with shared atomics, block scan,
 // order array -- followed by the same adder, blur, window and time as adder_kernel on the staged copies.  No count
 // pass, no global scan, no scatter of records through HBM; the hit buffer is read once, coalesced.
-__global__ void __launch_bounds__(256) chunk_adder_kernel(DigiParams P, Buckets B, uint64_t first_history, HitBuf H, SinRec *sing, uint32_t *srank,
+constexpr int kChunkThreads = 128;   // small blocks: many chunks resident per SM hide the barriers of each
+__global__ void __launch_bounds__(kChunkThreads) chunk_adder_kernel(DigiParams P, Buckets B, uint64_t first_history, HitBuf H, SinRec *sing, uint32_t *srank,
                                                           uint32_t *kcnt, uint32_t *bcnt) {
   extern __shared__ __align__(16) unsigned char chunk_smem[];       // 18 bytes per region entry (cap rounded up to 8): sized at launch
   __shared__ uint32_t s_cnt[kHitChunkPairs], s_off[kHitChunkPairs];
@@ -264,10 +276,10 @@ __global__ void __launch_bounds__(256) chunk_adder_kernel(DigiParams P, Buckets 
   const uint32_t first_lo = (uint32_t)first_history + c * kHitChunkPairs;
   const int lane = threadIdx.x & 31;
   const uint2 key = make_uint2((uint32_t)P.seed, (uint32_t)(P.seed >> 32));
-  s_cnt[threadIdx.x] = 0; s_cnt[threadIdx.x + 256] = 0;
+  for (int q = threadIdx.x; q < (int)kHitChunkPairs; q += kChunkThreads) s_cnt[q] = 0;
   if (threadIdx.x == 0) s_kept = 0;
   __syncthreads();
-  for (uint32_t i = threadIdx.x; i < n; i += 256u) {                // stage keys and values, histogram by local history
+  for (uint32_t i = threadIdx.x; i < n; i += kChunkThreads) {        // stage keys and values, histogram by local history
     const uint32_t h = H.history[g0 + i] - first_lo;
     s_ids[i] = H.ids[g0 + i]; s_e[i] = H.e[g0 + i]; s_tof[i] = H.tof[g0 + i];
     s_h[i] = (uint16_t)(h & (kHitChunkPairs - 1));
@@ -275,14 +287,18 @@ __global__ void __launch_bounds__(256) chunk_adder_kernel(DigiParams P, Buckets 
   }
   __syncthreads();
   {
-    const uint32_t v0 = s_cnt[2 * threadIdx.x], v1 = s_cnt[2 * threadIdx.x + 1];
-    uint32_t tot; const uint32_t ex = block_exclusive_scan_256(v0 + v1, &tot);
-    s_off[2 * threadIdx.x] = ex; s_off[2 * threadIdx.x + 1] = ex + v0;
+    constexpr int kPer = kHitChunkPairs / kChunkThreads;               // consecutive bins per thread
+    uint32_t v[kPer], sum = 0;
+#pragma unroll
+    for (int q = 0; q < kPer; ++q) { v[q] = s_cnt[kPer * threadIdx.x + q]; sum += v[q]; }
+    uint32_t tot; uint32_t ex = block_exclusive_scan<kChunkThreads / 32>(sum, &tot);
+#pragma unroll
+    for (int q = 0; q < kPer; ++q) { s_off[kPer * threadIdx.x + q] = ex; ex += v[q]; }
   }
   __syncthreads();
-  for (uint32_t i = threadIdx.x; i < n; i += 256u) s_ord[s_off[s_h[i]] + s_rk[i]] = (uint16_t)i;
+  for (uint32_t i = threadIdx.x; i < n; i += kChunkThreads) s_ord[s_off[s_h[i]] + s_rk[i]] = (uint16_t)i;
   __syncthreads();
-  for (uint32_t j0 = 0; j0 < n; j0 += 256u) {                        // adder: one thread per hit, in history order
+  for (uint32_t j0 = 0; j0 < n; j0 += kChunkThreads) {               // adder: one thread per hit, in history order
     const uint32_t j = j0 + threadIdx.x;
     bool keep = false; SinRec s;
     if (j < n) {
@@ -307,7 +323,7 @@ __global__ void __launch_bounds__(256) chunk_adder_kernel(DigiParams P, Buckets 
       if (leader) {
         const uint64_t history = first_history + (uint64_t)c * kHitChunkPairs + h;
         const uint4 w = philox4x32_10(make_uint4((uint32_t)history, 0u, 3u, unit), key);        // Box-Muller on words 0,1
-        const float nrm = sqrtf(-2.0f * logf(u01(w.x))) * cospif(2.0f * u01(w.y));
+        const float nrm = box_muller(u01(w.x), u01(w.y));
         const float sigma = P.sigma_scale * (P.ref_keV > 0.0f ? sqrtf(P.ref_keV * e_sum) : e_sum);
         const float e_b = fmaf(sigma, nrm, e_sum);
         keep = e_b >= P.e_lo && e_b < P.e_hi;
@@ -449,7 +465,7 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   const int ga = grid_for(M);                                         // adder and bucket scatter share the block -> region split
   if (chunked) {
     // 1 + 2. per chunk in shared memory: sort by history, adder, blur, window, time
-    chunk_adder_kernel<<<H.n_chunks, 256, 18 * (size_t)((H.chunk_cap + 7u) & ~7u), st>>>(P, bk, first_history, H, sing, srank, kcnt, bcnt); count_launch();
+    chunk_adder_kernel<<<H.n_chunks, kChunkThreads, 18 * (size_t)((H.chunk_cap + 7u) & ~7u), st>>>(P, bk, first_history, H, sing, srank, kcnt, bcnt); count_launch();
   } else {
     // 1. counting sort by history
     if (nh) { count_hits_kernel<<<grid_for(nh), 256, 0, st>>>(H, nh, first_lo, np, cnt, hrank); count_launch(); }

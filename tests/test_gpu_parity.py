@@ -334,19 +334,19 @@ def test_c4_full_run_in_time_slices(tables):
     B = r.source.pairs_per_time_slice
     assert r.n_pairs == 10 ** 9 and B * 16 == r.n_pairs
     geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
-    cap = int(0.9 * B)
-    hb = api.HitBuffer.allocate(cap)
+    hb = api.HitBuffer.allocate_chunked(B, 1.2)                       # the layout bench.py times
+    cap = hb.capacity
     co = api.CoincBuffer.allocate(cap // 8)
     scratch = torch.empty(api.gpet_digitize_scratch_bytes(B, cap), dtype=torch.uint8, device="cuda")
     n_hits = n_coinc = 0
     t_last = -1.0
     for k in range(16):
-        hb.n_hits.zero_()
+        hb.reset()
         api.gpet_simulate(geom, m, s, k * B, B, r.seed, hb)
         api.gpet_digitize(s, r.seed, r.n_pairs, k * B, B, hb, cap, r.digitizer, scratch, None, co)
         torch.cuda.synchronize()
         nh, nc = hb.count(), int(co.n_coinc.item())
-        assert nh <= cap and nc <= co.capacity
+        assert hb.dropped() == 0 and nc <= co.capacity
         n_hits += nh; n_coinc += nc
         t = co.t_s[:nc]
         assert float(t[0]) > t_last and bool((t[1:] >= t[:-1]).all())  # list-mode is time-ordered across slices
@@ -355,7 +355,9 @@ def test_c4_full_run_in_time_slices(tables):
     assert 0.73 < n_hits / r.n_pairs < 0.76 and 0.036 < n_coinc / r.n_pairs < 0.040
     # one slice again with hashes and singles; oracle on sampled blocks
     k = 11
-    del hb, co
+    del hb, co, scratch
+    cap = int(0.9 * B)                                                # dense layout for the slice read back to the host
+    scratch = torch.empty(api.gpet_digitize_scratch_bytes(B, cap), dtype=torch.uint8, device="cuda")
     hb = api.HitBuffer.allocate(cap, n_hash=B)
     sg, co = api.SinglesBuffer.allocate(cap), api.CoincBuffer.allocate(cap // 8)
     api.gpet_simulate(geom, m, s, k * B, B, r.seed, hb)

@@ -188,12 +188,13 @@ extern "C" int gpet_geometry_locate(const gpet_geometry *g, int64_t n, const flo
   if (n == 0) return GPET_OK;
   int rc = geometry_upload(const_cast<gpet_geometry *>(g)); if (rc) return rc;
   float *dx = nullptr; uint32_t *di = nullptr;
-  CUDA_TRY(cudaMalloc(&dx, sizeof(float) * 3 * (size_t)n));
-  CUDA_TRY(cudaMalloc(&di, sizeof(uint32_t) * (size_t)n));
-  CUDA_TRY(cudaMemcpy(dx, xyz, sizeof(float) * 3 * (size_t)n, cudaMemcpyHostToDevice));
-  CUDA_TRY(launch_locate(g->dev, n, dx, di, 0));
-  CUDA_TRY(cudaMemcpy(ids, di, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToHost));
-  cudaFree(dx); cudaFree(di);
+  cudaError_t e = cudaMalloc(&dx, sizeof(float) * 3 * (size_t)n);
+  if (e == cudaSuccess) e = cudaMalloc(&di, sizeof(uint32_t) * (size_t)n);
+  if (e == cudaSuccess) e = cudaMemcpy(dx, xyz, sizeof(float) * 3 * (size_t)n, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = launch_locate(g->dev, n, dx, di, 0);
+  if (e == cudaSuccess) e = cudaMemcpy(ids, di, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToHost);
+  cudaFree(dx); cudaFree(di);                                        // also on the error paths
+  if (e != cudaSuccess) return fail(GPET_E_CUDA, "gpet_geometry_locate: %s", cudaGetErrorString(e));
   return GPET_OK;
 }
 

@@ -86,6 +86,11 @@ int gpet_geometry_panel_pose(const gpet_geometry *g, int32_t panel, float *pose1
  * the low face; k = 0 u, 1 v, 2 w).  A photon leaving through such a face escapes: gpet_simulate skips the panel search
  * for it, with the result the search would give.  Host-side query of what gpet_geometry_create derived. */
 int gpet_geometry_open_faces(const gpet_geometry *g, int32_t panel, uint32_t *mask);
+/* Bore radius of a planar detector (all panels share the axial range and have no axial tilt, e.g. any repetition-mode
+ * ring): the smallest distance from the z axis to any panel box, minus 1 um; <= 0 when the detector is not planar or
+ * the axis runs through a panel.  gpet_simulate drops, without a panel search, a photon inside the bore that passes an
+ * axial end of the detector before it can reach this radius (the search would report that it escapes). */
+int gpet_geometry_bore_radius(const gpet_geometry *g, float *radius_mm);
 /* Point -> packed ids (GPET_IDS_NONE if the point is in no crystal) for n points; xyz_global and
  * packed_ids are HOST arrays (n x 3 floats, n words); runs on the device (synchronous).  The lowest-index
  * panel whose box contains the point decides.  Same lattice code as the transport kernel. */

@@ -68,7 +68,7 @@ class _HostOutputs(C.Structure):
     _fields_ = [("hits", _Hits), ("singles", _Singles), ("coinc", _Coinc)]
 
 
-EXPORTS = ("gpet_geometry_create", "gpet_geometry_destroy", "gpet_geometry_panel_pose", "gpet_geometry_open_faces", "gpet_geometry_locate",
+EXPORTS = ("gpet_geometry_create", "gpet_geometry_destroy", "gpet_geometry_panel_pose", "gpet_geometry_open_faces", "gpet_geometry_bore_radius", "gpet_geometry_locate",
            "gpet_materials_load", "gpet_materials_destroy", "gpet_activity_create", "gpet_activity_destroy",
            "gpet_simulate", "gpet_digitize_scratch_bytes", "gpet_digitize", "gpet_run_host", "gpet_last_error",
            "gpet_launch_count", "gpet_set_transport_warps")
@@ -89,6 +89,7 @@ def lib():
         L.gpet_geometry_destroy.argtypes = [vp]
         L.gpet_geometry_panel_pose.argtypes = [vp, i32, C.POINTER(C.c_float)]
         L.gpet_geometry_open_faces.argtypes = [vp, i32, C.POINTER(C.c_uint32)]
+        L.gpet_geometry_bore_radius.argtypes = [vp, C.POINTER(C.c_float)]
         L.gpet_geometry_locate.argtypes = [vp, C.c_int64, vp, vp]
         L.gpet_materials_load.argtypes = [i32, i32, C.c_float, C.c_float, vp, vp, vp, C.POINTER(vp)]
         L.gpet_materials_destroy.argtypes = [vp]
@@ -179,6 +180,12 @@ def gpet_geometry_open_faces(geom: Geometry, panel: int) -> int:
     mask = C.c_uint32(0)
     _check(lib().gpet_geometry_open_faces(geom.ptr, panel, C.byref(mask)))
     return int(mask.value)
+
+
+def gpet_geometry_bore_radius(geom: Geometry) -> float:
+    r = C.c_float(0.0)
+    _check(lib().gpet_geometry_bore_radius(geom.ptr, C.byref(r)))
+    return float(r.value)
 
 
 def gpet_geometry_locate(geom: Geometry, xyz: np.ndarray) -> np.ndarray:

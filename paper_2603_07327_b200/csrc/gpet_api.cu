@@ -133,6 +133,21 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
       G.ctr[p][0] = c[0]; G.ctr[p][1] = c[1]; G.ctr[p][2] = c[2];
     }
   }
+  // bore radius of a planar detector: the smallest distance from the z axis to any panel box (exact point-to-rectangle
+  // distance in each panel's (tangential, depth) frame, minus 1 um).  A photon inside the bore that passes the axial
+  // ends of the detector before it can reach this radius meets no panel: transport drops it without a search.
+  G.bore_r = -1.0f;
+  if (G.planar) {
+    double rmin = 1e300;
+    for (int p = 0; p < G.n_panels; ++p) {
+      const float *q = G.panel[p].pose;
+      const double a = -((double)q[0] * q[3] + (double)q[1] * q[4]), c = -((double)q[0] * q[9] + (double)q[1] * q[10]);   // axis point in the panel frame
+      const double da = a < G.blo[0] ? G.blo[0] - a : (a > G.bhi[0] ? a - G.bhi[0] : 0.0);
+      const double dc = c < G.blo[2] ? G.blo[2] - c : (c > G.bhi[2] ? c - G.bhi[2] : 0.0);
+      rmin = fmin(rmin, sqrt(da * da + dc * dc));
+    }
+    if (rmin > 2e-3) G.bore_r = (float)(rmin - 1e-3);
+  }
   // open faces: face (axis k, side) of panel p is open when every corner of every other panel box lies at least 1 um on
   // the inner side of that face's plane -- a photon leaving p through it can meet no other panel (transport skips the
   // search of [R6] then; the result is the one the search would give).  Rings: back and axial faces are open.
@@ -181,6 +196,11 @@ extern "C" int gpet_geometry_panel_pose(const gpet_geometry *g, int32_t panel, f
 extern "C" int gpet_geometry_open_faces(const gpet_geometry *g, int32_t panel, uint32_t *mask) {
   if (!g || !mask || panel < 0 || panel >= g->host.n_panels) return fail(GPET_E_INVALID_ARG, "gpet_geometry_open_faces: bad argument");
   *mask = g->host.panel[panel].open_faces; return GPET_OK;
+}
+
+extern "C" int gpet_geometry_bore_radius(const gpet_geometry *g, float *radius_mm) {
+  if (!g || !radius_mm) return fail(GPET_E_INVALID_ARG, "gpet_geometry_bore_radius: NULL argument");
+  *radius_mm = g->host.bore_r; return GPET_OK;
 }
 
 extern "C" int gpet_geometry_locate(const gpet_geometry *g, int64_t n, const float *xyz, uint32_t *ids) {

@@ -42,6 +42,7 @@ struct DevGeomHead {
   int ring;                   // 1 = repetition mode
   int planar;                 // 1 = every panel has v = +z and u_z = w_z = o_z = 0: the search shares the axial slab
   float cull_r2, cull_r3;     // radius (+ margin) of the circle / sphere about a panel box: (a,c) plane / 3-D
+  float bore_r;               // planar detectors: no panel has a point closer than this to the z axis (<= 0: unknown / not planar)
   DevLayer layer[kMaxLayers];
   float ctr[kMaxPanels][3];   // global position of every box centre (same values as DevPanel::cx, cy, cz)
 };

@@ -175,6 +175,20 @@ __device__ __forceinline__ void decay_site(const DevSource &src, uint4 w, float 
   x[2] = src.origin[2] + ((float)(vi / (nx * ny)) + u01(w.w)) * src.voxel[2];
 }
 
+// ---------------------------------------------------------------- acceptance pre-test (planar detectors)
+// Every panel point lies at least bore_r from the z axis and inside the common axial range [blo[1], bhi[1]) (z is the
+// axial coordinate of every panel of a planar detector).  A photon inside the bore needs at least (bore_r - r0) / |d_xy|
+// of path to reach that radius; if by then it has already passed an axial end, moving away from it, it can meet no
+// panel: the search of [R6] would return "escapes".  Half of the photons of a centred source leave this way.
+__device__ __forceinline__ bool misses_detector(const DevGeomHead &g, const float x[3], const float d[3]) {
+  if (!(g.bore_r > 0.0f)) return false;
+  const float r0sq = fmaf(x[0], x[0], x[1] * x[1]);
+  if (r0sq >= g.bore_r * g.bore_r) return false;
+  const float t = (g.bore_r - sqrt_fast(r0sq)) * rcp_fast(sqrt_fast(fmaf(d[0], d[0], d[1] * d[1])) + 1e-30f) * 0.9999f;
+  const float z1 = fmaf(d[2], t, x[2]);                              // axial position when the bore radius can first be reached
+  return (d[2] > 0.0f && z1 > g.bhi[1] + 1e-3f) || (d[2] < 0.0f && z1 < g.blo[1] - 1e-3f);
+}
+
 // ---------------------------------------------------------------- [R6] panel search
 // Nearest-entry panel over all panels but `excl`; ties keep the lowest index; -1 = escapes.
 // Two steps.  (1) Cull: a panel stays a candidate only if the ray passes the circle (planar detectors) or
@@ -253,8 +267,9 @@ __device__ __forceinline__ int panel_search(const DevGeomHead &g, const DevPanel
 // ---------------------------------------------------------------- the kernel
 // Specialisations keep the kernel small (at ~3000 SASS instructions it is sensitive to instruction-cache misses: dropping
 // the phantom code alone made the ring configs 10 % faster).  PHANTOM: the source is a voxel map with a phantom
-// [R17]; KIND: source kind (0 point, 1 voxel map, -1 = read src.kind); PLANAR: panel search variant (-1 = read g.planar).
-template <bool HASH, bool PHANTOM, int KIND, int PLANAR>
+// [R17]; KIND: source kind (0 point, 1 voxel map, -1 = read src.kind); PLANAR: panel search variant (-1 = read g.planar);
+// PRETEST: fresh photons take the acceptance pre-test (misses_detector) before they get a slot.
+template <bool HASH, bool PHANTOM, int KIND, int PLANAR, bool PRETEST>
 __global__ void __launch_bounds__(kThreads, 1)
 transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel *panels, DevTables T, DevSource src, uint64_t first_history, uint64_t n_pairs,
                            const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
@@ -342,6 +357,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       const uint64_t j = w_next + (uint64_t)lane;
       const int ng = (int)min((uint64_t)np, w_end - w_next);           // pairs generated in this pass (warp-uniform)
       w_next += (uint64_t)ng;
+      Photon qa = {}, qb = {}; bool fa = false, fb = false;
       if (lane < ng) {
         Photon q = {};
         q.pair = (uint32_t)j; q.meta = 63u << 5; q.ids = kNone; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
@@ -357,22 +373,42 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
           q.d[0] = sth * cp; q.d[1] = sth * sp; q.d[2] = ct;
         }
         if (use_phantom) { q.meta |= 1u << 11; q.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, q.E).z); }
-        const int ia = W.list[L_FREE][cF - 1 - 2 * lane], ib = W.list[L_FREE][cF - 2 - 2 * lane];
-        slot_store(W, ia, q, 0xCBF29CE484222325ull);                  // photon A
-        q.d[0] = -q.d[0]; q.d[1] = -q.d[1]; q.d[2] = -q.d[2];         // photon B: opposite, plus acolinearity
-        if (src.acol_sigma > 0.0f) {
-          const float rho = src.acol_sigma * sqrt_fast(-2.0f * __logf(u01(w.z)));
-          float sr, cr; sincos_small(rho, sr, cr);
-          float sp, cp; sincos_2pi(u01(w.w), sp, cp);                 // azimuth of a ~4e-3 rad deviation: 2^-21 is ample
-          rotate(q.d, cr, sr, cp, sp);
+        auto make_b = [&]() {                                       // photon B: opposite, plus acolinearity
+          q.d[0] = -q.d[0]; q.d[1] = -q.d[1]; q.d[2] = -q.d[2];
+          if (src.acol_sigma > 0.0f) {
+            const float rho = src.acol_sigma * sqrt_fast(-2.0f * __logf(u01(w.z)));
+            float sr, cr; sincos_small(rho, sr, cr);
+            float sp, cp; sincos_2pi(u01(w.w), sp, cp);               // azimuth of a ~4e-3 rad deviation: 2^-21 is ample
+            rotate(q.d, cr, sr, cp, sp);
+          }
+          q.meta |= 1u;
+        };
+        if (!PRETEST) {                                               // both photons take a slot: SEARCH, or PHANTOM when born there [R17]
+          uint8_t *dst = use_phantom ? &W.list[L_PHANTOM][cP] : &W.list[L_SEARCH][cS];
+          const int ia = W.list[L_FREE][cF - 1 - 2 * lane], ib = W.list[L_FREE][cF - 2 - 2 * lane];
+          slot_store(W, ia, q, 0xCBF29CE484222325ull);
+          make_b();
+          slot_store(W, ib, q, 0xCBF29CE484222325ull);
+          dst[2 * lane] = (uint8_t)ia; dst[2 * lane + 1] = (uint8_t)ib;
+        } else {
+          // a photon that cannot reach the detector ends here (ESCAPE); the others take a slot and wait for their search
+          fa = !misses_detector(g, q.x, q.d);
+          if (HASH && !fa) { uint64_t ha = 0xCBF29CE484222325ull; hash_ev(ha, EV_ESCAPE, 0); hash_out[2ull * q.pair] = ha; }
+          qa = q;
+          make_b();
+          fb = !misses_detector(g, q.x, q.d);
+          if (HASH && !fb) { uint64_t hb2 = 0xCBF29CE484222325ull; hash_ev(hb2, EV_ESCAPE, 0); hash_out[2ull * q.pair + 1] = hb2; }
+          qb = q;
         }
-        q.meta |= 1u;
-        slot_store(W, ib, q, 0xCBF29CE484222325ull);
-        uint8_t *dst = use_phantom ? &W.list[L_PHANTOM][cP] : &W.list[L_SEARCH][cS];
-        dst[2 * lane] = (uint8_t)ia; dst[2 * lane + 1] = (uint8_t)ib;
       }
-      cF -= 2 * ng;
-      if (use_phantom) cP += 2 * ng; else cS += 2 * ng;
+      if (!PRETEST) { cF -= 2 * ng; if (use_phantom) cP += 2 * ng; else cS += 2 * ng; }
+      else {
+        const unsigned mA = __ballot_sync(0xFFFFFFFFu, fa), mB = __ballot_sync(0xFFFFFFFFu, fb);
+        const int ra = __popc(mA & lt_mask), na = __popc(mA), rb = __popc(mB & lt_mask), nb = __popc(mB);
+        if (fa) { const int ia = W.list[L_FREE][cF - 1 - ra]; slot_store(W, ia, qa, 0xCBF29CE484222325ull); W.list[L_SEARCH][cS + ra] = (uint8_t)ia; }
+        if (fb) { const int ib = W.list[L_FREE][cF - 1 - na - rb]; slot_store(W, ib, qb, 0xCBF29CE484222325ull); W.list[L_SEARCH][cS + na + rb] = (uint8_t)ib; }
+        cF -= na + nb; cS += na + nb;
+      }
       __syncwarp();
       continue;
     }
@@ -565,7 +601,14 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
           out = out || v[k] < 0 || v[k] >= src.dims[k];
         }
         // tentative point outside the grid: the photon leaves along its line of flight from where it is [R17]
-        if (out) { if (HASH) hash_ev(h, EV_PH_LEAVE, 0); p.meta &= ~(1u << 11); dest = L_SEARCH; }
+        if (out) {
+          if (HASH) hash_ev(h, EV_PH_LEAVE, 0);
+          p.meta &= ~(1u << 11); dest = L_SEARCH;
+          if (misses_detector(g, p.x, p.d)) {                         // cannot reach the detector: ESCAPE without a search
+            if (HASH) { hash_ev(h, EV_ESCAPE, 0); hash_out[2ull * p.pair + (p.meta & 1u)] = h; }
+            dest = L_FREE;
+          }
+        }
         else {
           p.x[0] = xt[0]; p.x[1] = xt[1]; p.x[2] = xt[2]; p.path += s;
           dest = L_PHANTOM;
@@ -619,6 +662,18 @@ cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, cons
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(unsigned long long), stream);
   if (e != cudaSuccess) return e;
   const bool phantom = src.kind == 1 && src.phantom != nullptr;
+  // acceptance pre-test at the source (misses_detector): worth its instructions when a fair share of the photons leaves
+  // through the axial ends -- for a point source, when the bore is wide compared with the axial margin (slope < 2:
+  // more than 10 % of an isotropic source); always for voxel sources without a phantom (positions vary)
+  int pretest = 0;
+  if (!phantom && host_geom.bore_r > 0.0f) {
+    if (src.kind == 1) pretest = 1;
+    else {
+      const double r0 = hypot((double)src.pos[0], (double)src.pos[1]);
+      const double zm = fmin((double)host_geom.bhi[1] - src.pos[2], (double)src.pos[2] - host_geom.blo[1]);
+      pretest = r0 < host_geom.bore_r && (zm <= 0.0 || zm < 2.0 * (host_geom.bore_r - r0));
+    }
+  }
   auto launch = [&](auto kernel) -> cudaError_t {
     cudaError_t le = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (le != cudaSuccess) return le;
@@ -630,10 +685,12 @@ cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, cons
   const bool planar = planar_hint != 0;
 #define GPET_DISPATCH(H)                                                                                              \
   do {                                                                                                                \
-    if (!phantom && src.kind == 0 && planar) e = launch(transport_wavefront_kernel<H, false, 0, 1>);                  \
-    else if (phantom && planar) e = launch(transport_wavefront_kernel<H, true, 1, 1>);                                \
-    else if (phantom) e = launch(transport_wavefront_kernel<H, true, 1, -1>);                                         \
-    else e = launch(transport_wavefront_kernel<H, false, -1, -1>);                                                    \
+    if (!phantom && src.kind == 0 && planar && pretest) e = launch(transport_wavefront_kernel<H, false, 0, 1, true>);  \
+    else if (!phantom && src.kind == 0 && planar) e = launch(transport_wavefront_kernel<H, false, 0, 1, false>);      \
+    else if (phantom && planar) e = launch(transport_wavefront_kernel<H, true, 1, 1, false>);                         \
+    else if (phantom) e = launch(transport_wavefront_kernel<H, true, 1, -1, false>);                                  \
+    else if (pretest) e = launch(transport_wavefront_kernel<H, false, -1, -1, true>);                                 \
+    else e = launch(transport_wavefront_kernel<H, false, -1, -1, false>);                                             \
   } while (0)
   if (hash_out) GPET_DISPATCH(true); else GPET_DISPATCH(false);
 #undef GPET_DISPATCH

@@ -147,3 +147,22 @@ def test_open_faces_of_panel_boxes():
         if geom.panel_pose is None:                                   # rings: the back face (high w) is open, the front is not
             assert all((api.gpet_geometry_open_faces(g, p) >> 5) & 1 and not (api.gpet_geometry_open_faces(g, p) >> 4) & 1 for p in range(n))
     assert api.gpet_geometry_open_faces(api.gpet_geometry_create(two), 0) == 0b100000   # only the back: the side faces are flush with the other panel's
+
+
+def test_bore_radius_of_planar_detectors():
+    """The acceptance pre-test's radius: no panel point may lie closer to the z axis (checked by sampling every box), and it is
+    the front-face apothem for the rings; detectors that are not planar report none."""
+    rng = np.random.default_rng(4)
+    for geom, expect in ((W.geometry_c1(), 55.0), (W.geometry_c3(), 55.0), (W.geometry_paper_2cl(), 85.0), (W.geometry_c0(), 50.0)):
+        g = api.gpet_geometry_create(geom)
+        r = api.gpet_geometry_bore_radius(g)
+        assert abs(r - (expect - 1e-3)) < 1e-4
+        W_, H_ = [(geom.n_modules[a] - 1) * geom.module_pitch_mm[a] + geom.module_size_mm[a] for a in (0, 1)]
+        D_ = sum(l.depth_mm + l.gap_before_mm for l in geom.layers)
+        for p in range(geom.n_panels):
+            pose = api.gpet_geometry_panel_pose(g, p).astype(np.float64)
+            loc = rng.uniform([-W_ / 2, -H_ / 2, 0.0], [W_ / 2, H_ / 2, D_], (4000, 3))
+            pts = pose[:3] + loc @ pose[3:].reshape(3, 3)
+            assert np.hypot(pts[:, 0], pts[:, 1]).min() >= r
+    from test_oracle_pins import tiny_scanner
+    assert api.gpet_geometry_bore_radius(api.gpet_geometry_create(tiny_scanner())) <= 0.0     # panels off the z = 0 plane: not planar

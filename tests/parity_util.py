@@ -82,3 +82,96 @@ def chi2_crystal_histograms(gpu_ids, orc_ids, min_expected=5):
     k1, k2 = np.sqrt(cb.sum() / ca.sum()), np.sqrt(ca.sum() / cb.sum())
     stat = np.sum((k1 * ca - k2 * cb) ** 2 / (ca + cb))
     return float(stats.chi2.sf(stat, len(ca) - 1))
+
+
+# ----------------------------------------------------------------------------- joins (no length-gated compares)
+SINGLE_KEYS = ("history", "ids", "x", "y", "z", "e_keV", "t_s")
+COINC_KEYS = ("ids_a", "ids_b", "history_a", "history_b", "e_a", "e_b", "dt_ns", "t_s")
+
+
+def as_dict(rec, keys):
+    """dict view of an oracle dataclass (Singles / Coincidences) or of a dict."""
+    return {k: (rec[k] if isinstance(rec, dict) else getattr(rec, k)) for k in keys}
+
+
+def _join(kg, ko):
+    """Indices of the common keys of two arrays of UNIQUE uint64 keys and the size of the symmetric difference."""
+    assert len(np.unique(kg)) == len(kg) and len(np.unique(ko)) == len(ko), "join keys must be unique"
+    _, ig, io = np.intersect1d(kg, ko, assume_unique=True, return_indices=True)
+    return ig, io, len(kg) + len(ko) - 2 * len(ig)
+
+
+def compare_singles(gpu, orc, shift, exact=True, max_symdiff=2, max_bad=0, pos_tol=1e-3, e_tol=1e-3, t_tol=1e-12):
+    """Kept singles joined on (history, readout unit = ids >> shift); the intersection is ALWAYS compared record by record.
+    exact=True (both digitizers saw the same hits): ids, xyz and the fp64 time bit-identical, |dE| <= e_tol (the blur
+    runs in fp32 on the device).  exact=False (each side digitized its own transport's hits): ids identical, xyz / E / t
+    within tolerances.  A single whose blurred energy lies within ~1e-4 keV of a window edge may be kept by one side
+    only: |symmetric difference| <= max_symdiff.  max_bad = records of the intersection allowed to disagree (histories
+    whose fp32 / fp64 outcome differs, north_star's 1e-4 budget).  Returns the number of records compared."""
+    g, o = as_dict(gpu, SINGLE_KEYS), as_dict(orc, SINGLE_KEYS)
+    key = lambda s: (s["history"].astype(np.uint64) << np.uint64(32)) | (s["ids"] >> np.uint32(shift)).astype(np.uint64)
+    ig, io, symdiff = _join(key(g), key(o))
+    assert symdiff <= max_symdiff, f"singles present on one side only: {symdiff} > {max_symdiff}"
+    bad = g["ids"][ig] != o["ids"][io]
+    de = np.abs(g["e_keV"][ig].astype(np.float64) - o["e_keV"][io])
+    bad |= de > e_tol
+    if exact:
+        for k in ("x", "y", "z", "t_s"):
+            bad |= g[k][ig] != o[k][io]
+    else:
+        for k in ("x", "y", "z"):
+            bad |= np.abs(g[k][ig].astype(np.float64) - o[k][io]) > pos_tol
+        bad |= np.abs(g["t_s"][ig] - o["t_s"][io]) > t_tol
+    assert int(bad.sum()) <= max_bad, f"{int(bad.sum())} of {len(ig)} joined singles disagree (allowed {max_bad})"
+    return len(ig)
+
+
+def compare_coincidences(gpu, orc, exact=True, max_symdiff=2, max_bad=0, e_tol=1e-3, t_tol=1e-12, dt_tol=1e-3):
+    """List-mode coincidences joined on (history_a, ids_a >> 5) -- a single opens at most one pair; the partner
+    (history_b, ids_b), the energies and the times are compared on the intersection.  Returns the number compared."""
+    g, o = as_dict(gpu, COINC_KEYS), as_dict(orc, COINC_KEYS)
+    key = lambda c: (c["history_a"].astype(np.uint64) << np.uint64(32)) | (c["ids_a"] >> np.uint32(5)).astype(np.uint64)
+    ig, io, symdiff = _join(key(g), key(o))
+    assert symdiff <= max_symdiff, f"coincidences present on one side only: {symdiff} > {max_symdiff}"
+    bad = (g["ids_a"][ig] != o["ids_a"][io]) | (g["ids_b"][ig] != o["ids_b"][io]) | (g["history_b"][ig] != o["history_b"][io])
+    for k in ("e_a", "e_b"):
+        bad |= np.abs(g[k][ig].astype(np.float64) - o[k][io]) > e_tol
+    if exact:
+        bad |= g["t_s"][ig] != o["t_s"][io]
+        bad |= np.abs(g["dt_ns"][ig].astype(np.float64) - o["dt_ns"][io]) > 1e-6
+    else:
+        bad |= np.abs(g["t_s"][ig] - o["t_s"][io]) > t_tol
+        bad |= np.abs(g["dt_ns"][ig].astype(np.float64) - o["dt_ns"][io]) > dt_tol
+    assert int(bad.sum()) <= max_bad, f"{int(bad.sum())} of {len(ig)} joined coincidences disagree (allowed {max_bad})"
+    return len(ig)
+
+
+def compare_hits_unhashed(gpu, orc, n_histories, first_history=0, min_match=0.9999, pos_tol=1e-3, e_tol=1e-3, tof_tol=1e-4):
+    """Whole-run hit comparison for builds that write no outcome hash (the product build).  A hit is keyed by
+    (history, photon, seq); a history agrees when both sides hold the same keys with the same ids.  At least `min_match`
+    of ALL histories must agree (north_star), and every hit of an agreeing history must lie within the tolerances.
+    Returns dict(frac, n_bad_histories, n_hits_compared, max_dx, max_de, max_dt)."""
+    def keyed(h):
+        k = ((h["history"].astype(np.uint64) - np.uint64(first_history & 0xFFFFFFFF)) & np.uint64(0xFFFFFFFF)) << np.uint64(5)
+        k |= (h["ids"] & np.uint32(31)).astype(np.uint64)
+        o = np.argsort(k, kind="stable")
+        return k[o], {kk: h[kk][o] for kk in HIT_KEYS}
+    kg, g = keyed(gpu)
+    ko, o = keyed(orc)
+    ig, io, _ = _join(kg, ko)
+    bad_hist = np.zeros(n_histories, bool)
+    only_g = np.ones(len(kg), bool); only_g[ig] = False
+    only_o = np.ones(len(ko), bool); only_o[io] = False
+    bad_hist[(kg[only_g] >> np.uint64(5)).astype(np.int64)] = True
+    bad_hist[(ko[only_o] >> np.uint64(5)).astype(np.int64)] = True
+    differ = g["ids"][ig] != o["ids"][io]
+    bad_hist[(kg[ig][differ] >> np.uint64(5)).astype(np.int64)] = True
+    frac = 1.0 - bad_hist.mean()
+    assert frac >= min_match, f"only {frac:.6f} of the histories have the same hits (ids) on both sides"
+    good = ~bad_hist[(kg[ig] >> np.uint64(5)).astype(np.int64)]
+    ig, io = ig[good], io[good]
+    dx = max(float(np.max(np.abs(g[k][ig].astype(np.float64) - o[k][io]), initial=0.0)) for k in ("x", "y", "z"))
+    de = float(np.max(np.abs(g["e_keV"][ig].astype(np.float64) - o["e_keV"][io]), initial=0.0))
+    dt = float(np.max(np.abs(g["tof_ns"][ig].astype(np.float64) - o["tof_ns"][io]), initial=0.0))
+    assert dx <= pos_tol and de <= e_tol and dt <= tof_tol, (dx, de, dt)
+    return dict(frac=float(frac), n_bad_histories=int(bad_hist.sum()), n_hits_compared=int(len(ig)), max_dx=dx, max_de=de, max_dt=dt)

@@ -24,7 +24,7 @@ TOF_TOL = 1e-4              # ns  (= 0.03 mm of path; fp32 path sums differ by ~
 def run_both(run, tables, n=None, first=0):
     n = n or run.n_pairs
     g, gh, cnt = PU.gpu_simulate(run, tables, n_pairs=n, first_history=first)
-    o = O.simulate(run.geometry, tables, run.source, n, run.seed, first_history=first, want_hash=True, threads=8)
+    o = O.simulate(run.geometry, tables, run.source, n, run.seed, first_history=first, want_hash=True, threads=16)
     return g, gh, cnt, o
 
 
@@ -150,13 +150,14 @@ def test_deterministic_rays_index_bit_exact(tables):
 
 
 # ----------------------------------------------------------------------------- digitizer
-@pytest.mark.parametrize("level", [0, 1, 2])
-def test_digitizer_equals_oracle_on_oracle_hits(tables, level):
-    """Same hits in (oracle-made, shuffled) -> singles and coincidences must be identical records."""
+@pytest.mark.parametrize("level,ref_keV", [(0, 511.0), (1, 511.0), (2, 511.0), (1, 0.0)])
+def test_digitizer_equals_oracle_on_oracle_hits(tables, level, ref_keV):
+    """Same hits in (oracle-made, shuffled) -> singles and coincidences must be identical records, at the three readout
+    levels and with the constant-fraction blur (blur_ref_keV = 0 [R25])."""
     n = 300_001
     src = W.source_point((10.0, 0.0, 4.0), activity_bq=5.0e7)         # hot enough for randoms and multiples
     o = O.simulate(W.geometry_c3(), tables, src, n, 404, first_history=1000, threads=8)
-    dig = W.Digitizer(0.15, 511.0, 350.0, 650.0, 4.0, level)
+    dig = W.Digitizer(0.15, ref_keV, 350.0, 650.0, 4.0, level)
     osg, oco, _ = O.digitize(src, 404, 10 * n, o.hits, dig)
     perm = np.random.default_rng(2).permutation(len(o.hits))
     hb = PU.upload_hits(PU.oracle_hits_dict(o.hits), perm)
@@ -166,16 +167,14 @@ def test_digitizer_equals_oracle_on_oracle_hits(tables, level):
     api.gpet_digitize(s, 404, 10 * n, 1000, n, hb, len(o.hits), dig, scratch, sg, co)
     torch.cuda.synchronize()
     gs, gc = sg.to_numpy(), co.to_numpy()
-    # energies are blurred in fp32 on the device: a single within ~1e-4 keV of a window edge may flip
-    assert abs(len(gs["ids"]) - len(osg.ids)) <= 2
-    if len(gs["ids"]) == len(osg.ids):
-        assert np.array_equal(gs["ids"], osg.ids) and np.array_equal(gs["history"], osg.history)
-        assert np.array_equal(gs["t_s"], osg.t_s)                     # fp64 times are bit-identical
-        assert np.max(np.abs(gs["e_keV"] - osg.e_keV)) < E_TOL
-        assert all(np.array_equal(gs[k], getattr(osg, k)) for k in ("x", "y", "z"))
-        assert np.array_equal(gc["ids_a"], oco.ids_a) and np.array_equal(gc["ids_b"], oco.ids_b)
-        assert np.array_equal(gc["history_a"], oco.history_a) and np.array_equal(gc["history_b"], oco.history_b)
-        assert np.array_equal(gc["t_s"], oco.t_s) and np.max(np.abs(gc["dt_ns"] - oco.dt_ns)) < 1e-6
+    # Same hits in: every record of the join on (history, unit) is compared -- ids, xyz and the fp64 time bit for bit,
+    # |dE| <= 1e-3 keV (the blur runs in fp32 on the device: a single within ~1e-4 keV of a window edge may be kept by
+    # one side only, hence a symmetric difference of at most 2 singles, each of which can make or break one pair).
+    shift = (5, 20, 26)[level]
+    n_cmp = PU.compare_singles(gs, osg, shift, exact=True, max_symdiff=2)
+    assert n_cmp >= len(osg.ids) - 2 and n_cmp > 90_000
+    n_cmp = PU.compare_coincidences(gc, oco, exact=True, max_symdiff=4)
+    assert n_cmp >= len(oco.ids_a) - 4
     assert len(oco.ids_a) > 5000 and np.sum(oco.history_a != oco.history_b) > 50
     assert np.all(np.diff(gs["t_s"]) >= 0)
 
@@ -240,36 +239,60 @@ def test_run_host_matches_device_path(tables):
 
 
 # ----------------------------------------------------------------------------- full size, bench launch configuration
-def full_size_sampled(run, tables, hits_per_pair, n_blocks=24, block=4096):
-    """A config at its full size in the configuration bench.py times; the oracle recomputes random blocks of
-    histories (it can start anywhere: draws are keyed by history id).  Returns the GPU hits (buffer order)."""
+def gpu_product_run(run, tables, hits_per_pair, n=None):
+    """The PRODUCT build (no outcome hashes, 128 slots per warp, chunked hit layout -- what bench.py times): transport +
+    digitizer of one batch.  Returns (hits, singles, coincidences) as numpy dicts and the device time of the two calls."""
+    n = n or run.n_pairs
     geom, m, s = api.gpet_geometry_create(run.geometry), api.gpet_materials_load(tables), api.DeviceSource(run.source)
-    hb = api.HitBuffer.allocate(int(hits_per_pair * run.n_pairs), n_hash=run.n_pairs)
-    api.gpet_simulate(geom, m, s, 0, run.n_pairs, run.seed, hb)
-    torch.cuda.synchronize()
-    assert hb.count() <= hb.capacity
-    gh = hb.outcome_hash.cpu().numpy().view(np.uint64).reshape(-1, 2)
-    g = hb.to_numpy()
-    rng = np.random.default_rng(5)
-    starts = np.concatenate([[0, run.n_pairs - block], rng.integers(0, run.n_pairs - block, n_blocks - 2)])
-    same = tot = 0
-    for st in starts:
-        o = O.simulate(run.geometry, tables, run.source, block, run.seed, first_history=int(st), want_hash=True, threads=4)
-        ok = np.all(gh[st:st + block] == o.outcome_hash, axis=1)
-        same += int(ok.sum()); tot += block
-        sel = (g["history"] >= st) & (g["history"] < st + block)
-        part = PU.canonical({k: v[sel] for k, v in g.items()})
-        PU.compare_hits(part, PU.oracle_hits_dict(o.hits), gh[st:st + block], o.outcome_hash, first_history=int(st),
-                        pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
-    assert same / tot >= MIN_MATCH, (same, tot)
-    return g, hb.count()
+    hb = api.HitBuffer.allocate_chunked(n, hits_per_pair)
+    cap = hb.capacity
+    sg, co = api.SinglesBuffer.allocate(cap), api.CoincBuffer.allocate(cap // 4)
+    scratch = torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda")
+    st = torch.cuda.current_stream()
+    best = float("inf")
+    for rep in range(2):                                              # the second pass is the timed one
+        hb.reset()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(st)
+        api.gpet_simulate(geom, m, s, 0, n, run.seed, hb, st)
+        api.gpet_digitize(s, run.seed, n, 0, n, hb, cap, run.digitizer, scratch, sg, co, st)
+        b.record(st)
+        torch.cuda.synchronize()
+        best = min(best, a.elapsed_time(b))
+    assert hb.dropped() == 0, "hit buffer overflow in test"
+    assert int(co.n_coinc.item()) <= co.capacity
+    return hb.to_numpy(), sg.to_numpy(), co.to_numpy(), best
 
 
-def test_c1_full_size_sampled_histories(tables):
-    """configs[1] at its full 1e7 pairs + properties that hold at any size."""
+def whole_run_against_oracle(run, tables, hits_per_pair):
+    """One config position at its FULL size through the product build, next to the oracle's whole run: hits of every
+    history, then singles and coincidences (each side digitizes its own hits).  Budgets: north_star's 1e-4 of the
+    histories may differ in their discrete outcome (fp32 vs fp64 decisions); the records of those histories may differ or
+    be missing on one side, so the joins allow 1e-4 of each list (+ 2 for window-edge flips of the blur)."""
+    n = run.n_pairs
+    g, gs, gc, ms = gpu_product_run(run, tables, hits_per_pair)
+    o = O.simulate(run.geometry, tables, run.source, n, run.seed, threads=16)
+    res = PU.compare_hits_unhashed(g, PU.oracle_hits_dict(o.hits), n, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= MIN_MATCH and res["n_hits_compared"] >= (1.0 - 5e-4) * len(o.hits), res
+    assert PU.chi2_crystal_histograms(g["ids"], o.hits.ids) > 0.01
+    osg, oco, _ = O.digitize(run.source, run.seed, n, o.hits, run.digitizer)
+    bs, bc = int(1e-4 * len(osg.ids)) + 2, int(1e-4 * len(oco.ids_a)) + 2
+    ns = PU.compare_singles(gs, osg, 20, exact=False, max_symdiff=bs, max_bad=bs)
+    nc = PU.compare_coincidences(gc, oco, exact=False, max_symdiff=bc, max_bad=bc)
+    assert ns >= len(osg.ids) - bs and nc >= len(oco.ids_a) - bc and nc > 100_000
+    assert np.all(np.diff(gs["t_s"]) >= 0) and np.all(np.diff(gc["t_s"]) >= 0)
+    res.update(n_hits=len(g["ids"]), n_singles_compared=ns, n_coinc_compared=nc, ms=ms, pairs_per_s=n / (ms * 1e-3))
+    return g, o, res
+
+
+def test_c1_full_size_hash_build_whole_run(tables):
+    """configs[1] at its full 1e7 pairs through the parity (hash) build: the outcome hash of EVERY history next to the
+    oracle's, every hit of the agreeing histories within tolerance, + properties that hold at any size."""
     r = W.config_runs("C1")[0]
-    g, nh = full_size_sampled(r, tables, 1.2)
-    assert 0.76 < nh / r.n_pairs < 0.79                               # SURVEY 8(a): 0.77 hits per pair
+    g, gh, cnt, o = run_both(r, tables)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= MIN_MATCH and res["n_hits_compared"] > 7_600_000, res
+    assert 0.76 < cnt / r.n_pairs < 0.79                              # SURVEY 8(a): 0.77 hits per pair
     counts = np.bincount(g["ids"] >> 26, minlength=12)
     from scipy import stats
     assert stats.chisquare(counts).pvalue > 1e-4                      # centred source: every panel equally hit
@@ -277,52 +300,41 @@ def test_c1_full_size_sampled_histories(tables):
     assert abs(up - down) < 5 * np.sqrt(up + down)                    # axial symmetry
 
 
-def test_c1_full_size_digitizer_sampled_histories(tables):
-    """The digitizer at configs[1]'s full size, scratch and buffers sized as bench.py sizes them: the singles of sampled
-    history blocks (they depend on no other history [R24]) equal the oracle's records, the singles are time-ordered, and
-    every coincidence is a window-mate pair of consecutive singles on different panels [R27]."""
+def test_c1_full_size_product_build_whole_run(tables):
+    """configs[1] at 1e7 pairs in the launch configuration bench.py times (product build, chunked hits, scratch and
+    buffers sized the same way): all hits, singles and coincidences next to the oracle's whole run."""
     r = W.config_runs("C1")[0]
-    n = r.n_pairs
-    geom, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
-    hb = api.HitBuffer.allocate_chunked(n, 1.2)                       # bench.py's hit buffer: chunked layout, 1.2 hits per pair
-    cap = hb.capacity
-    sg, co = api.SinglesBuffer.allocate(cap), api.CoincBuffer.allocate(cap // 4)
-    scratch = torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda")
-    api.gpet_simulate(geom, m, s, 0, n, r.seed, hb)
-    api.gpet_digitize(s, r.seed, n, 0, n, hb, cap, r.digitizer, scratch, sg, co)
-    torch.cuda.synchronize()
-    assert hb.dropped() == 0
-    gs, gc = sg.to_numpy(), co.to_numpy()
-    assert 0.32 < len(gs["ids"]) / n < 0.35 and 0.055 < len(gc["ids_a"]) / n < 0.060
-    assert np.all(np.diff(gs["t_s"]) >= 0)
-    rng = np.random.default_rng(11)
-    for st in np.concatenate([[0, n - 4096], rng.integers(0, n - 4096, 10)]):
-        o = O.simulate(r.geometry, tables, r.source, 4096, r.seed, first_history=int(st), threads=4)
-        osg, _, _ = O.digitize(r.source, r.seed, n, o.hits, r.digitizer)
-        sel = (gs["history"] >= st) & (gs["history"] < st + 4096)
-        assert abs(int(sel.sum()) - len(osg.ids)) <= 1               # one of the ~1e-5 mismatching histories, or a window-edge flip
-        if int(sel.sum()) == len(osg.ids):
-            assert np.array_equal(gs["history"][sel], osg.history) and np.array_equal(gs["ids"][sel] >> 5, osg.ids >> 5)
-            assert np.max(np.abs(gs["t_s"][sel] - osg.t_s)) < 1e-12 and np.max(np.abs(gs["e_keV"][sel] - osg.e_keV)) < E_TOL
-    # every coincidence: two consecutive singles within the window, on different panels, and no third single in the window
-    pos = np.searchsorted(gs["t_s"], gc["t_s"])
-    idx = np.arange(len(gs["t_s"]))
-    key = gs["history"].astype(np.uint64) << np.uint64(32) | gs["ids"].astype(np.uint64)
-    a = np.array([p if key[p] == (np.uint64(h) << np.uint64(32) | np.uint64(i)) else p + 1 for p, h, i in
-                  zip(pos[:2000], gc["history_a"][:2000], gc["ids_a"][:2000])])
-    assert np.array_equal(gs["ids"][a], gc["ids_a"][:2000]) and np.array_equal(gs["ids"][a + 1], gc["ids_b"][:2000])
-    tau = r.digitizer.window_ns * 1e-9
-    assert np.all(gs["t_s"][a + 1] - gs["t_s"][a] < tau) and np.all((gs["ids"][a] >> 26) != (gs["ids"][a + 1] >> 26))
-    assert np.all(gs["t_s"][a + 2] - gs["t_s"][a] >= tau)
+    g, o, res = whole_run_against_oracle(r, tables, 1.2)
+    print("C1 whole run:", res)
+    assert 0.32 < res["n_singles_compared"] / r.n_pairs < 0.35 and 0.055 < res["n_coinc_compared"] / r.n_pairs < 0.060
 
 
-@pytest.mark.parametrize("cfg,idx,lo,hi", [("C2", 4, 1.38, 1.48), ("C3", 21, 1.19, 1.29)])
-def test_c2_c3_full_size_sampled_histories(tables, cfg, idx, lo, hi):
-    """configs[2] (x = 50 mm) and configs[3] (x = 50 mm, z = 16 mm) at 1e7 pairs: the positions with the most hits."""
+SWEEP = [("C2", i) for i in range(5)] + [("C3", i) for i in range(22)]
+SWEEP_RATE = {}
+
+
+@pytest.mark.parametrize("cfg,idx", SWEEP)
+def test_c2_c3_every_position_at_full_size(tables, cfg, idx):
+    """BASELINE.json configs[2] (5 radial offsets) and configs[3] (11 radial x 2 axial offsets): EVERY position at its
+    full 1e7 pairs through the product build -- hits, singles and coincidences against the oracle's whole run,
+    per-layer ids present, per-crystal chi-square."""
     r = W.config_runs(cfg)[idx]
-    g, nh = full_size_sampled(r, tables, 2.0, n_blocks=16)
-    assert lo < nh / r.n_pairs < hi
-    assert ((g["ids"] >> 18) & 3).max() == 1                          # both layers recorded (PAPER.md:37)
+    g, o, res = whole_run_against_oracle(r, tables, 2.0)
+    SWEEP_RATE[(cfg, idx)] = res["pairs_per_s"]
+    print(f"{r.name}: {res}")
+    assert ((g["ids"] >> 18) & 3).max() == 1 and ((o.hits.ids >> 18) & 3).max() == 1   # both layers recorded (PAPER.md:37)
+    assert 0.70 < res["n_hits"] / r.n_pairs < 1.50
+
+
+def test_sweep_rates_are_reported(tables):
+    """pairs/s of every sweep position (transport + digitizer, product build).  Off-centre positions produce up to 1.9 x
+    the hits of the centred one, so they are not expected to run at the centred rate; the 10 % bar of north_star is for
+    the three layer configurations at the same position (test_layer_configurations_run_within_ten_percent)."""
+    if not SWEEP_RATE:
+        pytest.skip("sweep did not run in this session")
+    for k in sorted(SWEEP_RATE):
+        print(k, f"{SWEEP_RATE[k]:.3e} pairs/s")
+    assert min(SWEEP_RATE.values()) > 1e9
 
 
 def test_c4_full_run_in_time_slices(tables):
@@ -366,7 +378,7 @@ def test_c4_full_run_in_time_slices(tables):
     gh = hb.outcome_hash.cpu().numpy().view(np.uint64).reshape(-1, 2)
     g, gs = hb.to_numpy(), sg.to_numpy()
     rng = np.random.default_rng(6)
-    same = tot = 0
+    same = tot = n_singles_cmp = 0
     for st in np.concatenate([[0, B - 2048], rng.integers(0, B - 2048, 10)]):
         first = k * B + int(st)
         o = O.simulate(r.geometry, tables, r.source, 2048, r.seed, first_history=first, want_hash=True, threads=4)
@@ -379,11 +391,11 @@ def test_c4_full_run_in_time_slices(tables):
         if ok.all():                                                  # same hits in -> the same singles out
             osg, _, _ = O.digitize(r.source, r.seed, r.n_pairs, o.hits, r.digitizer)
             ss = (gs["history"] >= first) & (gs["history"] < first + 2048)
-            assert abs(int(ss.sum()) - len(osg.ids)) <= 1            # a blurred energy within 1e-4 keV of a window edge may flip
-            if int(ss.sum()) == len(osg.ids):
-                assert np.array_equal(gs["ids"][ss], osg.ids) and np.array_equal(gs["t_s"][ss], osg.t_s)
-                assert np.max(np.abs(gs["e_keV"][ss] - osg.e_keV)) < E_TOL
-    assert same / tot >= MIN_MATCH
+            # joined on (history, module): always compared; a blurred energy within 1e-4 keV of a window edge may flip one
+            n_cmp = PU.compare_singles({kk: v[ss] for kk, v in gs.items()}, osg, 20, exact=False, max_symdiff=1)
+            assert n_cmp >= len(osg.ids) - 1
+            n_singles_cmp += n_cmp
+    assert same / tot >= MIN_MATCH and n_singles_cmp > 3000
 
 
 # ----------------------------------------------------------------------------- north_star: layers cost nothing
@@ -600,3 +612,57 @@ def test_chunked_hit_layout_equals_the_dense_one(tables, cfg, idx, n):
     torch.cuda.synchronize()
     assert tight.count() == dense.count() and tight.dropped() > 0
     assert tight.dropped() == dense.count() - int(np.minimum(tight.chunk_fill[:-1].cpu().numpy(), 128).sum())
+
+
+# ----------------------------------------------------------------------------- branches no config reaches (VERDICT r1 weak #2)
+def test_weighted_activity_map_parity(tables):
+    """[R13] decay sites from a map with unequal activities (integer weights, `first cumulative weight above the target`
+    search): outcome hashes and hits against the oracle on C1's ring, and voxel populations in proportion."""
+    rng = np.random.default_rng(3)
+    dims = (24, 20, 16)
+    act = rng.choice(np.array([0.0, 0.05, 0.3, 1.0], np.float32), size=(dims[2], dims[1], dims[0]), p=[0.4, 0.2, 0.2, 0.2])
+    src = W.Source(1, (0, 0, 0), 0.5, 1e6, 0, act, None, -1, dims, (0.5, 0.25, 1.0), (-6.0, -2.5, -8.0))
+    r = W.Run("weighted", W.geometry_c1(), src, 300_001, 88)
+    g, gh, cnt, o = run_both(r, tables)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= MIN_MATCH and cnt > 200_000, res
+
+
+def test_phantom_rayleigh_parity_and_thomson_distribution(tables):
+    """[R17, R20] Rayleigh scattering inside the phantom (no config's water has mu_R > 0): hash parity with the oracle in
+    a thick medium (several deflections per photon), and in a thin one the single deflections of the CUDA path's own
+    photons follow the Thomson distribution (the same check that pins the oracle)."""
+    from test_oracle_pins import phantom_rayleigh_setup, single_rayleigh_deflections, check_thomson
+    geom, t, src = phantom_rayleigh_setup(mu_r=4.0)
+    r = W.Run("ph_rayleigh", geom, src, 300_001, 12)
+    g, gh, cnt, o = run_both(r, t)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= MIN_MATCH and cnt == 2 * r.n_pairs, res      # closed absorber: every photon is caught
+    geom, t, src = phantom_rayleigh_setup()
+    r = W.Run("ph_rayleigh_thin", geom, src, 2_000_000, 12)
+    g, gh, cnt = PU.gpu_simulate(r, t)
+    check_thomson(*single_rayleigh_deflections(g, gh, r.n_pairs))
+
+
+def test_panel_search_tie_goes_to_the_lowest_index(tables):
+    """[R6] diagonal rays of a square ring reach two overlapping front faces at bit-identical distances: the CUDA path
+    must enter the lower-index panel, as the oracle does (pinned on the CPU by exact arithmetic)."""
+    from test_oracle_pins import square_ring, const_tables
+    geom, t = square_ring(), const_tables(5.0, 0.0, 0.0)
+    s2 = float(np.float32(1.0 / np.sqrt(2.0)))
+    for d, want_a, want_b in (((s2, s2, 0), 0, 2), ((s2, -s2, 0), 0, 1), ((-s2, s2, 0), 1, 0), ((-s2, -s2, 0), 2, 0)):
+        r = W.Run("tie", geom, W.source_beam((0.0, 0.0, 0.0), d), 2000, 5)
+        g, gh, cnt, o = run_both(r, t)
+        assert np.array_equal(gh, o.outcome_hash) and np.array_equal(g["ids"], o.hits.ids) and cnt == 2 * r.n_pairs
+        pa = g["ids"][(g["ids"] >> 4) & 1 == 0] >> 26
+        pb = g["ids"][(g["ids"] >> 4) & 1 == 1] >> 26
+        assert np.all(pa == want_a) and np.all(pb == want_b), (d, np.unique(pa), np.unique(pb))
+
+
+def test_ring_handedness_against_hand_written_numbers(tables):
+    """[R5] the same hand-written (point -> ids) table that pins the oracle's ring placement, through gpet_geometry_locate."""
+    g = api.gpet_geometry_create(W.geometry_c1())
+    pack = lambda panel, mx, my, ix, iy: (panel << 26) | ((mx + 2 * my) << 20) | ((ix + 16 * iy) << 5)
+    pts = np.array([[56.0, 3.5, 0.5], [56.0, -3.5, 0.5], [56.0, 0.5, -20.5], [-3.5, 56.0, 0.5], [3.5, 56.0, 0.5], [-56.0, -3.5, 0.5]], np.float32)
+    want = [pack(0, 1, 2, 3, 0), pack(0, 0, 2, 12, 0), pack(0, 1, 0, 0, 11), pack(3, 1, 2, 3, 0), pack(3, 0, 2, 12, 0), pack(6, 1, 2, 3, 0)]
+    assert list(api.gpet_geometry_locate(g, pts)) == want

@@ -48,23 +48,40 @@ def upload_hits(hits: dict, order=None) -> "api.HitBuffer":
     return hb
 
 
+POS_CAP = 2e-2   # mm: no hit of a history with the oracle's outcome hash may be further off than this (see compare_hits)
+
+
 def compare_hits(gpu: dict, orc: dict, gpu_hash, orc_hash, first_history=0, pos_tol=1e-3, e_tol=1e-3, tof_tol=1e-4):
-    """Per-history comparison.  Returns dict(n_histories, n_match, frac, max_dx, max_de, max_dt).
-    Histories whose outcome hash agrees must have identical ids and agree within the tolerances."""
+    """Per-history comparison against the oracle (north_star: >= 99.99 % of the histories with an identical discrete
+    outcome, and for those positions within 1e-3 mm and energies within 1e-3 keV).
+
+    A history AGREES when its two outcome hashes equal the oracle's AND every one of its hits lies within the tolerances;
+    `frac` is the share of agreeing histories and is what the 99.99 % bar is applied to.  Histories with equal hashes must
+    hold identical ids (asserted).  The continuous values of a hash-matching history are allowed a tail: a photon that
+    scatters in one panel and enters the next at grazing incidence turns a transverse fp32 rounding of ~5e-6 mm into
+    (5e-6 / cos of the incidence angle) along its line of flight -- measured 2.4e-3 mm at most in 1e7 pairs of C1
+    (DESIGN.md 7).  Such a history counts AGAINST the 99.99 %; none may be off by more than POS_CAP, energies and
+    times of hash-matching histories stay within their tolerances without exception."""
     n = len(orc_hash)
     same = np.all(np.asarray(gpu_hash).reshape(-1, 2) == np.asarray(orc_hash).reshape(-1, 2), axis=1)
-    ok_g = same[(gpu["history"] - np.uint32(first_history)).astype(np.int64)]
-    ok_o = same[(orc["history"] - np.uint32(first_history)).astype(np.int64)]
+    hg = (gpu["history"] - np.uint32(first_history)).astype(np.int64)
+    ho = (orc["history"] - np.uint32(first_history)).astype(np.int64)
+    ok_g, ok_o = same[hg], same[ho]
     g = {k: v[ok_g] for k, v in gpu.items()}
     o = {k: v[ok_o] for k, v in orc.items()}
     assert len(g["ids"]) == len(o["ids"]), "matching histories must hold the same number of hits"
     assert np.array_equal(g["history"], o["history"]) and np.array_equal(g["ids"], o["ids"])
-    dx = max(float(np.max(np.abs(g[k].astype(np.float64) - o[k]), initial=0.0)) for k in ("x", "y", "z"))
+    dxs = np.maximum.reduce([np.abs(g[k].astype(np.float64) - o[k]) for k in ("x", "y", "z")]) if len(g["ids"]) else np.zeros(0)
+    dx = float(np.max(dxs, initial=0.0))
     de = float(np.max(np.abs(g["e_keV"].astype(np.float64) - o["e_keV"]), initial=0.0))
     dt = float(np.max(np.abs(g["tof_ns"].astype(np.float64) - o["tof_ns"]), initial=0.0))
-    assert dx <= pos_tol and de <= e_tol and dt <= tof_tol, (dx, de, dt)
-    return dict(n_histories=n, n_match=int(same.sum()), frac=float(same.mean()), n_hits_compared=int(len(g["ids"])),
-                max_dx=dx, max_de=de, max_dt=dt)
+    assert dx <= POS_CAP and de <= e_tol and dt <= tof_tol, (dx, de, dt)
+    off = dxs > pos_tol
+    agree = same.copy()
+    agree[hg[ok_g][off]] = False
+    return dict(n_histories=n, n_match=int(agree.sum()), frac=float(agree.mean()), frac_hash=float(same.mean()),
+                n_hits_compared=int(len(g["ids"])), n_hits_beyond_tol=int(off.sum()), max_dx=dx, max_de=de, max_dt=dt,
+                dx_q999=float(np.quantile(dxs, 0.999)) if len(dxs) else 0.0, dx_q99999=float(np.quantile(dxs, 0.99999)) if len(dxs) else 0.0)
 
 
 def chi2_crystal_histograms(gpu_ids, orc_ids, min_expected=5):
@@ -148,9 +165,10 @@ def compare_coincidences(gpu, orc, exact=True, max_symdiff=2, max_bad=0, e_tol=1
 
 def compare_hits_unhashed(gpu, orc, n_histories, first_history=0, min_match=0.9999, pos_tol=1e-3, e_tol=1e-3, tof_tol=1e-4):
     """Whole-run hit comparison for builds that write no outcome hash (the product build).  A hit is keyed by
-    (history, photon, seq); a history agrees when both sides hold the same keys with the same ids.  At least `min_match`
-    of ALL histories must agree (north_star), and every hit of an agreeing history must lie within the tolerances.
-    Returns dict(frac, n_bad_histories, n_hits_compared, max_dx, max_de, max_dt)."""
+    (history, photon, seq); a history AGREES when both sides hold the same keys with the same ids and every hit lies
+    within the tolerances (a flipped accept / reject can leave the ids unchanged, so without hashes the continuous values
+    are part of the verdict).  At least `min_match` of ALL histories must agree (north_star).
+    Returns dict(frac, n_bad_histories, n_hits_compared, max_dx, max_de, max_dt over the agreeing histories)."""
     def keyed(h):
         k = ((h["history"].astype(np.uint64) - np.uint64(first_history & 0xFFFFFFFF)) & np.uint64(0xFFFFFFFF)) << np.uint64(5)
         k |= (h["ids"] & np.uint32(31)).astype(np.uint64)
@@ -164,14 +182,15 @@ def compare_hits_unhashed(gpu, orc, n_histories, first_history=0, min_match=0.99
     only_o = np.ones(len(ko), bool); only_o[io] = False
     bad_hist[(kg[only_g] >> np.uint64(5)).astype(np.int64)] = True
     bad_hist[(ko[only_o] >> np.uint64(5)).astype(np.int64)] = True
-    differ = g["ids"][ig] != o["ids"][io]
-    bad_hist[(kg[ig][differ] >> np.uint64(5)).astype(np.int64)] = True
+    hist = (kg[ig] >> np.uint64(5)).astype(np.int64)
+    dxs = np.maximum.reduce([np.abs(g[k][ig].astype(np.float64) - o[k][io]) for k in ("x", "y", "z")])
+    des = np.abs(g["e_keV"][ig].astype(np.float64) - o["e_keV"][io])
+    dts = np.abs(g["tof_ns"][ig].astype(np.float64) - o["tof_ns"][io])
+    differ = (g["ids"][ig] != o["ids"][io]) | (dxs > pos_tol) | (des > e_tol) | (dts > tof_tol)
+    bad_hist[hist[differ]] = True
     frac = 1.0 - bad_hist.mean()
-    assert frac >= min_match, f"only {frac:.6f} of the histories have the same hits (ids) on both sides"
-    good = ~bad_hist[(kg[ig] >> np.uint64(5)).astype(np.int64)]
-    ig, io = ig[good], io[good]
-    dx = max(float(np.max(np.abs(g[k][ig].astype(np.float64) - o[k][io]), initial=0.0)) for k in ("x", "y", "z"))
-    de = float(np.max(np.abs(g["e_keV"][ig].astype(np.float64) - o["e_keV"][io]), initial=0.0))
-    dt = float(np.max(np.abs(g["tof_ns"][ig].astype(np.float64) - o["tof_ns"][io]), initial=0.0))
-    assert dx <= pos_tol and de <= e_tol and dt <= tof_tol, (dx, de, dt)
-    return dict(frac=float(frac), n_bad_histories=int(bad_hist.sum()), n_hits_compared=int(len(ig)), max_dx=dx, max_de=de, max_dt=dt)
+    assert frac >= min_match, f"only {frac:.6f} of the histories agree (same hits within tolerance on both sides)"
+    good = ~bad_hist[hist]
+    return dict(frac=float(frac), n_bad_histories=int(bad_hist.sum()), n_hits_compared=int(good.sum()),
+                max_dx=float(np.max(dxs[good], initial=0.0)), max_de=float(np.max(des[good], initial=0.0)),
+                max_dt=float(np.max(dts[good], initial=0.0)))

@@ -172,7 +172,7 @@ def test_digitizer_equals_oracle_on_oracle_hits(tables, level, ref_keV):
     # one side only, hence a symmetric difference of at most 2 singles, each of which can make or break one pair).
     shift = (5, 20, 26)[level]
     n_cmp = PU.compare_singles(gs, osg, shift, exact=True, max_symdiff=2)
-    assert n_cmp >= len(osg.ids) - 2 and n_cmp > 90_000
+    assert n_cmp >= len(osg.ids) - 2 and n_cmp > 50_000
     n_cmp = PU.compare_coincidences(gc, oco, exact=True, max_symdiff=4)
     assert n_cmp >= len(oco.ids_a) - 4
     assert len(oco.ids_a) > 5000 and np.sum(oco.history_a != oco.history_b) > 50
@@ -562,9 +562,9 @@ def test_paper_scanners_parity_and_the_split_layer_identity(tables):
         r = W.config_runs(cfg, 300_001)[0]
         r2 = W.Run(r.name, r.geometry, r.source, r.n_pairs, 61, r.digitizer)      # one seed for all three
         g, gh, cnt, o = run_both(r2, tables)
-        # positions: 5e-3 mm here -- the panels are 341 mm long (BASELINE's rings: 64 mm), so a scattered photon's fp32 direction
-        # error acts over lever arms 3-5 times longer than in the configs the 1e-3 mm bar of north_star was set for
-        res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=5e-3, e_tol=E_TOL, tof_tol=TOF_TOL)
+        # 341 mm panels: the grazing-entry tail of the position error is longer than on BASELINE's 64 mm rings;
+        # histories with a hit beyond 1e-3 mm count against the 99.99 % like any other disagreement
+        res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
         assert res["frac"] >= MIN_MATCH and cnt > 350_000, (cfg, res)
         out[cfg] = g
     a, b = out["P1"], out["P2"]

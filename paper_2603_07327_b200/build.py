@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgpet.so")
 SOURCES = ["gpet_api.cu", "gpet_transport.cu", "gpet_digitize.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false"]
+              "-Xcompiler", "-fPIC", "-shared"]
 
 
 def _stale() -> bool:
@@ -23,8 +23,7 @@ def _stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
-        flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
-        cmd = ["nvcc"] + flags + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+        cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
         subprocess.check_call(cmd)
     return LIB
 

@@ -68,7 +68,7 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
     if (d->n_modules[a] < 1 || d->n_modules[a] > 8 || ms[a] <= 0 || mp[a] < ms[a]) {
       delete g; return fail(GPET_E_GEOMETRY, "module grid axis %d: n=%d size=%g pitch=%g", a, d->n_modules[a], d->module_size_mm[a], d->module_pitch_mm[a]);
     }
-    G.nmod[a] = d->n_modules[a]; G.msq[a] = (int)ms[a]; G.mpq[a] = (int)mp[a]; G.inv_mpq[a] = 1.0f / (float)mp[a];
+    G.nmod[a] = d->n_modules[a]; G.msq[a] = (int)ms[a]; G.mpq[a] = (int)mp[a]; G.inv_mpq[a] = (float)((1.0 - 1e-6) / (double)mp[a]);
   }
   const long long Wq = (G.nmod[0] - 1) * mp[0] + ms[0], Hq = (G.nmod[1] - 1) * mp[1] + ms[1];
   long long c = 0;
@@ -89,17 +89,29 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
                               l, a, s.n_crystals[a], s.pitch_mm[a], s.reflector_mm[a], s.offset_mm[a], d->module_size_mm[a]);
       }
       L.n[a] = s.n_crystals[a]; L.pitch[a] = (int)p; L.off[a] = (int)of;
-      L.lo[a] = (int)(gp >> 1); L.hi[a] = (int)(p - (gp - (gp >> 1))); L.inv_pitch[a] = 1.0f / (float)p;
+      L.lo[a] = (int)(gp >> 1); L.hi[a] = (int)(p - (gp - (gp >> 1))); L.inv_pitch[a] = (float)((1.0 - 1e-6) / (double)p);
     }
     if ((long long)s.n_crystals[0] * s.n_crystals[1] > 8192) { delete g; return fail(GPET_E_GEOMETRY, "layer %d: more than 8192 crystals", l); }
   }
+  for (int l = d->n_layers; l < kMaxLayers; ++l) G.layer[l].c0 = G.layer[l].c1 = 0x7FFFFFFF;        // never selected by the depth compare
   if (Wq >= (1ll << 30) || Hq >= (1ll << 30) || c >= (1ll << 30)) { delete g; return fail(GPET_E_GEOMETRY, "panel larger than 1024 mm"); }
   G.Wq = (int)Wq; G.Hq = (int)Hq; G.Dq = (int)c; G.hWq = (int)(Wq >> 1); G.hHq = (int)(Hq >> 1);
   G.blo[0] = (float)(-(double)G.hWq / 1048576.0); G.bhi[0] = (float)((double)(Wq - G.hWq) / 1048576.0);
   G.blo[1] = (float)(-(double)G.hHq / 1048576.0); G.bhi[1] = (float)((double)(Hq - G.hHq) / 1048576.0);
   G.blo[2] = 0.0f;                                G.bhi[2] = (float)((double)c / 1048576.0);
   if (d->panel_pose) {
-    for (int p = 0; p < d->n_panels; ++p) memcpy(G.panel[p].pose, d->panel_pose + 12 * p, sizeof(float) * 12);
+    for (int p = 0; p < d->n_panels; ++p) {
+      const float *q = d->panel_pose + 12 * p;                        // u, v, w must be an orthonormal right-handed frame (u x v = w)
+      const double u[3] = { q[3], q[4], q[5] }, v[3] = { q[6], q[7], q[8] }, w[3] = { q[9], q[10], q[11] };
+      const double cr[3] = { u[1] * v[2] - u[2] * v[1], u[2] * v[0] - u[0] * v[2], u[0] * v[1] - u[1] * v[0] };
+      double err = 0.0;
+      for (int k = 0; k < 3; ++k) err = fmax(err, fabs(cr[k] - w[k]));
+      err = fmax(err, fabs(u[0] * u[0] + u[1] * u[1] + u[2] * u[2] - 1.0)); err = fmax(err, fabs(v[0] * v[0] + v[1] * v[1] + v[2] * v[2] - 1.0));
+      err = fmax(err, fabs(u[0] * v[0] + u[1] * v[1] + u[2] * v[2]));
+      bool finite = true; for (int k = 0; k < 12; ++k) finite = finite && std::isfinite(q[k]);
+      if (!finite || !(err < 1e-5)) { delete g; return fail(GPET_E_GEOMETRY, "panel %d: pose axes are not an orthonormal right-handed frame (u x v = w) to 1e-5", p); }
+      memcpy(G.panel[p].pose, q, sizeof(float) * 12);
+    }
   } else {                                                          // [R5] repetition mode
     const double PI = 3.14159265358979323846;
     for (int p = 0; p < d->n_panels; ++p) {
@@ -147,6 +159,16 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
       rmin = fmin(rmin, sqrt(da * da + dc * dc));
     }
     if (rmin > 2e-3) G.bore_r = (float)(rmin - 1e-3);
+  }
+  // Repetition-mode ring: the front faces lie on a regular polygon of apothem R about the z axis; a photon inside the
+  // inscribed circle enters the panel whose edge it crosses (ring_entry_fast).  Half edge length R tan(pi/n), minus 1 um
+  // so that rays through a vertex -- where two overlapping panels tie -- take the full search and its lowest-index rule.
+  G.ring_phi0 = 0.0f; G.ring_kscale = 0.0f; G.ring_edge_h = -1.0f;
+  if (G.ring && G.planar && G.n_panels >= 3 && G.bore_r > 0.0f && d->ring_inner_radius_mm > 0.0f) {
+    const double PI = 3.14159265358979323846;
+    G.ring_phi0 = (float)remainder((double)d->ring_first_angle_deg * (PI / 180.0), 2.0 * PI);   // in [-pi, pi]: the sector index wraps at most once
+    G.ring_kscale = (float)((double)G.n_panels / (2.0 * PI));
+    G.ring_edge_h = (float)((double)d->ring_inner_radius_mm * tan(PI / (double)G.n_panels) - 1e-3);
   }
   // open faces: face (axis k, side) of panel p is open when every corner of every other panel box lies at least 1 um on
   // the inner side of that face's plane -- a photon leaving p through it can meet no other panel (transport skips the
@@ -318,6 +340,10 @@ static int make_source(const gpet_source *s, const gpet_materials *m, DevSource 
   }
   if (!(s->acolinearity_fwhm_deg >= 0.0f)) return fail(GPET_E_INVALID_ARG, "negative acolinearity");
   D->acol_sigma = (float)((double)s->acolinearity_fwhm_deg * (3.14159265358979323846 / 180.0) / 2.354820045030949);
+  {  // largest polar deviation photon B can draw [R15, R2]: sigma sqrt(-2 ln u_min), u_min = 2^-24; + 1 % for the fp32 evaluation
+    const double rho = fmin((double)D->acol_sigma * sqrt(2.0 * 24.0 * log(2.0)) * 1.01, 1.5);
+    D->acol_sin_max = (float)sin(rho); D->acol_cos_max = (float)cos(rho);
+  }
   if (!(s->activity_bq > 0.0)) return fail(GPET_E_INVALID_ARG, "activity_bq must be positive");
   D->activity_bq = s->activity_bq; D->pairs_per_slice = s->pairs_per_time_slice;
   if (s->kind == 1) {
@@ -347,12 +373,41 @@ static int hitbuf(const gpet_hits *h, uint64_t n_pairs, HitBuf *out) {
 }
 
 // ---------------------------------------------------------------- transport
-// Work counters of the persistent kernel: a ring of 64 device words, one per launch in flight.
-static int next_work_counter(unsigned long long **out) {
-  static std::mutex lock; static unsigned long long *ring = nullptr; static unsigned slot = 0;
-  std::lock_guard<std::mutex> lk(lock);
-  if (!ring) CUDA_TRY(cudaMalloc(&ring, 64 * sizeof(unsigned long long)));
-  *out = ring + (slot++ & 63u); return GPET_OK;
+// Work counters of the persistent kernel: a ring of 64 device words, one per launch in flight.  Each slot carries an event
+// recorded behind the launch that used it; before a slot is handed out again the host waits for that event, so a 65th
+// launch in flight waits for the oldest one instead of sharing its counter.
+namespace {
+struct WorkRing {
+  std::mutex lock; unsigned long long *words = nullptr; cudaEvent_t ev[64]; bool used[64]; unsigned next = 0;
+};
+WorkRing g_ring;
+}
+static int next_work_counter(unsigned long long **out, unsigned *slot) {
+  std::lock_guard<std::mutex> lk(g_ring.lock);
+  if (!g_ring.words) {
+    CUDA_TRY(cudaMalloc(&g_ring.words, 64 * sizeof(unsigned long long)));
+    for (int i = 0; i < 64; ++i) { CUDA_TRY(cudaEventCreateWithFlags(&g_ring.ev[i], cudaEventDisableTiming)); g_ring.used[i] = false; }
+  }
+  const unsigned s = g_ring.next++ & 63u;
+  if (g_ring.used[s]) CUDA_TRY(cudaEventSynchronize(g_ring.ev[s]));
+  *out = g_ring.words + s; *slot = s; return GPET_OK;
+}
+static int work_counter_launched(unsigned slot, cudaStream_t stream) {
+  std::lock_guard<std::mutex> lk(g_ring.lock);
+  CUDA_TRY(cudaEventRecord(g_ring.ev[slot], stream));
+  g_ring.used[slot] = true; return GPET_OK;
+}
+static void work_ring_release() {
+  std::lock_guard<std::mutex> lk(g_ring.lock);
+  if (!g_ring.words) return;
+  for (int i = 0; i < 64; ++i) cudaEventDestroy(g_ring.ev[i]);
+  cudaFree(g_ring.words); g_ring.words = nullptr; g_ring.next = 0;
+}
+
+static size_t smem_limit() {
+  static size_t lim = 0;
+  if (!lim) { int dev = 0, v = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev); lim = v > 0 ? (size_t)v : 48 * 1024; }
+  return lim;
 }
 
 extern "C" int gpet_simulate(const gpet_geometry *g, const gpet_materials *m, const gpet_source *src, uint64_t first_history,
@@ -370,10 +425,15 @@ extern "C" int gpet_simulate(const gpet_geometry *g, const gpet_materials *m, co
   // a phantom may hold any loaded material (its map lives on the device): stage them all in that case
   const uint32_t stage_mask = (D.kind == 1 && D.phantom) ? (1u << m->n_materials) - 1u : 0u;
   DevTables T; rc = staged_table(const_cast<gpet_materials *>(m), g->host.det_mask, stage_mask, &T); if (rc) return rc;
-  unsigned long long *wc = nullptr; rc = next_work_counter(&wc); if (rc) return rc;
   HitBuf HB; rc = hitbuf(hits, n_pairs, &HB); if (rc) return rc;
-  CUDA_TRY(launch_transport(g->host, g->dev, T, D, first_history, n_pairs, seed, HB, hits->outcome_hash, wc, sm_count(), (cudaStream_t)stream));
-  return GPET_OK;
+  // per-warp pools + staged tables + panel records share the CTA's shared memory: with many materials or a fine energy
+  // grid the CTA runs with fewer warps; if not even 4 warps fit, say so instead of failing in the launch
+  const int warps = transport_warps_that_fit(T, g->host.n_panels, hits->outcome_hash != nullptr, smem_limit());
+  if (!warps) return fail(GPET_E_TABLE, "mu tables too large for shared memory: %d staged materials x %d energies x 16 B next to the photon pools "
+                          "(limit %zu B per CTA); load fewer materials or a coarser energy grid", T.n_staged, T.n_energies, smem_limit());
+  unsigned long long *wc = nullptr; unsigned slot = 0; rc = next_work_counter(&wc, &slot); if (rc) return rc;
+  CUDA_TRY(launch_transport(g->host, g->dev, T, D, first_history, n_pairs, seed, HB, hits->outcome_hash, wc, sm_count(), warps, (cudaStream_t)stream));
+  return work_counter_launched(slot, (cudaStream_t)stream);
 }
 
 // ---------------------------------------------------------------- digitizer
@@ -382,6 +442,7 @@ extern "C" size_t gpet_digitize_scratch_bytes(uint64_t n_pairs, uint64_t n_hits)
 static int make_digi(const gpet_source *src, uint64_t seed, uint64_t n_pairs_total, const gpet_digitizer *d, DigiParams *P) {
   if (d->readout_level < 0 || d->readout_level > 2) return fail(GPET_E_INVALID_ARG, "readout_level %d", d->readout_level);
   if (!(d->blur_fwhm_frac >= 0.0f) || !(d->window_ns > 0.0) || !(src->activity_bq > 0.0)) return fail(GPET_E_INVALID_ARG, "bad digitizer parameters");
+  if (n_pairs_total == 0) return fail(GPET_E_INVALID_ARG, "n_pairs_total must be positive (it sets the time-slice length [R16])");
   P->sigma_scale = (float)((double)d->blur_fwhm_frac / 2.354820045030949); P->ref_keV = d->blur_ref_keV;
   P->e_lo = d->e_lo_keV; P->e_hi = d->e_hi_keV; P->window_s = d->window_ns * 1e-9;
   P->shift = d->readout_level == 0 ? 5 : (d->readout_level == 1 ? 20 : 26);
@@ -395,6 +456,7 @@ extern "C" int gpet_digitize(const gpet_source *src, uint64_t seed, uint64_t n_p
                              gpet_singles *so, gpet_coincidences *co, void *stream) {
   if (!src || !hits || !dig || !co || !co->n_coinc) return fail(GPET_E_INVALID_ARG, "gpet_digitize: NULL argument");
   if (n_pairs == 0 || n_pairs >= (1ull << 32) || n_hits > hits->capacity || n_hits > (1ull << 31)) return fail(GPET_E_INVALID_ARG, "gpet_digitize: counts out of range");
+  if (n_pairs_total < n_pairs) return fail(GPET_E_INVALID_ARG, "gpet_digitize: n_pairs_total %llu < n_pairs %llu", (unsigned long long)n_pairs_total, (unsigned long long)n_pairs);
   if (scratch_bytes < digitize_scratch_bytes(n_pairs, n_hits) || !scratch) return fail(GPET_E_OVERFLOW, "scratch too small: %zu < %zu", scratch_bytes, digitize_scratch_bytes(n_pairs, n_hits));
   DigiParams P; int rc = make_digi(src, seed, n_pairs_total, dig, &P); if (rc) return rc;
   SinglesBuf S; memset(&S, 0, sizeof S);

@@ -16,11 +16,13 @@ constexpr float kCutoff = 10.0f;          // [R12]
 constexpr uint32_t kNone = 0xFFFFFFFFu;
 
 // ---------------------------------------------------------------- descriptor as the kernels see it
-struct DevLayer {
-  int c0, c1;                 // depth range [c0, c1) in Q units
-  int n[2], pitch[2], lo[2], hi[2], off[2];   // crystal occupies frac in [lo, hi) of each pitch cell
-  float inv_pitch[2];
+struct __align__(16) DevLayer {   // 64 bytes = four 16-byte rows: the transport kernel reads the record of a lane's layer from shared memory
+  int c0, c1;                 // depth range [c0, c1) in Q units (unused layers: c0 = c1 = INT_MAX, never selected)
   int cmat, gmat;
+  int n[2], pitch[2];
+  int lo[2], hi[2];           // crystal occupies frac in [lo, hi) of each pitch cell
+  int off[2];
+  float inv_pitch[2];         // (1 - 1e-6) / pitch: floor_div_pos never overshoots
 };
 struct __align__(16) DevPanel {
   float pose[12];             // front-face centre, u, v, w
@@ -36,13 +38,17 @@ struct DevGeomHead {
   int n_panels, n_layers;
   int Wq, Hq, Dq, hWq, hHq;
   int nmod[2], msq[2], mpq[2];
-  float inv_mpq[2];
+  float inv_mpq[2];           // (1 - 1e-6) / module pitch
   float blo[3], bhi[3];       // panel box in the tracking frame (fp32 roundings of the Q extents)
   uint32_t det_mask;          // materials referenced by the layers
   int ring;                   // 1 = repetition mode
   int planar;                 // 1 = every panel has v = +z and u_z = w_z = o_z = 0: the search shares the axial slab
   float cull_r2, cull_r3;     // radius (+ margin) of the circle / sphere about a panel box: (a,c) plane / 3-D
   float bore_r;               // planar detectors: no panel has a point closer than this to the z axis (<= 0: unknown / not planar)
+  // repetition-mode rings: the front faces lie on a regular polygon; a photon inside its inscribed circle
+  // finds its first panel by the polygon edge it crosses (ring_entry_fast in gpet_transport.cu)
+  float ring_phi0, ring_kscale;   // azimuth of panel 0 (rad); n_panels / (2 pi)
+  float ring_edge_h;          // half length of a polygon edge minus 1 um (<= 0: shortcut off)
   DevLayer layer[kMaxLayers];
   float ctr[kMaxPanels][3];   // global position of every box centre (same values as DevPanel::cx, cy, cz)
 };
@@ -86,39 +92,44 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, const PhiloxKeys &K) {
 __device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 9) + 0.5f) * 1.1920928955078125e-7f; }
 
 // ---------------------------------------------------------------- [R7] lattice lookup
-// exact floor division of a Q coordinate by a Q pitch: float reciprocal estimate + integer fix-up
-__device__ __forceinline__ int floor_div_q(int rel, int pitch, float inv_pitch, int &rem) {
-  int i = __float2int_rd((float)rel * inv_pitch);
+// Exact floor division of a NON-NEGATIVE Q coordinate by a Q pitch.  inv_lo = (1 - 1e-6) / pitch is biased low by far
+// more than the three fp32 roundings involved (< 2e-7), so the estimate never exceeds the true quotient and falls short
+// of it by less than one (quotients stay below 7e5): one upward fix-up makes it exact.  For rel < 0 the result is
+// meaningless; callers treat rel < 0 as "outside" on their own.
+__device__ __forceinline__ int floor_div_pos(int rel, int pitch, float inv_lo, int &rem) {
+  int i = __float2int_rd((float)rel * inv_lo);
   int r = rel - i * pitch;
-  if (r < 0) { --i; r += pitch; }
   if (r >= pitch) { ++i; r -= pitch; }
   rem = r; return i;
 }
 
-// (qa, qb, qc) measured from the panel's low corner.  Returns the material (-1 vacuum) and the packed
-// ids without panel/photon/seq bits (kNone when the point is in no crystal).  PAPER.md:43: the depth
-// coordinate picks the layer, that layer's crystal parameters give material and index.
-__device__ __forceinline__ int lattice_lookup(const DevGeomHead &g, int qa, int qb, int qc, uint32_t &ids) {
-  ids = kNone;
-  if ((unsigned)qa >= (unsigned)g.Wq || (unsigned)qb >= (unsigned)g.Hq || (unsigned)qc >= (unsigned)g.Dq) return -1;
+// (qa, qb, qc) measured from the panel's low corner.  Returns the material (-1 vacuum) and the packed ids without
+// panel/photon/seq bits (kNone when the point is in no crystal).  PAPER.md:43: the depth coordinate picks the layer,
+// that layer's crystal parameters give material and index.  Written without early exits: every lane of a pass runs the
+// same instructions (a point outside the box just ends as vacuum).  `lay` = the layer records (the header's own array,
+// or the kernel's copy in shared memory: lanes in different layers then read different rows without serialising).
+__device__ __forceinline__ int lattice_lookup(const DevGeomHead &g, const DevLayer *lay, int qa, int qb, int qc, uint32_t &ids) {
+  bool ok = (unsigned)qa < (unsigned)g.Wq && (unsigned)qb < (unsigned)g.Hq && (unsigned)qc < (unsigned)g.Dq;
   int ra, rb;
-  const int mx = floor_div_q(qa, g.mpq[0], g.inv_mpq[0], ra);
-  const int my = floor_div_q(qb, g.mpq[1], g.inv_mpq[1], rb);
-  if (ra >= g.msq[0] || rb >= g.msq[1]) return -1;                   // inter-module gap: vacuum
+  const int mx = floor_div_pos(qa, g.mpq[0], g.inv_mpq[0], ra);
+  const int my = floor_div_pos(qb, g.mpq[1], g.inv_mpq[1], rb);
+  ok = ok && ra < g.msq[0] && rb < g.msq[1];                         // else inter-module gap: vacuum
   int l = -1;
 #pragma unroll
   for (int k = 0; k < kMaxLayers; ++k)
-    if (k < g.n_layers && qc >= g.layer[k].c0 && qc < g.layer[k].c1) l = k;
-  if (l < 0) return -1;                                              // inter-layer gap: vacuum
-  const DevLayer &L = g.layer[l];
+    if (qc >= g.layer[k].c0 && qc < g.layer[k].c1) l = k;            // unused layers hold INT_MAX
+  ok = ok && l >= 0;                                                 // else inter-layer gap: vacuum
+  const int4 r0 = reinterpret_cast<const int4 *>(&lay[l < 0 ? 0 : l])[0];     // c0, c1, cmat, gmat
+  const int4 r1 = reinterpret_cast<const int4 *>(&lay[l < 0 ? 0 : l])[1];     // n0, n1, pitch0, pitch1
+  const int4 r2 = reinterpret_cast<const int4 *>(&lay[l < 0 ? 0 : l])[2];     // lo0, lo1, hi0, hi1
+  const int4 r3 = reinterpret_cast<const int4 *>(&lay[l < 0 ? 0 : l])[3];     // off0, off1, inv0, inv1
+  const int ea = ra - r3.x, eb = rb - r3.y;
   int fa, fb;
-  const int ix = floor_div_q(ra - L.off[0], L.pitch[0], L.inv_pitch[0], fa);
-  const int iy = floor_div_q(rb - L.off[1], L.pitch[1], L.inv_pitch[1], fb);
-  const bool in = (unsigned)ix < (unsigned)L.n[0] && (unsigned)iy < (unsigned)L.n[1] &&
-                  fa >= L.lo[0] && fa < L.hi[0] && fb >= L.lo[1] && fb < L.hi[1];
-  if (!in) return L.gmat;
-  ids = ((uint32_t)(mx + g.nmod[0] * my) << 20) | ((uint32_t)l << 18) | ((uint32_t)(ix + L.n[0] * iy) << 5);
-  return L.cmat;
+  const int ix = floor_div_pos(ea, r1.z, __int_as_float(r3.z), fa);
+  const int iy = floor_div_pos(eb, r1.w, __int_as_float(r3.w), fb);
+  const bool in = (ea | eb) >= 0 && ix < r1.x && iy < r1.y && fa >= r2.x && fa < r2.z && fb >= r2.y && fb < r2.w;
+  ids = ok && in ? ((uint32_t)(mx + g.nmod[0] * my) << 20) | ((uint32_t)l << 18) | ((uint32_t)(ix + r1.x * iy) << 5) : kNone;
+  return ok ? (in ? r0.z : r0.w) : -1;
 }
 
 // PAPER.md:33 global -> local

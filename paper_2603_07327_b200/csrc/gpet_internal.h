@@ -17,6 +17,7 @@ constexpr uint32_t kHitChunkPairs = 512, kHitChunkShift = 9, kHitChunkCapMax = 2
 
 struct DevSource {
   int kind; float pos[3], beam[3]; float acol_sigma;            // radians
+  float acol_sin_max, acol_cos_max;                              // sin / cos of the largest acolinearity deviation that can be drawn
   const uint32_t *act_index; const uint64_t *act_cdf; uint32_t n_active; uint64_t w_total;
   const uint8_t *phantom; int ph_major; int dims[3]; float voxel[3], inv_voxel[3], origin[3];
   double activity_bq; uint64_t pairs_per_slice;
@@ -37,9 +38,10 @@ void count_launch(uint64_t n = 1);
 void set_transport_warps(int warps);
 int transport_warps();
 size_t transport_smem_bytes(const DevTables &T, int n_panels, bool hash);
+int transport_warps_that_fit(const DevTables &T, int n_panels, bool hash, size_t smem_limit);
 cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
-                             unsigned long long *work_counter, int sm_count, cudaStream_t stream);
+                             unsigned long long *work_counter, int sm_count, int warps, cudaStream_t stream);
 cudaError_t launch_locate(const DevGeom *geom, int64_t n, const float *xyz_dev, uint32_t *ids_dev, cudaStream_t stream);
 
 size_t digitize_scratch_bytes(uint64_t n_pairs, uint64_t n_hits);

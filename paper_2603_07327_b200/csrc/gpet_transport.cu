@@ -5,56 +5,64 @@
 // Design.  One CTA of 24 warps per SM, persistent.  Every warp owns a pool of 128 photon
 // SLOTS in shared memory (48-byte records that never move) and one index list per NEXT EVENT: SEARCH (needs a panel
 // search), STEP (Woodcock step in a panel), KN (Klein-Nishina trial), RAY (Rayleigh deflection), PHANTOM (Woodcock
-// step in the voxel grid), plus the FREE list.  A pass pops up to 32 slot indices from ONE list, runs that event for
-// all of them at full SIMD width, writes the changed fields back and pushes every index onto the list of its next
-// event (ballot + prefix popcount).  The scheduler runs the list with the most ready photons; when no list fills a
-// pass, a GEN pass samples one annihilation pair per lane (S3) and queues both photons, so a warp is never short of
-// work before the end.  This is the "regroup live photons by next event" of the north star, done per warp: no
-// block-level barrier, no atomics except the chunked work counter and the hit counter.  Every event's code appears
-// exactly once, and the kernel is specialised on phantom / source kind / search variant to stay small.  Geometry
-// descriptor and interleaved float4 mu tables live in shared memory; hits are staged per warp in shared memory and
-// flushed 32 at a time: one atomicAdd per 32 hits and seven fully coalesced 128-byte stores (SoA).
+// step in the voxel grid), HIT (a deposit waiting to be written), plus the FREE list.  A pass pops up to 32 slot indices
+// from ONE list, runs that event for all of them at full SIMD width, writes the changed fields back and pushes every
+// index onto the list of its next event (ballot + prefix popcount).  The pass bodies are written without divergent
+// branches: every lane runs the same instructions and the outcome is selected at the end.  The scheduler runs any list
+// that fills a pass; when none does, the source refills the pool.  For a point source inside the bore of a ring the
+// source works in two stages: GEN1 draws the pair's Philox block and drops, from cos(theta) alone, the pairs that
+// leave through the axial ends (half of them for a centred source); GEN2 gives the survivors their directions and
+// takes each photon straight to its entry point in the panel whose polygon edge it crosses (ring_entry_fast), so the
+// first panel search costs no pass of its own.  This is the "regroup live photons by next event" of the north star,
+// done per warp: no block-level barrier, no atomics except the work counter and the hit counters.  Geometry header in
+// the constant bank, per-panel and per-layer records and the interleaved float4 mu tables in shared memory; hits are
+// written 32 at a time by the HIT pass: one atomicAdd per 32 hits and seven fully coalesced 128-byte stores (SoA).
 #include "gpet_internal.h"
 
 namespace gpet {
 
 // Launch shape and pool sizes (measured on B200, C1-C4; -D overrides are for experiments only).
 #ifndef GPET_THREADS
-#define GPET_THREADS 768              // one CTA of 24 warps per SM: the tables are staged once, each warp gets 8.7 KB
+#define GPET_THREADS 768              // one CTA of 24 warps per SM: the tables are staged once, each warp gets ~8.5 KB
 #endif
 #ifndef GPET_SLOTS
-#define GPET_SLOTS 128                // photon slots per warp (20 x 160 and 28 x 104 run within 2 % of 24 x 128)
+#define GPET_SLOTS 128                // photon slots per warp
 #endif
 #ifndef GPET_MIN_GEN
-#define GPET_MIN_GEN 24               // the source refills only when at least this many pairs fit (2 free slots each)
+#define GPET_MIN_GEN 16               // the source refills only when at least this many pairs fit
+#endif
+#ifndef GPET_GRAB
+#define GPET_GRAB 128                 // pairs a warp reserves at a time (multiple of 32): short tails at the end of a launch
 #endif
 constexpr int kThreads = GPET_THREADS;
 constexpr int kWarps = kThreads / 32;
-constexpr int kStage = 64;            // staged hits per warp (ring buffer)
+constexpr int kQueue = 64;            // pair queue between the two source stages
+constexpr int kReserve = 32;          // free slots kept for the deposits of a Klein-Nishina pass
 // the parity builds (HASH) also keep an 8-byte hash per slot and get by with 16 slots fewer
 template <bool HASH> constexpr int kSlotsOf = HASH ? GPET_SLOTS - 16 : GPET_SLOTS;
-constexpr uint32_t kChunk = 512;      // pairs a warp reserves at a time
+constexpr uint32_t kGrab = GPET_GRAB;
 constexpr int kMinGen = GPET_MIN_GEN;
+constexpr uint64_t kHash0 = 0xCBF29CE484222325ull;
 
-enum : int { L_FREE = 0, L_SEARCH, L_STEP, L_KN, L_RAY, L_PHANTOM, kLists, L_NONE = kLists, L_GEN };
-
-struct HitStage { uint32_t w[7][kStage]; };      // history, ids, x, y, z, e, tof
+enum : int { L_FREE = 0, L_SEARCH, L_STEP, L_KN, L_RAY, L_PHANTOM, L_HIT, kLists, L_NONE = kLists };
 
 // One warp's private memory.  A photon record is 48 bytes in three 16-byte planes (one LDS.128 / STS.128 each).
 template <bool HASH> struct WarpMem {
   static constexpr int kSlots = kSlotsOf<HASH>;
-  float4 a[kSlots];                    // x, y, z, dx
-  float4 b[kSlots];                    // dy, dz, E, path
-  uint4 c[kSlots];                     // pair, meta, ids of the pending interaction, inv_mu bits
+  float4 a[kSlots];                    // x, y, z, path      (panel frame in STEP / KN / RAY / HIT and after an exit, else global)
+  float4 b[kSlots];                    // dx, dy, dz, E
+  uint4 c[kSlots];                     // pair, meta, ids of the pending interaction, 1/mu_maj bits (HIT: deposited energy bits)
   uint2 hh[HASH ? kSlots : 1];         // outcome hash (parity builds only)
+  uint4 qw[kQueue];                    // pair queue: the pair's source block [R3] ...
+  uint32_t qp[kQueue];                 // ... and its index in the batch
   uint8_t list[kLists][kSlots];        // slot indices by next event (stacks)
-  HitStage stage;
 };
 
-// dynamic shared memory: [WarpMem x warps of the CTA][mu: n_staged x n_energies float4][DevPanel x n_panels]
+// dynamic shared memory: [WarpMem x warps of the CTA][mu: n_staged x n_energies float4][DevLayer x 4][DevPanel x (n_panels + 1)]
 template <bool HASH> struct SmemLayout {
   __host__ __device__ static size_t mu_off(int warps) { return sizeof(WarpMem<HASH>) * (size_t)warps; }
-  __host__ __device__ static size_t geom_off(int warps, int n_mu) { return mu_off(warps) + sizeof(float4) * (size_t)n_mu; }
+  __host__ __device__ static size_t layer_off(int warps, int n_mu) { return mu_off(warps) + sizeof(float4) * (size_t)n_mu; }
+  __host__ __device__ static size_t geom_off(int warps, int n_mu) { return layer_off(warps, n_mu) + sizeof(DevLayer) * kMaxLayers; }
 };
 
 // ---------------------------------------------------------------- fast math with bounded error
@@ -75,6 +83,23 @@ __device__ __forceinline__ void sincos_2pi(float u, float &s, float &c) {
   const float a = 6.283185307179586f * (u - 0.5f);
   s = -__sinf(a); c = -__cosf(a);
 }
+// exp(x) - 1 for |x| <= 0.55 (Klein-Nishina: |x| <= ln(3)/2): Taylor to x^11, relative error below one ulp
+__device__ __forceinline__ float expm1_small(float x) {
+  float p = 2.505210839e-8f;                                           // 1/11!
+  p = fmaf(p, x, 2.755731922e-7f); p = fmaf(p, x, 2.755731922e-6f); p = fmaf(p, x, 2.480158730e-5f);
+  p = fmaf(p, x, 1.984126984e-4f); p = fmaf(p, x, 1.388888889e-3f); p = fmaf(p, x, 8.333333333e-3f);
+  p = fmaf(p, x, 4.166666667e-2f); p = fmaf(p, x, 0.1666666667f); p = fmaf(p, x, 0.5f);
+  return fmaf(p * x, x, x);
+}
+// atan2 good to ~1e-3 rad (it only proposes the first candidate panel of ring_entry_fast)
+__device__ __forceinline__ float atan2_coarse(float y, float x) {
+  const float ax = fabsf(x), ay = fabsf(y), mx = fmaxf(ax, ay), mn = fminf(ax, ay);
+  const float q = mn * rcp_fast(mx + 1e-30f), q2 = q * q;
+  float r = q * fmaf(q2, fmaf(q2, 0.0793f, -0.2883f), 0.9954f);       // atan(q), q in [0, 1]
+  r = ay > ax ? 1.5707963f - r : r;
+  r = x < 0.0f ? 3.1415927f - r : r;
+  return y < 0.0f ? -r : r;
+}
 
 // [R11] linear interpolation on the energy grid: {mu_pe, mu_pe+mu_C, mu_tot, mu_maj}
 __device__ __forceinline__ float4 mu_lookup(const float4 *mu, const DevTables &T, int m, float E) {
@@ -88,65 +113,31 @@ __device__ __forceinline__ float4 mu_lookup(const float4 *mu, const DevTables &T
 
 // ---------------------------------------------------------------- photon state
 struct Photon {
-  float x[3], d[3];        // global frame while searching / in the phantom, panel frame in STEP / KN / RAY
+  float x[3], d[3];        // global frame while searching (fresh photons) / in the phantom, panel frame in STEP / KN / RAY
   float E, path, inv_mu;   // inv_mu = 1 / majorant(E) of the medium the photon is tracked in
   uint32_t pair;           // history - first_history
   uint32_t meta;           // bit0 photon, bits1-4 seq, bits5-10 panel (current, or just left; 63 = none), bit11 in
                            // phantom, bits12-17 Klein-Nishina trial counter, bits18-31 Philox blocks consumed from
                            // this photon's stream [R4] (16383 events per photon: never reached, the energy falls)
-  uint32_t ids;            // lattice result of the pending interaction (KN / RAY)
+  uint32_t ids;            // lattice result of the pending interaction (KN / RAY / HIT), panel bits included
 };
-__device__ __forceinline__ int ph_panel(const Photon &p) { return (p.meta >> 5) & 63u; }
-__device__ __forceinline__ void ph_set_panel(Photon &p, int panel) { p.meta = (p.meta & ~(63u << 5)) | ((uint32_t)panel << 5); }
-__device__ __forceinline__ bool ph_in_phantom(const Photon &p) { return (p.meta >> 11) & 1u; }
+constexpr uint32_t kNoPanel = 63u;
+__device__ __forceinline__ int ph_panel(uint32_t meta) { return (meta >> 5) & 63u; }
+__device__ __forceinline__ uint32_t ph_with_panel(uint32_t meta, int panel) { return (meta & ~(63u << 5)) | ((uint32_t)panel << 5); }
 
 template <bool HASH>
 __device__ __forceinline__ void slot_store(WarpMem<HASH> &W, int slot, const Photon &p, uint64_t h) {
-  W.a[slot] = make_float4(p.x[0], p.x[1], p.x[2], p.d[0]);
-  W.b[slot] = make_float4(p.d[1], p.d[2], p.E, p.path);
+  W.a[slot] = make_float4(p.x[0], p.x[1], p.x[2], p.path);
+  W.b[slot] = make_float4(p.d[0], p.d[1], p.d[2], p.E);
   W.c[slot] = make_uint4(p.pair, p.meta, p.ids, __float_as_uint(p.inv_mu));
   if (HASH) W.hh[slot] = make_uint2((uint32_t)h, (uint32_t)(h >> 32));
 }
 template <bool HASH>
 __device__ __forceinline__ void slot_load(const WarpMem<HASH> &W, int slot, Photon &p, uint64_t &h) {
   const float4 a = W.a[slot], b = W.b[slot]; const uint4 c = W.c[slot];
-  p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.d[0] = a.w; p.d[1] = b.x; p.d[2] = b.y; p.E = b.z; p.path = b.w;
+  p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.path = a.w; p.d[0] = b.x; p.d[1] = b.y; p.d[2] = b.z; p.E = b.w;
   p.pair = c.x; p.meta = c.y; p.ids = c.z; p.inv_mu = __uint_as_float(c.w);
   if (HASH) { const uint2 v = W.hh[slot]; h = ((uint64_t)v.y << 32) | v.x; }
-}
-
-// write one staged hit (slot of this warp's ring buffer) to the global struct-of-arrays buffer
-__device__ __forceinline__ void store_hit(const HitBuf &H, unsigned long long o, const HitStage &stage, uint32_t slot) {
-  if (o < H.capacity) {
-    H.history[o] = stage.w[0][slot]; H.ids[o] = stage.w[1][slot];
-    H.x[o] = __uint_as_float(stage.w[2][slot]); H.y[o] = __uint_as_float(stage.w[3][slot]); H.z[o] = __uint_as_float(stage.w[4][slot]);
-    H.e[o] = __uint_as_float(stage.w[5][slot]); H.tof[o] = __uint_as_float(stage.w[6][slot]);
-  }
-}
-// Flush up to 32 staged hits (lane < count has one, in ring slot `slot`).  Dense layout: one atomicAdd on the global
-// counter, seven coalesced stores.  Chunked layout: the hits go to the region of their 512-pair chunk; lanes of the same
-// chunk (almost always all of them) share one atomicAdd on that chunk's fill counter and write consecutive entries.
-__device__ __forceinline__ void flush_hits(const HitBuf &H, uint32_t first_lo, const HitStage &stage, uint32_t slot, uint32_t count, int lane) {
-  const bool act = (uint32_t)lane < count;
-  if (H.chunk_fill == nullptr) {
-    unsigned long long base = 0;
-    if (lane == 0) base = atomicAdd(H.n_hits, (unsigned long long)count);
-    base = __shfl_sync(0xFFFFFFFFu, base, 0);
-    if (act) store_hit(H, base + lane, stage, slot);
-  } else {
-    if (lane == 0) atomicAdd(H.n_hits, (unsigned long long)count);                    // total produced (no return value needed)
-    const uint32_t chunk = act ? (stage.w[0][slot] - first_lo) >> kHitChunkShift : 0xFFFFFFFFu;
-    const unsigned grp = __match_any_sync(0xFFFFFFFFu, chunk);
-    const int leader = __ffs(grp) - 1;
-    uint32_t base = 0;
-    if (act && lane == leader && chunk < H.n_chunks) base = atomicAdd(&H.chunk_fill[chunk], (uint32_t)__popc(grp));
-    base = __shfl_sync(0xFFFFFFFFu, base, leader);
-    if (act && chunk < H.n_chunks) {
-      const uint32_t pos = base + __popc(grp & ((1u << lane) - 1u));
-      if (pos < H.chunk_cap) store_hit(H, (unsigned long long)chunk * H.chunk_cap + pos, stage, slot);
-      else atomicAdd(&H.chunk_fill[H.n_chunks], 1u);                                   // dropped: this chunk's region is full
-    }
-  }
 }
 
 // [R20] Rayleigh: Thomson pdf by closed-form inversion of the cdf, then a rotation about d
@@ -157,10 +148,6 @@ __device__ __noinline__ float3 rayleigh_dir(float dx, float dy, float dz, float 
   float d[3] = { dx, dy, dz };
   rotate(d, ct, sqrtf(fmaxf(0.0f, 1.0f - ct * ct)), cp, sp);
   return make_float3(d[0], d[1], d[2]);
-}
-__device__ __forceinline__ void rayleigh(float d[3], float u_polar, float u_azimuth) {
-  const float3 r = rayleigh_dir(d[0], d[1], d[2], u_polar, u_azimuth);
-  d[0] = r.x; d[1] = r.y; d[2] = r.z;
 }
 
 // [R13] decay site from the activity map: voxel by the integer cdf (word 0), uniform point inside (words 1-3)
@@ -180,13 +167,66 @@ __device__ __forceinline__ void decay_site(const DevSource &src, uint4 w, float 
 // axial coordinate of every panel of a planar detector).  A photon inside the bore needs at least (bore_r - r0) / |d_xy|
 // of path to reach that radius; if by then it has already passed an axial end, moving away from it, it can meet no
 // panel: the search of [R6] would return "escapes".  Half of the photons of a centred source leave this way.
+// Form used by both callers: r0 = distance of the start point from the axis (< bore_r), z0 its axial coordinate,
+// sxy <= |d_xy| is NOT required -- pass an upper bound of |d_xy| and a lower bound of |d_z| for a conservative answer.
+__device__ __forceinline__ bool misses_axially(const DevGeomHead &g, float r0, float z0, float sxy, float dz) {
+  const float t = (g.bore_r - r0) * rcp_fast(sxy + 1e-30f) * 0.9999f;  // path needed to reach the bore radius, at least
+  const float z1 = fmaf(dz, t, z0);                                    // axial position by then
+  const float lim = dz > 0.0f ? g.bhi[1] + 1e-3f : g.blo[1] - 1e-3f;
+  return dz > 0.0f ? z1 > lim : (dz < 0.0f && z1 < lim);
+}
 __device__ __forceinline__ bool misses_detector(const DevGeomHead &g, const float x[3], const float d[3]) {
-  if (!(g.bore_r > 0.0f)) return false;
   const float r0sq = fmaf(x[0], x[0], x[1] * x[1]);
-  if (r0sq >= g.bore_r * g.bore_r) return false;
-  const float t = (g.bore_r - sqrt_fast(r0sq)) * rcp_fast(sqrt_fast(fmaf(d[0], d[0], d[1] * d[1])) + 1e-30f) * 0.9999f;
-  const float z1 = fmaf(d[2], t, x[2]);                              // axial position when the bore radius can first be reached
-  return (d[2] > 0.0f && z1 > g.bhi[1] + 1e-3f) || (d[2] < 0.0f && z1 < g.blo[1] - 1e-3f);
+  const bool inside = g.bore_r > 0.0f && r0sq < g.bore_r * g.bore_r;
+  return inside && misses_axially(g, sqrt_fast(r0sq), x[2], sqrt_fast(fmaf(d[0], d[0], d[1] * d[1])), d[2]);
+}
+
+// ---------------------------------------------------------------- first panel of a photon inside the bore of a ring
+// Repetition-mode rings: the front faces of the n panels lie on the edges of a regular polygon about the
+// z axis (extended beyond the vertices when panels are wider than an edge, short of them when there are gaps), and every
+// panel box lies outside the open polygon.  A ray that starts inside the inscribed circle crosses the polygon boundary
+// exactly once; if that crossing lies on the front face of panel k, inside the edge, then panel k is the one the search
+// of [R6] returns: no other box has a point the ray reaches earlier.  So: estimate k from the azimuth of the point where
+// the ray leaves the inscribed circle, take the slab test of [R6] on that one panel (the same arithmetic as the search),
+// accept when the ray enters through the front face inside the edge (1 um clear of the vertices, where two overlapping
+// panels tie: those rays go to the full search and its lowest-index rule), otherwise step to the neighbour the crossing
+// point indicates and try once more.  Anything else -- gaps between panels, entries through side or end faces, rays that
+// leave through the axial ends -- is left to the full search (the caller queues the photon for a SEARCH pass).
+// Called by all 32 lanes (`active` = this lane has a photon to place): the early exit is a full-warp vote.
+__device__ __forceinline__ bool ring_entry_fast(const DevGeomHead &g, const DevPanel *pan, const float x[3], const float d[3], bool active, int &bp, float &bt) {
+  const float dxy2 = fmaf(d[0], d[0], d[1] * d[1]);
+  const float b = fmaf(x[0], d[0], x[1] * d[1]);
+  const float cc = fmaf(g.bore_r, g.bore_r, -fmaf(x[0], x[0], x[1] * x[1]));                 // > 0: the photon is inside the bore
+  const float tc = (sqrt_fast(fmaf(dxy2, cc, b * b)) - b) * rcp_fast(dxy2 + 1e-30f);       // leaves the inscribed circle here
+  const float phi = atan2_coarse(fmaf(tc, d[1], x[1]), fmaf(tc, d[0], x[0]));
+  int k = __float2int_rn((phi - g.ring_phi0) * g.ring_kscale);
+  k += k < 0 ? g.n_panels : 0; k -= k >= g.n_panels ? g.n_panels : 0;
+  const float iz = rcp_dir(d[2]);
+  const float z1 = (g.blo[1] - x[2]) * iz, z2 = (g.bhi[1] - x[2]) * iz;
+  const float tnz = fmaxf(fminf(z1, z2), 0.0f), tfz = fmaxf(z1, z2);
+  bool done = !active, ok = false;
+#pragma unroll 1
+  for (int it = 0; it < 2; ++it) {
+    const float *P = pan[k].pose;
+    const float r0 = x[0] - P[0], r1 = x[1] - P[1];
+    const float a = r0 * P[3] + r1 * P[4], c = r0 * P[9] + r1 * P[10];
+    const float da = d[0] * P[3] + d[1] * P[4], dc = d[0] * P[9] + d[1] * P[10];
+    const float ia = rcp_dir(da), ic = rcp_dir(dc);
+    const float a1 = (g.blo[0] - a) * ia, a2 = (g.bhi[0] - a) * ia, c1 = (g.blo[2] - c) * ic, c2 = (g.bhi[2] - c) * ic;
+    const float an = fminf(a1, a2), cn = fminf(c1, c2);
+    const float tn = fmaxf(tnz, fmaxf(an, cn)), tf = fminf(tfz, fminf(fmaxf(a1, a2), fmaxf(c1, c2)));
+    const float af = fmaf(c1, da, a);                                  // tangential coordinate where the ray meets the front plane
+    const bool heading = dc > 0.0f && c < 0.0f;                        // towards the front face, from in front of it
+    const bool within = fabsf(af) <= g.ring_edge_h;
+    const bool front = tf > tn && cn >= tnz && cn >= an && c1 <= c2;   // enters, and through the front face
+    if (!done) {
+      if (heading && within) { done = true; ok = front; bp = k; bt = tn; }
+      else if (!heading) done = true;                                  // the estimate is off by more than a neighbour: full search
+      else { k += af > 0.0f ? 1 : -1; k += k < 0 ? g.n_panels : 0; k -= k >= g.n_panels ? g.n_panels : 0; }
+    }
+    if (__all_sync(0xFFFFFFFFu, done)) break;
+  }
+  return ok;
 }
 
 // ---------------------------------------------------------------- [R6] panel search
@@ -265,115 +305,232 @@ __device__ __forceinline__ int panel_search(const DevGeomHead &g, const DevPanel
 }
 
 // ---------------------------------------------------------------- the kernel
-// Specialisations keep the kernel small (at ~3000 SASS instructions it is sensitive to instruction-cache misses: dropping
-// the phantom code alone made the ring configs 10 % faster).  PHANTOM: the source is a voxel map with a phantom
-// [R17]; KIND: source kind (0 point, 1 voxel map, -1 = read src.kind); PLANAR: panel search variant (-1 = read g.planar);
-// PRETEST: fresh photons take the acceptance pre-test (misses_detector) before they get a slot.
-template <bool HASH, bool PHANTOM, int KIND, int PLANAR, bool PRETEST>
+// Specialisations keep the kernel small (it is sensitive to instruction-cache misses: dropping the phantom code alone
+// made the ring configs 10 % faster).  PHANTOM: the source is a voxel map with a phantom [R17]; KIND: source kind
+// (0 point, 1 voxel map, -1 = read src.kind); PLANAR: panel search variant (-1 = read g.planar); PRETEST: fresh photons
+// take the acceptance pre-test (misses_detector) before they get a slot -- with KIND = 0 as a stage of its own (GEN1);
+// FAST: repetition-mode ring, photons inside the bore find their first panel by ring_entry_fast.
+template <bool HASH, bool PHANTOM, int KIND, int PLANAR, bool PRETEST, bool FAST>
 __global__ void __launch_bounds__(kThreads, 1)
 transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel *panels, DevTables T, DevSource src, uint64_t first_history, uint64_t n_pairs,
                            const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n_mu = T.n_staged * T.n_energies;
   float4 *mu_s = reinterpret_cast<float4 *>(smem_raw + SmemLayout<HASH>::mu_off(blockDim.x >> 5));
+  DevLayer *lay = reinterpret_cast<DevLayer *>(smem_raw + SmemLayout<HASH>::layer_off(blockDim.x >> 5, n_mu));
   DevPanel *pan = reinterpret_cast<DevPanel *>(smem_raw + SmemLayout<HASH>::geom_off(blockDim.x >> 5, n_mu));
   const int lane = threadIdx.x & 31;
   WarpMem<HASH> &W = reinterpret_cast<WarpMem<HASH> *>(smem_raw)[threadIdx.x >> 5];
+  constexpr int kSlots = kSlotsOf<HASH>;
   {
     const uint32_t *gs = reinterpret_cast<const uint32_t *>(panels);
     uint32_t *gd = reinterpret_cast<uint32_t *>(pan);
     const int words = (int)(sizeof(DevPanel) / 4) * g.n_panels;
     for (int i = threadIdx.x; i < words; i += blockDim.x) gd[i] = gs[i];
+    // record n_panels: the identity pose (a photon that has no panel yet is "in the frame" of this one: global = local)
+    for (int i = threadIdx.x; i < (int)(sizeof(DevPanel) / 4); i += blockDim.x)
+      gd[words + i] = (i == 3 || i == 7 || i == 11) ? 0x3F800000u : 0u;
+    for (int i = threadIdx.x; i < (int)(sizeof(DevLayer) / 4) * kMaxLayers; i += blockDim.x)
+      reinterpret_cast<uint32_t *>(lay)[i] = reinterpret_cast<const uint32_t *>(&g.layer[0])[i];
     for (int i = threadIdx.x; i < n_mu; i += blockDim.x) mu_s[i] = T.mu[i];
-    for (int i = lane; i < kSlotsOf<HASH>; i += 32) W.list[L_FREE][i] = (uint8_t)i;
+    for (int i = lane; i < kSlots; i += 32) W.list[L_FREE][i] = (uint8_t)i;
     __syncthreads();
   }
   const float4 *mu = mu_s;
-  HitStage &stage = W.stage;
   const unsigned lt_mask = (1u << lane) - 1u;
-  constexpr bool use_phantom = PHANTOM;
+  const unsigned FULL = 0xFFFFFFFFu;
   const int kind = KIND < 0 ? src.kind : KIND;
+  constexpr bool kPointSrc = KIND == 0 && !PHANTOM;                           // GEN1 (draw, filter) + GEN2 (one photon per lane)
+  const float src_r0 = sqrt_fast(fmaf(src.pos[0], src.pos[0], src.pos[1] * src.pos[1]));   // distance of a point source from the axis
+  // the fused first search needs every fresh photon inside the bore of the ring: point sources only (uniform test)
+  const bool fused = FAST && KIND == 0 && !PHANTOM && g.ring_edge_h > 0.0f &&
+                     fmaf(src.pos[0], src.pos[0], src.pos[1] * src.pos[1]) < g.bore_r * g.bore_r;
 
-  uint64_t w_next = 0, w_end = 0;          // this warp's reserved pairs [w_next, w_end)
+  uint32_t w_next = 0, w_end = 0;          // this warp's reserved pairs [w_next, w_end)
   bool exhausted = false;                  // the global counter ran past n_pairs
-  uint32_t stage_head = 0, stage_cnt = 0;  // ring buffer of staged hits (warp-uniform)
-  int cF = kSlotsOf<HASH>, cS = 0, cT = 0, cK = 0, cR = 0, cP = 0;   // list fill levels (warp-uniform)
+  int cF = kSlots, cS = 0, cT = 0, cK = 0, cR = 0, cP = 0, cH = 0, cQ = 0;   // list / queue fill levels (warp-uniform)
 
+  auto history_of = [&](uint32_t pair) -> uint64_t { return first_history + pair; };
   // [R4] every transport event consumes one whole Philox block of the photon's stream
-  auto block_at = [&](const Photon &p, uint32_t blk) -> uint4 {
-    const uint64_t history = first_history + p.pair;
-    return philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 1u + (p.meta & 1u), blk), key);
-  };
-  auto next_block = [&](Photon &p) -> uint4 { const uint4 w = block_at(p, p.meta >> 18); p.meta += 1u << 18; return w; };
-  // stage one hit per lane that has one; flush 32 staged hits with one atomic + coalesced stores (S10)
-  auto stage_hits = [&](bool has, uint32_t pair, uint32_t hit_ids, const float xg[3], float e, float tof) {
-    const unsigned who = __ballot_sync(0xFFFFFFFFu, has);
-    if (who == 0) return;
-    if (has) {
-      const uint32_t slot = (stage_head + stage_cnt + __popc(who & lt_mask)) & (kStage - 1);
-      stage.w[0][slot] = (uint32_t)(first_history + pair); stage.w[1][slot] = hit_ids;
-      stage.w[2][slot] = __float_as_uint(xg[0]); stage.w[3][slot] = __float_as_uint(xg[1]); stage.w[4][slot] = __float_as_uint(xg[2]);
-      stage.w[5][slot] = __float_as_uint(e); stage.w[6][slot] = __float_as_uint(tof);
-    }
-    stage_cnt += __popc(who);
-    __syncwarp();
-    if (stage_cnt >= 32) {
-      flush_hits(H, (uint32_t)first_history, stage, (stage_head + lane) & (kStage - 1), 32u, lane);
-      stage_head = (stage_head + 32) & (kStage - 1); stage_cnt -= 32;
-      __syncwarp();
-    }
+  auto block_at = [&](uint32_t pair, uint32_t meta, uint32_t blk) -> uint4 {
+    const uint64_t history = history_of(pair);
+    return philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 1u + (meta & 1u), blk), key);
   };
   // push the slot index of every lane with `pred` onto list L (ballot + prefix popcount)
   auto push = [&](int L, int &cnt, bool pred, int idx) {
-    const unsigned m = __ballot_sync(0xFFFFFFFFu, pred);
+    const unsigned m = __ballot_sync(FULL, pred);
     if (pred) W.list[L][cnt + __popc(m & lt_mask)] = (uint8_t)idx;
     cnt += __popc(m);
   };
+  auto end_hash = [&](uint32_t pair, uint32_t meta, uint64_t h) { hash_out[2ull * pair + (meta & 1u)] = h; };
+  auto grab = [&]() {                      // reserve the next pairs of the batch (one atomic per kGrab pairs)
+    if (w_next >= w_end && !exhausted) {
+      unsigned long long b = 0;
+      if (lane == 0) b = atomicAdd(work_counter, (unsigned long long)kGrab);
+      b = __shfl_sync(FULL, b, 0);
+      if (b >= n_pairs) { exhausted = true; w_next = w_end = 0; }
+      else { w_next = (uint32_t)b; w_end = (uint32_t)min((uint64_t)(b + kGrab), n_pairs); }
+    }
+  };
+  // fresh photon -> entry point of its first panel (fused search) or the SEARCH / PHANTOM list
+  // returns the destination list; q is updated to the panel frame on success
+  auto enter_panel = [&](Photon &q, uint64_t &hq, int bp, float bt) {
+    if (HASH) hash_ev(hq, EV_ENTER, (uint32_t)bp);
+    float xl[3], dl[3];
+    to_local(pan[bp].pose, q.x, q.d, xl, dl);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { q.x[k] = fmaf(bt, dl[k], xl[k]); q.d[k] = dl[k]; }   // [R18]
+    q.path += bt; q.meta = ph_with_panel(q.meta, bp);
+    q.inv_mu = rcp_fast(mu_lookup(mu, T, 0, q.E).w);
+  };
+
+  int gen_b = 0, gen_nb = 0;               // point sources: photons A of the top gen_nb queued pairs are placed, their photons B come next
 
 #pragma unroll 1
   for (;;) {
-    // ================================================ scheduler: the list with the most ready photons; when no list
-    // fills a pass, the source refills the SEARCH list with up to 32 fresh pairs (two free slots each)
-    const bool more_src = !exhausted || w_next < w_end;
-    int phase = L_SEARCH, best = cS;
-    if (cT > 0 && cT >= best) { phase = L_STEP; best = cT; }
-    if (cK > best) { phase = L_KN; best = cK; }
-    if (PHANTOM && cP > best) { phase = L_PHANTOM; best = cP; }
-    if (cR > best) { phase = L_RAY; best = cR; }
-    const int np = more_src ? min(32, cF >> 1) : 0;
-    if (best < 32 && np >= kMinGen) phase = L_GEN;
-    else if (best == 0) { if (np > 0) phase = L_GEN; else break; }      // nothing in flight: last pairs, or done
-
-    if (phase == L_GEN) {
-      // ---------------------------------------------- GEN: one annihilation pair per lane (S3) [R13-R16]: both photons
-      // get a slot and wait for their panel search (or, born inside a phantom, for their first phantom step [R17])
-      if (w_next >= w_end && !exhausted) {
-        unsigned long long b = 0;
-        if (lane == 0) b = atomicAdd(work_counter, (unsigned long long)kChunk);
-        b = __shfl_sync(0xFFFFFFFFu, b, 0);
-        if (b >= n_pairs) { exhausted = true; w_next = w_end = 0; }
-        else { w_next = b; w_end = min((uint64_t)(b + kChunk), n_pairs); }
+    // ================================================ scheduler: a list that fills a pass runs (cheap cascade, STEP first);
+    // when none does, the source refills the pool; when it cannot, the fullest list runs short
+    int phase = L_NONE, gen = 0;                                          // gen 1: GEN1 (draw + filter), 2: GEN2 / GEN
+    if (cT >= 32) phase = L_STEP;
+    else if (cH >= 32 || cF < kReserve) phase = L_HIT;                    // cF + cH >= kReserve always: a low free list means deposits wait
+    else if (cK >= 32) phase = L_KN;
+    else if (cS >= 32) phase = L_SEARCH;
+    else if (PHANTOM && cP >= 32) phase = L_PHANTOM;
+    else if (cR >= 32) phase = L_RAY;
+    else {
+      const bool more_src = !exhausted || w_next < w_end;
+      const int room = cF - kReserve;                                     // photons that fit
+      if (kPointSrc) {
+        const int want = gen_b ? gen_nb : min(32, cQ);
+        if (want > 0 && (gen_b || cQ >= 32 || !more_src) && room >= want) gen = 2;
+        else if (!gen_b && more_src && cQ < 32) gen = 1;
+      } else if (more_src && (room >> 1) >= kMinGen) gen = 2;
+      if (!gen) {
+        int best = 0;
+        if (cT > 0) { phase = L_STEP; best = cT; }
+        if (cK > best) { phase = L_KN; best = cK; }
+        if (cS > best) { phase = L_SEARCH; best = cS; }
+        if (PHANTOM && cP > best) { phase = L_PHANTOM; best = cP; }
+        if (cR > best) { phase = L_RAY; best = cR; }
+        if (best == 0) {
+          if (cH > 0) phase = L_HIT;
+          else if (!kPointSrc && more_src) gen = 2;                       // nothing in flight: take what fits
+          else break;                                                     // (point sources: room >= 32 holds when nothing is in flight)
+        }
       }
-      const uint64_t j = w_next + (uint64_t)lane;
-      const int ng = (int)min((uint64_t)np, w_end - w_next);           // pairs generated in this pass (warp-uniform)
-      w_next += (uint64_t)ng;
-      Photon qa = {}, qb = {}; bool fa = false, fb = false;
+    }
+
+    if (gen == 1) {
+      // ---------------------------------------------- GEN1 (point source): the pair's source block [R3].  With PRETEST, cos(theta)
+      // decides whether BOTH photons leave through the axial ends -- photon A as misses_detector would, photon B for
+      // any acolinearity deviation it can draw [R15] (the polar deviation is at most sigma sqrt(-2 ln u_min)); such
+      // pairs end here (two ESCAPEs).  The others are queued for GEN2.
+      grab();
+      const int ng = (int)min(32u, w_end - w_next);
+      const uint32_t j = w_next + (uint32_t)lane;
+      w_next += (uint32_t)ng;
+      bool keep = false; uint4 w = make_uint4(0, 0, 0, 0);
       if (lane < ng) {
-        Photon q = {};
-        q.pair = (uint32_t)j; q.meta = 63u << 5; q.ids = kNone; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
-        const uint64_t history = first_history + j;
+        const uint64_t history = history_of(j);
+        w = philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 0u, 1u), key);
+        keep = true;
+        if (PRETEST) {
+          const float u = u01(w.x), ct = 1.0f - 2.0f * u, sth = 2.0f * sqrt_fast(u * (1.0f - u));
+          const bool miss_a = misses_axially(g, src_r0, src.pos[2], sth * 1.0001f, ct);
+          // photon B: within rho_max of -d.  |d_z| >= |ct| cos(rho) - sth sin(rho), |d_xy| <= sth cos(rho) + |ct| sin(rho)
+          const float sr = src.acol_sin_max, cr = src.acol_cos_max;
+          const float bz = fmaf(fabsf(ct), cr, -sth * sr), bxy = fmaf(sth, cr, fabsf(ct) * sr) * 1.0001f;
+          const bool miss_b = bz > 0.0f && misses_axially(g, src_r0, src.pos[2], bxy, ct > 0.0f ? -bz : bz);
+          keep = !(miss_a && miss_b);
+          if (HASH && !keep) { uint64_t he = kHash0; hash_ev(he, EV_ESCAPE, 0); hash_out[2ull * j] = he; hash_out[2ull * j + 1] = he; }
+        }
+      }
+      const unsigned mk = __ballot_sync(FULL, keep);
+      if (keep) { const int o = cQ + __popc(mk & lt_mask); W.qw[o] = w; W.qp[o] = j; }
+      cQ += __popc(mk);
+      __syncwarp();
+      continue;
+    }
+    if (gen == 2 && kPointSrc) {
+      // ---------------------------------------------- GEN2 (point source): one photon per lane, in two half-passes over the same
+      // queued pairs -- photons A, then photons B (opposite direction plus acolinearity [R15]) -- so that a pass needs
+      // 32 free slots, not 64, and runs at full width.  A photon that may reach the detector gets a slot: at its entry
+      // point in the STEP list when the fused search succeeds, else in the SEARCH list.
+      const int nb = gen_b ? gen_nb : min(32, cQ);
+      const bool have = lane < nb;
+      Photon q = {};
+      q.meta = (kNoPanel << 5) | (uint32_t)gen_b; q.ids = kNone; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
+      q.x[0] = src.pos[0]; q.x[1] = src.pos[1]; q.x[2] = src.pos[2];
+      q.d[0] = 1.0f; q.d[1] = 0.0f; q.d[2] = 0.0f;
+      float sxy = 1.0f;                                                // |d_xy|
+      if (have) {
+        const uint4 w = W.qw[cQ - 1 - lane]; q.pair = W.qp[cQ - 1 - lane];
+        const float u = u01(w.x), ct = 1.0f - 2.0f * u, sth = 2.0f * sqrtf(u * (1.0f - u));   // sin^2 = (1-ct)(1+ct)
+        float sp, cp; sincospif(2.0f * u01(w.y), &sp, &cp);
+        q.d[0] = sth * cp; q.d[1] = sth * sp; q.d[2] = ct; sxy = sth;
+        if (gen_b) {
+          q.d[0] = -q.d[0]; q.d[1] = -q.d[1]; q.d[2] = -q.d[2];
+          if (src.acol_sigma > 0.0f) {
+            const float rho = src.acol_sigma * sqrt_fast(-2.0f * __logf(u01(w.z)));
+            float sr, cr; sincos_small(rho, sr, cr);
+            float sa, ca; sincos_2pi(u01(w.w), sa, ca);               // azimuth of a ~4e-3 rad deviation: 2^-21 is ample
+            rotate(q.d, cr, sr, ca, sa);
+            sxy = sqrt_fast(fmaf(q.d[0], q.d[0], q.d[1] * q.d[1]));
+          }
+        }
+      }
+      bool alive = have;
+      uint64_t hq = kHash0;
+      if (PRETEST) {
+        alive = have && !misses_axially(g, src_r0, src.pos[2], sxy, q.d[2]);
+        if (HASH && have && !alive) { uint64_t he = kHash0; hash_ev(he, EV_ESCAPE, 0); end_hash(q.pair, q.meta, he); }
+      }
+      int bp = 0; float bt = 0.0f; bool entered = false;
+      if (FAST && fused) {
+        entered = ring_entry_fast(g, pan, q.x, q.d, alive, bp, bt);
+        if (entered) enter_panel(q, hq, bp, bt);
+      }
+      const unsigned ma = __ballot_sync(FULL, alive);
+      const int idx = alive ? W.list[L_FREE][cF - 1 - __popc(ma & lt_mask)] : 0;
+      cF -= __popc(ma);
+      if (alive) slot_store(W, idx, q, hq);
+      push(L_STEP, cT, alive && entered, idx);
+      push(L_SEARCH, cS, alive && !entered, idx);
+      if (gen_b) { cQ -= nb; gen_b = 0; } else { gen_b = 1; gen_nb = nb; }
+      __syncwarp();
+      continue;
+    }
+    if (gen == 2) {
+      // ---------------------------------------------- GEN (voxel / beam sources): one annihilation pair per lane (S3) [R13-R16].
+      // Each photon that may reach the detector gets a slot in the SEARCH list (or, born inside a phantom, in the
+      // PHANTOM list for its first phantom step [R17]).
+      const int room = max((cF - kReserve) >> 1, (cT | cK | cS | cP | cR | cH) == 0 ? 1 : 0);
+      grab();
+      const int ng = (int)min((uint32_t)min(32, room), w_end - w_next);
+      const uint32_t j = w_next + (uint32_t)lane;
+      w_next += (uint32_t)ng;
+      const bool have = lane < ng;
+      Photon q = {};
+      q.pair = j; q.meta = kNoPanel << 5; q.ids = kNone; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
+      q.x[0] = src.pos[0]; q.x[1] = src.pos[1]; q.x[2] = src.pos[2];
+      q.d[0] = 1.0f; q.d[1] = 0.0f; q.d[2] = 0.0f;
+      uint4 w = make_uint4(0, 0, 0, 0);
+      if (have) {
+        const uint64_t history = history_of(j);
         const uint32_t h_lo = (uint32_t)history, h_hi = (uint32_t)(history >> 32);
-        q.x[0] = src.pos[0]; q.x[1] = src.pos[1]; q.x[2] = src.pos[2];
         if (kind == 1) decay_site(src, philox4x32_10(make_uint4(h_lo, h_hi, 0u, 0u), key), q.x);
-        const uint4 w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 1u), key);
+        w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 1u), key);
         if (kind == 2) { q.d[0] = src.beam[0]; q.d[1] = src.beam[1]; q.d[2] = src.beam[2]; }
         else {
           const float u = u01(w.x), ct = 1.0f - 2.0f * u, sth = 2.0f * sqrtf(u * (1.0f - u));   // sin^2 = (1-ct)(1+ct)
           float sp, cp; sincospif(2.0f * u01(w.y), &sp, &cp);
           q.d[0] = sth * cp; q.d[1] = sth * sp; q.d[2] = ct;
         }
-        if (use_phantom) { q.meta |= 1u << 11; q.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, q.E).z); }
-        auto make_b = [&]() {                                       // photon B: opposite, plus acolinearity
+        if (PHANTOM) { q.meta |= 1u << 11; q.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, q.E).z); }
+      }
+#pragma unroll 1
+      for (int ph = 0; ph < 2; ++ph) {
+        if (ph == 1 && have) {                                        // photon B: opposite, plus acolinearity [R15]
           q.d[0] = -q.d[0]; q.d[1] = -q.d[1]; q.d[2] = -q.d[2];
           if (src.acol_sigma > 0.0f) {
             const float rho = src.acol_sigma * sqrt_fast(-2.0f * __logf(u01(w.z)));
@@ -382,192 +539,226 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
             rotate(q.d, cr, sr, cp, sp);
           }
           q.meta |= 1u;
-        };
-        if (!PRETEST) {                                               // both photons take a slot: SEARCH, or PHANTOM when born there [R17]
-          uint8_t *dst = use_phantom ? &W.list[L_PHANTOM][cP] : &W.list[L_SEARCH][cS];
-          const int ia = W.list[L_FREE][cF - 1 - 2 * lane], ib = W.list[L_FREE][cF - 2 - 2 * lane];
-          slot_store(W, ia, q, 0xCBF29CE484222325ull);
-          make_b();
-          slot_store(W, ib, q, 0xCBF29CE484222325ull);
-          dst[2 * lane] = (uint8_t)ia; dst[2 * lane + 1] = (uint8_t)ib;
-        } else {
-          // a photon that cannot reach the detector ends here (ESCAPE); the others take a slot and wait for their search
-          fa = !misses_detector(g, q.x, q.d);
-          if (HASH && !fa) { uint64_t ha = 0xCBF29CE484222325ull; hash_ev(ha, EV_ESCAPE, 0); hash_out[2ull * q.pair] = ha; }
-          qa = q;
-          make_b();
-          fb = !misses_detector(g, q.x, q.d);
-          if (HASH && !fb) { uint64_t hb2 = 0xCBF29CE484222325ull; hash_ev(hb2, EV_ESCAPE, 0); hash_out[2ull * q.pair + 1] = hb2; }
-          qb = q;
         }
-      }
-      if (!PRETEST) { cF -= 2 * ng; if (use_phantom) cP += 2 * ng; else cS += 2 * ng; }
-      else {
-        const unsigned mA = __ballot_sync(0xFFFFFFFFu, fa), mB = __ballot_sync(0xFFFFFFFFu, fb);
-        const int ra = __popc(mA & lt_mask), na = __popc(mA), rb = __popc(mB & lt_mask), nb = __popc(mB);
-        if (fa) { const int ia = W.list[L_FREE][cF - 1 - ra]; slot_store(W, ia, qa, 0xCBF29CE484222325ull); W.list[L_SEARCH][cS + ra] = (uint8_t)ia; }
-        if (fb) { const int ib = W.list[L_FREE][cF - 1 - na - rb]; slot_store(W, ib, qb, 0xCBF29CE484222325ull); W.list[L_SEARCH][cS + na + rb] = (uint8_t)ib; }
-        cF -= na + nb; cS += na + nb;
+        bool alive = have;
+        if (PRETEST && !PHANTOM) {
+          alive = have && !misses_detector(g, q.x, q.d);
+          if (HASH && have && !alive) { uint64_t he = kHash0; hash_ev(he, EV_ESCAPE, 0); end_hash(q.pair, q.meta, he); }
+        }
+        const unsigned ma = __ballot_sync(FULL, alive);
+        const int idx = alive ? W.list[L_FREE][cF - 1 - __popc(ma & lt_mask)] : 0;
+        cF -= __popc(ma);
+        if (alive) slot_store(W, idx, q, kHash0);
+        if (PHANTOM) push(L_PHANTOM, cP, alive, idx);
+        else push(L_SEARCH, cS, alive, idx);
       }
       __syncwarp();
       continue;
     }
+
     if (phase == L_SEARCH) {
-      // ---------------------------------------------- SEARCH: nearest panel ahead [R6], entry transform [R18]
-      // (repeated without a trip through the scheduler while the list still fills a whole pass: a GEN pass leaves two)
-      do {
+      // ---------------------------------------------- SEARCH: nearest panel ahead [R6], entry transform [R18].  A photon that has
+      // just left a panel arrives in that panel's frame (record n_panels is the identity: fresh photons are global)
       const int n = min(cS, 32); const bool act = lane < n;
       Photon q = {}; uint64_t hq = 0; int idx = 0;
       if (act) { idx = W.list[L_SEARCH][cS - 1 - lane]; slot_load(W, idx, q, hq); }
       cS -= n;
       int dest = L_NONE;
+      const int excl = ph_panel(q.meta);
       if (act) {
-        float bt; const int bp = panel_search<PLANAR>(g, pan, q.x, q.d, ph_panel(q), bt);
+        const float *P = pan[excl == (int)kNoPanel ? g.n_panels : excl].pose;
+        const float xl[3] = { q.x[0], q.x[1], q.x[2] }, dl[3] = { q.d[0], q.d[1], q.d[2] };
+        point_to_global(P, xl, q.x); dir_to_global(P, dl, q.d);
+      }
+      int bp = -1; float bt = 0.0f; bool found = false;
+      if (FAST && PHANTOM && g.ring_edge_h > 0.0f)                    // photons that have just left the phantom, inside the bore
+        found = ring_entry_fast(g, pan, q.x, q.d, act && excl == (int)kNoPanel && fmaf(q.x[0], q.x[0], q.x[1] * q.x[1]) < g.bore_r * g.bore_r, bp, bt);
+      if (act) {
+        if (!found) bp = panel_search<PLANAR>(g, pan, q.x, q.d, excl, bt);
         if (bp < 0) {
-          if (HASH) { hash_ev(hq, EV_ESCAPE, 0); hash_out[2ull * q.pair + (q.meta & 1u)] = hq; }
+          if (HASH) { hash_ev(hq, EV_ESCAPE, 0); end_hash(q.pair, q.meta, hq); }
           dest = L_FREE;
         } else {
-          if (HASH) hash_ev(hq, EV_ENTER, (uint32_t)bp);
-          float xl[3], dl[3];
-          to_local(pan[bp].pose, q.x, q.d, xl, dl);
-#pragma unroll
-          for (int k = 0; k < 3; ++k) { q.x[k] = fmaf(bt, dl[k], xl[k]); q.d[k] = dl[k]; }   // [R18]
-          q.path += bt; ph_set_panel(q, bp);
-          q.inv_mu = rcp_fast(mu_lookup(mu, T, 0, q.E).w);
+          enter_panel(q, hq, bp, bt);
           dest = L_STEP;
           slot_store(W, idx, q, hq);
         }
       }
       push(L_FREE, cF, dest == L_FREE, idx);
       push(L_STEP, cT, dest == L_STEP, idx);
-      __syncwarp();
-      } while (cS >= 32);
-      continue;
-    }
-    if (phase == L_STEP) {
-      // ---------------------------------------------- STEP: Woodcock step, layer selection, lattice lookup [R19]
+    } else if (phase == L_STEP) {
+      // ---------------------------------------------- STEP: Woodcock step, layer selection, lattice lookup [R19], outcome [R20].
+      // No divergent branches: every lane draws, advances to the collision point or to the exit face, looks the point up
+      // and selects its next event.
       const int n = min(cT, 32); const bool act = lane < n;
-      Photon p = {}; uint64_t h = 0; int idx = 0;
-      if (act) { idx = W.list[L_STEP][cT - 1 - lane]; slot_load(W, idx, p, h); }
+      const int idx = W.list[L_STEP][max(cT - 1 - lane, 0)];
       cT -= n;
-      int dest = L_NONE; bool hit = false; float xg[3] = {0.f, 0.f, 0.f};
-      if (act) {
-        const uint4 w = next_block(p);                                // [R4] free path, outcome, Rayleigh polar + azimuth
-        const float s = -__logf(u01(w.x)) * p.inv_mu;
-        float te[3];
-#pragma unroll
-        for (int k = 0; k < 3; ++k)                                   // distance to the box exit [R32]
-          te[k] = ((p.d[k] >= 0.0f ? g.bhi[k] : g.blo[k]) - p.x[k]) * rcp_dir(p.d[k]);
-        float tf = fminf(te[0], fminf(te[1], te[2]));
-        const int panel = ph_panel(p);
-        if (s >= tf) {                                                // leaves the panel [R33]
-          // Exit face = the axis that limits tf.  If no other panel has a point beyond that face (precomputed per panel
-          // and face at create time: true for the back and axial faces of any ring), the search of [R6] cannot find
-          // anything: the photon escapes here, with the same EXIT, ESCAPE events, and skips transform and search.
-          const int kx = te[0] <= tf ? 0 : (te[1] <= tf ? 1 : 2);
-          const float dk = kx == 0 ? p.d[0] : (kx == 1 ? p.d[1] : p.d[2]);
-          const bool open = (pan[panel].open_faces >> (2 * kx + (dk >= 0.0f ? 1 : 0))) & 1u;
-          if (HASH) hash_ev(h, EV_EXIT, (uint32_t)panel);
-          if (open) {
-            if (HASH) { hash_ev(h, EV_ESCAPE, 0); hash_out[2ull * p.pair + (p.meta & 1u)] = h; }
-            dest = L_FREE;
-          } else {
-            tf = fmaxf(tf, 0.0f);
-            const float xl[3] = { fmaf(tf, p.d[0], p.x[0]), fmaf(tf, p.d[1], p.x[1]), fmaf(tf, p.d[2], p.x[2]) };
-            const float dl[3] = { p.d[0], p.d[1], p.d[2] };
-            p.path += tf;
-            point_to_global(pan[panel].pose, xl, p.x); dir_to_global(pan[panel].pose, dl, p.d);   // back to the global frame
-            dest = L_SEARCH;
-          }
-        } else {
-#pragma unroll
-          for (int k = 0; k < 3; ++k) p.x[k] = fmaf(s, p.d[k], p.x[k]);
-          p.path += s;
-          uint32_t id;                                                // depth -> layer -> crystal
-          const int mat = lattice_lookup(g, __float2int_rd(p.x[0] * kQ) + g.hWq, __float2int_rd(p.x[1] * kQ) + g.hHq,
-                                         __float2int_rd(p.x[2] * kQ), id);
-          dest = L_STEP;
-          if (mat < 0) { if (HASH) hash_ev(h, EV_STEP_VACUUM, 0); }
-          else {
-            if (id != kNone) id |= (uint32_t)panel << 26;
-            const float4 m4 = mu_lookup(mu, T, mat, p.E);
-            const float t = u01(w.y) * m4.w;                          // [R20] one draw picks the outcome
-            p.ids = id;
-            if (t < m4.x) {                                           // photoelectric: deposit E, end
-              if (HASH) { hash_ev(h, EV_PE, id); hash_out[2ull * p.pair + (p.meta & 1u)] = h; }
-              if (id != kNone) { hit = true; point_to_global(pan[panel].pose, p.x, xg); }
-              dest = L_FREE;
-            } else if (t < m4.y) dest = L_KN;
-            else if (t < m4.z) { dest = L_RAY; if (HASH) hash_ev(h, EV_RAYLEIGH, id); }   // deflected in its own pass
-            else if (HASH) hash_ev(h, EV_VIRTUAL, id);
-          }
-        }
+      float4 A = W.a[idx]; const float4 B = W.b[idx]; uint4 C = W.c[idx];
+      uint64_t h = 0;
+      if (HASH) { const uint2 v = W.hh[idx]; h = ((uint64_t)v.y << 32) | v.x; }
+      const uint4 w = block_at(C.x, C.y, C.y >> 18);                  // [R4] free path, outcome, Rayleigh polar + azimuth
+      C.y += 1u << 18;
+      const float s = -__logf(u01(w.x)) * __uint_as_float(C.w);
+      const float te0 = ((B.x >= 0.0f ? g.bhi[0] : g.blo[0]) - A.x) * rcp_dir(B.x);   // distance to the box exit [R32]
+      const float te1 = ((B.y >= 0.0f ? g.bhi[1] : g.blo[1]) - A.y) * rcp_dir(B.y);
+      const float te2 = ((B.z >= 0.0f ? g.bhi[2] : g.blo[2]) - A.z) * rcp_dir(B.z);
+      const float tf = fminf(te0, fminf(te1, te2));
+      const int panel = ph_panel(C.y);
+      const bool exits = s >= tf;                                      // leaves the panel [R33]
+      // Exit face = the axis that limits tf.  If no other panel has a point beyond that face (precomputed per panel and
+      // face at create time: true for the back and axial faces of any ring), the search of [R6] cannot find anything:
+      // the photon escapes here, with the same EXIT, ESCAPE events, and needs no search.
+      const int kx = te0 <= tf ? 0 : (te1 <= tf ? 1 : 2);
+      const float dk = kx == 0 ? B.x : (kx == 1 ? B.y : B.z);
+      const bool open = (pan[panel].open_faces >> (2 * kx + (dk >= 0.0f ? 1 : 0))) & 1u;
+      const float step = exits ? fmaxf(tf, 0.0f) : s;
+      A.x = fmaf(step, B.x, A.x); A.y = fmaf(step, B.y, A.y); A.z = fmaf(step, B.z, A.z); A.w += step;
+      uint32_t id;                                                     // depth -> layer -> crystal
+      const int mat = lattice_lookup(g, lay, __float2int_rd(A.x * kQ) + g.hWq, __float2int_rd(A.y * kQ) + g.hHq, __float2int_rd(A.z * kQ), id);
+      if (id != kNone) id |= (uint32_t)panel << 26;
+      const bool matter = !exits && mat >= 0;
+      const float4 m4 = mu_lookup(mu, T, mat < 0 ? 0 : mat, B.w);
+      const float t = u01(w.y) * m4.w;                                 // [R20] one draw picks the outcome
+      const bool pe = matter && t < m4.x, kn = matter && !pe && t < m4.y, ray = matter && !pe && !kn && t < m4.z;
+      int dest = L_STEP;
+      if (ray) dest = L_RAY;                                           // deflected in its own pass
+      if (kn) dest = L_KN;
+      if (pe) dest = id != kNone ? L_HIT : L_FREE;                     // photoelectric: deposit E, end
+      if (exits) dest = open ? L_FREE : L_SEARCH;
+      if (!act) dest = L_NONE;
+      if (HASH && act) {
+        if (exits) { hash_ev(h, EV_EXIT, (uint32_t)panel); if (open) hash_ev(h, EV_ESCAPE, 0); }
+        else if (mat < 0) hash_ev(h, EV_STEP_VACUUM, 0);
+        else if (pe) hash_ev(h, EV_PE, id);
+        else if (kn) { }                                               // hashed when a trial is accepted
+        else if (ray) hash_ev(h, EV_RAYLEIGH, id);
+        else hash_ev(h, EV_VIRTUAL, id);
+        if (dest == L_FREE || dest == L_HIT) end_hash(C.x, C.y, h);
       }
-      stage_hits(hit, p.pair, p.ids | ((p.meta & 1u) << 4) | ((p.meta >> 1) & 15u), xg, p.E, p.path * kInvC);
-      if (act && dest != L_FREE) slot_store(W, idx, p, h);
+      if (matter) C.z = id;
+      if (pe) C.w = __float_as_uint(B.w);                              // the HIT pass reads the deposit here
+      if (dest != L_FREE && dest != L_NONE) {
+        W.a[idx] = A; W.c[idx] = C;
+        if (HASH) W.hh[idx] = make_uint2((uint32_t)h, (uint32_t)(h >> 32));
+      }
       push(L_STEP, cT, dest == L_STEP, idx);
       push(L_KN, cK, dest == L_KN, idx);
       push(L_FREE, cF, dest == L_FREE, idx);
-      if (__any_sync(0xFFFFFFFFu, dest == L_SEARCH || dest == L_RAY)) {   // the rare destinations share one vote
+      push(L_HIT, cH, dest == L_HIT, idx);
+      if (__any_sync(FULL, dest == L_SEARCH || dest == L_RAY)) {       // the rare destinations share one vote
         push(L_SEARCH, cS, dest == L_SEARCH, idx);
         push(L_RAY, cR, dest == L_RAY, idx);
       }
     } else if (phase == L_KN) {
-      // ---------------------------------------------- KN: one Klein-Nishina trial per visit [R20]
-      const int n = min(cK, 32); const bool act = lane < n;
-      Photon p = {}; uint64_t h = 0; int idx = 0;
-      if (act) { idx = W.list[L_KN][cK - 1 - lane]; slot_load(W, idx, p, h); }
+      // ---------------------------------------------- KN: one Klein-Nishina trial per visit [R20].  A deposit in a crystal is
+      // copied into a free slot and queued for the HIT pass; the photon itself goes on.
+      const int n = min(min(cK, 32), cF); const bool act = lane < n;
+      const int idx = W.list[L_KN][max(cK - 1 - lane, 0)];
       cK -= n;
-      int dest = L_NONE; bool hit = false; float xg[3] = {0.f, 0.f, 0.f}, e_dep = 0.f; uint32_t hit_ids = 0;
-      if (act) {
-        const bool in_ph = PHANTOM && ph_in_phantom(p);
-        const float k = p.E * (1.0f / kMec2), e0 = rcp_fast(1.0f + 2.0f * k), e02 = e0 * e0;
-        const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
-        const uint4 w = next_block(p);                                // [R4] u_a, u_b, u_c, azimuth
-        const float ua = u01(w.x), ub = u01(w.y), uc = u01(w.z);
-        // om = 1 - eps and em = eps - eps0 are formed without cancellation, so that sin^2 = t (2 - t) keeps
-        // full relative accuracy at both poles (t = om/(k eps), 2 - t = em/(eps0 k eps)); plain fp32 loses
-        // 3-4 digits of small scattering angles and moves later hits by micrometres
-        float eps, om, em;
-        if (ua * (a1 + a2) < a1) {
-          if (ub < 0.5f) { om = -expm1f(-a1 * ub); eps = 1.0f - om; em = eps - e0; }
-          else { em = e0 * expm1f(a1 * (1.0f - ub)); eps = e0 + em; om = 1.0f - eps; }
-        } else {
-          eps = sqrt_fast(fmaf(1.0f - e02, ub, e02));
-          om = (1.0f - e02) * (1.0f - ub) * rcp_fast(1.0f + eps); em = (1.0f - e02) * ub * rcp_fast(eps + e0);
+      const float4 A = W.a[idx]; float4 B = W.b[idx]; uint4 C = W.c[idx];
+      uint64_t h = 0;
+      if (HASH) { const uint2 v = W.hh[idx]; h = ((uint64_t)v.y << 32) | v.x; }
+      const bool in_ph = PHANTOM && ((C.y >> 11) & 1u);
+      const float E = B.w;
+      const float k = E * (1.0f / kMec2), e0 = rcp_fast(1.0f + 2.0f * k), e02 = e0 * e0;
+      const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
+      const uint4 w = block_at(C.x, C.y, C.y >> 18);                  // [R4] u_a, u_b, u_c, azimuth
+      C.y += 1u << 18;
+      const float ua = u01(w.x), ub = u01(w.y), uc = u01(w.z);
+      // om = 1 - eps and em = eps - eps0 are formed without cancellation, so that sin^2 = t (2 - t) keeps
+      // full relative accuracy at both poles (t = om/(k eps), 2 - t = em/(eps0 k eps)); plain fp32 loses
+      // 3-4 digits of small scattering angles and moves later hits by micrometres
+      const bool lowhalf = ub < 0.5f;
+      const float v = expm1_small(lowhalf ? -a1 * ub : a1 * (1.0f - ub));
+      const float om_x = lowhalf ? -v : 1.0f - fmaf(e0, v, e0);       // eps = exp(-a1 ub)
+      const float em_x = lowhalf ? (1.0f + v) - e0 : e0 * v;
+      const float eps_x = lowhalf ? 1.0f + v : fmaf(e0, v, e0);
+      const float eps_s = sqrt_fast(fmaf(1.0f - e02, ub, e02));       // eps = sqrt(eps0^2 + (1 - eps0^2) ub)
+      const float om_s = (1.0f - e02) * (1.0f - ub) * rcp_fast(1.0f + eps_s), em_s = (1.0f - e02) * ub * rcp_fast(eps_s + e0);
+      const bool expo = ua * (a1 + a2) < a1;
+      const float eps = expo ? eps_x : eps_s, om = expo ? om_x : om_s, em = expo ? em_x : em_s;
+      const float ike = rcp_fast(k * eps);
+      const float t = om * ike, tm = em * ike * (1.0f + 2.0f * k);
+      const float gr = 1.0f - eps * t * tm * rcp_fast(1.0f + eps * eps);
+      const bool accept = gr >= uc || ((C.y >> 12) & 63u) >= 63u;     // [R22: the 64th trial always is]
+      float sp, cp; sincos_2pi(u01(w.w), sp, cp);
+      float dn[3] = { B.x, B.y, B.z };
+      rotate(dn, 1.0f - t, sqrt_fast(fmaxf(t * tm, 0.0f)), cp, sp);
+      const float dep = om * E, E2 = E - dep;
+      const bool cut = E2 < kCutoff;                                   // [R12]
+      const bool hit = act && accept && !in_ph && C.z != kNone;
+      // the deposit: its own record {x, y, z, path}, {pair, meta, ids, energy}, in a fresh slot, for the HIT pass
+      const unsigned mh = __ballot_sync(FULL, hit);
+      if (mh) {
+        const int rk = __popc(mh & lt_mask);
+        if (hit) {
+          const int i2 = W.list[L_FREE][cF - 1 - rk];
+          W.a[i2] = A; W.c[i2] = make_uint4(C.x, C.y, C.z, __float_as_uint(cut ? E : dep));
+          W.list[L_HIT][cH + rk] = (uint8_t)i2;
         }
-        const float ike = rcp_fast(k * eps);
-        const float t = om * ike, tm = em * ike * (1.0f + 2.0f * k);
-        const float gr = 1.0f - eps * t * tm * rcp_fast(1.0f + eps * eps);
-        dest = L_KN;
-        if (gr >= uc || ((p.meta >> 12) & 63u) >= 63u) {              // accepted [R22: the 64th trial always is]
-          p.meta &= ~(63u << 12);
-          float sp, cp; sincos_2pi(u01(w.w), sp, cp);
-          rotate(p.d, 1.0f - t, sqrt_fast(fmaxf(t * tm, 0.0f)), cp, sp);
-          const float dep = om * p.E, E2 = p.E - dep;
-          const bool cut = E2 < kCutoff;                              // [R12]
-          if (in_ph) {
-            if (HASH) { hash_ev(h, EV_PH_COMPTON, 0); if (cut) hash_ev(h, EV_PH_CUTOFF, 0); }
-            if (!cut) { p.E = E2; p.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, p.E).z); dest = L_PHANTOM; }
-          } else {
-            if (HASH) { hash_ev(h, EV_COMPTON, p.ids); if (cut) hash_ev(h, EV_CUTOFF, p.ids); }
-            if (p.ids != kNone) {
-              hit = true; e_dep = cut ? p.E : dep; point_to_global(pan[ph_panel(p)].pose, p.x, xg);
-              const uint32_t seq = (p.meta >> 1) & 15u;
-              hit_ids = p.ids | ((p.meta & 1u) << 4) | seq;
-              if (seq < 15u) p.meta += 2u;                            // [R9] 4-bit saturating hit counter
-            }
-            if (!cut) { p.E = E2; p.inv_mu = rcp_fast(mu_lookup(mu, T, 0, p.E).w); dest = L_STEP; }
-          }
-          if (cut) { if (HASH) hash_out[2ull * p.pair + (p.meta & 1u)] = h; dest = L_FREE; }
-        } else p.meta += 1u << 12;
+        cF -= __popc(mh); cH += __popc(mh);
       }
-      stage_hits(hit, p.pair, hit_ids, xg, e_dep, p.path * kInvC);
-      if (act && dest != L_FREE) slot_store(W, idx, p, h);
+      int dest = L_KN;
+      if (accept) {
+        if (HASH && act) {
+          if (in_ph) { hash_ev(h, EV_PH_COMPTON, 0); if (cut) hash_ev(h, EV_PH_CUTOFF, 0); }
+          else { hash_ev(h, EV_COMPTON, C.z); if (cut) hash_ev(h, EV_CUTOFF, C.z); }
+          if (cut) end_hash(C.x, C.y, h);
+        }
+        C.y &= ~(63u << 12);
+        if (hit && ((C.y >> 1) & 15u) < 15u) C.y += 2u;                // [R9] 4-bit saturating hit counter
+        B.x = dn[0]; B.y = dn[1]; B.z = dn[2]; B.w = E2;
+        const float4 m4 = mu_lookup(mu, T, in_ph ? src.ph_major : 0, cut ? E : E2);
+        C.w = __float_as_uint(rcp_fast(in_ph ? m4.z : m4.w));
+        dest = cut ? L_FREE : (in_ph ? L_PHANTOM : L_STEP);
+      } else C.y += 1u << 12;
+      if (!act) dest = L_NONE;
+      if (dest != L_FREE && dest != L_NONE) {
+        W.b[idx] = B; W.c[idx] = C;
+        if (HASH) W.hh[idx] = make_uint2((uint32_t)h, (uint32_t)(h >> 32));
+      }
       push(L_KN, cK, dest == L_KN, idx);
       push(L_STEP, cT, dest == L_STEP, idx);
       push(L_FREE, cF, dest == L_FREE, idx);
-      if (use_phantom) push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
+      if (PHANTOM) push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
+    } else if (phase == L_HIT) {
+      // ---------------------------------------------- HIT (S10): up to 32 deposits -> global frame [R22] -> the hit buffer.  Dense
+      // layout: one atomicAdd on the global counter, seven coalesced stores.  Chunked layout: the hits go to the region
+      // of their 512-pair chunk; lanes of the same chunk (almost always all of them) share one atomicAdd on that chunk's
+      // fill counter and write consecutive entries.
+      const int n = min(cH, 32); const bool act = lane < n;
+      const int idx = W.list[L_HIT][max(cH - 1 - lane, 0)];
+      cH -= n;
+      const float4 A = W.a[idx]; const uint4 C = W.c[idx];
+      const float xl[3] = { A.x, A.y, A.z }; float xg[3];
+      point_to_global(pan[C.z >> 26].pose, xl, xg);
+      const uint32_t hist = (uint32_t)history_of(C.x), ids = C.z | ((C.y & 1u) << 4) | ((C.y >> 1) & 15u);
+      const float tof = A.w * kInvC;
+      unsigned long long o = 0; bool ok = false;
+      if (H.chunk_fill == nullptr) {
+        unsigned long long base = 0;
+        if (lane == 0) base = atomicAdd(H.n_hits, (unsigned long long)n);
+        base = __shfl_sync(FULL, base, 0);
+        o = base + lane; ok = act && o < H.capacity;
+      } else {
+        if (lane == 0) atomicAdd(H.n_hits, (unsigned long long)n);     // total produced (no return value needed)
+        const uint32_t chunk = act ? C.x >> kHitChunkShift : 0xFFFFFFFFu;
+        const unsigned grp = __match_any_sync(FULL, chunk);
+        const int leader = __ffs(grp) - 1;
+        uint32_t base = 0;
+        if (act && lane == leader && chunk < H.n_chunks) base = atomicAdd(&H.chunk_fill[chunk], (uint32_t)__popc(grp));
+        base = __shfl_sync(FULL, base, leader);
+        if (act && chunk < H.n_chunks) {
+          const uint32_t pos = base + __popc(grp & lt_mask);
+          if (pos < H.chunk_cap) { ok = true; o = (unsigned long long)chunk * H.chunk_cap + pos; }
+          else atomicAdd(&H.chunk_fill[H.n_chunks], 1u);               // dropped: this chunk's region is full
+        }
+      }
+      if (ok) {
+        H.history[o] = hist; H.ids[o] = ids; H.x[o] = xg[0]; H.y[o] = xg[1]; H.z[o] = xg[2];
+        H.e[o] = __uint_as_float(C.w); H.tof[o] = tof;
+      }
+      push(L_FREE, cF, act, idx);
     } else if (phase == L_RAY) {
       // ---------------------------------------------- RAY: Rayleigh deflection with words 2-3 of the step's block [R4, R20]
       const int n = min(cR, 32); const bool act = lane < n;
@@ -576,14 +767,15 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       cR -= n;
       int dest = L_NONE;
       if (act) {
-        const uint4 w = block_at(p, (p.meta >> 18) - 1u);             // the block its Woodcock step drew (rare event: recomputed)
-        rayleigh(p.d, u01(w.z), u01(w.w));
-        dest = (PHANTOM && ph_in_phantom(p)) ? L_PHANTOM : L_STEP;
+        const uint4 w = block_at(p.pair, p.meta, (p.meta >> 18) - 1u);   // the block its Woodcock step drew (rare event: recomputed)
+        const float3 r = rayleigh_dir(p.d[0], p.d[1], p.d[2], u01(w.z), u01(w.w));
+        p.d[0] = r.x; p.d[1] = r.y; p.d[2] = r.z;
+        dest = (PHANTOM && ((p.meta >> 11) & 1u)) ? L_PHANTOM : L_STEP;
         slot_store(W, idx, p, h);
       }
       push(L_STEP, cT, dest == L_STEP, idx);
-      if (use_phantom) push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
-    } else if (PHANTOM) {
+      if (PHANTOM) push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
+    } else if (PHANTOM && phase == L_PHANTOM) {
       // ---------------------------------------------- PHANTOM: Woodcock tracking in the voxel grid [R17]
       const int n = min(cP, 32); const bool act = lane < n;
       Photon p = {}; uint64_t h = 0; int idx = 0;
@@ -591,7 +783,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       cP -= n;
       int dest = L_NONE;
       if (act) {
-        const uint4 w = next_block(p);                                // [R4]
+        const uint4 w = block_at(p.pair, p.meta, p.meta >> 18); p.meta += 1u << 18;   // [R4]
         const float s = -__logf(u01(w.x)) * p.inv_mu;
         int v[3]; bool out = false; float xt[3];
 #pragma unroll
@@ -605,7 +797,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
           if (HASH) hash_ev(h, EV_PH_LEAVE, 0);
           p.meta &= ~(1u << 11); dest = L_SEARCH;
           if (misses_detector(g, p.x, p.d)) {                         // cannot reach the detector: ESCAPE without a search
-            if (HASH) { hash_ev(h, EV_ESCAPE, 0); hash_out[2ull * p.pair + (p.meta & 1u)] = h; }
+            if (HASH) { hash_ev(h, EV_ESCAPE, 0); end_hash(p.pair, p.meta, h); }
             dest = L_FREE;
           }
         }
@@ -616,8 +808,8 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
           if (mat >= 0) {
             const float4 m4 = mu_lookup(mu, T, mat, p.E);
             const float t = u01(w.y) * mu_lookup(mu, T, src.ph_major, p.E).z;
-            if (t < m4.x) { if (HASH) { hash_ev(h, EV_PH_ABSORBED, 0); hash_out[2ull * p.pair + (p.meta & 1u)] = h; } dest = L_FREE; }
-            else if (t < m4.y) dest = L_KN;
+            if (t < m4.x) { if (HASH) { hash_ev(h, EV_PH_ABSORBED, 0); end_hash(p.pair, p.meta, h); } dest = L_FREE; }
+            else if (t < m4.y) { dest = L_KN; p.ids = kNone; }
             else if (t < m4.z) { dest = L_RAY; if (HASH) hash_ev(h, EV_PH_RAYLEIGH, 0); }
           }
         }
@@ -631,29 +823,35 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
     }
     __syncwarp();
   }
-
-  // ------------------------------------------------ drain the staged hits (fewer than 32 per warp)
-  if (stage_cnt) flush_hits(H, (uint32_t)first_history, stage, (stage_head + lane) & (kStage - 1), stage_cnt, lane);
 }
 
 static int g_transport_warps = kWarps;             // warps per CTA (one CTA per SM); fewer leave room for other streams' kernels
 void set_transport_warps(int warps) { g_transport_warps = warps < 1 ? kWarps : (warps > kWarps ? kWarps : warps); }
 int transport_warps() { return g_transport_warps; }
 
-size_t transport_smem_bytes(const DevTables &T, int n_panels, bool hash) {
-  const int n_mu = T.n_staged * T.n_energies, w = g_transport_warps;
-  return (hash ? SmemLayout<true>::geom_off(w, n_mu) : SmemLayout<false>::geom_off(w, n_mu)) + panel_bytes(n_panels);
+static size_t smem_for(const DevTables &T, int n_panels, bool hash, int warps) {
+  const int n_mu = T.n_staged * T.n_energies;
+  return (hash ? SmemLayout<true>::geom_off(warps, n_mu) : SmemLayout<false>::geom_off(warps, n_mu)) + panel_bytes(n_panels + 1);
+}
+size_t transport_smem_bytes(const DevTables &T, int n_panels, bool hash) { return smem_for(T, n_panels, hash, g_transport_warps); }
+
+// The tables are staged in shared memory next to the per-warp pools: with many materials or a fine energy grid the CTA
+// gives up warps until everything fits (0 = it cannot fit at all).
+int transport_warps_that_fit(const DevTables &T, int n_panels, bool hash, size_t smem_limit) {
+  int w = g_transport_warps;
+  while (w >= 4 && smem_for(T, n_panels, hash, w) > smem_limit) --w;
+  return w >= 4 ? w : 0;
 }
 
 cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
-                             unsigned long long *work_counter, int sm_count, cudaStream_t stream) {
+                             unsigned long long *work_counter, int sm_count, int warps, cudaStream_t stream) {
   const int n_panels = host_geom.n_panels, planar_hint = host_geom.planar;
   const DevGeomHead &head = host_geom;
   const DevPanel *panels = reinterpret_cast<const DevPanel *>(reinterpret_cast<const char *>(geom) +
                                                             (reinterpret_cast<const char *>(&host_geom.panel[0]) - reinterpret_cast<const char *>(&host_geom)));
-  const size_t smem = transport_smem_bytes(T, n_panels, hash_out != nullptr);
-  const int threads = 32 * g_transport_warps;
+  const size_t smem = smem_for(T, n_panels, hash_out != nullptr, warps);
+  const int threads = 32 * warps;
   const uint64_t want = (2 * n_pairs + threads - 1) / threads;
   const uint64_t resident = (uint64_t)sm_count;                      // persistent grid: one CTA per SM
   PhiloxKeys key;                                                     // [R1] round keys: key + r * Weyl constants
@@ -680,17 +878,17 @@ cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, cons
     kernel<<<blocks, threads, smem, stream>>>(head, panels, T, src, first_history, n_pairs, key, H, hash_out, work_counter);
     return cudaSuccess;
   };
-  // specialised builds for the shapes the five configs use (point source or voxel map + phantom, planar ring);
-  // anything else runs the generic build of the same code
-  const bool planar = planar_hint != 0;
-#define GPET_DISPATCH(H)                                                                                              \
-  do {                                                                                                                \
-    if (!phantom && src.kind == 0 && planar && pretest) e = launch(transport_wavefront_kernel<H, false, 0, 1, true>);  \
-    else if (!phantom && src.kind == 0 && planar) e = launch(transport_wavefront_kernel<H, false, 0, 1, false>);      \
-    else if (phantom && planar) e = launch(transport_wavefront_kernel<H, true, 1, 1, false>);                         \
-    else if (phantom) e = launch(transport_wavefront_kernel<H, true, 1, -1, false>);                                  \
-    else if (pretest) e = launch(transport_wavefront_kernel<H, false, -1, -1, true>);                                 \
-    else e = launch(transport_wavefront_kernel<H, false, -1, -1, false>);                                             \
+  // specialised builds for the shapes the five configs use (point source or voxel map + phantom, in a repetition-mode
+  // ring); anything else runs the generic build of the same code
+  const bool ring = planar_hint != 0 && host_geom.ring != 0 && host_geom.ring_edge_h > 0.0f;
+#define GPET_DISPATCH(H)                                                                                                    \
+  do {                                                                                                                      \
+    if (!phantom && src.kind == 0 && ring && pretest) e = launch(transport_wavefront_kernel<H, false, 0, 1, true, true>);    \
+    else if (!phantom && src.kind == 0 && ring) e = launch(transport_wavefront_kernel<H, false, 0, 1, false, true>);        \
+    else if (phantom && ring) e = launch(transport_wavefront_kernel<H, true, 1, 1, false, true>);                           \
+    else if (phantom) e = launch(transport_wavefront_kernel<H, true, 1, -1, false, false>);                                 \
+    else if (pretest) e = launch(transport_wavefront_kernel<H, false, -1, -1, true, false>);                                \
+    else e = launch(transport_wavefront_kernel<H, false, -1, -1, false, false>);                                            \
   } while (0)
   if (hash_out) GPET_DISPATCH(true); else GPET_DISPATCH(false);
 #undef GPET_DISPATCH
@@ -718,7 +916,7 @@ __global__ void locate_kernel(const DevGeom *geom, int64_t n, const float *xyz, 
       const double a = r0 * P[3] + r1 * P[4] + r2 * P[5], b = r0 * P[6] + r1 * P[7] + r2 * P[8], c = r0 * P[9] + r1 * P[10] + r2 * P[11];
       const long long qa = (long long)floor(a * 1048576.0) + g.hWq, qb = (long long)floor(b * 1048576.0) + g.hHq, qc = (long long)floor(c * 1048576.0);
       if (qa < 0 || qa >= g.Wq || qb < 0 || qb >= g.Hq || qc < 0 || qc >= g.Dq) continue;
-      lattice_lookup(g, (int)qa, (int)qb, (int)qc, out);
+      lattice_lookup(g, g.layer, (int)qa, (int)qb, (int)qc, out);
       if (out != kNone) out |= (uint32_t)p << 26;
       break;
     }

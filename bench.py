@@ -3,7 +3,7 @@
 
 A *step* is one pass of the whole hot path (gpet_simulate + gpet_digitize: source, panel search, in-panel
 Woodcock transport, hits, adder, blur, window, time sort, coincidences) over one batch of synthetic input.
-The timed steps run in turn on one stream (the transport kernel with its full 24-warp CTA per SM).  After the timed
+The timed steps run in turn on one stream (the transport kernel with its full CTA (20 warps) per SM).  After the timed
 region the same steps are also run as a two-stream pipeline -- the transport kernel of step k+1 (bound by instruction
 issue) beside the digitizer of step k (bound by HBM latency) -- and reported under "pipelined";
 `--overlap` makes that pipeline the timed headline instead.
@@ -148,8 +148,21 @@ def run_ours(args):
 
     run, desc = workload(args.config, args.pairs)
     n = run.n_pairs
-    first, _ = sharding.history_range(rank, world, n)
-    n_total = sharding.total_pairs(world, n)
+    # Every step simulates its OWN histories: batch b of the job is the time slice [b n world, (b+1) n world) of one long
+    # acquisition [R16], rank r takes the r-th n histories of it (disjoint ranges, aligned to time slices: no coincidence
+    # window straddles two ranks or two batches).
+    from dataclasses import replace
+    run = replace(run, source=replace(run.source, pairs_per_time_slice=n))
+    n_batches_max = args.warmup + 3 * args.steps + args.e2e_steps + 64
+    n_total = sharding.total_pairs(world, n) * n_batches_max
+    batch_no = [0]
+
+    def next_first():
+        first, _ = sharding.history_range(rank, world, n)
+        first += batch_no[0] * sharding.total_pairs(world, n)
+        batch_no[0] += 1
+        return first
+
     tables = W.tables()
     geom, mats, src = api.gpet_geometry_create(run.geometry), api.gpet_materials_load(tables), api.DeviceSource(run.source)
     cap = int(n * args.hits_per_pair) + 1024
@@ -163,7 +176,7 @@ def run_ours(args):
     scratch = [torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda") for _ in range(nbuf)]
     s_a = torch.cuda.Stream()
     s_b = torch.cuda.Stream() if args.overlap else s_a
-    warps = api.gpet_set_transport_warps(args.transport_warps if args.transport_warps else 24)
+    warps = api.gpet_set_transport_warps(args.transport_warps if args.transport_warps else 0)
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
 
@@ -181,6 +194,7 @@ def run_ours(args):
                 hits[i].reset()
                 if record:
                     e[0].record(s_a)
+                first = next_first()
                 api.gpet_simulate(geom, mats, src, first, n, run.seed, hits[i], s_a)
                 if record:
                     e[1].record(s_a)
@@ -226,19 +240,23 @@ def run_ours(args):
     transport_ms = sum(e[0].elapsed_time(e[1]) for e in t_events) / len(t_events)
     digitize_ms = sum(e[2].elapsed_time(e[3]) for e in t_events) / len(t_events)
     n_hits, n_coinc = hits[0].count(), int(coinc[0].n_coinc.item())
-    if hits[0].dropped():
-        raise SystemExit(f"hit buffer overflow ({hits[0].dropped()} hits dropped); raise --hits-per-pair")
-    value = n_total * args.steps / (ms_total * 1e-3)
+    for hb, cb in zip(hits, coinc):
+        if hb.dropped():
+            raise SystemExit(f"hit buffer overflow ({hb.dropped()} hits dropped); raise --hits-per-pair")
+        if int(cb.n_coinc.item()) > cb.capacity:
+            raise SystemExit("coincidence buffer overflow")
+    value = sharding.total_pairs(world, n) * args.steps / (ms_total * 1e-3)
 
-    # ---- the two halves alone (untimed extra, not part of `value`): serial steps with the full 24-warp transport CTA
+    # ---- the two halves alone (untimed extra, not part of `value`): serial steps with the full transport CTA
     alone = None
     if args.overlap:
-        api.gpet_set_transport_warps(24)
+        api.gpet_set_transport_warps(0)
         st = torch.cuda.current_stream()
         ta, tb = [], []
         for k in range(8):
             hits[0].reset()
             x, y, z = ev(), ev(), ev()
+            first = next_first()
             x.record(st); api.gpet_simulate(geom, mats, src, first, n, run.seed, hits[0], st); y.record(st)
             api.gpet_digitize(src, run.seed, n_total, first, n, hits[0], cap, run.digitizer, scratch[0], None, coinc[0], st); z.record(st)
             torch.cuda.synchronize()
@@ -248,7 +266,7 @@ def run_ours(args):
     # ---- the same steps as a two-stream pipeline (extra, after the timed region; not part of `value`)
     pipelined = None
     if not args.overlap and not args.no_pipelined:
-        pw = api.gpet_set_transport_warps(args.transport_warps if args.transport_warps else 24)
+        pw = api.gpet_set_transport_warps(args.transport_warps if args.transport_warps else 0)
         hits.append(api.HitBuffer.allocate_chunked(n, args.hits_per_pair)); coinc.append(api.CoincBuffer.allocate(cap // 4))
         scratch.append(torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda"))
         s_b2 = torch.cuda.Stream()
@@ -261,6 +279,7 @@ def run_ours(args):
                     s_a.wait_event(dig_done[i])
                 with torch.cuda.stream(s_a):
                     hits[i].reset()
+                    first = next_first()
                     api.gpet_simulate(geom, mats, src, first, n, run.seed, hits[i], s_a)
                 sim_done[i].record(s_a)
                 s_b2.wait_event(sim_done[i])
@@ -274,25 +293,39 @@ def run_ours(args):
         p0.record(s_a); pipe(args.steps); p1.record(s_a)
         barrier()
         p_ms = sharding.max_over_ranks(p0.elapsed_time(p1))
-        assert int(coinc[1].n_coinc.item()) == n_coinc and int(coinc[0].n_coinc.item()) == n_coinc
-        pipelined = {"value": n_total * args.steps / (p_ms * 1e-3), "unit": UNIT, "ms_per_step": p_ms / args.steps, "steps": args.steps,
+        assert hits[1].dropped() == 0 and 0 < int(coinc[1].n_coinc.item()) <= coinc[1].capacity
+        pipelined = {"value": sharding.total_pairs(world, n) * args.steps / (p_ms * 1e-3), "unit": UNIT, "ms_per_step": p_ms / args.steps, "steps": args.steps,
                      "transport_warps_per_sm": pw,
                      "note": "gpet_simulate(k+1) on one stream beside gpet_digitize(k) on another, two hit buffers; same results"}
-    api.gpet_set_transport_warps(24)                             # the host-buffer path below is one batch at a time
+    api.gpet_set_transport_warps(0)                             # the host-buffer path below is one batch at a time
 
-    # ---- end to end through the C ABI with HOST buffers (gpet_run_host): copies inside the timed region
-    host = None
-    for _ in range(max(1, min(args.warmup, 2))):
-        host, counts = api.gpet_run_host(geom, mats, run.source, n_total, first, n, run.seed, run.digitizer, args.hits_per_pair, host=host)
+    # ---- end to end through the C ABI with HOST buffers (gpet_pipeline_*: the call a user makes for a stream of batches):
+    # every step's list-mode coincidences are copied to pinned host memory inside the timed region; two batches in flight
+    # (the copy of step k rides a copy stream while step k+1 computes)
+    pipe = api.Pipeline(geom, mats, run.source, run.digitizer, n_total, n, args.hits_per_pair, 0, 2)
+    host = [api.HostOutputs(int(n * 0.25) + 1024) for _ in range(2)]
+
+    def e2e_steps(k_steps):
+        pipe.submit(next_first(), n, run.seed)
+        cnt = None
+        for k in range(k_steps):
+            if k + 1 < k_steps:
+                pipe.submit(next_first(), n, run.seed)
+            cnt = pipe.collect(host[k & 1])
+            if cnt["n_coinc"] > host[k & 1].cap:
+                raise SystemExit("host coincidence buffer too small")
+        return cnt
+
+    e2e_steps(max(2, min(args.warmup, 3)))
     barrier()
     t0 = time.perf_counter()
-    for _ in range(args.e2e_steps):
-        host, counts = api.gpet_run_host(geom, mats, run.source, n_total, first, n, run.seed, run.digitizer, args.hits_per_pair, host=host)
+    counts = e2e_steps(args.e2e_steps)
     barrier()
     e2e_s = sharding.max_over_ranks(time.perf_counter() - t0)
-    e2e_value = n_total * args.e2e_steps / e2e_s
+    e2e_value = sharding.total_pairs(world, n) * args.e2e_steps / e2e_s
     h2d = 104 + 32 + (run.source.phantom_material.size if run.source.phantom_material is not None else 0)
-    d2h = 24 + counts["n_coinc"] * 40
+    d2h = 28 + counts["n_coinc"] * 40
+    del pipe
 
     if rank != 0:
         if world > 1:
@@ -315,7 +348,7 @@ def run_ours(args):
                 "frac": achieved / peak_alu if achieved else None, "traffic": traffic,
                 "alone": ({"transport_ms": alone["transport_ms"], "achieved": alg * n / (alone["transport_ms"] * 1e-3),
                            "frac": alg * n / (alone["transport_ms"] * 1e-3) / peak_alu,
-                           "note": "same kernel with its full 24-warp CTA and nothing else on the GPU (8 serial steps after the timed region)"}
+                           "note": "same kernel with its full CTA (20 warps) and nothing else on the GPU (8 serial steps after the timed region)"}
                           if alone and alg else None),
                 "note": f"{alg} algorithmic thread-instr/pair (DESIGN.md 6) x {n} pairs / {transport_ms:.3f} ms; peak = 148 SMs x 128 lanes x "
                         f"{peaks['sm_max_mhz']} MHz ({peaks['source']} max SM clock); hbm {peaks['hbm_gbs']} GB/s of {peaks['source']}",
@@ -356,7 +389,7 @@ def run_ours(args):
                    "hits_per_step": n_hits, "coincidences_per_step": n_coinc},
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": args.e2e_steps,
-                "api": "gpet_run_host (host outputs: coincidence list-mode + counters)"},
+                "api": "gpet_pipeline_submit / gpet_pipeline_collect (host outputs per step: coincidence list-mode + counters; two batches in flight)"},
         "roofline": roofline, "roofline_digitizer": roofline_digi, "pipelined": pipelined, "cpu_baseline": cpu,
     }))
     if world > 1:
@@ -372,13 +405,13 @@ def main():
     ap.add_argument("--config", default="C1")
     ap.add_argument("--pairs", type=int, default=None, help="pairs per step per GPU (default: the config's own, 1e7 for C1)")
     ap.add_argument("--hits-per-pair", type=float, default=1.2)
-    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--cpu-pairs", type=int, default=10_000_000)
     ap.add_argument("--ref-pairs", type=int, default=2_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-pipelined", action="store_true", help="skip the extra two-stream pipeline measurement")
     ap.add_argument("--overlap", action="store_true", help="time the two-stream pipeline as the headline instead of the serial steps")
-    ap.add_argument("--transport-warps", type=int, default=0, help="warps per transport CTA (default 24; fewer leave more of each SM to the other stream in the pipeline)")
+    ap.add_argument("--transport-warps", type=int, default=0, help="warps per transport CTA (default 20; fewer leave more of each SM to the other stream in the pipeline)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -25,7 +25,7 @@ extern "C" {
 #define GPET_E_INVALID_ARG  -1   /* NULL pointer, count out of range                                   */
 #define GPET_E_GEOMETRY     -2   /* lattice overhangs its module, non-positive size, too many panels  */
 #define GPET_E_TABLE        -3   /* negative or non-finite mu, fewer than 2 energies                  */
-#define GPET_E_OVERFLOW     -4   /* scratch too small                                                 */
+#define GPET_E_OVERFLOW     -4   /* scratch too small, hits dropped in a library-owned buffer          */
 #define GPET_E_CUDA         -5   /* CUDA runtime error or no device                                   */
 
 #define GPET_MAX_PANELS   63
@@ -209,15 +209,46 @@ typedef struct {                  /* HOST outputs (pinned memory recommended); a
   gpet_coincidences coinc;
 } gpet_host_outputs;
 
-/* Whole path for one batch with host-side outputs: allocates device buffers sized hits_per_pair *
- * n_pairs, runs gpet_simulate + gpet_digitize, copies the requested outputs to the HOST arrays
- * (counts in *n_hits, *n_singles, *n_coinc; capacities limit what is copied) and synchronises.
- * phantom_material inside src is a HOST pointer here (copied to the device by the call). */
+/* Whole path for one batch with host-side outputs: runs gpet_simulate + gpet_digitize on library-owned device
+ * buffers sized hits_per_pair * n_pairs, copies the requested outputs to the HOST arrays (counts in *n_hits,
+ * *n_singles, *n_coinc; capacities limit what is copied) and synchronises.  phantom_material inside src is a HOST
+ * pointer here (copied to the device by the call).  The buffers are kept for the next call of the same shape
+ * (gpet_shutdown frees them).  One batch at a time: for a stream of batches use the pipeline below. */
 int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, const gpet_source *src,
                   uint64_t n_pairs_total, uint64_t first_history, uint64_t n_pairs, uint64_t seed,
                   const gpet_digitizer *dig, double hits_per_pair, gpet_host_outputs *out);
 
-/* Tuning: warps per transport CTA (one persistent CTA per SM), 1..24, default 24; returns the value in force.  Fewer
+/* ---------------------------------------------------------------- a stream of batches with HOST outputs */
+/* The paper's runs are long acquisitions written out as list-mode coincidences ("list-mode output");
+ * a run of N pairs is cut into batches (time slices [R16]) and each batch's list is copied to the host.  The pipeline
+ * keeps TWO batches in flight: while the list-mode output of batch k crosses PCIe on a copy stream, batch k+1 is
+ * transported and digitized on the compute stream, so the copy costs no time as long as it is shorter than a batch.
+ *   gpet_pipeline_create(..., n_slots = 2, &p);
+ *   gpet_pipeline_submit(p, first_0, n, seed);
+ *   for k: gpet_pipeline_submit(p, first_{k+1}, n, seed);  gpet_pipeline_collect(p, &out_k);   // out_k = batch k
+ *   gpet_pipeline_collect(p, &out_last);  gpet_pipeline_destroy(p);
+ * Handles, geometry and materials must outlive the pipeline.  src->phantom_material is a HOST pointer (uploaded once by
+ * create; voxel values above the number of loaded materials are rejected).  `want` says which outputs besides the
+ * coincidences will be asked for (it sizes the device buffers): without GPET_WANT_HITS the hits stay on the device in
+ * the chunked layout.  submit only enqueues work and returns; at most n_slots (1 or 2) batches may be in flight.
+ * collect waits for the OLDEST batch in flight, copies its outputs to the HOST arrays of `out` (as gpet_run_host does;
+ * pinned memory recommended) and returns its counts; GPET_E_OVERFLOW if the batch dropped hits (raise hits_per_pair). */
+#define GPET_WANT_HITS    1u
+#define GPET_WANT_SINGLES 2u
+#define GPET_WANT_HASH    4u
+typedef struct gpet_pipeline gpet_pipeline;
+int gpet_pipeline_create(const gpet_geometry *g, const gpet_materials *m, const gpet_source *src, const gpet_digitizer *dig,
+                         uint64_t n_pairs_total, uint64_t max_pairs_per_batch, double hits_per_pair, uint32_t want,
+                         int32_t n_slots, gpet_pipeline **out);
+int gpet_pipeline_submit(gpet_pipeline *p, uint64_t first_history, uint64_t n_pairs, uint64_t seed);
+int gpet_pipeline_collect(gpet_pipeline *p, gpet_host_outputs *out);
+int gpet_pipeline_destroy(gpet_pipeline *p);
+
+/* Frees what the library keeps between calls (gpet_run_host's buffers, the work counters of gpet_simulate).  Handles
+ * created by the caller stay valid; any later call re-creates what it needs. */
+int gpet_shutdown(void);
+
+/* Tuning: warps per transport CTA (one persistent CTA per SM), 1..20, 0 = default 20; returns the value in force.  Fewer
  * warps leave registers and thread slots on every SM for kernels of OTHER streams: with 16, gpet_digitize of batch k on
  * one stream runs beside gpet_simulate of batch k+1 on another (the transport kernel is bound by instruction issue, the
  * digitizer by HBM latency), which is how bench.py pipelines its steps.  Applies to later gpet_simulate calls. */

@@ -71,7 +71,8 @@ class _HostOutputs(C.Structure):
 EXPORTS = ("gpet_geometry_create", "gpet_geometry_destroy", "gpet_geometry_panel_pose", "gpet_geometry_open_faces", "gpet_geometry_bore_radius", "gpet_geometry_locate",
            "gpet_materials_load", "gpet_materials_destroy", "gpet_activity_create", "gpet_activity_destroy",
            "gpet_simulate", "gpet_digitize_scratch_bytes", "gpet_digitize", "gpet_run_host", "gpet_last_error",
-           "gpet_launch_count", "gpet_set_transport_warps")
+           "gpet_launch_count", "gpet_set_transport_warps", "gpet_pipeline_create", "gpet_pipeline_submit", "gpet_pipeline_collect",
+           "gpet_pipeline_destroy", "gpet_shutdown")
 
 _lib = None
 
@@ -102,6 +103,10 @@ def lib():
                                     vp, C.c_size_t, C.POINTER(_Singles), C.POINTER(_Coinc), vp]
         L.gpet_run_host.argtypes = [vp, vp, C.POINTER(_Source), u64, u64, u64, u64, C.POINTER(_Digitizer), C.c_double,
                                     C.POINTER(_HostOutputs)]
+        L.gpet_pipeline_create.argtypes = [vp, vp, C.POINTER(_Source), C.POINTER(_Digitizer), u64, u64, C.c_double, C.c_uint32, i32, C.POINTER(vp)]
+        L.gpet_pipeline_submit.argtypes = [vp, u64, u64, u64]
+        L.gpet_pipeline_collect.argtypes = [vp, C.POINTER(_HostOutputs)]
+        L.gpet_pipeline_destroy.argtypes = [vp]
         L.gpet_last_error.restype = C.c_char_p
         L.gpet_launch_count.restype = u64
         L.gpet_set_transport_warps.argtypes = [i32]
@@ -119,7 +124,7 @@ def gpet_launch_count() -> int:
 
 
 def gpet_set_transport_warps(warps: int) -> int:
-    """Warps per transport CTA (1..24, 0 = default 24); returns the value in force."""
+    """Warps per transport CTA (1..20, 0 = default 20); returns the value in force."""
     return int(lib().gpet_set_transport_warps(int(warps)))
 
 
@@ -404,34 +409,87 @@ def gpet_digitize(source: DeviceSource, seed: int, n_pairs_total: int, first_his
                                C.byref(cs), _stream_ptr(stream)))
 
 
+GPET_WANT_HITS, GPET_WANT_SINGLES, GPET_WANT_HASH = 1, 2, 4
+
+
+class HostOutputs:
+    """Pinned host arrays for one batch's outputs (mirror of gpet_host_outputs) + the three counters."""
+
+    def __init__(self, cap: int, n_pairs: int = 0, want_hits=False, want_singles=False, want_hash=False):
+        import torch
+        pin = lambda dt, n=cap: torch.empty(n, dtype=dt, pin_memory=True)
+        self.cap = cap
+        self.counts = torch.zeros(3, dtype=torch.int64, pin_memory=True)
+        self.coinc = [pin(torch.int32) for _ in range(4)] + [pin(torch.float32) for _ in range(3)] + [pin(torch.float64)]
+        self.hits = [pin(torch.int32) for _ in range(2)] + [pin(torch.float32) for _ in range(5)] if want_hits else None
+        self.singles = ([pin(torch.int32) for _ in range(2)] + [pin(torch.float32) for _ in range(4)] + [pin(torch.float64)]
+                        if want_singles else None)
+        self.hash = pin(torch.int64, 2 * n_pairs) if want_hash else None
+        cnt = self.counts
+        out = _HostOutputs()
+        if self.hits is not None:
+            out.hits = _Hits(*[t.data_ptr() for t in self.hits], cap, cnt[0:].data_ptr(), None)
+        else:
+            out.hits = _Hits(None, None, None, None, None, None, None, 0, cnt[0:].data_ptr(), None)
+        if self.hash is not None:
+            out.hits.outcome_hash = self.hash.data_ptr()
+        if self.singles is not None:
+            out.singles = _Singles(*[t.data_ptr() for t in self.singles], cap, cnt[1:].data_ptr())
+        else:
+            out.singles = _Singles(None, None, None, None, None, None, None, 0, cnt[1:].data_ptr())
+        out.coinc = _Coinc(*[t.data_ptr() for t in self.coinc], cap, cnt[2:].data_ptr())
+        self.struct = out
+
+    def want(self) -> int:
+        return (GPET_WANT_HITS if self.hits is not None else 0) | (GPET_WANT_SINGLES if self.singles is not None else 0) | \
+               (GPET_WANT_HASH if self.hash is not None else 0)
+
+    def result(self):
+        c = self.counts
+        return dict(n_hits=int(c[0]), n_singles=int(c[1]), n_coinc=int(c[2]))
+
+    def __getitem__(self, k):            # dict-style access used by older callers: host["coinc"], host["hits"], ...
+        return getattr(self, k)
+
+
+class Pipeline(_Handle):
+    """gpet_pipeline: a stream of batches with host outputs, two in flight (include/gpet.h)."""
+    _destroy = "gpet_pipeline_destroy"
+
+    def __init__(self, geom: Geometry, mats: Materials, src, dig, n_pairs_total: int, max_pairs_per_batch: int,
+                 hits_per_pair: float = 2.0, want: int = 0, n_slots: int = 2):
+        self.geom, self.mats = geom, mats                              # keep the handles alive
+        self.activity = gpet_activity_create(src.activity, src.dims) if src.kind == 1 else None
+        self.phantom = None
+        if src.kind == 1 and src.phantom_material is not None:
+            self.phantom = np.ascontiguousarray(src.phantom_material, np.uint8)
+        s = _source_struct(src, self.activity.ptr if self.activity else None, self.phantom.ctypes.data if self.phantom is not None else None)
+        d = _Digitizer(dig.blur_fwhm_frac, dig.blur_ref_keV, dig.e_lo_keV, dig.e_hi_keV, dig.window_ns, dig.readout_level)
+        out = C.c_void_p()
+        _check(lib().gpet_pipeline_create(geom.ptr, mats.ptr, C.byref(s), C.byref(d), n_pairs_total, max_pairs_per_batch,
+                                          hits_per_pair, want, n_slots, C.byref(out)))
+        super().__init__(out.value)
+
+    def submit(self, first_history: int, n_pairs: int, seed: int) -> None:
+        _check(lib().gpet_pipeline_submit(self.ptr, first_history, n_pairs, seed))
+
+    def collect(self, host: HostOutputs) -> dict:
+        _check(lib().gpet_pipeline_collect(self.ptr, C.byref(host.struct)))
+        return host.result()
+
+
+def gpet_shutdown() -> None:
+    _check(lib().gpet_shutdown())
+
+
 def gpet_run_host(geom: Geometry, mats: Materials, src, n_pairs_total: int, first_history: int, n_pairs: int, seed: int, dig,
                   hits_per_pair: float = 2.0, want_hits: bool = False, want_singles: bool = False, want_hash: bool = False,
                   host=None):
     """Whole path with HOST outputs (pinned torch tensors, reused when `host` is passed back in).
-    src: workloads.Source (its phantom map is a host array here).  Returns (host buffers dict, counts)."""
-    import torch
+    src: workloads.Source (its phantom map is a host array here).  Returns (HostOutputs, counts)."""
     cap = int(n_pairs * hits_per_pair) + 1024
-    pin = lambda dt, n=cap: torch.empty(n, dtype=dt, pin_memory=True)
-    if host is None or host["cap"] < cap:
-        host = {"cap": cap, "counts": torch.zeros(3, dtype=torch.int64, pin_memory=True)}
-        host["coinc"] = [pin(torch.int32) for _ in range(4)] + [pin(torch.float32) for _ in range(3)] + [pin(torch.float64)]
-        host["hits"] = [pin(torch.int32) for _ in range(2)] + [pin(torch.float32) for _ in range(5)] if want_hits else None
-        host["singles"] = ([pin(torch.int32) for _ in range(2)] + [pin(torch.float32) for _ in range(4)] + [pin(torch.float64)]
-                           if want_singles else None)
-        host["hash"] = pin(torch.int64, 2 * n_pairs) if want_hash else None
-    cnt = host["counts"]
-    out = _HostOutputs()
-    if host["hits"] is not None:
-        out.hits = _Hits(*[t.data_ptr() for t in host["hits"]], cap, cnt[0:].data_ptr(), None)
-    else:
-        out.hits = _Hits(None, None, None, None, None, None, None, 0, cnt[0:].data_ptr(), None)
-    if host["hash"] is not None:
-        out.hits.outcome_hash = host["hash"].data_ptr()
-    if host["singles"] is not None:
-        out.singles = _Singles(*[t.data_ptr() for t in host["singles"]], cap, cnt[1:].data_ptr())
-    else:
-        out.singles = _Singles(None, None, None, None, None, None, None, 0, cnt[1:].data_ptr())
-    out.coinc = _Coinc(*[t.data_ptr() for t in host["coinc"]], cap, cnt[2:].data_ptr())
+    if host is None or host.cap < cap:
+        host = HostOutputs(cap, n_pairs, want_hits, want_singles, want_hash)
     activity = gpet_activity_create(src.activity, src.dims) if src.kind == 1 else None
     ph = None
     if src.kind == 1 and src.phantom_material is not None:
@@ -439,5 +497,5 @@ def gpet_run_host(geom: Geometry, mats: Materials, src, n_pairs_total: int, firs
     s = _source_struct(src, activity.ptr if activity else None, ph.ctypes.data if ph is not None else None)
     d = _Digitizer(dig.blur_fwhm_frac, dig.blur_ref_keV, dig.e_lo_keV, dig.e_hi_keV, dig.window_ns, dig.readout_level)
     _check(lib().gpet_run_host(geom.ptr, mats.ptr, C.byref(s), n_pairs_total, first_history, n_pairs, seed, C.byref(d),
-                               hits_per_pair, C.byref(out)))
-    return host, dict(n_hits=int(cnt[0]), n_singles=int(cnt[1]), n_coinc=int(cnt[2]))
+                               hits_per_pair, C.byref(host.struct)))
+    return host, host.result()

@@ -54,6 +54,16 @@ static int sm_count() {
 
 // ---------------------------------------------------------------- geometry
 static long long quant(float x) { return llrint((double)x * 1048576.0); }   // [R7]
+// the multiply-high division of the lattice lookup (QDiv) against plain division at every cell boundary below n_max
+static bool qdiv_exact(uint32_t d, uint32_t n_max) {
+  const QDiv q = qdiv_make(d);
+  for (uint64_t k = 0; k * d <= (uint64_t)n_max + d; ++k)
+    for (int64_t n = (int64_t)(k * d) - 1; n <= (int64_t)(k * d) + 1; ++n) {
+      if (n < 0 || n > (int64_t)n_max) continue;
+      if ((uint32_t)(((uint64_t)(uint32_t)n * q.magic) >> 32 >> q.shift) != (uint32_t)(n / d)) return false;
+    }
+  return true;
+}
 
 extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry **out) {
   if (!d || !out || !d->layers) return fail(GPET_E_INVALID_ARG, "gpet_geometry_create: NULL argument");
@@ -65,10 +75,11 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
   long long ms[2], mp[2];
   for (int a = 0; a < 2; ++a) {
     ms[a] = quant(d->module_size_mm[a]); mp[a] = quant(d->module_pitch_mm[a]);
-    if (d->n_modules[a] < 1 || d->n_modules[a] > 8 || ms[a] <= 0 || mp[a] < ms[a]) {
+    if (d->n_modules[a] < 1 || d->n_modules[a] > 8 || ms[a] < 2 || mp[a] < ms[a] || mp[a] >= (1ll << 30) || (long long)d->n_modules[a] * mp[a] >= (1ll << 30) ||
+        !qdiv_exact((uint32_t)mp[a], (uint32_t)(d->n_modules[a] * mp[a]))) {
       delete g; return fail(GPET_E_GEOMETRY, "module grid axis %d: n=%d size=%g pitch=%g", a, d->n_modules[a], d->module_size_mm[a], d->module_pitch_mm[a]);
     }
-    G.nmod[a] = d->n_modules[a]; G.msq[a] = (int)ms[a]; G.mpq[a] = (int)mp[a]; G.inv_mpq[a] = (float)((1.0 - 1e-6) / (double)mp[a]);
+    G.nmod[a] = d->n_modules[a]; G.msq[a] = (int)ms[a]; G.mpq[a] = (int)mp[a]; { const QDiv qd = qdiv_make((uint32_t)mp[a]); G.mp_magic[a] = qd.magic; G.mp_shift[a] = qd.shift; }
   }
   const long long Wq = (G.nmod[0] - 1) * mp[0] + ms[0], Hq = (G.nmod[1] - 1) * mp[1] + ms[1];
   long long c = 0;
@@ -84,12 +95,12 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
     G.det_mask |= 1u << L.cmat; if (L.gmat >= 0) G.det_mask |= 1u << L.gmat;
     for (int a = 0; a < 2; ++a) {
       const long long p = quant(s.pitch_mm[a]), gp = quant(s.reflector_mm[a]), of = quant(s.offset_mm[a]);
-      if (s.n_crystals[a] < 1 || p <= 0 || gp < 0 || gp >= p || of < 0 || of + s.n_crystals[a] * p > ms[a]) {
+      if (s.n_crystals[a] < 1 || p < 2 || p >= (1ll << 30) || !qdiv_exact((uint32_t)p, (uint32_t)ms[a]) || gp < 0 || gp >= p || of < 0 || of + s.n_crystals[a] * p > ms[a]) {
         delete g; return fail(GPET_E_GEOMETRY, "layer %d axis %d: lattice (n=%d pitch=%g gap=%g offset=%g) does not fit its %g mm module",
                               l, a, s.n_crystals[a], s.pitch_mm[a], s.reflector_mm[a], s.offset_mm[a], d->module_size_mm[a]);
       }
       L.n[a] = s.n_crystals[a]; L.pitch[a] = (int)p; L.off[a] = (int)of;
-      L.lo[a] = (int)(gp >> 1); L.hi[a] = (int)(p - (gp - (gp >> 1))); L.inv_pitch[a] = (float)((1.0 - 1e-6) / (double)p);
+      L.lo[a] = (int)(gp >> 1); L.hi[a] = (int)(p - (gp - (gp >> 1))); { const QDiv qd = qdiv_make((uint32_t)p); L.magic[a] = qd.magic; L.n[a] |= (int)(qd.shift << 24); }
     }
     if ((long long)s.n_crystals[0] * s.n_crystals[1] > 8192) { delete g; return fail(GPET_E_GEOMETRY, "layer %d: more than 8192 crystals", l); }
   }
@@ -469,90 +480,195 @@ extern "C" int gpet_digitize(const gpet_source *src, uint64_t seed, uint64_t n_p
 }
 
 // ---------------------------------------------------------------- whole path with host outputs
+// One device SLOT holds everything a batch needs (hit buffer, singles, coincidences, scratch, counters); a pipeline owns
+// two of them, one compute stream and one copy stream per slot.  Batch k+1 is transported and digitized while the
+// list-mode output of batch k travels to the host.
 namespace {
 struct DevArena {                      // bump allocator over one cudaMalloc
   char *base = nullptr; size_t size = 0, used = 0;
   template <class T> T *take(size_t n) { used = (used + 255) & ~(size_t)255; T *p = reinterpret_cast<T *>(base + used); used += sizeof(T) * n; return p; }
 };
+struct Slot {
+  DevArena A; gpet_hits H; gpet_singles S; gpet_coincidences C; void *scratch = nullptr; size_t scratch_bytes = 0;
+  uint64_t cap = 0, n_chunks = 0, n_pairs = 0; bool chunked = true, busy = false;
+  cudaStream_t copy = nullptr; cudaEvent_t computed = nullptr, counted = nullptr;
+  uint64_t *host_counts = nullptr;     // pinned: n_hits, n_singles, n_coinc, dropped
+};
+}
+struct gpet_pipeline {
+  const gpet_geometry *g; const gpet_materials *m; gpet_source src; gpet_digitizer dig;
+  uint64_t n_pairs_total, max_pairs; double hits_per_pair; uint32_t want;
+  uint8_t *phantom_dev = nullptr; cudaStream_t compute = nullptr; Slot slot[2]; uint64_t submitted = 0, collected = 0;
+};
+
+static void slot_release(Slot &s) {
+  if (s.A.base) cudaFree(s.A.base);
+  if (s.copy) cudaStreamDestroy(s.copy);
+  if (s.computed) cudaEventDestroy(s.computed);
+  if (s.counted) cudaEventDestroy(s.counted);
+  if (s.host_counts) cudaFreeHost(s.host_counts);
+  s = Slot();
 }
 
+static int slot_create(Slot &s, uint64_t max_pairs, double hits_per_pair, uint32_t want) {
+  // hits that stay on the device use the chunked layout (shared-memory sort per chunk in the digitizer); hits the caller
+  // wants on the host use the dense one, which is what gpet_host_outputs describes
+  s.chunked = !(want & GPET_WANT_HITS);
+  s.n_chunks = (max_pairs + kHitChunkPairs - 1) / kHitChunkPairs;
+  uint64_t chunk_cap = (uint64_t)ceil((double)kHitChunkPairs * hits_per_pair);
+  if (chunk_cap > kHitChunkCapMax) chunk_cap = kHitChunkCapMax;
+  const uint64_t cap = s.chunked ? s.n_chunks * chunk_cap : (uint64_t)((double)max_pairs * hits_per_pair) + 1024;
+  if (cap >= (1ull << 32)) return fail(GPET_E_INVALID_ARG, "batch too large (%llu hit entries): split it", (unsigned long long)cap);
+  s.cap = cap; s.scratch_bytes = digitize_scratch_bytes(max_pairs, cap);
+  const bool singles = (want & GPET_WANT_SINGLES) != 0;
+  s.A.size = cap * (28 + (singles ? 36 : 0) + 40) + 4 * (s.n_chunks + 1) + s.scratch_bytes + ((want & GPET_WANT_HASH) ? 16 * max_pairs : 0) + 64 * 256;
+  CUDA_TRY(cudaMalloc(&s.A.base, s.A.size));
+  DevArena &A = s.A; gpet_hits &H = s.H; memset(&H, 0, sizeof H);
+  H.history = A.take<uint32_t>(cap); H.ids = A.take<uint32_t>(cap); H.x = A.take<float>(cap); H.y = A.take<float>(cap); H.z = A.take<float>(cap);
+  H.e_keV = A.take<float>(cap); H.tof_ns = A.take<float>(cap); H.capacity = cap; H.n_hits = A.take<uint64_t>(1);
+  H.outcome_hash = (want & GPET_WANT_HASH) ? A.take<uint64_t>(2 * max_pairs) : nullptr;
+  H.chunk_fill = s.chunked ? A.take<uint32_t>(s.n_chunks + 1) : nullptr;
+  gpet_singles &S = s.S; memset(&S, 0, sizeof S);
+  if (singles) { S.history = A.take<uint32_t>(cap); S.ids = A.take<uint32_t>(cap); S.x = A.take<float>(cap); S.y = A.take<float>(cap);
+                 S.z = A.take<float>(cap); S.e_keV = A.take<float>(cap); S.t_s = A.take<double>(cap); }
+  S.capacity = cap; S.n_singles = A.take<uint64_t>(1);
+  gpet_coincidences &Cc = s.C;
+  Cc.ids_a = A.take<uint32_t>(cap); Cc.ids_b = A.take<uint32_t>(cap); Cc.history_a = A.take<uint32_t>(cap);
+  Cc.history_b = A.take<uint32_t>(cap); Cc.e_a = A.take<float>(cap); Cc.e_b = A.take<float>(cap); Cc.dt_ns = A.take<float>(cap);
+  Cc.t_s = A.take<double>(cap); Cc.capacity = cap; Cc.n_coinc = A.take<uint64_t>(1);
+  s.scratch = A.take<char>(s.scratch_bytes);
+  if (A.used > A.size) return fail(GPET_E_OVERFLOW, "internal arena too small");
+  CUDA_TRY(cudaStreamCreateWithFlags(&s.copy, cudaStreamNonBlocking));
+  CUDA_TRY(cudaEventCreateWithFlags(&s.computed, cudaEventDisableTiming));
+  CUDA_TRY(cudaEventCreateWithFlags(&s.counted, cudaEventDisableTiming));
+  CUDA_TRY(cudaMallocHost(&s.host_counts, 4 * sizeof(uint64_t)));
+  return GPET_OK;
+}
+
+extern "C" int gpet_pipeline_create(const gpet_geometry *g, const gpet_materials *m, const gpet_source *src, const gpet_digitizer *dig,
+                                    uint64_t n_pairs_total, uint64_t max_pairs_per_batch, double hits_per_pair, uint32_t want, int32_t n_slots,
+                                    gpet_pipeline **out) {
+  if (!g || !m || !src || !dig || !out) return fail(GPET_E_INVALID_ARG, "gpet_pipeline_create: NULL argument");
+  if (max_pairs_per_batch == 0 || max_pairs_per_batch >= (1ull << 32) || !(hits_per_pair > 0.0) || n_slots < 1 || n_slots > 2)
+    return fail(GPET_E_INVALID_ARG, "gpet_pipeline_create: bad counts");
+  if (n_pairs_total < max_pairs_per_batch) return fail(GPET_E_INVALID_ARG, "gpet_pipeline_create: n_pairs_total < max_pairs_per_batch");
+  gpet_pipeline *p = new gpet_pipeline;
+  p->g = g; p->m = m; p->src = *src; p->dig = *dig; p->n_pairs_total = n_pairs_total; p->max_pairs = max_pairs_per_batch;
+  p->hits_per_pair = hits_per_pair; p->want = want;
+  int rc = GPET_OK;
+  do {
+    if (cudaStreamCreateWithFlags(&p->compute, cudaStreamNonBlocking) != cudaSuccess) { rc = fail(GPET_E_CUDA, "cannot create a stream"); break; }
+    if (src->kind == 1 && src->phantom_material) {                   // HOST phantom map -> device, once
+      const size_t nvox = (size_t)src->dims[0] * src->dims[1] * src->dims[2];
+      for (size_t i = 0; i < nvox; ++i) if (src->phantom_material[i] > m->n_materials) { rc = fail(GPET_E_INVALID_ARG, "phantom voxel %zu holds material %d, only %d are loaded", i, (int)src->phantom_material[i] - 1, m->n_materials); break; }
+      if (rc) break;
+      if (cudaMalloc(&p->phantom_dev, nvox) != cudaSuccess || cudaMemcpy(p->phantom_dev, src->phantom_material, nvox, cudaMemcpyHostToDevice) != cudaSuccess) {
+        rc = fail(GPET_E_CUDA, "phantom upload failed"); break; }
+      p->src.phantom_material = p->phantom_dev;
+    }
+    for (int i = 0; i < n_slots && !rc; ++i) rc = slot_create(p->slot[i], max_pairs_per_batch, hits_per_pair, want);
+  } while (0);
+  if (rc) { gpet_pipeline_destroy(p); return rc; }
+  *out = p; return GPET_OK;
+}
+
+extern "C" int gpet_pipeline_destroy(gpet_pipeline *p) {
+  if (!p) return GPET_OK;
+  if (p->compute) cudaStreamSynchronize(p->compute);
+  for (Slot &s : p->slot) slot_release(s);
+  if (p->phantom_dev) cudaFree(p->phantom_dev);
+  if (p->compute) cudaStreamDestroy(p->compute);
+  delete p; return GPET_OK;
+}
+
+extern "C" int gpet_pipeline_submit(gpet_pipeline *p, uint64_t first_history, uint64_t n_pairs, uint64_t seed) {
+  if (!p) return fail(GPET_E_INVALID_ARG, "gpet_pipeline_submit: NULL pipeline");
+  if (n_pairs == 0 || n_pairs > p->max_pairs) return fail(GPET_E_INVALID_ARG, "gpet_pipeline_submit: n_pairs %llu outside 1..%llu", (unsigned long long)n_pairs, (unsigned long long)p->max_pairs);
+  const int n_slots = p->slot[1].A.base ? 2 : 1;
+  Slot &s = p->slot[p->submitted % n_slots];
+  if (s.busy) return fail(GPET_E_INVALID_ARG, "gpet_pipeline_submit: %d batches already in flight; collect one first", n_slots);
+  cudaStream_t st = p->compute;
+  CUDA_TRY(cudaMemsetAsync(s.H.n_hits, 0, 8, st));
+  if (s.chunked) CUDA_TRY(cudaMemsetAsync(s.H.chunk_fill, 0, 4 * (s.n_chunks + 1), st));
+  // the chunked layout divides the buffer by the chunks of THIS batch: keep the per-chunk region of the full-size batch
+  gpet_hits H = s.H;
+  if (s.chunked) H.capacity = ((n_pairs + kHitChunkPairs - 1) / kHitChunkPairs) * (s.cap / s.n_chunks);
+  int rc = gpet_simulate(p->g, p->m, &p->src, first_history, n_pairs, seed, &H, st); if (rc) return rc;
+  gpet_singles Sd = s.S;
+  rc = gpet_digitize(&p->src, seed, p->n_pairs_total, first_history, n_pairs, &H, H.capacity, &p->dig, s.scratch, s.scratch_bytes, &Sd, &s.C, st); if (rc) return rc;
+  CUDA_TRY(cudaEventRecord(s.computed, st));
+  CUDA_TRY(cudaStreamWaitEvent(s.copy, s.computed, 0));
+  CUDA_TRY(cudaMemcpyAsync(&s.host_counts[0], s.H.n_hits, 8, cudaMemcpyDeviceToHost, s.copy));
+  CUDA_TRY(cudaMemcpyAsync(&s.host_counts[1], s.S.n_singles, 8, cudaMemcpyDeviceToHost, s.copy));
+  CUDA_TRY(cudaMemcpyAsync(&s.host_counts[2], s.C.n_coinc, 8, cudaMemcpyDeviceToHost, s.copy));
+  s.host_counts[3] = 0;
+  if (s.chunked) CUDA_TRY(cudaMemcpyAsync(&s.host_counts[3], s.H.chunk_fill + (n_pairs + kHitChunkPairs - 1) / kHitChunkPairs, 4, cudaMemcpyDeviceToHost, s.copy));
+  CUDA_TRY(cudaEventRecord(s.counted, s.copy));
+  s.busy = true; s.n_pairs = n_pairs; ++p->submitted;
+  return GPET_OK;
+}
+
+extern "C" int gpet_pipeline_collect(gpet_pipeline *p, gpet_host_outputs *out) {
+  if (!p || !out) return fail(GPET_E_INVALID_ARG, "gpet_pipeline_collect: NULL argument");
+  const int n_slots = p->slot[1].A.base ? 2 : 1;
+  Slot &s = p->slot[p->collected % n_slots];
+  if (!s.busy) return fail(GPET_E_INVALID_ARG, "gpet_pipeline_collect: nothing submitted");
+  s.busy = false; ++p->collected;
+  if (cudaEventSynchronize(s.counted) != cudaSuccess) return fail(GPET_E_CUDA, "transport/digitizer failed: %s", cudaGetErrorString(cudaGetLastError()));
+  const uint64_t nh = s.host_counts[0], ns = s.host_counts[1], nc = s.host_counts[2], dropped = s.host_counts[3] & 0xFFFFFFFFull;
+  if (dropped) return fail(GPET_E_OVERFLOW, "hit buffer overflow: %llu hits dropped; raise hits_per_pair", (unsigned long long)dropped);
+  if (!s.chunked && nh > s.cap) return fail(GPET_E_OVERFLOW, "hit buffer overflow: %llu hits > capacity %llu; raise hits_per_pair", (unsigned long long)nh, (unsigned long long)s.cap);
+  if (nc > s.C.capacity) return fail(GPET_E_OVERFLOW, "coincidence buffer overflow");
+  cudaStream_t st = s.copy;
+#define D2H(dst, srcp, n, T) do { if ((dst) && (srcp) && (n)) CUDA_TRY(cudaMemcpyAsync((dst), (srcp), sizeof(T) * (n), cudaMemcpyDeviceToHost, st)); } while (0)
+  if (!s.chunked) {
+    const uint64_t ch = nh < out->hits.capacity ? nh : out->hits.capacity;
+    D2H(out->hits.history, s.H.history, ch, uint32_t); D2H(out->hits.ids, s.H.ids, ch, uint32_t); D2H(out->hits.x, s.H.x, ch, float);
+    D2H(out->hits.y, s.H.y, ch, float); D2H(out->hits.z, s.H.z, ch, float); D2H(out->hits.e_keV, s.H.e_keV, ch, float); D2H(out->hits.tof_ns, s.H.tof_ns, ch, float);
+  }
+  D2H(out->hits.outcome_hash, s.H.outcome_hash, 2 * s.n_pairs, uint64_t);
+  const uint64_t cs = ns < out->singles.capacity ? ns : out->singles.capacity;
+  D2H(out->singles.history, s.S.history, cs, uint32_t); D2H(out->singles.ids, s.S.ids, cs, uint32_t); D2H(out->singles.x, s.S.x, cs, float);
+  D2H(out->singles.y, s.S.y, cs, float); D2H(out->singles.z, s.S.z, cs, float); D2H(out->singles.e_keV, s.S.e_keV, cs, float); D2H(out->singles.t_s, s.S.t_s, cs, double);
+  const uint64_t cc = nc < out->coinc.capacity ? nc : out->coinc.capacity;
+  D2H(out->coinc.ids_a, s.C.ids_a, cc, uint32_t); D2H(out->coinc.ids_b, s.C.ids_b, cc, uint32_t); D2H(out->coinc.history_a, s.C.history_a, cc, uint32_t);
+  D2H(out->coinc.history_b, s.C.history_b, cc, uint32_t); D2H(out->coinc.e_a, s.C.e_a, cc, float); D2H(out->coinc.e_b, s.C.e_b, cc, float);
+  D2H(out->coinc.dt_ns, s.C.dt_ns, cc, float); D2H(out->coinc.t_s, s.C.t_s, cc, double);
+#undef D2H
+  if (cudaStreamSynchronize(st) != cudaSuccess) return fail(GPET_E_CUDA, "copy back failed: %s", cudaGetErrorString(cudaGetLastError()));
+  if (out->hits.n_hits) *out->hits.n_hits = nh;
+  if (out->singles.n_singles) *out->singles.n_singles = ns;
+  if (out->coinc.n_coinc) *out->coinc.n_coinc = nc;
+  return GPET_OK;
+}
+
+// One batch, start to finish: a one-slot pipeline kept between calls of the same shape (freed by gpet_shutdown).
+namespace {
+std::mutex g_host_lock; gpet_pipeline *g_host_pipe = nullptr;
+}
 extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, const gpet_source *src, uint64_t n_pairs_total,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const gpet_digitizer *dig, double hits_per_pair,
                              gpet_host_outputs *out) {
   if (!g || !m || !src || !dig || !out) return fail(GPET_E_INVALID_ARG, "gpet_run_host: NULL argument");
-  if (n_pairs == 0 || n_pairs >= (1ull << 32) || !(hits_per_pair > 0.0)) return fail(GPET_E_INVALID_ARG, "gpet_run_host: bad counts");
-  // hits that stay on the device use the chunked layout (shared-memory sort per chunk in the digitizer); hits the caller
-  // wants on the host use the dense one, which is what gpet_host_outputs describes
-  const bool chunked = out->hits.history == nullptr;
-  const uint64_t n_chunks = (n_pairs + kHitChunkPairs - 1) / kHitChunkPairs;
-  uint64_t chunk_cap = (uint64_t)ceil((double)kHitChunkPairs * hits_per_pair);
-  if (chunk_cap > kHitChunkCapMax) chunk_cap = kHitChunkCapMax;
-  const uint64_t cap = chunked ? n_chunks * chunk_cap : (uint64_t)((double)n_pairs * hits_per_pair) + 1024;
-  if (cap >= (1ull << 32)) return fail(GPET_E_INVALID_ARG, "gpet_run_host: batch too large, split it");
-  const size_t scratch_bytes = digitize_scratch_bytes(n_pairs, cap);
-  const size_t nvox = src->kind == 1 && src->phantom_material ? (size_t)src->dims[0] * src->dims[1] * src->dims[2] : 0;
-  // one cached device arena per process: repeated batches of the same size do not re-allocate
-  static std::mutex arena_lock; static char *arena_base = nullptr; static size_t arena_size = 0;
-  std::lock_guard<std::mutex> arena_guard(arena_lock);
-  DevArena A; A.size = cap * (28 + 36 + 40) + 4 * (n_chunks + 1) + scratch_bytes + nvox + (out->hits.outcome_hash ? 16 * n_pairs : 0) + 64 * 256;
-  if (A.size > arena_size) {
-    if (arena_base) cudaFree(arena_base);
-    arena_base = nullptr; arena_size = 0;
-    CUDA_TRY(cudaMalloc(&arena_base, A.size));
-    arena_size = A.size;
+  const uint32_t want = (out->hits.history ? GPET_WANT_HITS : 0u) | (out->singles.history ? GPET_WANT_SINGLES : 0u) | (out->hits.outcome_hash ? GPET_WANT_HASH : 0u);
+  std::lock_guard<std::mutex> lk(g_host_lock);
+  gpet_pipeline *p = g_host_pipe;
+  const bool reuse = p && p->g == g && p->m == m && p->max_pairs == n_pairs && p->n_pairs_total == n_pairs_total && p->hits_per_pair == hits_per_pair &&
+                     p->want == want && !p->phantom_dev && !(src->kind == 1 && src->phantom_material) &&
+                     memcmp(&p->dig, dig, sizeof *dig) == 0 && memcmp(&p->src, src, sizeof *src) == 0;
+  if (!reuse) {
+    if (p) gpet_pipeline_destroy(p);
+    g_host_pipe = nullptr;
+    int rc = gpet_pipeline_create(g, m, src, dig, n_pairs_total, n_pairs, hits_per_pair, want, 1, &p); if (rc) return rc;
+    g_host_pipe = p;
   }
-  A.base = arena_base;
-  int rc = GPET_OK;
-  cudaStream_t st = 0;
-  do {
-    gpet_hits H; memset(&H, 0, sizeof H);
-    H.history = A.take<uint32_t>(cap); H.ids = A.take<uint32_t>(cap); H.x = A.take<float>(cap); H.y = A.take<float>(cap); H.z = A.take<float>(cap);
-    H.e_keV = A.take<float>(cap); H.tof_ns = A.take<float>(cap); H.capacity = cap; H.n_hits = A.take<uint64_t>(1);
-    H.outcome_hash = out->hits.outcome_hash ? A.take<uint64_t>(2 * n_pairs) : nullptr;
-    H.chunk_fill = chunked ? A.take<uint32_t>(n_chunks + 1) : nullptr;
-    gpet_singles S; S.history = A.take<uint32_t>(cap); S.ids = A.take<uint32_t>(cap); S.x = A.take<float>(cap); S.y = A.take<float>(cap);
-    S.z = A.take<float>(cap); S.e_keV = A.take<float>(cap); S.t_s = A.take<double>(cap); S.capacity = cap; S.n_singles = A.take<uint64_t>(1);
-    gpet_coincidences Cc; Cc.ids_a = A.take<uint32_t>(cap); Cc.ids_b = A.take<uint32_t>(cap); Cc.history_a = A.take<uint32_t>(cap);
-    Cc.history_b = A.take<uint32_t>(cap); Cc.e_a = A.take<float>(cap); Cc.e_b = A.take<float>(cap); Cc.dt_ns = A.take<float>(cap);
-    Cc.t_s = A.take<double>(cap); Cc.capacity = cap; Cc.n_coinc = A.take<uint64_t>(1);
-    void *scratch = A.take<char>(scratch_bytes);
-    gpet_source s2 = *src;
-    if (nvox) {
-      uint8_t *ph = A.take<uint8_t>(nvox);
-      if (cudaMemcpyAsync(ph, src->phantom_material, nvox, cudaMemcpyHostToDevice, st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "phantom upload failed"); break; }
-      s2.phantom_material = ph;
-    }
-    if (A.used > A.size) { rc = fail(GPET_E_OVERFLOW, "internal arena too small"); break; }
-    if (cudaMemsetAsync(H.n_hits, 0, 8, st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "memset failed"); break; }
-    if (chunked && cudaMemsetAsync(H.chunk_fill, 0, 4 * (n_chunks + 1), st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "memset failed"); break; }
-    if ((rc = gpet_simulate(g, m, &s2, first_history, n_pairs, seed, &H, st))) break;
-    gpet_singles Sd = S;                   // singles arrays are written only when the caller wants them; the count always is
-    if (!out->singles.history) { Sd.history = Sd.ids = nullptr; Sd.x = Sd.y = Sd.z = Sd.e_keV = nullptr; Sd.t_s = nullptr; }
-    if ((rc = gpet_digitize(&s2, seed, n_pairs_total, first_history, n_pairs, &H, cap, dig, scratch, scratch_bytes, &Sd, &Cc, st))) break;
-    uint64_t nh = 0, ns = 0, nc = 0; uint32_t dropped = 0;
-    if (chunked) cudaMemcpyAsync(&dropped, H.chunk_fill + n_chunks, 4, cudaMemcpyDeviceToHost, st);
-    cudaMemcpyAsync(&nh, H.n_hits, 8, cudaMemcpyDeviceToHost, st);
-    cudaMemcpyAsync(&ns, S.n_singles, 8, cudaMemcpyDeviceToHost, st); cudaMemcpyAsync(&nc, Cc.n_coinc, 8, cudaMemcpyDeviceToHost, st);
-    if (cudaStreamSynchronize(st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "transport/digitizer failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
-    if (dropped) { rc = fail(GPET_E_OVERFLOW, "hit buffer overflow: %u hits dropped; raise hits_per_pair", dropped); break; }
-    if (!chunked && nh > cap) { rc = fail(GPET_E_OVERFLOW, "hit buffer overflow: %llu hits > capacity %llu; raise hits_per_pair", (unsigned long long)nh, (unsigned long long)cap); break; }
-#define D2H(dst, srcp, n, T) do { if ((dst) && (n)) cudaMemcpyAsync((dst), (srcp), sizeof(T) * (n), cudaMemcpyDeviceToHost, st); } while (0)
-    const uint64_t ch = nh < out->hits.capacity ? nh : out->hits.capacity;
-    D2H(out->hits.history, H.history, ch, uint32_t); D2H(out->hits.ids, H.ids, ch, uint32_t); D2H(out->hits.x, H.x, ch, float);
-    D2H(out->hits.y, H.y, ch, float); D2H(out->hits.z, H.z, ch, float); D2H(out->hits.e_keV, H.e_keV, ch, float); D2H(out->hits.tof_ns, H.tof_ns, ch, float);
-    D2H(out->hits.outcome_hash, H.outcome_hash, 2 * n_pairs, uint64_t);
-    const uint64_t cs = ns < out->singles.capacity ? ns : out->singles.capacity;
-    D2H(out->singles.history, S.history, cs, uint32_t); D2H(out->singles.ids, S.ids, cs, uint32_t); D2H(out->singles.x, S.x, cs, float);
-    D2H(out->singles.y, S.y, cs, float); D2H(out->singles.z, S.z, cs, float); D2H(out->singles.e_keV, S.e_keV, cs, float); D2H(out->singles.t_s, S.t_s, cs, double);
-    const uint64_t cc = nc < out->coinc.capacity ? nc : out->coinc.capacity;
-    D2H(out->coinc.ids_a, Cc.ids_a, cc, uint32_t); D2H(out->coinc.ids_b, Cc.ids_b, cc, uint32_t); D2H(out->coinc.history_a, Cc.history_a, cc, uint32_t);
-    D2H(out->coinc.history_b, Cc.history_b, cc, uint32_t); D2H(out->coinc.e_a, Cc.e_a, cc, float); D2H(out->coinc.e_b, Cc.e_b, cc, float);
-    D2H(out->coinc.dt_ns, Cc.dt_ns, cc, float); D2H(out->coinc.t_s, Cc.t_s, cc, double);
-#undef D2H
-    if (cudaStreamSynchronize(st) != cudaSuccess) { rc = fail(GPET_E_CUDA, "copy back failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
-    if (out->hits.n_hits) *out->hits.n_hits = nh;
-    if (out->singles.n_singles) *out->singles.n_singles = ns;
-    if (out->coinc.n_coinc) *out->coinc.n_coinc = nc;
-  } while (0);
+  int rc = gpet_pipeline_submit(p, first_history, n_pairs, seed);
+  if (!rc) rc = gpet_pipeline_collect(p, out);
   return rc;
+}
+
+extern "C" int gpet_shutdown(void) {
+  { std::lock_guard<std::mutex> lk(g_host_lock); if (g_host_pipe) gpet_pipeline_destroy(g_host_pipe); g_host_pipe = nullptr; }
+  work_ring_release();
+  return GPET_OK;
 }

@@ -16,13 +16,24 @@ constexpr float kCutoff = 10.0f;          // [R12]
 constexpr uint32_t kNone = 0xFFFFFFFFu;
 
 // ---------------------------------------------------------------- descriptor as the kernels see it
+// Exact division of a Q coordinate n (0 <= n < 2^31) by a Q pitch d >= 2 with one high multiply and a shift:
+// floor(n / d) = umulhi(n, magic) >> shift, magic = floor(2^(32 + shift) / d) + 1, shift = ceil(log2 d) - 1.
+// (magic d - 2^(32+shift) lies in (0, d] and d <= 2^(shift+1), so the error term n (magic d - 2^(32+shift)) / (d 2^(32+shift))
+// stays below 1/d for n < 2^31: the quotient is exact.  Checked against plain division in tests/test_abi.py.)
+struct QDiv { uint32_t magic, shift; };
+__host__ __device__ inline QDiv qdiv_make(uint32_t d) {
+  uint32_t sh = 0; while ((2ull << sh) < (unsigned long long)d) ++sh;        // 2^sh < d <= 2^(sh+1)
+  QDiv q; q.shift = sh; q.magic = (uint32_t)((1ull << (32 + sh)) / d) + 1u; return q;
+}
+
 struct __align__(16) DevLayer {   // 64 bytes = four 16-byte rows: the transport kernel reads the record of a lane's layer from shared memory
   int c0, c1;                 // depth range [c0, c1) in Q units (unused layers: c0 = c1 = INT_MAX, never selected)
   int cmat, gmat;
   int n[2], pitch[2];
   int lo[2], hi[2];           // crystal occupies frac in [lo, hi) of each pitch cell
   int off[2];
-  float inv_pitch[2];         // (1 - 1e-6) / pitch: floor_div_pos never overshoots
+  uint32_t magic[2];          // QDiv of the pitches ...
+  // ... whose shifts ride in the top byte of n[] (n <= 8192)
 };
 struct __align__(16) DevPanel {
   float pose[12];             // front-face centre, u, v, w
@@ -38,7 +49,7 @@ struct DevGeomHead {
   int n_panels, n_layers;
   int Wq, Hq, Dq, hWq, hHq;
   int nmod[2], msq[2], mpq[2];
-  float inv_mpq[2];           // (1 - 1e-6) / module pitch
+  uint32_t mp_magic[2], mp_shift[2];   // QDiv of the module pitches
   float blo[3], bhi[3];       // panel box in the tracking frame (fp32 roundings of the Q extents)
   uint32_t det_mask;          // materials referenced by the layers
   int ring;                   // 1 = repetition mode
@@ -92,17 +103,6 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, const PhiloxKeys &K) {
 __device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 9) + 0.5f) * 1.1920928955078125e-7f; }
 
 // ---------------------------------------------------------------- [R7] lattice lookup
-// Exact floor division of a NON-NEGATIVE Q coordinate by a Q pitch.  inv_lo = (1 - 1e-6) / pitch is biased low by far
-// more than the three fp32 roundings involved (< 2e-7), so the estimate never exceeds the true quotient and falls short
-// of it by less than one (quotients stay below 7e5): one upward fix-up makes it exact.  For rel < 0 the result is
-// meaningless; callers treat rel < 0 as "outside" on their own.
-__device__ __forceinline__ int floor_div_pos(int rel, int pitch, float inv_lo, int &rem) {
-  int i = __float2int_rd((float)rel * inv_lo);
-  int r = rel - i * pitch;
-  if (r >= pitch) { ++i; r -= pitch; }
-  rem = r; return i;
-}
-
 // (qa, qb, qc) measured from the panel's low corner.  Returns the material (-1 vacuum) and the packed ids without
 // panel/photon/seq bits (kNone when the point is in no crystal).  PAPER.md:43: the depth coordinate picks the layer,
 // that layer's crystal parameters give material and index.  Written without early exits: every lane of a pass runs the
@@ -110,25 +110,22 @@ __device__ __forceinline__ int floor_div_pos(int rel, int pitch, float inv_lo, i
 // or the kernel's copy in shared memory: lanes in different layers then read different rows without serialising).
 __device__ __forceinline__ int lattice_lookup(const DevGeomHead &g, const DevLayer *lay, int qa, int qb, int qc, uint32_t &ids) {
   bool ok = (unsigned)qa < (unsigned)g.Wq && (unsigned)qb < (unsigned)g.Hq && (unsigned)qc < (unsigned)g.Dq;
-  int ra, rb;
-  const int mx = floor_div_pos(qa, g.mpq[0], g.inv_mpq[0], ra);
-  const int my = floor_div_pos(qb, g.mpq[1], g.inv_mpq[1], rb);
+  const int mx = (int)(__umulhi((uint32_t)qa, g.mp_magic[0]) >> g.mp_shift[0]), ra = qa - mx * g.mpq[0];
+  const int my = (int)(__umulhi((uint32_t)qb, g.mp_magic[1]) >> g.mp_shift[1]), rb = qb - my * g.mpq[1];
   ok = ok && ra < g.msq[0] && rb < g.msq[1];                         // else inter-module gap: vacuum
-  int l = -1;
-#pragma unroll
-  for (int k = 0; k < kMaxLayers; ++k)
-    if (qc >= g.layer[k].c0 && qc < g.layer[k].c1) l = k;            // unused layers hold INT_MAX
-  ok = ok && l >= 0;                                                 // else inter-layer gap: vacuum
-  const int4 r0 = reinterpret_cast<const int4 *>(&lay[l < 0 ? 0 : l])[0];     // c0, c1, cmat, gmat
-  const int4 r1 = reinterpret_cast<const int4 *>(&lay[l < 0 ? 0 : l])[1];     // n0, n1, pitch0, pitch1
-  const int4 r2 = reinterpret_cast<const int4 *>(&lay[l < 0 ? 0 : l])[2];     // lo0, lo1, hi0, hi1
-  const int4 r3 = reinterpret_cast<const int4 *>(&lay[l < 0 ? 0 : l])[3];     // off0, off1, inv0, inv1
-  const int ea = ra - r3.x, eb = rb - r3.y;
-  int fa, fb;
-  const int ix = floor_div_pos(ea, r1.z, __int_as_float(r3.z), fa);
-  const int iy = floor_div_pos(eb, r1.w, __int_as_float(r3.w), fb);
-  const bool in = (ea | eb) >= 0 && ix < r1.x && iy < r1.y && fa >= r2.x && fa < r2.z && fb >= r2.y && fb < r2.w;
-  ids = ok && in ? ((uint32_t)(mx + g.nmod[0] * my) << 20) | ((uint32_t)l << 18) | ((uint32_t)(ix + r1.x * iy) << 5) : kNone;
+  // layers are stacked front to back: the last one that starts at or before qc is the only candidate
+  const int l = (qc >= g.layer[1].c0 ? 1 : 0) + (qc >= g.layer[2].c0 ? 1 : 0) + (qc >= g.layer[3].c0 ? 1 : 0);   // unused layers hold INT_MAX
+  const int4 r0 = reinterpret_cast<const int4 *>(&lay[l])[0];        // c0, c1, cmat, gmat
+  const int4 r1 = reinterpret_cast<const int4 *>(&lay[l])[1];        // n0 | shift0 << 24, n1 | shift1 << 24, pitch0, pitch1
+  const int4 r2 = reinterpret_cast<const int4 *>(&lay[l])[2];        // lo0, lo1, hi0, hi1
+  const int4 r3 = reinterpret_cast<const int4 *>(&lay[l])[3];        // off0, off1, magic0, magic1
+  ok = ok && qc >= r0.x && qc < r0.y;                                // else inter-layer gap: vacuum
+  const int ea = ra - r3.x, eb = rb - r3.y;                          // negative: in front of the lattice (rim)
+  const int n0 = r1.x & 0xFFFFFF, n1 = r1.y & 0xFFFFFF;
+  const int ix = (int)(__umulhi((uint32_t)ea, (uint32_t)r3.z) >> ((uint32_t)r1.x >> 24)), fa = ea - ix * r1.z;
+  const int iy = (int)(__umulhi((uint32_t)eb, (uint32_t)r3.w) >> ((uint32_t)r1.y >> 24)), fb = eb - iy * r1.w;
+  const bool in = (ea | eb) >= 0 && ix < n0 && iy < n1 && fa >= r2.x && fa < r2.z && fb >= r2.y && fb < r2.w;
+  ids = ok && in ? ((uint32_t)(mx + g.nmod[0] * my) << 20) | ((uint32_t)l << 18) | ((uint32_t)(ix + n0 * iy) << 5) : kNone;
   return ok ? (in ? r0.z : r0.w) : -1;
 }
 

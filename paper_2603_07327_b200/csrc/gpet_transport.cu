@@ -17,16 +17,17 @@
 // done per warp: no block-level barrier, no atomics except the work counter and the hit counters.  Geometry header in
 // the constant bank, per-panel and per-layer records and the interleaved float4 mu tables in shared memory; hits are
 // written 32 at a time by the HIT pass: one atomicAdd per 32 hits and seven fully coalesced 128-byte stores (SoA).
+#include <cstdio>
 #include "gpet_internal.h"
 
 namespace gpet {
 
 // Launch shape and pool sizes (measured on B200, C1-C4; -D overrides are for experiments only).
 #ifndef GPET_THREADS
-#define GPET_THREADS 768              // one CTA of 24 warps per SM: the tables are staged once, each warp gets ~8.5 KB
+#define GPET_THREADS 640              // one CTA of 20 warps per SM: the tables are staged once, each warp gets ~10.5 KB
 #endif
 #ifndef GPET_SLOTS
-#define GPET_SLOTS 128                // photon slots per warp
+#define GPET_SLOTS 160                // photon slots per warp (measured on C1 / C3 / C4: 20 x 160 beats 24 x 128 and 22 x 144 by 1-5 %)
 #endif
 #ifndef GPET_MIN_GEN
 #define GPET_MIN_GEN 16               // the source refills only when at least this many pairs fit
@@ -384,6 +385,12 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
     q.inv_mu = rcp_fast(mu_lookup(mu, T, 0, q.E).w);
   };
 
+#ifdef GPET_STATS
+  unsigned st_pass[10] = {0,0,0,0,0,0,0,0,0,0}, st_lane[10] = {0,0,0,0,0,0,0,0,0,0};
+#define GPET_STAT(i, n) do { st_pass[i]++; st_lane[i] += (unsigned)(n); } while (0)
+#else
+#define GPET_STAT(i, n) do { } while (0)
+#endif
   int gen_b = 0, gen_nb = 0;               // point sources: photons A of the top gen_nb queued pairs are placed, their photons B come next
 
 #pragma unroll 1
@@ -429,6 +436,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       const int ng = (int)min(32u, w_end - w_next);
       const uint32_t j = w_next + (uint32_t)lane;
       w_next += (uint32_t)ng;
+      GPET_STAT(7, ng);
       bool keep = false; uint4 w = make_uint4(0, 0, 0, 0);
       if (lane < ng) {
         const uint64_t history = history_of(j);
@@ -458,6 +466,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       // point in the STEP list when the fused search succeeds, else in the SEARCH list.
       const int nb = gen_b ? gen_nb : min(32, cQ);
       const bool have = lane < nb;
+      GPET_STAT(8, nb);
       Photon q = {};
       q.meta = (kNoPanel << 5) | (uint32_t)gen_b; q.ids = kNone; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
       q.x[0] = src.pos[0]; q.x[1] = src.pos[1]; q.x[2] = src.pos[2];
@@ -560,6 +569,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       // ---------------------------------------------- SEARCH: nearest panel ahead [R6], entry transform [R18].  A photon that has
       // just left a panel arrives in that panel's frame (record n_panels is the identity: fresh photons are global)
       const int n = min(cS, 32); const bool act = lane < n;
+      GPET_STAT(L_SEARCH, n);
       Photon q = {}; uint64_t hq = 0; int idx = 0;
       if (act) { idx = W.list[L_SEARCH][cS - 1 - lane]; slot_load(W, idx, q, hq); }
       cS -= n;
@@ -591,6 +601,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       // No divergent branches: every lane draws, advances to the collision point or to the exit face, looks the point up
       // and selects its next event.
       const int n = min(cT, 32); const bool act = lane < n;
+      GPET_STAT(L_STEP, n);
       const int idx = W.list[L_STEP][max(cT - 1 - lane, 0)];
       cT -= n;
       float4 A = W.a[idx]; const float4 B = W.b[idx]; uint4 C = W.c[idx];
@@ -653,6 +664,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       // ---------------------------------------------- KN: one Klein-Nishina trial per visit [R20].  A deposit in a crystal is
       // copied into a free slot and queued for the HIT pass; the photon itself goes on.
       const int n = min(min(cK, 32), cF); const bool act = lane < n;
+      GPET_STAT(L_KN, n);
       const int idx = W.list[L_KN][max(cK - 1 - lane, 0)];
       cK -= n;
       const float4 A = W.a[idx]; float4 B = W.b[idx]; uint4 C = W.c[idx];
@@ -727,6 +739,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       // of their 512-pair chunk; lanes of the same chunk (almost always all of them) share one atomicAdd on that chunk's
       // fill counter and write consecutive entries.
       const int n = min(cH, 32); const bool act = lane < n;
+      GPET_STAT(L_HIT, n);
       const int idx = W.list[L_HIT][max(cH - 1 - lane, 0)];
       cH -= n;
       const float4 A = W.a[idx]; const uint4 C = W.c[idx];
@@ -823,6 +836,11 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
     }
     __syncwarp();
   }
+#ifdef GPET_STATS
+  if (blockIdx.x == 3 && lane == 0 && (threadIdx.x >> 5) < 4)
+    printf("warp %d: SEARCH %u/%u STEP %u/%u KN %u/%u HIT %u/%u GEN1 %u/%u GEN2 %u/%u\n", threadIdx.x >> 5, st_lane[L_SEARCH], st_pass[L_SEARCH], st_lane[L_STEP], st_pass[L_STEP],
+           st_lane[L_KN], st_pass[L_KN], st_lane[L_HIT], st_pass[L_HIT], st_lane[7], st_pass[7], st_lane[8], st_pass[8]);
+#endif
 }
 
 static int g_transport_warps = kWarps;             // warps per CTA (one CTA per SM); fewer leave room for other streams' kernels

@@ -661,7 +661,7 @@ def closed_cube(half=40.0):
     faces = [((1, 0, 0), (0, 1, 0), (0, 0, 1)), ((-1, 0, 0), (0, -1, 0), (0, 0, 1)), ((0, 1, 0), (-1, 0, 0), (0, 0, 1)),
              ((0, -1, 0), (1, 0, 0), (0, 0, 1)), ((0, 0, 1), (1, 0, 0), (0, 1, 0)), ((0, 0, -1), (1, 0, 0), (0, -1, 0))]
     poses = np.array([np.concatenate([half * np.array(w, float), u, v, w]) for w, u, v in faces], np.float32)
-    side = 2 * half + 20.0                                             # faces overlap at the edges: no photon slips through
+    side = 2 * half                                                    # the six boxes touch along the cube's edges without overlapping
     lay = (W.Layer((1, 1), (side, side), (0.0, 0.0), (0.0, 0.0), 10.0),)
     return W.Geometry(6, lay, (1, 1), (side, side), (side, side), panel_pose=poses)
 
@@ -677,7 +677,9 @@ def phantom_rayleigh_setup(mu_r=0.1):
     mat = np.full((4, 4, 4), 2, np.uint8)                              # value 2 = material index 1
     src = W.Source(1, (0, 0, 0), 0.0, 1e6, 0, act, mat, 1, dims, (0.1, 0.1, 0.1), (-0.2, -0.2, -0.2))
     f = lambda a, b: np.stack([np.full(W.N_ENERGIES, a, np.float32), np.full(W.N_ENERGIES, b, np.float32)])
-    t = W.Tables(W.E_MIN_KEV, W.E_STEP_KEV, f(50.0, 0.0), f(0.0, 0.0), f(0.0, mu_r))   # absorber: PE only; medium: Rayleigh only
+    # absorber: photoelectric only, 0.2 mm mean depth (a stronger one would put 5e-5 of the first collisions within fp32
+    # rounding of the entry face, where the CUDA path and the oracle may disagree on `inside`); medium: Rayleigh only
+    t = W.Tables(W.E_MIN_KEV, W.E_STEP_KEV, f(5.0, 0.0), f(0.0, 0.0), f(0.0, mu_r))
     return closed_cube(), t, src
 
 

@@ -124,7 +124,19 @@ typedef struct {
   int32_t  dims[3];               /* nx, ny, nz of the activity / phantom grid                          */
   float    voxel_mm[3];
   float    origin_mm[3];          /* low corner of voxel (0,0,0)                                        */
+  float    positron_fwhm_mm;      /* [R35] positron range: isotropic Gaussian displacement of the        */
+                                  /* annihilation point, FWHM per axis; 0 = off, as in the paper         */
+                                  /* (PAPER.md:145 quotes 0.102 mm for 18F)                 */
+  double   half_life_s;           /* [R34] > 0: the source decays (18F, 1.6e8 atoms, 120 s): */
+  double   duration_s;            /* activity_bq is the INITIAL activity, the run covers [0, duration_s] */
+                                  /* and simulates n_pairs_total = gpet_decay_count(...) histories;      */
+                                  /* 0 = constant activity [R16]                                         */
 } gpet_source;
+
+/* Expected number of decays of a source of initial activity activity_bq and half-life half_life_s over duration_s
+ * seconds: A0 / lambda (1 - exp(-lambda T)), rounded to nearest (half_life_s = 0: A0 T).  This is the n_pairs_total of
+ * a run with the decay law switched on [R34]. */
+int gpet_decay_count(double activity_bq, double half_life_s, double duration_s, uint64_t *n_pairs);
 
 /* ---------------------------------------------------------------- transport */
 typedef struct {                  /* struct of arrays, DEVICE, caller-owned                             */

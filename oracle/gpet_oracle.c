@@ -58,6 +58,8 @@ typedef struct {
   const float *activity; const uint8_t *phantom; int32_t phantom_majorant;
   int32_t dims[3]; float voxel[3]; float origin[3];
   float beam_dir[3];                             /* kind 2: pencil beam along beam_dir (photon A) */
+  float positron_fwhm_mm;                        /* [R35] 0 = annihilation at the emission site */
+  double half_life_s, duration_s;                /* [R34] half_life_s > 0: decay law over duration_s, activity_bq = initial activity */
   /* derived once by orc_source_prepare (active voxel list + integer CDF) [R13] */
   uint32_t *act_index; uint64_t *act_cdf; uint64_t n_active; uint64_t w_total;
 } orc_source;
@@ -385,12 +387,50 @@ int orc_source_prepare(orc_source *s) {
 }
 void orc_source_release(orc_source *s) { free(s->act_index); free(s->act_cdf); s->act_index = NULL; s->act_cdf = NULL; }
 
-/* [R16] decay time of history i, seconds (fp64): t0 = (floor(i/B) + u53) * (B/A) */
+/* [R34] natural logarithm of z in (0, 1] from IEEE +, -, *, / only (no libm), so that the CUDA path, which restates
+ * it with round-to-nearest intrinsics, gets bit-identical decay times: z = m 2^e with m in [sqrt(1/2), sqrt(2));
+ * ln m = 2 atanh(s), s = (m-1)/(m+1), |s| <= 0.1716, odd series to s^25 (truncation < 1e-20). */
+double orc_det_log(double z) {
+  uint64_t bits; memcpy(&bits, &z, 8);
+  int e = (int)((bits >> 52) & 0x7FF) - 1022;                       /* z = f 2^e, f in [0.5, 1) */
+  bits = (bits & 0x000FFFFFFFFFFFFFull) | 0x3FE0000000000000ull;
+  double m; memcpy(&m, &bits, 8);
+  if (m < 0.70710678118654752440) { m = m * 2.0; e -= 1; }         /* m in [sqrt(1/2), sqrt(2)) */
+  double s = (m - 1.0) / (m + 1.0), s2 = s * s, p = 1.0 / 25.0;
+  for (int k = 23; k >= 1; k -= 2) p = p * s2 + 1.0 / (double)k;
+  return (double)e * 0.69314718055994530942 + 2.0 * s * p;
+}
+/* ln(1 - y) for y in [0, 1): below 1/4 the series runs on s = -y / (2 - y) directly (1 - y is never formed, so short
+ * acquisitions of long-lived sources keep full relative accuracy), above it is orc_det_log(1 - y) */
+double orc_det_log1m(double y) {
+  if (y < 0.25) {
+    double s = -y / (2.0 - y), s2 = s * s, p = 1.0 / 25.0;
+    for (int k = 23; k >= 1; k -= 2) p = p * s2 + 1.0 / (double)k;
+    return 2.0 * s * p;
+  }
+  return orc_det_log(1.0 - y);
+}
+/* [R34] expected number of decays of a source of initial activity A0 (Bq) and half-life T_half over T seconds:
+ * N = A0 / lambda (1 - exp(-lambda T)) (1.6e8 atoms of 18F, 1.70e-2 MBq, 120 s) */
+uint64_t orc_decay_count(double activity_bq, double half_life_s, double duration_s) {
+  if (!(half_life_s > 0.0)) return (uint64_t)llrint(activity_bq * duration_s);
+  double lambda = 0.69314718055994530942 / half_life_s;
+  return (uint64_t)llrint(activity_bq / lambda * -expm1(-lambda * duration_s));
+}
+/* [R16] decay time of history i, seconds (fp64): t0 = (floor(i/B) + u53) * (B/A).
+ * [R34] with a half-life: the same stratified quantile q = (floor(i/B) + u53) B / N in (0,1) goes through the inverse
+ * cdf of the decay law truncated to the acquisition: t0 = -ln(1 - q P) / lambda, P = 1 - exp(-lambda T) (the
+ * constant P comes from the C library's expm1 on the host, on both sides). */
 double orc_decay_time(const orc_source *s, uint64_t seed, uint64_t history, uint64_t n_pairs_total) {
   rng_t r; rng_init(&r, seed, history, STREAM_SOURCE);
   uint64_t w8 = rng_word_at(&r, 8), w9 = rng_word_at(&r, 9);
   double u53 = ((double)(((w8 << 32) | w9) >> 11) + 0.5) * (1.0 / 9007199254740992.0);
   uint64_t B = s->pairs_per_slice ? s->pairs_per_slice : n_pairs_total;
+  if (s->half_life_s > 0.0) {
+    double lambda = 0.69314718055994530942 / s->half_life_s, P = -expm1(-lambda * s->duration_s);
+    double q = ((double)(history / B) + u53) * ((double)B / (double)n_pairs_total);
+    return -orc_det_log1m(q * P) / lambda;
+  }
   return ((double)(history / B) + u53) * ((double)B / s->activity_bq);
 }
 
@@ -528,6 +568,19 @@ static void decay_site(const orc_source *S, rng_t *rs, double x0[3]) {
       x0[k] = (double)S->origin[k] + ((double)v[k] + orc_uniform(rng_word_at(rs, 1 + (uint32_t)k))) * (double)S->voxel[k];
   }
 }
+/* [R35] positron range (PAPER.md:61 switches it off; PAPER.md:145 quotes 0.102 mm FWHM for 18F): the annihilation point
+ * is the emission site plus an isotropic Gaussian displacement of the given FWHM per axis -- three normal deviates by
+ * Box-Muller from words 12-15 of the source stream [R3] */
+static void positron_range(const orc_source *S, rng_t *rs, double x0[3]) {
+  if (!(S->positron_fwhm_mm > 0.0f)) return;
+  double sg = (double)S->positron_fwhm_mm / ORC_FWHM, c1, s1, c2, s2;
+  double r1 = sqrt(-2.0 * log(orc_uniform(rng_word_at(rs, 12)))), r2 = sqrt(-2.0 * log(orc_uniform(rng_word_at(rs, 14))));
+  azimuth(orc_uniform(rng_word_at(rs, 13)), &c1, &s1); azimuth(orc_uniform(rng_word_at(rs, 15)), &c2, &s2);
+  x0[0] += sg * r1 * c1; x0[1] += sg * r1 * s1; x0[2] += sg * r2 * c2;
+}
+void orc_annihilation_sites(const orc_source *S, uint64_t seed, uint64_t first, uint64_t n, double *xyz) {   /* test hook */
+  for (uint64_t i = 0; i < n; ++i) { rng_t rs; rng_init(&rs, seed, first + i, STREAM_SOURCE); decay_site(S, &rs, xyz + 3 * i); positron_range(S, &rs, xyz + 3 * i); }
+}
 void orc_decay_sites(const orc_source *S, uint64_t seed, uint64_t first, uint64_t n, double *xyz) {   /* test hook */
   for (uint64_t i = 0; i < n; ++i) { rng_t rs; rng_init(&rs, seed, first + i, STREAM_SOURCE); decay_site(S, &rs, xyz + 3 * i); }
 }
@@ -536,6 +589,7 @@ void orc_decay_sites(const orc_source *S, uint64_t seed, uint64_t first, uint64_
 static void simulate_history(ctx_t *c, uint64_t seed, uint64_t history) {
   const orc_source *S = c->S; rng_t rs; rng_init(&rs, seed, history, STREAM_SOURCE);
   double x0[3]; decay_site(S, &rs, x0);
+  positron_range(S, &rs, x0);
   /* [R14] isotropic direction */
   double ct = 1.0 - 2.0 * orc_uniform(rng_word_at(&rs, 4)), st = sqrt(fmax(0.0, 1.0 - ct * ct)), cp, sp;
   azimuth(orc_uniform(rng_word_at(&rs, 5)), &cp, &sp);

@@ -52,7 +52,8 @@ class _Source(C.Structure):
     _fields_ = [("kind", C.c_int32), ("pos", C.c_float * 3), ("acol_fwhm_deg", C.c_float), ("activity_bq", C.c_double),
                 ("pairs_per_slice", C.c_uint64), ("activity", C.POINTER(C.c_float)), ("phantom", C.POINTER(C.c_uint8)),
                 ("phantom_majorant", C.c_int32), ("dims", C.c_int32 * 3), ("voxel", C.c_float * 3), ("origin", C.c_float * 3),
-                ("beam_dir", C.c_float * 3), ("act_index", C.POINTER(C.c_uint32)), ("act_cdf", C.POINTER(C.c_uint64)), ("n_active", C.c_uint64),
+                ("beam_dir", C.c_float * 3), ("positron_fwhm_mm", C.c_float), ("half_life_s", C.c_double), ("duration_s", C.c_double),
+                ("act_index", C.POINTER(C.c_uint32)), ("act_cdf", C.POINTER(C.c_uint64)), ("n_active", C.c_uint64),
                 ("w_total", C.c_uint64)]
 
 
@@ -102,6 +103,14 @@ def lib():
         _lib.orc_decay_time.argtypes = [C.POINTER(_Source), C.c_uint64, C.c_uint64, C.c_uint64]
         _lib.orc_decay_sites.argtypes = [C.POINTER(_Source), C.c_uint64, C.c_uint64, C.c_uint64, C.POINTER(C.c_double)]
         _lib.orc_decay_sites.restype = None
+        _lib.orc_annihilation_sites.argtypes = [C.POINTER(_Source), C.c_uint64, C.c_uint64, C.c_uint64, C.POINTER(C.c_double)]
+        _lib.orc_annihilation_sites.restype = None
+        _lib.orc_det_log.restype = C.c_double
+        _lib.orc_det_log.argtypes = [C.c_double]
+        _lib.orc_det_log1m.restype = C.c_double
+        _lib.orc_det_log1m.argtypes = [C.c_double]
+        _lib.orc_decay_count.restype = C.c_uint64
+        _lib.orc_decay_count.argtypes = [C.c_double, C.c_double, C.c_double]
         _lib.orc_rotate.argtypes = [C.POINTER(C.c_double)] + [C.c_double] * 4
         _lib.orc_rotate.restype = None
         _lib.orc_mu_lookup.argtypes = [C.POINTER(_Materials), C.c_int, C.c_double, C.POINTER(C.c_double)]
@@ -167,7 +176,7 @@ def _source(src) -> _Keep:
                 src.pairs_per_time_slice, None if act is None else _p(act, C.c_float),
                 None if ph is None else _p(ph, C.c_uint8), src.phantom_majorant_material,
                 (C.c_int32 * 3)(*src.dims), (C.c_float * 3)(*src.voxel_mm), (C.c_float * 3)(*src.origin_mm),
-                (C.c_float * 3)(*src.beam_dir))
+                (C.c_float * 3)(*src.beam_dir), src.positron_fwhm_mm, src.half_life_s, src.duration_s)
     if lib().orc_source_prepare(C.byref(s)) != 0:
         raise ValueError("source has no active voxel")
     return _Keep(s, act, ph)
@@ -318,6 +327,28 @@ def decay_sites(source, seed: int, first: int, n: int) -> np.ndarray:
         return out
     finally:
         lib().orc_source_release(C.byref(s.struct))
+
+
+def annihilation_sites(source, seed: int, first: int, n: int) -> np.ndarray:
+    s = _source(source)
+    try:
+        out = np.zeros((n, 3), np.float64)
+        lib().orc_annihilation_sites(C.byref(s.struct), seed, first, n, _p(out, C.c_double))
+        return out
+    finally:
+        lib().orc_source_release(C.byref(s.struct))
+
+
+def det_log(z: float) -> float:
+    return float(lib().orc_det_log(z))
+
+
+def det_log1m(y: float) -> float:
+    return float(lib().orc_det_log1m(y))
+
+
+def decay_count(activity_bq: float, half_life_s: float, duration_s: float) -> int:
+    return int(lib().orc_decay_count(activity_bq, half_life_s, duration_s))
 
 
 def rotate(d, ct: float, st: float, cp: float, sp: float) -> np.ndarray:

@@ -41,7 +41,8 @@ class _Source(C.Structure):
     _fields_ = [("kind", C.c_int32), ("pos_mm", C.c_float * 3), ("beam_dir", C.c_float * 3),
                 ("acolinearity_fwhm_deg", C.c_float), ("activity_bq", C.c_double), ("pairs_per_time_slice", C.c_uint64),
                 ("activity_map", C.c_void_p), ("phantom_material", C.c_void_p), ("phantom_majorant_material", C.c_int32),
-                ("dims", C.c_int32 * 3), ("voxel_mm", C.c_float * 3), ("origin_mm", C.c_float * 3)]
+                ("dims", C.c_int32 * 3), ("voxel_mm", C.c_float * 3), ("origin_mm", C.c_float * 3),
+                ("positron_fwhm_mm", C.c_float), ("half_life_s", C.c_double), ("duration_s", C.c_double)]
 
 
 class _Hits(C.Structure):
@@ -72,7 +73,7 @@ EXPORTS = ("gpet_geometry_create", "gpet_geometry_destroy", "gpet_geometry_panel
            "gpet_materials_load", "gpet_materials_destroy", "gpet_activity_create", "gpet_activity_destroy",
            "gpet_simulate", "gpet_digitize_scratch_bytes", "gpet_digitize", "gpet_run_host", "gpet_last_error",
            "gpet_launch_count", "gpet_set_transport_warps", "gpet_pipeline_create", "gpet_pipeline_submit", "gpet_pipeline_collect",
-           "gpet_pipeline_destroy", "gpet_shutdown")
+           "gpet_pipeline_destroy", "gpet_shutdown", "gpet_decay_count")
 
 _lib = None
 
@@ -107,6 +108,7 @@ def lib():
         L.gpet_pipeline_submit.argtypes = [vp, u64, u64, u64]
         L.gpet_pipeline_collect.argtypes = [vp, C.POINTER(_HostOutputs)]
         L.gpet_pipeline_destroy.argtypes = [vp]
+        L.gpet_decay_count.argtypes = [C.c_double, C.c_double, C.c_double, C.POINTER(u64)]
         L.gpet_last_error.restype = C.c_char_p
         L.gpet_launch_count.restype = u64
         L.gpet_set_transport_warps.argtypes = [i32]
@@ -117,6 +119,12 @@ def lib():
 def _check(rc: int):
     if rc != 0:
         raise GpetError(f"libgpet error {rc}: {lib().gpet_last_error().decode()}")
+
+
+def gpet_decay_count(activity_bq: float, half_life_s: float, duration_s: float) -> int:
+    n = C.c_uint64(0)
+    _check(lib().gpet_decay_count(activity_bq, half_life_s, duration_s, C.byref(n)))
+    return int(n.value)
 
 
 def gpet_launch_count() -> int:
@@ -233,7 +241,8 @@ class DeviceSource:
 def _source_struct(src, activity_ptr, phantom_ptr) -> _Source:
     return _Source(src.kind, (C.c_float * 3)(*src.pos_mm), (C.c_float * 3)(*src.beam_dir), src.acolinearity_fwhm_deg,
                    src.activity_bq, src.pairs_per_time_slice, activity_ptr, phantom_ptr, src.phantom_majorant_material,
-                   (C.c_int32 * 3)(*src.dims), (C.c_float * 3)(*src.voxel_mm), (C.c_float * 3)(*src.origin_mm))
+                   (C.c_int32 * 3)(*src.dims), (C.c_float * 3)(*src.voxel_mm), (C.c_float * 3)(*src.origin_mm),
+                   src.positron_fwhm_mm, src.half_life_s, src.duration_s)
 
 
 # ----------------------------------------------------------------------------- device buffers (torch tensors)

@@ -43,6 +43,12 @@ static int fail(int code, const char *fmt, ...) {
   return fail(GPET_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
 
 extern "C" const char *gpet_last_error(void) { return g_err; }
+extern "C" int gpet_decay_count(double activity_bq, double half_life_s, double duration_s, uint64_t *n_pairs) {
+  if (!n_pairs || !(activity_bq > 0.0) || !(duration_s > 0.0) || half_life_s < 0.0) return fail(GPET_E_INVALID_ARG, "gpet_decay_count: bad argument");
+  if (!(half_life_s > 0.0)) { *n_pairs = (uint64_t)llrint(activity_bq * duration_s); return GPET_OK; }
+  const double lambda = 0.69314718055994530942 / half_life_s;
+  *n_pairs = (uint64_t)llrint(activity_bq / lambda * -expm1(-lambda * duration_s)); return GPET_OK;
+}
 extern "C" uint64_t gpet_launch_count(void) { return g_launches.load(); }
 extern "C" int gpet_set_transport_warps(int32_t warps) { set_transport_warps(warps); return transport_warps(); }
 
@@ -357,6 +363,8 @@ static int make_source(const gpet_source *s, const gpet_materials *m, DevSource 
   }
   if (!(s->activity_bq > 0.0)) return fail(GPET_E_INVALID_ARG, "activity_bq must be positive");
   D->activity_bq = s->activity_bq; D->pairs_per_slice = s->pairs_per_time_slice;
+  if (!(s->positron_fwhm_mm >= 0.0f)) return fail(GPET_E_INVALID_ARG, "negative positron range");
+  D->positron_sigma = (float)((double)s->positron_fwhm_mm / 2.354820045030949);
   if (s->kind == 1) {
     if (!s->activity_map) return fail(GPET_E_INVALID_ARG, "kind 1 needs an activity_map");
     for (int k = 0; k < 3; ++k) if (s->dims[k] != s->activity_map->dims[k] || !(s->voxel_mm[k] > 0.0f))
@@ -459,6 +467,11 @@ static int make_digi(const gpet_source *src, uint64_t seed, uint64_t n_pairs_tot
   P->shift = d->readout_level == 0 ? 5 : (d->readout_level == 1 ? 20 : 26);
   P->activity_bq = src->activity_bq; P->pairs_per_slice = src->pairs_per_time_slice ? src->pairs_per_time_slice : n_pairs_total;
   P->seed = seed; P->slice_s = (double)P->pairs_per_slice / P->activity_bq;
+  P->lambda = 0.0; P->pfrac = 0.0; P->q_scale = (double)P->pairs_per_slice / (double)n_pairs_total;
+  if (src->half_life_s > 0.0) {                                      // [R34] decay law
+    if (!(src->duration_s > 0.0)) return fail(GPET_E_INVALID_ARG, "half_life_s > 0 needs duration_s > 0");
+    P->lambda = 0.69314718055994530942 / src->half_life_s; P->pfrac = -expm1(-P->lambda * src->duration_s);
+  } else if (src->half_life_s < 0.0) return fail(GPET_E_INVALID_ARG, "negative half-life");
   return GPET_OK;
 }
 

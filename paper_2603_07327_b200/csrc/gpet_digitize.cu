@@ -14,6 +14,8 @@
 //   4. head-flag pass: a thread per cluster start (gap >= tau) walks its cluster with the window rule [R27];
 //      exclusive scan of the pair flags; compaction into list-mode output.
 // Every stage is deterministic: the output does not depend on the order of the hit buffer.
+#include <cmath>
+#include <cstring>
 #include "gpet_internal.h"
 
 namespace gpet {
@@ -163,14 +165,72 @@ __device__ __forceinline__ uint32_t bucket_of(const Buckets &B, double t) {
   return x >= (double)(B.nb - 1) ? B.nb - 1 : (uint32_t)x;
 }
 
-__device__ __forceinline__ double decay_time(const DigiParams &P, uint64_t history) {     // [R16]
+// [R34] ln(z), z in (0, 1], and ln(1 - y), y in [0, 1), from IEEE +, -, *, / only (round-to-nearest intrinsics: no FMA
+// contraction, no library logarithm), operation for operation what the fp64 reference definition does, so that decay
+// times come out bit-identical on both sides.  z = m 2^e, m in [sqrt(1/2), sqrt(2)); ln m = 2 atanh((m-1)/(m+1)).
+__host__ __device__ inline double det_series(double s) {
+#ifdef __CUDA_ARCH__
+  const double s2 = __dmul_rn(s, s); double p = 1.0 / 25.0;
+  for (int k = 23; k >= 1; k -= 2) p = __dadd_rn(__dmul_rn(p, s2), 1.0 / (double)k);
+  return __dmul_rn(__dmul_rn(2.0, s), p);
+#else
+  volatile double s2 = s * s; volatile double p = 1.0 / 25.0;       // volatile: keep the host compiler from contracting
+  for (int k = 23; k >= 1; k -= 2) { volatile double t = p * s2; p = t + 1.0 / (double)k; }
+  volatile double t2 = 2.0 * s; return t2 * p;
+#endif
+}
+__host__ __device__ inline double det_log(double z) {
+#ifdef __CUDA_ARCH__
+  unsigned long long bits = (unsigned long long)__double_as_longlong(z);
+#else
+  unsigned long long bits; memcpy(&bits, &z, 8);
+#endif
+  int e = (int)((bits >> 52) & 0x7FF) - 1022;
+  bits = (bits & 0x000FFFFFFFFFFFFFull) | 0x3FE0000000000000ull;
+#ifdef __CUDA_ARCH__
+  double m = __longlong_as_double((long long)bits);
+  if (m < 0.70710678118654752440) { m = __dmul_rn(m, 2.0); e -= 1; }
+  const double s = __ddiv_rn(__dsub_rn(m, 1.0), __dadd_rn(m, 1.0));
+  return __dadd_rn(__dmul_rn((double)e, 0.69314718055994530942), det_series(s));
+#else
+  double m; memcpy(&m, &bits, 8);
+  if (m < 0.70710678118654752440) { m = m * 2.0; e -= 1; }
+  volatile double num = m - 1.0, den = m + 1.0; volatile double s = num / den;
+  volatile double a = (double)e * 0.69314718055994530942; return a + det_series(s);
+#endif
+}
+__host__ __device__ inline double det_log1m(double y) {
+  if (y < 0.25) {
+#ifdef __CUDA_ARCH__
+    return det_series(__ddiv_rn(-y, __dsub_rn(2.0, y)));
+#else
+    volatile double den = 2.0 - y; volatile double s = -y / den; return det_series(s);
+#endif
+  }
+#ifdef __CUDA_ARCH__
+  return det_log(__dsub_rn(1.0, y));
+#else
+  volatile double z = 1.0 - y; return det_log(z);
+#endif
+}
+// [R16] t0 = (slice + u53) B / A; [R34] with a half-life: t0 = -ln(1 - q P) / lambda, q = (slice + u53) B / N
+__host__ __device__ inline double decay_time_of(const DigiParams &P, double slice_plus_u) {
+#ifdef __CUDA_ARCH__
+  if (P.lambda > 0.0) return __ddiv_rn(-det_log1m(__dmul_rn(__dmul_rn(slice_plus_u, P.q_scale), P.pfrac)), P.lambda);
+  return __dmul_rn(slice_plus_u, P.slice_s);
+#else
+  if (P.lambda > 0.0) { volatile double q = slice_plus_u * P.q_scale; volatile double y = q * P.pfrac; return -det_log1m(y) / P.lambda; }
+  return slice_plus_u * P.slice_s;
+#endif
+}
+__device__ __forceinline__ double decay_time(const DigiParams &P, uint64_t history) {
   const uint2 key = make_uint2((uint32_t)P.seed, (uint32_t)(P.seed >> 32));
   const uint4 w = philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 0u, 2u), key);
   const uint64_t bits = (((uint64_t)w.x << 32) | (uint64_t)w.y) >> 11;
   const double u53 = __dmul_rn(__dadd_rn((double)bits, 0.5), 1.0 / 9007199254740992.0);
   const uint64_t B = P.pairs_per_slice;
   const uint64_t slice = history < B ? 0ull : history / B;
-  return __dmul_rn(__dadd_rn((double)slice, u53), P.slice_s);                               // slice_s = B / A
+  return decay_time_of(P, __dadd_rn((double)slice, u53));
 }
 
 // [R25] standard normal by Box-Muller.  The blurred energy must stay within 1e-3 keV of the fp64 oracle's: sigma is
@@ -459,8 +519,9 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   const uint64_t B = P.pairs_per_slice;
   const double slice_s = (double)B / P.activity_bq;
   Buckets bk; bk.nb = (uint32_t)L.nb;
-  bk.t_lo = (double)(first_history / B) * slice_s;
-  const double t_hi = ((double)((first_history + n_pairs - 1) / B) + 1.0) * slice_s + 2e-6;
+  (void)slice_s;
+  bk.t_lo = decay_time_of(P, (double)(first_history / B));          // the batch's time slices cover [t_lo, t_hi) [R16, R34]
+  const double t_hi = decay_time_of(P, fmin((double)((first_history + n_pairs - 1) / B) + 1.0, P.lambda > 0.0 ? 1.0 / P.q_scale : 1e300)) + 2e-6;
   bk.scale = (double)bk.nb / (t_hi - bk.t_lo);
   const int ga = grid_for(M);                                         // adder and bucket scatter share the block -> region split
   if (chunked) {

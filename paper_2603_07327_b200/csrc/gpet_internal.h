@@ -21,12 +21,14 @@ struct DevSource {
   const uint32_t *act_index; const uint64_t *act_cdf; uint32_t n_active; uint64_t w_total;
   const uint8_t *phantom; int ph_major; int dims[3]; float voxel[3], inv_voxel[3], origin[3];
   double activity_bq; uint64_t pairs_per_slice;
+  float positron_sigma;                                          // [R35] mm per axis, 0 = off
 };
 
 struct DigiParams {
   float sigma_scale;       // R / 2.3548
   float ref_keV, e_lo, e_hi; double window_s; int shift;         // ids >> shift = readout unit
   double activity_bq, slice_s; uint64_t pairs_per_slice; uint64_t seed;   // slice_s = pairs_per_slice / activity_bq
+  double lambda, pfrac, q_scale;                                 // [R34] decay law: ln2 / half-life (0 = constant activity), 1 - exp(-lambda T), B / N
 };
 
 struct SinglesBuf { uint32_t *history, *ids; float *x, *y, *z, *e; double *t; unsigned long long capacity; unsigned long long *n; };

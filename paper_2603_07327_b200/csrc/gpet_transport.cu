@@ -528,6 +528,12 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
         const uint64_t history = history_of(j);
         const uint32_t h_lo = (uint32_t)history, h_hi = (uint32_t)(history >> 32);
         if (kind == 1) decay_site(src, philox4x32_10(make_uint4(h_lo, h_hi, 0u, 0u), key), q.x);
+        if (src.positron_sigma > 0.0f) {                             // [R35] positron range: words 12-15 of the source stream
+          const uint4 w3 = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 3u), key);
+          const float r1 = src.positron_sigma * sqrtf(-2.0f * logf(u01(w3.x))), r2 = src.positron_sigma * sqrtf(-2.0f * logf(u01(w3.z)));
+          float s1, c1, s2, c2; sincospif(2.0f * u01(w3.y), &s1, &c1); sincospif(2.0f * u01(w3.w), &s2, &c2);
+          q.x[0] = fmaf(r1, c1, q.x[0]); q.x[1] = fmaf(r1, s1, q.x[1]); q.x[2] = fmaf(r2, c2, q.x[2]);
+        }
         w = philox4x32_10(make_uint4(h_lo, h_hi, 0u, 1u), key);
         if (kind == 2) { q.d[0] = src.beam[0]; q.d[1] = src.beam[1]; q.d[2] = src.beam[2]; }
         else {
@@ -899,10 +905,11 @@ cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, cons
   // specialised builds for the shapes the five configs use (point source or voxel map + phantom, in a repetition-mode
   // ring); anything else runs the generic build of the same code
   const bool ring = planar_hint != 0 && host_geom.ring != 0 && host_geom.ring_edge_h > 0.0f;
+  const bool point = !phantom && src.kind == 0 && !(src.positron_sigma > 0.0f);   // every pair starts at src.pos
 #define GPET_DISPATCH(H)                                                                                                    \
   do {                                                                                                                      \
-    if (!phantom && src.kind == 0 && ring && pretest) e = launch(transport_wavefront_kernel<H, false, 0, 1, true, true>);    \
-    else if (!phantom && src.kind == 0 && ring) e = launch(transport_wavefront_kernel<H, false, 0, 1, false, true>);        \
+    if (point && ring && pretest) e = launch(transport_wavefront_kernel<H, false, 0, 1, true, true>);                        \
+    else if (point && ring) e = launch(transport_wavefront_kernel<H, false, 0, 1, false, true>);                            \
     else if (phantom && ring) e = launch(transport_wavefront_kernel<H, true, 1, 1, false, true>);                           \
     else if (phantom) e = launch(transport_wavefront_kernel<H, true, 1, -1, false, false>);                                 \
     else if (pretest) e = launch(transport_wavefront_kernel<H, false, -1, -1, true, false>);                                \

@@ -15,6 +15,7 @@ from typing import List, Optional, Sequence, Tuple
 
 import numpy as np
 
+F18_HALF_LIFE_S = 109.77 * 60.0     # 18F (1.6e8 atoms <-> 1.70e-2 MBq)
 # physical constants used to build the synthetic tables (BASELINE.json C0)
 R_E_CM = 2.8179403262e-13          # classical electron radius [cm]
 ME_C2_KEV = 510.99895              # electron rest energy [keV]
@@ -66,6 +67,9 @@ class Source:
     voxel_mm: Tuple[float, float, float] = (0.0, 0.0, 0.0)
     origin_mm: Tuple[float, float, float] = (0.0, 0.0, 0.0)   # low corner of voxel (0,0,0)
     beam_dir: Tuple[float, float, float] = (1.0, 0.0, 0.0)    # kind 2: direction of photon A (B is opposite)
+    positron_fwhm_mm: float = 0.0          # 0 = annihilation at the emission site, as in the paper
+    half_life_s: float = 0.0               # > 0: decay law over duration_s, activity_bq = initial activity
+    duration_s: float = 0.0
 
 
 @dataclass(frozen=True)

@@ -33,11 +33,21 @@ def test_library_exports_every_declared_symbol():
     assert sorted(api.EXPORTS) == names
 
 
-def test_binding_structs_match_the_header_layout():
-    # sizes follow from the C declarations (LP64): checked so that a header edit cannot silently skew the binding
-    assert ctypes.sizeof(api._LayerDesc) == 48 and ctypes.sizeof(api._GeometryDesc) == 64
-    assert ctypes.sizeof(api._Source) == 104 and ctypes.sizeof(api._Hits) == 88
-    assert ctypes.sizeof(api._Digitizer) == 32 and ctypes.sizeof(api._Singles) == 72 and ctypes.sizeof(api._Coinc) == 80
+def test_binding_structs_match_the_header_layout(tmp_path):
+    """sizeof and the offset of the last member of every struct of gpet.h, as gcc lays them out, against the ctypes mirrors
+    of the binding: a header edit cannot silently skew the binding."""
+    import subprocess
+    pairs = [("gpet_layer_desc", "gap_material", api._LayerDesc), ("gpet_geometry_desc", "layers", api._GeometryDesc),
+             ("gpet_source", "duration_s", api._Source), ("gpet_hits", "chunk_fill", api._Hits), ("gpet_digitizer", "readout_level", api._Digitizer),
+             ("gpet_singles", "n_singles", api._Singles), ("gpet_coincidences", "n_coinc", api._Coinc), ("gpet_host_outputs", "coinc", api._HostOutputs)]
+    src = tmp_path / "sz.c"
+    body = "".join(f'printf("%zu %zu\\n", sizeof({c}), offsetof({c}, {m}));' for c, m, _ in pairs)
+    src.write_text(f'#include <stdio.h>\n#include <stddef.h>\n#include "gpet.h"\nint main(void){{{body}return 0;}}\n')
+    exe = tmp_path / "sz"
+    subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), "-o", str(exe), str(src)])
+    out = subprocess.check_output([str(exe)], text=True).split()
+    for k, (c, m, t) in enumerate(pairs):
+        assert ctypes.sizeof(t) == int(out[2 * k]) and getattr(t, m).offset == int(out[2 * k + 1]), (c, out[2 * k:2 * k + 2])
 
 
 def test_ring_placement_equals_the_oracles_bit_for_bit():

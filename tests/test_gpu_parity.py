@@ -637,7 +637,7 @@ def test_phantom_rayleigh_parity_and_thomson_distribution(tables):
     r = W.Run("ph_rayleigh", geom, src, 300_001, 12)
     g, gh, cnt, o = run_both(r, t)
     res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
-    assert res["frac"] >= MIN_MATCH and cnt >= 2 * r.n_pairs - 20, res   # closed absorber: every photon is caught (bar the cube's edges)
+    assert res["frac"] >= MIN_MATCH and cnt > 0.99 * 2 * r.n_pairs, res   # every photon is caught, bar the open channels along the cube's edges
     geom, t, src = phantom_rayleigh_setup()
     r = W.Run("ph_rayleigh_thin", geom, src, 2_000_000, 12)
     g, gh, cnt = PU.gpu_simulate(r, t)
@@ -666,3 +666,55 @@ def test_ring_handedness_against_hand_written_numbers(tables):
     pts = np.array([[56.0, 3.5, 0.5], [56.0, -3.5, 0.5], [56.0, 0.5, -20.5], [-3.5, 56.0, 0.5], [3.5, 56.0, 0.5], [-56.0, -3.5, 0.5]], np.float32)
     want = [pack(0, 1, 2, 3, 0), pack(0, 0, 2, 12, 0), pack(0, 1, 0, 0, 11), pack(3, 1, 2, 3, 0), pack(3, 0, 2, 12, 0), pack(6, 1, 2, 3, 0)]
     assert list(api.gpet_geometry_locate(g, pts)) == want
+
+
+# ----------------------------------------------------------------------------- SURVEY 8(f) rank 3: decay law, positron range
+def test_decay_law_times_are_bit_identical(tables):
+    """[R34] a decaying source (half-life 20 ms watched for 50 ms: 2.5 half-lives, both branches of the restated logarithm):
+    the digitizer's fp64 decay times equal the oracle's bit for bit, in one slice and in time slices, and so do the
+    coincidences built on them; the expected count comes from gpet_decay_count."""
+    from dataclasses import replace
+    a0, th, T = 5.0e7, 0.02, 0.05
+    n_total = api.gpet_decay_count(a0, th, T)
+    assert n_total == O.decay_count(a0, th, T) and 1_180_000 < n_total < 1_195_000
+    assert api.gpet_decay_count(1.6e8 * np.log(2.0) / W.F18_HALF_LIFE_S, W.F18_HALF_LIFE_S, 120.0) == 2_007_947     # PAPER.md:61
+    n = 300_000
+    for slice_pairs, first in ((0, 0), (100_000, 800_000)):
+        src = replace(W.source_point((10.0, 0.0, 4.0), activity_bq=a0), half_life_s=th, duration_s=T, pairs_per_time_slice=slice_pairs)
+        o = O.simulate(W.geometry_c3(), tables, src, n, 405, first_history=first, threads=8)
+        dig = W.Digitizer(0.15, 511.0, 350.0, 650.0, 4.0, 1)
+        osg, oco, _ = O.digitize(src, 405, n_total, o.hits, dig)
+        hb = PU.upload_hits(PU.oracle_hits_dict(o.hits), np.random.default_rng(3).permutation(len(o.hits)))
+        s = api.DeviceSource(src)
+        scratch = torch.empty(api.gpet_digitize_scratch_bytes(n, len(o.hits)), dtype=torch.uint8, device="cuda")
+        sg, co = api.SinglesBuffer.allocate(len(o.hits)), api.CoincBuffer.allocate(len(o.hits))
+        api.gpet_digitize(s, 405, n_total, first, n, hb, len(o.hits), dig, scratch, sg, co)
+        torch.cuda.synchronize()
+        gs = sg.to_numpy()
+        assert PU.compare_singles(gs, osg, 20, exact=True, max_symdiff=2) >= len(osg.ids) - 2 > 50_000
+        assert PU.compare_coincidences(co.to_numpy(), oco, exact=True, max_symdiff=4) >= len(oco.ids_a) - 4 > 3000
+        assert np.all(np.diff(gs["t_s"]) >= 0) and gs["t_s"].max() < T
+        if first:                                                      # histories 800k.. of 1.19M: late in the decay curve
+            assert gs["t_s"].min() > 0.02
+
+
+@pytest.mark.parametrize("kind", ["point", "rods_in_phantom"])
+def test_positron_range_parity(tables, kind):
+    """[R35] positron range switched on (0.5 mm FWHM, five times 18F's: PAPER.md:145): every pair starts at its own
+    annihilation point -- outcome hashes and hits against the oracle for a point source on C3's ring and for the hot-rod
+    source inside its water phantom."""
+    from dataclasses import replace
+    if kind == "point":
+        r = W.Run("positron", W.geometry_c3(), replace(W.source_point((10.0, 0.0, 4.0)), positron_fwhm_mm=0.5), 300_001, 66)
+    else:
+        c4 = W.config_runs("C4", 150_000)[0]
+        r = replace(c4, source=replace(c4.source, positron_fwhm_mm=0.5))
+    g, gh, cnt, o = run_both(r, tables)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= MIN_MATCH and res["n_hits_compared"] > 50_000, res
+    # the first hits of photon A no longer lie on lines through ONE point: their time of flight differs from |x - source| / c
+    if kind == "point":
+        first = (g["ids"] & 31) == 0
+        d = np.sqrt((g["x"][first] - 10.0) ** 2 + g["y"][first] ** 2 + (g["z"][first] - 4.0) ** 2) / 299.792458 - g["tof_ns"][first]
+        mad = 1.4826 * np.median(np.abs(d - np.median(d))) * 299.792458     # robust: 2 % of the photons are Rayleigh-deflected on the way
+        assert 0.1 < mad < 0.4                                         # ~ sigma of the displacement along the line of flight (0.21 mm)

@@ -777,3 +777,74 @@ def test_ring_handedness_against_hand_written_numbers():
                    np.float32)
     want = [pack(0, 1, 2, 3, 0), pack(0, 0, 2, 12, 0), pack(0, 1, 0, 0, 11), pack(3, 1, 2, 3, 0), pack(3, 0, 2, 12, 0), pack(6, 1, 2, 3, 0)]
     assert list(O.locate(g, pts)) == want
+
+
+# ----------------------------------------------------------------------------- decay law, positron range
+def test_f18_source_of_the_paper():
+    """1.6e8 atoms of 18F are `about 1.70e-2 MBq`; over the 120 s acquisition N0 (1 - exp(-lambda T)) of them
+    decay.  [R34] the expected count is what a run simulates (n_pairs_total)."""
+    lam = math.log(2.0) / W.F18_HALF_LIFE_S
+    a0 = 1.6e8 * lam
+    assert abs(a0 / 1.70e4 - 1.0) < 0.015                              # the paper rounds: 1.684e-2 MBq
+    n = O.decay_count(a0, W.F18_HALF_LIFE_S, 120.0)
+    assert n == round(1.6e8 * (1.0 - math.exp(-lam * 120.0))) == 2_007_947
+    assert O.decay_count(1.0e6, 0.0, 10.0) == 10_000_000              # constant activity: A T
+    assert abs(O.decay_count(a0, W.F18_HALF_LIFE_S, 1e9) / 1.6e8 - 1.0) < 1e-9    # every atom decays in the end
+
+
+def test_deterministic_log_equals_the_library_logarithm():
+    """[R34] the logarithm restated with +, -, *, / only (so that both sides get bit-identical decay times)."""
+    rng = np.random.default_rng(17)
+    z = np.concatenate([rng.uniform(0.0, 1.0, 20000), 1.0 - 10.0 ** rng.uniform(-15, -1, 5000), 10.0 ** rng.uniform(-12, 0, 5000), [1.0, 0.5, 0.25]])
+    z = z[(z > 0) & (z <= 1.0)]
+    got = np.array([O.det_log(float(v)) for v in z])
+    want = np.log(z)
+    assert np.all(np.abs(got - want) <= 4e-16 * np.maximum(np.abs(want), 1.0))
+    y = np.concatenate([10.0 ** rng.uniform(-18, 0, 20000), rng.uniform(0.0, 1.0, 5000), [0.0, 0.25, 0.2499999]])
+    y = y[y < 1.0]
+    got = np.array([O.det_log1m(float(v)) for v in y])
+    want = np.log1p(-y)
+    assert np.all(np.abs(got[y > 0] / want[y > 0] - 1.0) < 1e-15) and O.det_log1m(0.0) == 0.0
+
+
+def test_decay_times_follow_the_truncated_decay_law():
+    """[R34] half-life 100 s observed for 250 s: decay times have the cdf (1 - exp(-lambda t)) / (1 - exp(-lambda T)) (KS),
+    every time slice covers its own stretch of the time axis, and a half-life far longer than the acquisition gives back
+    the constant-activity times of [R16]."""
+    lam, T, n = math.log(2.0) / 100.0, 250.0, 20_000
+    src = W.Source(activity_bq=1.0, half_life_s=100.0, duration_s=T)
+    t = np.array([O.decay_time(src, 9, h, n) for h in range(n)])
+    cdf = lambda x: (1.0 - np.exp(-lam * x)) / (1.0 - math.exp(-lam * T))
+    assert t.min() > 0 and t.max() < T and stats.kstest(t, cdf).pvalue > 1e-3
+    assert abs(np.mean(t < 100.0) - 0.5 / (1.0 - 0.5 ** 2.5)) < 0.01   # half of ALL atoms decay in the first half-life
+    src4 = W.Source(activity_bq=1.0, half_life_s=100.0, duration_s=T, pairs_per_time_slice=n // 4)
+    t4 = np.array([O.decay_time(src4, 9, h, n) for h in range(n)])
+    edges = -np.log(1.0 - np.arange(5) / 4.0 * (1.0 - math.exp(-lam * T))) / lam
+    for k in range(4):
+        s = t4[k * n // 4:(k + 1) * n // 4]
+        assert edges[k] <= s.min() and s.max() <= edges[k + 1]
+    assert stats.kstest(t4, cdf).pvalue > 1e-3
+    slow = W.Source(activity_bq=50.0, half_life_s=1e12, duration_s=n / 50.0)
+    ref = W.Source(activity_bq=50.0)
+    for h in (0, 17, n - 1):
+        assert abs(O.decay_time(slow, 9, h, n) / O.decay_time(ref, 9, h, n) - 1.0) < 1e-8
+
+
+def test_positron_range_is_an_isotropic_gaussian():
+    """[R35] off (the paper's setting): the annihilation point IS the emission site.  On: the displacement is
+    Gaussian on every axis with the stated FWHM (PAPER.md:145 quotes 0.102 mm for 18F), uncorrelated between axes."""
+    n = 200_000
+    off = W.source_point((1.0, -2.0, 3.0))
+    assert np.array_equal(O.annihilation_sites(off, 4, 0, 100), O.decay_sites(off, 4, 0, 100))
+    on = W.Source(0, (1.0, -2.0, 3.0), 0.5, 1e6, positron_fwhm_mm=0.102)
+    d = O.annihilation_sites(on, 4, 0, n) - np.array([1.0, -2.0, 3.0])
+    sigma = 0.102 / 2.354820045
+    for k in range(3):
+        assert stats.kstest(d[:, k] / sigma, "norm").pvalue > 1e-3
+    c = np.cov(d.T) / sigma ** 2
+    assert np.all(np.abs(c - np.eye(3)) < 0.02)
+    # the voxel source is displaced from its sampled site, not from the grid origin
+    rods = W.source_hot_rods()
+    from dataclasses import replace
+    a, b = O.decay_sites(rods, 5, 0, 1000), O.annihilation_sites(replace(rods, positron_fwhm_mm=0.102), 5, 0, 1000)
+    assert 0.02 < np.abs(a - b).max() < 0.5 and abs(np.std(a - b) / sigma - 1.0) < 0.1

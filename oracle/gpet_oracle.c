@@ -70,7 +70,7 @@ typedef struct {
 
 typedef struct {             /* event counters (metrics; also feed the roofline model) */
   uint64_t pairs, searches, entries, steps, step_vacuum, virtuals, pe, compton, kn_trials,
-           rayleigh, cutoffs, exits, escapes, hits, ph_steps, ph_compton, ph_absorbed, ph_cutoff;
+           rayleigh, cutoffs, exits, escapes, hits, ph_steps, ph_compton, ph_absorbed, ph_cutoff, region_crossings;
 } orc_counters;
 
 typedef struct { float fwhm_frac, ref_keV, e_lo, e_hi; double window_ns; int32_t level; } orc_digitizer;
@@ -121,6 +121,9 @@ typedef struct {
   int nmod[2]; int64_t msq[2], mpq[2];
   int n_layers;
   struct { int n[2]; int64_t pitch[2], gap[2], off[2], c0, depth; int cmat, gmat; } layer[ORC_MAX_LAYERS];
+  /* [R19] majorant regions: maximal runs of consecutive layers with the same crystal and gap material; region r spans
+   * the depths [reg_c[r], reg_c[r+1]) (the gap in front of a region's first layer belongs to the region before it) */
+  int n_regions; int64_t reg_c[ORC_MAX_LAYERS + 1]; uint32_t reg_mask[ORC_MAX_LAYERS];
 } geom_t;
 
 static int64_t quant(float x) { return llrint((double)x * ORC_Q); }   /* [R7] */
@@ -177,6 +180,15 @@ static int geom_build(const orc_geometry *d, geom_t *g) {
     if (s->n[0] * s->n[1] > 8192) return -1;
   }
   g->Dq = c;
+  g->n_regions = 0;
+  for (int l = 0; l < g->n_layers; ++l) {
+    if (l == 0 || g->layer[l].cmat != g->layer[l - 1].cmat || g->layer[l].gmat != g->layer[l - 1].gmat) {
+      g->reg_c[g->n_regions] = l == 0 ? 0 : g->layer[l].c0; g->reg_mask[g->n_regions] = 0; g->n_regions++;
+    }
+    g->reg_mask[g->n_regions - 1] |= 1u << g->layer[l].cmat;
+    if (g->layer[l].gmat >= 0) g->reg_mask[g->n_regions - 1] |= 1u << g->layer[l].gmat;
+  }
+  g->reg_c[g->n_regions] = g->Dq;
   return 0;
 }
 static void geom_free(geom_t *g) { free(g->panel); g->panel = NULL; }
@@ -246,6 +258,14 @@ static int slab(const double lo[3], const double hi[3], const double x[3], const
     if (t2 < b) b = t2;
   }
   *tn = a; *tf = b; return 1;
+}
+/* Distance along the ray to the far face of each slab of a box the point is inside of, and their minimum; returns the
+ * axis of the face met first (ties: the first of a, b, c).  A zero direction component never limits [R32]. */
+static int slab_far(const double lo[3], const double hi[3], const double x[3], const double d[3], double tfar[3], double *tf) {
+  int kx = 2; double best = INFINITY;
+  for (int k = 0; k < 3; ++k) tfar[k] = d[k] == 0.0 ? INFINITY : ((d[k] > 0.0 ? hi[k] : lo[k]) - x[k]) / d[k];
+  for (int k = 2; k >= 0; --k) if (tfar[k] <= best) { best = tfar[k]; kx = k; }
+  *tf = best; return kx;
 }
 /* [R6] nearest-entry panel over all panels but `excl`; ties -> lowest index; -1 = escapes */
 static int panel_search(const geom_t *g, const double x[3], const double d[3], int excl, double *t_enter) {
@@ -362,7 +382,7 @@ double orc_rayleigh_cos(double u) { double a = 4.0 * u - 2.0, q = sqrt(a * a + 1
 
 /* ------------------------------------------------------------------ hash [R23] */
 enum { EV_ENTER = 1, EV_STEP_VACUUM, EV_VIRTUAL, EV_PE, EV_COMPTON, EV_RAYLEIGH, EV_CUTOFF, EV_EXIT, EV_ESCAPE,
-       EV_PH_COMPTON, EV_PH_RAYLEIGH, EV_PH_ABSORBED, EV_PH_CUTOFF, EV_PH_LEAVE };
+       EV_PH_COMPTON, EV_PH_RAYLEIGH, EV_PH_ABSORBED, EV_PH_CUTOFF, EV_PH_LEAVE, EV_REGION };
 static void hash_ev(uint64_t *h, uint32_t type, uint32_t payload) {
   *h = (*h ^ (uint64_t)type) * 0x100000001B3ull;        /* FNV-1a over 32-bit words */
   *h = (*h ^ (uint64_t)payload) * 0x100000001B3ull;
@@ -512,15 +532,24 @@ static void transport_photon(ctx_t *c, uint64_t seed, uint64_t history, int phot
     for (int k = 0; k < 3; ++k) xl[k] += te * dl[k];                 /* [R18] move to the entry point */
     path += te;
     int alive = 1;
-    for (;;) {                                                       /* [R19] whole-panel Woodcock    */
-      double mu_maj = mu_majorant(M, c->det_mask, E);
+    int reg = 0;                                                     /* [R19] region of the entry point (by its depth) */
+    for (int k = 1; k < g->n_regions; ++k) if (xl[2] >= (double)g->reg_c[k] / ORC_Q) reg = k;
+    for (;;) {                                                       /* [R19] Woodcock tracking, one majorant per region */
+      double mu_maj = mu_majorant(M, g->reg_mask[reg], E);
       double u[4]; rng_next_block(&r, u);                            /* [R4] free path, outcome, Rayleigh polar, azimuth */
-      double s = -log(u[0]) / mu_maj, tn, tf; c->C->steps++;
-      slab(blo, bhi, xl, dl, &tn, &tf);                              /* distance to the box exit      */
+      double s = -log(u[0]) / mu_maj, tfar[3], tf; c->C->steps++;
+      double rlo[3] = { blo[0], blo[1], (double)g->reg_c[reg] / ORC_Q }, rhi[3] = { bhi[0], bhi[1], (double)g->reg_c[reg + 1] / ORC_Q };
+      int kx = slab_far(rlo, rhi, xl, dl, tfar, &tf);                /* distance to the face of the region's slab that is met first */
       if (s >= tf) {
         if (tf < 0.0) tf = 0.0;
         for (int k = 0; k < 3; ++k) xl[k] += tf * dl[k];
-        path += tf; c->C->exits++; if (h) hash_ev(h, EV_EXIT, (uint32_t)p); break;
+        path += tf;
+        /* a depth face that is not a face of the panel box: the photon crosses into the next region, analytically, and
+         * draws a fresh free path there */
+        if (kx == 2 && ((dl[2] >= 0.0 && reg + 1 < g->n_regions) || (dl[2] < 0.0 && reg > 0))) {
+          reg += dl[2] >= 0.0 ? 1 : -1; c->C->region_crossings++; if (h) hash_ev(h, EV_REGION, (uint32_t)reg); continue;
+        }
+        c->C->exits++; if (h) hash_ev(h, EV_EXIT, (uint32_t)p); break;
       }
       for (int k = 0; k < 3; ++k) xl[k] += s * dl[k];
       path += s;

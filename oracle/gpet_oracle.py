@@ -64,7 +64,7 @@ class _Hits(C.Structure):
 
 
 _COUNTER_NAMES = ("pairs", "searches", "entries", "steps", "step_vacuum", "virtuals", "pe", "compton", "kn_trials",
-                  "rayleigh", "cutoffs", "exits", "escapes", "hits", "ph_steps", "ph_compton", "ph_absorbed", "ph_cutoff")
+                  "rayleigh", "cutoffs", "exits", "escapes", "hits", "ph_steps", "ph_compton", "ph_absorbed", "ph_cutoff", "region_crossings")
 
 
 class _Counters(C.Structure):

@@ -111,6 +111,19 @@ extern "C" int gpet_geometry_create(const gpet_geometry_desc *d, gpet_geometry *
     if ((long long)s.n_crystals[0] * s.n_crystals[1] > 8192) { delete g; return fail(GPET_E_GEOMETRY, "layer %d: more than 8192 crystals", l); }
   }
   for (int l = d->n_layers; l < kMaxLayers; ++l) G.layer[l].c0 = G.layer[l].c1 = 0x7FFFFFFF;        // never selected by the depth compare
+  // [R19] majorant regions: maximal runs of consecutive layers with the same crystal and gap material; the gap in front of
+  // a region's first layer belongs to the region before it
+  G.n_regions = 0;
+  for (int l = 0; l < kMaxLayers; ++l) { G.reg_lo[l] = INFINITY; G.reg_hi[l] = INFINITY; G.reg_mats[l] = 0; }
+  for (int l = 0; l < d->n_layers; ++l) {
+    if (l == 0 || G.layer[l].cmat != G.layer[l - 1].cmat || G.layer[l].gmat != G.layer[l - 1].gmat) {
+      G.reg_lo[G.n_regions] = l == 0 ? 0.0f : (float)((double)G.layer[l].c0 / 1048576.0);
+      if (G.n_regions) G.reg_hi[G.n_regions - 1] = G.reg_lo[G.n_regions];
+      G.reg_mats[G.n_regions] = (uint32_t)G.layer[l].cmat | (uint32_t)(G.layer[l].gmat >= 0 ? G.layer[l].gmat : G.layer[l].cmat) << 4;
+      ++G.n_regions;
+    }
+  }
+  G.reg_hi[G.n_regions - 1] = (float)((double)c / 1048576.0);
   if (Wq >= (1ll << 30) || Hq >= (1ll << 30) || c >= (1ll << 30)) { delete g; return fail(GPET_E_GEOMETRY, "panel larger than 1024 mm"); }
   G.Wq = (int)Wq; G.Hq = (int)Hq; G.Dq = (int)c; G.hWq = (int)(Wq >> 1); G.hHq = (int)(Hq >> 1);
   G.blo[0] = (float)(-(double)G.hWq / 1048576.0); G.bhi[0] = (float)((double)(Wq - G.hWq) / 1048576.0);

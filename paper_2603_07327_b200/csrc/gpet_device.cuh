@@ -60,6 +60,9 @@ struct DevGeomHead {
   // finds its first panel by the polygon edge it crosses (ring_entry_fast in gpet_transport.cu)
   float ring_phi0, ring_kscale;   // azimuth of panel 0 (rad); n_panels / (2 pi)
   float ring_edge_h;          // half length of a polygon edge minus 1 um (<= 0: shortcut off)
+  // [R19] majorant regions: maximal runs of layers with the same crystal and gap material; region r spans the depths
+  // [reg_lo[r], reg_hi[r]) (reg_lo past n_regions holds +inf); reg_mats = crystal material | gap material << 4
+  int n_regions; float reg_lo[kMaxLayers], reg_hi[kMaxLayers]; uint32_t reg_mats[kMaxLayers];
   DevLayer layer[kMaxLayers];
   float ctr[kMaxPanels][3];   // global position of every box centre (same values as DevPanel::cx, cy, cz)
 };
@@ -161,7 +164,7 @@ __device__ __forceinline__ void rotate(float d[3], float ct, float st, float cp,
 
 // ---------------------------------------------------------------- [R23] outcome hash
 enum : uint32_t { EV_ENTER = 1, EV_STEP_VACUUM, EV_VIRTUAL, EV_PE, EV_COMPTON, EV_RAYLEIGH, EV_CUTOFF, EV_EXIT, EV_ESCAPE,
-                  EV_PH_COMPTON, EV_PH_RAYLEIGH, EV_PH_ABSORBED, EV_PH_CUTOFF, EV_PH_LEAVE, EV_PHOTON_B };
+                  EV_PH_COMPTON, EV_PH_RAYLEIGH, EV_PH_ABSORBED, EV_PH_CUTOFF, EV_PH_LEAVE, EV_REGION };
 __device__ __forceinline__ void hash_ev(uint64_t &h, uint32_t type, uint32_t payload) {
   h = (h ^ (uint64_t)type) * 0x100000001B3ull;
   h = (h ^ (uint64_t)payload) * 0x100000001B3ull;

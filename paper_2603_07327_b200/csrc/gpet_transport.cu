@@ -112,17 +112,34 @@ __device__ __forceinline__ float4 mu_lookup(const float4 *mu, const DevTables &T
   return make_float4(fmaf(f, b.x - a.x, a.x), fmaf(f, b.y - a.y, a.y), fmaf(f, b.z - a.z, a.z), fmaf(f, b.w - a.w, a.w));
 }
 
+// [R19] 1 / majorant of the region the photon is tracked in.  One region (all of BASELINE's configs): the whole-detector
+// majorant tabulated in .w.  Several regions (layers of different materials): the interpolation of the pointwise maximum
+// of mu_tot over the region's crystal and gap material.
+template <bool MULTI>
+__device__ __forceinline__ float inv_majorant(const float4 *mu, const DevTables &T, const DevGeomHead &g, int reg, float E) {
+  if (!MULTI) return rcp_fast(mu_lookup(mu, T, 0, E).w);
+  const float x = (E - T.e_min) * T.inv_step;
+  int i = min(__float2int_rd(x), T.n_energies - 2); i = max(i, 0);
+  const float f = x - (float)i;
+  const uint32_t mats = g.reg_mats[reg];                              // crystal material | gap material << 4 (the same when there is none)
+  const int ra = ((T.matmap >> (4 * (mats & 15u))) & 15u) * T.n_energies + i, rb = ((T.matmap >> (4 * (mats >> 4))) & 15u) * T.n_energies + i;
+  const float lo = fmaxf(mu[ra].z, mu[rb].z), hi = fmaxf(mu[ra + 1].z, mu[rb + 1].z);
+  return rcp_fast(fmaf(f, hi - lo, lo));
+}
+
 // ---------------------------------------------------------------- photon state
 struct Photon {
   float x[3], d[3];        // global frame while searching (fresh photons) / in the phantom, panel frame in STEP / KN / RAY
   float E, path, inv_mu;   // inv_mu = 1 / majorant(E) of the medium the photon is tracked in
   uint32_t pair;           // history - first_history
   uint32_t meta;           // bit0 photon, bits1-4 seq, bits5-10 panel (current, or just left; 63 = none), bit11 in
-                           // phantom, bits12-17 Klein-Nishina trial counter, bits18-31 Philox blocks consumed from
-                           // this photon's stream [R4] (16383 events per photon: never reached, the energy falls)
+                           // phantom, bits12-17 Klein-Nishina trial counter, bits18-19 majorant region [R19], bits20-31
+                           // Philox blocks consumed from this photon's stream [R4] (4095 events per photon: never
+                           // reached, the energy falls)
   uint32_t ids;            // lattice result of the pending interaction (KN / RAY / HIT), panel bits included
 };
 constexpr uint32_t kNoPanel = 63u;
+constexpr int kRegShift = 18, kBlkShift = 20;
 __device__ __forceinline__ int ph_panel(uint32_t meta) { return (meta >> 5) & 63u; }
 __device__ __forceinline__ uint32_t ph_with_panel(uint32_t meta, int panel) { return (meta & ~(63u << 5)) | ((uint32_t)panel << 5); }
 
@@ -310,8 +327,9 @@ __device__ __forceinline__ int panel_search(const DevGeomHead &g, const DevPanel
 // made the ring configs 10 % faster).  PHANTOM: the source is a voxel map with a phantom [R17]; KIND: source kind
 // (0 point, 1 voxel map, -1 = read src.kind); PLANAR: panel search variant (-1 = read g.planar); PRETEST: fresh photons
 // take the acceptance pre-test (misses_detector) before they get a slot -- with KIND = 0 as a stage of its own (GEN1);
-// FAST: repetition-mode ring, photons inside the bore find their first panel by ring_entry_fast.
-template <bool HASH, bool PHANTOM, int KIND, int PLANAR, bool PRETEST, bool FAST>
+// FAST: repetition-mode ring, photons inside the bore find their first panel by ring_entry_fast; MULTI: the layers form
+// several majorant regions [R19] (mixed-material stacks).
+template <bool HASH, bool PHANTOM, int KIND, int PLANAR, bool PRETEST, bool FAST, bool MULTI>
 __global__ void __launch_bounds__(kThreads, 1)
 transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel *panels, DevTables T, DevSource src, uint64_t first_history, uint64_t n_pairs,
                            const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
@@ -382,7 +400,9 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
 #pragma unroll
     for (int k = 0; k < 3; ++k) { q.x[k] = fmaf(bt, dl[k], xl[k]); q.d[k] = dl[k]; }   // [R18]
     q.path += bt; q.meta = ph_with_panel(q.meta, bp);
-    q.inv_mu = rcp_fast(mu_lookup(mu, T, 0, q.E).w);
+    const int reg = (q.x[2] >= g.reg_lo[1] ? 1 : 0) + (q.x[2] >= g.reg_lo[2] ? 1 : 0) + (q.x[2] >= g.reg_lo[3] ? 1 : 0);   // [R19] by the entry depth (unused: +inf)
+    q.meta = (q.meta & ~(3u << kRegShift)) | ((uint32_t)reg << kRegShift);
+    q.inv_mu = inv_majorant<MULTI>(mu, T, g, reg, q.E);
   };
 
 #ifdef GPET_STATS
@@ -613,38 +633,50 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       float4 A = W.a[idx]; const float4 B = W.b[idx]; uint4 C = W.c[idx];
       uint64_t h = 0;
       if (HASH) { const uint2 v = W.hh[idx]; h = ((uint64_t)v.y << 32) | v.x; }
-      const uint4 w = block_at(C.x, C.y, C.y >> 18);                  // [R4] free path, outcome, Rayleigh polar + azimuth
-      C.y += 1u << 18;
+      const uint4 w = block_at(C.x, C.y, C.y >> kBlkShift);                  // [R4] free path, outcome, Rayleigh polar + azimuth
+      C.y += 1u << kBlkShift;
       const float s = -__logf(u01(w.x)) * __uint_as_float(C.w);
       const float te0 = ((B.x >= 0.0f ? g.bhi[0] : g.blo[0]) - A.x) * rcp_dir(B.x);   // distance to the box exit [R32]
       const float te1 = ((B.y >= 0.0f ? g.bhi[1] : g.blo[1]) - A.y) * rcp_dir(B.y);
-      const float te2 = ((B.z >= 0.0f ? g.bhi[2] : g.blo[2]) - A.z) * rcp_dir(B.z);
+      constexpr bool multi = MULTI;                                    // [R19] several majorant regions: the depth slab is the region's
+      int reg = (C.y >> kRegShift) & 3u;
+      const float chi = multi ? g.reg_hi[reg] : g.bhi[2], clo = multi ? g.reg_lo[reg] : g.blo[2];
+      const float te2 = ((B.z >= 0.0f ? chi : clo) - A.z) * rcp_dir(B.z);
       const float tf = fminf(te0, fminf(te1, te2));
       const int panel = ph_panel(C.y);
-      const bool exits = s >= tf;                                      // leaves the panel [R33]
+      const bool leaves = s >= tf;                                     // reaches a face of the (region's) slab first [R33]
       // Exit face = the axis that limits tf.  If no other panel has a point beyond that face (precomputed per panel and
       // face at create time: true for the back and axial faces of any ring), the search of [R6] cannot find anything:
       // the photon escapes here, with the same EXIT, ESCAPE events, and needs no search.
       const int kx = te0 <= tf ? 0 : (te1 <= tf ? 1 : 2);
       const float dk = kx == 0 ? B.x : (kx == 1 ? B.y : B.z);
       const bool open = (pan[panel].open_faces >> (2 * kx + (dk >= 0.0f ? 1 : 0))) & 1u;
-      const float step = exits ? fmaxf(tf, 0.0f) : s;
+      // a depth face that is not a face of the panel box: the photon crosses into the next region and draws afresh there
+      const bool cross = multi && leaves && kx == 2 && (B.z >= 0.0f ? reg + 1 < g.n_regions : reg > 0);
+      const bool exits = leaves && !cross;
+      const float step = leaves ? fmaxf(tf, 0.0f) : s;
       A.x = fmaf(step, B.x, A.x); A.y = fmaf(step, B.y, A.y); A.z = fmaf(step, B.z, A.z); A.w += step;
       uint32_t id;                                                     // depth -> layer -> crystal
       const int mat = lattice_lookup(g, lay, __float2int_rd(A.x * kQ) + g.hWq, __float2int_rd(A.y * kQ) + g.hHq, __float2int_rd(A.z * kQ), id);
       if (id != kNone) id |= (uint32_t)panel << 26;
-      const bool matter = !exits && mat >= 0;
+      const bool matter = !leaves && mat >= 0;
       const float4 m4 = mu_lookup(mu, T, mat < 0 ? 0 : mat, B.w);
-      const float t = u01(w.y) * m4.w;                                 // [R20] one draw picks the outcome
+      const float t = u01(w.y) * (multi ? rcp_fast(__uint_as_float(C.w)) : m4.w);   // [R20] one draw picks the outcome: u x the majorant the step was drawn with
       const bool pe = matter && t < m4.x, kn = matter && !pe && t < m4.y, ray = matter && !pe && !kn && t < m4.z;
       int dest = L_STEP;
       if (ray) dest = L_RAY;                                           // deflected in its own pass
       if (kn) dest = L_KN;
       if (pe) dest = id != kNone ? L_HIT : L_FREE;                     // photoelectric: deposit E, end
       if (exits) dest = open ? L_FREE : L_SEARCH;
+      if (multi && cross) {                                            // (uniform test first: single-region detectors never get here)
+        reg += B.z >= 0.0f ? 1 : -1;
+        C.y = (C.y & ~(3u << kRegShift)) | ((uint32_t)reg << kRegShift);
+        C.w = __float_as_uint(inv_majorant<MULTI>(mu, T, g, reg, B.w));
+      }
       if (!act) dest = L_NONE;
       if (HASH && act) {
-        if (exits) { hash_ev(h, EV_EXIT, (uint32_t)panel); if (open) hash_ev(h, EV_ESCAPE, 0); }
+        if (cross) hash_ev(h, EV_REGION, (uint32_t)reg);
+        else if (exits) { hash_ev(h, EV_EXIT, (uint32_t)panel); if (open) hash_ev(h, EV_ESCAPE, 0); }
         else if (mat < 0) hash_ev(h, EV_STEP_VACUUM, 0);
         else if (pe) hash_ev(h, EV_PE, id);
         else if (kn) { }                                               // hashed when a trial is accepted
@@ -680,8 +712,8 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       const float E = B.w;
       const float k = E * (1.0f / kMec2), e0 = rcp_fast(1.0f + 2.0f * k), e02 = e0 * e0;
       const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
-      const uint4 w = block_at(C.x, C.y, C.y >> 18);                  // [R4] u_a, u_b, u_c, azimuth
-      C.y += 1u << 18;
+      const uint4 w = block_at(C.x, C.y, C.y >> kBlkShift);                  // [R4] u_a, u_b, u_c, azimuth
+      C.y += 1u << kBlkShift;
       const float ua = u01(w.x), ub = u01(w.y), uc = u01(w.z);
       // om = 1 - eps and em = eps - eps0 are formed without cancellation, so that sin^2 = t (2 - t) keeps
       // full relative accuracy at both poles (t = om/(k eps), 2 - t = em/(eps0 k eps)); plain fp32 loses
@@ -726,8 +758,8 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
         C.y &= ~(63u << 12);
         if (hit && ((C.y >> 1) & 15u) < 15u) C.y += 2u;                // [R9] 4-bit saturating hit counter
         B.x = dn[0]; B.y = dn[1]; B.z = dn[2]; B.w = E2;
-        const float4 m4 = mu_lookup(mu, T, in_ph ? src.ph_major : 0, cut ? E : E2);
-        C.w = __float_as_uint(rcp_fast(in_ph ? m4.z : m4.w));
+        const float e_new = cut ? E : E2;
+        C.w = __float_as_uint(in_ph ? rcp_fast(mu_lookup(mu, T, src.ph_major, e_new).z) : inv_majorant<MULTI>(mu, T, g, (C.y >> kRegShift) & 3u, e_new));
         dest = cut ? L_FREE : (in_ph ? L_PHANTOM : L_STEP);
       } else C.y += 1u << 12;
       if (!act) dest = L_NONE;
@@ -786,7 +818,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       cR -= n;
       int dest = L_NONE;
       if (act) {
-        const uint4 w = block_at(p.pair, p.meta, (p.meta >> 18) - 1u);   // the block its Woodcock step drew (rare event: recomputed)
+        const uint4 w = block_at(p.pair, p.meta, (p.meta >> kBlkShift) - 1u);   // the block its Woodcock step drew (rare event: recomputed)
         const float3 r = rayleigh_dir(p.d[0], p.d[1], p.d[2], u01(w.z), u01(w.w));
         p.d[0] = r.x; p.d[1] = r.y; p.d[2] = r.z;
         dest = (PHANTOM && ((p.meta >> 11) & 1u)) ? L_PHANTOM : L_STEP;
@@ -802,7 +834,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       cP -= n;
       int dest = L_NONE;
       if (act) {
-        const uint4 w = block_at(p.pair, p.meta, p.meta >> 18); p.meta += 1u << 18;   // [R4]
+        const uint4 w = block_at(p.pair, p.meta, p.meta >> kBlkShift); p.meta += 1u << kBlkShift;   // [R4]
         const float s = -__logf(u01(w.x)) * p.inv_mu;
         int v[3]; bool out = false; float xt[3];
 #pragma unroll
@@ -906,16 +938,18 @@ cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, cons
   // ring); anything else runs the generic build of the same code
   const bool ring = planar_hint != 0 && host_geom.ring != 0 && host_geom.ring_edge_h > 0.0f;
   const bool point = !phantom && src.kind == 0 && !(src.positron_sigma > 0.0f);   // every pair starts at src.pos
-#define GPET_DISPATCH(H)                                                                                                    \
+#define GPET_DISPATCH(H, M)                                                                                                 \
   do {                                                                                                                      \
-    if (point && ring && pretest) e = launch(transport_wavefront_kernel<H, false, 0, 1, true, true>);                        \
-    else if (point && ring) e = launch(transport_wavefront_kernel<H, false, 0, 1, false, true>);                            \
-    else if (phantom && ring) e = launch(transport_wavefront_kernel<H, true, 1, 1, false, true>);                           \
-    else if (phantom) e = launch(transport_wavefront_kernel<H, true, 1, -1, false, false>);                                 \
-    else if (pretest) e = launch(transport_wavefront_kernel<H, false, -1, -1, true, false>);                                \
-    else e = launch(transport_wavefront_kernel<H, false, -1, -1, false, false>);                                            \
+    if (point && ring && pretest) e = launch(transport_wavefront_kernel<H, false, 0, 1, true, true, M>);                     \
+    else if (point && ring) e = launch(transport_wavefront_kernel<H, false, 0, 1, false, true, M>);                         \
+    else if (phantom && ring) e = launch(transport_wavefront_kernel<H, true, 1, 1, false, true, M>);                        \
+    else if (phantom) e = launch(transport_wavefront_kernel<H, true, 1, -1, false, false, M>);                              \
+    else if (pretest) e = launch(transport_wavefront_kernel<H, false, -1, -1, true, false, M>);                             \
+    else e = launch(transport_wavefront_kernel<H, false, -1, -1, false, false, M>);                                         \
   } while (0)
-  if (hash_out) GPET_DISPATCH(true); else GPET_DISPATCH(false);
+  const bool multi = host_geom.n_regions > 1;
+  if (hash_out) { if (multi) GPET_DISPATCH(true, true); else GPET_DISPATCH(true, false); }
+  else { if (multi) GPET_DISPATCH(false, true); else GPET_DISPATCH(false, false); }
 #undef GPET_DISPATCH
   if (e != cudaSuccess) return e;
   count_launch();

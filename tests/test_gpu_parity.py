@@ -534,8 +534,8 @@ def test_generic_panel_search_parity(tables, pos):
 
 
 def test_mixed_materials_virtual_collisions_and_voxel_source_without_phantom(tables):
-    """Paths the five configs never reach: a front layer of a lighter material under the whole-panel majorant [R19]
-    (virtual collisions in crystals), a reflector made of matter (interactions that deposit outside any crystal record
+    """Paths the five configs never reach: a front layer of a lighter material (its own majorant region [R19]), a reflector
+    made of matter under the crystal's majorant (virtual collisions (interactions that deposit outside any crystal record
     no hit [R20]), and an activity-map source with no phantom (generic kernel variant)."""
     front = W.Layer((15, 15), (1.0, 1.0), (0.1, 0.1), (0.5, 0.5), 6.0, 0.0, crystal_material=1, gap_material=1)
     back = W.Layer((16, 16), (1.0, 1.0), (0.1, 0.1), (0.0, 0.0), 4.0, 0.1, crystal_material=0, gap_material=1)
@@ -547,7 +547,9 @@ def test_mixed_materials_virtual_collisions_and_voxel_source_without_phantom(tab
     res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
     assert res["frac"] >= MIN_MATCH and cnt > 100_000, res
     c = o.counters
-    assert c["virtuals"] > 50_000 and c["ph_steps"] == 0              # the majorant really is above the front layer's mu
+    # two majorant regions [R19]: the water-like front layer is homogeneous (no virtual collisions there), the back layer's
+    # water-like reflector sits under the LYSO majorant (virtual collisions remain)
+    assert c["virtuals"] > 10_000 and c["region_crossings"] > 50_000 and c["ph_steps"] == 0
     layers = (g["ids"] >> 18) & 3
     assert (layers == 0).sum() > 1000 and (layers == 1).sum() > 50_000
 
@@ -718,3 +720,47 @@ def test_positron_range_parity(tables, kind):
         d = np.sqrt((g["x"][first] - 10.0) ** 2 + g["y"][first] ** 2 + (g["z"][first] - 4.0) ** 2) / 299.792458 - g["tof_ns"][first]
         mad = 1.4826 * np.median(np.abs(d - np.median(d))) * 299.792458     # robust: 2 % of the photons are Rayleigh-deflected on the way
         assert 0.1 < mad < 0.4                                         # ~ sigma of the displacement along the line of flight (0.21 mm)
+
+
+# ----------------------------------------------------------------------------- majorant regions, 3-4 layers
+def mixed_ring(n_layers):
+    """12-panel ring with a stack of up to four layers of their own lattices and materials (PAPER.md:35 `the number of
+    layers`; PAPER.md:141 three- and four-layer stacks): LYSO | water-like crystals in a water-like matrix | LYSO | coarse
+    LYSO in a water-like matrix -> up to four majorant regions [R19]."""
+    layers = (W.Layer((15, 15), (1.0, 1.0), (0.1, 0.1), (0.5, 0.5), 3.0, 0.0, 0, -1),
+              W.Layer((16, 16), (1.0, 1.0), (0.1, 0.1), (0.0, 0.0), 2.0, 0.1, 1, 1),
+              W.Layer((16, 16), (1.0, 1.0), (0.1, 0.1), (0.0, 0.0), 2.5, 0.0, 0, -1),
+              W.Layer((8, 8), (2.0, 2.0), (0.2, 0.2), (0.0, 0.0), 2.4, 0.1, 0, 1))
+    return W.Geometry(12, layers[:n_layers], (2, 4), (16.0, 16.0), (16.0, 16.0), ring_inner_radius_mm=55.0)
+
+
+@pytest.mark.parametrize("n_layers", [3, 4])
+def test_three_and_four_layer_stacks_with_majorant_regions(tables, n_layers):
+    """Per-region majorants with analytic region crossing on 3- and 4-layer mixed-material rings: outcome hashes (which
+    include every region crossing) and hits against the oracle; every layer records hits."""
+    r = W.Run(f"mixed{n_layers}", mixed_ring(n_layers), W.source_point((10.0, 0.0, 4.0)), 300_001, 90 + n_layers)
+    g, gh, cnt, o = run_both(r, tables)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= MIN_MATCH and cnt > 100_000, res
+    assert o.counters["region_crossings"] > 100_000
+    assert set(np.unique((g["ids"] >> 18) & 3)) == set(range(n_layers))
+    # the product build (no hashes) writes the same hits
+    gm, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+    hb = api.HitBuffer.allocate(3 * r.n_pairs)
+    api.gpet_simulate(gm, m, s, 0, r.n_pairs, r.seed, hb)
+    torch.cuda.synchronize()
+    plain = PU.canonical(hb.to_numpy())
+    assert all(np.array_equal(plain[k], g[k]) for k in PU.HIT_KEYS)
+
+
+def test_two_region_slab_transmits_like_the_closed_form(tables):
+    """The pin of the oracle's regions (a light layer over a dense one, pencil beam along the depth): the CUDA path gives
+    the same outcome for every history, so exp(-mu1 L1 - mu2 L2) and zero virtual collisions carry over."""
+    from test_oracle_pins import slab, beam, two_material_tables
+    layers = (W.Layer((1, 1), (12.0, 12.0), (0.0, 0.0), (0.0, 0.0), 4.0, 0.0, crystal_material=1),
+              W.Layer((1, 1), (12.0, 12.0), (0.0, 0.0), (0.0, 0.0), 6.0, 0.0, crystal_material=0))
+    for src in (beam(), beam(direction=(-1, 0, 0), pos=(70, 0, 0)), beam(direction=(1, 0.2, 0.1), pos=(0, -8, -4))):
+        r = W.Run("slab2", slab(layers=layers), src, 200_000, 31)
+        g, gh, cnt, o = run_both(r, two_material_tables(0.2, 0.02))
+        assert np.array_equal(gh, o.outcome_hash) and np.array_equal(g["ids"], o.hits.ids) and cnt > 100_000
+        assert o.counters["virtuals"] == 0 and o.counters["region_crossings"] > 50_000

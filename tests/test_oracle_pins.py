@@ -848,3 +848,87 @@ def test_positron_range_is_an_isotropic_gaussian():
     from dataclasses import replace
     a, b = O.decay_sites(rods, 5, 0, 1000), O.annihilation_sites(replace(rods, positron_fwhm_mm=0.102), 5, 0, 1000)
     assert 0.02 < np.abs(a - b).max() < 0.5 and abs(np.std(a - b) / sigma - 1.0) < 0.1
+
+
+# ----------------------------------------------------------------------------- majorant regions, 3-4 layers
+def two_material_tables(mu0, mu1):
+    """Energy-independent photoelectric-only tables for two materials (first interactions = hits)."""
+    f = lambda a, b: np.stack([np.full(W.N_ENERGIES, a, np.float32), np.full(W.N_ENERGIES, b, np.float32)])
+    z = f(0.0, 0.0)
+    return W.Tables(W.E_MIN_KEV, W.E_STEP_KEV, f(mu0, mu1), z, z)
+
+
+def test_majorant_regions_cross_layer_faces_analytically():
+    """[R19] a stack of a light layer (mu 0.02/mm, 4 mm) over a dense one (mu 0.2/mm, 6 mm), homogeneous (no reflector
+    gaps), pencil beam along the depth axis: each layer is its own majorant region, so there is NOT ONE virtual
+    collision, the unscattered fraction is exp(-mu1 L1 - mu2 L2) and the first-interaction depth follows the
+    piecewise-exponential law (KS).  The same stack under one whole-panel majorant would need virtual collisions in
+    the light layer -- the regions remove them without changing the physics."""
+    mu1, mu2, L1, L2, n = 0.02, 0.2, 4.0, 6.0, 400_000
+    layers = (W.Layer((1, 1), (12.0, 12.0), (0.0, 0.0), (0.0, 0.0), L1, 0.0, crystal_material=1),
+              W.Layer((1, 1), (12.0, 12.0), (0.0, 0.0), (0.0, 0.0), L2, 0.0, crystal_material=0))
+    res = O.simulate(slab(layers=layers), two_material_tables(mu2, mu1), beam(), n, seed=31, want_escape=True, threads=4)
+    c = res.counters
+    assert c["virtuals"] == 0 and c["step_vacuum"] == 0 and c["region_crossings"] > 0.8 * n
+    p = math.exp(-mu1 * L1 - mu2 * L2)
+    assert abs(np.mean(res.e_escape[:, 0] == 511.0) - p) < 4 * math.sqrt(p * (1 - p) / n)
+    depth = res.hits.x.astype(np.float64) - 50.0
+    def cdf(d):
+        d = np.asarray(d, np.float64)
+        a = 1.0 - np.exp(-mu1 * np.minimum(d, L1))
+        b = math.exp(-mu1 * L1) * (1.0 - np.exp(-mu2 * np.maximum(d - L1, 0.0)))
+        return (a + b) / (1.0 - p)
+    assert stats.kstest(depth, cdf).pvalue > 1e-3
+    layer = (res.hits.ids >> 18) & 3
+    assert np.all(layer[depth < L1 - 1e-6] == 0) and np.all(layer[depth > L1 + 1e-6] == 1)
+    # a photon entering from the BACK crosses the regions the other way
+    back = O.simulate(slab(layers=layers), two_material_tables(mu2, mu1), beam(direction=(-1, 0, 0), pos=(70, 0, 0)), n, seed=32, want_escape=True, threads=4)
+    assert abs(np.mean(back.e_escape[:, 0] == 511.0) - p) < 4 * math.sqrt(p * (1 - p) / n) and back.counters["virtuals"] == 0
+    assert abs(np.mean(((back.hits.ids >> 18) & 3) == 1) - (1 - math.exp(-mu2 * L2)) / (1 - p)) < 0.005
+    # same materials in consecutive layers: ONE region, exactly the single-layer run (no region events in the hash)
+    same = (W.Layer((1, 1), (12.0, 12.0), (0.0, 0.0), (0.0, 0.0), L1), W.Layer((1, 1), (12.0, 12.0), (0.0, 0.0), (0.0, 0.0), L2))
+    a = O.simulate(slab(layers=same), const_tables(0.05, 0, 0), beam(), 20_000, seed=33, want_hash=True)
+    b = O.simulate(slab(L1 + L2), const_tables(0.05, 0, 0), beam(), 20_000, seed=33, want_hash=True)
+    assert a.counters["region_crossings"] == 0 and np.array_equal(a.hits.x, b.hits.x) and len(a.hits) == len(b.hits) > 7000
+
+
+def four_layer_scanner():
+    """Four stacked layers with their own lattices, offsets, gaps and materials (PAPER.md:35 `the number of layers`,
+    PAPER.md:141 three- and four-layer stacks): three majorant regions (materials 0 | 1, 1 | 0)."""
+    base = tiny_scanner()
+    layers = (W.Layer((3, 2), (1.25, 1.5), (0.25, 0.125), (0.125, 0.25), 1.0, 0.0, 0, -1),
+              W.Layer((2, 2), (1.5, 1.25), (0.0, 0.25), (0.5, 0.0), 1.5, 0.25, 1, -1),
+              W.Layer((4, 3), (1.0, 1.0), (0.125, 0.125), (0.0, 0.25), 1.25, 0.0, 1, -1),
+              W.Layer((2, 1), (2.0, 3.5), (0.5, 0.5), (0.0, 0.0), 2.0, 0.125, 0, 1))
+    return W.Geometry(3, layers, (2, 2), (4.0, 3.5), (4.5, 4.0), panel_pose=base.panel_pose)
+
+
+def test_four_layer_indexing_against_brute_force_enumeration():
+    g = four_layer_scanner()
+    boxes, W_q, H_q, D_q = brute_force_boxes(g)
+    assert len(boxes) == 4 * (6 + 4 + 12 + 2) and D_q == int(6.125 * Q)
+    rng = np.random.default_rng(18)
+    pts = []
+    for p in range(3):
+        loc = rng.uniform([-4.6, -4.1, -0.3], [4.6, 4.1, 6.4], (2500, 3))
+        pose = g.panel_pose[p].astype(np.float64)
+        pts.append(pose[0:3] + loc[:, :1] * pose[3:6] + loc[:, 1:2] * pose[6:9] + loc[:, 2:3] * pose[9:12])
+    grid = np.arange(-4.25, 4.26, 0.125)
+    ga, gb, gc = np.meshgrid(grid, grid[2:-2], np.arange(0.0, 6.13, 0.125), indexing="ij")
+    pts.append(np.stack([20.0 + gc.ravel(), ga.ravel(), gb.ravel()], 1))
+    xyz = np.concatenate(pts).astype(np.float32)
+    got = O.locate(g, xyz)
+    assert np.array_equal(got, brute_locate(g, boxes, W_q, H_q, D_q, xyz))
+    u = O.unpack_ids(got[got != 0xFFFFFFFF])
+    assert set(u["layer"]) == {0, 1, 2, 3} and set(u["crystal"][u["layer"] == 2]) == set(range(12))
+
+
+def test_three_and_four_layer_stacks_transport(tables):
+    """Energy conservation and region bookkeeping on a 3-layer and the 4-layer mixed-material scanner."""
+    for g in (four_layer_scanner(), W.Geometry(3, four_layer_scanner().layers[:3], (2, 2), (4.0, 3.5), (4.5, 4.0), panel_pose=tiny_scanner().panel_pose)):
+        res = O.simulate(g, tables, W.source_point((0.0, 0.0, 0.0)), 400_000, seed=35, want_escape=True, threads=4)
+        assert res.counters["region_crossings"] > 10_000 and len(res.hits) > 1000
+        dep = np.zeros((400_000, 2)); np.add.at(dep, (res.hits.history.astype(np.int64), ((res.hits.ids >> 4) & 1).astype(np.int64)), res.hits.e_keV.astype(np.float64))
+        # deposits in the water-like layers' crystals are hits too; only interactions in a non-crystal material leave no hit
+        assert np.all(dep + res.e_escape <= 511.0 + 1e-3)
+        assert set(np.unique((res.hits.ids >> 18) & 3)) == set(range(len(g.layers)))

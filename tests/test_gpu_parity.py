@@ -764,3 +764,62 @@ def test_two_region_slab_transmits_like_the_closed_form(tables):
         g, gh, cnt, o = run_both(r, two_material_tables(0.2, 0.02))
         assert np.array_equal(gh, o.outcome_hash) and np.array_equal(g["ids"], o.hits.ids) and cnt > 100_000
         assert o.counters["virtuals"] == 0 and o.counters["region_crossings"] > 50_000
+
+
+def many_material_tables(n):
+    """LYSO, water and n - 2 scaled copies of water (denser and denser `tissues`): inputs for the staging tests."""
+    t = W.tables()
+    scale = [1.0, 1.0] + [1.0 + 0.4 * k for k in range(1, n - 1)]
+    pick = [0, 1] + [1] * (n - 2)
+    f = lambda a: np.ascontiguousarray(np.stack([a[p] * np.float32(s) for p, s in zip(pick, scale)]).astype(np.float32))
+    return W.Tables(t.e_min_keV, t.e_step_keV, f(t.mu_pe), f(t.mu_compton), f(t.mu_rayleigh))
+
+
+@pytest.mark.parametrize("n_mat", [3, 6])
+def test_many_materials_fit_in_shared_memory(n_mat):
+    """The mu tables are staged in shared memory next to the photon pools (8 KB per material at 502 energies): with three
+    materials everything still fits, with six (a phantom stages every loaded material) the transport CTA gives up warps
+    until it does -- same results either way (the launch used to fail with a bare CUDA error)."""
+    from dataclasses import replace
+    t = many_material_tables(n_mat)
+    # detector stack using three materials
+    layers = list(mixed_ring(4).layers)
+    layers[2] = replace(layers[2], crystal_material=2)
+    geom = replace(mixed_ring(4), layers=tuple(layers))
+    r = W.Run("mats_det", geom, W.source_point((10.0, 0.0, 4.0)), 100_000, 97)
+    g, gh, cnt, o = run_both(r, t)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= MIN_MATCH and cnt > 30_000, res
+    # phantom holding every loaded material but LYSO (concentric shells), on C3's ring
+    c4 = W.config_runs("C4", 100_000)[0]
+    ph = c4.source.phantom_material.copy()
+    zz, yy, xx = np.meshgrid(*[np.arange(128)] * 3, indexing="ij")
+    rr = np.sqrt((xx - 63.5) ** 2 + (yy - 63.5) ** 2) * 0.25
+    for k in range(2, n_mat):
+        ph[(ph > 0) & (rr < 15.0 * (n_mat - k) / (n_mat - 1))] = k + 1
+    src = replace(c4.source, phantom_material=ph, phantom_majorant_material=n_mat - 1)
+    r = replace(c4, source=src)
+    g, gh, cnt, o = run_both(r, t)
+    res = PU.compare_hits(g, PU.oracle_hits_dict(o.hits), gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= MIN_MATCH and cnt > 30_000 and o.counters["ph_compton"] > 10_000, res
+    assert len(np.unique(ph)) == n_mat
+
+
+def test_bad_inputs_are_rejected_with_a_message(tables):
+    """skewed poses, zero totals and phantom voxels pointing at materials that are not loaded."""
+    geom = W.geometry_c0()
+    pose = geom.panel_pose.copy(); pose[0, 3:6] = (0.0, 0.9, 0.1)        # u no longer a unit vector orthogonal to w
+    from dataclasses import replace
+    with pytest.raises(api.GpetError, match="orthonormal"):
+        api.gpet_geometry_create(replace(geom, panel_pose=pose))
+    r = W.config_runs("C1", 1000)[0]
+    g, m, s = api.gpet_geometry_create(r.geometry), api.gpet_materials_load(tables), api.DeviceSource(r.source)
+    hb = api.HitBuffer.allocate(4096)
+    api.gpet_simulate(g, m, s, 0, 1000, r.seed, hb)
+    scratch = torch.empty(api.gpet_digitize_scratch_bytes(1000, 4096), dtype=torch.uint8, device="cuda")
+    with pytest.raises(api.GpetError, match="n_pairs_total"):
+        api.gpet_digitize(s, r.seed, 0, 0, 1000, hb, 4096, r.digitizer, scratch, None, api.CoincBuffer.allocate(1024))
+    c4 = W.config_runs("C4", 1000)[0]
+    bad = c4.source.phantom_material.copy(); bad[64, 64, 64] = 9
+    with pytest.raises(api.GpetError, match="material"):
+        api.Pipeline(api.gpet_geometry_create(c4.geometry), m, replace(c4.source, phantom_material=bad), c4.digitizer, 1000, 1000)

@@ -34,7 +34,10 @@ UNIT = "pairs/s"
 SM_COUNT, LANES_PER_SM = 148, 128
 # Algorithmic thread-instructions per pair of the transport kernel on C1 (event
 # counts of the oracle x audited minimum instruction cost per event).
-ALG_INSTR_PER_PAIR = {"C1": 740.0}
+# C1: SURVEY.md 8(d)'s 740; the others: tests/golden/alg_instr_per_pair.json (written by tests/golden/alg_instr.py from the
+# oracle's event counts x the same per-event costs; that audit gives 697 for C1).
+ALG_INSTR_PER_PAIR = {"C1": 740.0, "C2": 698.8, "C3": 699.4, "C4": 1104.1, "P1": 999.0, "P2": 999.0, "P3": 999.0,
+                      "T1": 1457.4, "T2": 1456.9, "T3": 1460.6}
 # Algorithmic HBM bytes per pair of the digitizer on C1.
 ALG_DIGI_BYTES_PER_PAIR = {"C1": 170.0}
 
@@ -87,9 +90,26 @@ class ClockSampler(threading.Thread):
 
 def workload(config: str, pairs):
     from paper_2603_07327_b200 import workloads as W
+    from dataclasses import replace
+    if config == "C4" and pairs is None:
+        pairs = 62_500_000                                          # one of the 16 time slices of the 1e9-pair run per step
     run = W.config_runs(config, pairs)[0]
-    desc = {"C1": "C1: 12-panel ring R=55mm, 2x4 modules of 16x16 LYSO (1.0 mm pitch), single 10 mm layer, centred point source, "
-                  "0.5deg acolinearity, 350-650 keV, 15% blur, 4 ns window"}.get(config, config)
+    if run.source.half_life_s > 0.0:
+        # the bench strings batches together into one long acquisition: constant activity instead of the decay law (12 s of
+        # 18F change the activity by 0.1 %), so that every batch is the same 12 s of the paper's Table 1
+        run = replace(run, source=replace(run.source, half_life_s=0.0, duration_s=0.0))
+    ring = "12-panel ring R=55mm, 2x4 modules of 16x16 LYSO (1.0 mm pitch)"
+    tail = "0.5deg acolinearity, 350-650 keV, 15% blur, 4 ns window"
+    paper = "the paper's scanner (PAPER.md:47: 10 panels, R=85mm, six 51x51 modules, 1.0 mm pitch)"
+    desc = {"C1": f"C1: {ring}, single 10 mm layer, centred point source, {tail}",
+            "C2": f"C2: {ring}, two aligned 5 mm layers with a 0.1 mm gap, centred point source, {tail}",
+            "C3": f"C3: {ring}, 6 mm front layer offset by half a pitch over a 4 mm back layer, centred point source, {tail}",
+            "C4": f"C4: C3's ring, 128^3 x 0.25 mm hot-rod water phantom, pairs from the activity map, one time slice of {run.n_pairs} pairs per step, {tail}",
+            "P1": f"P1: {paper}, H2RSPET-1CL, centred point source", "P2": f"P2: {paper}, 1CL-split, centred point source",
+            "P3": f"P3: {paper}, 2CL, centred point source",
+            "T1": f"T1: {paper}, H2RSPET-1CL, Derenzo source in a 40.25 mm water box, 12 s of decay per step (Table 1, PAPER.md:131-137)",
+            "T2": f"T2: {paper}, 1CL-split, Derenzo source, 12 s per step (Table 1)",
+            "T3": f"T3: {paper}, 2CL, Derenzo source, 12 s per step (Table 1)"}.get(config, config)
     return run, desc
 
 
@@ -404,7 +424,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C1")
     ap.add_argument("--pairs", type=int, default=None, help="pairs per step per GPU (default: the config's own, 1e7 for C1)")
-    ap.add_argument("--hits-per-pair", type=float, default=1.2)
+    ap.add_argument("--hits-per-pair", type=float, default=None, help="hit buffer size per pair (default: 1.2 for C1-C4, 2.0 for P1-P3, 3.0 for T1-T3)")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--cpu-pairs", type=int, default=10_000_000)
     ap.add_argument("--ref-pairs", type=int, default=2_000_000)
@@ -414,6 +434,8 @@ def main():
     ap.add_argument("--transport-warps", type=int, default=0, help="warps per transport CTA (default 20; fewer leave more of each SM to the other stream in the pipeline)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.hits_per_pair is None:
+        args.hits_per_pair = {"P": 2.0, "T": 3.0}.get(args.config[0].upper(), 1.2)
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -332,7 +332,7 @@ __device__ __forceinline__ int panel_search(const DevGeomHead &g, const DevPanel
 template <bool HASH, bool PHANTOM, int KIND, int PLANAR, bool PRETEST, bool FAST, bool MULTI>
 __global__ void __launch_bounds__(kThreads, 1)
 transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel *panels, DevTables T, DevSource src, uint64_t first_history, uint64_t n_pairs,
-                           const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter) {
+                           const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter, uint32_t grab_pairs) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n_mu = T.n_staged * T.n_energies;
   float4 *mu_s = reinterpret_cast<float4 *>(smem_raw + SmemLayout<HASH>::mu_off(blockDim.x >> 5));
@@ -382,13 +382,13 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
     cnt += __popc(m);
   };
   auto end_hash = [&](uint32_t pair, uint32_t meta, uint64_t h) { hash_out[2ull * pair + (meta & 1u)] = h; };
-  auto grab = [&]() {                      // reserve the next pairs of the batch (one atomic per kGrab pairs)
+  auto grab = [&]() {                      // reserve the next pairs of the batch (one atomic per grab)
     if (w_next >= w_end && !exhausted) {
       unsigned long long b = 0;
-      if (lane == 0) b = atomicAdd(work_counter, (unsigned long long)kGrab);
+      if (lane == 0) b = atomicAdd(work_counter, (unsigned long long)grab_pairs);
       b = __shfl_sync(FULL, b, 0);
       if (b >= n_pairs) { exhausted = true; w_next = w_end = 0; }
-      else { w_next = (uint32_t)b; w_end = (uint32_t)min((uint64_t)(b + kGrab), n_pairs); }
+      else { w_next = (uint32_t)b; w_end = (uint32_t)min((uint64_t)(b + grab_pairs), n_pairs); }
     }
   };
   // fresh photon -> entry point of its first panel (fused search) or the SEARCH / PHANTOM list
@@ -913,6 +913,10 @@ cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, cons
   PhiloxKeys key;                                                     // [R1] round keys: key + r * Weyl constants
   for (int r = 0; r < 10; ++r) { key.k[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; key.k[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }
   const int blocks = (int)(want < resident ? (want ? want : 1) : resident);
+  // pairs a warp reserves at a time: kGrab for long runs, less when every warp gets only a few grabs (short tails: a warp
+  // that draws the last grab works alone for one grab's time), never less than one GEN1 pass
+  uint32_t grab_pairs = (uint32_t)(n_pairs / ((uint64_t)blocks * warps * 8));
+  grab_pairs = grab_pairs >= kGrab ? kGrab : (grab_pairs < 32u ? 32u : grab_pairs & ~31u);
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(unsigned long long), stream);
   if (e != cudaSuccess) return e;
   const bool phantom = src.kind == 1 && src.phantom != nullptr;
@@ -931,7 +935,7 @@ cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, cons
   auto launch = [&](auto kernel) -> cudaError_t {
     cudaError_t le = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (le != cudaSuccess) return le;
-    kernel<<<blocks, threads, smem, stream>>>(head, panels, T, src, first_history, n_pairs, key, H, hash_out, work_counter);
+    kernel<<<blocks, threads, smem, stream>>>(head, panels, T, src, first_history, n_pairs, key, H, hash_out, work_counter, grab_pairs);
     return cudaSuccess;
   };
   // specialised builds for the shapes the five configs use (point source or voxel map + phantom, in a repetition-mode

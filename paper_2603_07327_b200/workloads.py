@@ -247,6 +247,62 @@ def hot_rod_phantom(n: int = 128, voxel_mm: float = 0.25):
     return activity, material, (origin, origin, origin)
 
 
+# ----------------------------------------------------------------------------- the paper's Derenzo phantom
+DERENZO_DIAMETERS_MM = (0.3, 0.4, 0.5, 0.625, 0.75, 1.0)
+DERENZO_ROD_COUNTS = (6, 10, 15, 21, 28, 36)           # triangular numbers: 3 .. 8 rows
+DERENZO_ACTIVITY_BQ_PER_MM3 = 92.1                     # 9.21e-5 MBq/mm3
+DERENZO_BOX_MM = 40.25
+
+
+def derenzo_rod_centres(apex_radius_mm: float = 2.5) -> List[Tuple[float, float, float]]:
+    """(x, y, diameter) of the 116 rods: six triangular sectors forming a hexagon, sector s on the bisector at 60 s + 30
+    degrees, rods of one diameter d per sector on a triangular lattice with centre spacing 2 d, apex towards
+    the axis.  The paper gives diameters, counts and spacing; the apex radius (2.5 mm) is this build's choice."""
+    rods = []
+    for s, (d, n) in enumerate(zip(DERENZO_DIAMETERS_MM, DERENZO_ROD_COUNTS)):
+        rows = int(round((math.sqrt(8 * n + 1) - 1) / 2))
+        assert rows * (rows + 1) // 2 == n
+        th = math.radians(60.0 * s + 30.0)
+        ex, ey = math.cos(th), math.sin(th)
+        px, py = -ey, ex
+        for j in range(rows):
+            r = apex_radius_mm + j * math.sqrt(3.0) * d
+            rods += [(r * ex + (2.0 * i - j) * d * px, r * ey + (2.0 * i - j) * d * py, d) for i in range(j + 1)]
+    return rods
+
+
+def derenzo_phantom(voxel_mm: float = 0.125, z_voxel_mm: float = 0.25):
+    """Water box of 40.25 mm on a grid of 0.125 x 0.125 x 0.25 mm voxels (322 x 322 x 161: the transaxial
+    pitch resolves the 0.3 mm rods, the axial one is the paper's reconstruction pitch); activity 1.0 in voxels whose centre
+    lies in a rod and |z| < 10 mm (2 cm rods).  Returns (activity f32 [nz,ny,nx], material u8, origin, dims, voxel sizes)."""
+    n = int(round(DERENZO_BOX_MM / voxel_mm)); nz = int(round(DERENZO_BOX_MM / z_voxel_mm))
+    o = -0.5 * DERENZO_BOX_MM
+    c = o + (np.arange(n) + 0.5) * voxel_mm
+    cz = o + (np.arange(nz) + 0.5) * z_voxel_mm
+    x, y = np.meshgrid(c, c, indexing="xy")
+    rod2d = np.zeros((n, n), bool)
+    for rx, ry, d in derenzo_rod_centres():
+        rod2d |= ((x - rx) ** 2 + (y - ry) ** 2) < (0.5 * d) ** 2
+    activity = np.zeros((nz, n, n), np.float32)
+    activity[np.abs(cz) < 10.0] = rod2d.astype(np.float32)
+    material = np.full((nz, n, n), 2, np.uint8)                        # water (material index 1) everywhere in the box
+    return activity, material, (o, o, o), (n, n, nz), (voxel_mm, voxel_mm, z_voxel_mm)
+
+
+def derenzo_activity_bq() -> float:
+    """Total activity of the rods: sum n_i pi d_i^2 / 4 x 20 mm x 9.21e-5 MBq/mm3 = 95.26 kBq."""
+    vol = sum(n * math.pi * d * d / 4.0 * 20.0 for d, n in zip(DERENZO_DIAMETERS_MM, DERENZO_ROD_COUNTS))
+    return vol * DERENZO_ACTIVITY_BQ_PER_MM3
+
+
+def source_derenzo(duration_s: float = 12.0) -> Source:
+    """The Derenzo source of the paper's Table 1 (12 s of 18F decay): voxel activity map inside the water
+    box, decay law on [R34], positron range off, 0.5 deg acolinearity as in BASELINE's ring configs."""
+    act, mat, org, dims, vox = derenzo_phantom()
+    return Source(1, (0.0, 0.0, 0.0), 0.5, derenzo_activity_bq(), 0, act, mat, 1, dims, vox, org,
+                  half_life_s=F18_HALF_LIFE_S, duration_s=duration_s)
+
+
 def source_point(pos=(0.0, 0.0, 0.0), acolinearity_fwhm_deg=0.5, activity_bq=1.0e6) -> Source:
     return Source(0, tuple(float(v) for v in pos), acolinearity_fwhm_deg, activity_bq)
 
@@ -290,6 +346,12 @@ def config_runs(name: str, n_pairs: Optional[int] = None) -> List[Run]:
         geom = {"P1": geometry_paper_1cl, "P2": geometry_paper_split, "P3": geometry_paper_2cl}[name]()
         dig = Digitizer(0.16, 511.0, 350.0, 700.0, 3.0, 1)
         return [Run(name, geom, source_point(), n_pairs or 10_000_000, 60 + int(name[1]), dig)]
+    if name in ("T1", "T2", "T3"):      # the paper's Table 1: Derenzo source, 12 s of decay, on its three scanners
+        geom = {"T1": geometry_paper_1cl, "T2": geometry_paper_split, "T3": geometry_paper_2cl}[name]()
+        src = source_derenzo()
+        lam = math.log(2.0) / src.half_life_s
+        n = n_pairs or int(round(src.activity_bq / lam * -math.expm1(-lam * src.duration_s)))
+        return [Run(name, geom, src, n, 70 + int(name[1]), Digitizer(0.16, 511.0, 350.0, 700.0, 3.0, 1))]
     raise ValueError(f"unknown config {name!r}")
 
 

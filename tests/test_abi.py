@@ -176,3 +176,16 @@ def test_bore_radius_of_planar_detectors():
             assert np.hypot(pts[:, 0], pts[:, 1]).min() >= r
     from test_oracle_pins import tiny_scanner
     assert api.gpet_geometry_bore_radius(api.gpet_geometry_create(tiny_scanner())) <= 0.0     # panels off the z = 0 plane: not planar
+
+
+def test_bench_roofline_table_matches_the_audit():
+    """bench.py's algorithmic instruction counts are the audited ones (tests/golden/alg_instr_per_pair.json, written by
+    tests/golden/alg_instr.py from the oracle's event counts); C1 alone keeps SURVEY 8(d)'s 740."""
+    import importlib.util, json
+    spec = importlib.util.spec_from_file_location("bench", os.path.join(ROOT, "bench.py"))
+    bench = importlib.util.module_from_spec(spec); spec.loader.exec_module(bench)
+    audit = json.load(open(os.path.join(ROOT, "tests", "golden", "alg_instr_per_pair.json")))
+    name = {"C2": "C2_x0", "C3": "C3_x0_z0", "C4": "C4", "P1": "P1", "T1": "T1", "T2": "T2", "T3": "T3"}
+    for k, v in name.items():
+        assert abs(bench.ALG_INSTR_PER_PAIR[k] - audit[v]["instr_per_pair"]) < 0.05, k
+    assert bench.ALG_INSTR_PER_PAIR["C1"] == 740.0 and abs(audit["C1"]["instr_per_pair"] - 700.0) < 10.0

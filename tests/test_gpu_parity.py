@@ -239,7 +239,7 @@ def test_run_host_matches_device_path(tables):
 
 
 # ----------------------------------------------------------------------------- full size, bench launch configuration
-def gpu_product_run(run, tables, hits_per_pair, n=None):
+def gpu_product_run(run, tables, hits_per_pair, n=None, reps=2):
     """The PRODUCT build (no outcome hashes, 128 slots per warp, chunked hit layout -- what bench.py times): transport +
     digitizer of one batch.  Returns (hits, singles, coincidences) as numpy dicts and the device time of the two calls."""
     n = n or run.n_pairs
@@ -250,7 +250,7 @@ def gpu_product_run(run, tables, hits_per_pair, n=None):
     scratch = torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda")
     st = torch.cuda.current_stream()
     best = float("inf")
-    for rep in range(2):                                              # the second pass is the timed one
+    for rep in range(reps):                                           # best of the passes after the first
         hb.reset()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(st)
@@ -258,19 +258,20 @@ def gpu_product_run(run, tables, hits_per_pair, n=None):
         api.gpet_digitize(s, run.seed, n, 0, n, hb, cap, run.digitizer, scratch, sg, co, st)
         b.record(st)
         torch.cuda.synchronize()
-        best = min(best, a.elapsed_time(b))
+        if rep:
+            best = min(best, a.elapsed_time(b))
     assert hb.dropped() == 0, "hit buffer overflow in test"
     assert int(co.n_coinc.item()) <= co.capacity
     return hb.to_numpy(), sg.to_numpy(), co.to_numpy(), best
 
 
-def whole_run_against_oracle(run, tables, hits_per_pair):
+def whole_run_against_oracle(run, tables, hits_per_pair, min_coinc=100_000, reps=2):
     """One config position at its FULL size through the product build, next to the oracle's whole run: hits of every
     history, then singles and coincidences (each side digitizes its own hits).  Budgets: north_star's 1e-4 of the
     histories may differ in their discrete outcome (fp32 vs fp64 decisions); the records of those histories may differ or
     be missing on one side, so the joins allow 1e-4 of each list (+ 2 for window-edge flips of the blur)."""
     n = run.n_pairs
-    g, gs, gc, ms = gpu_product_run(run, tables, hits_per_pair)
+    g, gs, gc, ms = gpu_product_run(run, tables, hits_per_pair, reps=reps)
     o = O.simulate(run.geometry, tables, run.source, n, run.seed, threads=16)
     res = PU.compare_hits_unhashed(g, PU.oracle_hits_dict(o.hits), n, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
     assert res["frac"] >= MIN_MATCH and res["n_hits_compared"] >= (1.0 - 5e-4) * len(o.hits), res
@@ -279,7 +280,7 @@ def whole_run_against_oracle(run, tables, hits_per_pair):
     bs, bc = int(1e-4 * len(osg.ids)) + 2, int(1e-4 * len(oco.ids_a)) + 2
     ns = PU.compare_singles(gs, osg, 20, exact=False, max_symdiff=bs, max_bad=bs)
     nc = PU.compare_coincidences(gc, oco, exact=False, max_symdiff=bc, max_bad=bc)
-    assert ns >= len(osg.ids) - bs and nc >= len(oco.ids_a) - bc and nc > 100_000
+    assert ns >= len(osg.ids) - bs and nc >= len(oco.ids_a) - bc and nc > min_coinc
     assert np.all(np.diff(gs["t_s"]) >= 0) and np.all(np.diff(gc["t_s"]) >= 0)
     res.update(n_hits=len(g["ids"]), n_singles_compared=ns, n_coinc_compared=nc, ms=ms, pairs_per_s=n / (ms * 1e-3))
     return g, o, res
@@ -823,3 +824,41 @@ def test_bad_inputs_are_rejected_with_a_message(tables):
     bad = c4.source.phantom_material.copy(); bad[64, 64, 64] = 9
     with pytest.raises(api.GpetError, match="material"):
         api.Pipeline(api.gpet_geometry_create(c4.geometry), m, replace(c4.source, phantom_material=bad), c4.digitizer, 1000, 1000)
+
+
+# ----------------------------------------------------------------------------- the paper's Table 1 workload
+TABLE1 = {}
+
+
+@pytest.mark.parametrize("cfg", ["T1", "T2", "T3"])
+def test_table1_derenzo_runs_against_the_oracle(tables, cfg):
+    """the Derenzo source (116 rods of 0.3-1.0 mm in a 40.25 mm water box, 9.21e-5 MBq/mm3, 12 s of 18F
+    decay = 1 142 344 decays) on H2RSPET-1CL / -1CL-split / -2CL, whole run through the product build with the decay law
+    on [R34]: hits, singles and coincidences against the oracle."""
+    r = W.config_runs(cfg)[0]
+    assert r.n_pairs == 1_142_344 == api.gpet_decay_count(r.source.activity_bq, r.source.half_life_s, r.source.duration_s)
+    g, o, res = whole_run_against_oracle(r, tables, 3.0, min_coinc=50_000, reps=8)   # a 12 s acquisition is a 0.6 ms run: best of 7
+    TABLE1[cfg] = dict(hits=res["n_hits"], coinc=res["n_coinc_compared"], ms=res["ms"], g=g)
+    print(f"{cfg}: hits/decay {res['n_hits'] / r.n_pairs:.3f} (paper 2.34), coincidences/hit {res['n_coinc_compared'] / res['n_hits']:.4f} "
+          f"(paper 0.1415), {res['ms']:.3f} ms per 12 s acquisition (paper: 41 s on a TITAN Xp, I/O included)")
+    assert gsafe(res["n_hits"] / r.n_pairs, 1.2, 1.7)
+
+
+def gsafe(v, lo, hi):
+    return lo < v < hi
+
+
+def test_table1_layer_configurations_cost_the_same(tables):
+    """PAPER.md:121 (Table 1): `no measurable increase in simulation time` from 1CL to split to 2CL, here on the Derenzo
+    workload with ONE seed for the three scanners (a 12 s acquisition is a 0.6 ms run: different seeds alone move it by a
+    few percent); and the split scanner records the single-layer scanner's hits."""
+    from dataclasses import replace
+    ms, hits = [], []
+    for cfg in ("T1", "T2", "T3"):
+        r = replace(W.config_runs(cfg)[0], seed=70)
+        g, _, _, t = gpu_product_run(r, tables, 3.0, reps=8)
+        ms.append(t); hits.append(PU.canonical(g))
+    assert max(ms) / min(ms) < 1.10, ms
+    strip = ~np.uint32(3 << 18)
+    assert np.array_equal(hits[0]["ids"] & strip, hits[1]["ids"] & strip) and np.array_equal(hits[0]["x"], hits[1]["x"])
+    assert 0.96 < len(hits[2]["ids"]) / len(hits[0]["ids"]) < 1.0        # paper: 2 620 170 / 2 671 908 = 0.981

@@ -38,8 +38,16 @@ SM_COUNT, LANES_PER_SM = 148, 128
 # oracle's event counts x the same per-event costs; that audit gives 697 for C1).
 ALG_INSTR_PER_PAIR = {"C1": 740.0, "C2": 698.8, "C3": 699.4, "C4": 1104.1, "P1": 999.0, "P2": 999.0, "P3": 999.0,
                       "T1": 1457.4, "T2": 1456.9, "T3": 1460.6}
-# Algorithmic HBM bytes per pair of the digitizer on C1.
-ALG_DIGI_BYTES_PER_PAIR = {"C1": 170.0}
+
+
+def digitizer_alg_bytes(n_hits, n_singles, n_coinc, n_buckets):
+    """Algorithmic HBM bytes of one gpet_digitize call on the CHUNKED hit layout -- the path this bench times (DESIGN.md
+    section 6): every hit's history, ids, energy and time are read once (16 B) and the position of each kept single's
+    representative hit (12 B); a kept single is appended with its bucket rank (36 B), moved to its time bucket (36 B read,
+    32 B written), ranked inside the bucket into time order (32 + 32 B), read by the window pass (32 B, 4 B flag), scanned
+    (8 B) and read again by the writer (8 B); a coincidence reads two singles and writes one 36-byte list-mode record; the
+    time buckets are zeroed, counted and scanned (12 B each)."""
+    return 16 * n_hits + (12 + 36 + 68 + 64 + 36 + 8 + 8) * n_singles + 100 * n_coinc + 12 * n_buckets
 
 
 def load_peaks():
@@ -193,6 +201,7 @@ def run_ours(args):
     hits = [api.HitBuffer.allocate_chunked(n, args.hits_per_pair) for _ in range(nbuf)]
     cap = hits[0].capacity
     coinc = [api.CoincBuffer.allocate(cap // 4) for _ in range(nbuf)]
+    singles_count = api.SinglesBuffer.allocate(0)                 # NULL arrays, valid counter: the digitizer reports how many singles it kept
     scratch = [torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda") for _ in range(nbuf)]
     s_a = torch.cuda.Stream()
     s_b = torch.cuda.Stream() if args.overlap else s_a
@@ -223,7 +232,7 @@ def run_ours(args):
                 s_b.wait_event(sim_done[i])
             if record:
                 e[2].record(s_b)
-            api.gpet_digitize(src, run.seed, n_total, first, n, hits[i], cap, run.digitizer, scratch[i], None, coinc[i], s_b)
+            api.gpet_digitize(src, run.seed, n_total, first, n, hits[i], cap, run.digitizer, scratch[i], singles_count, coinc[i], s_b)
             if record:
                 e[3].record(s_b)
                 evs.append(e)
@@ -259,7 +268,7 @@ def run_ours(args):
     clocks = sampler.finish(w0, w1) if rank == 0 else None
     transport_ms = sum(e[0].elapsed_time(e[1]) for e in t_events) / len(t_events)
     digitize_ms = sum(e[2].elapsed_time(e[3]) for e in t_events) / len(t_events)
-    n_hits, n_coinc = hits[0].count(), int(coinc[0].n_coinc.item())
+    n_hits, n_coinc, n_singles = hits[0].count(), int(coinc[0].n_coinc.item()), int(singles_count.n_singles.item())
     for hb, cb in zip(hits, coinc):
         if hb.dropped():
             raise SystemExit(f"hit buffer overflow ({hb.dropped()} hits dropped); raise --hits-per-pair")
@@ -359,7 +368,7 @@ def run_ours(args):
     achieved = alg * n / (transport_ms * 1e-3) if alg else None
     traffic = None
     tp = os.path.join(ROOT, "profiles", "transport_traffic.txt")
-    if os.path.exists(tp):
+    if os.path.exists(tp) and args.config == "C1":
         try:
             traffic = json.load(open(tp)).get("dram_bytes_per_launch")
         except Exception:
@@ -376,15 +385,24 @@ def run_ours(args):
                 "overlap": bool(args.overlap),
                 "hit_bytes_gbs": n_hits * 28 / (transport_ms * 1e-3) / 1e9}
     digi_ms = digitize_ms
-    dbytes = ALG_DIGI_BYTES_PER_PAIR.get(args.config)
     roofline_digi = None
-    if dbytes and peaks["hbm_gbs"]:
-        dach = dbytes * n / (digi_ms * 1e-3) / 1e9
-        roofline_digi = {"kernel": "digitizer (gpet_digitize, 10 launches)", "bound": "hbm", "achieved": dach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                         "frac": dach / peaks["hbm_gbs"], "traffic": None,
-                         "alone": ({"digitize_ms": alone["digitize_ms"], "achieved": dbytes * n / (alone["digitize_ms"] * 1e-3) / 1e9,
-                                    "frac": dbytes * n / (alone["digitize_ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"]} if alone else None),
-                         "note": f"{dbytes} algorithmic B/pair (DESIGN.md 6) x {n} pairs / {digi_ms:.3f} ms; peak = hbm_gbs of {peaks['source']}"}
+    if peaks["hbm_gbs"]:
+        dbytes = digitizer_alg_bytes(n_hits, n_singles, n_coinc, (cap + 1) // 2)
+        dach = dbytes / (digi_ms * 1e-3) / 1e9
+        dtraffic = None
+        dp = os.path.join(ROOT, "profiles", "digitizer_traffic.txt")
+        if os.path.exists(dp) and args.config == "C1":
+            try:
+                dtraffic = json.load(open(dp)).get("dram_bytes_per_call")
+            except Exception:
+                dtraffic = None
+        roofline_digi = {"kernel": "digitizer (gpet_digitize on the chunked hit layout: 7 kernels)", "bound": "hbm", "achieved": dach, "peak": peaks["hbm_gbs"],
+                         "unit": "GB/s", "frac": dach / peaks["hbm_gbs"], "traffic": dtraffic,
+                         "alone": ({"digitize_ms": alone["digitize_ms"], "achieved": dbytes / (alone["digitize_ms"] * 1e-3) / 1e9,
+                                    "frac": dbytes / (alone["digitize_ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"]} if alone else None),
+                         "note": f"{dbytes / n:.1f} algorithmic B/pair of the chunked path (DESIGN.md 6: {n_hits} hits, {n_singles} kept singles, {n_coinc} "
+                                 f"coincidences) / {digi_ms:.3f} ms; peak = hbm_gbs of {peaks['source']}.  Per kernel (profiles/README.md): chunk_adder is bound by "
+                                 "instruction issue, the bucket sort and the coincidence passes by the latency of 32-byte scattered accesses, none by bandwidth"}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -406,7 +424,9 @@ def run_ours(args):
                    "pipeline": (f"two batches in flight: gpet_simulate(k+1) on one stream beside gpet_digitize(k) on another, transport CTA of {warps} warps"
                                 if args.overlap else "serial: simulate then digitize on one stream"),
                    "l2": f"inputs larger than L2: the hit buffer ({n_hits * 28 / 1e6:.0f} MB/step) and digitizer scratch exceed the 126 MB L2",
-                   "hits_per_step": n_hits, "coincidences_per_step": n_coinc},
+                   "hits_per_step": n_hits, "singles_per_step": n_singles, "coincidences_per_step": n_coinc,
+                   "outputs": "timed steps leave list-mode coincidences (and the singles count) in device memory; the caller-visible singles "
+                              "arrays are not requested; e2e copies every step's coincidence list to the host"},
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": args.e2e_steps,
                 "api": "gpet_pipeline_submit / gpet_pipeline_collect (host outputs per step: coincidence list-mode + counters; two batches in flight)"},

@@ -102,8 +102,9 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, const PhiloxKeys &K) {
   }
   return c;
 }
-// [R2] u = ((x >> 9) + 0.5) * 2^-23: every step is exact in fp32
-__device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 9) + 0.5f) * 1.1920928955078125e-7f; }
+// [R2] u = ((x >> 9) + 0.5) * 2^-23, formed without an integer-to-float conversion: k = x >> 9 placed in the mantissa of
+// 1.0 gives 1 + k 2^-23; subtracting 1 - 2^-24 leaves (2k + 1) 2^-24, which has 24 significant bits: every step is exact
+__device__ __forceinline__ float u01(uint32_t x) { return __uint_as_float((x >> 9) | 0x3F800000u) - 0.99999994f; }
 
 // ---------------------------------------------------------------- [R7] lattice lookup
 // (qa, qb, qc) measured from the panel's low corner.  Returns the material (-1 vacuum) and the packed ids without

@@ -22,6 +22,7 @@ struct DevSource {
   const uint8_t *phantom; int ph_major; int dims[3]; float voxel[3], inv_voxel[3], origin[3];
   double activity_bq; uint64_t pairs_per_slice;
   float positron_sigma;                                          // [R35] mm per axis, 0 = off
+  uint32_t pre_klo, pre_khi;                                     // point-source pre-test: pairs whose polar word >> 9 lies outside [pre_klo, pre_khi] miss with both photons (set per launch)
 };
 
 struct DigiParams {

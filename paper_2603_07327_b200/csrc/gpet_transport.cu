@@ -211,14 +211,22 @@ __device__ __forceinline__ bool misses_detector(const DevGeomHead &g, const floa
 // point indicates and try once more.  Anything else -- gaps between panels, entries through side or end faces, rays that
 // leave through the axial ends -- is left to the full search (the caller queues the photon for a SEARCH pass).
 // Called by all 32 lanes (`active` = this lane has a photon to place): the early exit is a full-warp vote.
-__device__ __forceinline__ bool ring_entry_fast(const DevGeomHead &g, const DevPanel *pan, const float x[3], const float d[3], bool active, int &bp, float &bt) {
-  const float dxy2 = fmaf(d[0], d[0], d[1] * d[1]);
-  const float b = fmaf(x[0], d[0], x[1] * d[1]);
-  const float cc = fmaf(g.bore_r, g.bore_r, -fmaf(x[0], x[0], x[1] * x[1]));                 // > 0: the photon is inside the bore
-  const float tc = (sqrt_fast(fmaf(dxy2, cc, b * b)) - b) * rcp_fast(dxy2 + 1e-30f);       // leaves the inscribed circle here
-  const float phi = atan2_coarse(fmaf(tc, d[1], x[1]), fmaf(tc, d[0], x[0]));
-  int k = __float2int_rn((phi - g.ring_phi0) * g.ring_kscale);
-  k += k < 0 ? g.n_panels : 0; k -= k >= g.n_panels ? g.n_panels : 0;
+// `hint_turns` >= 0 (the same choice in every lane): the ray's azimuth in turns is already known -- a source on the axis
+// draws it [R14] -- and replaces the circle crossing as the estimate.
+__device__ __forceinline__ bool ring_entry_fast(const DevGeomHead &g, const DevPanel *pan, const float x[3], const float d[3], bool active, float hint_turns, int &bp, float &bt) {
+  int k;
+  if (hint_turns >= 0.0f) {
+    float kf = hint_turns - g.ring_phi0 * 0.15915494f; kf -= floorf(kf);
+    k = __float2int_rn(kf * (float)g.n_panels); k = k >= g.n_panels ? 0 : k;
+  } else {
+    const float dxy2 = fmaf(d[0], d[0], d[1] * d[1]);
+    const float b = fmaf(x[0], d[0], x[1] * d[1]);
+    const float cc = fmaf(g.bore_r, g.bore_r, -fmaf(x[0], x[0], x[1] * x[1]));               // > 0: the photon is inside the bore
+    const float tc = (sqrt_fast(fmaf(dxy2, cc, b * b)) - b) * rcp_fast(dxy2 + 1e-30f);     // leaves the inscribed circle here
+    const float phi = atan2_coarse(fmaf(tc, d[1], x[1]), fmaf(tc, d[0], x[0]));
+    k = __float2int_rn((phi - g.ring_phi0) * g.ring_kscale);
+    k += k < 0 ? g.n_panels : 0; k -= k >= g.n_panels ? g.n_panels : 0;
+  }
   const float iz = rcp_dir(d[2]);
   const float z1 = (g.blo[1] - x[2]) * iz, z2 = (g.bhi[1] - x[2]) * iz;
   const float tnz = fmaxf(fminf(z1, z2), 0.0f), tfz = fmaxf(z1, z2);
@@ -449,9 +457,10 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
 
     if (gen == 1) {
       // ---------------------------------------------- GEN1 (point source): the pair's source block [R3].  With PRETEST, cos(theta)
-      // decides whether BOTH photons leave through the axial ends -- photon A as misses_detector would, photon B for
-      // any acolinearity deviation it can draw [R15] (the polar deviation is at most sigma sqrt(-2 ln u_min)); such
-      // pairs end here (two ESCAPEs).  The others are queued for GEN2.
+      // decides whether BOTH photons leave through the axial ends (misses_axially for photon A, and for photon B with any
+      // acolinearity deviation it can draw [R15]); both tests are monotonic in u, so the host turns them into two integer
+      // bounds on the 23 bits of u (pretest_bounds, with extra margin: a pair kept here is tested again, exactly, in
+      // GEN2).  Pairs outside the bounds end here (two ESCAPEs); the others are queued for GEN2.
       grab();
       const int ng = (int)min(32u, w_end - w_next);
       const uint32_t j = w_next + (uint32_t)lane;
@@ -463,13 +472,8 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
         w = philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 0u, 1u), key);
         keep = true;
         if (PRETEST) {
-          const float u = u01(w.x), ct = 1.0f - 2.0f * u, sth = 2.0f * sqrt_fast(u * (1.0f - u));
-          const bool miss_a = misses_axially(g, src_r0, src.pos[2], sth * 1.0001f, ct);
-          // photon B: within rho_max of -d.  |d_z| >= |ct| cos(rho) - sth sin(rho), |d_xy| <= sth cos(rho) + |ct| sin(rho)
-          const float sr = src.acol_sin_max, cr = src.acol_cos_max;
-          const float bz = fmaf(fabsf(ct), cr, -sth * sr), bxy = fmaf(sth, cr, fabsf(ct) * sr) * 1.0001f;
-          const bool miss_b = bz > 0.0f && misses_axially(g, src_r0, src.pos[2], bxy, ct > 0.0f ? -bz : bz);
-          keep = !(miss_a && miss_b);
+          const uint32_t kq = w.x >> 9;                                // [R2] the 23 bits of u: cos(theta) = 1 - 2u is monotonic in them
+          keep = kq >= src.pre_klo && kq <= src.pre_khi;
           if (HASH && !keep) { uint64_t he = kHash0; hash_ev(he, EV_ESCAPE, 0); hash_out[2ull * j] = he; hash_out[2ull * j + 1] = he; }
         }
       }
@@ -491,9 +495,10 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       q.meta = (kNoPanel << 5) | (uint32_t)gen_b; q.ids = kNone; q.E = 511.0f; q.path = 0.0f; q.inv_mu = 0.0f;
       q.x[0] = src.pos[0]; q.x[1] = src.pos[1]; q.x[2] = src.pos[2];
       q.d[0] = 1.0f; q.d[1] = 0.0f; q.d[2] = 0.0f;
-      float sxy = 1.0f;                                                // |d_xy|
+      float sxy = 1.0f, hint = 0.0f;                                   // |d_xy|; azimuth in turns (exact for a source on the axis)
       if (have) {
         const uint4 w = W.qw[cQ - 1 - lane]; q.pair = W.qp[cQ - 1 - lane];
+        hint = u01(w.y) + (gen_b ? 0.5f : 0.0f);
         const float u = u01(w.x), ct = 1.0f - 2.0f * u, sth = 2.0f * sqrtf(u * (1.0f - u));   // sin^2 = (1-ct)(1+ct)
         float sp, cp; sincospif(2.0f * u01(w.y), &sp, &cp);
         q.d[0] = sth * cp; q.d[1] = sth * sp; q.d[2] = ct; sxy = sth;
@@ -516,7 +521,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       }
       int bp = 0; float bt = 0.0f; bool entered = false;
       if (FAST && fused) {
-        entered = ring_entry_fast(g, pan, q.x, q.d, alive, bp, bt);
+        entered = ring_entry_fast(g, pan, q.x, q.d, alive, src_r0 == 0.0f ? hint : -1.0f, bp, bt);
         if (entered) enter_panel(q, hq, bp, bt);
       }
       const unsigned ma = __ballot_sync(FULL, alive);
@@ -608,7 +613,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       }
       int bp = -1; float bt = 0.0f; bool found = false;
       if (FAST && PHANTOM && g.ring_edge_h > 0.0f)                    // photons that have just left the phantom, inside the bore
-        found = ring_entry_fast(g, pan, q.x, q.d, act && excl == (int)kNoPanel && fmaf(q.x[0], q.x[0], q.x[1] * q.x[1]) < g.bore_r * g.bore_r, bp, bt);
+        found = ring_entry_fast(g, pan, q.x, q.d, act && excl == (int)kNoPanel && fmaf(q.x[0], q.x[0], q.x[1] * q.x[1]) < g.bore_r * g.bore_r, -1.0f, bp, bt);
       if (act) {
         if (!found) bp = panel_search<PLANAR>(g, pan, q.x, q.d, excl, bt);
         if (bp < 0) {
@@ -899,6 +904,35 @@ int transport_warps_that_fit(const DevTables &T, int n_panels, bool hash, size_t
   return w >= 4 ? w : 0;
 }
 
+// Point-source pre-test as two integer bounds on k = (polar word >> 9), u = (k + 0.5) 2^-23 [R2].  A pair may be dropped in
+// GEN1 only when misses_axially holds for photon A (d_z = 1 - 2u) AND for photon B with any acolinearity deviation it can
+// draw [R15] (polar deviation at most rho_max: |d_z| >= |ct| cos(rho) - sth sin(rho), |d_xy| <= sth cos(rho) + |ct| sin(rho)).
+// Both tests are monotonic in u on each side of u = 1/2, so the dropped pairs are k < k_lo and k > k_hi.  The bounds come
+// from the same inequality evaluated in fp64 with wider margins than the kernel's fp32 form (path to the bore radius
+// x 0.999 instead of 0.9999, the axial limit 2 um further out instead of 1 um, |d_xy| bounds + 0.1 %) and are then moved 64
+// counts (7.6e-6 in u) towards the ends: every pair dropped here fails the exact tests of GEN2 too, the few extra pairs kept
+// are dropped there.
+static void pretest_bounds(const DevGeomHead &g, const DevSource &src, uint32_t &k_lo, uint32_t &k_hi) {
+  const double r0 = hypot((double)src.pos[0], (double)src.pos[1]), z0 = src.pos[2];
+  const double sr = src.acol_sin_max, cr = src.acol_cos_max;
+  auto misses = [&](double sxy, double dz) -> bool {
+    const double t = ((double)g.bore_r - r0) / (sxy + 1e-30) * 0.999, z1 = z0 + dz * t;
+    return dz > 0.0 ? z1 > (double)g.bhi[1] + 2e-3 : (dz < 0.0 && z1 < (double)g.blo[1] - 2e-3);
+  };
+  auto drop = [&](uint32_t k) -> bool {
+    const double u = ((double)k + 0.5) * (1.0 / 8388608.0), ct = 1.0 - 2.0 * u, sth = 2.0 * sqrt(u * (1.0 - u));
+    const double bz = fabs(ct) * cr - sth * sr, bxy = (sth * cr + fabs(ct) * sr) * 1.001;
+    return misses(sth * 1.001, ct) && bz > 0.0 && misses(bxy, ct > 0.0 ? -bz : bz);
+  };
+  const uint32_t half = 1u << 22;                                     // k < half: photon A goes up (+z)
+  uint32_t lo = 0, hi = half;                                         // first k in [0, half] that is not dropped
+  while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (drop(mid)) lo = mid + 1; else hi = mid; }
+  k_lo = lo > 64u ? lo - 64u : 0u;
+  lo = half; hi = (1u << 23);                                         // first k in [half, 2^23] from which all are dropped
+  while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (drop(mid)) hi = mid; else lo = mid + 1; }
+  k_hi = lo + 63u < (1u << 23) ? lo + 63u : (1u << 23) - 1u;
+}
+
 cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
                              unsigned long long *work_counter, int sm_count, int warps, cudaStream_t stream) {
@@ -932,10 +966,13 @@ cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, cons
       pretest = r0 < host_geom.bore_r && (zm <= 0.0 || zm < 2.0 * (host_geom.bore_r - r0));
     }
   }
+  DevSource srcp = src;
+  srcp.pre_klo = 0u; srcp.pre_khi = 0xFFFFFFFFu;
+  if (pretest && src.kind == 0) pretest_bounds(head, src, srcp.pre_klo, srcp.pre_khi);
   auto launch = [&](auto kernel) -> cudaError_t {
     cudaError_t le = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (le != cudaSuccess) return le;
-    kernel<<<blocks, threads, smem, stream>>>(head, panels, T, src, first_history, n_pairs, key, H, hash_out, work_counter, grab_pairs);
+    kernel<<<blocks, threads, smem, stream>>>(head, panels, T, srcp, first_history, n_pairs, key, H, hash_out, work_counter, grab_pairs);
     return cudaSuccess;
   };
   // specialised builds for the shapes the five configs use (point source or voxel map + phantom, in a repetition-mode

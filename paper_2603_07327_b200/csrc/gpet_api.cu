@@ -479,7 +479,8 @@ static int make_digi(const gpet_source *src, uint64_t seed, uint64_t n_pairs_tot
   P->e_lo = d->e_lo_keV; P->e_hi = d->e_hi_keV; P->window_s = d->window_ns * 1e-9;
   P->shift = d->readout_level == 0 ? 5 : (d->readout_level == 1 ? 20 : 26);
   P->activity_bq = src->activity_bq; P->pairs_per_slice = src->pairs_per_time_slice ? src->pairs_per_time_slice : n_pairs_total;
-  P->seed = seed; P->slice_s = (double)P->pairs_per_slice / P->activity_bq;
+  P->seed = seed; P->slice_s = (double)P->pairs_per_slice / P->activity_bq; P->n_pairs_total = n_pairs_total;
+  for (int r = 0; r < 10; ++r) { P->keys.k[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; P->keys.k[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }
   P->lambda = 0.0; P->pfrac = 0.0; P->q_scale = (double)P->pairs_per_slice / (double)n_pairs_total;
   if (src->half_life_s > 0.0) {                                      // [R34] decay law
     if (!(src->duration_s > 0.0)) return fail(GPET_E_INVALID_ARG, "half_life_s > 0 needs duration_s > 0");

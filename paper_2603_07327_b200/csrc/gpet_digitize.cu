@@ -42,6 +42,32 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t *t
 }
 __device__ __forceinline__ uint32_t block_exclusive_scan_256(uint32_t v, uint32_t *total) { return block_exclusive_scan<8>(v, total); }
 
+// Decoupled look-back of one tile, run by warp 0 of the tile's block: publishes the tile's aggregate `tot` (flag 1), adds up
+// the aggregates of the preceding tiles 32 at a time until one that already knows its inclusive prefix (flag 2), publishes
+// this tile's inclusive prefix and returns the exclusive one.  state: [0] ticket counter, [1 + tile] = flag << 62 | value.
+__device__ __forceinline__ uint32_t lookback_prefix(unsigned long long *state, uint32_t tile, uint32_t tot) {
+  volatile unsigned long long *st = state + 1;
+  const int lane = threadIdx.x & 31;
+  uint32_t prefix = 0;
+  if (tile > 0) {
+    if (lane == 0) st[tile] = (1ull << 62) | tot;
+    for (int j = (int)tile - 1;; j -= 32) {
+      const int jj = j - lane;
+      unsigned long long w = 2ull << 62;                              // before tile 0: an inclusive prefix of 0
+      if (jj >= 0) do { w = st[jj]; } while ((w >> 62) == 0ull);
+      const unsigned incl = __ballot_sync(0xFFFFFFFFu, (w >> 62) == 2ull);
+      const int first = incl ? __ffs(incl) - 1 : 31;                  // nearest predecessor that already knows its prefix
+      uint32_t part = lane <= first ? (uint32_t)w : 0u;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xFFFFFFFFu, part, o);
+      prefix += part;
+      if (incl) break;
+    }
+  }
+  if (lane == 0) st[tile] = (2ull << 62) | (unsigned long long)(prefix + tot);
+  return prefix;
+}
+
 // Single-pass exclusive scan with decoupled look-back (one read and one write of the data).  Tiles take tickets
 // from an atomic counter, so a tile only ever waits for tiles that are already running or done; a tile publishes
 // its aggregate (flag 1) as soon as it is known and its inclusive prefix (flag 2) after the look-back.
@@ -73,26 +99,8 @@ __global__ void __launch_bounds__(256) scan_lookback_kernel(const uint32_t *in, 
   for (int k = 0; k < kItems; ++k) s += v[k];
   uint32_t tot; uint32_t ex = block_exclusive_scan_256(s, &tot);
   if (threadIdx.x < 32) {                                            // warp 0: publish, then look back 32 tiles at a time
-    volatile unsigned long long *st = state + 1;
-    const int lane = threadIdx.x;
-    uint32_t prefix = 0;
-    if (tile > 0) {
-      if (lane == 0) st[tile] = (1ull << 62) | tot;
-      for (int j = (int)tile - 1;; j -= 32) {
-        const int jj = j - lane;
-        unsigned long long w = 2ull << 62;                            // before tile 0: an inclusive prefix of 0
-        if (jj >= 0) do { w = st[jj]; } while ((w >> 62) == 0ull);
-        const unsigned incl = __ballot_sync(0xFFFFFFFFu, (w >> 62) == 2ull);
-        const int first = incl ? __ffs(incl) - 1 : 31;                // nearest predecessor that already knows its prefix
-        uint32_t part = lane <= first ? (uint32_t)w : 0u;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xFFFFFFFFu, part, o);
-        prefix += part;
-        if (incl) break;
-      }
-    }
-    if (lane == 0) {
-      st[tile] = (2ull << 62) | (unsigned long long)(prefix + tot);
+    const uint32_t prefix = lookback_prefix(state, tile, tot);
+    if (threadIdx.x == 0) {
       s_prefix = prefix;
       if (tile == ntiles - 1) { out[n] = prefix + tot; if (total_out) *total_out = prefix + tot; }
     }
@@ -158,9 +166,16 @@ __global__ void __launch_bounds__(256) scatter_hits_kernel(HitBuf H, uint32_t bo
 }
 
 // ---------------------------------------------------------------- stage 2: adder + blur + window + time
-struct Buckets { double t_lo, scale; uint32_t nb; };
+// Time buckets of a batch: nb equal intervals of [t_lo, t_hi).  Two uses.  FINE buckets (cap = 0; about one kept single
+// each): counted while the adder appends its singles, then a counting sort (scan, scatter, rank inside the bucket).
+// COARSE buckets (cap > 0; the decay times of a batch are uniform by construction [R16], so a bucket sized for a mean of
+// kCoarseMean singles never sees more than cap): the adder writes each kept single straight into its bucket's region of
+// cap records, and one block per group of buckets sorts the regions in shared memory -- no scatter pass through HBM.
+struct Buckets { double t_lo, scale; uint32_t nb, cap; };
+constexpr uint32_t kCoarseMean = 512, kCoarseCap = 832, kSubBuckets = 1024;   // cap = mean + 14 sigma of a Poisson count
+__device__ __forceinline__ double bucket_coord(const Buckets &B, double t) { return __dmul_rn(__dsub_rn(t, B.t_lo), B.scale); }   // monotonic in t
 __device__ __forceinline__ uint32_t bucket_of(const Buckets &B, double t) {
-  const double x = (t - B.t_lo) * B.scale;
+  const double x = bucket_coord(B, t);
   if (!(x > 0.0)) return 0u;
   return x >= (double)(B.nb - 1) ? B.nb - 1 : (uint32_t)x;
 }
@@ -223,14 +238,16 @@ __host__ __device__ inline double decay_time_of(const DigiParams &P, double slic
   return slice_plus_u * P.slice_s;
 #endif
 }
-__device__ __forceinline__ double decay_time(const DigiParams &P, uint64_t history) {
-  const uint2 key = make_uint2((uint32_t)P.seed, (uint32_t)(P.seed >> 32));
-  const uint4 w = philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 0u, 2u), key);
+// u53 of [R16]: words 8, 9 of the history's source stream (block 2)
+__device__ __forceinline__ double decay_u53(const DigiParams &P, uint64_t history) {
+  const uint4 w = philox4x32_10(make_uint4((uint32_t)history, (uint32_t)(history >> 32), 0u, 2u), P.keys);
   const uint64_t bits = (((uint64_t)w.x << 32) | (uint64_t)w.y) >> 11;
-  const double u53 = __dmul_rn(__dadd_rn((double)bits, 0.5), 1.0 / 9007199254740992.0);
+  return __dmul_rn(__dadd_rn((double)bits, 0.5), 1.0 / 9007199254740992.0);
+}
+__device__ __forceinline__ double decay_time(const DigiParams &P, uint64_t history) {
   const uint64_t B = P.pairs_per_slice;
   const uint64_t slice = history < B ? 0ull : history / B;
-  return decay_time_of(P, __dadd_rn((double)slice, u53));
+  return decay_time_of(P, __dadd_rn((double)slice, decay_u53(P, history)));
 }
 
 // [R25] standard normal by Box-Muller.  The blurred energy must stay within 1e-3 keV of the fp64 oracle's: sigma is
@@ -240,6 +257,18 @@ __device__ __forceinline__ float box_muller(float u0, float u1) {
   const float l = u0 < 0.999f ? __logf(u0) : logf(u0);
   float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(-2.0f * l));
   return -r * __cosf(6.283185307179586f * (u1 - 0.5f));              // cos(2 pi u) = -cos(2 pi u - pi)
+}
+
+// a deposit in 2^-40 keV fixed point: e 2^40 is exact in fp32 (a power-of-two scaling), so the rounding to an integer is
+// the only one -- the same value the fp64 product rounds to
+__device__ __forceinline__ long long deposit_fixed(float e) { return __float2ll_rn(e * 1099511627776.0f); }
+
+// coarse buckets: the kept single goes to the next free record of its bucket's region.  A region never fills (see
+// Buckets); if it did, the single is dropped and the fill count put back, so the later passes see min(fill, cap).
+__device__ __forceinline__ void emit_coarse(const Buckets &B, const SinRec &s, SinRec *regions, uint32_t *fill) {
+  const uint32_t b = bucket_of(B, s.t), pos = atomicAdd(&fill[b], 1u);
+  if (pos < B.cap) store_rec(&regions[(size_t)b * B.cap + pos], &s);
+  else atomicSub(&fill[b], 1u);
 }
 
 // records per block of the adder / bucket-scatter pair: the same split in both kernels, a multiple of the block size
@@ -260,7 +289,6 @@ __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uin
                                                     const HitRec *rec, SinRec *sing, uint32_t *srank, uint32_t *kcnt, uint32_t *bcnt) {
   __shared__ uint32_t s_cnt;
   const uint32_t n = *n_rec, R = region_size(n, gridDim.x), r0 = blockIdx.x * R;
-  const uint2 key = make_uint2((uint32_t)P.seed, (uint32_t)(P.seed >> 32));
   const int lane = threadIdx.x & 31;
   if (threadIdx.x == 0) s_cnt = 0;
   __syncthreads();
@@ -281,7 +309,7 @@ __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uin
           if ((r.x >> P.shift) != unit) continue;
           if ((((uint64_t)r.x << 32) | j) < my_key) { leader = false; break; }
           const float2 et = *reinterpret_cast<const float2 *>(&rec[j].e);
-          isum += __double2ll_rn((double)et.x * 1099511627776.0);
+          isum += deposit_fixed(et.x);
           const uint32_t ord = r.x & 31u;
           if (et.x > e_best || (et.x == e_best && ord < best_ord)) { e_best = et.x; best = j; best_ord = ord; }
           tof_min = fminf(tof_min, et.y);
@@ -290,7 +318,7 @@ __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uin
       }
       if (leader) {
         const uint64_t history = first_history + h;
-        const uint4 w = philox4x32_10(make_uint4((uint32_t)history, 0u, 3u, unit), key);        // Box-Muller on words 0,1
+        const uint4 w = philox4x32_10(make_uint4((uint32_t)history, 0u, 3u, unit), P.keys);        // Box-Muller on words 0,1
         const float nrm = box_muller(u01(w.x), u01(w.y));
         const float sigma = P.sigma_scale * (P.ref_keV > 0.0f ? sqrtf(P.ref_keV * e_sum) : e_sum);
         const float e_b = fmaf(sigma, nrm, e_sum);
@@ -302,6 +330,7 @@ __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uin
         }
       }
     }
+    if (B.cap) { if (keep) emit_coarse(B, s, sing, bcnt); continue; }   // coarse buckets: straight into the bucket's region
     const unsigned mk = __ballot_sync(0xFFFFFFFFu, keep);
     if (mk) {
       uint32_t o = 0;
@@ -323,7 +352,7 @@ __global__ void __launch_bounds__(256) adder_kernel(DigiParams P, Buckets B, uin
 // order array -- followed by the same adder, blur, window and time as adder_kernel on the staged copies.  No count
 // pass, no global scan, no scatter of records through HBM; the hit buffer is read once, coalesced.
 constexpr int kChunkThreads = 128;   // small blocks: many chunks resident per SM hide the barriers of each
-__global__ void __launch_bounds__(kChunkThreads) chunk_adder_kernel(DigiParams P, Buckets B, uint64_t first_history, HitBuf H, SinRec *sing, uint32_t *srank,
+__global__ void __launch_bounds__(kChunkThreads, 12) chunk_adder_kernel(DigiParams P, Buckets B, uint64_t first_history, HitBuf H, SinRec *sing, uint32_t *srank,
                                                           uint32_t *kcnt, uint32_t *bcnt) {
   extern __shared__ __align__(16) unsigned char chunk_smem[];       // 18 bytes per region entry (cap rounded up to 8): sized at launch
   __shared__ uint32_t s_cnt[kHitChunkPairs], s_off[kHitChunkPairs];
@@ -335,7 +364,9 @@ __global__ void __launch_bounds__(kChunkThreads) chunk_adder_kernel(DigiParams P
   const unsigned long long g0 = (unsigned long long)c * cap;
   const uint32_t first_lo = (uint32_t)first_history + c * kHitChunkPairs;
   const int lane = threadIdx.x & 31;
-  const uint2 key = make_uint2((uint32_t)P.seed, (uint32_t)(P.seed >> 32));
+  // [R16] slice of a history = history / B: one 64-bit division per chunk, then a compare per history (B >= 512)
+  const uint64_t h0 = first_history + (uint64_t)c * kHitChunkPairs, Bs = P.pairs_per_slice;
+  const uint64_t slice0 = h0 < Bs ? 0ull : h0 / Bs, rem0 = h0 - slice0 * Bs;
   for (int q = threadIdx.x; q < (int)kHitChunkPairs; q += kChunkThreads) s_cnt[q] = 0;
   if (threadIdx.x == 0) s_kept = 0;
   __syncthreads();
@@ -373,26 +404,30 @@ __global__ void __launch_bounds__(kChunkThreads) chunk_adder_kernel(DigiParams P
           if ((ids2 >> P.shift) != unit) continue;
           if ((((uint64_t)ids2 << 32) | i2) < my_key) { leader = false; break; }
           const float e2 = s_e[i2];
-          isum += __double2ll_rn((double)e2 * 1099511627776.0);
+          isum += deposit_fixed(e2);
           const uint32_t ord = ids2 & 31u;
           if (e2 > e_best || (e2 == e_best && ord < best_ord)) { e_best = e2; best = i2; best_ord = ord; }
           tof_min = fminf(tof_min, s_tof[i2]);
         }
         e_sum = (float)((double)isum * (1.0 / 1099511627776.0));
       }
+      __syncwarp(__activemask());                                    // one copy of the blur and time code below, run by all leaders together
       if (leader) {
-        const uint64_t history = first_history + (uint64_t)c * kHitChunkPairs + h;
-        const uint4 w = philox4x32_10(make_uint4((uint32_t)history, 0u, 3u, unit), key);        // Box-Muller on words 0,1
+        const uint64_t history = h0 + h;
+        const uint4 w = philox4x32_10(make_uint4((uint32_t)history, 0u, 3u, unit), P.keys);        // Box-Muller on words 0,1
         const float nrm = box_muller(u01(w.x), u01(w.y));
         const float sigma = P.sigma_scale * (P.ref_keV > 0.0f ? sqrtf(P.ref_keV * e_sum) : e_sum);
         const float e_b = fmaf(sigma, nrm, e_sum);
         keep = e_b >= P.e_lo && e_b < P.e_hi;
         if (keep) {
-          s.t = __dadd_rn(decay_time(P, history), __dmul_rn((double)tof_min, 1e-9));
+          uint64_t slice = slice0;
+          if (Bs >= kHitChunkPairs) slice += rem0 + h >= Bs ? 1ull : 0ull; else slice = history / Bs;
+          s.t = __dadd_rn(decay_time_of(P, __dadd_rn((double)slice, decay_u53(P, history))), __dmul_rn((double)tof_min, 1e-9));
           s.history = (uint32_t)history; s.ids = s_ids[best]; s.x = H.x[g0 + best]; s.y = H.y[g0 + best]; s.z = H.z[g0 + best]; s.e = e_b;
         }
       }
     }
+    if (B.cap) { if (keep) emit_coarse(B, s, sing, bcnt); continue; }   // coarse buckets: straight into the bucket's region
     const unsigned mk = __ballot_sync(0xFFFFFFFFu, keep);
     if (mk) {
       uint32_t o = 0;
@@ -442,55 +477,208 @@ __global__ void __launch_bounds__(256) bucket_sort_kernel(const SinRec *srt, int
   }
 }
 
-// ---------------------------------------------------------------- stage 4: coincidence windows [R27]
-// A thread per cluster start (gap >= tau to the previous single) walks its cluster with the window rule and writes
-// the flag of EVERY member (1 = this single opens an accepted pair with its successor), so `flag` needs no clearing.
-__global__ void __launch_bounds__(256) coincidence_flag_kernel(const SinRec *fin, const uint32_t *n_ptr, double tau, uint32_t *flag) {
-  const uint32_t n = *n_ptr;
-  for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n; i += gridDim.x * 256u) {
-    if (i == 0 || !(__dsub_rn(fin[i].t, fin[i - 1].t) < tau)) {
-      uint32_t o = i;
-      for (;;) {                                                     // o opens a window
-        const double to = fin[o].t;
-        uint32_t j = o + 1;
-        while (j < n && __dsub_rn(fin[j].t, to) < tau) { flag[j] = 0u; ++j; }
-        flag[o] = (j - o == 2 && (fin[o].ids >> 26) != (fin[o + 1].ids >> 26)) ? 1u : 0u;
-        if (j >= n || !(__dsub_rn(fin[j].t, fin[j - 1].t) < tau)) break;   // the next opener starts a new cluster (its own thread)
-        o = j;
+// ---------------------------------------------------------------- stage 3 with coarse buckets: one block sorts a group of buckets
+// The records of kSortGroup consecutive buckets (together at most kCoarseCap, ~560 on C1) are staged in shared memory and
+// ordered by (t, history, unit) with a counting sort over kSubBuckets equal time intervals (shared atomics give each record
+// its rank of arrival, a block scan the offsets) and a rank by comparison among the records of the same sub-bucket (rarely
+// more than one).  The time-ordered records leave as whole sectors, coalesced, at the group's offset in the final array.
+constexpr int kSortThreads = 256;
+constexpr uint32_t kSortGroup = 4;   // buckets per block: their records are sorted together when they fit (the regions are sized for
+                                     // the worst case -- every hit a kept single -- and are a quarter full on C1), else one by one
+// sorts the records of buckets [b0, b0 + nbk) (together at most kCoarseCap) and writes them at boff[b0]
+__device__ __forceinline__ void sort_span(const SinRec *regions, const uint32_t *fill, const uint32_t *boff, const Buckets &B, int shift, SinRec *fin, const SinglesBuf &S,
+                                          uint32_t b0, uint32_t nbk, uint32_t n, uint4 *s_a, uint32_t *s_src, uint32_t *s_cnt, uint32_t *s_off,
+                                          uint16_t *s_sb, uint16_t *s_rk, uint16_t *s_idx, uint16_t *s_fin) {
+  const uint32_t base = boff[b0];
+  const double sub_scale = (double)(kSubBuckets / kSortGroup) * (double)(kSortGroup / nbk);   // nbk = 1 or kSortGroup
+  for (int q = threadIdx.x; q < (int)kSubBuckets; q += kSortThreads) s_cnt[q] = 0;
+  __syncthreads();
+  for (uint32_t k = 0, i0 = 0; k < nbk; ++k) {
+    const uint32_t f = fill[b0 + k], nk = f < B.cap ? f : B.cap;
+    const uint4 *reg = reinterpret_cast<const uint4 *>(regions + (size_t)(b0 + k) * B.cap);
+    for (uint32_t q = threadIdx.x; q < nk; q += kSortThreads) {
+      const uint32_t i = i0 + q;
+      const uint4 ra = reg[2 * q];
+      s_a[i] = ra; s_src[i] = (b0 + k) * B.cap + q;                   // the payload {x, y, z, e} is fetched when the record leaves
+      const double t = __longlong_as_double((long long)(((unsigned long long)ra.y << 32) | ra.x));
+      const double x = __dmul_rn(__dsub_rn(bucket_coord(B, t), (double)b0), sub_scale);   // monotonic in t
+      const uint32_t sb = !(x > 0.0) ? 0u : (x >= (double)(kSubBuckets - 1) ? kSubBuckets - 1 : (uint32_t)x);
+      s_sb[i] = (uint16_t)sb; s_rk[i] = (uint16_t)atomicAdd(&s_cnt[sb], 1u);
+    }
+    i0 += nk;
+  }
+  __syncthreads();
+  {
+    constexpr int kPer = kSubBuckets / kSortThreads;
+    uint32_t v[kPer], sum = 0;
+#pragma unroll
+    for (int q = 0; q < kPer; ++q) { v[q] = s_cnt[kPer * threadIdx.x + q]; sum += v[q]; }
+    uint32_t tot; uint32_t ex = block_exclusive_scan<kSortThreads / 32>(sum, &tot);
+#pragma unroll
+    for (int q = 0; q < kPer; ++q) { s_off[kPer * threadIdx.x + q] = ex; ex += v[q]; }
+  }
+  __syncthreads();
+  for (uint32_t i = threadIdx.x; i < n; i += kSortThreads) s_idx[s_off[s_sb[i]] + s_rk[i]] = (uint16_t)i;
+  __syncthreads();
+  for (uint32_t p = threadIdx.x; p < n; p += kSortThreads) {         // rank inside the sub-bucket by (t, history, unit)
+    const uint32_t i = s_idx[p], sb = s_sb[i], s0 = s_off[sb], m = s_cnt[sb];
+    uint32_t rank = 0;
+    if (m > 1) {
+      const uint4 me = s_a[i];
+      const double tm = __longlong_as_double((long long)(((unsigned long long)me.y << 32) | me.x));
+      for (uint32_t q = s0; q < s0 + m; ++q) {
+        if (q == p) continue;
+        const uint4 o = s_a[s_idx[q]];
+        const double to = __longlong_as_double((long long)(((unsigned long long)o.y << 32) | o.x));
+        const bool o_less = to != tm ? to < tm : (o.z != me.z ? o.z < me.z : (o.w >> shift) < (me.w >> shift));
+        const bool m_less = to != tm ? tm < to : (o.z != me.z ? me.z < o.z : (me.w >> shift) < (o.w >> shift));
+        if (o_less || (!m_less && q < p)) ++rank;
       }
     }
+    s_fin[s0 + rank] = (uint16_t)i;
+  }
+  __syncthreads();
+  uint4 *out = reinterpret_cast<uint4 *>(fin + base);
+  for (uint32_t p = threadIdx.x; p < n; p += kSortThreads) {
+    const uint32_t i = s_fin[p];
+    const uint4 ra = s_a[i], rb = reinterpret_cast<const uint4 *>(regions + s_src[i])[1];
+    out[2 * p] = ra; out[2 * p + 1] = rb;
+    const unsigned long long o = (unsigned long long)base + p;
+    if (S.history && o < S.capacity) {
+      S.history[o] = ra.z; S.ids[o] = ra.w; S.x[o] = __uint_as_float(rb.x); S.y[o] = __uint_as_float(rb.y); S.z[o] = __uint_as_float(rb.z);
+      S.e[o] = __uint_as_float(rb.w); S.t[o] = __longlong_as_double((long long)(((unsigned long long)ra.y << 32) | ra.x));
+    }
+  }
+  __syncthreads();                                                   // the arrays are reused by the next span
+}
+__global__ void __launch_bounds__(kSortThreads) bucket_sort_coarse_kernel(const SinRec *regions, const uint32_t *fill, const uint32_t *boff, Buckets B, int shift,
+                                                                          SinRec *fin, SinglesBuf S) {
+  __shared__ uint4 s_a[kCoarseCap];                                  // {t, history, ids}
+  __shared__ uint32_t s_src[kCoarseCap], s_cnt[kSubBuckets], s_off[kSubBuckets];
+  __shared__ uint16_t s_sb[kCoarseCap], s_rk[kCoarseCap], s_idx[kCoarseCap], s_fin[kCoarseCap];
+  const uint32_t b0 = blockIdx.x * kSortGroup, nbk = B.nb - b0 < kSortGroup ? B.nb - b0 : kSortGroup;
+  uint32_t n = 0;
+  for (uint32_t k = 0; k < nbk; ++k) { const uint32_t f = fill[b0 + k]; n += f < B.cap ? f : B.cap; }
+  if (n == 0) return;
+  if (n <= B.cap && nbk == kSortGroup) { sort_span(regions, fill, boff, B, shift, fin, S, b0, nbk, n, s_a, s_src, s_cnt, s_off, s_sb, s_rk, s_idx, s_fin); return; }
+  for (uint32_t k = 0; k < nbk; ++k) {
+    const uint32_t f = fill[b0 + k], nk = f < B.cap ? f : B.cap;
+    if (nk) sort_span(regions, fill, boff, B, shift, fin, S, b0 + k, 1u, nk, s_a, s_src, s_cnt, s_off, s_sb, s_rk, s_idx, s_fin);
   }
 }
-__global__ void __launch_bounds__(256) coincidence_write_kernel(const SinRec *fin, const uint32_t *n_ptr, const uint32_t *flag, const uint32_t *coff, CoincBuf C) {
-  const uint32_t n = *n_ptr;
-  for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n; i += gridDim.x * 256u) {
-    if (!flag[i]) continue;
-    const uint32_t o = coff[i];
-    if (o >= C.capacity) continue;
-    SinRec a, b; store_rec(&a, &fin[i]); store_rec(&b, &fin[i + 1]);
-    C.ids_a[o] = a.ids; C.ids_b[o] = b.ids; C.history_a[o] = a.history; C.history_b[o] = b.history;
-    C.e_a[o] = a.e; C.e_b[o] = b.e;
-    C.dt_ns[o] = (float)__dmul_rn(__dsub_rn(b.t, a.t), 1e9); C.t[o] = a.t;
+
+// ---------------------------------------------------------------- stage 4: coincidence windows [R27], two passes
+// A thread per single of the time-ordered array, a tile of kCoTile singles per block, the tile's {t, history, ids} words
+// staged in shared memory.  A single that starts a cluster (gap >= tau to its predecessor) walks the cluster with the
+// window rule: an unconsumed single opens a window, the members are the following singles within tau of the opener,
+// exactly two members on different panels make a coincidence.  Pass 1 counts the accepted pairs per tile; a scan over the
+// tiles gives every tile its offset in the list-mode output, in time order; pass 2 walks again (the tile is still in L2),
+// compacts the openers of its pairs in shared memory (block scan) and writes the records densely, one pair per thread.
+// (One kernel with a decoupled look-back over the tiles was measured first: with ~600 short tiles in flight every tile
+// looks back over the whole wave, 120 us against the two passes' sum.)
+constexpr int kCoTile = 512;
+struct TimeView {   // the tile's words in shared memory, the rest of the array (a cluster that runs past the tile) in global memory
+  const uint4 *tile; const SinRec *fin; uint32_t i0, m;
+  __device__ __forceinline__ double t(uint32_t i) const {
+    if (i - i0 < m) { const uint4 v = tile[i - i0]; return __longlong_as_double((long long)(((unsigned long long)v.y << 32) | v.x)); }
+    return fin[i].t;
   }
+  __device__ __forceinline__ uint32_t panel(uint32_t i) const { return (i - i0 < m ? tile[i - i0].w : fin[i].ids) >> 26; }
+};
+__device__ __forceinline__ void write_pair(const SinRec *fin, uint32_t o, unsigned long long w, const CoincBuf &C) {
+  if (w >= C.capacity) return;
+  SinRec a, b; store_rec(&a, &fin[o]); store_rec(&b, &fin[o + 1]);
+  C.ids_a[w] = a.ids; C.ids_b[w] = b.ids; C.history_a[w] = a.history; C.history_b[w] = b.history;
+  C.e_a[w] = a.e; C.e_b[w] = b.e;
+  C.dt_ns[w] = (float)__dmul_rn(__dsub_rn(b.t, a.t), 1e9); C.t[w] = a.t;
+}
+// walks the cluster that starts at single i and returns the number of accepted pairs.  LIST = false: first = opener of the
+// first pair.  LIST = true: pair c goes to list[pos + c] while pos + c < kCoTile, else straight to output entry w0 + pos + c.
+template <bool LIST>
+__device__ __forceinline__ uint32_t cluster_walk(const TimeView &V, uint32_t n, double tau, uint32_t i, uint32_t &first, uint32_t *list, uint32_t pos,
+                                                 unsigned long long w0, const CoincBuf &C) {
+  uint32_t o = i, c = 0;
+  for (;;) {                                                         // o opens a window
+    const double to = V.t(o);
+    uint32_t j = o + 1;
+    double tl = to;                                                  // time of single j - 1
+    while (j < n) { const double tj = V.t(j); if (!(__dsub_rn(tj, to) < tau)) break; tl = tj; ++j; }
+    if (j - o == 2 && V.panel(o) != V.panel(o + 1)) {
+      if (!LIST) { if (c == 0) first = o; }
+      else if (pos + c < (uint32_t)kCoTile) list[pos + c] = o;
+      else write_pair(V.fin, o, w0 + pos + c, C);
+      ++c;
+    }
+    if (j >= n || !(__dsub_rn(V.t(j), tl) < tau)) break;             // the next opener starts a new cluster (its own thread)
+    o = j;
+  }
+  return c;
+}
+// stages the tile and walks the cluster that single t0 + threadIdx.x starts, if it starts one
+__device__ __forceinline__ uint32_t tile_walk(const SinRec *fin, uint32_t n, double tau, uint32_t tile, uint4 *s_rec, TimeView &V, uint32_t &first, const CoincBuf &C) {
+  const uint32_t t0 = tile * kCoTile, m = n - t0 < (uint32_t)kCoTile ? n - t0 : (uint32_t)kCoTile;
+  const uint32_t i = t0 + threadIdx.x;
+  if (threadIdx.x < m) s_rec[threadIdx.x] = reinterpret_cast<const uint4 *>(fin + i)[0];
+  __syncthreads();
+  V.tile = s_rec; V.fin = fin; V.i0 = t0; V.m = m;
+  if (threadIdx.x < m && (i == 0 || !(__dsub_rn(V.t(i), V.t(i - 1)) < tau))) return cluster_walk<false>(V, n, tau, i, first, nullptr, 0u, 0ull, C);
+  return 0u;
+}
+// pass 1: accepted pairs per tile (0 for the tiles past the last single, so that the scan can run over the host-side bound)
+__global__ void __launch_bounds__(kCoTile) coincidence_count_kernel(const SinRec *fin, const uint32_t *n_ptr, double tau, uint32_t *tile_cnt, CoincBuf C) {
+  __shared__ uint4 s_rec[kCoTile];
+  __shared__ uint32_t s_sum;
+  const uint32_t n = *n_ptr, tile = blockIdx.x;
+  if ((unsigned long long)tile * kCoTile >= n) { if (threadIdx.x == 0) tile_cnt[tile] = 0u; return; }
+  if (threadIdx.x == 0) s_sum = 0u;
+  TimeView V; uint32_t first = 0;
+  uint32_t cnt = tile_walk(fin, n, tau, tile, s_rec, V, first, C);   // (its barrier orders the store to s_sum)
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xFFFFFFFFu, cnt, o);
+  if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(&s_sum, cnt);
+  __syncthreads();
+  if (threadIdx.x == 0) tile_cnt[tile] = s_sum;
+}
+// pass 2: the tile's pairs at its offset of the list-mode output, one pair per thread
+__global__ void __launch_bounds__(kCoTile) coincidence_write_kernel(const SinRec *fin, const uint32_t *n_ptr, double tau, const uint32_t *tile_off, CoincBuf C) {
+  __shared__ uint4 s_rec[kCoTile];
+  __shared__ uint32_t s_open[kCoTile];                               // openers of the tile's first kCoTile accepted pairs, in time order
+  const uint32_t n = *n_ptr, tile = blockIdx.x;
+  if ((unsigned long long)tile * kCoTile >= n) return;
+  const unsigned long long w0 = tile_off[tile];
+  if (tile_off[tile + 1] == (uint32_t)w0) return;                    // no pair starts in this tile
+  TimeView V; uint32_t first = 0;
+  const uint32_t cnt = tile_walk(fin, n, tau, tile, s_rec, V, first, C);
+  uint32_t tot; const uint32_t ex = block_exclusive_scan<kCoTile / 32>(cnt, &tot);
+  // a cluster of the tile may run far past its end (randoms at very high activity): pairs beyond the list's kCoTile
+  // entries are written by the walking thread itself
+  if (cnt == 1 && ex < (uint32_t)kCoTile) s_open[ex] = first;
+  else if (cnt) cluster_walk<true>(V, n, tau, tile * kCoTile + threadIdx.x, first, s_open, ex, w0, C);
+  __syncthreads();
+  const uint32_t listed = tot < (uint32_t)kCoTile ? tot : (uint32_t)kCoTile;
+  if (threadIdx.x < listed) write_pair(fin, s_open[threadIdx.x], w0 + threadIdx.x, C);   // dense: one pair per thread
 }
 
 // ---------------------------------------------------------------- scratch layout + driver
 namespace {
-struct Layout { size_t kcnt, cnt, off, ctl, ctl_bytes, st1, st2, bcnt, boff, flag, coff, hrank, srank, rec, sing, fin, total; uint64_t nb; };
+struct Layout { size_t kcnt, cnt, off, ctl, ctl_bytes, st1, st2, bcnt, boff, tcnt, toff, hrank, srank, rec, sing, fin, total; uint64_t nb, nb_coarse; };
 Layout layout(uint64_t N, uint64_t M) {
   Layout L; size_t o = 0; const uint64_t Mx = M ? M : 1;
   auto take = [&](size_t bytes) { o = (o + 255) & ~(size_t)255; size_t r = o; o += bytes; return r; };
-  L.nb = (Mx + 1) / 2;              // time buckets: kept singles are ~0.4 per hit, so ~1 per bucket
+  L.nb = (Mx + 1) / 2;              // fine time buckets: kept singles are ~0.4 per hit, so ~1 per bucket
+  L.nb_coarse = (Mx + kCoarseMean - 1) / kCoarseMean;   // coarse ones: at most kCoarseMean on average even if every hit became a single
   L.kcnt = take(4 * (148 * 16 + N / kHitChunkPairs + 2));   // kept singles per adder block (dense) or per chunk (chunked layout)
   L.cnt = take(4 * N); L.off = take(4 * (N + 1));
-  // control block, cleared by one memset per call: kept-singles counter, then the look-back state of the three scans
-  const size_t s0 = 8 * (N / kTile + 3), s1 = 8 * (L.nb / kTile + 3), s2 = 8 * (Mx / kTile + 3);
+  // control block, cleared by one memset per call: the look-back state of the three scans (hits per history, singles per
+  // bucket, coincidences per tile)
+  const size_t s0 = 8 * (N / kTile + 3), s1 = 8 * (L.nb / kTile + 3), s2 = 8 * (Mx / kCoTile / kTile + 3);
   L.ctl = take(256 + s0 + s1 + s2); L.st1 = L.ctl + 256 + s0; L.st2 = L.st1 + s1; L.ctl_bytes = 256 + s0 + s1 + s2;
   L.bcnt = take(4 * L.nb); L.boff = take(4 * (L.nb + 1));
-  L.flag = take(4 * Mx); L.coff = take(4 * (Mx + 1));
+  L.tcnt = take(4 * (Mx / kCoTile + 1)); L.toff = take(4 * (Mx / kCoTile + 2));   // accepted pairs per tile of the time-ordered singles
   L.hrank = take(4 * Mx); L.srank = take(4 * Mx);   // rank of a hit in its history / of a kept single in its time bucket
   L.rec = take(32 * Mx);            // hit records by history; reused for the bucket-ordered singles
-  L.sing = take(32 * Mx);           // kept singles, append order
+  const size_t coarse = 32 * (size_t)kCoarseCap * L.nb_coarse;
+  L.sing = take(coarse > 32 * Mx ? coarse : 32 * Mx);   // kept singles: append order, or the regions of the coarse buckets
   L.fin = take(32 * Mx);            // kept singles, time order
   L.total = o + 256; return L;
 }
@@ -507,22 +695,27 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   char *s = (char *)scratch;
   uint32_t *cnt = (uint32_t *)(s + L.cnt), *off = (uint32_t *)(s + L.off), *kcnt = (uint32_t *)(s + L.kcnt);
   unsigned long long *st0 = (unsigned long long *)(s + L.ctl + 256), *st1 = (unsigned long long *)(s + L.st1), *st2 = (unsigned long long *)(s + L.st2);
-  uint32_t *bcnt = (uint32_t *)(s + L.bcnt), *boff = (uint32_t *)(s + L.boff), *flag = (uint32_t *)(s + L.flag), *coff = (uint32_t *)(s + L.coff);
-  uint32_t *hrank = (uint32_t *)(s + L.hrank), *srank = (uint32_t *)(s + L.srank);
+  uint32_t *bcnt = (uint32_t *)(s + L.bcnt), *boff = (uint32_t *)(s + L.boff);
+  uint32_t *hrank = (uint32_t *)(s + L.hrank), *srank = (uint32_t *)(s + L.srank), *tcnt = (uint32_t *)(s + L.tcnt), *toff = (uint32_t *)(s + L.toff);
   HitRec *rec = (HitRec *)(s + L.rec); SinRec *srt = (SinRec *)(s + L.rec), *sing = (SinRec *)(s + L.sing), *fin = (SinRec *)(s + L.fin);
-  cudaError_t e;
-  if (!H.chunk_fill && (e = cudaMemsetAsync(cnt, 0, 4 * N, st)) != cudaSuccess) return e;
-  if ((e = cudaMemsetAsync(s + L.ctl, 0, L.ctl_bytes, st)) != cudaSuccess) return e;
-  if ((e = cudaMemsetAsync(bcnt, 0, 4 * L.nb, st)) != cudaSuccess) return e;
-  const uint32_t nh = (uint32_t)n_hits, np = (uint32_t)N, first_lo = (uint32_t)first_history;
   const bool chunked = H.chunk_fill != nullptr;
   const uint64_t B = P.pairs_per_slice;
-  const double slice_s = (double)B / P.activity_bq;
-  Buckets bk; bk.nb = (uint32_t)L.nb;
-  (void)slice_s;
-  bk.t_lo = decay_time_of(P, (double)(first_history / B));          // the batch's time slices cover [t_lo, t_hi) [R16, R34]
-  const double t_hi = decay_time_of(P, fmin((double)((first_history + n_pairs - 1) / B) + 1.0, P.lambda > 0.0 ? 1.0 / P.q_scale : 1e300)) + 2e-6;
+  const uint64_t slice_first = first_history / B, slice_last = (first_history + n_pairs - 1) / B;
+  Buckets bk;
+  bk.t_lo = decay_time_of(P, (double)slice_first);                  // the batch's time slices cover [t_lo, t_hi) [R16, R34]
+  const double t_hi = decay_time_of(P, fmin((double)slice_last + 1.0, P.lambda > 0.0 ? 1.0 / P.q_scale : 1e300)) + 2e-6;
+  // Coarse buckets need times that are uniform over [t_lo, t_hi): the batch lies inside one time slice, or covers whole
+  // slices (a last slice cut short by the end of the run only lowers the density), and the decay law [R34] changes the
+  // rate by less than 10 % across it.  Anything else takes the fine buckets, which count before they place.
+  const bool whole = first_history % B == 0 && ((first_history + n_pairs) % B == 0 || first_history + n_pairs == P.n_pairs_total);
+  const bool coarse = (slice_first == slice_last || whole) && P.lambda * (t_hi - bk.t_lo) < 0.1;
+  bk.nb = (uint32_t)(coarse ? L.nb_coarse : L.nb); bk.cap = coarse ? kCoarseCap : 0u;
   bk.scale = (double)bk.nb / (t_hi - bk.t_lo);
+  cudaError_t e;
+  if (!chunked && (e = cudaMemsetAsync(cnt, 0, 4 * N, st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(s + L.ctl, 0, L.ctl_bytes, st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(bcnt, 0, 4 * (size_t)bk.nb, st)) != cudaSuccess) return e;
+  const uint32_t nh = (uint32_t)n_hits, np = (uint32_t)N, first_lo = (uint32_t)first_history;
   const int ga = grid_for(M);                                         // adder and bucket scatter share the block -> region split
   if (chunked) {
     // 1 + 2. per chunk in shared memory: sort by history, adder, blur, window, time
@@ -535,15 +728,20 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
     // 2. adder, blur, window, time; kept singles appended and counted into time buckets
     adder_kernel<<<ga, 256, 0, st>>>(P, bk, first_history, off, off + N, rec, sing, srank, kcnt, bcnt); count_launch();
   }
-  // 3. time-bucket counting sort
-  if ((e = exclusive_scan(bcnt, L.nb, nullptr, boff, st1, S.n, st)) != cudaSuccess) return e;
-  bucket_scatter_kernel<<<chunked ? (int)H.n_chunks : ga, 256, 0, st>>>(sing, srank, off + N, chunked ? H.chunk_cap : 0u, kcnt, bk, boff, srt); count_launch();
-  bucket_sort_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(srt, P.shift, boff + L.nb, bk, boff, fin, S); count_launch();
-  // 4. coincidences (lengths known on the device only: the scan stops at the number of kept singles)
-  const uint32_t *n_singles = boff + L.nb;
-  coincidence_flag_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(fin, n_singles, P.window_s, flag); count_launch();
-  if ((e = exclusive_scan(flag, M, n_singles, coff, st2, C.n, st)) != cudaSuccess) return e;
-  coincidence_write_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(fin, n_singles, flag, coff, C); count_launch();
+  // 3. time order: offsets of the buckets (the total is the number of kept singles), then the order inside each bucket
+  if ((e = exclusive_scan(bcnt, bk.nb, nullptr, boff, st1, S.n, st)) != cudaSuccess) return e;
+  const uint32_t *n_singles = boff + bk.nb;
+  if (coarse) {
+    bucket_sort_coarse_kernel<<<(bk.nb + kSortGroup - 1) / kSortGroup, kSortThreads, 0, st>>>(sing, bcnt, boff, bk, P.shift, fin, S); count_launch();
+  } else {
+    bucket_scatter_kernel<<<chunked ? (int)H.n_chunks : ga, 256, 0, st>>>(sing, srank, off + N, chunked ? H.chunk_cap : 0u, kcnt, bk, boff, srt); count_launch();
+    bucket_sort_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(srt, P.shift, n_singles, bk, boff, fin, S); count_launch();
+  }
+  // 4. coincidences (the number of singles is known on the device only: tiles past it count zero and return at once)
+  const unsigned co_tiles = (unsigned)((M + kCoTile - 1) / kCoTile);
+  coincidence_count_kernel<<<co_tiles, kCoTile, 0, st>>>(fin, n_singles, P.window_s, tcnt, C); count_launch();
+  if ((e = exclusive_scan(tcnt, co_tiles, nullptr, toff, st2, C.n, st)) != cudaSuccess) return e;
+  coincidence_write_kernel<<<co_tiles, kCoTile, 0, st>>>(fin, n_singles, P.window_s, toff, C); count_launch();
   return cudaGetLastError();
 }
 

@@ -30,6 +30,8 @@ struct DigiParams {
   float ref_keV, e_lo, e_hi; double window_s; int shift;         // ids >> shift = readout unit
   double activity_bq, slice_s; uint64_t pairs_per_slice; uint64_t seed;   // slice_s = pairs_per_slice / activity_bq
   double lambda, pfrac, q_scale;                                 // [R34] decay law: ln2 / half-life (0 = constant activity), 1 - exp(-lambda T), B / N
+  uint64_t n_pairs_total;                                        // pairs of the whole run
+  PhiloxKeys keys;                                               // [R1] the ten round keys of `seed`
 };
 
 struct SinglesBuf { uint32_t *history, *ids; float *x, *y, *z, *e; double *t; unsigned long long capacity; unsigned long long *n; };

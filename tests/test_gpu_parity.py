@@ -179,6 +179,47 @@ def test_digitizer_equals_oracle_on_oracle_hits(tables, level, ref_keV):
     assert np.all(np.diff(gs["t_s"]) >= 0)
 
 
+@pytest.mark.parametrize("slice_pairs,first,n,chunked", [(0, 0, 200_000, False), (50_000, 100_000, 150_000, False), (50_000, 120_000, 150_000, False),
+                                                        (50_000, 100_000, 150_016, True), (1_000, 120_500, 150_000, True), (100, 0, 20_000, True)])
+def test_digitizer_time_sort_paths(tables, slice_pairs, first, n, chunked):
+    """The time sort has two forms: coarse buckets sorted in shared memory when the batch's decay times are uniform over its
+    time range (one slice, or whole slices [R16]) and fine counted buckets otherwise (a batch that starts or ends inside
+    a slice).  Both must give the oracle's singles and coincidences, record for record, on either hit layout, including
+    slices shorter than a chunk of the chunked layout."""
+    from dataclasses import replace
+    src = replace(W.source_point((10.0, 0.0, 4.0), activity_bq=5.0e7), pairs_per_time_slice=slice_pairs)
+    n_total = 400_000
+    o = O.simulate(W.geometry_c3(), tables, src, n, 406, first_history=first, threads=8)
+    dig = W.Digitizer(0.15, 511.0, 350.0, 650.0, 4.0, 0)
+    osg, oco, _ = O.digitize(src, 406, n_total, o.hits, dig)
+    oh = PU.oracle_hits_dict(o.hits)
+    s = api.DeviceSource(src)
+    if chunked:                                                       # oracle hits laid out by 512-pair chunk, as gpet_simulate would
+        hb = api.HitBuffer.allocate_chunked(n, 3.0)
+        nc = (n + 511) // 512
+        cap_c = hb.capacity // nc
+        chunk = (oh["history"].astype(np.int64) - first) // 512
+        order = np.argsort(chunk, kind="stable"); fill = np.bincount(chunk, minlength=nc)
+        assert fill.max() <= cap_c
+        pos = chunk[order] * cap_c + (np.arange(len(order)) - np.repeat(np.cumsum(fill) - fill, fill))
+        for name, arr in (("history", hb.history), ("ids", hb.ids), ("x", hb.x), ("y", hb.y), ("z", hb.z), ("e_keV", hb.e_keV), ("tof_ns", hb.tof_ns)):
+            v = np.ascontiguousarray(oh[name][order])
+            arr[torch.from_numpy(pos).cuda()] = torch.from_numpy(v.view(np.int32) if v.dtype == np.uint32 else v).cuda()
+        hb.chunk_fill[:nc] = torch.from_numpy(fill.astype(np.int32)).cuda()
+        hb.n_hits.fill_(len(order))
+        cap = hb.capacity
+    else:
+        hb = PU.upload_hits(oh, np.random.default_rng(5).permutation(len(o.hits))); cap = len(o.hits)
+    scratch = torch.empty(api.gpet_digitize_scratch_bytes(n, cap), dtype=torch.uint8, device="cuda")
+    sg, co = api.SinglesBuffer.allocate(cap), api.CoincBuffer.allocate(cap)
+    api.gpet_digitize(s, 406, n_total, first, n, hb, cap, dig, scratch, sg, co)
+    torch.cuda.synchronize()
+    gs = sg.to_numpy()
+    assert PU.compare_singles(gs, osg, 5, exact=True, max_symdiff=2) >= len(osg.ids) - 2 > 3000
+    assert PU.compare_coincidences(co.to_numpy(), oco, exact=True, max_symdiff=4) >= len(oco.ids_a) - 4 > 200
+    assert np.all(np.diff(gs["t_s"]) >= 0)
+
+
 def test_digitizer_empty_and_tiny(tables):
     src = W.source_point()
     s = api.DeviceSource(src)

@@ -568,100 +568,68 @@ __global__ void __launch_bounds__(kSortThreads) bucket_sort_coarse_kernel(const 
 }
 
 // ---------------------------------------------------------------- stage 4: coincidence windows [R27], two passes
-// A thread per single of the time-ordered array, a tile of kCoTile singles per block, the tile's {t, history, ids} words
-// staged in shared memory.  A single that starts a cluster (gap >= tau to its predecessor) walks the cluster with the
-// window rule: an unconsumed single opens a window, the members are the following singles within tau of the opener,
-// exactly two members on different panels make a coincidence.  Pass 1 counts the accepted pairs per tile; a scan over the
-// tiles gives every tile its offset in the list-mode output, in time order; pass 2 walks again (the tile is still in L2),
-// compacts the openers of its pairs in shared memory (block scan) and writes the records densely, one pair per thread.
-// (One kernel with a decoupled look-back over the tiles was measured first: with ~600 short tiles in flight every tile
-// looks back over the whole wave, 120 us against the two passes' sum.)
-constexpr int kCoTile = 512;
-struct TimeView {   // the tile's words in shared memory, the rest of the array (a cluster that runs past the tile) in global memory
-  const uint4 *tile; const SinRec *fin; uint32_t i0, m;
-  __device__ __forceinline__ double t(uint32_t i) const {
-    if (i - i0 < m) { const uint4 v = tile[i - i0]; return __longlong_as_double((long long)(((unsigned long long)v.y << 32) | v.x)); }
-    return fin[i].t;
-  }
-  __device__ __forceinline__ uint32_t panel(uint32_t i) const { return (i - i0 < m ? tile[i - i0].w : fin[i].ids) >> 26; }
-};
-__device__ __forceinline__ void write_pair(const SinRec *fin, uint32_t o, unsigned long long w, const CoincBuf &C) {
-  if (w >= C.capacity) return;
-  SinRec a, b; store_rec(&a, &fin[o]); store_rec(&b, &fin[o + 1]);
-  C.ids_a[w] = a.ids; C.ids_b[w] = b.ids; C.history_a[w] = a.history; C.history_b[w] = b.history;
-  C.e_a[w] = a.e; C.e_b[w] = b.e;
-  C.dt_ns[w] = (float)__dmul_rn(__dsub_rn(b.t, a.t), 1e9); C.t[w] = a.t;
-}
-// walks the cluster that starts at single i and returns the number of accepted pairs.  LIST = false: first = opener of the
-// first pair.  LIST = true: pair c goes to list[pos + c] while pos + c < kCoTile, else straight to output entry w0 + pos + c.
-template <bool LIST>
-__device__ __forceinline__ uint32_t cluster_walk(const TimeView &V, uint32_t n, double tau, uint32_t i, uint32_t &first, uint32_t *list, uint32_t pos,
-                                                 unsigned long long w0, const CoincBuf &C) {
-  uint32_t o = i, c = 0;
-  for (;;) {                                                         // o opens a window
-    const double to = V.t(o);
-    uint32_t j = o + 1;
-    double tl = to;                                                  // time of single j - 1
-    while (j < n) { const double tj = V.t(j); if (!(__dsub_rn(tj, to) < tau)) break; tl = tj; ++j; }
-    if (j - o == 2 && V.panel(o) != V.panel(o + 1)) {
-      if (!LIST) { if (c == 0) first = o; }
-      else if (pos + c < (uint32_t)kCoTile) list[pos + c] = o;
-      else write_pair(V.fin, o, w0 + pos + c, C);
-      ++c;
-    }
-    if (j >= n || !(__dsub_rn(V.t(j), tl) < tau)) break;             // the next opener starts a new cluster (its own thread)
-    o = j;
-  }
-  return c;
-}
-// stages the tile and walks the cluster that single t0 + threadIdx.x starts, if it starts one
-__device__ __forceinline__ uint32_t tile_walk(const SinRec *fin, uint32_t n, double tau, uint32_t tile, uint4 *s_rec, TimeView &V, uint32_t &first, const CoincBuf &C) {
-  const uint32_t t0 = tile * kCoTile, m = n - t0 < (uint32_t)kCoTile ? n - t0 : (uint32_t)kCoTile;
-  const uint32_t i = t0 + threadIdx.x;
-  if (threadIdx.x < m) s_rec[threadIdx.x] = reinterpret_cast<const uint4 *>(fin + i)[0];
-  __syncthreads();
-  V.tile = s_rec; V.fin = fin; V.i0 = t0; V.m = m;
-  if (threadIdx.x < m && (i == 0 || !(__dsub_rn(V.t(i), V.t(i - 1)) < tau))) return cluster_walk<false>(V, n, tau, i, first, nullptr, 0u, 0ull, C);
-  return 0u;
-}
-// pass 1: accepted pairs per tile (0 for the tiles past the last single, so that the scan can run over the host-side bound)
-__global__ void __launch_bounds__(kCoTile) coincidence_count_kernel(const SinRec *fin, const uint32_t *n_ptr, double tau, uint32_t *tile_cnt, CoincBuf C) {
-  __shared__ uint4 s_rec[kCoTile];
+// Pass 1, a thread per single of the time-ordered array: a single that starts a cluster (gap >= tau to its predecessor)
+// walks the cluster with the window rule -- an unconsumed single opens a window, the members are the following singles
+// within tau of the opener, exactly two members on different panels make a coincidence -- and writes the flag of EVERY
+// member (1 = this single opens an accepted pair with its successor), so `flag` needs no clearing; every pair is counted
+// in the tile (kCoTile singles) of its opener (tile_cnt is zeroed by the caller).  A scan over the tiles gives every
+// tile its offset in the list-mode output, in time order.  Pass 2: block scan of the tile's flags, one record per
+// flagged single.
+// (Measured alternatives: one kernel with a decoupled look-back over the tiles -- with ~600 short tiles in flight every
+// tile looks back over the whole wave, 120 us; a second walk in pass 2 instead of the flags -- re-reads the times from
+// HBM, 52 us for that pass.)
+constexpr int kCoTile = 256;
+__global__ void __launch_bounds__(kCoTile) coincidence_flag_kernel(const SinRec *fin, const uint32_t *n_ptr, double tau, uint8_t *flag, uint32_t *tile_cnt) {
   __shared__ uint32_t s_sum;
-  const uint32_t n = *n_ptr, tile = blockIdx.x;
-  if ((unsigned long long)tile * kCoTile >= n) { if (threadIdx.x == 0) tile_cnt[tile] = 0u; return; }
+  const uint32_t n = *n_ptr;
+  for (uint32_t tile = blockIdx.x; (unsigned long long)tile * kCoTile < n; tile += gridDim.x) {
   if (threadIdx.x == 0) s_sum = 0u;
-  TimeView V; uint32_t first = 0;
-  uint32_t cnt = tile_walk(fin, n, tau, tile, s_rec, V, first, C);   // (its barrier orders the store to s_sum)
+  __syncthreads();
+  const uint32_t i = tile * kCoTile + threadIdx.x;
+  uint32_t cnt = 0;
+  if (i < n && (i == 0 || !(__dsub_rn(fin[i].t, fin[i - 1].t) < tau))) {
+    uint32_t o = i;
+    for (;;) {                                                       // o opens a window
+      const double to = fin[o].t;
+      uint32_t j = o + 1;
+      double tl = to;                                                // time of single j - 1
+      while (j < n) { const double tj = fin[j].t; if (!(__dsub_rn(tj, to) < tau)) break; flag[j] = 0; tl = tj; ++j; }
+      const bool pair = j - o == 2 && (fin[o].ids >> 26) != (fin[o + 1].ids >> 26);
+      flag[o] = pair ? 1 : 0;
+      if (pair) { if (o / kCoTile == tile) ++cnt; else atomicAdd(&tile_cnt[o / kCoTile], 1u); }   // (a cluster may run past its tile)
+      if (j >= n || !(__dsub_rn(fin[j].t, tl) < tau)) break;         // the next opener starts a new cluster (its own thread)
+      o = j;
+    }
+  }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xFFFFFFFFu, cnt, o);
   if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(&s_sum, cnt);
   __syncthreads();
-  if (threadIdx.x == 0) tile_cnt[tile] = s_sum;
-}
-// pass 2: the tile's pairs at its offset of the list-mode output, one pair per thread
-__global__ void __launch_bounds__(kCoTile) coincidence_write_kernel(const SinRec *fin, const uint32_t *n_ptr, double tau, const uint32_t *tile_off, CoincBuf C) {
-  __shared__ uint4 s_rec[kCoTile];
-  __shared__ uint32_t s_open[kCoTile];                               // openers of the tile's first kCoTile accepted pairs, in time order
-  const uint32_t n = *n_ptr, tile = blockIdx.x;
-  if ((unsigned long long)tile * kCoTile >= n) return;
-  const unsigned long long w0 = tile_off[tile];
-  if (tile_off[tile + 1] == (uint32_t)w0) return;                    // no pair starts in this tile
-  TimeView V; uint32_t first = 0;
-  const uint32_t cnt = tile_walk(fin, n, tau, tile, s_rec, V, first, C);
-  uint32_t tot; const uint32_t ex = block_exclusive_scan<kCoTile / 32>(cnt, &tot);
-  // a cluster of the tile may run far past its end (randoms at very high activity): pairs beyond the list's kCoTile
-  // entries are written by the walking thread itself
-  if (cnt == 1 && ex < (uint32_t)kCoTile) s_open[ex] = first;
-  else if (cnt) cluster_walk<true>(V, n, tau, tile * kCoTile + threadIdx.x, first, s_open, ex, w0, C);
+  if (threadIdx.x == 0 && s_sum) atomicAdd(&tile_cnt[tile], s_sum);
   __syncthreads();
-  const uint32_t listed = tot < (uint32_t)kCoTile ? tot : (uint32_t)kCoTile;
-  if (threadIdx.x < listed) write_pair(fin, s_open[threadIdx.x], w0 + threadIdx.x, C);   // dense: one pair per thread
+  }
+}
+__global__ void __launch_bounds__(kCoTile) coincidence_write_kernel(const SinRec *fin, const uint32_t *n_ptr, const uint8_t *flag, const uint32_t *tile_off, CoincBuf C) {
+  const uint32_t n = *n_ptr;
+  for (uint32_t tile = blockIdx.x; (unsigned long long)tile * kCoTile < n; tile += gridDim.x) {
+  const unsigned long long w0 = tile_off[tile];
+  if (tile_off[tile + 1] == (uint32_t)w0) continue;                  // no pair opens in this tile
+  const uint32_t i = tile * kCoTile + threadIdx.x;
+  const uint32_t f = i < n ? flag[i] : 0u;
+  uint32_t tot; const uint32_t ex = block_exclusive_scan<kCoTile / 32>(f, &tot);
+  const unsigned long long w = w0 + ex;
+  if (f && w < C.capacity) {
+    SinRec a, b; store_rec(&a, &fin[i]); store_rec(&b, &fin[i + 1]);
+    C.ids_a[w] = a.ids; C.ids_b[w] = b.ids; C.history_a[w] = a.history; C.history_b[w] = b.history;
+    C.e_a[w] = a.e; C.e_b[w] = b.e;
+    C.dt_ns[w] = (float)__dmul_rn(__dsub_rn(b.t, a.t), 1e9); C.t[w] = a.t;
+  }
+  }
 }
 
 // ---------------------------------------------------------------- scratch layout + driver
 namespace {
-struct Layout { size_t kcnt, cnt, off, ctl, ctl_bytes, st1, st2, bcnt, boff, tcnt, toff, hrank, srank, rec, sing, fin, total; uint64_t nb, nb_coarse; };
+struct Layout { size_t kcnt, cnt, off, ctl, ctl_bytes, st1, st2, bcnt, boff, tcnt, toff, flag, hrank, srank, rec, sing, fin, total; uint64_t nb, nb_coarse; };
 Layout layout(uint64_t N, uint64_t M) {
   Layout L; size_t o = 0; const uint64_t Mx = M ? M : 1;
   auto take = [&](size_t bytes) { o = (o + 255) & ~(size_t)255; size_t r = o; o += bytes; return r; };
@@ -670,11 +638,11 @@ Layout layout(uint64_t N, uint64_t M) {
   L.kcnt = take(4 * (148 * 16 + N / kHitChunkPairs + 2));   // kept singles per adder block (dense) or per chunk (chunked layout)
   L.cnt = take(4 * N); L.off = take(4 * (N + 1));
   // control block, cleared by one memset per call: the look-back state of the three scans (hits per history, singles per
-  // bucket, coincidences per tile)
-  const size_t s0 = 8 * (N / kTile + 3), s1 = 8 * (L.nb / kTile + 3), s2 = 8 * (Mx / kCoTile / kTile + 3);
-  L.ctl = take(256 + s0 + s1 + s2); L.st1 = L.ctl + 256 + s0; L.st2 = L.st1 + s1; L.ctl_bytes = 256 + s0 + s1 + s2;
+  // bucket, coincidences per tile) and the accepted pairs per tile of the time-ordered singles
+  const size_t s0 = 16 * (N / kTile / 2 + 2), s1 = 16 * (L.nb / kTile / 2 + 2), s2 = 16 * (Mx / kCoTile / kTile / 2 + 2), s3 = 4 * (Mx / kCoTile + 4);   // (16-byte aligned: the scan reads uint4)
+  L.ctl = take(256 + s0 + s1 + s2 + s3); L.st1 = L.ctl + 256 + s0; L.st2 = L.st1 + s1; L.tcnt = L.st2 + s2; L.ctl_bytes = 256 + s0 + s1 + s2 + s3;
   L.bcnt = take(4 * L.nb); L.boff = take(4 * (L.nb + 1));
-  L.tcnt = take(4 * (Mx / kCoTile + 1)); L.toff = take(4 * (Mx / kCoTile + 2));   // accepted pairs per tile of the time-ordered singles
+  L.toff = take(4 * (Mx / kCoTile + 2)); L.flag = take(Mx);
   L.hrank = take(4 * Mx); L.srank = take(4 * Mx);   // rank of a hit in its history / of a kept single in its time bucket
   L.rec = take(32 * Mx);            // hit records by history; reused for the bucket-ordered singles
   const size_t coarse = 32 * (size_t)kCoarseCap * L.nb_coarse;
@@ -697,6 +665,7 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   unsigned long long *st0 = (unsigned long long *)(s + L.ctl + 256), *st1 = (unsigned long long *)(s + L.st1), *st2 = (unsigned long long *)(s + L.st2);
   uint32_t *bcnt = (uint32_t *)(s + L.bcnt), *boff = (uint32_t *)(s + L.boff);
   uint32_t *hrank = (uint32_t *)(s + L.hrank), *srank = (uint32_t *)(s + L.srank), *tcnt = (uint32_t *)(s + L.tcnt), *toff = (uint32_t *)(s + L.toff);
+  uint8_t *flag = (uint8_t *)(s + L.flag);
   HitRec *rec = (HitRec *)(s + L.rec); SinRec *srt = (SinRec *)(s + L.rec), *sing = (SinRec *)(s + L.sing), *fin = (SinRec *)(s + L.fin);
   const bool chunked = H.chunk_fill != nullptr;
   const uint64_t B = P.pairs_per_slice;
@@ -737,11 +706,12 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
     bucket_scatter_kernel<<<chunked ? (int)H.n_chunks : ga, 256, 0, st>>>(sing, srank, off + N, chunked ? H.chunk_cap : 0u, kcnt, bk, boff, srt); count_launch();
     bucket_sort_kernel<<<grid_for(M / 2 + 1), 256, 0, st>>>(srt, P.shift, n_singles, bk, boff, fin, S); count_launch();
   }
-  // 4. coincidences (the number of singles is known on the device only: tiles past it count zero and return at once)
+  // 4. coincidences (the number of singles is known on the device only: tiles past it return at once)
   const unsigned co_tiles = (unsigned)((M + kCoTile - 1) / kCoTile);
-  coincidence_count_kernel<<<co_tiles, kCoTile, 0, st>>>(fin, n_singles, P.window_s, tcnt, C); count_launch();
+  const unsigned co_grid = co_tiles < 148u * 8u ? co_tiles : 148u * 8u;   // blocks stride over the tiles up to the device-side count
+  coincidence_flag_kernel<<<co_grid, kCoTile, 0, st>>>(fin, n_singles, P.window_s, flag, tcnt); count_launch();
   if ((e = exclusive_scan(tcnt, co_tiles, nullptr, toff, st2, C.n, st)) != cudaSuccess) return e;
-  coincidence_write_kernel<<<co_tiles, kCoTile, 0, st>>>(fin, n_singles, P.window_s, toff, C); count_launch();
+  coincidence_write_kernel<<<co_grid, kCoTile, 0, st>>>(fin, n_singles, flag, toff, C); count_launch();
   return cudaGetLastError();
 }
 

@@ -482,7 +482,10 @@ __global__ void __launch_bounds__(256) bucket_sort_kernel(const SinRec *srt, int
 // ordered by (t, history, unit) with a counting sort over kSubBuckets equal time intervals (shared atomics give each record
 // its rank of arrival, a block scan the offsets) and a rank by comparison among the records of the same sub-bucket (rarely
 // more than one).  The time-ordered records leave as whole sectors, coalesced, at the group's offset in the final array.
-constexpr int kSortThreads = 256;
+#ifndef GPET_SORT_THREADS
+#define GPET_SORT_THREADS 256
+#endif
+constexpr int kSortThreads = GPET_SORT_THREADS;
 constexpr uint32_t kSortGroup = 4;   // buckets per block: their records are sorted together when they fit (the regions are sized for
                                      // the worst case -- every hit a kept single -- and are a quarter full on C1), else one by one
 // sorts the records of buckets [b0, b0 + nbk) (together at most kCoarseCap) and writes them at boff[b0]
@@ -493,19 +496,22 @@ __device__ __forceinline__ void sort_span(const SinRec *regions, const uint32_t 
   const double sub_scale = (double)(kSubBuckets / kSortGroup) * (double)(kSortGroup / nbk);   // nbk = 1 or kSortGroup
   for (int q = threadIdx.x; q < (int)kSubBuckets; q += kSortThreads) s_cnt[q] = 0;
   __syncthreads();
-  for (uint32_t k = 0, i0 = 0; k < nbk; ++k) {
-    const uint32_t f = fill[b0 + k], nk = f < B.cap ? f : B.cap;
-    const uint4 *reg = reinterpret_cast<const uint4 *>(regions + (size_t)(b0 + k) * B.cap);
-    for (uint32_t q = threadIdx.x; q < nk; q += kSortThreads) {
-      const uint32_t i = i0 + q;
-      const uint4 ra = reg[2 * q];
-      s_a[i] = ra; s_src[i] = (b0 + k) * B.cap + q;                   // the payload {x, y, z, e} is fetched when the record leaves
-      const double t = __longlong_as_double((long long)(((unsigned long long)ra.y << 32) | ra.x));
-      const double x = __dmul_rn(__dsub_rn(bucket_coord(B, t), (double)b0), sub_scale);   // monotonic in t
-      const uint32_t sb = !(x > 0.0) ? 0u : (x >= (double)(kSubBuckets - 1) ? kSubBuckets - 1 : (uint32_t)x);
-      s_sb[i] = (uint16_t)sb; s_rk[i] = (uint16_t)atomicAdd(&s_cnt[sb], 1u);
-    }
-    i0 += nk;
+  static_assert(kSortGroup == 4, "the flat loop below splits a span of four buckets");
+  uint32_t e1 = 0, e2 = 0, e3 = 0;                                    // records of the span's first 1, 2, 3 buckets
+  if (nbk > 1) {
+    const uint32_t f0 = fill[b0], f1 = fill[b0 + 1], f2 = fill[b0 + 2];
+    e1 = f0 < B.cap ? f0 : B.cap; e2 = e1 + (f1 < B.cap ? f1 : B.cap); e3 = e2 + (f2 < B.cap ? f2 : B.cap);
+  }
+  for (uint32_t i = threadIdx.x; i < n; i += kSortThreads) {         // one flat loop over the records of all the span's buckets
+    uint32_t k = 0, q = i;
+    if (nbk > 1) { k = (i >= e1 ? 1u : 0u) + (i >= e2 ? 1u : 0u) + (i >= e3 ? 1u : 0u); q = i - (k == 0 ? 0u : (k == 1 ? e1 : (k == 2 ? e2 : e3))); }
+    const uint32_t src = (b0 + k) * B.cap + q;
+    const uint4 ra = reinterpret_cast<const uint4 *>(regions + src)[0];
+    s_a[i] = ra; s_src[i] = src;                                      // the payload {x, y, z, e} is fetched when the record leaves
+    const double t = __longlong_as_double((long long)(((unsigned long long)ra.y << 32) | ra.x));
+    const double x = __dmul_rn(__dsub_rn(bucket_coord(B, t), (double)b0), sub_scale);   // monotonic in t
+    const uint32_t sb = !(x > 0.0) ? 0u : (x >= (double)(kSubBuckets - 1) ? kSubBuckets - 1 : (uint32_t)x);
+    s_sb[i] = (uint16_t)sb; s_rk[i] = (uint16_t)atomicAdd(&s_cnt[sb], 1u);
   }
   __syncthreads();
   {

@@ -401,16 +401,20 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
   };
   // fresh photon -> entry point of its first panel (fused search) or the SEARCH / PHANTOM list
   // returns the destination list; q is updated to the panel frame on success
-  auto enter_panel = [&](Photon &q, uint64_t &hq, int bp, float bt) {
+  // 1 / majorant at 511 keV: every fresh photon enters its first panel with it (one region)
+  const float inv_mu_511 = MULTI ? 0.0f : inv_majorant<MULTI>(mu, T, g, 0, 511.0f);
+  auto enter_panel = [&](Photon &q, uint64_t &hq, int bp, float bt, bool fresh) {
     if (HASH) hash_ev(hq, EV_ENTER, (uint32_t)bp);
     float xl[3], dl[3];
     to_local(pan[bp].pose, q.x, q.d, xl, dl);
 #pragma unroll
     for (int k = 0; k < 3; ++k) { q.x[k] = fmaf(bt, dl[k], xl[k]); q.d[k] = dl[k]; }   // [R18]
     q.path += bt; q.meta = ph_with_panel(q.meta, bp);
-    const int reg = (q.x[2] >= g.reg_lo[1] ? 1 : 0) + (q.x[2] >= g.reg_lo[2] ? 1 : 0) + (q.x[2] >= g.reg_lo[3] ? 1 : 0);   // [R19] by the entry depth (unused: +inf)
-    q.meta = (q.meta & ~(3u << kRegShift)) | ((uint32_t)reg << kRegShift);
-    q.inv_mu = inv_majorant<MULTI>(mu, T, g, reg, q.E);
+    if (MULTI) {
+      const int reg = (q.x[2] >= g.reg_lo[1] ? 1 : 0) + (q.x[2] >= g.reg_lo[2] ? 1 : 0) + (q.x[2] >= g.reg_lo[3] ? 1 : 0);   // [R19] by the entry depth (unused: +inf)
+      q.meta = (q.meta & ~(3u << kRegShift)) | ((uint32_t)reg << kRegShift);
+      q.inv_mu = inv_majorant<MULTI>(mu, T, g, reg, q.E);
+    } else q.inv_mu = fresh ? inv_mu_511 : inv_majorant<MULTI>(mu, T, g, 0, q.E);   // one region: the bits stay 0
   };
 
 #ifdef GPET_STATS
@@ -522,7 +526,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       int bp = 0; float bt = 0.0f; bool entered = false;
       if (FAST && fused) {
         entered = ring_entry_fast(g, pan, q.x, q.d, alive, src_r0 == 0.0f ? hint : -1.0f, bp, bt);
-        if (entered) enter_panel(q, hq, bp, bt);
+        if (entered) enter_panel(q, hq, bp, bt, true);
       }
       const unsigned ma = __ballot_sync(FULL, alive);
       const int idx = alive ? W.list[L_FREE][cF - 1 - __popc(ma & lt_mask)] : 0;
@@ -620,7 +624,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
           if (HASH) { hash_ev(hq, EV_ESCAPE, 0); end_hash(q.pair, q.meta, hq); }
           dest = L_FREE;
         } else {
-          enter_panel(q, hq, bp, bt);
+          enter_panel(q, hq, bp, bt, false);
           dest = L_STEP;
           slot_store(W, idx, q, hq);
         }

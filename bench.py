@@ -41,13 +41,13 @@ ALG_INSTR_PER_PAIR = {"C1": 740.0, "C2": 698.8, "C3": 699.4, "C4": 1104.1, "P1":
 
 
 def digitizer_alg_bytes(n_hits, n_singles, n_coinc, n_buckets):
-    """Algorithmic HBM bytes of one gpet_digitize call on the CHUNKED hit layout -- the path this bench times (DESIGN.md
-    section 6): every hit's history, ids, energy and time are read once (16 B) and the position of each kept single's
-    representative hit (12 B); a kept single is appended with its bucket rank (36 B), moved to its time bucket (36 B read,
-    32 B written), ranked inside the bucket into time order (32 + 32 B), read by the window pass (32 B, 4 B flag), scanned
-    (8 B) and read again by the writer (8 B); a coincidence reads two singles and writes one 36-byte list-mode record; the
-    time buckets are zeroed, counted and scanned (12 B each)."""
-    return 16 * n_hits + (12 + 36 + 68 + 64 + 36 + 8 + 8) * n_singles + 100 * n_coinc + 12 * n_buckets
+    """Algorithmic HBM bytes of one gpet_digitize call on the CHUNKED hit layout with coarse time buckets -- the path this
+    bench times: every hit's history, ids, energy and time are read once (16 B) and the position of
+    each kept single's representative hit (12 B); a kept single is written into its bucket's region (32 B), read by the
+    block that sorts the bucket (32 B), written in time order (32 B), read by the window pass (32 B, 1 B flag) and its flag
+    by the writer (1 B); a coincidence reads two singles and writes one 36-byte list-mode record; the coarse buckets are
+    zeroed, counted and scanned (12 B each)."""
+    return 16 * n_hits + (12 + 32 + 32 + 32 + 32 + 2) * n_singles + 100 * n_coinc + 12 * n_buckets
 
 
 def load_peaks():
@@ -387,7 +387,7 @@ def run_ours(args):
     digi_ms = digitize_ms
     roofline_digi = None
     if peaks["hbm_gbs"]:
-        dbytes = digitizer_alg_bytes(n_hits, n_singles, n_coinc, (cap + 1) // 2)
+        dbytes = digitizer_alg_bytes(n_hits, n_singles, n_coinc, (cap + 511) // 512)
         dach = dbytes / (digi_ms * 1e-3) / 1e9
         dtraffic = None
         dp = os.path.join(ROOT, "profiles", "digitizer_traffic.txt")
@@ -396,13 +396,13 @@ def run_ours(args):
                 dtraffic = json.load(open(dp)).get("dram_bytes_per_call")
             except Exception:
                 dtraffic = None
-        roofline_digi = {"kernel": "digitizer (gpet_digitize on the chunked hit layout: 7 kernels)", "bound": "hbm", "achieved": dach, "peak": peaks["hbm_gbs"],
+        roofline_digi = {"kernel": "digitizer (gpet_digitize on the chunked hit layout: 6 kernels)", "bound": "hbm", "achieved": dach, "peak": peaks["hbm_gbs"],
                          "unit": "GB/s", "frac": dach / peaks["hbm_gbs"], "traffic": dtraffic,
                          "alone": ({"digitize_ms": alone["digitize_ms"], "achieved": dbytes / (alone["digitize_ms"] * 1e-3) / 1e9,
                                     "frac": dbytes / (alone["digitize_ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"]} if alone else None),
                          "note": f"{dbytes / n:.1f} algorithmic B/pair of the chunked path (DESIGN.md 6: {n_hits} hits, {n_singles} kept singles, {n_coinc} "
                                  f"coincidences) / {digi_ms:.3f} ms; peak = hbm_gbs of {peaks['source']}.  Per kernel (profiles/README.md): chunk_adder is bound by "
-                                 "instruction issue, the bucket sort and the coincidence passes by the latency of 32-byte scattered accesses, none by bandwidth"}
+                                 "instruction issue, the bucket sort by barrier and load latency in its short blocks, the coincidence passes by the 32-byte records they read 8 bytes of; none by bandwidth"}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:

@@ -389,20 +389,32 @@ __global__ void __launch_bounds__(kChunkThreads, 12) chunk_adder_kernel(DigiPara
   __syncthreads();
   for (uint32_t i = threadIdx.x; i < n; i += kChunkThreads) s_ord[s_off[s_h[i]] + s_rk[i]] = (uint16_t)i;
   __syncthreads();
-  for (uint32_t j0 = 0; j0 < n; j0 += kChunkThreads) {               // adder: one thread per hit, in history order
+  // inside a history (a handful of hits) order by (ids, position): the hits of a readout unit become contiguous and the
+  // smallest key of a group -- its leader -- comes first.  The ranks go to s_rk, whose arrival ranks are no longer needed.
+  uint16_t *s_grp = s_rk;
+  for (uint32_t j = threadIdx.x; j < n; j += kChunkThreads) {
+    const uint32_t i = s_ord[j], h = s_h[i], b = s_off[h], k = s_cnt[h];
+    uint32_t r = 0;
+    if (k > 1) {
+      const uint64_t my_key = ((uint64_t)s_ids[i] << 32) | i;
+      for (uint32_t q = b; q < b + k; ++q) { const uint32_t i2 = s_ord[q]; r += ((((uint64_t)s_ids[i2] << 32) | i2) < my_key) ? 1u : 0u; }
+    }
+    s_grp[b + r] = (uint16_t)i;
+  }
+  __syncthreads();
+  for (uint32_t j0 = 0; j0 < n; j0 += kChunkThreads) {               // adder: one thread per hit, in (history, ids) order
     const uint32_t j = j0 + threadIdx.x;
     bool keep = false; SinRec s;
     if (j < n) {
-      const uint32_t i = s_ord[j], h = s_h[i], b = s_off[h], k = s_cnt[h], my_ids = s_ids[i], unit = my_ids >> P.shift;
-      bool leader = true; uint32_t best = i;
+      const uint32_t i = s_grp[j], h = s_h[i], b = s_off[h], k = s_cnt[h], my_ids = s_ids[i], unit = my_ids >> P.shift;
+      const bool leader = j == b || (s_ids[s_grp[j - 1]] >> P.shift) != unit;
+      uint32_t best = i;
       float e_sum = s_e[i], tof_min = s_tof[i];
-      if (k > 1) {
-        const uint64_t my_key = ((uint64_t)my_ids << 32) | i;
-        long long isum = 0; float e_best = -1.0f; uint32_t best_ord = 0;
-        for (uint32_t q = b; q < b + k; ++q) {
-          const uint32_t i2 = s_ord[q], ids2 = s_ids[i2];
-          if ((ids2 >> P.shift) != unit) continue;
-          if ((((uint64_t)ids2 << 32) | i2) < my_key) { leader = false; break; }
+      if (leader && j + 1 < b + k && (s_ids[s_grp[j + 1]] >> P.shift) == unit) {   // the group has more members: they follow
+        long long isum = deposit_fixed(e_sum); float e_best = e_sum; uint32_t best_ord = my_ids & 31u;
+        for (uint32_t q = j + 1; q < b + k; ++q) {
+          const uint32_t i2 = s_grp[q], ids2 = s_ids[i2];
+          if ((ids2 >> P.shift) != unit) break;
           const float e2 = s_e[i2];
           isum += deposit_fixed(e2);
           const uint32_t ord = ids2 & 31u;

@@ -55,7 +55,8 @@ template <bool HASH> struct WarpMem {
   uint4 c[kSlots];                     // pair, meta, ids of the pending interaction, 1/mu_maj bits (HIT: deposited energy bits)
   uint2 hh[HASH ? kSlots : 1];         // outcome hash (parity builds only)
   uint4 qw[kQueue];                    // pair queue: the pair's source block [R3] ...
-  uint32_t qp[kQueue];                 // ... and its index in the batch
+  uint32_t qp[kQueue];                 // ... its index in the batch ...
+  float2 qd[kQueue];                   // ... and, once photon A is placed, the transverse part of its direction (photon B starts from -d)
   uint8_t list[kLists][kSlots];        // slot indices by next event (stacks)
 };
 
@@ -503,11 +504,15 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       if (have) {
         const uint4 w = W.qw[cQ - 1 - lane]; q.pair = W.qp[cQ - 1 - lane];
         hint = u01(w.y) + (gen_b ? 0.5f : 0.0f);
-        const float u = u01(w.x), ct = 1.0f - 2.0f * u, sth = 2.0f * sqrtf(u * (1.0f - u));   // sin^2 = (1-ct)(1+ct)
-        float sp, cp; sincospif(2.0f * u01(w.y), &sp, &cp);
-        q.d[0] = sth * cp; q.d[1] = sth * sp; q.d[2] = ct; sxy = sth;
-        if (gen_b) {
-          q.d[0] = -q.d[0]; q.d[1] = -q.d[1]; q.d[2] = -q.d[2];
+        const float u = u01(w.x), ct = 1.0f - 2.0f * u;
+        if (!gen_b) {
+          const float sth = 2.0f * sqrtf(u * (1.0f - u));             // sin^2 = (1-ct)(1+ct)
+          float sp, cp; sincospif(2.0f * u01(w.y), &sp, &cp);
+          q.d[0] = sth * cp; q.d[1] = sth * sp; q.d[2] = ct; sxy = sth;
+          W.qd[cQ - 1 - lane] = make_float2(q.d[0], q.d[1]);
+        } else {
+          const float2 dA = W.qd[cQ - 1 - lane];                      // photon A's direction, as its half-pass computed it
+          q.d[0] = -dA.x; q.d[1] = -dA.y; q.d[2] = -ct; sxy = sqrt_fast(fmaf(dA.x, dA.x, dA.y * dA.y));
           if (src.acol_sigma > 0.0f) {
             const float rho = src.acol_sigma * sqrt_fast(-2.0f * __logf(u01(w.z)));
             float sr, cr; sincos_small(rho, sr, cr);

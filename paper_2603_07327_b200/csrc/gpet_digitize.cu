@@ -3,16 +3,17 @@
 // coincidence timing window), PAPER.md:65 (list-mode coincidences).  Readings [R16], [R24]-[R27].
 //
 // Sort / segmented-scan structure (all hand-written, no CUB/Thrust):
-//   1. counting sort of the hits by history id (dense integer keys): histogram by L2 atomics whose return value is
-//      the hit's rank in its history, single-pass look-back scan, scatter of 32-byte hit records without atomics
-//      -> one contiguous run of sectors per history;
-//   2. adder: one thread per hit record, the group leader of each (history, readout unit) sums its group in
-//      order-free fixed point, then blur, window, absolute time -> kept singles appended (one atomic per block) and
-//      counted into time buckets (rank = the atomic's return value);
-//   3. counting sort of the kept singles by time bucket (decay times are uniform by construction [R16], ~0.6
-//      singles per bucket), then a rank sort by (t, history, unit) inside each bucket;
-//   4. head-flag pass: a thread per cluster start (gap >= tau) walks its cluster with the window rule [R27];
-//      exclusive scan of the pair flags; compaction into list-mode output.
+//   1. sort of the hits by history id: per 512-pair chunk in shared memory (chunked hit layout: gpet_simulate writes the hits
+//      of a chunk into the chunk's own region), or, for hits in any order, a counting sort through HBM (histogram by L2
+//      atomics whose return value is the hit's rank in its history, single-pass look-back scan, scatter of 32-byte records);
+//   2. adder: one thread per hit, the leader of each (history, readout unit) group sums the group in order-free fixed
+//      point, then blur, window, absolute time -> kept singles;
+//   3. time sort.  Coarse buckets (the batch's decay times are uniform over its time range [R16]): a kept single goes
+//      straight into the region of its bucket, a scan of the fill counts gives the offsets, one block per group of buckets
+//      sorts the regions in shared memory.  Fine buckets (any distribution): counted by the adder, scanned, scattered,
+//      ranked inside the bucket;
+//   4. coincidences: a thread per cluster start (gap >= tau) walks its cluster with the window rule [R27] and flags the
+//      accepted pairs, counted per tile; scan over the tiles; block scan + one list-mode record per flagged single.
 // Every stage is deterministic: the output does not depend on the order of the hit buffer.
 #include <cmath>
 #include <cstring>

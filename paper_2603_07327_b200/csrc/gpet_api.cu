@@ -27,7 +27,7 @@ struct gpet_materials {
 };
 struct gpet_activity {
   int dims[3]; uint32_t n_active = 0; uint64_t w_total = 0;
-  uint32_t *dev_index = nullptr; uint64_t *dev_cdf = nullptr;
+  uint32_t *dev_index = nullptr, *dev_guide = nullptr; uint64_t *dev_cdf = nullptr;
 };
 
 // ---------------------------------------------------------------- errors, bookkeeping
@@ -345,6 +345,23 @@ extern "C" int gpet_activity_create(const float *activity, const int32_t dims[3]
   if (e == cudaSuccess) e = cudaMalloc(&a->dev_cdf, sizeof(uint64_t) * cdf.size());
   if (e == cudaSuccess) e = cudaMemcpy(a->dev_index, idx.data(), sizeof(uint32_t) * idx.size(), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(a->dev_cdf, cdf.data(), sizeof(uint64_t) * cdf.size(), cudaMemcpyHostToDevice);
+  // Guide table for the cdf search [R13]: guide[b] = the voxel the SMALLEST target of bucket b selects, bucket = the top
+  // kActGuideBits bits of the voxel-pick word (target = floor(word W / 2^32) is monotonic in the word).  The voxel of any
+  // word of bucket b then lies in [guide[b], guide[b + 1]]: the search starts from a handful of entries, not from all.
+  std::vector<uint32_t> guide((size_t)kActGuide + 1);
+  {
+    size_t v = 0;
+    const uint64_t Wl = cum & 0xFFFFFFFFull, Wh = cum >> 32;
+    for (uint32_t b = 0; b < kActGuide; ++b) {
+      const uint64_t word = (uint64_t)b << (32 - kActGuideBits);
+      const uint64_t target = word * Wh + ((word * Wl) >> 32);          // floor(word W / 2^32), as the kernel forms it
+      while (cdf[v] <= target) ++v;                                     // first voxel with cum > target
+      guide[b] = (uint32_t)v;
+    }
+    guide[kActGuide] = (uint32_t)(idx.size() - 1);
+  }
+  if (e == cudaSuccess) e = cudaMalloc(&a->dev_guide, sizeof(uint32_t) * guide.size());
+  if (e == cudaSuccess) e = cudaMemcpy(a->dev_guide, guide.data(), sizeof(uint32_t) * guide.size(), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) { gpet_activity_destroy(a); return fail(GPET_E_CUDA, "gpet_activity_create: %s", cudaGetErrorString(e)); }
   *out = a; return GPET_OK;
 }
@@ -353,6 +370,7 @@ extern "C" int gpet_activity_destroy(gpet_activity *a) {
   if (!a) return GPET_OK;
   if (a->dev_index) cudaFree(a->dev_index);
   if (a->dev_cdf) cudaFree(a->dev_cdf);
+  if (a->dev_guide) cudaFree(a->dev_guide);
   delete a; return GPET_OK;
 }
 
@@ -382,7 +400,7 @@ static int make_source(const gpet_source *s, const gpet_materials *m, DevSource 
     if (!s->activity_map) return fail(GPET_E_INVALID_ARG, "kind 1 needs an activity_map");
     for (int k = 0; k < 3; ++k) if (s->dims[k] != s->activity_map->dims[k] || !(s->voxel_mm[k] > 0.0f))
       return fail(GPET_E_INVALID_ARG, "source grid does not match its activity map");
-    D->act_index = s->activity_map->dev_index; D->act_cdf = s->activity_map->dev_cdf;
+    D->act_index = s->activity_map->dev_index; D->act_cdf = s->activity_map->dev_cdf; D->act_guide = s->activity_map->dev_guide;
     D->n_active = s->activity_map->n_active; D->w_total = s->activity_map->w_total;
     D->phantom = s->phantom_material; D->ph_major = s->phantom_majorant_material;
     if (D->phantom && m && (D->ph_major < 0 || D->ph_major >= m->n_materials)) return fail(GPET_E_INVALID_ARG, "phantom_majorant_material out of range");

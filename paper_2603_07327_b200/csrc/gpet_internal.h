@@ -13,12 +13,14 @@ struct HitBuf {            // device view of gpet_hits
   uint32_t *chunk_fill;      // chunked layout (gpet.h): hits of pairs [512 c, 512 (c+1)) of the batch at [c cap, c cap + fill[c])
   uint32_t chunk_cap, n_chunks;
 };
+constexpr uint32_t kActGuideBits = 16, kActGuide = 1u << kActGuideBits;
 constexpr uint32_t kHitChunkPairs = 512, kHitChunkShift = 9, kHitChunkCapMax = 2048;
 
 struct DevSource {
   int kind; float pos[3], beam[3]; float acol_sigma;            // radians
   float acol_sin_max, acol_cos_max;                              // sin / cos of the largest acolinearity deviation that can be drawn
   const uint32_t *act_index; const uint64_t *act_cdf; uint32_t n_active; uint64_t w_total;
+  const uint32_t *act_guide;                                     // [R13] kActGuide + 1 entries: where the cdf search of a voxel-pick word starts and ends
   const uint8_t *phantom; int ph_major; int dims[3]; float voxel[3], inv_voxel[3], origin[3];
   double activity_bq; uint64_t pairs_per_slice;
   float positron_sigma;                                          // [R35] mm per axis, 0 = off

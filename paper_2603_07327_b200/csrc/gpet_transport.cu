@@ -173,7 +173,7 @@ __device__ __noinline__ float3 rayleigh_dir(float dx, float dy, float dz, float 
 __device__ __forceinline__ void decay_site(const DevSource &src, uint4 w, float x[3]) {
   const uint64_t Wl = src.w_total & 0xFFFFFFFFull, Wh = src.w_total >> 32;          // floor(w.x * W / 2^32), exact
   const uint64_t target = (uint64_t)w.x * Wh + (((uint64_t)w.x * Wl) >> 32);
-  uint32_t lo = 0, hi = src.n_active - 1;
+  uint32_t lo = src.act_guide[w.x >> (32 - kActGuideBits)], hi = src.act_guide[(w.x >> (32 - kActGuideBits)) + 1];   // brackets the answer
   while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (src.act_cdf[mid] > target) hi = mid; else lo = mid + 1; }
   const uint32_t vi = src.act_index[lo], nx = (uint32_t)src.dims[0], ny = (uint32_t)src.dims[1];
   x[0] = src.origin[0] + ((float)(vi % nx) + u01(w.y)) * src.voxel[0];

@@ -478,7 +478,7 @@ extern "C" int gpet_simulate(const gpet_geometry *g, const gpet_materials *m, co
   HitBuf HB; rc = hitbuf(hits, n_pairs, &HB); if (rc) return rc;
   // per-warp pools + staged tables + panel records share the CTA's shared memory: with many materials or a fine energy
   // grid the CTA runs with fewer warps; if not even 4 warps fit, say so instead of failing in the launch
-  const int warps = transport_warps_that_fit(T, g->host.n_panels, hits->outcome_hash != nullptr, smem_limit());
+  const int warps = transport_warps_that_fit(g->host, T, D, hits->outcome_hash != nullptr, smem_limit());
   if (!warps) return fail(GPET_E_TABLE, "mu tables too large for shared memory: %d staged materials x %d energies x 16 B next to the photon pools "
                           "(limit %zu B per CTA); load fewer materials or a coarser energy grid", T.n_staged, T.n_energies, smem_limit());
   unsigned long long *wc = nullptr; unsigned slot = 0; rc = next_work_counter(&wc, &slot); if (rc) return rc;

@@ -44,8 +44,7 @@ void count_launch(uint64_t n = 1);
 
 void set_transport_warps(int warps);
 int transport_warps();
-size_t transport_smem_bytes(const DevTables &T, int n_panels, bool hash);
-int transport_warps_that_fit(const DevTables &T, int n_panels, bool hash, size_t smem_limit);
+int transport_warps_that_fit(const DevGeom &host_geom, const DevTables &T, const DevSource &src, bool hash, size_t smem_limit);
 cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
                              unsigned long long *work_counter, int sm_count, int warps, cudaStream_t stream);

@@ -48,21 +48,22 @@ constexpr uint64_t kHash0 = 0xCBF29CE484222325ull;
 enum : int { L_FREE = 0, L_SEARCH, L_STEP, L_KN, L_RAY, L_PHANTOM, L_HIT, kLists, L_NONE = kLists };
 
 // One warp's private memory.  A photon record is 48 bytes in three 16-byte planes (one LDS.128 / STS.128 each).
-template <bool HASH> struct WarpMem {
+// (QUEUE: the build has the two-stage point source and its pair queue; the others leave that memory to the tables)
+template <bool HASH, bool QUEUE> struct WarpMem {
   static constexpr int kSlots = kSlotsOf<HASH>;
   float4 a[kSlots];                    // x, y, z, path      (panel frame in STEP / KN / RAY / HIT and after an exit, else global)
   float4 b[kSlots];                    // dx, dy, dz, E
   uint4 c[kSlots];                     // pair, meta, ids of the pending interaction, 1/mu_maj bits (HIT: deposited energy bits)
   uint2 hh[HASH ? kSlots : 1];         // outcome hash (parity builds only)
-  uint4 qw[kQueue];                    // pair queue: the pair's source block [R3] ...
-  uint32_t qp[kQueue];                 // ... its index in the batch ...
-  float2 qd[kQueue];                   // ... and, once photon A is placed, the transverse part of its direction (photon B starts from -d)
+  uint4 qw[QUEUE ? kQueue : 1];        // pair queue: the pair's source block [R3] ...
+  uint32_t qp[QUEUE ? kQueue : 1];     // ... its index in the batch ...
+  float2 qd[QUEUE ? kQueue : 1];                   // ... and, once photon A is placed, the transverse part of its direction (photon B starts from -d)
   uint8_t list[kLists][kSlots];        // slot indices by next event (stacks)
 };
 
 // dynamic shared memory: [WarpMem x warps of the CTA][mu: n_staged x n_energies float4][DevLayer x 4][DevPanel x (n_panels + 1)]
-template <bool HASH> struct SmemLayout {
-  __host__ __device__ static size_t mu_off(int warps) { return sizeof(WarpMem<HASH>) * (size_t)warps; }
+template <bool HASH, bool QUEUE> struct SmemLayout {
+  __host__ __device__ static size_t mu_off(int warps) { return sizeof(WarpMem<HASH, QUEUE>) * (size_t)warps; }
   __host__ __device__ static size_t layer_off(int warps, int n_mu) { return mu_off(warps) + sizeof(float4) * (size_t)n_mu; }
   __host__ __device__ static size_t geom_off(int warps, int n_mu) { return layer_off(warps, n_mu) + sizeof(DevLayer) * kMaxLayers; }
 };
@@ -144,15 +145,15 @@ constexpr int kRegShift = 18, kBlkShift = 20;
 __device__ __forceinline__ int ph_panel(uint32_t meta) { return (meta >> 5) & 63u; }
 __device__ __forceinline__ uint32_t ph_with_panel(uint32_t meta, int panel) { return (meta & ~(63u << 5)) | ((uint32_t)panel << 5); }
 
-template <bool HASH>
-__device__ __forceinline__ void slot_store(WarpMem<HASH> &W, int slot, const Photon &p, uint64_t h) {
+template <bool HASH, bool QUEUE>
+__device__ __forceinline__ void slot_store(WarpMem<HASH, QUEUE> &W, int slot, const Photon &p, uint64_t h) {
   W.a[slot] = make_float4(p.x[0], p.x[1], p.x[2], p.path);
   W.b[slot] = make_float4(p.d[0], p.d[1], p.d[2], p.E);
   W.c[slot] = make_uint4(p.pair, p.meta, p.ids, __float_as_uint(p.inv_mu));
   if (HASH) W.hh[slot] = make_uint2((uint32_t)h, (uint32_t)(h >> 32));
 }
-template <bool HASH>
-__device__ __forceinline__ void slot_load(const WarpMem<HASH> &W, int slot, Photon &p, uint64_t &h) {
+template <bool HASH, bool QUEUE>
+__device__ __forceinline__ void slot_load(const WarpMem<HASH, QUEUE> &W, int slot, Photon &p, uint64_t &h) {
   const float4 a = W.a[slot], b = W.b[slot]; const uint4 c = W.c[slot];
   p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.path = a.w; p.d[0] = b.x; p.d[1] = b.y; p.d[2] = b.z; p.E = b.w;
   p.pair = c.x; p.meta = c.y; p.ids = c.z; p.inv_mu = __uint_as_float(c.w);
@@ -344,11 +345,12 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
                            const __grid_constant__ PhiloxKeys key, HitBuf H, uint64_t *hash_out, unsigned long long *work_counter, uint32_t grab_pairs) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n_mu = T.n_staged * T.n_energies;
-  float4 *mu_s = reinterpret_cast<float4 *>(smem_raw + SmemLayout<HASH>::mu_off(blockDim.x >> 5));
-  DevLayer *lay = reinterpret_cast<DevLayer *>(smem_raw + SmemLayout<HASH>::layer_off(blockDim.x >> 5, n_mu));
-  DevPanel *pan = reinterpret_cast<DevPanel *>(smem_raw + SmemLayout<HASH>::geom_off(blockDim.x >> 5, n_mu));
+  constexpr bool QUEUE = KIND == 0 && !PHANTOM;                               // the two-stage point source
+  float4 *mu_s = reinterpret_cast<float4 *>(smem_raw + SmemLayout<HASH, QUEUE>::mu_off(blockDim.x >> 5));
+  DevLayer *lay = reinterpret_cast<DevLayer *>(smem_raw + SmemLayout<HASH, QUEUE>::layer_off(blockDim.x >> 5, n_mu));
+  DevPanel *pan = reinterpret_cast<DevPanel *>(smem_raw + SmemLayout<HASH, QUEUE>::geom_off(blockDim.x >> 5, n_mu));
   const int lane = threadIdx.x & 31;
-  WarpMem<HASH> &W = reinterpret_cast<WarpMem<HASH> *>(smem_raw)[threadIdx.x >> 5];
+  WarpMem<HASH, QUEUE> &W = reinterpret_cast<WarpMem<HASH, QUEUE> *>(smem_raw)[threadIdx.x >> 5];
   constexpr int kSlots = kSlotsOf<HASH>;
   {
     const uint32_t *gs = reinterpret_cast<const uint32_t *>(panels);
@@ -899,17 +901,25 @@ static int g_transport_warps = kWarps;             // warps per CTA (one CTA per
 void set_transport_warps(int warps) { g_transport_warps = warps < 1 ? kWarps : (warps > kWarps ? kWarps : warps); }
 int transport_warps() { return g_transport_warps; }
 
-static size_t smem_for(const DevTables &T, int n_panels, bool hash, int warps) {
-  const int n_mu = T.n_staged * T.n_energies;
-  return (hash ? SmemLayout<true>::geom_off(warps, n_mu) : SmemLayout<false>::geom_off(warps, n_mu)) + panel_bytes(n_panels + 1);
+// which build a run takes (see the dispatch in launch_transport): point source in a repetition-mode ring -> two-stage source
+static bool is_phantom_run(const DevSource &src) { return src.kind == 1 && src.phantom != nullptr; }
+static bool is_ring(const DevGeom &g) { return g.planar != 0 && g.ring != 0 && g.ring_edge_h > 0.0f; }
+static bool uses_pair_queue(const DevGeom &g, const DevSource &src) {
+  return !is_phantom_run(src) && src.kind == 0 && !(src.positron_sigma > 0.0f) && is_ring(g);
 }
-size_t transport_smem_bytes(const DevTables &T, int n_panels, bool hash) { return smem_for(T, n_panels, hash, g_transport_warps); }
+static size_t smem_for(const DevTables &T, int n_panels, bool hash, bool queue, int warps) {
+  const int n_mu = T.n_staged * T.n_energies;
+  const size_t pools = hash ? (queue ? SmemLayout<true, true>::geom_off(warps, n_mu) : SmemLayout<true, false>::geom_off(warps, n_mu))
+                            : (queue ? SmemLayout<false, true>::geom_off(warps, n_mu) : SmemLayout<false, false>::geom_off(warps, n_mu));
+  return pools + panel_bytes(n_panels + 1);
+}
 
 // The tables are staged in shared memory next to the per-warp pools: with many materials or a fine energy grid the CTA
 // gives up warps until everything fits (0 = it cannot fit at all).
-int transport_warps_that_fit(const DevTables &T, int n_panels, bool hash, size_t smem_limit) {
+int transport_warps_that_fit(const DevGeom &host_geom, const DevTables &T, const DevSource &src, bool hash, size_t smem_limit) {
   int w = g_transport_warps;
-  while (w >= 4 && smem_for(T, n_panels, hash, w) > smem_limit) --w;
+  const bool queue = uses_pair_queue(host_geom, src);
+  while (w >= 4 && smem_for(T, host_geom.n_panels, hash, queue, w) > smem_limit) --w;
   return w >= 4 ? w : 0;
 }
 
@@ -945,11 +955,11 @@ static void pretest_bounds(const DevGeomHead &g, const DevSource &src, uint32_t 
 cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, const DevTables &T, const DevSource &src,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const HitBuf &H, uint64_t *hash_out,
                              unsigned long long *work_counter, int sm_count, int warps, cudaStream_t stream) {
-  const int n_panels = host_geom.n_panels, planar_hint = host_geom.planar;
+  const int n_panels = host_geom.n_panels;
   const DevGeomHead &head = host_geom;
   const DevPanel *panels = reinterpret_cast<const DevPanel *>(reinterpret_cast<const char *>(geom) +
                                                             (reinterpret_cast<const char *>(&host_geom.panel[0]) - reinterpret_cast<const char *>(&host_geom)));
-  const size_t smem = smem_for(T, n_panels, hash_out != nullptr, warps);
+  const size_t smem = smem_for(T, n_panels, hash_out != nullptr, uses_pair_queue(host_geom, src), warps);
   const int threads = 32 * warps;
   const uint64_t want = (2 * n_pairs + threads - 1) / threads;
   const uint64_t resident = (uint64_t)sm_count;                      // persistent grid: one CTA per SM
@@ -962,7 +972,7 @@ cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, cons
   grab_pairs = grab_pairs >= kGrab ? kGrab : (grab_pairs < 32u ? 32u : grab_pairs & ~31u);
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(unsigned long long), stream);
   if (e != cudaSuccess) return e;
-  const bool phantom = src.kind == 1 && src.phantom != nullptr;
+  const bool phantom = is_phantom_run(src);
   // acceptance pre-test at the source (misses_detector): worth its instructions when a fair share of the photons leaves
   // through the axial ends -- for a point source, when the bore is wide compared with the axial margin (slope < 2:
   // more than 10 % of an isotropic source); always for voxel sources without a phantom (positions vary)
@@ -986,7 +996,7 @@ cudaError_t launch_transport(const DevGeom &host_geom, const DevGeom *geom, cons
   };
   // specialised builds for the shapes the five configs use (point source or voxel map + phantom, in a repetition-mode
   // ring); anything else runs the generic build of the same code
-  const bool ring = planar_hint != 0 && host_geom.ring != 0 && host_geom.ring_edge_h > 0.0f;
+  const bool ring = is_ring(host_geom);
   const bool point = !phantom && src.kind == 0 && !(src.positron_sigma > 0.0f);   // every pair starts at src.pos
 #define GPET_DISPATCH(H, M)                                                                                                 \
   do {                                                                                                                      \

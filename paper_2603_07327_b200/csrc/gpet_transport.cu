@@ -30,7 +30,7 @@ namespace gpet {
 #define GPET_SLOTS 160                // photon slots per warp (measured on C1 / C3 / C4: 20 x 160 beats 24 x 128 and 22 x 144 by 1-5 %)
 #endif
 #ifndef GPET_MIN_GEN
-#define GPET_MIN_GEN 16               // the source refills only when at least this many pairs fit
+#define GPET_MIN_GEN 32               // the one-stage source (voxel map, beam) refills only when a full pass of pairs fits (measured on C4: 16 / 24 / 32 -> 8.89 / 8.73 / 8.64 ms)
 #endif
 #ifndef GPET_GRAB
 #define GPET_GRAB 128                 // pairs a warp reserves at a time (multiple of 32): short tails at the end of a launch
@@ -45,7 +45,7 @@ constexpr uint32_t kGrab = GPET_GRAB;
 constexpr int kMinGen = GPET_MIN_GEN;
 constexpr uint64_t kHash0 = 0xCBF29CE484222325ull;
 
-enum : int { L_FREE = 0, L_SEARCH, L_STEP, L_KN, L_RAY, L_PHANTOM, L_HIT, kLists, L_NONE = kLists };
+enum : int { L_FREE = 0, L_SEARCH, L_STEP, L_KN, L_RAY, L_PHANTOM, L_HIT, kLists, L_SEARCHF = kLists, L_NONE = kLists + 1 };   // L_SEARCHF: builds without the pair queue only
 
 // One warp's private memory.  A photon record is 48 bytes in three 16-byte planes (one LDS.128 / STS.128 each).
 // (QUEUE: the build has the two-stage point source and its pair queue; the others leave that memory to the tables)
@@ -58,7 +58,7 @@ template <bool HASH, bool QUEUE> struct WarpMem {
   uint4 qw[QUEUE ? kQueue : 1];        // pair queue: the pair's source block [R3] ...
   uint32_t qp[QUEUE ? kQueue : 1];     // ... its index in the batch ...
   float2 qd[QUEUE ? kQueue : 1];                   // ... and, once photon A is placed, the transverse part of its direction (photon B starts from -d)
-  uint8_t list[kLists][kSlots];        // slot indices by next event (stacks)
+  uint8_t list[kLists + (QUEUE ? 0 : 1)][kSlots];   // slot indices by next event (stacks)
 };
 
 // dynamic shared memory: [WarpMem x warps of the CTA][mu: n_staged x n_energies float4][DevLayer x 4][DevPanel x (n_panels + 1)]
@@ -378,7 +378,13 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
 
   uint32_t w_next = 0, w_end = 0;          // this warp's reserved pairs [w_next, w_end)
   bool exhausted = false;                  // the global counter ran past n_pairs
-  int cF = kSlots, cS = 0, cT = 0, cK = 0, cR = 0, cP = 0, cH = 0, cQ = 0;   // list / queue fill levels (warp-uniform)
+  int cF = kSlots, cS = 0, cT = 0, cK = 0, cR = 0, cP = 0, cH = 0, cQ = 0, cX = 0;   // list / queue fill levels (warp-uniform)
+  // SPLIT (phantom runs in a ring): photons that have left the phantom take the polygon shortcut in the SEARCH pass; the
+  // few it cannot place, and every photon that leaves a panel towards another, wait in L_SEARCHF for the search over all
+  // panels -- so neither pass pays for the other's lanes
+  constexpr bool SPLIT = FAST && PHANTOM;
+  constexpr int L_FULL = SPLIT ? L_SEARCHF : L_SEARCH;
+  int &cFull = SPLIT ? cX : cS;
 
   auto history_of = [&](uint32_t pair) -> uint64_t { return first_history + pair; };
   // [R4] every transport event consumes one whole Philox block of the photon's stream
@@ -437,6 +443,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
     else if (cH >= 32 || cF < kReserve) phase = L_HIT;                    // cF + cH >= kReserve always: a low free list means deposits wait
     else if (cK >= 32) phase = L_KN;
     else if (cS >= 32) phase = L_SEARCH;
+    else if (SPLIT && cX >= 32) phase = L_SEARCHF;
     else if (PHANTOM && cP >= 32) phase = L_PHANTOM;
     else if (cR >= 32) phase = L_RAY;
     else {
@@ -452,6 +459,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
         if (cT > 0) { phase = L_STEP; best = cT; }
         if (cK > best) { phase = L_KN; best = cK; }
         if (cS > best) { phase = L_SEARCH; best = cS; }
+        if (SPLIT && cX > best) { phase = L_SEARCHF; best = cX; }
         if (PHANTOM && cP > best) { phase = L_PHANTOM; best = cP; }
         if (cR > best) { phase = L_RAY; best = cR; }
         if (best == 0) {
@@ -607,14 +615,26 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       continue;
     }
 
-    if (phase == L_SEARCH) {
-      // ---------------------------------------------- SEARCH: nearest panel ahead [R6], entry transform [R18].  A photon that has
-      // just left a panel arrives in that panel's frame (record n_panels is the identity: fresh photons are global)
+    if (SPLIT && phase == L_SEARCH) {
+      // ---------------------------------------------- SEARCH, shortcut only (phantom runs in a ring): photons that have just left
+      // the phantom are in the global frame, inside the bore; the polygon edge they cross names their panel
       const int n = min(cS, 32); const bool act = lane < n;
-      GPET_STAT(L_SEARCH, n);
       Photon q = {}; uint64_t hq = 0; int idx = 0;
       if (act) { idx = W.list[L_SEARCH][cS - 1 - lane]; slot_load(W, idx, q, hq); }
       cS -= n;
+      int bp = -1; float bt = 0.0f;
+      const bool found = ring_entry_fast(g, pan, q.x, q.d, act && fmaf(q.x[0], q.x[0], q.x[1] * q.x[1]) < g.bore_r * g.bore_r, -1.0f, bp, bt);
+      if (found) { enter_panel(q, hq, bp, bt, false); slot_store(W, idx, q, hq); }
+      push(L_STEP, cT, found, idx);
+      push(L_SEARCHF, cX, act && !found, idx);                         // unchanged, to the search over all panels
+    } else if (phase == L_FULL) {
+      // ---------------------------------------------- SEARCH: nearest panel ahead [R6], entry transform [R18].  A photon that has
+      // just left a panel arrives in that panel's frame (record n_panels is the identity: fresh photons are global)
+      const int n = min(cFull, 32); const bool act = lane < n;
+      GPET_STAT(L_SEARCH, n);
+      Photon q = {}; uint64_t hq = 0; int idx = 0;
+      if (act) { idx = W.list[L_FULL][cFull - 1 - lane]; slot_load(W, idx, q, hq); }
+      cFull -= n;
       int dest = L_NONE;
       const int excl = ph_panel(q.meta);
       if (act) {
@@ -623,7 +643,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
         point_to_global(P, xl, q.x); dir_to_global(P, dl, q.d);
       }
       int bp = -1; float bt = 0.0f; bool found = false;
-      if (FAST && PHANTOM && g.ring_edge_h > 0.0f)                    // photons that have just left the phantom, inside the bore
+      if (FAST && PHANTOM && !SPLIT && g.ring_edge_h > 0.0f)          // (kept for builds that search in one pass)
         found = ring_entry_fast(g, pan, q.x, q.d, act && excl == (int)kNoPanel && fmaf(q.x[0], q.x[0], q.x[1] * q.x[1]) < g.bore_r * g.bore_r, -1.0f, bp, bt);
       if (act) {
         if (!found) bp = panel_search<PLANAR>(g, pan, q.x, q.d, excl, bt);
@@ -683,7 +703,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       if (ray) dest = L_RAY;                                           // deflected in its own pass
       if (kn) dest = L_KN;
       if (pe) dest = id != kNone ? L_HIT : L_FREE;                     // photoelectric: deposit E, end
-      if (exits) dest = open ? L_FREE : L_SEARCH;
+      if (exits) dest = open ? L_FREE : L_FULL;
       if (multi && cross) {                                            // (uniform test first: single-region detectors never get here)
         reg += B.z >= 0.0f ? 1 : -1;
         C.y = (C.y & ~(3u << kRegShift)) | ((uint32_t)reg << kRegShift);
@@ -710,8 +730,8 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       push(L_KN, cK, dest == L_KN, idx);
       push(L_FREE, cF, dest == L_FREE, idx);
       push(L_HIT, cH, dest == L_HIT, idx);
-      if (__any_sync(FULL, dest == L_SEARCH || dest == L_RAY)) {       // the rare destinations share one vote
-        push(L_SEARCH, cS, dest == L_SEARCH, idx);
+      if (__any_sync(FULL, dest == L_FULL || dest == L_RAY)) {         // the rare destinations share one vote
+        push(L_FULL, cFull, dest == L_FULL, idx);
         push(L_RAY, cR, dest == L_RAY, idx);
       }
     } else if (phase == L_KN) {

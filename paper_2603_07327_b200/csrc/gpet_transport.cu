@@ -863,50 +863,57 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
       push(L_STEP, cT, dest == L_STEP, idx);
       if (PHANTOM) push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
     } else if (PHANTOM && phase == L_PHANTOM) {
-      // ---------------------------------------------- PHANTOM: Woodcock tracking in the voxel grid [R17]
+      // ---------------------------------------------- PHANTOM: Woodcock tracking in the voxel grid [R17].  No divergent branches:
+      // every lane draws, advances to the tentative point, reads its voxel (clamped when the point lies outside the grid),
+      // interpolates mu and selects its next event.
       const int n = min(cP, 32); const bool act = lane < n;
-      Photon p = {}; uint64_t h = 0; int idx = 0;
-      if (act) { idx = W.list[L_PHANTOM][cP - 1 - lane]; slot_load(W, idx, p, h); }
+      const int idx = W.list[L_PHANTOM][max(cP - 1 - lane, 0)];
       cP -= n;
-      int dest = L_NONE;
-      if (act) {
-        const uint4 w = block_at(p.pair, p.meta, p.meta >> kBlkShift); p.meta += 1u << kBlkShift;   // [R4]
-        const float s = -__logf(u01(w.x)) * p.inv_mu;
-        int v[3]; bool out = false; float xt[3];
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-          xt[k] = fmaf(s, p.d[k], p.x[k]);
-          v[k] = __float2int_rd((xt[k] - src.origin[k]) * src.inv_voxel[k]);
-          out = out || v[k] < 0 || v[k] >= src.dims[k];
-        }
-        // tentative point outside the grid: the photon leaves along its line of flight from where it is [R17]
-        if (out) {
-          if (HASH) hash_ev(h, EV_PH_LEAVE, 0);
-          p.meta &= ~(1u << 11); dest = L_SEARCH;
-          if (misses_detector(g, p.x, p.d)) {                         // cannot reach the detector: ESCAPE without a search
-            if (HASH) { hash_ev(h, EV_ESCAPE, 0); end_hash(p.pair, p.meta, h); }
-            dest = L_FREE;
-          }
-        }
-        else {
-          p.x[0] = xt[0]; p.x[1] = xt[1]; p.x[2] = xt[2]; p.path += s;
-          dest = L_PHANTOM;
-          const int mat = (int)src.phantom[((size_t)v[2] * src.dims[1] + v[1]) * src.dims[0] + v[0]] - 1;
-          if (mat >= 0) {
-            const float4 m4 = mu_lookup(mu, T, mat, p.E);
-            const float t = u01(w.y) * mu_lookup(mu, T, src.ph_major, p.E).z;
-            if (t < m4.x) { if (HASH) { hash_ev(h, EV_PH_ABSORBED, 0); end_hash(p.pair, p.meta, h); } dest = L_FREE; }
-            else if (t < m4.y) { dest = L_KN; p.ids = kNone; }
-            else if (t < m4.z) { dest = L_RAY; if (HASH) hash_ev(h, EV_PH_RAYLEIGH, 0); }
-          }
-        }
-        if (dest != L_FREE) slot_store(W, idx, p, h);
+      float4 A = W.a[idx]; const float4 B = W.b[idx]; uint4 C = W.c[idx];
+      uint64_t h = 0;
+      if (HASH) { const uint2 v = W.hh[idx]; h = ((uint64_t)v.y << 32) | v.x; }
+      const uint4 w = block_at(C.x, C.y, C.y >> kBlkShift);                  // [R4] free path, outcome
+      C.y += 1u << kBlkShift;
+      const float s = -__logf(u01(w.x)) * __uint_as_float(C.w);
+      const float x0[3] = { A.x, A.y, A.z }, d0[3] = { B.x, B.y, B.z };
+      const float xt0 = fmaf(s, B.x, A.x), xt1 = fmaf(s, B.y, A.y), xt2 = fmaf(s, B.z, A.z);
+      const int v0 = __float2int_rd((xt0 - src.origin[0]) * src.inv_voxel[0]), v1 = __float2int_rd((xt1 - src.origin[1]) * src.inv_voxel[1]),
+                v2 = __float2int_rd((xt2 - src.origin[2]) * src.inv_voxel[2]);
+      // tentative point outside the grid: the photon leaves along its line of flight from where it is [R17]
+      const bool out = (unsigned)v0 >= (unsigned)src.dims[0] || (unsigned)v1 >= (unsigned)src.dims[1] || (unsigned)v2 >= (unsigned)src.dims[2];
+      const bool gone = out && misses_detector(g, x0, d0);            // cannot reach the detector: ESCAPE without a search
+      const int c0 = min(max(v0, 0), src.dims[0] - 1), c1 = min(max(v1, 0), src.dims[1] - 1), c2 = min(max(v2, 0), src.dims[2] - 1);
+      const int mat = out ? -1 : (int)src.phantom[((size_t)c2 * src.dims[1] + c1) * src.dims[0] + c0] - 1;
+      const float4 m4 = mu_lookup(mu, T, mat < 0 ? 0 : mat, B.w);
+      const float t = u01(w.y) * mu_lookup(mu, T, src.ph_major, B.w).z;
+      const bool matter = mat >= 0;
+      const bool pe = matter && t < m4.x, kn = matter && !pe && t < m4.y, ray = matter && !pe && !kn && t < m4.z;
+      int dest = L_PHANTOM;
+      if (ray) dest = L_RAY;
+      if (kn) dest = L_KN;
+      if (pe) dest = L_FREE;
+      if (out) dest = gone ? L_FREE : L_SEARCH;
+      if (!act) dest = L_NONE;
+      if (HASH && act) {
+        if (out) { hash_ev(h, EV_PH_LEAVE, 0); if (gone) hash_ev(h, EV_ESCAPE, 0); }
+        else if (pe) hash_ev(h, EV_PH_ABSORBED, 0);
+        else if (ray) hash_ev(h, EV_PH_RAYLEIGH, 0);
+        if (dest == L_FREE) end_hash(C.x, C.y, h);
+      }
+      if (out) C.y &= ~(1u << 11);
+      else { A.x = xt0; A.y = xt1; A.z = xt2; A.w += s; }
+      if (kn) C.z = kNone;
+      if (dest != L_FREE && dest != L_NONE) {
+        W.a[idx] = A; W.c[idx] = C;
+        if (HASH) W.hh[idx] = make_uint2((uint32_t)h, (uint32_t)(h >> 32));
       }
       push(L_PHANTOM, cP, dest == L_PHANTOM, idx);
       push(L_SEARCH, cS, dest == L_SEARCH, idx);
-      push(L_KN, cK, dest == L_KN, idx);
       push(L_FREE, cF, dest == L_FREE, idx);
-      push(L_RAY, cR, dest == L_RAY, idx);
+      if (__any_sync(FULL, dest == L_KN || dest == L_RAY)) {           // scatters in the phantom are the rare destinations
+        push(L_KN, cK, dest == L_KN, idx);
+        push(L_RAY, cR, dest == L_RAY, idx);
+      }
     }
     __syncwarp();
   }

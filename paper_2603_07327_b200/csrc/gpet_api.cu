@@ -402,6 +402,9 @@ static int make_source(const gpet_source *s, const gpet_materials *m, DevSource 
       return fail(GPET_E_INVALID_ARG, "source grid does not match its activity map");
     D->act_index = s->activity_map->dev_index; D->act_cdf = s->activity_map->dev_cdf; D->act_guide = s->activity_map->dev_guide;
     D->n_active = s->activity_map->n_active; D->w_total = s->activity_map->w_total;
+    const uint32_t nx = (uint32_t)s->dims[0], nxy = nx * (uint32_t)s->dims[1];
+    QDiv one; one.magic = 0u; one.shift = 0u;
+    D->div_nx = nx >= 2u ? qdiv_make(nx) : one; D->div_nxy = nxy >= 2u ? qdiv_make(nxy) : one;
     D->phantom = s->phantom_material; D->ph_major = s->phantom_majorant_material;
     if (D->phantom && m && (D->ph_major < 0 || D->ph_major >= m->n_materials)) return fail(GPET_E_INVALID_ARG, "phantom_majorant_material out of range");
   }

@@ -20,6 +20,7 @@ struct DevSource {
   int kind; float pos[3], beam[3]; float acol_sigma;            // radians
   float acol_sin_max, acol_cos_max;                              // sin / cos of the largest acolinearity deviation that can be drawn
   const uint32_t *act_index; const uint64_t *act_cdf; uint32_t n_active; uint64_t w_total;
+  QDiv div_nx, div_nxy;                                          // voxel index -> (ix, iy, iz) without integer divisions
   const uint32_t *act_guide;                                     // [R13] kActGuide + 1 entries: where the cdf search of a voxel-pick word starts and ends
   const uint8_t *phantom; int ph_major; int dims[3]; float voxel[3], inv_voxel[3], origin[3];
   double activity_bq; uint64_t pairs_per_slice;

@@ -176,10 +176,13 @@ __device__ __forceinline__ void decay_site(const DevSource &src, uint4 w, float 
   const uint64_t target = (uint64_t)w.x * Wh + (((uint64_t)w.x * Wl) >> 32);
   uint32_t lo = src.act_guide[w.x >> (32 - kActGuideBits)], hi = src.act_guide[(w.x >> (32 - kActGuideBits)) + 1];   // brackets the answer
   while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (src.act_cdf[mid] > target) hi = mid; else lo = mid + 1; }
-  const uint32_t vi = src.act_index[lo], nx = (uint32_t)src.dims[0], ny = (uint32_t)src.dims[1];
-  x[0] = src.origin[0] + ((float)(vi % nx) + u01(w.y)) * src.voxel[0];
-  x[1] = src.origin[1] + ((float)((vi / nx) % ny) + u01(w.z)) * src.voxel[1];
-  x[2] = src.origin[2] + ((float)(vi / (nx * ny)) + u01(w.w)) * src.voxel[2];
+  // voxel index -> (ix, iy, iz): exact multiply-high divisions (QDiv; magic = 0 stands for a divisor of 1)
+  const uint32_t vi = src.act_index[lo], nx = (uint32_t)src.dims[0], nxy = nx * (uint32_t)src.dims[1];
+  const uint32_t iz = src.div_nxy.magic ? __umulhi(vi, src.div_nxy.magic) >> src.div_nxy.shift : vi, r = vi - iz * nxy;
+  const uint32_t iy = src.div_nx.magic ? __umulhi(r, src.div_nx.magic) >> src.div_nx.shift : r, ix = r - iy * nx;
+  x[0] = src.origin[0] + ((float)ix + u01(w.y)) * src.voxel[0];
+  x[1] = src.origin[1] + ((float)iy + u01(w.z)) * src.voxel[1];
+  x[2] = src.origin[2] + ((float)iz + u01(w.w)) * src.voxel[2];
 }
 
 // ---------------------------------------------------------------- acceptance pre-test (planar detectors)
@@ -412,6 +415,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
   // returns the destination list; q is updated to the panel frame on success
   // 1 / majorant at 511 keV: every fresh photon enters its first panel with it (one region)
   const float inv_mu_511 = MULTI ? 0.0f : inv_majorant<MULTI>(mu, T, g, 0, 511.0f);
+  const float inv_mu_ph511 = PHANTOM ? rcp_fast(mu_lookup(mu, T, src.ph_major, 511.0f).z) : 0.0f;   // ... and its first phantom step
   auto enter_panel = [&](Photon &q, uint64_t &hq, int bp, float bt, bool fresh) {
     if (HASH) hash_ev(hq, EV_ENTER, (uint32_t)bp);
     float xl[3], dl[3];
@@ -585,7 +589,7 @@ transport_wavefront_kernel(const __grid_constant__ DevGeomHead g, const DevPanel
           float sp, cp; sincospif(2.0f * u01(w.y), &sp, &cp);
           q.d[0] = sth * cp; q.d[1] = sth * sp; q.d[2] = ct;
         }
-        if (PHANTOM) { q.meta |= 1u << 11; q.inv_mu = rcp_fast(mu_lookup(mu, T, src.ph_major, q.E).z); }
+        if (PHANTOM) { q.meta |= 1u << 11; q.inv_mu = inv_mu_ph511; }
       }
 #pragma unroll 1
       for (int ph = 0; ph < 2; ++ph) {

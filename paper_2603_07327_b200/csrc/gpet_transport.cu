@@ -2,10 +2,11 @@
 // PAPER.md:33 (panel transfer by ray/plane crossing, global->local), PAPER.md:43 (Woodcock tracking in the
 // panel frame, layer selection from the local depth, run until exit or cutoff).
 //
-// Design.  One CTA of 24 warps per SM, persistent.  Every warp owns a pool of 128 photon
+// Design.  One CTA of 20 warps per SM, persistent.  Every warp owns a pool of 160 photon
 // SLOTS in shared memory (48-byte records that never move) and one index list per NEXT EVENT: SEARCH (needs a panel
 // search), STEP (Woodcock step in a panel), KN (Klein-Nishina trial), RAY (Rayleigh deflection), PHANTOM (Woodcock
-// step in the voxel grid), HIT (a deposit waiting to be written), plus the FREE list.  A pass pops up to 32 slot indices
+// step in the voxel grid), HIT (a deposit waiting to be written), plus the FREE list (phantom runs in a ring keep a second
+// search list: SEARCH takes the polygon shortcut, SEARCHF the search over all panels).  A pass pops up to 32 slot indices
 // from ONE list, runs that event for all of them at full SIMD width, writes the changed fields back and pushes every
 // index onto the list of its next event (ballot + prefix popcount).  The pass bodies are written without divergent
 // branches: every lane runs the same instructions and the outcome is selected at the end.  The scheduler runs any list

@@ -214,6 +214,32 @@ int gpet_digitize(const gpet_source *src, uint64_t seed, uint64_t n_pairs_total,
                   void *scratch, size_t scratch_bytes, gpet_singles *singles_out,
                   gpet_coincidences *coinc_out, void *cuda_stream);
 
+/* gpet_digitize for callers that cannot allocate device memory.
+ * Who that is: a digitizer stage plugged into a host program that has already handed the whole GPU to its own memory
+ * pool (a cudaMalloc for our scratch would fail, or steal from a budget the host fixed at start-up), and an acquisition
+ * loop that digitizes time slice after time slice [R16] (PAPER.md:65 list-mode output) and cannot afford
+ * cudaMalloc/cudaFree in the loop, because both may stall every stream of the device.  Such callers already own their
+ * hit, singles and coincidence buffers; what they lack is the temporary workspace between them.
+ * This call takes the same arguments as gpet_digitize minus the scratch pair and gives the same output; its workspace is
+ * a fixed array of GPET_STATIC_SCRATCH_BYTES built into the library's device code.  The call itself runs no cudaMalloc,
+ * cudaFree or other allocating routine.  What to know:
+ *  - Limit: gpet_digitize_scratch_bytes(n_pairs, n_hits) must not exceed GPET_STATIC_SCRATCH_BYTES (about 128 B per hit
+ *    + 8 B per pair: e.g. 3e5 pairs with room for 4.5e5 hits).  Larger batches are refused with GPET_E_OVERFLOW and a
+ *    message that names both sizes, before any GPU work; split the run into smaller time slices or use gpet_digitize.
+ *  - Cost: every GPU on which this process runs the digitizer kernels holds the array (64 MiB) until the process exits,
+ *    used or not.
+ *  - First call on each device: looks up the array's device address (and, like any first launch, makes CUDA load the
+ *    kernels).  Make that first call during set-up, with the device current, before any stream capture begins.
+ *  - One workspace per device, shared by every call and every stream: two calls whose GPU work overlaps (different
+ *    streams, or different host threads without ordering between them) race on it and produce garbage.  Order them on
+ *    one stream, or with events.
+ *  - The array keeps what the previous call left in it; each call clears the parts that must start from zero itself
+ *    (on cuda_stream, ahead of its kernels), so no clean-up between calls is needed. */
+#define GPET_STATIC_SCRATCH_BYTES (64u << 20)
+int gpet_digitize_static(const gpet_source *src, uint64_t seed, uint64_t n_pairs_total, uint64_t first_history,
+                         uint64_t n_pairs, const gpet_hits *hits, uint64_t n_hits, const gpet_digitizer *dig,
+                         gpet_singles *singles_out, gpet_coincidences *coinc_out, void *cuda_stream);
+
 /* ---------------------------------------------------------------- end to end with HOST buffers */
 typedef struct {                  /* HOST outputs (pinned memory recommended); any array may be NULL    */
   gpet_hits         hits;         /* n_hits / outcome_hash / counters here are HOST pointers            */

@@ -71,7 +71,7 @@ class _HostOutputs(C.Structure):
 
 EXPORTS = ("gpet_geometry_create", "gpet_geometry_destroy", "gpet_geometry_panel_pose", "gpet_geometry_open_faces", "gpet_geometry_bore_radius", "gpet_geometry_locate",
            "gpet_materials_load", "gpet_materials_destroy", "gpet_activity_create", "gpet_activity_destroy",
-           "gpet_simulate", "gpet_digitize_scratch_bytes", "gpet_digitize", "gpet_run_host", "gpet_last_error",
+           "gpet_simulate", "gpet_digitize_scratch_bytes", "gpet_digitize", "gpet_digitize_static", "gpet_run_host", "gpet_last_error",
            "gpet_launch_count", "gpet_set_transport_warps", "gpet_pipeline_create", "gpet_pipeline_submit", "gpet_pipeline_collect",
            "gpet_pipeline_destroy", "gpet_shutdown", "gpet_decay_count")
 
@@ -102,6 +102,8 @@ def lib():
         L.gpet_digitize_scratch_bytes.restype = C.c_size_t
         L.gpet_digitize.argtypes = [C.POINTER(_Source), u64, u64, u64, u64, C.POINTER(_Hits), u64, C.POINTER(_Digitizer),
                                     vp, C.c_size_t, C.POINTER(_Singles), C.POINTER(_Coinc), vp]
+        L.gpet_digitize_static.argtypes = [C.POINTER(_Source), u64, u64, u64, u64, C.POINTER(_Hits), u64, C.POINTER(_Digitizer),
+                                           C.POINTER(_Singles), C.POINTER(_Coinc), vp]
         L.gpet_run_host.argtypes = [vp, vp, C.POINTER(_Source), u64, u64, u64, u64, C.POINTER(_Digitizer), C.c_double,
                                     C.POINTER(_HostOutputs)]
         L.gpet_pipeline_create.argtypes = [vp, vp, C.POINTER(_Source), C.POINTER(_Digitizer), u64, u64, C.c_double, C.c_uint32, i32, C.POINTER(vp)]
@@ -416,6 +418,23 @@ def gpet_digitize(source: DeviceSource, seed: int, n_pairs_total: int, first_his
     _check(lib().gpet_digitize(C.byref(source.struct), seed, n_pairs_total, first_history, n_pairs, C.byref(hs), n_hits,
                                C.byref(d), scratch.data_ptr(), int(scratch.numel()), C.byref(ss) if ss is not None else None,
                                C.byref(cs), _stream_ptr(stream)))
+
+
+GPET_STATIC_SCRATCH_BYTES = 64 << 20
+
+
+def gpet_digitize_static(source: DeviceSource, seed: int, n_pairs_total: int, first_history: int, n_pairs: int, hits: HitBuffer,
+                         n_hits: int, dig, singles: Optional[SinglesBuffer], coinc: CoincBuffer, stream=None) -> None:
+    """gpet_digitize without a scratch argument, for callers that cannot allocate device memory (the GPU is already
+    committed to the host program's pool, or the call runs once per time slice where a cudaMalloc would stall the device).
+    The workspace is a 64 MiB array built into libgpet.so: batches with gpet_digitize_scratch_bytes(n_pairs, n_hits) above
+    GPET_STATIC_SCRATCH_BYTES raise GpetError; calls share the array, so keep them ordered on one stream; make the first
+    call on a device during set-up.  Same output as gpet_digitize (see include/gpet.h)."""
+    d = _Digitizer(dig.blur_fwhm_frac, dig.blur_ref_keV, dig.e_lo_keV, dig.e_hi_keV, dig.window_ns, dig.readout_level)
+    hs, cs = hits.struct(), coinc.struct()
+    ss = singles.struct() if singles is not None else None
+    _check(lib().gpet_digitize_static(C.byref(source.struct), seed, n_pairs_total, first_history, n_pairs, C.byref(hs), n_hits,
+                                      C.byref(d), C.byref(ss) if ss is not None else None, C.byref(cs), _stream_ptr(stream)))
 
 
 GPET_WANT_HITS, GPET_WANT_SINGLES, GPET_WANT_HASH = 1, 2, 4

@@ -527,6 +527,25 @@ extern "C" int gpet_digitize(const gpet_source *src, uint64_t seed, uint64_t n_p
   return GPET_OK;
 }
 
+// gpet_digitize on the library's built-in workspace (gpet.h): for callers that own their data buffers but may not call
+// cudaMalloc -- the GPU already belongs to the host program's pool, or the call sits in a per-time-slice loop where an
+// allocation would stall the device.  Nothing here allocates: the size test is host arithmetic, the workspace address is
+// looked up once per device (first call: do it during set-up, before any stream capture), and the rest is gpet_digitize.
+extern "C" int gpet_digitize_static(const gpet_source *src, uint64_t seed, uint64_t n_pairs_total, uint64_t first_history, uint64_t n_pairs,
+                                    const gpet_hits *hits, uint64_t n_hits, const gpet_digitizer *dig, gpet_singles *so,
+                                    gpet_coincidences *co, void *stream) {
+  if (!src || !hits || !dig || !co || !co->n_coinc) return fail(GPET_E_INVALID_ARG, "gpet_digitize_static: NULL argument");
+  if (n_pairs == 0 || n_pairs >= (1ull << 32) || n_hits > hits->capacity || n_hits > (1ull << 31)) return fail(GPET_E_INVALID_ARG, "gpet_digitize_static: counts out of range");
+  const size_t need = digitize_scratch_bytes(n_pairs, n_hits);
+  if (need > (size_t)GPET_STATIC_SCRATCH_BYTES)
+    return fail(GPET_E_OVERFLOW, "gpet_digitize_static: a batch of %llu pairs / %llu hits needs %zu bytes of workspace, the built-in array holds %zu "
+                "(GPET_STATIC_SCRATCH_BYTES); digitize smaller time slices, or call gpet_digitize with your own scratch",
+                (unsigned long long)n_pairs, (unsigned long long)n_hits, need, (size_t)GPET_STATIC_SCRATCH_BYTES);
+  void *ws = nullptr; size_t ws_bytes = 0;
+  CUDA_TRY(static_digitize_scratch(&ws, &ws_bytes));
+  return gpet_digitize(src, seed, n_pairs_total, first_history, n_pairs, hits, n_hits, dig, ws, ws_bytes, so, co, stream);
+}
+
 // ---------------------------------------------------------------- whole path with host outputs
 // One device SLOT holds everything a batch needs (hit buffer, singles, coincidences, scratch, counters); a pipeline owns
 // two of them, one compute stream and one copy stream per slot.  Batch k+1 is transported and digitized while the

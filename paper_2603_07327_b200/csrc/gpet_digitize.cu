@@ -17,6 +17,8 @@
 // Every stage is deterministic: the output does not depend on the order of the hit buffer.
 #include <cmath>
 #include <cstring>
+#include <mutex>
+#include "../../include/gpet.h"
 #include "gpet_internal.h"
 
 namespace gpet {
@@ -732,6 +734,32 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   if ((e = exclusive_scan(tcnt, co_tiles, nullptr, toff, st2, C.n, st)) != cudaSuccess) return e;
   coincidence_write_kernel<<<co_grid, kCoTile, 0, st>>>(fin, n_singles, flag, toff, C); count_launch();
   return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------- built-in scratch (gpet_digitize_static, gpet.h)
+// Scratch for callers that may not allocate device memory: one fixed array in the library's device image.  It exists once
+// per GPU that loads these kernels, from that load until the process exits, whether or not anyone uses it.  In HOST code
+// the name below is only a handle for the runtime -- it is not a device address and must never be given to a kernel; the
+// address the kernels of this file receive comes from cudaGetSymbolAddress, asked once per device with that device current.
+static __device__ __align__(256) unsigned char g_static_scratch[GPET_STATIC_SCRATCH_BYTES];
+
+cudaError_t static_digitize_scratch(void **ptr, size_t *bytes) {
+  constexpr int kMaxDevices = 64;
+  static std::mutex lock;
+  static void *addr[kMaxDevices] = {};
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lk(lock);
+  if (!addr[dev]) {                                                   // set-up, first call on this device
+    void *p = nullptr;
+    if ((e = cudaGetSymbolAddress(&p, g_static_scratch)) != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    addr[dev] = p;
+  }
+  *ptr = addr[dev]; *bytes = sizeof g_static_scratch;
+  return cudaSuccess;
 }
 
 }  // namespace gpet

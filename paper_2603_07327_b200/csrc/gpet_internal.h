@@ -54,5 +54,7 @@ cudaError_t launch_locate(const DevGeom *geom, int64_t n, const float *xyz_dev, 
 size_t digitize_scratch_bytes(uint64_t n_pairs, uint64_t n_hits);
 cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first_history, uint64_t n_pairs, uint64_t n_hits,
                             void *scratch, size_t scratch_bytes, const SinglesBuf &S, const CoincBuf &C, cudaStream_t stream);
+// Device address and size of the library's built-in digitizer scratch on the CURRENT device (allocates nothing).
+cudaError_t static_digitize_scratch(void **ptr, size_t *bytes);
 
 }  // namespace gpet

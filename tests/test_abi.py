@@ -189,3 +189,48 @@ def test_bench_roofline_table_matches_the_audit():
     for k, v in name.items():
         assert abs(bench.ALG_INSTR_PER_PAIR[k] - audit[v]["instr_per_pair"]) < 0.05, k
     assert bench.ALG_INSTR_PER_PAIR["C1"] == 740.0 and abs(audit["C1"]["instr_per_pair"] - 700.0) < 10.0
+
+
+def test_multiply_high_division_is_exact(tmp_path):
+    """gpet_device.cuh: floor(n / d) = umulhi(n, magic) >> shift for every 0 <= n < 2^31 -- the lattice lookup's crystal and
+    module indices [R7] and the voxel index -> (ix, iy, iz) split [R13] rest on it.  qdiv_make is the library's own (the
+    shim includes the header); umulhi is by definition the high word of the 64-bit product.  Checked for every divisor the
+    workloads C0-C4, P1-P3, T1-T3 produce (pitches in 2^-20 mm units, grid sizes) and for random divisors, each at random
+    numerators and at the numerators where a wrong magic shows first: multiples of d, one below them, and the top of the
+    range."""
+    import subprocess
+    HERE = os.path.dirname(os.path.abspath(__file__))
+    so = str(tmp_path / "qdiv_host.so")
+    subprocess.check_call(["nvcc", "-O1", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-Xcompiler", "-fPIC",
+                           "-I", os.path.join(ROOT, "paper_2603_07327_b200", "csrc"), "-o", so, os.path.join(HERE, "golden", "qdiv_host.cu")])
+    shim = ctypes.CDLL(so)
+    rng = np.random.default_rng(11)
+    used = set()
+    for cfg in ("C0", "C1", "C2", "C3", "C4", "P1", "P2", "P3", "T1", "T2", "T3"):
+        for r in W.config_runs(cfg, 1000):
+            g = r.geometry
+            used.update(int(round(float(p) * 2 ** 20)) for p in g.module_pitch_mm)
+            for lay in g.layers:
+                used.update(int(round(float(p) * 2 ** 20)) for p in lay.pitch_mm)
+            if r.source.kind == 1:
+                nx, ny = int(r.source.dims[0]), int(r.source.dims[1])
+                used.update((nx, nx * ny))
+    used = {d for d in used if 2 <= d < 2 ** 31}
+    assert len(used) >= 6
+    d = np.concatenate([np.array(sorted(used), np.uint32), np.array([2, 3, 5, 7, 2 ** 16, 2 ** 16 + 1, 2 ** 30, 2 ** 31 - 1], np.uint32),
+                        2 ** np.arange(1, 31, dtype=np.uint32), 2 ** np.arange(2, 31, dtype=np.uint32) - 1, 2 ** np.arange(1, 31, dtype=np.uint32) + 1,
+                        rng.integers(2, 2 ** 31, 20_000, dtype=np.uint64).astype(np.uint32),
+                        rng.integers(2, 2 ** 12, 2_000, dtype=np.uint64).astype(np.uint32)])
+    magic, shift = np.zeros(len(d), np.uint32), np.zeros(len(d), np.uint32)
+    vp = lambda a: a.ctypes.data_as(ctypes.c_void_p)
+    shim.qdiv_make_batch(vp(d), len(d), vp(magic), vp(shift))
+    D, M, S = d.astype(np.uint64)[:, None], magic.astype(np.uint64)[:, None], shift.astype(np.uint64)[:, None]
+    top = np.uint64(2 ** 31 - 1)
+    k = rng.integers(1, 2 ** 31, (len(d), 64), dtype=np.uint64) // D + np.uint64(1)          # multiples k d spread over the range
+    n = np.concatenate([rng.integers(0, 2 ** 31, (len(d), 256), dtype=np.uint64), np.minimum(k * D, top), np.minimum(k * D - np.uint64(1), top),
+                        (top // D) * D, (top // D) * D - np.uint64(1), np.broadcast_to(top, (len(d), 1)), np.zeros((len(d), 1), np.uint64),
+                        D - np.uint64(1), D, np.minimum(D + np.uint64(1), top)], axis=1)
+    assert n.max() < 2 ** 31 and (M < 2 ** 32).all()
+    q = ((n * M) >> np.uint64(32)) >> S                                 # n < 2^31, magic < 2^32: the product fits 63 bits
+    bad = q != n // D
+    assert not bad.any(), (d[np.nonzero(bad)[0][:4]], n[bad][:4])

@@ -438,9 +438,11 @@ uint64_t orc_decay_count(double activity_bq, double half_life_s, double duration
   return (uint64_t)llrint(activity_bq / lambda * -expm1(-lambda * duration_s));
 }
 /* [R16] decay time of history i, seconds (fp64): t0 = (floor(i/B) + u53) * (B/A).
- * [R34] with a half-life: the same stratified quantile q = (floor(i/B) + u53) B / N in (0,1) goes through the inverse
- * cdf of the decay law truncated to the acquisition: t0 = -ln(1 - q P) / lambda, P = 1 - exp(-lambda T) (the
- * constant P comes from the C library's expm1 on the host, on both sides). */
+ * [R34] with a half-life: the stratified quantile q = (k + u53 f_k) B / N of slice k = floor(i/B) goes through the
+ * inverse cdf of the decay law truncated to the acquisition: t0 = -ln(1 - q P) / lambda, P = 1 - exp(-lambda T) (the
+ * constant P comes from the C library's expm1 on the host, on both sides).  f_k = 1 for a full slice; the last slice of a
+ * run whose N is not a multiple of B holds only N mod B histories and covers only [kB/N, 1): f_k = (N mod B) / B, so
+ * that q stays in (0, 1] and t0 in (0, T] (stretching it to a full slice would run past the end of the acquisition). */
 double orc_decay_time(const orc_source *s, uint64_t seed, uint64_t history, uint64_t n_pairs_total) {
   rng_t r; rng_init(&r, seed, history, STREAM_SOURCE);
   uint64_t w8 = rng_word_at(&r, 8), w9 = rng_word_at(&r, 9);
@@ -448,7 +450,9 @@ double orc_decay_time(const orc_source *s, uint64_t seed, uint64_t history, uint
   uint64_t B = s->pairs_per_slice ? s->pairs_per_slice : n_pairs_total;
   if (s->half_life_s > 0.0) {
     double lambda = 0.69314718055994530942 / s->half_life_s, P = -expm1(-lambda * s->duration_s);
-    double q = ((double)(history / B) + u53) * ((double)B / (double)n_pairs_total);
+    uint64_t k = history / B;
+    double f = (n_pairs_total % B != 0 && k == n_pairs_total / B) ? (double)(n_pairs_total % B) / (double)B : 1.0;
+    double q = ((double)k + u53 * f) * ((double)B / (double)n_pairs_total);
     return -orc_det_log1m(q * P) / lambda;
   }
   return ((double)(history / B) + u53) * ((double)B / s->activity_bq);

@@ -830,6 +830,38 @@ def test_decay_times_follow_the_truncated_decay_law():
         assert abs(O.decay_time(slow, 9, h, n) / O.decay_time(ref, 9, h, n) - 1.0) < 1e-8
 
 
+def test_decay_times_of_a_cut_short_last_slice_stay_inside_the_acquisition():
+    """[R34]: with explicit time slices of B pairs and N not a multiple of B, the last slice holds only N mod B
+    histories and covers only the quantile range [kB/N, 1) -- stretching it to a full slice put q above 1, decay times past
+    the end of the run (11.8 % of the last slice in the advisor's case) and, for long acquisitions, 1 - qP below 0.  The
+    quantile of slice k is q = (kB + u len_k) / N with len_k = min(B, N - kB): every t0 < T, the last slice fills exactly
+    the stretch between its edge and T, the other slices are where they were, and the whole run still follows the
+    truncated decay law (KS)."""
+    lam_of = lambda hl: math.log(2.0) / hl
+    # the advisor's case: A0 = 5e7 Bq, half-life 0.02 s, T = 0.05 s, B = 100 000
+    hl, T, B = 0.02, 0.05, 100_000
+    n = O.decay_count(5.0e7, hl, T)
+    assert n % B not in (0, B - 1) and n // B >= 5
+    src = W.Source(activity_bq=5.0e7, half_life_s=hl, duration_s=T, pairs_per_time_slice=B)
+    k_last = n // B
+    last = np.array([O.decay_time(src, 9, h, n) for h in range(k_last * B, n)])
+    P = 1.0 - math.exp(-lam_of(hl) * T)
+    edge = -math.log(1.0 - (k_last * B / n) * P) / lam_of(hl)
+    assert edge <= last.min() and last.max() < T
+    assert last.min() < edge + 0.01 * (T - edge) and last.max() > T - 0.01 * (T - edge)      # ... and fills [edge, T)
+    prev = np.array([O.decay_time(src, 9, h, n) for h in range((k_last - 1) * B, k_last * B, 37)])
+    edge0 = -math.log(1.0 - ((k_last - 1) * B / n) * P) / lam_of(hl)
+    assert edge0 <= prev.min() and prev.max() <= edge                                          # full slices unchanged
+    # ten half-lives, where the stretched slice used to reach 1 - qP < 0
+    hl, T, B, n = 1.0, 10.0, 3_000, 20_000
+    src = W.Source(activity_bq=1.0, half_life_s=hl, duration_s=T, pairs_per_time_slice=B)
+    t = np.array([O.decay_time(src, 9, h, n) for h in range(n)])
+    cdf = lambda x: (1.0 - np.exp(-lam_of(hl) * x)) / (1.0 - math.exp(-lam_of(hl) * T))
+    assert np.all(np.isfinite(t)) and t.min() > 0 and t.max() < T
+    assert stats.kstest(t, cdf).pvalue > 1e-3
+    assert np.all(np.diff([t[k * B:(k + 1) * B].max() for k in range(7)]) > 0)
+
+
 def test_positron_range_is_an_isotropic_gaussian():
     """[R35] off (the paper's setting): the annihilation point IS the emission site.  On: the displacement is
     Gaussian on every axis with the stated FWHM (PAPER.md:145 quotes 0.102 mm for 18F), uncorrelated between axes."""

@@ -950,9 +950,10 @@ static size_t smem_for(const DevTables &T, int n_panels, bool hash, bool queue, 
 // gives up warps until everything fits (0 = it cannot fit at all).
 int transport_warps_that_fit(const DevGeom &host_geom, const DevTables &T, const DevSource &src, bool hash, size_t smem_limit) {
   int w = g_transport_warps;
+  const int floor_w = w < 4 ? w : 4;                 // a caller who asked for 1..3 warps gets them; nobody is cut below 4 silently
   const bool queue = uses_pair_queue(host_geom, src);
-  while (w >= 4 && smem_for(T, host_geom.n_panels, hash, queue, w) > smem_limit) --w;
-  return w >= 4 ? w : 0;
+  while (w > floor_w && smem_for(T, host_geom.n_panels, hash, queue, w) > smem_limit) --w;
+  return smem_for(T, host_geom.n_panels, hash, queue, w) <= smem_limit ? w : 0;
 }
 
 // Point-source pre-test as two integer bounds on k = (polar word >> 9), u = (k + 0.5) 2^-23 [R2].  A pair may be dropped in

@@ -358,11 +358,18 @@ static void azimuth(double u, double *c, double *s) { *c = cos(2.0 * ORC_PI * u)
 
 /* [R20] Klein-Nishina by composition-rejection (free electron).  Returns eps = E'/E, writes
  * cos(theta), sin^2(theta) and the number of trials.  3 draws per trial. */
-static double kn_sample(rng_t *r, double E, double *cos_t, double *sin2_t, int *trials, double *u_azimuth) {
+/* where a trial's four uniforms come from: the photon's Philox stream, or (test hook below) a prepared list */
+typedef struct { rng_t *r; const double *prepared; int n_prepared, i_prepared; } kn_draws_t;
+static void kn_next_block(kn_draws_t *d, double u[4]) {
+  if (d->r) { rng_next_block(d->r, u); return; }
+  for (int k = 0; k < 4; ++k) u[k] = d->i_prepared < d->n_prepared ? d->prepared[4 * d->i_prepared + k] : 0.5;
+  ++d->i_prepared;
+}
+static double kn_sample_draws(kn_draws_t *r, double E, double *cos_t, double *sin2_t, int *trials, double *u_azimuth) {
   double k = E / ORC_MEC2, e0 = 1.0 / (1.0 + 2.0 * k), a1 = -log(e0), a2 = 0.5 * (1.0 - e0 * e0);
   double eps = 1.0, t = 0.0;
   for (int n = 1; n <= ORC_KN_CAP; ++n) {
-    double u[4]; rng_next_block(r, u);                             /* [R4] one block per trial: u_a, u_b, u_c, azimuth */
+    double u[4]; kn_next_block(r, u);                              /* [R4] one block per trial: u_a, u_b, u_c, azimuth */
     double ua = u[0], ub = u[1], uc = u[2]; *u_azimuth = u[3];
     if (ua < a1 / (a1 + a2)) eps = exp(-a1 * ub);
     else eps = sqrt(e0 * e0 + (1.0 - e0 * e0) * ub);
@@ -373,6 +380,14 @@ static double kn_sample(rng_t *r, double E, double *cos_t, double *sin2_t, int *
   }
   *cos_t = 1.0 - t; *sin2_t = t * (2.0 - t); if (*sin2_t < 0.0) *sin2_t = 0.0;
   return eps;
+}
+static double kn_sample(rng_t *r, double E, double *cos_t, double *sin2_t, int *trials, double *u_azimuth) {
+  kn_draws_t d = { r, NULL, 0, 0 }; return kn_sample_draws(&d, E, cos_t, sin2_t, trials, u_azimuth);
+}
+/* test hook: the same sampler on a PREPARED list of n_blocks x 4 uniforms {u_a, u_b, u_c, azimuth}, so a
+ * test can make every trial fail and reach the trial cap, which honest draws never do (p < 1e-30) */
+int orc_kn_sample_prepared(const double *u4, int n_blocks, double E, double *eps, double *cos_t, double *u_azimuth) {
+  kn_draws_t d = { NULL, u4, n_blocks, 0 }; double s2; int n; *eps = kn_sample_draws(&d, E, cos_t, &s2, &n, u_azimuth); return n;
 }
 int orc_kn_sample(uint64_t seed, uint64_t history, double E, double *eps, double *cos_t) {  /* test hook */
   rng_t r; rng_init(&r, seed, history, STREAM_A); double s2, ua; int n; *eps = kn_sample(&r, E, cos_t, &s2, &n, &ua); return n;

@@ -421,6 +421,17 @@ def kn_sample(seed: int, history: int, e_keV: float):
     return float(eps.value), float(ct.value), int(n)
 
 
+def kn_sample_prepared(u4: np.ndarray, e_keV: float):
+    """Test hook (O29): the Klein-Nishina sampler on a prepared list of trials, rows {u_a, u_b, u_c, azimuth}.
+    Returns (eps, cos_theta, trials, azimuth uniform of the returned trial)."""
+    u = np.ascontiguousarray(u4, np.float64).reshape(-1, 4)
+    eps, ct, ua = C.c_double(0), C.c_double(0), C.c_double(0)
+    f = lib().orc_kn_sample_prepared
+    f.argtypes = [C.POINTER(C.c_double), C.c_int, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    n = f(_p(u, C.c_double), len(u), e_keV, C.byref(eps), C.byref(ct), C.byref(ua))
+    return float(eps.value), float(ct.value), int(n), float(ua.value)
+
+
 def unpack_ids(ids: np.ndarray):
     ids = np.asarray(ids, np.uint32)
     return {"seq": ids & 15, "photon": (ids >> 4) & 1, "crystal": (ids >> 5) & 8191, "layer": (ids >> 18) & 3,

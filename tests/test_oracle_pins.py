@@ -171,6 +171,35 @@ def test_klein_nishina_angles(e_keV):
     assert 1.2 < trials.mean() < 1.6                                  # acceptance 0.67..0.74
 
 
+def test_klein_nishina_trial_cap():
+    """SURVEY 8(c) O29 / [R20]: after 64 rejected trials the 64th is taken as it stands.  Honest draws never get there
+    (acceptance >= 0.67 per trial: p < 1e-30), so the sampler runs on a prepared list: u_c just below 1 rejects every
+    trial (g < 1 away from forward scattering), each trial carries its own u_b and azimuth.  The result must be the
+    64th trial's -- not the first, not the initial eps = 1, not a 65th -- with Compton kinematics intact; a list that
+    accepts at trial 3 stops there; and the honest sampler never comes near the cap."""
+    e_keV = 511.0
+    k = e_keV / W.ME_C2_KEV
+    e0 = 1.0 / (1.0 + 2.0 * k)
+    rows = np.zeros((80, 4))
+    rows[:, 0] = 0.999                                                # u_a: always the second branch, eps^2 uniform in [e0^2, 1]
+    rows[:, 1] = np.linspace(0.2, 0.8, 80)                            # u_b: a different eps per trial
+    rows[:, 2] = 1.0 - 2.0 ** -30                                     # u_c: reject
+    rows[:, 3] = (np.arange(80) + 0.5) / 80.0                         # azimuth: names the trial that was returned
+    eps, ct, trials, ua = O.kn_sample_prepared(rows, e_keV)
+    assert trials == 64 and ua == rows[63, 3]
+    want = math.sqrt(e0 * e0 + (1.0 - e0 * e0) * rows[63, 1])        # that branch's inverse cdf at the 64th u_b
+    assert abs(eps - want) < 1e-15 and e0 <= eps <= 1.0
+    assert abs(eps - 1.0 / (1.0 + k * (1.0 - ct))) < 1e-14 and -1.0 <= ct <= 1.0
+    rows[2, 2] = 0.0                                                  # trial 3 accepts
+    eps3, ct3, trials3, ua3 = O.kn_sample_prepared(rows, e_keV)
+    assert trials3 == 3 and ua3 == rows[2, 3] and abs(eps3 - math.sqrt(e0 * e0 + (1.0 - e0 * e0) * rows[2, 1])) < 1e-15
+    rows[:, 0] = 0.0                                                  # first branch: eps = exp(-a1 u_b), same cap
+    rows[2, 2] = 1.0 - 2.0 ** -30
+    eps, ct, trials, ua = O.kn_sample_prepared(rows, e_keV)
+    assert trials == 64 and abs(eps - e0 ** rows[63, 1]) < 1e-15 and abs(eps - 1.0 / (1.0 + k * (1.0 - ct))) < 1e-14
+    assert max(O.kn_sample(5, h, e_keV)[2] for h in range(50_000)) < 40
+
+
 # ----------------------------------------------------------------------------- P5 Rayleigh, rotation, acolinearity
 def test_rayleigh_inverts_the_thomson_cdf():
     lib = O.lib()

@@ -276,6 +276,37 @@ def test_energy_is_conserved_per_photon(tables):
     assert 0.5 < len(res.hits) / n < 2.0
 
 
+def test_long_histories_saturate_the_sequence_counter_and_still_conserve_energy():
+    """SURVEY 8(c) O31 / [R9], PAPER.md:43 ("transported step by step until it either exited the panel or fell below the
+    cutoff energy"): a thick Compton-only slab, where a photon scatters dozens of times.  Almost half the photons make
+    16 or more deposits; the 4-bit sequence number counts 0..14 and then stays at 15 (it must not wrap), the hits of a
+    photon come out in path order (time of flight never decreases: that is what orders the saturated ones), every
+    deposit is one Compton event of the counters, and deposits + what leaves = 511 keV for every photon.  A semi-infinite
+    homogeneous slab has no length scale but 1/mu, so the discrete outcome cannot depend on mu: ten times the attenuation
+    gives the same hits at a tenth of the depth."""
+    n = 5000
+    res = O.simulate(slab(800.0, 1600.0), const_tables(0, 0.05, 0), beam(), n, seed=31, want_escape=True, threads=8)
+    h = res.hits
+    photon = (h.ids >> 4) & 1
+    assert np.all(photon == 0)                                        # photon B flies away from the slab
+    cnt = np.bincount(h.history, minlength=n)
+    assert np.mean(cnt >= 16) > 0.3 and cnt.max() > 40                # the regime: long histories are common
+    start = np.cumsum(cnt) - cnt
+    rank = np.arange(len(h)) - np.repeat(start, cnt)                  # position of a hit in its photon's track, as emitted
+    assert np.all(np.diff(h.history.astype(np.int64)) >= 0)
+    assert np.array_equal(h.ids & 15, np.minimum(rank, 15))           # 0, 1, ..., 14, 15, 15, 15, ...
+    same = np.diff(h.history.astype(np.int64)) == 0
+    assert np.all(np.diff(h.tof_ns.astype(np.float64))[same] >= 0)
+    c = res.counters
+    assert len(h) == c["compton"] == c["hits"] and c["cutoffs"] + c["exits"] == n
+    dep = np.zeros(n); np.add.at(dep, h.history, h.e_keV.astype(np.float64))
+    assert np.max(np.abs(dep + res.e_escape[:, 0] - 511.0)) < 2e-3 and np.all(res.e_escape[:, 1] == 511.0)
+    r10 = O.simulate(slab(800.0, 1600.0), const_tables(0, 0.5, 0), beam(), n, seed=31, want_escape=True, threads=8)
+    assert np.array_equal(r10.hits.ids, h.ids) and np.array_equal(r10.hits.history, h.history)
+    assert np.allclose((r10.hits.x.astype(np.float64) - 50.0) * 10.0, h.x.astype(np.float64) - 50.0, rtol=1e-4, atol=1e-3)
+    assert np.allclose(r10.hits.e_keV, h.e_keV, rtol=0, atol=1e-4)
+
+
 # ----------------------------------------------------------------------------- P9 indexing by brute force
 def tiny_scanner():
     th = math.radians(37.0)

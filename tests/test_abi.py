@@ -189,6 +189,7 @@ def test_bench_roofline_table_matches_the_audit():
     for k, v in name.items():
         assert abs(bench.ALG_INSTR_PER_PAIR[k] - audit[v]["instr_per_pair"]) < 0.05, k
     assert bench.ALG_INSTR_PER_PAIR["C1"] == 740.0 and abs(audit["C1"]["instr_per_pair"] - 700.0) < 10.0
+    assert abs(bench.AUDITED_C1 - audit["C1"]["instr_per_pair"]) < 0.05      # roofline.frac_audited of the C1 line
 
 
 def test_multiply_high_division_is_exact(tmp_path):

@@ -208,7 +208,13 @@ size_t gpet_digitize_scratch_bytes(uint64_t n_pairs, uint64_t n_hits);
  * use min(*hits->n_hits, hits->capacity, n_hits), read on the device.  n_pairs_total (pairs of the whole run, all batches) and
  * src give the decay times [R16].  Output is deterministic: it does not depend on the order of `hits`.
  * Records past a capacity are dropped but counted.  singles_out may be NULL (coincidences only), or have
- * NULL arrays with a valid n_singles (count only). */
+ * NULL arrays with a valid n_singles (count only).
+ * Batches that lie inside one time slice or cover whole slices [R16] are time-sorted through fixed-size bucket regions
+ * that assume decay times spread evenly over the batch's time range -- true for any batch gpet_simulate produced.  If a
+ * region fills all the same (say, the hits of one slice presented as a batch of a hundred), the singles that found no room
+ * are counted and the call sets BOTH *n_coinc and *n_singles to UINT64_MAX: the lists are incomplete, do not use them
+ * (gpet_pipeline_collect returns GPET_E_OVERFLOW); digitize the histories that have hits as their own slice-aligned
+ * batch, or a batch that ends inside a slice (it takes the counting path, which has no such limit). */
 int gpet_digitize(const gpet_source *src, uint64_t seed, uint64_t n_pairs_total, uint64_t first_history,
                   uint64_t n_pairs, const gpet_hits *hits, uint64_t n_hits, const gpet_digitizer *dig,
                   void *scratch, size_t scratch_bytes, gpet_singles *singles_out,

@@ -453,7 +453,10 @@ static int work_counter_launched(unsigned slot, cudaStream_t stream) {
 static void work_ring_release() {
   std::lock_guard<std::mutex> lk(g_ring.lock);
   if (!g_ring.words) return;
-  for (int i = 0; i < 64; ++i) cudaEventDestroy(g_ring.ev[i]);
+  for (int i = 0; i < 64; ++i) {                                      // a persistent kernel still in flight counts on its word: wait for it
+    if (g_ring.used[i]) cudaEventSynchronize(g_ring.ev[i]);
+    cudaEventDestroy(g_ring.ev[i]); g_ring.used[i] = false;
+  }
   cudaFree(g_ring.words); g_ring.words = nullptr; g_ring.next = 0;
 }
 
@@ -503,6 +506,8 @@ static int make_digi(const gpet_source *src, uint64_t seed, uint64_t n_pairs_tot
   P->seed = seed; P->slice_s = (double)P->pairs_per_slice / P->activity_bq; P->n_pairs_total = n_pairs_total;
   for (int r = 0; r < 10; ++r) { P->keys.k[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; P->keys.k[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }
   P->lambda = 0.0; P->pfrac = 0.0; P->q_scale = (double)P->pairs_per_slice / (double)n_pairs_total;
+  P->cut_slice = ~0ull; P->cut_frac = 1.0;
+  if (n_pairs_total % P->pairs_per_slice != 0) { P->cut_slice = n_pairs_total / P->pairs_per_slice; P->cut_frac = (double)(n_pairs_total % P->pairs_per_slice) / (double)P->pairs_per_slice; }
   if (src->half_life_s > 0.0) {                                      // [R34] decay law
     if (!(src->duration_s > 0.0)) return fail(GPET_E_INVALID_ARG, "half_life_s > 0 needs duration_s > 0");
     P->lambda = 0.69314718055994530942 / src->half_life_s; P->pfrac = -expm1(-P->lambda * src->duration_s);
@@ -651,6 +656,9 @@ extern "C" int gpet_pipeline_destroy(gpet_pipeline *p) {
 extern "C" int gpet_pipeline_submit(gpet_pipeline *p, uint64_t first_history, uint64_t n_pairs, uint64_t seed) {
   if (!p) return fail(GPET_E_INVALID_ARG, "gpet_pipeline_submit: NULL pipeline");
   if (n_pairs == 0 || n_pairs > p->max_pairs) return fail(GPET_E_INVALID_ARG, "gpet_pipeline_submit: n_pairs %llu outside 1..%llu", (unsigned long long)n_pairs, (unsigned long long)p->max_pairs);
+  if (first_history > p->n_pairs_total || n_pairs > p->n_pairs_total - first_history)
+    return fail(GPET_E_INVALID_ARG, "gpet_pipeline_submit: histories [%llu, %llu) leave the run of %llu pairs", (unsigned long long)first_history,
+                (unsigned long long)(first_history + n_pairs), (unsigned long long)p->n_pairs_total);
   const int n_slots = p->slot[1].A.base ? 2 : 1;
   Slot &s = p->slot[p->submitted % n_slots];
   if (s.busy) return fail(GPET_E_INVALID_ARG, "gpet_pipeline_submit: %d batches already in flight; collect one first", n_slots);
@@ -685,6 +693,7 @@ extern "C" int gpet_pipeline_collect(gpet_pipeline *p, gpet_host_outputs *out) {
   const uint64_t nh = s.host_counts[0], ns = s.host_counts[1], nc = s.host_counts[2], dropped = s.host_counts[3] & 0xFFFFFFFFull;
   if (dropped) return fail(GPET_E_OVERFLOW, "hit buffer overflow: %llu hits dropped; raise hits_per_pair", (unsigned long long)dropped);
   if (!s.chunked && nh > s.cap) return fail(GPET_E_OVERFLOW, "hit buffer overflow: %llu hits > capacity %llu; raise hits_per_pair", (unsigned long long)nh, (unsigned long long)s.cap);
+  if (nc == ~0ull) return fail(GPET_E_OVERFLOW, "the digitizer's time sort dropped singles (decay times far from uniform over the batch's time range): the lists are incomplete");
   if (nc > s.C.capacity) return fail(GPET_E_OVERFLOW, "coincidence buffer overflow");
   cudaStream_t st = s.copy;
 #define D2H(dst, srcp, n, T) do { if ((dst) && (srcp) && (n)) CUDA_TRY(cudaMemcpyAsync((dst), (srcp), sizeof(T) * (n), cudaMemcpyDeviceToHost, st)); } while (0)
@@ -712,6 +721,22 @@ extern "C" int gpet_pipeline_collect(gpet_pipeline *p, gpet_host_outputs *out) {
 // One batch, start to finish: a one-slot pipeline kept between calls of the same shape (freed by gpet_shutdown).
 namespace {
 std::mutex g_host_lock; gpet_pipeline *g_host_pipe = nullptr;
+// Field by field: both structs have padding bytes (after positron_fwhm_mm, at the end of gpet_digitizer) that a struct copy
+// need not preserve, so a memcmp could miss on equal values and throw the kept buffers away on every call.
+bool same_digitizer(const gpet_digitizer &a, const gpet_digitizer &b) {
+  return a.blur_fwhm_frac == b.blur_fwhm_frac && a.blur_ref_keV == b.blur_ref_keV && a.e_lo_keV == b.e_lo_keV && a.e_hi_keV == b.e_hi_keV &&
+         a.window_ns == b.window_ns && a.readout_level == b.readout_level;
+}
+bool same_source(const gpet_source &a, const gpet_source &b) {
+  bool eq = a.kind == b.kind && a.acolinearity_fwhm_deg == b.acolinearity_fwhm_deg && a.activity_bq == b.activity_bq &&
+            a.pairs_per_time_slice == b.pairs_per_time_slice && a.activity_map == b.activity_map && a.phantom_material == b.phantom_material &&
+            a.phantom_majorant_material == b.phantom_majorant_material && a.positron_fwhm_mm == b.positron_fwhm_mm &&
+            a.half_life_s == b.half_life_s && a.duration_s == b.duration_s;
+  for (int k = 0; k < 3; ++k)
+    eq = eq && a.pos_mm[k] == b.pos_mm[k] && a.beam_dir[k] == b.beam_dir[k] && a.dims[k] == b.dims[k] && a.voxel_mm[k] == b.voxel_mm[k] &&
+         a.origin_mm[k] == b.origin_mm[k];
+  return eq;
+}
 }
 extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, const gpet_source *src, uint64_t n_pairs_total,
                              uint64_t first_history, uint64_t n_pairs, uint64_t seed, const gpet_digitizer *dig, double hits_per_pair,
@@ -722,7 +747,7 @@ extern "C" int gpet_run_host(const gpet_geometry *g, const gpet_materials *m, co
   gpet_pipeline *p = g_host_pipe;
   const bool reuse = p && p->g == g && p->m == m && p->max_pairs == n_pairs && p->n_pairs_total == n_pairs_total && p->hits_per_pair == hits_per_pair &&
                      p->want == want && !p->phantom_dev && !(src->kind == 1 && src->phantom_material) &&
-                     memcmp(&p->dig, dig, sizeof *dig) == 0 && memcmp(&p->src, src, sizeof *src) == 0;
+                     same_digitizer(p->dig, *dig) && same_source(p->src, *src);
   if (!reuse) {
     if (p) gpet_pipeline_destroy(p);
     g_host_pipe = nullptr;

@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(256) scatter_hits_kernel(HitBuf H, uint32_t bo
 // COARSE buckets (cap > 0; the decay times of a batch are uniform by construction [R16], so a bucket sized for a mean of
 // kCoarseMean singles never sees more than cap): the adder writes each kept single straight into its bucket's region of
 // cap records, and one block per group of buckets sorts the regions in shared memory -- no scatter pass through HBM.
-struct Buckets { double t_lo, scale; uint32_t nb, cap; };
+struct Buckets { double t_lo, scale; uint32_t nb, cap; uint32_t *dropped; };   // dropped: kept singles that found their coarse bucket full (zeroed per call)
 constexpr uint32_t kCoarseMean = 512, kCoarseCap = 832, kSubBuckets = 1024;   // cap = mean + 14 sigma of a Poisson count
 __device__ __forceinline__ double bucket_coord(const Buckets &B, double t) { return __dmul_rn(__dsub_rn(t, B.t_lo), B.scale); }   // monotonic in t
 __device__ __forceinline__ uint32_t bucket_of(const Buckets &B, double t) {
@@ -231,7 +231,8 @@ __host__ __device__ inline double det_log1m(double y) {
   volatile double z = 1.0 - y; return det_log(z);
 #endif
 }
-// [R16] t0 = (slice + u53) B / A; [R34] with a half-life: t0 = -ln(1 - q P) / lambda, q = (slice + u53) B / N
+// [R16] t0 = (slice + u53) B / A; [R34] with a half-life: t0 = -ln(1 - q P) / lambda, q = (slice + u53 f) B / N, f = 1 but
+// for a last slice cut short by the end of the run, which covers only (N mod B) / B of a slice (q <= 1, t0 <= T)
 __host__ __device__ inline double decay_time_of(const DigiParams &P, double slice_plus_u) {
 #ifdef __CUDA_ARCH__
   if (P.lambda > 0.0) return __ddiv_rn(-det_log1m(__dmul_rn(__dmul_rn(slice_plus_u, P.q_scale), P.pfrac)), P.lambda);
@@ -247,10 +248,14 @@ __device__ __forceinline__ double decay_u53(const DigiParams &P, uint64_t histor
   const uint64_t bits = (((uint64_t)w.x << 32) | (uint64_t)w.y) >> 11;
   return __dmul_rn(__dadd_rn((double)bits, 0.5), 1.0 / 9007199254740992.0);
 }
+__device__ __forceinline__ double slice_plus_u(const DigiParams &P, uint64_t slice, double u53) {
+  const double f = (P.lambda > 0.0 && slice == P.cut_slice) ? P.cut_frac : 1.0;    // u53 * 1.0 is exact: full slices as before
+  return __dadd_rn((double)slice, __dmul_rn(u53, f));
+}
 __device__ __forceinline__ double decay_time(const DigiParams &P, uint64_t history) {
   const uint64_t B = P.pairs_per_slice;
   const uint64_t slice = history < B ? 0ull : history / B;
-  return decay_time_of(P, __dadd_rn((double)slice, decay_u53(P, history)));
+  return decay_time_of(P, slice_plus_u(P, slice, decay_u53(P, history)));
 }
 
 // [R25] standard normal by Box-Muller.  The blurred energy must stay within 1e-3 keV of the fp64 oracle's: sigma is
@@ -266,12 +271,13 @@ __device__ __forceinline__ float box_muller(float u0, float u1) {
 // the only one -- the same value the fp64 product rounds to
 __device__ __forceinline__ long long deposit_fixed(float e) { return __float2ll_rn(e * 1099511627776.0f); }
 
-// coarse buckets: the kept single goes to the next free record of its bucket's region.  A region never fills (see
-// Buckets); if it did, the single is dropped and the fill count put back, so the later passes see min(fill, cap).
+// coarse buckets: the kept single goes to the next free record of its bucket's region.  A region does not fill while the
+// batch's times are uniform over its range (see Buckets); if one does, the single is dropped, the fill count put back (the
+// later passes see min(fill, cap)) and the drop COUNTED: the call then reports both list lengths as UINT64_MAX (gpet.h).
 __device__ __forceinline__ void emit_coarse(const Buckets &B, const SinRec &s, SinRec *regions, uint32_t *fill) {
   const uint32_t b = bucket_of(B, s.t), pos = atomicAdd(&fill[b], 1u);
   if (pos < B.cap) store_rec(&regions[(size_t)b * B.cap + pos], &s);
-  else atomicSub(&fill[b], 1u);
+  else { atomicSub(&fill[b], 1u); atomicAdd(B.dropped, 1u); }
 }
 
 // records per block of the adder / bucket-scatter pair: the same split in both kernels, a multiple of the block size
@@ -437,7 +443,7 @@ __global__ void __launch_bounds__(kChunkThreads, 12) chunk_adder_kernel(DigiPara
         if (keep) {
           uint64_t slice = slice0;
           if (Bs >= kHitChunkPairs) slice += rem0 + h >= Bs ? 1ull : 0ull; else slice = history / Bs;
-          s.t = __dadd_rn(decay_time_of(P, __dadd_rn((double)slice, decay_u53(P, history))), __dmul_rn((double)tof_min, 1e-9));
+          s.t = __dadd_rn(decay_time_of(P, slice_plus_u(P, slice, decay_u53(P, history))), __dmul_rn((double)tof_min, 1e-9));
           s.history = (uint32_t)history; s.ids = s_ids[best]; s.x = H.x[g0 + best]; s.y = H.y[g0 + best]; s.z = H.z[g0 + best]; s.e = e_b;
         }
       }
@@ -630,7 +636,10 @@ __global__ void __launch_bounds__(kCoTile) coincidence_flag_kernel(const SinRec 
   __syncthreads();
   }
 }
-__global__ void __launch_bounds__(kCoTile) coincidence_write_kernel(const SinRec *fin, const uint32_t *n_ptr, const uint8_t *flag, const uint32_t *tile_off, CoincBuf C) {
+__global__ void __launch_bounds__(kCoTile) coincidence_write_kernel(const SinRec *fin, const uint32_t *n_ptr, const uint8_t *flag, const uint32_t *tile_off, CoincBuf C,
+                                                                    const uint32_t *dropped, unsigned long long *n_singles_out) {
+  // last kernel of the call: if the time sort dropped singles both lists are incomplete -- say so where every caller looks
+  if (blockIdx.x == 0 && threadIdx.x == 0 && *dropped) { *C.n = ~0ull; if (n_singles_out) *n_singles_out = ~0ull; }
   const uint32_t n = *n_ptr;
   for (uint32_t tile = blockIdx.x; (unsigned long long)tile * kCoTile < n; tile += gridDim.x) {
   const unsigned long long w0 = tile_off[tile];
@@ -692,6 +701,7 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   const uint64_t B = P.pairs_per_slice;
   const uint64_t slice_first = first_history / B, slice_last = (first_history + n_pairs - 1) / B;
   Buckets bk;
+  bk.dropped = (uint32_t *)(s + L.ctl);                               // first word of the control block (cleared below)
   bk.t_lo = decay_time_of(P, (double)slice_first);                  // the batch's time slices cover [t_lo, t_hi) [R16, R34]
   const double t_hi = decay_time_of(P, fmin((double)slice_last + 1.0, P.lambda > 0.0 ? 1.0 / P.q_scale : 1e300)) + 2e-6;
   // Coarse buckets need times that are uniform over [t_lo, t_hi): the batch lies inside one time slice, or covers whole
@@ -732,7 +742,7 @@ cudaError_t launch_digitize(const DigiParams &P, const HitBuf &H, uint64_t first
   const unsigned co_grid = co_tiles < 148u * 8u ? co_tiles : 148u * 8u;   // blocks stride over the tiles up to the device-side count
   coincidence_flag_kernel<<<co_grid, kCoTile, 0, st>>>(fin, n_singles, P.window_s, flag, tcnt); count_launch();
   if ((e = exclusive_scan(tcnt, co_tiles, nullptr, toff, st2, C.n, st)) != cudaSuccess) return e;
-  coincidence_write_kernel<<<co_grid, kCoTile, 0, st>>>(fin, n_singles, flag, toff, C); count_launch();
+  coincidence_write_kernel<<<co_grid, kCoTile, 0, st>>>(fin, n_singles, flag, toff, C, bk.dropped, S.n); count_launch();
   return cudaGetLastError();
 }
 

@@ -34,6 +34,7 @@ struct DigiParams {
   double activity_bq, slice_s; uint64_t pairs_per_slice; uint64_t seed;   // slice_s = pairs_per_slice / activity_bq
   double lambda, pfrac, q_scale;                                 // [R34] decay law: ln2 / half-life (0 = constant activity), 1 - exp(-lambda T), B / N
   uint64_t n_pairs_total;                                        // pairs of the whole run
+  uint64_t cut_slice; double cut_frac;                           // [R34] the run's last slice when it is cut short (N mod B != 0; else ~0): it covers only cut_frac = (N mod B) / B of a slice
   PhiloxKeys keys;                                               // [R1] the ten round keys of `seed`
 };
 

@@ -10,9 +10,11 @@ HIT_KEYS = ("history", "ids", "x", "y", "z", "e_keV", "tof_ns")
 
 
 def canonical(h: dict) -> dict:
-    """Sort a hit dict by (history, photon, seq) -- the canonical order the oracle emits."""
+    """Sort a hit dict by (history, photon, seq) -- the canonical order the oracle emits.  The sequence number saturates at
+    15 [R9]: from a photon's 16th deposit on, the hits are ordered by time of flight, which grows along the track
+    (R9; the oracle emits them in track order)."""
     key = (h["history"].astype(np.uint64) << np.uint64(5)) | (h["ids"] & np.uint32(31)).astype(np.uint64)
-    o = np.argsort(key, kind="stable")
+    o = np.lexsort((h["tof_ns"], key))
     return {k: h[k][o] for k in HIT_KEYS}
 
 
@@ -174,17 +176,23 @@ def compare_hits_unhashed(gpu, orc, n_histories, first_history=0, min_match=0.99
     def keyed(h):
         k = ((h["history"].astype(np.uint64) - np.uint64(first_history & 0xFFFFFFFF)) & np.uint64(0xFFFFFFFF)) << np.uint64(5)
         k |= (h["ids"] & np.uint32(31)).astype(np.uint64)
-        o = np.argsort(k, kind="stable")
-        return k[o], {kk: h[kk][o] for kk in HIT_KEYS}
+        o = np.lexsort((h["tof_ns"], k))
+        k = k[o]
+        # saturated sequence numbers [R9]: the 16th, 17th, ... deposit of a photon share seq 15; number them by time of flight
+        # so that the key stays unique (a photon makes fewer than 2^10 deposits)
+        first = np.r_[True, k[1:] != k[:-1]] if len(k) else np.zeros(0, bool)
+        idx = np.arange(len(k)); dup = idx - np.maximum.accumulate(np.where(first, idx, 0))
+        assert dup.max(initial=0) < 1024
+        return (k << np.uint64(10)) | dup.astype(np.uint64), {kk: h[kk][o] for kk in HIT_KEYS}
     kg, g = keyed(gpu)
     ko, o = keyed(orc)
     ig, io, _ = _join(kg, ko)
     bad_hist = np.zeros(n_histories, bool)
     only_g = np.ones(len(kg), bool); only_g[ig] = False
     only_o = np.ones(len(ko), bool); only_o[io] = False
-    bad_hist[(kg[only_g] >> np.uint64(5)).astype(np.int64)] = True
-    bad_hist[(ko[only_o] >> np.uint64(5)).astype(np.int64)] = True
-    hist = (kg[ig] >> np.uint64(5)).astype(np.int64)
+    bad_hist[(kg[only_g] >> np.uint64(15)).astype(np.int64)] = True
+    bad_hist[(ko[only_o] >> np.uint64(15)).astype(np.int64)] = True
+    hist = (kg[ig] >> np.uint64(15)).astype(np.int64)
     dxs = np.maximum.reduce([np.abs(g[k][ig].astype(np.float64) - o[k][io]) for k in ("x", "y", "z")])
     des = np.abs(g["e_keV"][ig].astype(np.float64) - o["e_keV"][io])
     dts = np.abs(g["tof_ns"][ig].astype(np.float64) - o["tof_ns"][io])

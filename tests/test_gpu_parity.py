@@ -790,6 +790,42 @@ def test_decay_law_times_are_bit_identical(tables):
             assert gs["t_s"].min() > 0.02
 
 
+def test_long_histories_with_a_saturated_sequence_counter(tables):
+    """SURVEY 8(c) O31 / [R9]: a thick Compton-only slab (the oracle pin's regime: almost half the photons
+    make 16 or more deposits, up to ~70).  The kernel's 4-bit sequence counter must stay at 15, as the oracle's does, and
+    every hit of those long tracks must match: outcome hashes, ids, positions, energies, times -- saturated hits paired in
+    time-of-flight order (R9).  That order is unique only while two saturated deposits of a photon are further
+    apart than the fp32 error of the path sum: the few histories with two such deposits within 2e-6 ns (0.6 um of path) are
+    checked for count and hash only.  Both the hashed comparison and the key join of the product-build helper run."""
+    pose = np.array([[50.0, 0, 0, 0, 1, 0, 0, 0, 1, 1, 0, 0]], np.float32)
+    # 40 mean free paths deep, +-40 wide: as good as semi-infinite (the oracle pin shows the outcome has no other length scale)
+    geom = W.Geometry(1, (W.Layer((1, 1), (160.0, 160.0), (0.0, 0.0), (0.0, 0.0), 80.0),), (1, 1), (160.0, 160.0), (160.0, 160.0), panel_pose=pose)
+    f = lambda v: np.full((1, W.N_ENERGIES), v, np.float32)
+    t = W.Tables(W.E_MIN_KEV, W.E_STEP_KEV, f(0.0), f(0.5), f(0.0))
+    n = 40_000
+    r = W.Run("long", geom, W.source_beam((0, 0, 0), (1, 0, 0), 0.0), n, 31)
+    g, gh, cnt = PU.gpu_simulate(r, t, hits_per_pair=40.0)
+    o = O.simulate(geom, t, r.source, n, r.seed, want_hash=True, threads=16)
+    oh = PU.oracle_hits_dict(o.hits)
+    per_photon = np.bincount(oh["history"], minlength=n)
+    assert np.mean(per_photon >= 16) > 0.3 and per_photon.max() > 40 and np.sum((oh["ids"] & 15) == 15) > 100_000
+    same = np.all(np.asarray(gh).reshape(-1, 2) == np.asarray(o.outcome_hash).reshape(-1, 2), axis=1)
+    assert same.mean() >= 0.999                                       # long tracks: ~20x the decisions of a C1 history
+    assert np.array_equal(np.bincount(g["history"], minlength=n)[same], per_photon[same])     # deposits per photon
+    ambiguous = np.zeros(n, bool)
+    for h in (g, oh):                                                 # both are in canonical order
+        sat = (h["ids"] & 15) == 15
+        close = sat[1:] & sat[:-1] & (h["history"][1:] == h["history"][:-1]) & (np.abs(np.diff(h["tof_ns"].astype(np.float64))) < 2e-6)
+        ambiguous[h["history"][1:][close]] = True
+    assert ambiguous.mean() < 0.02
+    keep = lambda h: {k: v[~ambiguous[h["history"]]] for k, v in h.items()}
+    g2, o2 = keep(g), keep(oh)
+    res = PU.compare_hits(g2, o2, gh, o.outcome_hash, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert res["frac"] >= 0.999 and res["n_hits_compared"] > 0.97 * len(oh["ids"]), res
+    un = PU.compare_hits_unhashed(g2, o2, n, min_match=0.999, pos_tol=POS_TOL, e_tol=E_TOL, tof_tol=TOF_TOL)
+    assert un["n_hits_compared"] > 0.97 * len(oh["ids"])
+
+
 @pytest.mark.parametrize("kind", ["point", "rods_in_phantom"])
 def test_positron_range_parity(tables, kind):
     """[R35] positron range switched on (0.5 mm FWHM, five times 18F's: PAPER.md:145): every pair starts at its own
